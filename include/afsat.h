@@ -1,0 +1,167 @@
+/*
+ * afsat.h -- C ABI of the B200-native AFSAT hot path (arxiv/paper_2606_06641).
+ *
+ * The library evaluates, for B candidate assignments X in [-1,1]^n at once, the Walsh-Fourier
+ * objective  F(X) = sum_k FE_{C_k}(X)  (Eq. (2)) and its gradient over a heterogeneous
+ * set of symmetric pseudo-Boolean constraints (Table 1 :87-97), fused with the projected
+ * gradient step, sign rounding and the exact discrete satisfied-constraint count of Alg. 1
+ * (PAPER.md:109-131).  Each FE is computed the way PAPER.md:59-67 (§2.1.2) describes: the
+ * generating polynomial prod_i (1 + w^l y_i) is evaluated at DFT points w^l, w = exp(2 pi i/(k+1)),
+ * and contracted with a precomputed coefficient vector built with the tailored, conjugate-symmetric
+ * DFT and deferred division of PAPER.md:141-147 (§3.5.1).  DESIGN.md states every reading.
+ *
+ * Conventions
+ *   - True <-> -1, False <-> +1.  Literal value y_i = lit_sign_i * x_{lit_var_i};
+ *     a literal is true iff y_i < 0.  A variable rounds to True iff x < 0 (x = 0, -0.0 -> False).
+ *   - X and G are VARIABLE-MAJOR, candidate-minor:  x[v * ldb + b],  0 <= v < n, 0 <= b < B <= ldb,
+ *     ldb % 32 == 0, base pointer 128-byte aligned.  Element type is float (dtype 32) or double
+ *     (dtype 64), fixed per context.  Columns b >= B are padding: never read as candidates,
+ *     G padding is written as 0, X padding is left untouched.
+ *   - Pointers named d_* are DEVICE pointers owned by the caller (e.g. torch tensors on the
+ *     context's device); pointers named h_* are HOST pointers.  `stream` is a cudaStream_t passed
+ *     as void* (NULL = the legacy default stream).  All d_* entry points are asynchronous on
+ *     `stream`; the caller synchronises.  The context owns only its internal tables/workspace.
+ *   - Every call returns AFSAT_OK (0) or a negative AFSAT_E_* code; no exceptions, no aborts.
+ *     afsat_last_error() returns a human-readable message for the last failing call.
+ *   - There is no CPU fallback: without a usable CUDA device afsat_create fails with AFSAT_E_CUDA.
+ */
+#ifndef AFSAT_H
+#define AFSAT_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct afsat_ctx afsat_ctx;
+
+/* Constraint types: PB forms of PAPER.md Table 1 (:87-97), identifiers of Table 2 (:252-262).
+ * tau = number of true literals among the k literals of the constraint.                        */
+enum afsat_type {
+    AFSAT_OR      = 0,  /* tau >= 1                                   param ignored          */
+    AFSAT_XOR     = 1,  /* tau mod 2 == param (1 = odd = the paper's XOR, 0 = even parity)     */
+    AFSAT_ATLEAST = 2,  /* tau >= param    (CARD >=; '>' t is ATLEAST t+1)       */
+    AFSAT_ATMOST  = 3,  /* tau <= param    (CARD '<' t is ATMOST t-1;  AMO = ATMOST 1)         */
+    AFSAT_EXACTLY = 4,  /* tau == param    (EK;  EO = EXACTLY 1)                               */
+    AFSAT_NAE     = 5   /* 0 < tau < k                                param ignored          */
+};
+
+enum afsat_error {
+    AFSAT_OK            =  0,
+    AFSAT_E_INVALID     = -1,  /* NULL pointer, bad size / dtype / ldb / alignment, unknown type  */
+    AFSAT_E_LENGTH      = -2,  /* a constraint has k < 1 or k > AFSAT_MAX_LEN                     */
+    AFSAT_E_VARIABLE    = -3,  /* literal variable index outside [0, n_vars)                      */
+    AFSAT_E_SIGN        = -4,  /* lit_sign not +1 / -1, or fixed[] not in {-1, 0, +1}             */
+    AFSAT_E_DUPLICATE   = -5,  /* the same variable twice in one constraint (FE is multilinear)   */
+    AFSAT_E_PARAM       = -6,  /* ATLEAST/ATMOST/EXACTLY with param < 0 or > k; XOR param not 0/1 */
+    AFSAT_E_NOMEM       = -7,
+    AFSAT_E_CUDA        = -8   /* no device / CUDA runtime error (text in afsat_last_error)       */
+};
+
+#define AFSAT_MAX_LEN 64       /* the paper's practical ceiling is ~50 literals    */
+
+/* afsat_create flags */
+#define AFSAT_FLAG_DEFAULT      0u
+/* Numerically robust variant of the same contraction: the product is
+ * taken over (1 + w^l)/2 + y_i (1 - w^l)/2 and contracted with the DFT of the truth table, so all
+ * factors have modulus <= 1.  Same FE, same kernels, different host tables.  Off by default: the
+ * default is the paper's prod_i (1 + w^l y_i).                                                   */
+#define AFSAT_FLAG_ROBUST       1u
+
+/*
+ * afsat_create -- build a context for one instance.
+ *   row_ptr[m+1], lit_var[nnz], lit_sign[nnz], type[m], param[m], fixed[n] (or NULL) are HOST
+ *   arrays in CSR form, borrowed for the duration of the call only (copied).
+ *   fixed[v]: 0 = free, -1 = fixed True (x = -1), +1 = fixed False (x = +1): the partial
+ *   assignment of PAPER.md:105-107; fixed variables use that value whatever X holds, receive zero
+ *   gradient and are never updated.
+ *   batch = B >= 1, ldb >= B with ldb % 32 == 0, dtype = 32 or 64, device = CUDA ordinal.
+ * Validates everything (see afsat_error), groups constraints by signature (type, k, param) and
+ * by length, precomputes per signature the exact integer coefficients, the conjugate-symmetric
+ * root table and the contracted weights (division deferred to the end), uploads the tables.
+ * Validation happens before the device is touched, so invalid input is reported even without a GPU.
+ */
+int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t *row_ptr,
+                 const int32_t *lit_var, const int8_t *lit_sign, const uint8_t *type,
+                 const int32_t *param, const int8_t *fixed, int32_t batch, int64_t ldb,
+                 int32_t dtype, int32_t device, uint32_t flags);
+
+void afsat_destroy(afsat_ctx *ctx);
+
+/* Message of the last failing call on ctx (ctx == NULL: last failing afsat_create of this thread). */
+const char *afsat_last_error(const afsat_ctx *ctx);
+
+/*
+ * afsat_eval_grad -- steps a1-a5:  F[b] = sum_C FE_C(X[:,b])  and  G[v][b] = dF[b]/dx_v.
+ *   d_x [n][ldb] (read), d_F [B] (written; may be NULL), d_G [n][ldb] (OVERWRITTEN, not
+ *   accumulated; rows of fixed variables and padding columns are 0; may be NULL for F only).
+ *   The gradient is the analytic leave-one-out product (prefix x suffix), never a division.
+ */
+int afsat_eval_grad(afsat_ctx *ctx, const void *d_x, void *d_F, void *d_G, void *stream);
+
+/*
+ * afsat_check -- steps a7-a8, integer only:  sat_count[b] = #constraints satisfied by the
+ *   sign-rounded X[:,b],  is_solution[b] = (sat_count[b] == m).  Bit-exact by construction.
+ */
+int afsat_check(afsat_ctx *ctx, const void *d_x, int32_t *d_sat_count, uint8_t *d_is_solution,
+                void *stream);
+
+/*
+ * afsat_step -- n_steps iterations of Alg. 1 with a fixed step eta, steps
+ * a1-a9 fused, no host round trip between iterations:
+ *     G = grad F(X(t-1));  X(t) = clamp(X(t-1) - eta G, -1, +1) on free variables of unsolved
+ *     candidates;  round;  count on X(t);  if all m satisfied: is_solution = 1,
+ *     first_step = step_base + t, and the candidate is frozen (executes no-ops).
+ *   X(0) itself is not checked (Alg. 1 checks after each step).
+ *   d_x [n][ldb] in/out.  d_F [B] (may be NULL): F at the final X.  d_sat_count [B]: satisfied
+ *   count at the final X.  d_is_solution [B], d_first_step [B] (-1 = none): if resume != 0 they
+ *   are read as the state left by an earlier call (frozen candidates stay frozen), else reset.
+ *   h_any_solved (may be NULL): 2 x int32 in PINNED, device-mapped host memory; [0] is set to 1
+ *   and [1] to the step index as soon as the first candidate is solved (poll without syncing).
+ */
+int afsat_step(afsat_ctx *ctx, void *d_x, double eta, int32_t n_steps, int32_t step_base,
+               int32_t resume, void *d_F, int32_t *d_sat_count, uint8_t *d_is_solution,
+               int32_t *d_first_step, int32_t *h_any_solved, void *stream);
+
+/*
+ * afsat_step_host -- the same as afsat_step (resume = 0, step_base = 0) for HOST buffers: copies
+ * h_x [n][ldb] to the device, runs n_steps, copies X, F, sat_count, is_solution, first_step back
+ * (any output pointer may be NULL) and synchronises.  Pinned host memory makes the copies
+ * asynchronous; pageable memory works too.  This is the end-to-end call bench.py times.
+ */
+int afsat_step_host(afsat_ctx *ctx, void *h_x, double eta, int32_t n_steps, void *h_F,
+                    int32_t *h_sat_count, uint8_t *h_is_solution, int32_t *h_first_step);
+
+/*
+ * afsat_host_tables -- HOST ONLY, no device needed: the contracted weight table of one signature,
+ * as the kernels consume it.  For every retained DFT point l the row
+ *     table[8*p .. 8*p+7] = { Re a, Im a, Re b, Im b, Re w, Im w, Re(w b), Im(w b) }
+ * such that  FE(y) = sum_p Re( w_p * prod_i (a_p + b_p y_i) )  and
+ *            dFE/dy_i = sum_p Re( w_p b_p * prod_{j != i} (a_p + b_p y_j) ).
+ * Real points (Im = 0 throughout) come first.  Returns the number of rows (<= AFSAT_MAX_LEN/2+1)
+ * or a negative error; table must hold 8 * (AFSAT_MAX_LEN/2 + 1) doubles; n_real (may be NULL)
+ * receives the number of real rows.
+ */
+int afsat_host_tables(int32_t type, int32_t k, int32_t param, uint32_t flags, double *table,
+                      int32_t *n_real);
+
+/* afsat_query -- counters and facts about a context. */
+enum afsat_query_key {
+    AFSAT_Q_KERNEL_LAUNCHES = 0,  /* kernels launched by this context so far                     */
+    AFSAT_Q_NUM_SIGNATURES  = 1,
+    AFSAT_Q_NUM_BUCKETS     = 2,  /* distinct constraint lengths                                 */
+    AFSAT_Q_NNZ             = 3,
+    AFSAT_Q_WORKSPACE_BYTES = 4,
+    AFSAT_Q_SM_COUNT        = 5,
+    AFSAT_Q_FP_INSTR_PER_CANDIDATE = 6  /* model count of FP instructions for one eval_grad of one
+                                           candidate over all constraints (DESIGN.md cost model)  */
+};
+int64_t afsat_query(const afsat_ctx *ctx, int32_t key);
+
+const char *afsat_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AFSAT_H */

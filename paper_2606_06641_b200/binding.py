@@ -1,0 +1,237 @@
+"""Thin ctypes binding over the C ABI of include/afsat.h -- argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels of libafsat_b200.so; PyTorch is used for
+device memory and streams.  There is NO CPU fallback: if the shared library is missing or no
+CUDA device is usable, the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+
+import numpy as np
+
+_PKG = Path(__file__).resolve().parent
+LIB_PATH = _PKG / "libafsat_b200.so"
+_lib = None
+
+FLAG_DEFAULT = 0
+FLAG_ROBUST = 1
+MAX_LEN = 64
+
+Q_KERNEL_LAUNCHES, Q_NUM_SIGNATURES, Q_NUM_BUCKETS, Q_NNZ, Q_WORKSPACE_BYTES, Q_SM_COUNT, \
+    Q_FP_INSTR_PER_CANDIDATE = range(7)
+
+ERROR_NAMES = {0: "AFSAT_OK", -1: "AFSAT_E_INVALID", -2: "AFSAT_E_LENGTH", -3: "AFSAT_E_VARIABLE",
+               -4: "AFSAT_E_SIGN", -5: "AFSAT_E_DUPLICATE", -6: "AFSAT_E_PARAM",
+               -7: "AFSAT_E_NOMEM", -8: "AFSAT_E_CUDA"}
+
+EXPORTS = ["afsat_create", "afsat_destroy", "afsat_last_error", "afsat_eval_grad", "afsat_check",
+           "afsat_step", "afsat_step_host", "afsat_host_tables", "afsat_query", "afsat_version"]
+
+
+class AfsatError(RuntimeError):
+    def __init__(self, code: int, message: str):
+        super().__init__(f"{ERROR_NAMES.get(code, code)}: {message}")
+        self.code = code
+
+
+def load_library():
+    """dlopen the in-tree CUDA library; raises (loudly) when it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not LIB_PATH.exists():
+        raise ImportError(f"{LIB_PATH} is missing: build it with "
+                          f"`python -m paper_2606_06641_b200.build` (no CPU fallback exists)")
+    L = C.CDLL(str(LIB_PATH))
+    vp, i32, i64, u32, dbl = C.c_void_p, C.c_int32, C.c_int64, C.c_uint32, C.c_double
+    L.afsat_create.restype = C.c_int
+    L.afsat_create.argtypes = [C.POINTER(vp), i32, i32, vp, vp, vp, vp, vp, vp, i32, i64, i32, i32, u32]
+    L.afsat_destroy.restype = None
+    L.afsat_destroy.argtypes = [vp]
+    L.afsat_last_error.restype = C.c_char_p
+    L.afsat_last_error.argtypes = [vp]
+    L.afsat_eval_grad.restype = C.c_int
+    L.afsat_eval_grad.argtypes = [vp, vp, vp, vp, vp]
+    L.afsat_check.restype = C.c_int
+    L.afsat_check.argtypes = [vp, vp, vp, vp, vp]
+    L.afsat_step.restype = C.c_int
+    L.afsat_step.argtypes = [vp, vp, dbl, i32, i32, i32, vp, vp, vp, vp, vp, vp]
+    L.afsat_step_host.restype = C.c_int
+    L.afsat_step_host.argtypes = [vp, vp, dbl, i32, vp, vp, vp, vp]
+    L.afsat_host_tables.restype = C.c_int
+    L.afsat_host_tables.argtypes = [i32, i32, i32, u32, vp, vp]
+    L.afsat_query.restype = i64
+    L.afsat_query.argtypes = [vp, i32]
+    L.afsat_version.restype = C.c_char_p
+    L.afsat_version.argtypes = []
+    _lib = L
+    return L
+
+
+def version() -> str:
+    return load_library().afsat_version().decode()
+
+
+def host_tables(ctype: int, k: int, param: int, flags: int = 0):
+    """(rows [P,8] float64, n_real) -- see afsat_host_tables in include/afsat.h.  Host only."""
+    L = load_library()
+    tab = np.zeros((MAX_LEN // 2 + 1, 8), dtype=np.float64)
+    n_real = C.c_int32(0)
+    rc = L.afsat_host_tables(ctype, k, param, flags, tab.ctypes.data, C.addressof(n_real))
+    if rc < 0:
+        raise AfsatError(rc, "afsat_host_tables")
+    return tab[:rc].copy(), int(n_real.value)
+
+
+def _np_ptr(a):
+    return None if a is None else a.ctypes.data
+
+
+def _stream_ptr(stream):
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(stream.cuda_stream)
+
+
+class Context:
+    """An afsat_ctx for one instance.  Tensors are torch CUDA tensors, variable-major [n, ldb]."""
+
+    def __init__(self, n_vars, row_ptr, lit_var, lit_sign, ctype, param, fixed=None, *, batch,
+                 ldb=None, dtype=32, device=0, flags=0):
+        L = load_library()
+        self._L = L
+        self._h = C.c_void_p(None)
+        row_ptr = np.ascontiguousarray(row_ptr, dtype=np.int64)
+        lit_var = np.ascontiguousarray(lit_var, dtype=np.int32)
+        lit_sign = np.ascontiguousarray(lit_sign, dtype=np.int8)
+        ctype = np.ascontiguousarray(ctype, dtype=np.uint8)
+        param = np.ascontiguousarray(param, dtype=np.int32)
+        fixed = None if fixed is None else np.ascontiguousarray(fixed, dtype=np.int8)
+        self.n = int(n_vars)
+        self.m = int(row_ptr.shape[0] - 1)
+        self.B = int(batch)
+        self.ldb = int(ldb) if ldb is not None else (self.B + 31) // 32 * 32
+        self.dtype = int(dtype)
+        self.device = int(device)
+        rc = L.afsat_create(C.byref(self._h), self.n, self.m, _np_ptr(row_ptr), _np_ptr(lit_var),
+                            _np_ptr(lit_sign), _np_ptr(ctype), _np_ptr(param), _np_ptr(fixed),
+                            self.B, self.ldb, self.dtype, self.device, int(flags))
+        if rc != 0:
+            msg = L.afsat_last_error(None).decode()
+            self._h = C.c_void_p(None)
+            raise AfsatError(rc, msg)
+
+    @classmethod
+    def from_instance(cls, inst, *, batch=None, dtype=32, device=0, flags=0, ldb=None):
+        return cls(inst.n_vars, inst.row_ptr, inst.lit_var, inst.lit_sign, inst.ctype, inst.param,
+                   inst.fixed, batch=int(batch if batch is not None else inst.batch), ldb=ldb,
+                   dtype=dtype, device=device, flags=flags)
+
+    # ---- helpers -------------------------------------------------------------------------
+    def _torch_dtype(self):
+        import torch
+        return torch.float32 if self.dtype == 32 else torch.float64
+
+    def _check_x(self, x):
+        import torch
+        if not (isinstance(x, torch.Tensor) and x.is_cuda and x.dtype == self._torch_dtype()
+                and x.is_contiguous() and tuple(x.shape) == (self.n, self.ldb)
+                and x.device.index == self.device):
+            raise ValueError(f"expected a contiguous CUDA tensor [{self.n},{self.ldb}] "
+                             f"{self._torch_dtype()} on device {self.device}")
+        if x.data_ptr() % 128:
+            raise ValueError("X must be 128-byte aligned")
+
+    def _raise(self, rc):
+        if rc != 0:
+            raise AfsatError(rc, self._L.afsat_last_error(self._h).decode())
+
+    def new_tensor(self, fill=None):
+        import torch
+        return torch.zeros((self.n, self.ldb), dtype=self._torch_dtype(), device=f"cuda:{self.device}")
+
+    # ---- entry points (same names as the C ABI) ---------------------------------------------
+    def eval_grad(self, x, F=None, G=None, *, want_F=True, want_G=True, stream=None):
+        import torch
+        self._check_x(x)
+        dev = x.device
+        if want_F and F is None:
+            F = torch.empty(self.B, dtype=x.dtype, device=dev)
+        if want_G and G is None:
+            G = torch.empty_like(x)
+        if G is not None:
+            self._check_x(G)
+        rc = self._L.afsat_eval_grad(self._h, x.data_ptr(), F.data_ptr() if F is not None else None,
+                                     G.data_ptr() if G is not None else None, _stream_ptr(stream))
+        self._raise(rc)
+        return F, G
+
+    def check(self, x, sat_count=None, is_solution=None, *, stream=None):
+        import torch
+        self._check_x(x)
+        if sat_count is None:
+            sat_count = torch.empty(self.B, dtype=torch.int32, device=x.device)
+        if is_solution is None:
+            is_solution = torch.empty(self.B, dtype=torch.uint8, device=x.device)
+        rc = self._L.afsat_check(self._h, x.data_ptr(), sat_count.data_ptr(), is_solution.data_ptr(),
+                                 _stream_ptr(stream))
+        self._raise(rc)
+        return sat_count, is_solution
+
+    def step(self, x, eta, n_steps, *, step_base=0, state=None, want_F=True, F=None,
+             h_any_solved=None, stream=None):
+        """In-place n_steps of PGD on x.  Returns (F, sat_count, is_solution, first_step)."""
+        import torch
+        self._check_x(x)
+        dev = x.device
+        if want_F and F is None:
+            F = torch.empty(self.B, dtype=x.dtype, device=dev)
+        sat = torch.empty(self.B, dtype=torch.int32, device=dev)
+        if state is None:
+            sol = torch.empty(self.B, dtype=torch.uint8, device=dev)
+            first = torch.empty(self.B, dtype=torch.int32, device=dev)
+            resume = 0
+        else:
+            sol, first = state
+            resume = 1
+        hp = None
+        if h_any_solved is not None:
+            assert h_any_solved.is_pinned() and h_any_solved.dtype == torch.int32 and h_any_solved.numel() >= 2
+            hp = h_any_solved.data_ptr()
+        rc = self._L.afsat_step(self._h, x.data_ptr(), float(eta), int(n_steps), int(step_base), resume,
+                                F.data_ptr() if F is not None else None, sat.data_ptr(), sol.data_ptr(),
+                                first.data_ptr(), hp, _stream_ptr(stream))
+        self._raise(rc)
+        return F, sat, sol, first
+
+    def step_host(self, h_x, eta, n_steps, *, want_F=True):
+        """End-to-end call on HOST buffers (numpy or pinned torch CPU tensors), synchronous.
+        h_x [n, ldb] is updated in place.  Returns (F, sat_count, is_solution, first_step) numpy."""
+        np_dtype = np.float32 if self.dtype == 32 else np.float64
+        xp = h_x.data_ptr() if hasattr(h_x, "data_ptr") else h_x.ctypes.data
+        assert tuple(h_x.shape) == (self.n, self.ldb)
+        F = np.empty(self.B, dtype=np_dtype) if want_F else None
+        sat = np.empty(self.B, dtype=np.int32)
+        sol = np.empty(self.B, dtype=np.uint8)
+        first = np.empty(self.B, dtype=np.int32)
+        rc = self._L.afsat_step_host(self._h, xp, float(eta), int(n_steps), _np_ptr(F), sat.ctypes.data,
+                                     sol.ctypes.data, first.ctypes.data)
+        self._raise(rc)
+        return F, sat, sol, first
+
+    def query(self, key: int) -> int:
+        return int(self._L.afsat_query(self._h, key))
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            self._L.afsat_destroy(self._h)
+            self._h = C.c_void_p(None)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -2,7 +2,7 @@
 
 This module holds NONE of the method's arithmetic (no Fourier coefficients, no FE, no
 gradient, no satisfaction predicate): it only draws constraint tables, masks and starting
-points.  It imports numpy only, so both ``oracle/`` users and the CUDA binding's users can
+points.  It imports numpy only, so the tests of the CPU oracle and the users of the CUDA binding can
 consume exactly the same arrays.
 
 The paper's own workloads (hard random k-SAT; the random-cardinality and
@@ -63,6 +63,11 @@ def _draw_subsets(rng: np.random.Generator, n: int, k: int, count: int) -> np.nd
     Draw k independent uniform indices per row and redraw the rows that contain a repeat
     (SURVEY.md §8(d)); conditional on no repeat the row is a uniform ordered k-subset.
     """
+    if k > n:
+        raise ValueError(f"cannot draw {k} distinct variables out of {n}")
+    if k * k > 2 * n:
+        # rejection would rarely succeed: take the first k entries of a uniform permutation per row
+        return np.argsort(rng.random((count, n)), axis=1)[:, :k].astype(np.int32)
     out = rng.integers(0, n, size=(count, k), dtype=np.int64)
     if k == 1:
         return out.astype(np.int32)
