@@ -154,10 +154,22 @@ enum afsat_query_key {
     AFSAT_Q_NNZ             = 3,
     AFSAT_Q_WORKSPACE_BYTES = 4,
     AFSAT_Q_SM_COUNT        = 5,
-    AFSAT_Q_FP_INSTR_PER_CANDIDATE = 6  /* model count of FP instructions for one eval_grad of one
+    AFSAT_Q_FP_INSTR_PER_CANDIDATE = 6, /* model count of FP instructions for one eval_grad of one
                                            candidate over all constraints (DESIGN.md cost model)  */
+    AFSAT_Q_PROFILED_EVAL_NS = 7,       /* afsat_set_profiling: device time of the evaluation kernels
+                                           (a1-a5, a7-a8) since profiling was switched on, in ns;
+                                           SYNCHRONISES with the recorded events                  */
+    AFSAT_Q_PROFILED_EVAL_LAUNCHES = 8  /* number of evaluation-kernel launches in that time       */
 };
 int64_t afsat_query(const afsat_ctx *ctx, int32_t key);
+
+/*
+ * afsat_set_profiling -- on != 0: bracket every evaluation-kernel launch of this context with CUDA
+ * events on the launching stream (the roofline numerator of bench.py is measured this way, live,
+ * inside the step); on == 0: stop.  Either call resets the accumulated time.  Costs two event
+ * records per launch, so it is off by default and off in every timed headline region.
+ */
+int afsat_set_profiling(afsat_ctx *ctx, int32_t on);
 
 const char *afsat_version(void);
 

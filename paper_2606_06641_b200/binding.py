@@ -20,14 +20,15 @@ FLAG_ROBUST = 1
 MAX_LEN = 64
 
 Q_KERNEL_LAUNCHES, Q_NUM_SIGNATURES, Q_NUM_BUCKETS, Q_NNZ, Q_WORKSPACE_BYTES, Q_SM_COUNT, \
-    Q_FP_INSTR_PER_CANDIDATE = range(7)
+    Q_FP_INSTR_PER_CANDIDATE, Q_PROFILED_EVAL_NS, Q_PROFILED_EVAL_LAUNCHES = range(9)
 
 ERROR_NAMES = {0: "AFSAT_OK", -1: "AFSAT_E_INVALID", -2: "AFSAT_E_LENGTH", -3: "AFSAT_E_VARIABLE",
                -4: "AFSAT_E_SIGN", -5: "AFSAT_E_DUPLICATE", -6: "AFSAT_E_PARAM",
                -7: "AFSAT_E_NOMEM", -8: "AFSAT_E_CUDA"}
 
 EXPORTS = ["afsat_create", "afsat_destroy", "afsat_last_error", "afsat_eval_grad", "afsat_check",
-           "afsat_step", "afsat_step_host", "afsat_host_tables", "afsat_query", "afsat_version"]
+           "afsat_step", "afsat_step_host", "afsat_host_tables", "afsat_query", "afsat_version",
+           "afsat_set_profiling"]
 
 
 class AfsatError(RuntimeError):
@@ -64,6 +65,8 @@ def load_library():
     L.afsat_host_tables.argtypes = [i32, i32, i32, u32, vp, vp]
     L.afsat_query.restype = i64
     L.afsat_query.argtypes = [vp, i32]
+    L.afsat_set_profiling.restype = C.c_int
+    L.afsat_set_profiling.argtypes = [vp, i32]
     L.afsat_version.restype = C.c_char_p
     L.afsat_version.argtypes = []
     _lib = L
@@ -221,6 +224,14 @@ class Context:
                                      sol.ctypes.data, first.ctypes.data)
         self._raise(rc)
         return F, sat, sol, first
+
+    def set_profiling(self, on: bool):
+        self._raise(self._L.afsat_set_profiling(self._h, 1 if on else 0))
+
+    def profiled_eval_ms(self):
+        """(device ms spent in the evaluation kernels, number of their launches) since
+        set_profiling(True); synchronises."""
+        return self.query(Q_PROFILED_EVAL_NS) * 1e-6, self.query(Q_PROFILED_EVAL_LAUNCHES)
 
     def query(self, key: int) -> int:
         return int(self._L.afsat_query(self._h, key))

@@ -51,6 +51,11 @@ struct afsat_ctx {
     cudaStream_t own_stream = nullptr;
     size_t ws_bytes = 0;
     int64_t launches = 0;
+    // afsat_set_profiling: event pairs around the evaluation-kernel launches
+    bool profiling = false;
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_events;
+    double prof_ns = 0.0;
+    int64_t prof_launches = 0;
     std::string err;
 };
 
@@ -93,6 +98,35 @@ inline int64_t cost_of(int k, int n_real, int n_cplx) { return (int64_t)k * (12 
 
 inline int warps_per_cta(const afsat_ctx *c) { return (int)std::min<int64_t>(8, c->ldb / 32); }
 
+// brackets one evaluation-kernel launch with events when profiling is on
+struct ProfScope {
+    afsat_ctx *c; cudaStream_t st; cudaEvent_t e0 = nullptr, e1 = nullptr;
+    ProfScope(afsat_ctx *c_, cudaStream_t st_) : c(c_), st(st_)
+    {
+        if (!c->profiling) return;
+        if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) { e0 = e1 = nullptr; return; }
+        cudaEventRecord(e0, st);
+    }
+    ~ProfScope()
+    {
+        if (!e0) return;
+        cudaEventRecord(e1, st);
+        c->prof_events.emplace_back(e0, e1);
+    }
+};
+
+void prof_drain(afsat_ctx *c, bool keep)
+{
+    for (auto &pr : c->prof_events) {
+        if (keep && cudaEventSynchronize(pr.second) == cudaSuccess) {
+            float ms = 0.f;
+            if (cudaEventElapsedTime(&ms, pr.first, pr.second) == cudaSuccess) { c->prof_ns += (double)ms * 1e6; ++c->prof_launches; }
+        }
+        cudaEventDestroy(pr.first); cudaEventDestroy(pr.second);
+    }
+    c->prof_events.clear();
+}
+
 template <typename T>
 int launch_eval(afsat_ctx *ctx, const T *x, T *G, T *Fpart, int32_t *satacc, bool grad, cudaStream_t st)
 {
@@ -104,6 +138,7 @@ int launch_eval(afsat_ctx *ctx, const T *x, T *G, T *Fpart, int32_t *satacc, boo
     for (int cls = 0; cls < N_CLS; ++cls) {
         const int nit = ctx->cls_begin[cls + 1] - ctx->cls_begin[cls];
         if (nit == 0) continue;
+        ProfScope prof(ctx, st);
         p.items = ctx->d_items + ctx->cls_begin[cls];
         p.item_index_base = ctx->cls_begin[cls];
         if (cls != CLS_LONG) {
@@ -449,9 +484,19 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
     return AFSAT_OK;
 }
 
+int afsat_set_profiling(afsat_ctx *ctx, int32_t on)
+{
+    if (!ctx) return AFSAT_E_INVALID;
+    prof_drain(ctx, false);
+    ctx->prof_ns = 0.0; ctx->prof_launches = 0;
+    ctx->profiling = on != 0;
+    return AFSAT_OK;
+}
+
 void afsat_destroy(afsat_ctx *ctx)
 {
     if (!ctx) return;
+    prof_drain(ctx, false);
     cudaFree(ctx->d_lits); cudaFree(ctx->d_cons_sig); cudaFree(ctx->d_sigs); cudaFree(ctx->d_rows);
     cudaFree(ctx->d_fixed); cudaFree(ctx->d_items); cudaFree(ctx->d_G); cudaFree(ctx->d_Fpart);
     cudaFree(ctx->d_satacc); cudaFree(ctx->d_any);
@@ -544,6 +589,10 @@ int afsat_step_host(afsat_ctx *ctx, void *h_x, double eta, int32_t n_steps, void
 int64_t afsat_query(const afsat_ctx *ctx, int32_t key)
 {
     if (!ctx) return -1;
+    if (key == AFSAT_Q_PROFILED_EVAL_NS || key == AFSAT_Q_PROFILED_EVAL_LAUNCHES) {
+        prof_drain(const_cast<afsat_ctx *>(ctx), true);
+        return key == AFSAT_Q_PROFILED_EVAL_NS ? (int64_t)ctx->prof_ns : ctx->prof_launches;
+    }
     switch (key) {
     case AFSAT_Q_KERNEL_LAUNCHES: return ctx->launches;
     case AFSAT_Q_NUM_SIGNATURES:  return ctx->n_sigs;

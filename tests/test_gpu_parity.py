@@ -1,0 +1,318 @@
+"""GPU parity tests (`-m gpu`): the CUDA path, called through the C ABI (ctypes binding), against
+the long-double CPU oracle on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star, restated in DESIGN.md "Tolerances"):
+  fp32: |F - F*| <= 1e-4 * m + 1e-5 * |F*| ; |G - G*| <= 1e-4 per component   (k <= 20)
+  fp64: 1e-10 on F (abs, times max(1, m/1000) for the summation) and on G
+  discrete outputs (sat_count, is_solution, first_step): bit-exact.
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle as O
+from paper_2606_06641_b200 import binding as Bd
+from paper_2606_06641_b200 import build as Build
+from paper_2606_06641_b200 import instances as I
+from tests import refmath as R
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    Build.build()
+    assert torch.cuda.is_available()
+
+
+def dev(x):
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+def tol_F(m, Fstar, dtype):
+    if dtype == 32:
+        return 1e-4 * max(m, 1) + 1e-5 * np.abs(Fstar)
+    return 1e-10 * max(1.0, m / 1000.0) + 1e-12 * np.abs(Fstar)
+
+
+def run_eval(inst, x_np, B, dtype, flags=0):
+    """GPU eval_grad on x_np [n, ldb]; returns (F, G) as float64 numpy."""
+    ctx = Bd.Context.from_instance(inst, batch=B, ldb=x_np.shape[1], dtype=dtype, flags=flags)
+    x = dev(x_np.astype(np.float32 if dtype == 32 else np.float64))
+    F, G = ctx.eval_grad(x)
+    torch.cuda.synchronize()
+    out = F.cpu().numpy().astype(np.float64), G.cpu().numpy().astype(np.float64)
+    ctx.close()
+    return out
+
+
+def assert_eval_parity(inst, x_np, B, dtype, gtol=None, flags=0):
+    F, G = run_eval(inst, x_np, B, dtype, flags)
+    Fo, Go = O.eval_grad(inst, x_np.astype(np.float64), B)
+    assert np.all(np.abs(F - Fo) <= tol_F(inst.n_cons, Fo, dtype)), np.abs(F - Fo).max()
+    gtol = gtol if gtol is not None else (1e-4 if dtype == 32 else 1e-10)
+    err = np.abs(G[:, :B] - Go[:, :B]).max() if B else 0.0
+    assert err <= gtol, err
+    assert np.all(G[:, B:] == 0)                                     # padding columns are zero
+    if inst.fixed is not None:
+        assert np.all(G[inst.fixed != 0] == 0)                       # masked gradient
+    return F, G
+
+
+# ---- single-shot eval_grad ---------------------------------------------------------------------
+
+@pytest.mark.parametrize("dtype", [32, 64])
+def test_cfg0_eval_grad(dtype):
+    inst = I.make_config(0)
+    x = I.make_x0(inst)
+    assert_eval_parity(inst, x, inst.batch, dtype)
+
+
+@pytest.mark.parametrize("dtype", [32, 64])
+@pytest.mark.parametrize("B", [1, 31, 100, 257])
+def test_mixed_all_types_ragged_batch(dtype, B):
+    """every type, k = 1..20, every parameter incl. trivial t = 0 / t = k, fixed variables,
+    batch sizes that are not multiples of 32 (ragged tail) and span several CTAs."""
+    inst = I.make_mixed(n=60, m=300, kmin=1, kmax=20, seed=11 + B, batch=B, with_fixed=True)
+    x = I.make_x0(inst, seed=5 + B, batch=B)
+    assert_eval_parity(inst, x, B, dtype)
+
+
+@pytest.mark.parametrize("dtype", [32, 64])
+def test_long_constraints_uniform_x(dtype):
+    """k = 21..64 (long path).  At uniform-random X fp32 holds ~2e-4, so the
+    fp32 gradient bound here is 1e-3; fp64 must reach 1e-10 up to k = 50 (reading A18)."""
+    kmax = 64 if dtype == 32 else 50
+    inst = I.make_mixed(n=80, m=120, kmin=21, kmax=kmax, seed=23, batch=64,
+                        types=[I.ATLEAST, I.ATMOST, I.EXACTLY, I.OR, I.NAE, I.XOR])
+    # keep cardinality thresholds central (the paper's workloads; t near 0/k is trivial anyway)
+    x = I.make_x0(inst, seed=77, batch=64)
+    F, G = run_eval(inst, x, 64, dtype)
+    Fo, Go = O.eval_grad(inst, x.astype(np.float64), 64)
+    if dtype == 32:
+        assert np.abs(F - Fo).max() <= 1e-4 * inst.n_cons + 1e-2
+        assert np.abs(G - Go).max() <= 5e-3
+    else:
+        assert np.abs(F - Fo).max() <= 1e-9
+        assert np.abs(G - Go).max() <= 1e-10
+
+
+@pytest.mark.parametrize("dtype", [32, 64])
+def test_corners_and_zero(dtype):
+    """x exactly +-1 (where PGD parks variables: factors vanish, division-based leave-one-out is
+    singular), x = 0 and -0.0.  FE_C = +-1 exactly at corners."""
+    inst = I.make_mixed(n=40, m=200, kmin=1, kmax=12, seed=3, batch=64, with_fixed=True)
+    rng = np.random.default_rng(9)
+    assign = rng.integers(0, 2, size=(inst.n_vars, 64)).astype(bool)
+    x = I.corner_x(inst, assign)
+    x[5, :8] = 0.0
+    x[6, :8] = -0.0
+    x[7, 8:16] = 0.25
+    F, G = assert_eval_parity(inst, x, 64, dtype)
+    sat, sol = O.check(inst, x.astype(np.float64), 64)
+    pure = np.ones(64, dtype=bool); pure[:16] = False            # columns that are pure corners
+    want = inst.n_cons - 2.0 * sat                               # sum of -1 (sat) / +1 (violated)
+    assert np.abs(F[pure] - want[pure]).max() <= (1e-3 if dtype == 32 else 1e-10)
+
+
+def test_empty_instance_and_single_constraint():
+    inst = I.make_mixed(n=8, m=1, kmin=3, kmax=3, seed=1, batch=32)
+    x = I.make_x0(inst, seed=2, batch=32)
+    assert_eval_parity(inst, x, 32, 32)
+    empty = I.Instance("none", 8, np.zeros(1, dtype=np.int64), np.zeros(0, dtype=np.int32),
+                       np.zeros(0, dtype=np.int8), np.zeros(0, dtype=np.uint8),
+                       np.zeros(0, dtype=np.int32), batch=32)
+    F, G = run_eval(empty, x, 32, 32)
+    assert np.all(F == 0) and np.all(G == 0)
+    ctx = Bd.Context.from_instance(empty, batch=32)
+    sat, sol = ctx.check(dev(x))
+    assert np.all(sat.cpu().numpy() == 0) and np.all(sol.cpu().numpy() == 1)   # 0 == m
+
+
+def test_robust_flag_same_values():
+    inst = I.make_mixed(n=60, m=150, kmin=2, kmax=40, seed=31, batch=64)
+    x = I.make_x0(inst, seed=4, batch=64)
+    F, G = run_eval(inst, x, 64, 64, flags=Bd.FLAG_ROBUST)
+    Fo, Go = O.eval_grad(inst, x.astype(np.float64), 64)
+    assert np.abs(F - Fo).max() <= 1e-10 and np.abs(G - Go).max() <= 1e-10
+
+
+def test_worked_k3_golden():
+    """tests/golden/worked_k3.txt (brute force of Eq. (1)) through the GPU."""
+    from pathlib import Path
+    y = [0.5, -0.25, 0.75]
+    for line in (Path(__file__).parent / "golden" / "worked_k3.txt").read_text().splitlines():
+        line = line.strip()
+        if not line or line.startswith("#"):
+            continue
+        head, _, fe_s, g_s = [s.strip() for s in line.split("|")]
+        tok = head.split()
+        t, p = int(tok[1]), int(tok[2])
+        fe, g = float(fe_s), [float(v) for v in g_s.split()]
+        inst = I.Instance("w", 3, np.array([0, 3], dtype=np.int64), np.arange(3, dtype=np.int32),
+                          np.ones(3, dtype=np.int8), np.array([t], dtype=np.uint8),
+                          np.array([p], dtype=np.int32), batch=1)
+        x = np.zeros((3, 32), dtype=np.float32)
+        x[:, 0] = y
+        F, G = run_eval(inst, x, 1, 32)
+        assert abs(F[0] - fe) < 1e-6 and np.abs(G[:, 0] - g).max() < 1e-6, (tok[0], F[0], G[:, 0])
+
+
+# ---- discrete check ----------------------------------------------------------------------------
+
+@pytest.mark.parametrize("dtype", [32, 64])
+def test_check_bit_exact(dtype):
+    inst = I.make_mixed(n=50, m=400, kmin=1, kmax=30, seed=19, batch=200, with_fixed=True)
+    x = I.make_x0(inst, seed=8, batch=200)
+    x[3, :50] = 0.0
+    x[4, :50] = -0.0
+    x[9, 50:80] = -1.0
+    ctx = Bd.Context.from_instance(inst, batch=200, ldb=x.shape[1], dtype=dtype)
+    sat, sol = ctx.check(dev(x.astype(np.float32 if dtype == 32 else np.float64)))
+    so, lo = O.check(inst, x.astype(np.float64), 200)
+    assert np.array_equal(sat.cpu().numpy(), so) and np.array_equal(sol.cpu().numpy(), lo)
+    assert np.array_equal(so, R.recount(inst, x, 200))
+
+
+def test_check_planted_solution():
+    base = I.make_mixed(n=64, m=300, kmin=2, kmax=16, seed=29, batch=64, with_fixed=True)
+    base.meta["admissible"] = [R.admissible_taus(int(t), int(k), int(p)) or [0]
+                               for t, k, p in zip(base.ctype, base.lengths(), base.param)]
+    ok = np.array([len(R.admissible_taus(int(t), int(k), int(p))) > 0
+                   for t, k, p in zip(base.ctype, base.lengths(), base.param)])
+    inst, hidden = I.plant_solution(base, seed=3)
+    x = I.corner_x(inst, np.repeat(hidden[:, None], 64, axis=1))
+    free = np.nonzero(inst.fixed == 0)[0]
+    x[free[0], 1] *= -1                                        # candidate 1: one variable flipped
+    ctx = Bd.Context.from_instance(inst, batch=64)
+    sat, sol = ctx.check(dev(x))
+    sat, sol = sat.cpu().numpy(), sol.cpu().numpy()
+    assert sat[0] == ok.sum() and sol[0] == (1 if ok.all() else 0)
+    assert np.array_equal(sat, R.recount(inst, x, 64))
+
+
+# ---- afsat_step: teacher-forced and free-running --------------------------------------------------
+
+@pytest.mark.parametrize("dtype", [32, 64])
+def test_step_teacher_forced(dtype):
+    """Each GPU step, started from the GPU's own X(t-1), must land within eta*1e-4 (fp32) /
+    1e-10 (fp64) of the oracle's step from the same X(t-1); discrete outputs computed from the
+    GPU's X(t) are bit-exact (SURVEY.md parity protocol (ii))."""
+    inst = I.make_mixed(n=48, m=260, kmin=1, kmax=14, seed=41, batch=96, with_fixed=True)
+    B, eta = 96, 0.1
+    x0 = I.make_x0(inst, seed=6, batch=B)
+    ctx = Bd.Context.from_instance(inst, batch=B, ldb=x0.shape[1], dtype=dtype)
+    npdt = np.float32 if dtype == 32 else np.float64
+    x = dev(x0.astype(npdt))
+    state = None
+    for t in range(1, 9):
+        prev = x.cpu().numpy().astype(np.float64)
+        F, sat, sol, first = ctx.step(x, eta, 1, step_base=t - 1, state=state)
+        state = (sol, first)
+        now = x.cpu().numpy().astype(np.float64)
+        st_prev = None if t == 1 else (sol_prev, first_prev)
+        Xo, Fo, sato, solo, firsto = O.step(inst, prev, eta, 1, B, step_base=t - 1, state=st_prev)
+        lim = eta * 1e-4 if dtype == 32 else 1e-10
+        assert np.abs(now[:, :B] - Xo[:, :B]).max() <= lim
+        s2, l2 = O.check(inst, now, B)                             # discrete outputs on GPU's X(t)
+        assert np.array_equal(sat.cpu().numpy(), s2)
+        sol_np = sol.cpu().numpy()
+        newly = (s2 == inst.n_cons)
+        if st_prev is not None:
+            assert np.all(sol_np[sol_prev != 0] == 1)
+            newly = newly | (sol_prev != 0)
+        assert np.array_equal(sol_np != 0, newly)
+        assert np.all(np.abs(F.cpu().numpy() - O.eval_grad(inst, now, B, grad=False))
+                      <= tol_F(inst.n_cons, Fo, dtype))
+        sol_prev, first_prev = sol_np.copy(), first.cpu().numpy().copy()
+
+
+@pytest.mark.parametrize("seed", [6641000, 6641002, 6641007])
+def test_cfg0_free_running_solve_rate(seed):
+    """Config 0 (n=50, m=213 3-SAT, B=64, 200 steps, eta=0.1): GPU-driven fp32 search vs the
+    oracle-driven search from the same x0: same solved flags (solve-rate), same first-solved steps."""
+    inst = I.make_config(0, instance_seed=seed)
+    x0 = I.make_x0(inst)
+    ctx = Bd.Context.from_instance(inst, dtype=32)
+    x = dev(x0)
+    F, sat, sol, first = ctx.step(x, inst.eta, inst.steps)
+    Xo, Fo, sato, solo, firsto = O.step(inst, x0.astype(np.float64), inst.eta, inst.steps, inst.batch)
+    assert np.array_equal(sol.cpu().numpy(), solo)
+    assert np.array_equal(first.cpu().numpy(), firsto)
+    assert np.array_equal(sat.cpu().numpy(), sato)
+    assert np.abs(x.cpu().numpy()[:, :64] - Xo[:, :64]).max() < 1e-3
+
+
+def test_step_multi_equals_repeated_single_and_freeze():
+    """n_steps in one call == the same number of single-step calls with resume (bit for bit), and
+    a solved candidate stays frozen."""
+    inst = I.make_config(0, instance_seed=6641007)
+    x0 = I.make_x0(inst)
+    ctx = Bd.Context.from_instance(inst)
+    xa, xb = dev(x0), dev(x0)
+    Fa, sata, sola, firsta = ctx.step(xa, 0.1, 60)
+    state = None
+    for t in range(60):
+        Fb, satb, solb, firstb = ctx.step(xb, 0.1, 1, step_base=t, state=state)
+        state = (solb, firstb)
+    assert torch.equal(sola, solb) and torch.equal(firsta, firstb) and torch.equal(sata, satb)
+    assert (xa - xb).abs().max().item() <= 1e-5       # RED order may differ run to run
+    # frozen: continue 20 steps, solved columns must not move
+    solved = sola.cpu().numpy().astype(bool)
+    before = xa.clone()
+    ctx.step(xa, 0.1, 20, step_base=60, state=(sola, firsta))
+    if solved.any():
+        cols = torch.from_numpy(np.nonzero(solved)[0]).cuda()
+        assert torch.equal(before[:, cols], xa[:, cols])
+
+
+def test_step_host_end_to_end():
+    inst = I.make_config(0)
+    x0 = I.make_x0(inst)
+    ctx = Bd.Context.from_instance(inst)
+    hx = torch.from_numpy(x0.copy()).pin_memory()
+    F, sat, sol, first = ctx.step_host(hx, 0.1, 50)
+    x = dev(x0)
+    F2, sat2, sol2, first2 = ctx.step(x, 0.1, 50)
+    assert np.array_equal(sat, sat2.cpu().numpy()) and np.array_equal(sol, sol2.cpu().numpy())
+    assert np.array_equal(first, first2.cpu().numpy())
+    assert np.abs(hx.numpy() - x.cpu().numpy()).max() <= 1e-5
+
+
+def test_any_solved_flag_pinned():
+    inst = I.make_config(0, instance_seed=6641007)
+    x = dev(I.make_x0(inst))
+    ctx = Bd.Context.from_instance(inst)
+    flag = torch.zeros(2, dtype=torch.int32).pin_memory()
+    F, sat, sol, first = ctx.step(x, 0.1, 200, h_any_solved=flag)
+    torch.cuda.synchronize()
+    f = first.cpu().numpy()
+    if (f >= 0).any():
+        assert flag[0].item() == 1 and flag[1].item() == f[f >= 0].min()
+    else:
+        assert flag[0].item() == 0
+
+
+# ---- scaled-down versions of configs 1-4 (several tiles + ragged tails) -----------------------------
+
+@pytest.mark.parametrize("cfg,scale,B", [(1, 0.01, 96), (2, 0.05, 160), (4, 0.002, 96)])
+def test_config_shapes_small(cfg, scale, B):
+    inst = I.make_config(cfg, scale=scale, batch=B)
+    x = I.make_x0(inst, batch=B)
+    assert_eval_parity(inst, x, B, 32)
+    ctx = Bd.Context.from_instance(inst, batch=B)
+    sat, sol = ctx.check(dev(x))
+    so, lo = O.check(inst, x.astype(np.float64), B)
+    assert np.array_equal(sat.cpu().numpy(), so)
+
+
+def test_config3_small_both_precisions():
+    inst = I.make_config(3, scale=0.03, batch=64)
+    x = I.make_x0(inst, batch=64)
+    Fo, Go = O.eval_grad(inst, x.astype(np.float64), 64)
+    F64, G64 = run_eval(inst, x, 64, 64)
+    assert np.abs(F64 - Fo).max() <= 1e-9 and np.abs(G64 - Go).max() <= 1e-10
+    F32, G32 = run_eval(inst, x, 64, 32)
+    # fp32 at k = 30..50: reported, bounded loosely (<= 2e-4 per constraint at x0)
+    assert np.abs(F32 - Fo).max() <= 1e-4 * inst.n_cons + 1e-2
+    assert np.abs(G32 - Go).max() <= 2e-2
