@@ -66,6 +66,14 @@ __device__ __forceinline__ T gather_literal(const T *__restrict__ x, int64_t ldb
     return (lit < 0) ? -v : v;
 }
 
+// a7: the VARIABLE rounds to True iff x < 0 (x = 0, -0.0 -> False); a negated literal is true iff
+// the variable is False -- so the tie x = 0 makes the literal -x TRUE (y = -0.0 is not "< 0").
+template <typename T>
+__device__ __forceinline__ int literal_true(T y, int32_t lit)
+{
+    return (lit < 0) ? !(y > T(0)) : (y < T(0));      // y = -x for negated literals: x < 0 <=> y > 0
+}
+
 __device__ __forceinline__ int sat_bit(const SigDev &sg, int tau)
 {
     return (int)(((tau < 64) ? (sg.sat_lo >> tau) : (sg.sat_hi >> (tau - 64))) & 1ull);
@@ -143,7 +151,7 @@ __device__ __forceinline__ void run_item_reg(const EvalParams<T> &p, const Item 
 #pragma unroll
         for (int i = 0; i < K; ++i) {
             y[i] = gather_literal(p.x, p.ldb, b, lit[i]);
-            tau += (y[i] < T(0)) ? 1 : 0;
+            tau += literal_true(y[i], lit[i]);
             g[i] = T(0);
         }
         sat += sat_bit(sg, tau);
@@ -208,8 +216,9 @@ __global__ void __launch_bounds__(256) k_eval_long(const EvalParams<T> p, int km
         const SigDev sgd = p.sigs[p.cons_sig[c]];
         int tau = 0;
         for (int i = 0; i < k; ++i) {
-            const T yi = gather_literal(p.x, p.ldb, b, __ldg(L + i));
-            tau += (yi < T(0)) ? 1 : 0;
+            const int32_t lit_i = __ldg(L + i);
+            const T yi = gather_literal(p.x, p.ldb, b, lit_i);
+            tau += literal_true(yi, lit_i);
             sy[i * 32] = yi;
             sg[i * 32] = T(0);
         }
@@ -285,7 +294,10 @@ __global__ void __launch_bounds__(256) k_check(const EvalParams<T> p)
     for (int c = it.c_begin; c < it.c_end; ++c, L += k) {
         const SigDev sg = p.sigs[p.cons_sig[c]];
         int tau = 0;
-        for (int i = 0; i < k; ++i) tau += (gather_literal(p.x, p.ldb, b, __ldg(L + i)) < T(0)) ? 1 : 0;
+        for (int i = 0; i < k; ++i) {
+            const int32_t lit_i = __ldg(L + i);
+            tau += literal_true(gather_literal(p.x, p.ldb, b, lit_i), lit_i);
+        }
         sat += sat_bit(sg, tau);
     }
     atomicAdd(p.satacc + b, sat);
