@@ -10,6 +10,7 @@
 #include <tuple>
 #include <vector>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include "afsat_internal.h"
@@ -21,28 +22,38 @@ namespace {
 
 thread_local std::string g_create_error;
 
-enum { CLS_A = 0, CLS_B = 1, CLS_C = 2, CLS_LONG = 3, N_CLS = 4 };   // k in [1,8] [9,16] [17,24] [25,64]
-inline int class_of(int k) { return k <= 8 ? CLS_A : k <= 16 ? CLS_B : k <= 24 ? CLS_C : CLS_LONG; }
+// length classes: register kernels for k in [1,8] and [9,16], shared-memory kernel for [17,64]
+enum { CLS_A = 0, CLS_B = 1, CLS_LONG = 2, N_CLS = 3 };
+inline int class_of(int k) { return k <= 8 ? CLS_A : k <= 16 ? CLS_B : CLS_LONG; }
+
+struct ClassGeom {              // how one length class maps candidates onto a CTA
+    int V = 1;                  // candidates per lane
+    int warps = CTA_WARPS;      // warps per CTA
+    int Wc = 1, Wk = CTA_WARPS; // candidate sub-tiles x constraint groups
+    size_t smem = 0;            // dynamic shared memory (long kernel only)
+};
 
 }  // namespace
 
 struct afsat_ctx {
     int32_t n = 0, m = 0, B = 0, dtype = 32, device = 0, sm_count = 148;
-    int64_t ldb = 0, nnz = 0;
+    int64_t ldb = 0, nnz = 0, tile_w = 0;
     uint32_t flags = 0;
     size_t esz = 4;
     // device tables
-    int32_t *d_lits = nullptr, *d_cons_sig = nullptr;
+    int32_t *d_lits = nullptr;
     SigDev *d_sigs = nullptr;
     void *d_rows = nullptr;
     int8_t *d_fixed = nullptr;
     Item *d_items = nullptr;
-    int32_t n_items = 0, cls_begin[N_CLS + 1] = {0, 0, 0, 0, 0};
+    int32_t n_items = 0, cls_begin[N_CLS + 1] = {0, 0, 0, 0};
+    ClassGeom geom[N_CLS];
     int32_t kmax_long = 0;
     int32_t n_sigs = 0, n_buckets = 0;
     int64_t fp_instr_per_candidate = 0;
     // workspace
-    void *d_G = nullptr, *d_Fpart = nullptr;
+    void *d_G = nullptr, *d_Fpart = nullptr;      // G scratch [n][tile_w]; Fpart [n_items][ldb]
+    uint32_t *d_bits = nullptr;                    // sign bits [n][ldb/32]
     int32_t *d_satacc = nullptr, *d_any = nullptr;
     // buffers of afsat_step_host (lazy)
     void *dh_x = nullptr, *dh_F = nullptr;
@@ -96,7 +107,7 @@ int upload(afsat_ctx *ctx, U **p, const std::vector<U> &h)
 // model count of FP instructions for one (constraint, candidate): DESIGN.md cost model
 inline int64_t cost_of(int k, int n_real, int n_cplx) { return (int64_t)k * (12 * n_cplx + 4 * n_real) + 2 * n_cplx + n_real; }
 
-inline int warps_per_cta(const afsat_ctx *c) { return (int)std::min<int64_t>(8, c->ldb / 32); }
+inline int pow2_floor(int64_t v) { int p = 1; while ((int64_t)p * 2 <= v) p *= 2; return p; }
 
 // brackets one evaluation-kernel launch with events when profiling is on
 struct ProfScope {
@@ -127,36 +138,40 @@ void prof_drain(afsat_ctx *c, bool keep)
     c->prof_events.clear();
 }
 
+// ---- launch of the evaluation kernels (a1-a5) for the candidate tile [b_begin, b_begin + width) ----
 template <typename T>
-int launch_eval(afsat_ctx *ctx, const T *x, T *G, T *Fpart, int32_t *satacc, bool grad, cudaStream_t st)
+int launch_eval(afsat_ctx *ctx, const T *x, T *G, int64_t g_ld, int64_t g_b0, T *Fpart, int64_t b_begin, int64_t width,
+                cudaStream_t st)
 {
     EvalParams<T> p;
-    p.x = x; p.G = G; p.Fpart = Fpart; p.satacc = satacc;
-    p.lits = ctx->d_lits; p.cons_sig = ctx->d_cons_sig; p.sigs = ctx->d_sigs;
-    p.rows = (const T *)ctx->d_rows; p.B = ctx->B; p.ldb = ctx->ldb;
-    const int wpc = warps_per_cta(ctx);
+    p.x = x; p.G = G; p.g_ld = g_ld; p.g_b0 = g_b0; p.Fpart = Fpart;
+    p.lits = ctx->d_lits; p.sigs = ctx->d_sigs; p.rows = (const T *)ctx->d_rows;
+    p.B = ctx->B; p.ldb = ctx->ldb; p.b_begin = b_begin;
+    const bool grad = G != nullptr;
+    constexpr int VA = sizeof(T) == 4 ? 2 : 1;
     for (int cls = 0; cls < N_CLS; ++cls) {
         const int nit = ctx->cls_begin[cls + 1] - ctx->cls_begin[cls];
         if (nit == 0) continue;
         ProfScope prof(ctx, st);
+        const ClassGeom &g = ctx->geom[cls];
         p.items = ctx->d_items + ctx->cls_begin[cls];
-        p.item_index_base = ctx->cls_begin[cls];
-        if (cls != CLS_LONG) {
-            dim3 block(32 * wpc), grid(nit, (unsigned)((ctx->ldb + 32 * wpc - 1) / (32 * wpc)));
-            if (cls == CLS_A) { if (grad) k_eval_reg<T, 1, 8, true><<<grid, block, 0, st>>>(p); else k_eval_reg<T, 1, 8, false><<<grid, block, 0, st>>>(p); }
-            if (cls == CLS_B) { if (grad) k_eval_reg<T, 9, 16, true><<<grid, block, 0, st>>>(p); else k_eval_reg<T, 9, 16, false><<<grid, block, 0, st>>>(p); }
-            if (cls == CLS_C) { if (grad) k_eval_reg<T, 17, 24, true><<<grid, block, 0, st>>>(p); else k_eval_reg<T, 17, 24, false><<<grid, block, 0, st>>>(p); }
+        p.frow_base = ctx->cls_begin[cls];
+        p.Wc = g.Wc; p.Wk = g.Wk;
+        const int64_t per_cta = (int64_t)32 * g.V * g.Wc;
+        dim3 block(32 * g.warps), grid(nit, (unsigned)((width + per_cta - 1) / per_cta));
+        if (cls == CLS_A) {
+            if (grad) k_eval_reg<T, 1, 8, VA, true, 2><<<grid, block, 0, st>>>(p);
+            else      k_eval_reg<T, 1, 8, VA, false, 2><<<grid, block, 0, st>>>(p);
+        } else if (cls == CLS_B) {
+            if (grad) k_eval_reg<T, 9, 16, 1, true, 1><<<grid, block, 0, st>>>(p);
+            else      k_eval_reg<T, 9, 16, 1, false, 1><<<grid, block, 0, st>>>(p);
         } else {
-            const size_t per_warp = (size_t)4 * ctx->kmax_long * 32 * sizeof(T);
-            int w = (int)std::max<size_t>(1, std::min<size_t>((size_t)wpc, (160 * 1024) / per_warp));
-            const size_t smem = per_warp * w;
-            dim3 block(32 * w), grid(nit, (unsigned)((ctx->ldb + 32 * w - 1) / (32 * w)));
             if (grad) {
-                CU(cudaFuncSetAttribute(k_eval_long<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-                k_eval_long<T, true><<<grid, block, smem, st>>>(p, ctx->kmax_long);
+                CU(cudaFuncSetAttribute(k_eval_long<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem));
+                k_eval_long<T, true><<<grid, block, g.smem, st>>>(p, ctx->kmax_long);
             } else {
-                CU(cudaFuncSetAttribute(k_eval_long<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-                k_eval_long<T, false><<<grid, block, smem, st>>>(p, ctx->kmax_long);
+                CU(cudaFuncSetAttribute(k_eval_long<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem));
+                k_eval_long<T, false><<<grid, block, g.smem, st>>>(p, ctx->kmax_long);
             }
         }
         ++ctx->launches;
@@ -165,18 +180,30 @@ int launch_eval(afsat_ctx *ctx, const T *x, T *G, T *Fpart, int32_t *satacc, boo
     return AFSAT_OK;
 }
 
-template <typename T>
-int launch_check(afsat_ctx *ctx, const T *x, int32_t *satacc, cudaStream_t st)
+// a8 on the words [w_begin, w_end) of the sign-bit array
+int launch_check_bits(afsat_ctx *ctx, int64_t w_begin, int64_t w_end, cudaStream_t st)
 {
-    if (ctx->n_items == 0) return AFSAT_OK;
-    EvalParams<T> p;
-    p.x = x; p.G = nullptr; p.Fpart = nullptr; p.satacc = satacc;
-    p.lits = ctx->d_lits; p.cons_sig = ctx->d_cons_sig; p.sigs = ctx->d_sigs;
-    p.rows = (const T *)ctx->d_rows; p.B = ctx->B; p.ldb = ctx->ldb;
-    p.items = ctx->d_items; p.item_index_base = 0;
-    const int wpc = warps_per_cta(ctx);
-    dim3 block(32 * wpc), grid(ctx->n_items, (unsigned)((ctx->ldb + 32 * wpc - 1) / (32 * wpc)));
-    k_check<T><<<grid, block, 0, st>>>(p);
+    if (ctx->n_items == 0 || w_end <= w_begin) return AFSAT_OK;
+    CheckParams p;
+    p.bits = ctx->d_bits; p.ldw = ctx->ldb / 32; p.lits = ctx->d_lits; p.sigs = ctx->d_sigs; p.items = ctx->d_items;
+    p.satacc = ctx->d_satacc; p.B = ctx->B; p.w_begin = (int32_t)w_begin; p.w_end = (int32_t)w_end;
+    const int64_t nw = w_end - w_begin;
+    p.wpb = std::min(32, pow2_floor(nw));
+    if (p.wpb < nw && p.wpb < 32) p.wpb *= 2;                         // cover a ragged word count in one CTA row
+    p.wpb = std::min(p.wpb, 32);
+    dim3 grid(ctx->n_items, (unsigned)((nw + p.wpb - 1) / p.wpb));
+    k_check_bits<<<grid, CTA_THREADS, 0, st>>>(p);
+    ++ctx->launches;
+    CU(cudaPeekAtLastError());
+    return AFSAT_OK;
+}
+
+template <typename T>
+int launch_pack(afsat_ctx *ctx, const T *x, cudaStream_t st)
+{
+    const unsigned gx = (unsigned)((ctx->ldb + CTA_THREADS - 1) / CTA_THREADS);
+    const unsigned gy = (unsigned)std::min<int64_t>(ctx->n, std::max<int64_t>(1, (int64_t)ctx->sm_count * 8 / gx));
+    k_pack_signs<T><<<dim3(gx, gy), CTA_THREADS, 0, st>>>(x, ctx->d_bits, ctx->n, ctx->B, ctx->ldb);
     ++ctx->launches;
     CU(cudaPeekAtLastError());
     return AFSAT_OK;
@@ -195,8 +222,11 @@ template <typename T>
 int eval_grad_t(afsat_ctx *ctx, const T *x, T *F, T *G, cudaStream_t st)
 {
     if (G) CU(cudaMemsetAsync(G, 0, (size_t)ctx->n * ctx->ldb * sizeof(T), st));
-    int rc = launch_eval<T>(ctx, x, G, F ? (T *)ctx->d_Fpart : nullptr, nullptr, G != nullptr, st);
-    if (rc) return rc;
+    for (int64_t b0 = 0; b0 < ctx->B; b0 += ctx->tile_w) {            // candidate tiles keep X/G tiles L2-resident
+        const int64_t w = std::min<int64_t>(ctx->tile_w, ctx->ldb - b0);
+        int rc = launch_eval<T>(ctx, x, G, ctx->ldb, 0, F ? (T *)ctx->d_Fpart : nullptr, b0, w, st);
+        if (rc) return rc;
+    }
     if (F) return reduce_F<T>(ctx, F, st);
     return AFSAT_OK;
 }
@@ -211,37 +241,43 @@ int step_t(afsat_ctx *ctx, T *x, double eta, int n_steps, int step_base, int res
         ++ctx->launches;
     }
     CU(cudaMemsetAsync(ctx->d_any, 0, 2 * sizeof(int32_t), st));
-    CU(cudaMemsetAsync(ctx->d_satacc, 0, (size_t)ctx->ldb * sizeof(int32_t), st));
-    CU(cudaMemsetAsync(ctx->d_G, 0, (size_t)ctx->n * ctx->ldb * sizeof(T), st));
-    const int upd_rows = std::min(ctx->n, std::max(1, (ctx->sm_count * 16) / std::max<int>(1, (int)((ctx->ldb + 255) / 256))));
-    dim3 ugrid((unsigned)((ctx->ldb + 255) / 256), upd_rows), ublock(256);
+    const int64_t tw = ctx->tile_w;
     for (int t = 1; t <= n_steps; ++t) {
-        // gradient at X(t-1); from t = 2 on the same pass also counts the satisfied constraints of
-        // X(t-1) (the check that Alg. 1 performs after step t-1), so the literals are read once.
-        int rc = launch_eval<T>(ctx, x, (T *)ctx->d_G, nullptr, t >= 2 ? ctx->d_satacc : nullptr, true, st);
-        if (rc) return rc;
-        if (t >= 2) {
-            k_flags<<<gb, tb, 0, st>>>(ctx->d_satacc, B, ctx->m, 0, step_base + t - 1, n_steps, sat, sol, first,
-                                       ctx->d_any, h_any_dev);
+        for (int64_t b0 = 0; b0 < B; b0 += tw) {
+            const int64_t w = std::min<int64_t>(tw, ctx->ldb - b0);
+            // a1-a5: gradient at X(t-1) into the (zeroed) tile scratch
+            int rc = launch_eval<T>(ctx, x, (T *)ctx->d_G, tw, b0, nullptr, b0, w, st);
+            if (rc) return rc;
+            // a6, a7, a9: X(t) = clamp(X(t-1) - eta G) on free variables of unsolved candidates, sign bits, G reset
+            const unsigned gx = (unsigned)((w + CTA_THREADS - 1) / CTA_THREADS);
+            const unsigned gy = (unsigned)std::min<int64_t>(ctx->n, std::max<int64_t>(1, (int64_t)ctx->sm_count * 8 / gx));
+            k_update<T><<<dim3(gx, gy), CTA_THREADS, 0, st>>>(x, (T *)ctx->d_G, tw, b0, ctx->d_fixed, sol, ctx->d_bits, (T)eta,
+                                                              ctx->n, B, ctx->ldb, b0, b0 + w);
             ++ctx->launches;
+            CU(cudaPeekAtLastError());
+            // a8: exact count on X(t)
+            rc = launch_check_bits(ctx, b0 / 32, (b0 + w) / 32, st);
+            if (rc) return rc;
         }
-        k_update<T><<<ugrid, ublock, 0, st>>>(x, (T *)ctx->d_G, ctx->d_fixed, sol, (T)eta, ctx->n, B, ctx->ldb);
+        k_flags<<<gb, tb, 0, st>>>(ctx->d_satacc, B, ctx->m, 1, step_base + t, sat, sol, first, ctx->d_any, h_any_dev);
         ++ctx->launches;
         CU(cudaPeekAtLastError());
     }
-    // tail: count (and optionally F) on the final X(T)
-    int rc;
-    if (F) {
-        rc = launch_eval<T>(ctx, x, nullptr, (T *)ctx->d_Fpart, ctx->d_satacc, false, st);
-        if (!rc) rc = reduce_F<T>(ctx, F, st);
-    } else {
-        rc = launch_check<T>(ctx, x, ctx->d_satacc, st);
+    if (n_steps == 0) {                                               // no step: count on X as it is, mark nothing
+        int rc = launch_pack<T>(ctx, x, st);
+        if (!rc) rc = launch_check_bits(ctx, 0, ctx->ldb / 32, st);
+        if (rc) return rc;
+        k_flags<<<gb, tb, 0, st>>>(ctx->d_satacc, B, ctx->m, 0, step_base, sat, sol, first, ctx->d_any, h_any_dev);
+        ++ctx->launches;
+        CU(cudaPeekAtLastError());
     }
-    if (rc) return rc;
-    k_flags<<<gb, tb, 0, st>>>(ctx->d_satacc, B, ctx->m, 1, step_base + n_steps, n_steps, sat, sol, first,
-                               ctx->d_any, h_any_dev);
-    ++ctx->launches;
-    CU(cudaPeekAtLastError());
+    if (F) {                                                          // objective at the final X
+        for (int64_t b0 = 0; b0 < B; b0 += tw) {
+            int rc = launch_eval<T>(ctx, x, nullptr, 0, 0, (T *)ctx->d_Fpart, b0, std::min<int64_t>(tw, ctx->ldb - b0), st);
+            if (rc) return rc;
+        }
+        return reduce_F<T>(ctx, F, st);
+    }
     return AFSAT_OK;
 }
 
@@ -351,7 +387,15 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
         memset(&d, 0, sizeof d);
         d.row_off = (int32_t)(rows.size() / 8);
         d.n_real = (int16_t)hs.n_real; d.n_cplx = (int16_t)hs.n_cplx;
-        d.sat_lo = hs.satmask_lo; d.sat_hi = hs.satmask_hi;
+        {   // discrete check scans the smaller of {satisfied, violated} counts (k_check_bits)
+            const int kk = hs.k;
+            auto mask_upto = [](int nbits) { return nbits >= 64 ? ~0ull : ((1ull << nbits) - 1ull); };
+            const uint64_t full_lo = mask_upto(std::min(kk + 1, 64)), full_hi = kk + 1 > 64 ? mask_upto(kk + 1 - 64) : 0ull;
+            const int nsat = __builtin_popcountll(hs.satmask_lo) + __builtin_popcountll(hs.satmask_hi);
+            if (2 * nsat <= kk + 1) { d.scan_lo = hs.satmask_lo; d.scan_hi = hs.satmask_hi; d.scan_is_sat = 1; }
+            else { d.scan_lo = ~hs.satmask_lo & full_lo; d.scan_hi = ~hs.satmask_hi & full_hi; d.scan_is_sat = 0; }
+            d.k = kk;
+        }
         rows.insert(rows.end(), hs.rows, hs.rows + 8 * (hs.n_real + hs.n_cplx));
         sig_k[kv.second] = hs.k;
         sig_cost[kv.second] = (int)cost_of(hs.k, hs.n_real, hs.n_cplx);
@@ -383,32 +427,65 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
         lit_off[n_cons] = w;
     }
 
-    // ---- work items: chunks of one length, sized by the cost model ------------------------------
+    // ---- candidate tile: X tile + G tile must stay L2-resident ------------
+    const size_t esz = dtype == 32 ? 4 : 8;
+    int64_t tile_w = ldb;
+    {
+        int64_t budget = (int64_t)48 << 20;                            // bytes of L2 for the X and G tiles
+        if (const char *e = getenv("AFSAT_L2_TILE_BYTES")) { long long v = atoll(e); if (v > 0) budget = v; }
+        const int64_t per_col = (int64_t)2 * n_vars * (int64_t)esz;
+        if (per_col * ldb > budget) tile_w = std::max<int64_t>(64, budget / per_col / 64 * 64);
+        if (const char *e = getenv("AFSAT_TILE_W")) { long long v = atoll(e); if (v >= 32 && v % 32 == 0) tile_w = v; }
+        tile_w = std::min<int64_t>(tile_w, ldb);
+    }
+
+    // ---- class geometry ---------------------------------------------------------------------------------
     int sm_count = 148;
-    const int wpc = (int)std::min<int64_t>(8, ldb / 32);
-    const int64_t tiles_y = (ldb + 32 * wpc - 1) / (32 * wpc);
-    const int64_t chunks_wanted = std::max<int64_t>(1, (int64_t)148 * 32 / tiles_y);
-    const int64_t cost_budget = std::max<int64_t>(1, total_cost / chunks_wanted);
+    ClassGeom geom[N_CLS];
+    int kmax_long = 0;
+    for (int32_t j = 0; j < n_cons; ++j) { const int k = sig_k[cons_sig[j]]; if (class_of(k) == CLS_LONG) kmax_long = std::max(kmax_long, k); }
+    for (int cls = 0; cls < N_CLS; ++cls) {
+        ClassGeom &g = geom[cls];
+        g.V = (cls == CLS_A && dtype == 32) ? 2 : 1;
+        g.warps = CTA_WARPS;
+        if (cls == CLS_LONG) {
+            const size_t fixed_b = (size_t)MAX_ROWS * 8 * esz + (size_t)LIT_CHUNK * 4 + (size_t)CTA_WARPS * 32 * esz;
+            const size_t per_warp = (size_t)4 * std::max(kmax_long, 1) * 32 * esz;
+            g.warps = pow2_floor(std::max<int64_t>(1, std::min<int64_t>(CTA_WARPS, (int64_t)((200 * 1024 - fixed_b) / per_warp))));
+            g.smem = fixed_b + per_warp * g.warps;
+        }
+        const int64_t cw = 32 * g.V;
+        g.Wc = std::min(g.warps, pow2_floor(std::max<int64_t>(1, (tile_w + cw - 1) / cw)));
+        if ((int64_t)g.Wc * cw < tile_w && g.Wc < g.warps && (int64_t)g.Wc * cw * 2 <= tile_w + cw - 1) g.Wc *= 2;
+        g.Wk = g.warps / g.Wc;
+    }
+
+    // ---- work items: chunks of ONE signature, sized by the cost model and by the literal staging buffer ----
     std::vector<Item> items;
-    int32_t cls_begin[N_CLS + 1] = {0, 0, 0, 0, 0};
-    int n_buckets = 0, kmax_long = 0;
+    int32_t cls_begin[N_CLS + 1] = {0, 0, 0, 0};
+    int n_buckets = 0;
     {
         int32_t j = 0;
-        int cur_cls = 0;
+        int cur_cls = 0, last_k = -1;
         while (j < n_cons) {
-            const int k = sig_k[cons_sig[j]];
+            const int sg = cons_sig[j];
+            const int k = sig_k[sg];
             int32_t e = j;
-            int64_t bucket_cost = 0;
-            while (e < n_cons && sig_k[cons_sig[e]] == k) { bucket_cost += sig_cost[cons_sig[e]]; ++e; }
-            ++n_buckets;
+            while (e < n_cons && cons_sig[e] == sg) ++e;
+            if (k != last_k) { ++n_buckets; last_k = k; }
             const int cls = class_of(k);
             while (cur_cls < cls) cls_begin[++cur_cls] = (int32_t)items.size();
-            if (cls == CLS_LONG) kmax_long = std::max(kmax_long, k);
-            const int64_t avg_cost = std::max<int64_t>(1, bucket_cost / (e - j));
-            int64_t chunk = std::min<int64_t>(1024, std::max<int64_t>(cls == CLS_LONG ? 1 : 4, (cost_budget + avg_cost - 1) / avg_cost));
+            const ClassGeom &g = geom[cls];
+            const int64_t tiles_y = (tile_w + (int64_t)32 * g.V * g.Wc - 1) / ((int64_t)32 * g.V * g.Wc);
+            const int64_t chunks_wanted = std::max<int64_t>(1, (int64_t)148 * 16 / tiles_y);
+            const int64_t cost_budget = std::max<int64_t>(1, total_cost / chunks_wanted);
+            const int64_t cost1 = std::max<int64_t>(1, sig_cost[sg]);
+            int64_t chunk = std::max<int64_t>(g.Wk, (cost_budget + cost1 - 1) / cost1);
+            chunk = std::min<int64_t>(chunk, LIT_CHUNK / k);
+            chunk = std::max<int64_t>(1, chunk);
             for (int32_t s = j; s < e; s += (int32_t)chunk) {
                 Item it;
-                it.k = k; it.c_begin = s; it.c_end = (int32_t)std::min<int64_t>(e, s + chunk); it.pad = 0;
+                it.k = k; it.sig = sg; it.c_begin = s; it.c_end = (int32_t)std::min<int64_t>(e, s + chunk);
                 it.lit_base = lit_off[s];
                 items.push_back(it);
             }
@@ -423,7 +500,9 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
     ctx->n = n_vars; ctx->m = n_cons; ctx->B = batch; ctx->ldb = ldb; ctx->dtype = dtype; ctx->device = device;
     ctx->flags = flags; ctx->esz = dtype == 32 ? 4 : 8; ctx->nnz = nnz; ctx->n_sigs = n_sigs; ctx->n_buckets = n_buckets;
     ctx->n_items = (int32_t)items.size(); ctx->kmax_long = kmax_long; ctx->fp_instr_per_candidate = total_cost;
+    ctx->tile_w = tile_w;
     memcpy(ctx->cls_begin, cls_begin, sizeof cls_begin);
+    for (int cls = 0; cls < N_CLS; ++cls) ctx->geom[cls] = geom[cls];
 
 #define CREATE_FAIL(rc_)                                   \
     do {                                                   \
@@ -449,7 +528,6 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
         ctx->sm_count = sm_count;
     }
     CREATE_FAIL(upload(ctx, &ctx->d_lits, lits));
-    CREATE_FAIL(upload(ctx, &ctx->d_cons_sig, cons_sig));
     CREATE_FAIL(upload(ctx, &ctx->d_sigs, sigs));
     CREATE_FAIL(upload(ctx, &ctx->d_items, items));
     if (dtype == 32) {
@@ -469,11 +547,12 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
     }
     {
         char *g = nullptr, *fp = nullptr;
-        CREATE_FAIL(dev_alloc(ctx, &g, (size_t)n_vars * ldb * ctx->esz, true));
+        CREATE_FAIL(dev_alloc(ctx, &g, (size_t)n_vars * tile_w * ctx->esz, true));
         ctx->d_G = g;
         CREATE_FAIL(dev_alloc(ctx, &fp, (size_t)std::max<int>(1, ctx->n_items) * ldb * ctx->esz, true));
         ctx->d_Fpart = fp;
     }
+    CREATE_FAIL(dev_alloc(ctx, &ctx->d_bits, (size_t)n_vars * (size_t)(ldb / 32), true));
     CREATE_FAIL(dev_alloc(ctx, &ctx->d_satacc, (size_t)ldb, true));
     CREATE_FAIL(dev_alloc(ctx, &ctx->d_any, 2, true));
     {
@@ -497,7 +576,7 @@ void afsat_destroy(afsat_ctx *ctx)
 {
     if (!ctx) return;
     prof_drain(ctx, false);
-    cudaFree(ctx->d_lits); cudaFree(ctx->d_cons_sig); cudaFree(ctx->d_sigs); cudaFree(ctx->d_rows);
+    cudaFree(ctx->d_lits); cudaFree(ctx->d_bits); cudaFree(ctx->d_sigs); cudaFree(ctx->d_rows);
     cudaFree(ctx->d_fixed); cudaFree(ctx->d_items); cudaFree(ctx->d_G); cudaFree(ctx->d_Fpart);
     cudaFree(ctx->d_satacc); cudaFree(ctx->d_any);
     cudaFree(ctx->dh_x); cudaFree(ctx->dh_F); cudaFree(ctx->dh_sat); cudaFree(ctx->dh_first); cudaFree(ctx->dh_sol);
@@ -523,9 +602,8 @@ int afsat_check(afsat_ctx *ctx, const void *d_x, int32_t *d_sat_count, uint8_t *
     int rc = set_device(ctx);
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
-    CU(cudaMemsetAsync(ctx->d_satacc, 0, (size_t)ctx->ldb * sizeof(int32_t), st));
-    rc = ctx->dtype == 32 ? launch_check<float>(ctx, (const float *)d_x, ctx->d_satacc, st)
-                          : launch_check<double>(ctx, (const double *)d_x, ctx->d_satacc, st);
+    rc = ctx->dtype == 32 ? launch_pack<float>(ctx, (const float *)d_x, st) : launch_pack<double>(ctx, (const double *)d_x, st);
+    if (!rc) rc = launch_check_bits(ctx, 0, ctx->ldb / 32, st);
     if (rc) return rc;
     k_check_finish<<<(ctx->B + 127) / 128, 128, 0, st>>>(ctx->d_satacc, ctx->B, ctx->m, d_sat_count, d_is_solution);
     ++ctx->launches;

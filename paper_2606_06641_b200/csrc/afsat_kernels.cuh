@@ -1,15 +1,21 @@
 // afsat_kernels.cuh -- sm_100a device code of the AFSAT hot path.
 //
-// Mapping: LANE = CANDIDATE.  X is variable-major [n][ldb], so the k literal
-// gathers of a constraint are k coalesced 128-byte row segments per warp, the constraint's
-// literal list / signature / weight rows are warp-uniform (no divergence), and all prefix
-// products live in registers.  A CTA covers one chunk of constraints of one length bucket
-// (blockIdx.x -> work item) times 32*warps candidates (blockIdx.y).
+// Mapping: LANE = V adjacent CANDIDATES.  X is variable-major [n][ldb], so
+// the k literal gathers of a constraint are k coalesced, vectorised row segments per warp
+// (LDG.64 for fp32, V = 2), the constraint's literal list / weight rows are warp-uniform (no
+// divergence; they are staged once per work item in shared memory), and all prefix products live in
+// registers.  A work item is a chunk of constraints of ONE signature (type, k, param); a CTA runs
+// one item for Wc x (32 V) candidates, its Wk = warps/Wc warp groups interleaving the constraints.
 //
-// Per constraint and DFT point p the thread evaluates (afsat.h afsat_host_tables)
+// Per constraint and retained DFT point p the thread evaluates (afsat_host_tables)
 //     f_i = a_p + b_p y_i,  P = prod_i f_i,  FE += Re(w_p P),
 //     dFE/dy_i += Re( (w_p b_p) * prefix_{i-1} * suffix_{i+1} )        (leave-one-out, no division)
-// and scatter-adds s_i dFE/dy_i into G[v_i][b] with one coalesced RED per literal per warp.
+// and scatter-adds s_i dFE/dy_i into G[v_i][b..b+V) with one coalesced vector RED per literal.
+//
+// Sign rounding and the exact discrete count (a7, a8) never touch floating point beyond the one
+// compare x < 0: k_update / k_pack_signs emit one bit per (variable, candidate) with a warp
+// ballot, and k_check_bits counts true literals for 32 candidates at a time in bit-sliced integer
+// arithmetic.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -20,304 +26,487 @@ constexpr int32_t LIT_NEG   = (int32_t)0x80000000u;  // y = -x (or the constant 
 constexpr int32_t LIT_FIXED = 0x40000000;            // y is the constant +-1, no gradient
 constexpr int32_t LIT_VAR   = 0x3FFFFFFF;
 
+constexpr int LIT_CHUNK = 4096;       // packed literals staged in shared memory per work item
+constexpr int CTA_THREADS = 256;
+constexpr int CTA_WARPS = CTA_THREADS / 32;
+constexpr int MAX_ROWS = 33;          // retained DFT points per signature: H <= 64/2 + 1
+
 struct SigDev {                 // 32 bytes, one per signature (type, k, param)
     int32_t row_off;            // first row in the weight table (8 scalars per row)
     int16_t n_real, n_cplx;     // real rows first, then complex rows
-    uint64_t sat_lo, sat_hi;    // bit tau: satisfied with tau true literals
-    int64_t pad;
+    uint64_t scan_lo, scan_hi;  // bit tau set: tau is in the SCANNED set of the discrete check
+    int32_t scan_is_sat;        // 1: scanned set = satisfied counts; 0: = violated counts (smaller)
+    int32_t k;
 };
 
-struct Item {                   // one CTA-sized chunk of constraints of a single length k
-    int32_t k;
+struct Item {                   // one CTA-sized chunk of constraints of a single signature
+    int32_t k, sig;
     int32_t c_begin, c_end;     // constraint range in bucket order
-    int32_t pad;
     int64_t lit_base;           // offset of c_begin's first packed literal
 };
 
 template <typename T>
 struct EvalParams {
     const T *x;                 // [n][ldb]
-    T *G;                       // [n][ldb] accumulated with RED (must be zero on entry) or null
-    T *Fpart;                   // [n_items][ldb] per-item partial objective or null
-    int32_t *satacc;            // [ldb] satisfied-count accumulator (RED.ADD.S32) or null
+    T *G;                       // gradient accumulator (RED; zero on entry) or null
+    int64_t g_ld;               // leading dimension of G (ldb, or the tile width of the scratch)
+    int64_t g_b0;               // G column of candidate b is (b - g_b0)
+    T *Fpart;                   // [n_frows][ldb] per-(item, warp group) partial objective or null
     const int32_t *lits;        // packed literals, bucket order
-    const int32_t *cons_sig;    // signature id per constraint, bucket order
     const SigDev *sigs;
     const T *rows;              // weight table
     const Item *items;          // items of this launch
-    int32_t item_index_base;    // row of Fpart for items[0]
+    int32_t frow_base;          // row of Fpart for (items[0], group 0)
     int32_t B;
     int64_t ldb;
+    int64_t b_begin;            // first candidate of this launch's tile
+    int32_t Wc, Wk;             // warps of a CTA: Wc candidate sub-tiles x Wk constraint groups
 };
 
 template <typename T> __device__ __forceinline__ T fma_(T a, T b, T c);
 template <> __device__ __forceinline__ float fma_<float>(float a, float b, float c) { return fmaf(a, b, c); }
 template <> __device__ __forceinline__ double fma_<double>(double a, double b, double c) { return fma(a, b, c); }
 
-template <typename T> __device__ __forceinline__ void red_add(T *p, T v) { atomicAdd(p, v); }
+// ---- vector gather / vector RED ------------------------------------------------------------------
+template <typename T, int V> struct VecIO;
+template <> struct VecIO<float, 1> {
+    static __device__ __forceinline__ void load(const float *p, float (&v)[1]) { v[0] = __ldg(p); }
+    static __device__ __forceinline__ void red(float *p, const float (&v)[1]) { atomicAdd(p, v[0]); }
+};
+template <> struct VecIO<float, 2> {
+    static __device__ __forceinline__ void load(const float *p, float (&v)[2])
+    {
+        const float2 t = __ldg(reinterpret_cast<const float2 *>(p));
+        v[0] = t.x; v[1] = t.y;
+    }
+    static __device__ __forceinline__ void red(float *p, const float (&v)[2])
+    {
+        asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(v[0]), "f"(v[1]) : "memory");
+    }
+};
+template <> struct VecIO<float, 4> {
+    static __device__ __forceinline__ void load(const float *p, float (&v)[4])
+    {
+        const float4 t = __ldg(reinterpret_cast<const float4 *>(p));
+        v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w;
+    }
+    static __device__ __forceinline__ void red(float *p, const float (&v)[4])
+    {
+        asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(v[0]), "f"(v[1]), "f"(v[2]), "f"(v[3])
+                     : "memory");
+    }
+};
+template <> struct VecIO<double, 1> {
+    static __device__ __forceinline__ void load(const double *p, double (&v)[1]) { v[0] = __ldg(p); }
+    static __device__ __forceinline__ void red(double *p, const double (&v)[1]) { atomicAdd(p, v[0]); }
+};
+template <> struct VecIO<double, 2> {
+    static __device__ __forceinline__ void load(const double *p, double (&v)[2])
+    {
+        const double2 t = __ldg(reinterpret_cast<const double2 *>(p));
+        v[0] = t.x; v[1] = t.y;
+    }
+    static __device__ __forceinline__ void red(double *p, const double (&v)[2])
+    {
+        atomicAdd(p, v[0]); atomicAdd(p + 1, v[1]);
+    }
+};
 
-// ---- literal gather (a1) + sign rounding and count (a7, a8) --------------------------------
-template <typename T>
-__device__ __forceinline__ T gather_literal(const T *__restrict__ x, int64_t ldb, int64_t b, int32_t lit)
+// ---- a2-a4 for one constraint of compile-time length K and V candidates, all in registers --------
+// tab: the signature's rows in shared memory, 8 scalars per row {Re a, Im a, Re b, Im b, Re w, Im w,
+// Re(w b), Im(w b)}, real rows first.
+template <typename T, int K, int V, bool GRAD>
+__device__ __forceinline__ void eval_points_reg(const T (&y)[K][V], const T *__restrict__ tab, int n_real,
+                                                int n_cplx, T (&fe)[V], T (&g)[K][V])
 {
-    T v;
-    if (lit & LIT_FIXED) v = T(1);                                   // warp-uniform branch
-    else v = x[(int64_t)(lit & LIT_VAR) * ldb + b];
-    return (lit < 0) ? -v : v;
-}
-
-// a7: the VARIABLE rounds to True iff x < 0 (x = 0, -0.0 -> False); a negated literal is true iff
-// the variable is False -- so the tie x = 0 makes the literal -x TRUE (y = -0.0 is not "< 0").
-template <typename T>
-__device__ __forceinline__ int literal_true(T y, int32_t lit)
-{
-    return (lit < 0) ? !(y > T(0)) : (y < T(0));      // y = -x for negated literals: x < 0 <=> y > 0
-}
-
-__device__ __forceinline__ int sat_bit(const SigDev &sg, int tau)
-{
-    return (int)(((tau < 64) ? (sg.sat_lo >> tau) : (sg.sat_hi >> (tau - 64))) & 1ull);
-}
-
-// ---- a2-a4 for one constraint of compile-time length K, everything in registers -------------
-template <typename T, int K, bool GRAD, bool STORE_F>
-__device__ __forceinline__ void eval_points_reg(const T (&y)[K], const T *__restrict__ rows,
-                                                int n_real, int n_cplx, T &fe, T (&g)[K])
-{
-    const T *r = rows;
+    const T *r = tab;
     for (int p = 0; p < n_real; ++p, r += 8) {                       // self-conjugate points
         const T a = r[0], b = r[2], w = r[4], wb = r[6];
-        T pre[K];
-        T run = fma_(b, y[0], a);
-        pre[0] = T(1);
 #pragma unroll
-        for (int i = 1; i < K; ++i) { pre[i] = run; run *= fma_(b, y[i], a); }
-        fe = fma_(w, run, fe);
-        if (GRAD) {
-            T suf = wb;
+        for (int v = 0; v < V; ++v) {
+            T pre[K], f[K];
 #pragma unroll
-            for (int i = K - 1; i >= 1; --i) { g[i] = fma_(pre[i], suf, g[i]); suf *= fma_(b, y[i], a); }
-            g[0] += suf;
+            for (int i = 0; i < K; ++i) f[i] = fma_(b, y[i][v], a);
+            T run = f[0];
+#pragma unroll
+            for (int i = 1; i < K; ++i) { pre[i] = run; run *= f[i]; }
+            fe[v] = fma_(w, run, fe[v]);
+            if (GRAD) {
+                T suf = wb;
+#pragma unroll
+                for (int i = K - 1; i >= 1; --i) { g[i][v] = fma_(pre[i], suf, g[i][v]); suf *= f[i]; }
+                g[0][v] += suf;                                       // prefix_0 = 1
+            }
         }
     }
     for (int p = 0; p < n_cplx; ++p, r += 8) {                       // one of each conjugate pair
-        const T ar = r[0], ai = r[1], br = r[2], bi = r[3], wr = r[4], wi = r[5];
-        T pr[K], pi[K], fr[STORE_F ? K : 1], fi[STORE_F ? K : 1];
-        T rr = fma_(br, y[0], ar), ri = fma_(bi, y[0], ai);
-        pr[0] = T(1); pi[0] = T(0);
-        if (STORE_F) { fr[0] = rr; fi[0] = ri; }
+        const T ar = r[0], ai = r[1], br = r[2], bi = r[3], wr = r[4], wi = r[5], wbr = r[6], wbi = r[7];
 #pragma unroll
-        for (int i = 1; i < K; ++i) {
-            const T f_r = fma_(br, y[i], ar), f_i = fma_(bi, y[i], ai);
-            if (STORE_F) { fr[i] = f_r; fi[i] = f_i; }
-            pr[i] = rr; pi[i] = ri;
-            const T nr = fma_(rr, f_r, -(ri * f_i));
-            const T ni = fma_(rr, f_i, ri * f_r);
-            rr = nr; ri = ni;
-        }
-        fe = fma_(wr, rr, fe);
-        fe = fma_(-wi, ri, fe);
-        if (GRAD) {
-            T sr = r[6], si = r[7];                                   // suffix seeded with w b
+        for (int v = 0; v < V; ++v) {
+            T pr[K], pi[K], fr[K], fi[K];
 #pragma unroll
-            for (int i = K - 1; i >= 1; --i) {
-                g[i] = fma_(pr[i], sr, g[i]);
-                g[i] = fma_(-pi[i], si, g[i]);
-                const T f_r = STORE_F ? fr[i] : fma_(br, y[i], ar);
-                const T f_i = STORE_F ? fi[i] : fma_(bi, y[i], ai);
-                const T nr = fma_(sr, f_r, -(si * f_i));
-                const T ni = fma_(sr, f_i, si * f_r);
-                sr = nr; si = ni;
-            }
-            g[0] += sr;                                               // prefix_0 = 1
-        }
-    }
-}
-
-template <typename T, int K, bool GRAD>
-__device__ __forceinline__ void run_item_reg(const EvalParams<T> &p, const Item &it, int64_t b, int item_row)
-{
-    const bool live = b < p.B;
-    T fe_acc = T(0);
-    int sat = 0;
-    const int32_t *L = p.lits + it.lit_base;
-    for (int c = it.c_begin; c < it.c_end; ++c, L += K) {
-        const SigDev sg = p.sigs[p.cons_sig[c]];
-        int32_t lit[K];
-        T y[K], g[K];
-        int tau = 0;
+            for (int i = 0; i < K; ++i) { fr[i] = fma_(br, y[i][v], ar); fi[i] = fma_(bi, y[i][v], ai); }
+            T rr = fr[0], ri = fi[0];
 #pragma unroll
-        for (int i = 0; i < K; ++i) lit[i] = __ldg(L + i);
-#pragma unroll
-        for (int i = 0; i < K; ++i) {
-            y[i] = gather_literal(p.x, p.ldb, b, lit[i]);
-            tau += literal_true(y[i], lit[i]);
-            g[i] = T(0);
-        }
-        sat += sat_bit(sg, tau);
-        eval_points_reg<T, K, GRAD, (K <= 10)>(y, p.rows + (int64_t)sg.row_off * 8, sg.n_real, sg.n_cplx, fe_acc, g);
-        if (GRAD && live) {
-#pragma unroll
-            for (int i = 0; i < K; ++i)
-                if (!(lit[i] & LIT_FIXED))
-                    red_add(p.G + (int64_t)(lit[i] & LIT_VAR) * p.ldb + b, (lit[i] < 0) ? -g[i] : g[i]);
-        }
-    }
-    if (live) {
-        if (p.Fpart) p.Fpart[(int64_t)item_row * p.ldb + b] = fe_acc;
-        if (p.satacc) atomicAdd(p.satacc + b, sat);
-    }
-}
-
-template <typename T, int K, int KHI, bool GRAD>
-struct DispatchK {
-    static __device__ __forceinline__ void go(const EvalParams<T> &p, const Item &it, int64_t b, int row)
-    {
-        if (it.k == K) run_item_reg<T, K, GRAD>(p, it, b, row);
-        else DispatchK<T, K + 1, KHI, GRAD>::go(p, it, b, row);
-    }
-};
-template <typename T, int KHI, bool GRAD>
-struct DispatchK<T, KHI, KHI, GRAD> {
-    static __device__ __forceinline__ void go(const EvalParams<T> &p, const Item &it, int64_t b, int row)
-    {
-        run_item_reg<T, KHI, GRAD>(p, it, b, row);
-    }
-};
-
-// Register kernel for one class of lengths [KLO, KHI]; it.k is CTA-uniform.
-template <typename T, int KLO, int KHI, bool GRAD>
-__global__ void __launch_bounds__(256) k_eval_reg(const EvalParams<T> p)
-{
-    const Item it = p.items[blockIdx.x];
-    const int64_t b = (int64_t)blockIdx.y * blockDim.x + threadIdx.x;
-    if (b >= p.ldb) return;
-    DispatchK<T, KLO, KHI, GRAD>::go(p, it, b, p.item_index_base + blockIdx.x);
-}
-
-// ---- generic kernel for long constraints (runtime k <= 64): prefix products staged in shared
-// memory as [i][lane] columns (conflict-free), suffix running in registers ---------------------
-template <typename T, bool GRAD>
-__global__ void __launch_bounds__(256) k_eval_long(const EvalParams<T> p, int kmax)
-{
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    const Item it = p.items[blockIdx.x];
-    const int64_t b = (int64_t)blockIdx.y * blockDim.x + threadIdx.x;
-    if (b >= p.ldb) return;                                   // whole warps only (ldb % 32 == 0)
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    T *sy = reinterpret_cast<T *>(smem_raw) + (size_t)warp * 4 * kmax * 32 + lane;
-    T *spr = sy + (size_t)kmax * 32, *spi = spr + (size_t)kmax * 32, *sg = spi + (size_t)kmax * 32;
-    const int k = it.k;
-    const bool live = b < p.B;
-    T fe_acc = T(0);
-    int sat = 0;
-    const int32_t *L = p.lits + it.lit_base;
-    for (int c = it.c_begin; c < it.c_end; ++c, L += k) {
-        const SigDev sgd = p.sigs[p.cons_sig[c]];
-        int tau = 0;
-        for (int i = 0; i < k; ++i) {
-            const int32_t lit_i = __ldg(L + i);
-            const T yi = gather_literal(p.x, p.ldb, b, lit_i);
-            tau += literal_true(yi, lit_i);
-            sy[i * 32] = yi;
-            sg[i * 32] = T(0);
-        }
-        sat += sat_bit(sgd, tau);
-        const T *r = p.rows + (int64_t)sgd.row_off * 8;
-        for (int q = 0; q < sgd.n_real; ++q, r += 8) {
-            const T a = r[0], bb = r[2], w = r[4], wb = r[6];
-            T run = T(1);
-            for (int i = 0; i < k; ++i) { spr[i * 32] = run; run *= fma_(bb, sy[i * 32], a); }
-            fe_acc = fma_(w, run, fe_acc);
-            if (GRAD) {
-                T suf = wb;
-                for (int i = k - 1; i >= 0; --i) {
-                    sg[i * 32] = fma_(spr[i * 32], suf, sg[i * 32]);
-                    suf *= fma_(bb, sy[i * 32], a);
-                }
-            }
-        }
-        for (int q = 0; q < sgd.n_cplx; ++q, r += 8) {
-            const T ar = r[0], ai = r[1], br = r[2], bi = r[3], wr = r[4], wi = r[5];
-            T rr = T(1), ri = T(0);
-            for (int i = 0; i < k; ++i) {
-                const T yi = sy[i * 32];
-                const T f_r = fma_(br, yi, ar), f_i = fma_(bi, yi, ai);
-                spr[i * 32] = rr; spi[i * 32] = ri;
-                const T nr = fma_(rr, f_r, -(ri * f_i));
-                const T ni = fma_(rr, f_i, ri * f_r);
+            for (int i = 1; i < K; ++i) {
+                pr[i] = rr; pi[i] = ri;
+                const T nr = fma_(rr, fr[i], -(ri * fi[i]));
+                const T ni = fma_(rr, fi[i], ri * fr[i]);
                 rr = nr; ri = ni;
             }
-            fe_acc = fma_(wr, rr, fe_acc);
-            fe_acc = fma_(-wi, ri, fe_acc);
+            fe[v] = fma_(wr, rr, fe[v]);
+            fe[v] = fma_(-wi, ri, fe[v]);
             if (GRAD) {
-                T sr = r[6], si = r[7];
-                for (int i = k - 1; i >= 0; --i) {
-                    const T yi = sy[i * 32];
-                    T gi = sg[i * 32];
-                    gi = fma_(spr[i * 32], sr, gi);
-                    gi = fma_(-spi[i * 32], si, gi);
-                    sg[i * 32] = gi;
-                    const T f_r = fma_(br, yi, ar), f_i = fma_(bi, yi, ai);
-                    const T nr = fma_(sr, f_r, -(si * f_i));
-                    const T ni = fma_(sr, f_i, si * f_r);
+                T sr = wbr, si = wbi;                                 // suffix seeded with w b
+#pragma unroll
+                for (int i = K - 1; i >= 1; --i) {
+                    g[i][v] = fma_(pr[i], sr, g[i][v]);
+                    g[i][v] = fma_(-pi[i], si, g[i][v]);
+                    const T nr = fma_(sr, fr[i], -(si * fi[i]));
+                    const T ni = fma_(sr, fi[i], si * fr[i]);
                     sr = nr; si = ni;
                 }
+                g[0][v] += sr;                                        // prefix_0 = 1
             }
         }
-        if (GRAD && live) {
-            for (int i = 0; i < k; ++i) {
-                const int32_t lit = __ldg(L + i);
-                if (!(lit & LIT_FIXED)) {
-                    const T gi = sg[i * 32];
-                    red_add(p.G + (int64_t)(lit & LIT_VAR) * p.ldb + b, (lit < 0) ? -gi : gi);
-                }
-            }
-        }
-    }
-    if (live) {
-        if (p.Fpart) p.Fpart[(int64_t)(p.item_index_base + blockIdx.x) * p.ldb + b] = fe_acc;
-        if (p.satacc) atomicAdd(p.satacc + b, sat);
     }
 }
 
-// ---- integer-only check (a7, a8): no floating-point arithmetic beyond the sign test ----------
-template <typename T>
-__global__ void __launch_bounds__(256) k_check(const EvalParams<T> p)
+// One work item for this thread's V candidates; returns the item's partial objective in fe.
+template <typename T, int K, int V, bool GRAD>
+__device__ __forceinline__ void run_item_reg(const EvalParams<T> &p, const int32_t *__restrict__ s_lits,
+                                             const T *__restrict__ s_tab, int n_real, int n_cplx, int nc, int wk,
+                                             int64_t b, T (&fe)[V])
 {
-    const Item it = p.items[blockIdx.x];
-    const int64_t b = (int64_t)blockIdx.y * blockDim.x + threadIdx.x;
-    if (b >= p.B) return;
-    const int k = it.k;
-    int sat = 0;
-    const int32_t *L = p.lits + it.lit_base;
-    for (int c = it.c_begin; c < it.c_end; ++c, L += k) {
-        const SigDev sg = p.sigs[p.cons_sig[c]];
-        int tau = 0;
-        for (int i = 0; i < k; ++i) {
-            const int32_t lit_i = __ldg(L + i);
-            tau += literal_true(gather_literal(p.x, p.ldb, b, lit_i), lit_i);
+    const bool all_live = b + V <= p.B;
+    for (int c = wk; c < nc; c += p.Wk) {
+        const int32_t *L = s_lits + c * K;
+        int32_t lit[K];
+        T y[K][V], g[K][V];
+#pragma unroll
+        for (int i = 0; i < K; ++i) lit[i] = L[i];
+#pragma unroll
+        for (int i = 0; i < K; ++i) {
+            if (lit[i] & LIT_FIXED) {                                 // warp-uniform branch
+#pragma unroll
+                for (int v = 0; v < V; ++v) y[i][v] = T(1);
+            } else {
+                VecIO<T, V>::load(p.x + (int64_t)(lit[i] & LIT_VAR) * p.ldb + b, y[i]);
+            }
+#pragma unroll
+            for (int v = 0; v < V; ++v) { y[i][v] = (lit[i] < 0) ? -y[i][v] : y[i][v]; g[i][v] = T(0); }
         }
-        sat += sat_bit(sg, tau);
+        eval_points_reg<T, K, V, GRAD>(y, s_tab, n_real, n_cplx, fe, g);
+        if (GRAD) {
+#pragma unroll
+            for (int i = 0; i < K; ++i) {
+                if (lit[i] & LIT_FIXED) continue;                     // masked gradient
+                T gi[V];
+#pragma unroll
+                for (int v = 0; v < V; ++v) gi[v] = (lit[i] < 0) ? -g[i][v] : g[i][v];
+                T *dst = p.G + (int64_t)(lit[i] & LIT_VAR) * p.g_ld + (b - p.g_b0);
+                if (all_live) VecIO<T, V>::red(dst, gi);
+                else {
+#pragma unroll
+                    for (int v = 0; v < V; ++v)
+                        if (b + v < p.B) atomicAdd(dst + v, gi[v]);
+                }
+            }
+        }
     }
-    atomicAdd(p.satacc + b, sat);
+}
+
+template <typename T, int K, int KHI, int V, bool GRAD>
+struct DispatchK {
+    static __device__ __forceinline__ void go(const EvalParams<T> &p, int k, const int32_t *s_lits, const T *s_tab,
+                                              int n_real, int n_cplx, int nc, int wk, int64_t b, T (&fe)[V])
+    {
+        if (k == K) run_item_reg<T, K, V, GRAD>(p, s_lits, s_tab, n_real, n_cplx, nc, wk, b, fe);
+        else DispatchK<T, K + 1, KHI, V, GRAD>::go(p, k, s_lits, s_tab, n_real, n_cplx, nc, wk, b, fe);
+    }
+};
+template <typename T, int KHI, int V, bool GRAD>
+struct DispatchK<T, KHI, KHI, V, GRAD> {
+    static __device__ __forceinline__ void go(const EvalParams<T> &p, int k, const int32_t *s_lits, const T *s_tab,
+                                              int n_real, int n_cplx, int nc, int wk, int64_t b, T (&fe)[V])
+    {
+        run_item_reg<T, KHI, V, GRAD>(p, s_lits, s_tab, n_real, n_cplx, nc, wk, b, fe);
+    }
+};
+
+// Stage the item's weight rows and literal list in shared memory (coalesced, once per CTA).
+template <typename T>
+__device__ __forceinline__ void stage_item(const EvalParams<T> &p, const Item &it, const SigDev &sg, T *s_tab,
+                                           int32_t *s_lits)
+{
+    const int nrows8 = (sg.n_real + sg.n_cplx) * 8;
+    for (int i = threadIdx.x; i < nrows8; i += blockDim.x) s_tab[i] = p.rows[(int64_t)sg.row_off * 8 + i];
+    const int nl = (it.c_end - it.c_begin) * it.k;
+    for (int i = threadIdx.x; i < nl; i += blockDim.x) s_lits[i] = __ldg(p.lits + it.lit_base + i);
+}
+
+// Sum the Wk warp groups' partial objectives in a fixed order and write Fpart[item][b].
+template <typename T, int V>
+__device__ __forceinline__ void store_item_F(const EvalParams<T> &p, T (*s_F)[32 * V], const T (&fe)[V], int warp,
+                                             int lane, int wk, int64_t b, bool active)
+{
+    if (!p.Fpart) return;
+#pragma unroll
+    for (int v = 0; v < V; ++v) s_F[warp][lane * V + v] = fe[v];
+    __syncthreads();
+    if (wk == 0 && active) {
+#pragma unroll
+        for (int v = 0; v < V; ++v) {
+            T s = T(0);
+            for (int g = 0; g < p.Wk; ++g) s += s_F[warp + g * p.Wc][lane * V + v];
+            if (b + v < p.B) p.Fpart[(int64_t)(p.frow_base + blockIdx.x) * p.ldb + b + v] = s;
+        }
+    }
+}
+
+// Register kernel for one class of lengths [KLO, KHI]; the item's k and signature are CTA-uniform.
+template <typename T, int KLO, int KHI, int V, bool GRAD, int MINB>
+__global__ void __launch_bounds__(CTA_THREADS, MINB) k_eval_reg(const EvalParams<T> p)
+{
+    __shared__ __align__(16) T s_tab[(KHI / 2 + 1) * 8];
+    __shared__ int32_t s_lits[LIT_CHUNK];
+    __shared__ T s_F[CTA_WARPS][32 * V];
+    const Item it = p.items[blockIdx.x];
+    const SigDev sg = p.sigs[it.sig];
+    stage_item(p, it, sg, s_tab, s_lits);
+    __syncthreads();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int wc = warp % p.Wc, wk = warp / p.Wc;
+    const int64_t b = p.b_begin + ((int64_t)blockIdx.y * p.Wc + wc) * (32 * V) + lane * V;
+    const bool active = b < p.ldb && b < p.B;
+    T fe[V];
+#pragma unroll
+    for (int v = 0; v < V; ++v) fe[v] = T(0);
+    if (active)
+        DispatchK<T, KLO, KHI, V, GRAD>::go(p, it.k, s_lits, s_tab, sg.n_real, sg.n_cplx, it.c_end - it.c_begin, wk, b, fe);
+    store_item_F<T, V>(p, s_F, fe, warp, lane, wk, b, active);
+}
+
+// ---- generic kernel for long constraints (runtime k <= 64), V = 1: literal values, prefix products
+// and partial gradients staged in shared memory as [i][lane] columns (conflict-free), suffix
+// running in registers ------------------------------------------------------------------------------
+template <typename T, bool GRAD>
+__global__ void __launch_bounds__(CTA_THREADS) k_eval_long(const EvalParams<T> p, int kmax)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T *s_tab = reinterpret_cast<T *>(smem_raw);                       // [MAX_ROWS * 8]
+    int32_t *s_lits = reinterpret_cast<int32_t *>(s_tab + MAX_ROWS * 8);   // [LIT_CHUNK]
+    T *s_F = reinterpret_cast<T *>(s_lits + LIT_CHUNK);                // [CTA_WARPS][32]
+    T *s_work = s_F + CTA_WARPS * 32;                                  // [warps][4][kmax][32]
+    const Item it = p.items[blockIdx.x];
+    const SigDev sgd = p.sigs[it.sig];
+    stage_item(p, it, sgd, s_tab, s_lits);
+    __syncthreads();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int wc = warp % p.Wc, wk = warp / p.Wc;
+    const int64_t b = p.b_begin + ((int64_t)blockIdx.y * p.Wc + wc) * 32 + lane;
+    const bool active = b < p.ldb && b < p.B;
+    T fe_acc[1] = {T(0)};
+    if (active) {
+        T *sy = s_work + (size_t)warp * 4 * kmax * 32 + lane;
+        T *spr = sy + (size_t)kmax * 32, *spi = spr + (size_t)kmax * 32, *sg = spi + (size_t)kmax * 32;
+        const int k = it.k, nc = it.c_end - it.c_begin;
+        for (int c = wk; c < nc; c += p.Wk) {
+            const int32_t *L = s_lits + c * k;
+            for (int i = 0; i < k; ++i) {
+                const int32_t lit = L[i];
+                T v = (lit & LIT_FIXED) ? T(1) : __ldg(p.x + (int64_t)(lit & LIT_VAR) * p.ldb + b);
+                sy[i * 32] = (lit < 0) ? -v : v;
+                sg[i * 32] = T(0);
+            }
+            const T *r = s_tab;
+            for (int q = 0; q < sgd.n_real; ++q, r += 8) {
+                const T a = r[0], bb = r[2], w = r[4], wb = r[6];
+                T run = T(1);
+                for (int i = 0; i < k; ++i) { spr[i * 32] = run; run *= fma_(bb, sy[i * 32], a); }
+                fe_acc[0] = fma_(w, run, fe_acc[0]);
+                if (GRAD) {
+                    T suf = wb;
+                    for (int i = k - 1; i >= 0; --i) {
+                        sg[i * 32] = fma_(spr[i * 32], suf, sg[i * 32]);
+                        suf *= fma_(bb, sy[i * 32], a);
+                    }
+                }
+            }
+            for (int q = 0; q < sgd.n_cplx; ++q, r += 8) {
+                const T ar = r[0], ai = r[1], br = r[2], bi = r[3], wr = r[4], wi = r[5];
+                T rr = T(1), ri = T(0);
+                for (int i = 0; i < k; ++i) {
+                    const T yi = sy[i * 32];
+                    const T f_r = fma_(br, yi, ar), f_i = fma_(bi, yi, ai);
+                    spr[i * 32] = rr; spi[i * 32] = ri;
+                    const T nr = fma_(rr, f_r, -(ri * f_i));
+                    const T ni = fma_(rr, f_i, ri * f_r);
+                    rr = nr; ri = ni;
+                }
+                fe_acc[0] = fma_(wr, rr, fe_acc[0]);
+                fe_acc[0] = fma_(-wi, ri, fe_acc[0]);
+                if (GRAD) {
+                    T sr = r[6], si = r[7];
+                    for (int i = k - 1; i >= 0; --i) {
+                        const T yi = sy[i * 32];
+                        T gi = sg[i * 32];
+                        gi = fma_(spr[i * 32], sr, gi);
+                        gi = fma_(-spi[i * 32], si, gi);
+                        sg[i * 32] = gi;
+                        const T f_r = fma_(br, yi, ar), f_i = fma_(bi, yi, ai);
+                        const T nr = fma_(sr, f_r, -(si * f_i));
+                        const T ni = fma_(sr, f_i, si * f_r);
+                        sr = nr; si = ni;
+                    }
+                }
+            }
+            if (GRAD) {
+                for (int i = 0; i < k; ++i) {
+                    const int32_t lit = L[i];
+                    if (!(lit & LIT_FIXED)) {
+                        const T gi = sg[i * 32];
+                        atomicAdd(p.G + (int64_t)(lit & LIT_VAR) * p.g_ld + (b - p.g_b0), (lit < 0) ? -gi : gi);
+                    }
+                }
+            }
+        }
+    }
+    store_item_F<T, 1>(p, reinterpret_cast<T(*)[32]>(s_F), fe_acc, warp, lane, wk, b, active);
+}
+
+// ---- a7: sign rounding as one bit per (variable, candidate): bits[v][b / 32] bit (b % 32) = (x < 0)
+template <typename T>
+__global__ void __launch_bounds__(CTA_THREADS) k_pack_signs(const T *__restrict__ x, uint32_t *__restrict__ bits, int n,
+                                                           int B, int64_t ldb)
+{
+    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= ldb) return;                                             // whole warps (ldb % 32 == 0)
+    const int64_t ldw = ldb >> 5;
+    for (int v = blockIdx.y; v < n; v += gridDim.y) {
+        const bool t = (b < B) && (x[(int64_t)v * ldb + b] < T(0));   // True iff x < 0 (0, -0.0 -> False)
+        const uint32_t w = __ballot_sync(0xffffffffu, t);
+        if ((threadIdx.x & 31) == 0) bits[(int64_t)v * ldw + (b >> 5)] = w;
+    }
+}
+
+// ---- a6 + a7 + a9: projected step on the candidate tile [b_begin, b_end), gradient scratch reset,
+// sign bits of the NEW x.  Frozen (solved) candidates and fixed variables keep their x.
+template <typename T>
+__global__ void __launch_bounds__(CTA_THREADS) k_update(T *__restrict__ x, T *__restrict__ G, int64_t g_ld, int64_t g_b0,
+                                                       const int8_t *__restrict__ fixed,
+                                                       const uint8_t *__restrict__ is_solution, uint32_t *__restrict__ bits,
+                                                       T eta, int n, int B, int64_t ldb, int64_t b_begin, int64_t b_end)
+{
+    const int64_t b = b_begin + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= b_end) return;                                           // tiles are multiples of 32
+    const bool live = b < B;
+    const bool upd = live && !is_solution[b];
+    const int64_t ldw = ldb >> 5;
+    for (int v = blockIdx.y; v < n; v += gridDim.y) {
+        const int64_t idx = (int64_t)v * ldb + b, gidx = (int64_t)v * g_ld + (b - g_b0);
+        const T g = G[gidx];
+        G[gidx] = T(0);
+        T xv = x[idx];
+        if (upd && !fixed[v]) {
+            xv = fma_(-eta, g, xv);
+            xv = xv > T(1) ? T(1) : xv;
+            xv = xv < T(-1) ? T(-1) : xv;
+            x[idx] = xv;
+        }
+        const uint32_t w = __ballot_sync(0xffffffffu, live && (xv < T(0)));
+        if ((threadIdx.x & 31) == 0) bits[(int64_t)v * ldw + (b >> 5)] = w;
+    }
+}
+
+// ---- a8: exact discrete count, integer only.  One thread = one 32-candidate word; the number tau
+// of true literals is kept BIT-SLICED (t[j] holds bit j of tau for 32 candidates), the predicate is
+// evaluated by scanning the smaller of {satisfied counts, violated counts}, and the per-candidate
+// number of satisfied constraints of the item is again a bit-sliced counter.
+struct CheckParams {
+    const uint32_t *bits;       // [n][ldw]
+    int64_t ldw;
+    const int32_t *lits;
+    const SigDev *sigs;
+    const Item *items;
+    int32_t *satacc;            // [ldb]
+    int32_t B;
+    int32_t w_begin, w_end;     // word range of this launch
+    int32_t wpb;                // words per CTA (power of two <= 32)
+};
+
+__global__ void __launch_bounds__(CTA_THREADS) k_check_bits(const CheckParams p)
+{
+    __shared__ int32_t s_lits[LIT_CHUNK];
+    __shared__ int32_t s_cnt[32 * 32];
+    const Item it = p.items[blockIdx.x];
+    const SigDev sg = p.sigs[it.sig];
+    const int k = it.k, nc = it.c_end - it.c_begin;
+    for (int i = threadIdx.x; i < nc * k; i += blockDim.x) s_lits[i] = __ldg(p.lits + it.lit_base + i);
+    for (int i = threadIdx.x; i < p.wpb * 32; i += blockDim.x) s_cnt[i] = 0;
+    __syncthreads();
+    const int wi = threadIdx.x % p.wpb, grp = threadIdx.x / p.wpb, ngrp = blockDim.x / p.wpb;
+    const int word = p.w_begin + blockIdx.y * p.wpb + wi;
+    const bool valid = word < p.w_end;
+    int nb = 1;
+    while ((1 << nb) <= k) ++nb;                                      // bits of tau in [0, k]
+    uint32_t cnt[13];
+#pragma unroll
+    for (int j = 0; j < 13; ++j) cnt[j] = 0u;
+    if (valid) {
+        for (int c = grp; c < nc; c += ngrp) {
+            uint32_t t[7] = {0u, 0u, 0u, 0u, 0u, 0u, 0u};
+            const int32_t *L = s_lits + c * k;
+            for (int i = 0; i < k; ++i) {
+                const int32_t lit = L[i];
+                uint32_t m = (lit & LIT_FIXED) ? 0u : __ldg(p.bits + (int64_t)(lit & LIT_VAR) * p.ldw + word);
+                if (lit < 0) m = ~m;                                  // literal true = variable true XOR negated
+#pragma unroll
+                for (int j = 0; j < 7; ++j)
+                    if (j < nb) { const uint32_t s = t[j] ^ m; m &= t[j]; t[j] = s; }
+            }
+            uint32_t acc = 0u;
+            for (int tau = 0; tau <= k; ++tau) {
+                const uint64_t bit = tau < 64 ? (sg.scan_lo >> tau) : (sg.scan_hi >> (tau - 64));
+                if (!(bit & 1ull)) continue;
+                uint32_t eq = 0xffffffffu;
+#pragma unroll
+                for (int j = 0; j < 7; ++j)
+                    if (j < nb) eq &= ((tau >> j) & 1) ? t[j] : ~t[j];
+                acc |= eq;
+            }
+            uint32_t carry = sg.scan_is_sat ? acc : ~acc;             // 1 = constraint satisfied
+#pragma unroll
+            for (int j = 0; j < 13; ++j) { const uint32_t s = cnt[j] ^ carry; carry &= cnt[j]; cnt[j] = s; }
+        }
+        for (int bit = 0; bit < 32; ++bit) {
+            int val = 0;
+#pragma unroll
+            for (int j = 0; j < 13; ++j) val |= (int)((cnt[j] >> bit) & 1u) << j;
+            if (val) atomicAdd(&s_cnt[wi * 32 + bit], val);
+        }
+    }
+    __syncthreads();
+    const int64_t b0 = ((int64_t)p.w_begin + (int64_t)blockIdx.y * p.wpb) * 32;
+    for (int i = threadIdx.x; i < p.wpb * 32; i += blockDim.x) {
+        const int64_t b = b0 + i;
+        if (b < p.B && b < (int64_t)p.w_end * 32 && s_cnt[i]) atomicAdd(p.satacc + b, s_cnt[i]);
+    }
 }
 
 // ---- F[b] = sum over items of Fpart[item][b], fixed order, accumulated in double ------------
 template <typename T>
-__global__ void k_reduce_F(const T *__restrict__ Fpart, int n_items, int64_t ldb, int B, T *__restrict__ F)
+__global__ void k_reduce_F(const T *__restrict__ Fpart, int n_rows, int64_t ldb, int B, T *__restrict__ F)
 {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= B) return;
     double s = 0.0;
-    for (int i = 0; i < n_items; ++i) s += (double)Fpart[(int64_t)i * ldb + b];
+    for (int i = 0; i < n_rows; ++i) s += (double)Fpart[(int64_t)i * ldb + b];
     F[b] = (T)s;
 }
 
-// ---- per-candidate state machine of Alg. 1 (a8, a9) -----------------------------------------
-// mode 0 (inside the loop, step t >= 2): satacc holds the count on X(t-1); newly solved candidates
-//        get first_step = step_base + t - 1 and freeze.  mode 1 (tail): count on the final X(T).
-__global__ void k_flags(int32_t *__restrict__ satacc, int B, int m, int mode, int step_value, int n_steps,
+// ---- per-candidate state machine of Alg. 1 (a8, a9): satacc holds the count on the current X ----
+__global__ void k_flags(int32_t *__restrict__ satacc, int B, int m, int mark_solved, int step_value,
                         int32_t *__restrict__ sat_count, uint8_t *__restrict__ is_solution,
                         int32_t *__restrict__ first_step, int32_t *__restrict__ d_any, volatile int32_t *h_any)
 {
@@ -325,8 +514,8 @@ __global__ void k_flags(int32_t *__restrict__ satacc, int B, int m, int mode, in
     if (b >= B) return;
     const int s = satacc[b];
     satacc[b] = 0;
-    if (mode == 1) sat_count[b] = s;
-    if ((mode == 0 || n_steps >= 1) && s == m && !is_solution[b]) {
+    sat_count[b] = s;
+    if (mark_solved && s == m && !is_solution[b]) {
         is_solution[b] = 1;
         first_step[b] = step_value;
         if (atomicCAS(d_any, 0, 1) == 0) {
@@ -352,27 +541,6 @@ __global__ void k_reset_state(int B, uint8_t *is_solution, int32_t *first_step)
 {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b < B) { is_solution[b] = 0; first_step[b] = -1; }
-}
-
-// ---- projected step (a6) + freeze (a9) + gradient reset, elementwise over [n][ldb] ----------
-template <typename T>
-__global__ void __launch_bounds__(256) k_update(T *__restrict__ x, T *__restrict__ G, const int8_t *__restrict__ fixed,
-                                               const uint8_t *__restrict__ is_solution, T eta, int n, int B, int64_t ldb)
-{
-    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= ldb) return;
-    const bool upd = (b < B) && !is_solution[b];
-    for (int v = blockIdx.y; v < n; v += gridDim.y) {
-        const int64_t idx = (int64_t)v * ldb + b;
-        const T g = G[idx];
-        G[idx] = T(0);
-        if (upd && !fixed[v]) {
-            T nx = fma_(-eta, g, x[idx]);
-            nx = nx > T(1) ? T(1) : nx;
-            nx = nx < T(-1) ? T(-1) : nx;
-            x[idx] = nx;
-        }
-    }
 }
 
 }  // namespace afsat
