@@ -160,8 +160,9 @@ int launch_eval(afsat_ctx *ctx, const T *x, T *G, int64_t g_ld, int64_t g_b0, T 
         const int64_t per_cta = (int64_t)32 * g.V * g.Wc;
         dim3 block(32 * g.warps), grid(nit, (unsigned)((width + per_cta - 1) / per_cta));
         if (cls == CLS_A) {
-            if (grad) k_eval_reg<T, 1, 8, VA, true, 2><<<grid, block, 0, st>>>(p);
-            else      k_eval_reg<T, 1, 8, VA, false, 2><<<grid, block, 0, st>>>(p);
+            constexpr int MB = sizeof(T) == 4 ? 2 : 1;
+            if (grad) k_eval_reg<T, 1, 8, VA, true, MB><<<grid, block, 0, st>>>(p);
+            else      k_eval_reg<T, 1, 8, VA, false, MB><<<grid, block, 0, st>>>(p);
         } else if (cls == CLS_B) {
             if (grad) k_eval_reg<T, 9, 16, 1, true, 1><<<grid, block, 0, st>>>(p);
             else      k_eval_reg<T, 9, 16, 1, false, 1><<<grid, block, 0, st>>>(p);
@@ -226,6 +227,11 @@ int eval_grad_t(afsat_ctx *ctx, const T *x, T *F, T *G, cudaStream_t st)
         const int64_t w = std::min<int64_t>(ctx->tile_w, ctx->ldb - b0);
         int rc = launch_eval<T>(ctx, x, G, ctx->ldb, 0, F ? (T *)ctx->d_Fpart : nullptr, b0, w, st);
         if (rc) return rc;
+    }
+    if (G && ctx->B < ctx->ldb && (ctx->B & 1)) {                     // a lane pair straddles B: clear the spill
+        k_zero_pad<T><<<std::min(1024, ctx->n), 128, 0, st>>>(G, ctx->n, ctx->B, ctx->ldb);
+        ++ctx->launches;
+        CU(cudaPeekAtLastError());
     }
     if (F) return reduce_F<T>(ctx, F, st);
     return AFSAT_OK;
@@ -487,6 +493,8 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
                 Item it;
                 it.k = k; it.sig = sg; it.c_begin = s; it.c_end = (int32_t)std::min<int64_t>(e, s + chunk);
                 it.lit_base = lit_off[s];
+                it.has_fixed = 0; it.pad = 0;
+                for (int64_t q = lit_off[s]; q < lit_off[it.c_end]; ++q) if (lits[q] & LIT_FIXED) { it.has_fixed = 1; break; }
                 items.push_back(it);
             }
             j = e;

@@ -43,6 +43,7 @@ struct Item {                   // one CTA-sized chunk of constraints of a singl
     int32_t k, sig;
     int32_t c_begin, c_end;     // constraint range in bucket order
     int64_t lit_base;           // offset of c_begin's first packed literal
+    int32_t has_fixed, pad;     // some literal of the chunk is a fixed variable
 };
 
 template <typename T>
@@ -172,14 +173,30 @@ __device__ __forceinline__ void eval_points_reg(const T (&y)[K][V], const T *__r
     }
 }
 
+// sign flip by the literal's polarity bit (bit 31 of the packed literal): one LOP3 per value
+__device__ __forceinline__ float flip_sign(float v, int32_t lit)
+{
+    return __int_as_float(__float_as_int(v) ^ (lit & LIT_NEG));
+}
+__device__ __forceinline__ double flip_sign(double v, int32_t lit)
+{
+    return __hiloint2double(__double2hiint(v) ^ (lit & LIT_NEG), __double2loint(v));
+}
+
 // One work item for this thread's V candidates; returns the item's partial objective in fe.
-template <typename T, int K, int V, bool GRAD>
+// FIXED = the item contains fixed literals (constant y = +-1, no gather, no gradient).
+// Padding candidates (b >= B inside a live lane pair) are computed and scattered like live ones:
+// G's padding columns are scratch here and are reset by the caller.
+template <typename T, int K, int V, bool GRAD, bool FIXED>
 __device__ __forceinline__ void run_item_reg(const EvalParams<T> &p, const int32_t *__restrict__ s_lits,
                                              const T *__restrict__ s_tab, int n_real, int n_cplx, int nc, int wk,
                                              int64_t b, T (&fe)[V])
 {
-    const bool all_live = b + V <= p.B;
-    for (int c = wk; c < nc; c += p.Wk) {
+    const char *xb = reinterpret_cast<const char *>(p.x + b);
+    char *gb = reinterpret_cast<char *>(p.G + (b - p.g_b0));
+    const uint32_t x_ld = (uint32_t)(p.ldb * (int64_t)sizeof(T)), g_ld = (uint32_t)(p.g_ld * (int64_t)sizeof(T));
+    const int Wk = p.Wk;
+    for (int c = wk; c < nc; c += Wk) {
         const int32_t *L = s_lits + c * K;
         int32_t lit[K];
         T y[K][V], g[K][V];
@@ -187,30 +204,24 @@ __device__ __forceinline__ void run_item_reg(const EvalParams<T> &p, const int32
         for (int i = 0; i < K; ++i) lit[i] = L[i];
 #pragma unroll
         for (int i = 0; i < K; ++i) {
-            if (lit[i] & LIT_FIXED) {                                 // warp-uniform branch
+            if (FIXED && (lit[i] & LIT_FIXED)) {                      // warp-uniform branch
 #pragma unroll
                 for (int v = 0; v < V; ++v) y[i][v] = T(1);
             } else {
-                VecIO<T, V>::load(p.x + (int64_t)(lit[i] & LIT_VAR) * p.ldb + b, y[i]);
+                VecIO<T, V>::load(reinterpret_cast<const T *>(xb + (uint64_t)(uint32_t)(lit[i] & LIT_VAR) * x_ld), y[i]);
             }
 #pragma unroll
-            for (int v = 0; v < V; ++v) { y[i][v] = (lit[i] < 0) ? -y[i][v] : y[i][v]; g[i][v] = T(0); }
+            for (int v = 0; v < V; ++v) { y[i][v] = flip_sign(y[i][v], lit[i]); g[i][v] = T(0); }
         }
         eval_points_reg<T, K, V, GRAD>(y, s_tab, n_real, n_cplx, fe, g);
         if (GRAD) {
 #pragma unroll
             for (int i = 0; i < K; ++i) {
-                if (lit[i] & LIT_FIXED) continue;                     // masked gradient
+                if (FIXED && (lit[i] & LIT_FIXED)) continue;          // masked gradient
                 T gi[V];
 #pragma unroll
-                for (int v = 0; v < V; ++v) gi[v] = (lit[i] < 0) ? -g[i][v] : g[i][v];
-                T *dst = p.G + (int64_t)(lit[i] & LIT_VAR) * p.g_ld + (b - p.g_b0);
-                if (all_live) VecIO<T, V>::red(dst, gi);
-                else {
-#pragma unroll
-                    for (int v = 0; v < V; ++v)
-                        if (b + v < p.B) atomicAdd(dst + v, gi[v]);
-                }
+                for (int v = 0; v < V; ++v) gi[v] = flip_sign(g[i][v], lit[i]);
+                VecIO<T, V>::red(reinterpret_cast<T *>(gb + (uint64_t)(uint32_t)(lit[i] & LIT_VAR) * g_ld), gi);
             }
         }
     }
@@ -218,19 +229,15 @@ __device__ __forceinline__ void run_item_reg(const EvalParams<T> &p, const int32
 
 template <typename T, int K, int KHI, int V, bool GRAD>
 struct DispatchK {
-    static __device__ __forceinline__ void go(const EvalParams<T> &p, int k, const int32_t *s_lits, const T *s_tab,
-                                              int n_real, int n_cplx, int nc, int wk, int64_t b, T (&fe)[V])
+    static __device__ __forceinline__ void go(const EvalParams<T> &p, int k, bool has_fixed, const int32_t *s_lits,
+                                              const T *s_tab, int n_real, int n_cplx, int nc, int wk, int64_t b, T (&fe)[V])
     {
-        if (k == K) run_item_reg<T, K, V, GRAD>(p, s_lits, s_tab, n_real, n_cplx, nc, wk, b, fe);
-        else DispatchK<T, K + 1, KHI, V, GRAD>::go(p, k, s_lits, s_tab, n_real, n_cplx, nc, wk, b, fe);
-    }
-};
-template <typename T, int KHI, int V, bool GRAD>
-struct DispatchK<T, KHI, KHI, V, GRAD> {
-    static __device__ __forceinline__ void go(const EvalParams<T> &p, int k, const int32_t *s_lits, const T *s_tab,
-                                              int n_real, int n_cplx, int nc, int wk, int64_t b, T (&fe)[V])
-    {
-        run_item_reg<T, KHI, V, GRAD>(p, s_lits, s_tab, n_real, n_cplx, nc, wk, b, fe);
+        if (k == K) {
+            if (has_fixed) run_item_reg<T, K, V, GRAD, true>(p, s_lits, s_tab, n_real, n_cplx, nc, wk, b, fe);
+            else run_item_reg<T, K, V, GRAD, false>(p, s_lits, s_tab, n_real, n_cplx, nc, wk, b, fe);
+        } else if (K < KHI) {
+            DispatchK<T, (K < KHI ? K + 1 : K), KHI, V, GRAD>::go(p, k, has_fixed, s_lits, s_tab, n_real, n_cplx, nc, wk, b, fe);
+        }
     }
 };
 
@@ -283,7 +290,8 @@ __global__ void __launch_bounds__(CTA_THREADS, MINB) k_eval_reg(const EvalParams
 #pragma unroll
     for (int v = 0; v < V; ++v) fe[v] = T(0);
     if (active)
-        DispatchK<T, KLO, KHI, V, GRAD>::go(p, it.k, s_lits, s_tab, sg.n_real, sg.n_cplx, it.c_end - it.c_begin, wk, b, fe);
+        DispatchK<T, KLO, KHI, V, GRAD>::go(p, it.k, it.has_fixed != 0, s_lits, s_tab, sg.n_real, sg.n_cplx,
+                                            it.c_end - it.c_begin, wk, b, fe);
     store_item_F<T, V>(p, s_F, fe, warp, lane, wk, b, active);
 }
 
@@ -492,6 +500,16 @@ __global__ void __launch_bounds__(CTA_THREADS) k_check_bits(const CheckParams p)
         const int64_t b = b0 + i;
         if (b < p.B && b < (int64_t)p.w_end * 32 && s_cnt[i]) atomicAdd(p.satacc + b, s_cnt[i]);
     }
+}
+
+// zero the padding columns [B, ldb) of a caller-owned gradient (vector REDs of a lane pair that
+// straddles B spill into them)
+template <typename T>
+__global__ void k_zero_pad(T *__restrict__ G, int n, int B, int64_t ldb)
+{
+    const int64_t np = ldb - B;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < (int64_t)n * np; i += (int64_t)gridDim.x * blockDim.x)
+        G[(i / np) * ldb + B + (i % np)] = T(0);
 }
 
 // ---- F[b] = sum over items of Fpart[item][b], fixed order, accumulated in double ------------
