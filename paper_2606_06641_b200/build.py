@@ -46,7 +46,7 @@ def build(force: bool = False, verbose: bool = False) -> Path:
         objs.append(obj)
     for src in SOURCES_CU:
         obj = objdir / (src.stem + ".o")
-        cmd = [NVCC, *NVCC_FLAGS, "-c", str(src), "-o", str(obj)]
+        cmd = [NVCC, *NVCC_FLAGS, *os.environ.get("AFSAT_NVCC_FLAGS", "").split(), "-c", str(src), "-o", str(obj)]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
             print(" ".join(cmd), flush=True)

@@ -18,6 +18,15 @@
 
 using namespace afsat;
 
+// tuning knobs of the k <= 8 fp32 register kernel: candidates per lane and
+// the occupancy the register allocator is held to
+#ifndef AFSAT_A_V
+#define AFSAT_A_V 2
+#endif
+#ifndef AFSAT_A_MINB
+#define AFSAT_A_MINB 2
+#endif
+
 namespace {
 
 thread_local std::string g_create_error;
@@ -148,7 +157,7 @@ int launch_eval(afsat_ctx *ctx, const T *x, T *G, int64_t g_ld, int64_t g_b0, T 
     p.lits = ctx->d_lits; p.sigs = ctx->d_sigs; p.rows = (const T *)ctx->d_rows;
     p.B = ctx->B; p.ldb = ctx->ldb; p.b_begin = b_begin;
     const bool grad = G != nullptr;
-    constexpr int VA = sizeof(T) == 4 ? 2 : 1;
+    constexpr int VA = sizeof(T) == 4 ? AFSAT_A_V : 1;
     for (int cls = 0; cls < N_CLS; ++cls) {
         const int nit = ctx->cls_begin[cls + 1] - ctx->cls_begin[cls];
         if (nit == 0) continue;
@@ -160,7 +169,7 @@ int launch_eval(afsat_ctx *ctx, const T *x, T *G, int64_t g_ld, int64_t g_b0, T 
         const int64_t per_cta = (int64_t)32 * g.V * g.Wc;
         dim3 block(32 * g.warps), grid(nit, (unsigned)((width + per_cta - 1) / per_cta));
         if (cls == CLS_A) {
-            constexpr int MB = sizeof(T) == 4 ? 2 : 1;
+            constexpr int MB = sizeof(T) == 4 ? AFSAT_A_MINB : 1;
             if (grad) k_eval_reg<T, 1, 8, VA, true, MB><<<grid, block, 0, st>>>(p);
             else      k_eval_reg<T, 1, 8, VA, false, MB><<<grid, block, 0, st>>>(p);
         } else if (cls == CLS_B) {
@@ -452,7 +461,7 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
     for (int32_t j = 0; j < n_cons; ++j) { const int k = sig_k[cons_sig[j]]; if (class_of(k) == CLS_LONG) kmax_long = std::max(kmax_long, k); }
     for (int cls = 0; cls < N_CLS; ++cls) {
         ClassGeom &g = geom[cls];
-        g.V = (cls == CLS_A && dtype == 32) ? 2 : 1;
+        g.V = (cls == CLS_A && dtype == 32) ? AFSAT_A_V : 1;
         g.warps = CTA_WARPS;
         if (cls == CLS_LONG) {
             const size_t fixed_b = (size_t)MAX_ROWS * 8 * esz + (size_t)LIT_CHUNK * 4 + (size_t)CTA_WARPS * 32 * esz;

@@ -27,7 +27,10 @@ constexpr int32_t LIT_FIXED = 0x40000000;            // y is the constant +-1, n
 constexpr int32_t LIT_VAR   = 0x3FFFFFFF;
 
 constexpr int LIT_CHUNK = 4096;       // packed literals staged in shared memory per work item
-constexpr int CTA_THREADS = 256;
+#ifndef AFSAT_CTA_THREADS
+#define AFSAT_CTA_THREADS 256
+#endif
+constexpr int CTA_THREADS = AFSAT_CTA_THREADS;
 constexpr int CTA_WARPS = CTA_THREADS / 32;
 constexpr int MAX_ROWS = 33;          // retained DFT points per signature: H <= 64/2 + 1
 
