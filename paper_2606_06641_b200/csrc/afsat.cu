@@ -201,7 +201,9 @@ int launch_check_bits(afsat_ctx *ctx, int64_t w_begin, int64_t w_end, cudaStream
     p.wpb = std::min(32, pow2_floor(nw));
     if (p.wpb < nw && p.wpb < 32) p.wpb *= 2;                         // cover a ragged word count in one CTA row
     p.wpb = std::min(p.wpb, 32);
-    dim3 grid(ctx->n_items, (unsigned)((nw + p.wpb - 1) / p.wpb));
+    p.n_items = ctx->n_items;
+    const unsigned gy = (unsigned)((nw + p.wpb - 1) / p.wpb);
+    dim3 grid((unsigned)std::max<int64_t>(1, std::min<int64_t>(ctx->n_items, (int64_t)ctx->sm_count * 4 / gy)), gy);
     k_check_bits<<<grid, CTA_THREADS, 0, st>>>(p);
     ++ctx->launches;
     CU(cudaPeekAtLastError());
@@ -264,10 +266,14 @@ int step_t(afsat_ctx *ctx, T *x, double eta, int n_steps, int step_base, int res
             int rc = launch_eval<T>(ctx, x, (T *)ctx->d_G, tw, b0, nullptr, b0, w, st);
             if (rc) return rc;
             // a6, a7, a9: X(t) = clamp(X(t-1) - eta G) on free variables of unsolved candidates, sign bits, G reset
-            const unsigned gx = (unsigned)((w + CTA_THREADS - 1) / CTA_THREADS);
-            const unsigned gy = (unsigned)std::min<int64_t>(ctx->n, std::max<int64_t>(1, (int64_t)ctx->sm_count * 8 / gx));
+            const int cols = (int)std::min<int64_t>(CTA_THREADS, w);                 // w is a multiple of 32
+            const int ucols = CTA_THREADS % cols == 0 ? cols : 32;
+            const unsigned gx = (unsigned)((w + ucols - 1) / ucols);
+            const int rpp = CTA_THREADS / ucols;
+            const unsigned gy = (unsigned)std::max<int64_t>(1, std::min<int64_t>((ctx->n + rpp * UPD_UNROLL - 1) / (rpp * UPD_UNROLL),
+                                                                                   (int64_t)ctx->sm_count * 8 / gx));
             k_update<T><<<dim3(gx, gy), CTA_THREADS, 0, st>>>(x, (T *)ctx->d_G, tw, b0, ctx->d_fixed, sol, ctx->d_bits, (T)eta,
-                                                              ctx->n, B, ctx->ldb, b0, b0 + w);
+                                                              ctx->n, B, ctx->ldb, b0, b0 + w, ucols);
             ++ctx->launches;
             CU(cudaPeekAtLastError());
             // a8: exact count on X(t)

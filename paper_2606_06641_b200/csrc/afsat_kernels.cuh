@@ -403,30 +403,51 @@ __global__ void __launch_bounds__(CTA_THREADS) k_pack_signs(const T *__restrict_
 
 // ---- a6 + a7 + a9: projected step on the candidate tile [b_begin, b_end), gradient scratch reset,
 // sign bits of the NEW x.  Frozen (solved) candidates and fixed variables keep their x.
+// Thread layout: cols = min(tile width, CTA_THREADS) adjacent candidates x (CTA_THREADS / cols)
+// variables per CTA pass, UPD_UNROLL independent rows in flight per thread.
+constexpr int UPD_UNROLL = 4;
 template <typename T>
 __global__ void __launch_bounds__(CTA_THREADS) k_update(T *__restrict__ x, T *__restrict__ G, int64_t g_ld, int64_t g_b0,
                                                        const int8_t *__restrict__ fixed,
                                                        const uint8_t *__restrict__ is_solution, uint32_t *__restrict__ bits,
-                                                       T eta, int n, int B, int64_t ldb, int64_t b_begin, int64_t b_end)
+                                                       T eta, int n, int B, int64_t ldb, int64_t b_begin, int64_t b_end,
+                                                       int cols)
 {
-    const int64_t b = b_begin + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= b_end) return;                                           // tiles are multiples of 32
+    const int col = threadIdx.x % cols, r = threadIdx.x / cols, rows_per_pass = blockDim.x / cols;
+    const int64_t b = b_begin + (int64_t)blockIdx.x * cols + col;
+    if (b >= b_end) return;                                           // tiles and cols are multiples of 32
     const bool live = b < B;
     const bool upd = live && !is_solution[b];
     const int64_t ldw = ldb >> 5;
-    for (int v = blockIdx.y; v < n; v += gridDim.y) {
-        const int64_t idx = (int64_t)v * ldb + b, gidx = (int64_t)v * g_ld + (b - g_b0);
-        const T g = G[gidx];
-        G[gidx] = T(0);
-        T xv = x[idx];
-        if (upd && !fixed[v]) {
-            xv = fma_(-eta, g, xv);
-            xv = xv > T(1) ? T(1) : xv;
-            xv = xv < T(-1) ? T(-1) : xv;
-            x[idx] = xv;
+    const int stride = gridDim.y * rows_per_pass;
+    for (int v0 = blockIdx.y * rows_per_pass + r; v0 < n; v0 += stride * UPD_UNROLL) {
+        T g[UPD_UNROLL], xv[UPD_UNROLL];
+        int8_t fx[UPD_UNROLL];
+#pragma unroll
+        for (int u = 0; u < UPD_UNROLL; ++u) {
+            const int v = v0 + u * stride;
+            if (v < n) {
+                g[u] = G[(int64_t)v * g_ld + (b - g_b0)];
+                xv[u] = x[(int64_t)v * ldb + b];
+                fx[u] = fixed[v];
+            }
         }
-        const uint32_t w = __ballot_sync(0xffffffffu, live && (xv < T(0)));
-        if ((threadIdx.x & 31) == 0) bits[(int64_t)v * ldw + (b >> 5)] = w;
+#pragma unroll
+        for (int u = 0; u < UPD_UNROLL; ++u) {
+            const int v = v0 + u * stride;
+            if (v < n) {                                              // warp-uniform (v depends on the warp's row only)
+                G[(int64_t)v * g_ld + (b - g_b0)] = T(0);
+                T nx = xv[u];
+                if (upd && !fx[u]) {
+                    nx = fma_(-eta, g[u], nx);
+                    nx = nx > T(1) ? T(1) : nx;
+                    nx = nx < T(-1) ? T(-1) : nx;
+                    x[(int64_t)v * ldb + b] = nx;
+                }
+                const uint32_t w = __ballot_sync(0xffffffffu, live && (nx < T(0)));
+                if ((threadIdx.x & 31) == 0) bits[(int64_t)v * ldw + (b >> 5)] = w;
+            }
+        }
     }
 }
 
@@ -444,27 +465,45 @@ struct CheckParams {
     int32_t B;
     int32_t w_begin, w_end;     // word range of this launch
     int32_t wpb;                // words per CTA (power of two <= 32)
+    int32_t n_items;
 };
 
 __global__ void __launch_bounds__(CTA_THREADS) k_check_bits(const CheckParams p)
 {
     __shared__ int32_t s_lits[LIT_CHUNK];
     __shared__ int32_t s_cnt[32 * 32];
-    const Item it = p.items[blockIdx.x];
-    const SigDev sg = p.sigs[it.sig];
-    const int k = it.k, nc = it.c_end - it.c_begin;
-    for (int i = threadIdx.x; i < nc * k; i += blockDim.x) s_lits[i] = __ldg(p.lits + it.lit_base + i);
     for (int i = threadIdx.x; i < p.wpb * 32; i += blockDim.x) s_cnt[i] = 0;
-    __syncthreads();
     const int wi = threadIdx.x % p.wpb, grp = threadIdx.x / p.wpb, ngrp = blockDim.x / p.wpb;
     const int word = p.w_begin + blockIdx.y * p.wpb + wi;
     const bool valid = word < p.w_end;
-    int nb = 1;
-    while ((1 << nb) <= k) ++nb;                                      // bits of tau in [0, k]
     uint32_t cnt[13];
 #pragma unroll
     for (int j = 0; j < 13; ++j) cnt[j] = 0u;
-    if (valid) {
+    int nacc = 0;                                                     // constraints counted in cnt[] so far
+    auto flush = [&]() {                                              // bit-sliced counter -> per-candidate integers
+        for (int bit = 0; bit < 32; ++bit) {
+            int val = 0;
+#pragma unroll
+            for (int j = 0; j < 13; ++j) val |= (int)((cnt[j] >> bit) & 1u) << j;
+            if (val) atomicAdd(&s_cnt[wi * 32 + bit], val);
+        }
+#pragma unroll
+        for (int j = 0; j < 13; ++j) cnt[j] = 0u;
+        nacc = 0;
+    };
+    for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {   // persistent over work items
+        const Item it = p.items[item];
+        const SigDev sg = p.sigs[it.sig];
+        const int k = it.k, nc = it.c_end - it.c_begin;
+        __syncthreads();                                              // previous item's literals are consumed
+        for (int i = threadIdx.x; i < nc * k; i += blockDim.x) s_lits[i] = __ldg(p.lits + it.lit_base + i);
+        __syncthreads();
+        if (!valid) continue;
+        int nb = 1;
+        while ((1 << nb) <= k) ++nb;                                  // bits of tau in [0, k]
+        const int mine = (nc - grp + ngrp - 1) / ngrp;
+        if (nacc + mine > 8191) flush();
+        nacc += mine > 0 ? mine : 0;
         for (int c = grp; c < nc; c += ngrp) {
             uint32_t t[7] = {0u, 0u, 0u, 0u, 0u, 0u, 0u};
             const int32_t *L = s_lits + c * k;
@@ -490,13 +529,8 @@ __global__ void __launch_bounds__(CTA_THREADS) k_check_bits(const CheckParams p)
 #pragma unroll
             for (int j = 0; j < 13; ++j) { const uint32_t s = cnt[j] ^ carry; carry &= cnt[j]; cnt[j] = s; }
         }
-        for (int bit = 0; bit < 32; ++bit) {
-            int val = 0;
-#pragma unroll
-            for (int j = 0; j < 13; ++j) val |= (int)((cnt[j] >> bit) & 1u) << j;
-            if (val) atomicAdd(&s_cnt[wi * 32 + bit], val);
-        }
     }
+    if (valid && nacc) flush();
     __syncthreads();
     const int64_t b0 = ((int64_t)p.w_begin + (int64_t)blockIdx.y * p.wpb) * 32;
     for (int i = threadIdx.x; i < p.wpb * 32; i += blockDim.x) {
