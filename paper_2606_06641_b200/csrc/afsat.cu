@@ -31,7 +31,8 @@ namespace {
 
 thread_local std::string g_create_error;
 
-// length classes: register kernels for k in [1,8] and [9,16], shared-memory kernel for [17,64]
+// length classes: register kernels for k in [1,8] and [9,16] (one launch each, one separately compiled
+// body per length), shared-memory kernel for [17,64]
 enum { CLS_A = 0, CLS_B = 1, CLS_LONG = 2, N_CLS = 3 };
 inline int class_of(int k) { return k <= 8 ? CLS_A : k <= 16 ? CLS_B : CLS_LONG; }
 
@@ -55,7 +56,7 @@ struct afsat_ctx {
     void *d_rows = nullptr;
     int8_t *d_fixed = nullptr;
     Item *d_items = nullptr;
-    int32_t n_items = 0, cls_begin[N_CLS + 1] = {0, 0, 0, 0};
+    int32_t n_items = 0, cls_begin[N_CLS + 1] = {0};
     ClassGeom geom[N_CLS];
     int32_t kmax_long = 0;
     int32_t n_sigs = 0, n_buckets = 0;
@@ -147,6 +148,18 @@ void prof_drain(afsat_ctx *c, bool keep)
     c->prof_events.clear();
 }
 
+// k <= 8: fp32 with >= 2 candidates per lane runs the packed FFMA2 kernel, everything else the scalar one
+template <typename T, int VA, int MB>
+void (*pick_a(bool grad))(EvalParams<T>)
+{
+    using Fn = void (*)(EvalParams<T>);
+#ifndef AFSAT_NO_FFMA2
+    if constexpr (sizeof(T) == 4 && VA >= 2) return grad ? (Fn)k_eval_f2m<1, 8, VA / 2, true, MB> : (Fn)k_eval_f2m<1, 8, VA / 2, false, MB>;
+    else
+#endif
+        return grad ? (Fn)k_eval_km<T, 1, 8, VA, true, MB> : (Fn)k_eval_km<T, 1, 8, VA, false, MB>;
+}
+
 // ---- launch of the evaluation kernels (a1-a5) for the candidate tile [b_begin, b_begin + width) ----
 template <typename T>
 int launch_eval(afsat_ctx *ctx, const T *x, T *G, int64_t g_ld, int64_t g_b0, T *Fpart, int64_t b_begin, int64_t width,
@@ -168,13 +181,12 @@ int launch_eval(afsat_ctx *ctx, const T *x, T *G, int64_t g_ld, int64_t g_b0, T 
         p.Wc = g.Wc; p.Wk = g.Wk;
         const int64_t per_cta = (int64_t)32 * g.V * g.Wc;
         dim3 block(32 * g.warps), grid(nit, (unsigned)((width + per_cta - 1) / per_cta));
-        if (cls == CLS_A) {
+        if (cls != CLS_LONG) {
+            using Fn = void (*)(EvalParams<T>);
             constexpr int MB = sizeof(T) == 4 ? AFSAT_A_MINB : 1;
-            if (grad) k_eval_reg<T, 1, 8, VA, true, MB><<<grid, block, 0, st>>>(p);
-            else      k_eval_reg<T, 1, 8, VA, false, MB><<<grid, block, 0, st>>>(p);
-        } else if (cls == CLS_B) {
-            if (grad) k_eval_reg<T, 9, 16, 1, true, 1><<<grid, block, 0, st>>>(p);
-            else      k_eval_reg<T, 9, 16, 1, false, 1><<<grid, block, 0, st>>>(p);
+            Fn fn = cls == CLS_A ? pick_a<T, VA, MB>(grad)
+                                 : (grad ? (Fn)k_eval_km<T, 9, 16, 1, true, 1> : (Fn)k_eval_km<T, 9, 16, 1, false, 1>);
+            fn<<<grid, block, 0, st>>>(p);
         } else {
             if (grad) {
                 CU(cudaFuncSetAttribute(k_eval_long<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem));
@@ -483,7 +495,7 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
 
     // ---- work items: chunks of ONE signature, sized by the cost model and by the literal staging buffer ----
     std::vector<Item> items;
-    int32_t cls_begin[N_CLS + 1] = {0, 0, 0, 0};
+    int32_t cls_begin[N_CLS + 1] = {0};
     int n_buckets = 0;
     {
         int32_t j = 0;

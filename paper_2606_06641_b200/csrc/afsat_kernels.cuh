@@ -176,6 +176,111 @@ __device__ __forceinline__ void eval_points_reg(const T (&y)[K][V], const T *__r
     }
 }
 
+// ---- packed fp32 pairs (sm_100a FFMA2): one instruction evaluates BOTH candidates of a lane ---------
+// fma.rn.f32x2 issues at half the rate of FFMA but does two FMAs, so the FP32 pipe stays the bound
+// while the issue slots freed carry the integer / load-store overhead (measured: DESIGN.md "FFMA2").
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk(float lo, float hi)
+{
+    f32x2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r;
+}
+__device__ __forceinline__ void upk(f32x2 v, float &lo, float &hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c)
+{
+    f32x2 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b)
+{
+    f32x2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d;
+}
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b)
+{
+    f32x2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d;
+}
+
+// Rows of the packed table in shared memory: 12 pairs (c, c) per DFT point.
+//   real point:    {a, b, w, wb, -, -, -, -, -, -, -, -}
+//   complex point: {ar, ai, -ai, br, bi, -bi, wr, -wi, Re(wb), -Im(wb), -, -}
+// FFMA2 has no negated operands, so the negated imaginary parts are tabulated and the backward
+// walk carries the suffix as (Re s, -Im s).
+constexpr int ROW2 = 12;
+
+template <int K, int NP, bool GRAD>
+__device__ __forceinline__ void eval_points_f2(const f32x2 (&y)[K][NP], const f32x2 *__restrict__ tab, int n_real,
+                                               int n_cplx, f32x2 (&fe)[NP], f32x2 (&g)[K][NP])
+{
+    const f32x2 *r = tab;
+    for (int p = 0; p < n_real; ++p, r += ROW2) {                    // self-conjugate points
+        const f32x2 a = r[0], b = r[1], w = r[2], wb = r[3];
+        f32x2 pre[K][NP], f[K][NP], run[NP], suf[NP];
+#pragma unroll
+        for (int i = 0; i < K; ++i)
+#pragma unroll
+            for (int q = 0; q < NP; ++q) f[i][q] = fma2(b, y[i][q], a);
+#pragma unroll
+        for (int q = 0; q < NP; ++q) run[q] = f[0][q];
+#pragma unroll
+        for (int i = 1; i < K; ++i)
+#pragma unroll
+            for (int q = 0; q < NP; ++q) { pre[i][q] = run[q]; run[q] = mul2(run[q], f[i][q]); }
+#pragma unroll
+        for (int q = 0; q < NP; ++q) fe[q] = fma2(w, run[q], fe[q]);
+        if (GRAD) {
+#pragma unroll
+            for (int q = 0; q < NP; ++q) suf[q] = wb;
+#pragma unroll
+            for (int i = K - 1; i >= 1; --i)
+#pragma unroll
+                for (int q = 0; q < NP; ++q) { g[i][q] = fma2(pre[i][q], suf[q], g[i][q]); suf[q] = mul2(suf[q], f[i][q]); }
+#pragma unroll
+            for (int q = 0; q < NP; ++q) g[0][q] = add2(g[0][q], suf[q]);     // prefix_0 = 1
+        }
+    }
+    for (int p = 0; p < n_cplx; ++p, r += ROW2) {                    // one of each conjugate pair
+        const f32x2 ar = r[0], ai = r[1], nai = r[2], br = r[3], bi = r[4], nbi = r[5];
+        f32x2 pr[K][NP], pi[K][NP], fr[K][NP], fi[K][NP], nfi[K][NP], rr[NP], ri[NP];
+#pragma unroll
+        for (int i = 0; i < K; ++i)
+#pragma unroll
+            for (int q = 0; q < NP; ++q) {
+                fr[i][q] = fma2(br, y[i][q], ar); fi[i][q] = fma2(bi, y[i][q], ai); nfi[i][q] = fma2(nbi, y[i][q], nai);
+            }
+#pragma unroll
+        for (int q = 0; q < NP; ++q) { rr[q] = fr[0][q]; ri[q] = fi[0][q]; }
+#pragma unroll
+        for (int i = 1; i < K; ++i)
+#pragma unroll
+            for (int q = 0; q < NP; ++q) {
+                pr[i][q] = rr[q]; pi[i][q] = ri[q];
+                const f32x2 nr = fma2(rr[q], fr[i][q], mul2(ri[q], nfi[i][q]));   // Re: rr fr - ri fi
+                const f32x2 ni = fma2(rr[q], fi[i][q], mul2(ri[q], fr[i][q]));    // Im: rr fi + ri fr
+                rr[q] = nr; ri[q] = ni;
+            }
+#pragma unroll
+        for (int q = 0; q < NP; ++q) {
+            fe[q] = fma2(r[6], rr[q], fe[q]);                         // + wr Re P
+            fe[q] = fma2(r[7], ri[q], fe[q]);                         // - wi Im P
+        }
+        if (GRAD) {
+            f32x2 sr[NP], nsi[NP];                                    // suffix (Re s, -Im s) seeded with w b
+#pragma unroll
+            for (int q = 0; q < NP; ++q) { sr[q] = r[8]; nsi[q] = r[9]; }
+#pragma unroll
+            for (int i = K - 1; i >= 1; --i)
+#pragma unroll
+                for (int q = 0; q < NP; ++q) {
+                    g[i][q] = fma2(pr[i][q], sr[q], g[i][q]);         // Re(pre * suf) = pr sr - pi si
+                    g[i][q] = fma2(pi[i][q], nsi[q], g[i][q]);
+                    const f32x2 t_r = fma2(nsi[q], fi[i][q], mul2(sr[q], fr[i][q]));    // Re: sr fr - si fi
+                    const f32x2 t_n = fma2(nsi[q], fr[i][q], mul2(sr[q], nfi[i][q]));   // -Im: -(sr fi + si fr)
+                    sr[q] = t_r; nsi[q] = t_n;
+                }
+#pragma unroll
+            for (int q = 0; q < NP; ++q) g[0][q] = add2(g[0][q], sr[q]);          // prefix_0 = 1
+        }
+    }
+}
+
 // sign flip by the literal's polarity bit (bit 31 of the packed literal): one LOP3 per value
 __device__ __forceinline__ float flip_sign(float v, int32_t lit)
 {
@@ -230,19 +335,60 @@ __device__ __forceinline__ void run_item_reg(const EvalParams<T> &p, const int32
     }
 }
 
-template <typename T, int K, int KHI, int V, bool GRAD>
-struct DispatchK {
-    static __device__ __forceinline__ void go(const EvalParams<T> &p, int k, bool has_fixed, const int32_t *s_lits,
-                                              const T *s_tab, int n_real, int n_cplx, int nc, int wk, int64_t b, T (&fe)[V])
-    {
-        if (k == K) {
-            if (has_fixed) run_item_reg<T, K, V, GRAD, true>(p, s_lits, s_tab, n_real, n_cplx, nc, wk, b, fe);
-            else run_item_reg<T, K, V, GRAD, false>(p, s_lits, s_tab, n_real, n_cplx, nc, wk, b, fe);
-        } else if (K < KHI) {
-            DispatchK<T, (K < KHI ? K + 1 : K), KHI, V, GRAD>::go(p, k, has_fixed, s_lits, s_tab, n_real, n_cplx, nc, wk, b, fe);
+// The same for SHORT constraints, which are latency-bound on the gathers: the NEXT constraint's
+// literals and row segments are requested before the current one is evaluated (software pipelining).
+// FIXED = the item contains fixed literals (constant y = +-1, no gather, no gradient).
+// Padding candidates (b >= B inside a live lane pair) are computed and scattered like live ones:
+// G's padding columns are scratch here and are reset by the caller.
+template <typename T, int K, int V, bool GRAD, bool FIXED>
+__device__ __forceinline__ void run_item_pf(const EvalParams<T> &p, const int32_t *__restrict__ s_lits,
+                                             const T *__restrict__ s_tab, int n_real, int n_cplx, int nc, int wk,
+                                             int64_t b, T (&fe)[V])
+{
+    const char *xb = reinterpret_cast<const char *>(p.x + b);
+    char *gb = reinterpret_cast<char *>(p.G + (b - p.g_b0));
+    const uint32_t x_ld = (uint32_t)(p.ldb * (int64_t)sizeof(T)), g_ld = (uint32_t)(p.g_ld * (int64_t)sizeof(T));
+    const int Wk = p.Wk;
+    int32_t lit_n[K];
+    T y_n[K][V];
+    auto fetch = [&](int c) {
+        const int32_t *L = s_lits + c * K;
+#pragma unroll
+        for (int i = 0; i < K; ++i) lit_n[i] = L[i];
+#pragma unroll
+        for (int i = 0; i < K; ++i) {
+            if (FIXED && (lit_n[i] & LIT_FIXED)) {                    // warp-uniform branch
+#pragma unroll
+                for (int v = 0; v < V; ++v) y_n[i][v] = T(1);
+            } else {
+                VecIO<T, V>::load(reinterpret_cast<const T *>(xb + (uint64_t)(uint32_t)(lit_n[i] & LIT_VAR) * x_ld), y_n[i]);
+            }
+        }
+    };
+    if (wk < nc) fetch(wk);
+    for (int c = wk; c < nc; c += Wk) {
+        int32_t lit[K];
+        T y[K][V], g[K][V];
+#pragma unroll
+        for (int i = 0; i < K; ++i) {
+            lit[i] = lit_n[i];
+#pragma unroll
+            for (int v = 0; v < V; ++v) { y[i][v] = flip_sign(y_n[i][v], lit[i]); g[i][v] = T(0); }
+        }
+        if (c + Wk < nc) fetch(c + Wk);
+        eval_points_reg<T, K, V, GRAD>(y, s_tab, n_real, n_cplx, fe, g);
+        if (GRAD) {
+#pragma unroll
+            for (int i = 0; i < K; ++i) {
+                if (FIXED && (lit[i] & LIT_FIXED)) continue;          // masked gradient
+                T gi[V];
+#pragma unroll
+                for (int v = 0; v < V; ++v) gi[v] = flip_sign(g[i][v], lit[i]);
+                VecIO<T, V>::red(reinterpret_cast<T *>(gb + (uint64_t)(uint32_t)(lit[i] & LIT_VAR) * g_ld), gi);
+            }
         }
     }
-};
+}
 
 // Stage the item's weight rows and literal list in shared memory (coalesced, once per CTA).
 template <typename T>
@@ -274,11 +420,12 @@ __device__ __forceinline__ void store_item_F(const EvalParams<T> &p, T (*s_F)[32
     }
 }
 
-// Register kernel for one class of lengths [KLO, KHI]; the item's k and signature are CTA-uniform.
-template <typename T, int KLO, int KHI, int V, bool GRAD, int MINB>
-__global__ void __launch_bounds__(CTA_THREADS, MINB) k_eval_reg(const EvalParams<T> p)
+// Register kernel for constraints of length exactly K (one kernel per length: independent register
+// allocation and scheduling); the item's signature is CTA-uniform.
+template <typename T, int K, int V, bool GRAD, int MINB>
+__global__ void __launch_bounds__(CTA_THREADS, MINB) k_eval_k(const EvalParams<T> p)
 {
-    __shared__ __align__(16) T s_tab[(KHI / 2 + 1) * 8];
+    __shared__ __align__(16) T s_tab[((K + 1) / 2 + 1) * 8];    // H = floor((K+1)/2) + 1 DFT points
     __shared__ int32_t s_lits[LIT_CHUNK];
     __shared__ T s_F[CTA_WARPS][32 * V];
     const Item it = p.items[blockIdx.x];
@@ -292,10 +439,256 @@ __global__ void __launch_bounds__(CTA_THREADS, MINB) k_eval_reg(const EvalParams
     T fe[V];
 #pragma unroll
     for (int v = 0; v < V; ++v) fe[v] = T(0);
-    if (active)
-        DispatchK<T, KLO, KHI, V, GRAD>::go(p, it.k, it.has_fixed != 0, s_lits, s_tab, sg.n_real, sg.n_cplx,
-                                            it.c_end - it.c_begin, wk, b, fe);
+    if (active) {
+        const int nc = it.c_end - it.c_begin;
+        if (K <= 5) {
+            if (it.has_fixed) run_item_pf<T, K, V, GRAD, true>(p, s_lits, s_tab, sg.n_real, sg.n_cplx, nc, wk, b, fe);
+            else run_item_pf<T, K, V, GRAD, false>(p, s_lits, s_tab, sg.n_real, sg.n_cplx, nc, wk, b, fe);
+        } else {
+            if (it.has_fixed) run_item_reg<T, K, V, GRAD, true>(p, s_lits, s_tab, sg.n_real, sg.n_cplx, nc, wk, b, fe);
+            else run_item_reg<T, K, V, GRAD, false>(p, s_lits, s_tab, sg.n_real, sg.n_cplx, nc, wk, b, fe);
+        }
+    }
     store_item_F<T, V>(p, s_F, fe, warp, lane, wk, b, active);
+}
+
+// ---- packed-pair register kernel (fp32, NP pairs = 2 NP candidates per lane, FFMA2), length K --------
+template <int NP> struct PairIO;
+template <> struct PairIO<1> {
+    static __device__ __forceinline__ void load(const char *p, f32x2 (&v)[1]) { v[0] = __ldg(reinterpret_cast<const f32x2 *>(p)); }
+    static __device__ __forceinline__ void red(char *p, const f32x2 (&v)[1])
+    {
+        float a, b; upk(v[0], a, b);
+        asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(a), "f"(b) : "memory");
+    }
+};
+template <> struct PairIO<2> {
+    static __device__ __forceinline__ void load(const char *p, f32x2 (&v)[2])
+    {
+        const ulonglong2 t = __ldg(reinterpret_cast<const ulonglong2 *>(p));
+        v[0] = t.x; v[1] = t.y;
+    }
+    static __device__ __forceinline__ void red(char *p, const f32x2 (&v)[2])
+    {
+        float a, b, c, d; upk(v[0], a, b); upk(v[1], c, d);
+        asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
+    }
+};
+
+template <int K, int NP, bool GRAD, bool FIXED, bool PF>
+__device__ __forceinline__ void run_item_f2(const EvalParams<float> &p, const int32_t *__restrict__ s_lits,
+                                            const f32x2 *__restrict__ s_tab2, int n_real, int n_cplx, int nc, int wk,
+                                            int64_t b, f32x2 (&fe)[NP])
+{
+    const char *xb = reinterpret_cast<const char *>(p.x + b);
+    char *gb = reinterpret_cast<char *>(p.G + (b - p.g_b0));
+    const uint32_t x_ld = (uint32_t)(p.ldb * 4), g_ld = (uint32_t)(p.g_ld * 4);
+    const int Wk = p.Wk;
+    const f32x2 one2 = pk(1.0f, 1.0f);
+    int32_t lit_n[K];
+    f32x2 y_n[K][NP];
+    auto fetch = [&](int c) {
+        const int32_t *L = s_lits + c * K;
+#pragma unroll
+        for (int i = 0; i < K; ++i) lit_n[i] = L[i];
+#pragma unroll
+        for (int i = 0; i < K; ++i) {
+            if (FIXED && (lit_n[i] & LIT_FIXED)) {                    // warp-uniform branch
+#pragma unroll
+                for (int q = 0; q < NP; ++q) y_n[i][q] = one2;
+            } else {
+                PairIO<NP>::load(xb + (uint64_t)(uint32_t)(lit_n[i] & LIT_VAR) * x_ld, y_n[i]);
+            }
+        }
+    };
+    if (PF && wk < nc) fetch(wk);
+    for (int c = wk; c < nc; c += Wk) {
+        if (!PF) fetch(c);
+        int32_t lit[K];
+        f32x2 y[K][NP], g[K][NP];
+#pragma unroll
+        for (int i = 0; i < K; ++i) {
+            lit[i] = lit_n[i];
+            const uint32_t m = (uint32_t)(lit[i] & LIT_NEG);
+#pragma unroll
+            for (int q = 0; q < NP; ++q) { y[i][q] = y_n[i][q] ^ (((f32x2)m << 32) | m); g[i][q] = 0ull; }   // y = s x
+        }
+        if (PF && c + Wk < nc) fetch(c + Wk);
+        eval_points_f2<K, NP, GRAD>(y, s_tab2, n_real, n_cplx, fe, g);
+        if (GRAD) {
+#pragma unroll
+            for (int i = 0; i < K; ++i) {
+                if (FIXED && (lit[i] & LIT_FIXED)) continue;          // masked gradient
+                const uint32_t m = (uint32_t)(lit[i] & LIT_NEG);
+                f32x2 gi[NP];
+#pragma unroll
+                for (int q = 0; q < NP; ++q) gi[q] = g[i][q] ^ (((f32x2)m << 32) | m);
+#ifdef AFSAT_EXP_NORED
+                if (gi[0] == 0x123456789ull)
+#endif
+                PairIO<NP>::red(gb + (uint64_t)(uint32_t)(lit[i] & LIT_VAR) * g_ld, gi);
+            }
+        }
+    }
+}
+
+template <int K, int NP, bool GRAD, int MINB>
+__global__ void __launch_bounds__(CTA_THREADS, MINB) k_eval_f2(const EvalParams<float> p)
+{
+    constexpr int H = (K + 1) / 2 + 1;                                // DFT points floor((K+1)/2) + 1
+    constexpr int V = 2 * NP;
+    __shared__ __align__(16) f32x2 s_tab2[H * ROW2];
+    __shared__ int32_t s_lits[LIT_CHUNK];
+    __shared__ float s_F[CTA_WARPS][32 * V];
+    const Item it = p.items[blockIdx.x];
+    const SigDev sg = p.sigs[it.sig];
+    for (int i = threadIdx.x; i < (sg.n_real + sg.n_cplx) * ROW2; i += blockDim.x) {
+        const int q = i / ROW2, j = i % ROW2;
+        const float *r = p.rows + ((int64_t)sg.row_off + q) * 8;
+        float v = 0.f;
+        if (q < sg.n_real) { if (j < 4) v = r[2 * j]; }               // a, b, w, wb
+        else {
+            switch (j) {
+            case 0: v = r[0]; break;  case 1: v = r[1]; break;  case 2: v = -r[1]; break;
+            case 3: v = r[2]; break;  case 4: v = r[3]; break;  case 5: v = -r[3]; break;
+            case 6: v = r[4]; break;  case 7: v = -r[5]; break; case 8: v = r[6]; break;  case 9: v = -r[7]; break;
+            default: break;
+            }
+        }
+        s_tab2[i] = pk(v, v);
+    }
+    const int nl = (it.c_end - it.c_begin) * K;
+    for (int i = threadIdx.x; i < nl; i += blockDim.x) s_lits[i] = __ldg(p.lits + it.lit_base + i);
+    __syncthreads();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int wc = warp % p.Wc, wk = warp / p.Wc;
+    const int64_t b = p.b_begin + ((int64_t)blockIdx.y * p.Wc + wc) * (32 * V) + lane * V;
+    const bool active = b < p.ldb && b < p.B;
+    f32x2 fe2[NP];
+#pragma unroll
+    for (int q = 0; q < NP; ++q) fe2[q] = 0ull;
+    if (active) {
+        const int nc = it.c_end - it.c_begin;
+        constexpr bool PF = K <= 5;
+        if (it.has_fixed) run_item_f2<K, NP, GRAD, true, PF>(p, s_lits, s_tab2, sg.n_real, sg.n_cplx, nc, wk, b, fe2);
+        else run_item_f2<K, NP, GRAD, false, PF>(p, s_lits, s_tab2, sg.n_real, sg.n_cplx, nc, wk, b, fe2);
+    }
+    float fe[V];
+#pragma unroll
+    for (int q = 0; q < NP; ++q) upk(fe2[q], fe[2 * q], fe[2 * q + 1]);
+    store_item_F<float, V>(p, s_F, fe, warp, lane, wk, b, active);
+}
+
+// ---- one launch for a RANGE of lengths [KLO, KHI]: the CTA's item picks its length-K body, which is a
+// separately compiled (noinline) function so that every length keeps its own schedule and register
+// allocation while all lengths share one grid (no per-length launch tails) ---------------------------
+template <int K, int NP, bool GRAD>
+__device__ __noinline__ void item_body_f2(const EvalParams<float> &p, const int32_t *s_lits, const f32x2 *s_tab2,
+                                          float (*s_F)[64 * NP], int n_real, int n_cplx, int nc, bool has_fixed)
+{
+    constexpr int V = 2 * NP;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int wc = warp % p.Wc, wk = warp / p.Wc;
+    const int64_t b = p.b_begin + ((int64_t)blockIdx.y * p.Wc + wc) * (32 * V) + lane * V;
+    const bool active = b < p.ldb && b < p.B;
+    f32x2 fe2[NP];
+#pragma unroll
+    for (int q = 0; q < NP; ++q) fe2[q] = 0ull;
+    if (active) {
+        constexpr bool PF = K <= 5;
+        if (has_fixed) run_item_f2<K, NP, GRAD, true, PF>(p, s_lits, s_tab2, n_real, n_cplx, nc, wk, b, fe2);
+        else run_item_f2<K, NP, GRAD, false, PF>(p, s_lits, s_tab2, n_real, n_cplx, nc, wk, b, fe2);
+    }
+    float fe[V];
+#pragma unroll
+    for (int q = 0; q < NP; ++q) upk(fe2[q], fe[2 * q], fe[2 * q + 1]);
+    store_item_F<float, V>(p, s_F, fe, warp, lane, wk, b, active);
+}
+
+template <int K, int KHI, int NP, bool GRAD>
+struct SwitchF2 {
+    static __device__ __forceinline__ void go(int k, const EvalParams<float> &p, const int32_t *s_lits, const f32x2 *s_tab2,
+                                              float (*s_F)[64 * NP], int n_real, int n_cplx, int nc, bool has_fixed)
+    {
+        if (k == K) item_body_f2<K, NP, GRAD>(p, s_lits, s_tab2, s_F, n_real, n_cplx, nc, has_fixed);
+        else if (K < KHI) SwitchF2<(K < KHI ? K + 1 : K), KHI, NP, GRAD>::go(k, p, s_lits, s_tab2, s_F, n_real, n_cplx, nc, has_fixed);
+    }
+};
+
+template <int KLO, int KHI, int NP, bool GRAD, int MINB>
+__global__ void __launch_bounds__(CTA_THREADS, MINB) k_eval_f2m(const EvalParams<float> p)
+{
+    constexpr int H = (KHI + 1) / 2 + 1;
+    __shared__ __align__(16) f32x2 s_tab2[H * ROW2];
+    __shared__ int32_t s_lits[LIT_CHUNK];
+    __shared__ float s_F[CTA_WARPS][64 * NP];
+    const Item it = p.items[blockIdx.x];
+    const SigDev sg = p.sigs[it.sig];
+    for (int i = threadIdx.x; i < (sg.n_real + sg.n_cplx) * ROW2; i += blockDim.x) {
+        const int q = i / ROW2, j = i % ROW2;
+        const float *r = p.rows + ((int64_t)sg.row_off + q) * 8;
+        float v = 0.f;
+        if (q < sg.n_real) { if (j < 4) v = r[2 * j]; }               // a, b, w, wb
+        else {
+            switch (j) {
+            case 0: v = r[0]; break;  case 1: v = r[1]; break;  case 2: v = -r[1]; break;
+            case 3: v = r[2]; break;  case 4: v = r[3]; break;  case 5: v = -r[3]; break;
+            case 6: v = r[4]; break;  case 7: v = -r[5]; break; case 8: v = r[6]; break;  case 9: v = -r[7]; break;
+            default: break;
+            }
+        }
+        s_tab2[i] = pk(v, v);
+    }
+    const int nl = (it.c_end - it.c_begin) * it.k;
+    for (int i = threadIdx.x; i < nl; i += blockDim.x) s_lits[i] = __ldg(p.lits + it.lit_base + i);
+    __syncthreads();
+    SwitchF2<KLO, KHI, NP, GRAD>::go(it.k, p, s_lits, s_tab2, s_F, sg.n_real, sg.n_cplx, it.c_end - it.c_begin, it.has_fixed != 0);
+}
+
+template <typename T, int K, int V, bool GRAD>
+__device__ __noinline__ void item_body_k(const EvalParams<T> &p, const int32_t *s_lits, const T *s_tab, T (*s_F)[32 * V],
+                                         int n_real, int n_cplx, int nc, bool has_fixed)
+{
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int wc = warp % p.Wc, wk = warp / p.Wc;
+    const int64_t b = p.b_begin + ((int64_t)blockIdx.y * p.Wc + wc) * (32 * V) + lane * V;
+    const bool active = b < p.ldb && b < p.B;
+    T fe[V];
+#pragma unroll
+    for (int v = 0; v < V; ++v) fe[v] = T(0);
+    if (active) {
+        if (K <= 5) {
+            if (has_fixed) run_item_pf<T, K, V, GRAD, true>(p, s_lits, s_tab, n_real, n_cplx, nc, wk, b, fe);
+            else run_item_pf<T, K, V, GRAD, false>(p, s_lits, s_tab, n_real, n_cplx, nc, wk, b, fe);
+        } else {
+            if (has_fixed) run_item_reg<T, K, V, GRAD, true>(p, s_lits, s_tab, n_real, n_cplx, nc, wk, b, fe);
+            else run_item_reg<T, K, V, GRAD, false>(p, s_lits, s_tab, n_real, n_cplx, nc, wk, b, fe);
+        }
+    }
+    store_item_F<T, V>(p, s_F, fe, warp, lane, wk, b, active);
+}
+
+template <typename T, int K, int KHI, int V, bool GRAD>
+struct SwitchK {
+    static __device__ __forceinline__ void go(int k, const EvalParams<T> &p, const int32_t *s_lits, const T *s_tab,
+                                              T (*s_F)[32 * V], int n_real, int n_cplx, int nc, bool has_fixed)
+    {
+        if (k == K) item_body_k<T, K, V, GRAD>(p, s_lits, s_tab, s_F, n_real, n_cplx, nc, has_fixed);
+        else if (K < KHI) SwitchK<T, (K < KHI ? K + 1 : K), KHI, V, GRAD>::go(k, p, s_lits, s_tab, s_F, n_real, n_cplx, nc, has_fixed);
+    }
+};
+
+template <typename T, int KLO, int KHI, int V, bool GRAD, int MINB>
+__global__ void __launch_bounds__(CTA_THREADS, MINB) k_eval_km(const EvalParams<T> p)
+{
+    __shared__ __align__(16) T s_tab[((KHI + 1) / 2 + 1) * 8];
+    __shared__ int32_t s_lits[LIT_CHUNK];
+    __shared__ T s_F[CTA_WARPS][32 * V];
+    const Item it = p.items[blockIdx.x];
+    const SigDev sg = p.sigs[it.sig];
+    stage_item(p, it, sg, s_tab, s_lits);
+    __syncthreads();
+    SwitchK<T, KLO, KHI, V, GRAD>::go(it.k, p, s_lits, s_tab, s_F, sg.n_real, sg.n_cplx, it.c_end - it.c_begin, it.has_fixed != 0);
 }
 
 // ---- generic kernel for long constraints (runtime k <= 64), V = 1: literal values, prefix products
