@@ -70,6 +70,8 @@ struct afsat_ctx {
     int32_t *dh_sat = nullptr, *dh_first = nullptr;
     uint8_t *dh_sol = nullptr;
     cudaStream_t own_stream = nullptr;
+    cudaStream_t side_stream[N_CLS - 1] = {nullptr, nullptr};       // concurrent launches of the length classes
+    cudaEvent_t ev_fork = nullptr, ev_join[N_CLS - 1] = {nullptr, nullptr};
     size_t ws_bytes = 0;
     int64_t launches = 0;
     // afsat_set_profiling: event pairs around the evaluation-kernel launches
@@ -171,10 +173,25 @@ int launch_eval(afsat_ctx *ctx, const T *x, T *G, int64_t g_ld, int64_t g_b0, T 
     p.B = ctx->B; p.ldb = ctx->ldb; p.b_begin = b_begin;
     const bool grad = G != nullptr;
     constexpr int VA = sizeof(T) == 4 ? AFSAT_A_V : 1;
+    // The length classes are independent (they only share the RED target), so their launches run
+    // CONCURRENTLY: class 0 on the caller's stream, the others on forked side streams that join back.
+    int n_active = 0;
+    for (int cls = 0; cls < N_CLS; ++cls) n_active += ctx->cls_begin[cls + 1] > ctx->cls_begin[cls];
+    ProfScope prof(ctx, st);                                          // brackets the whole launch set
+    const bool fork = n_active > 1;
+    if (fork) CU(cudaEventRecord(ctx->ev_fork, st));
+    int side = 0;
+    cudaStream_t user_st = st;
     for (int cls = 0; cls < N_CLS; ++cls) {
         const int nit = ctx->cls_begin[cls + 1] - ctx->cls_begin[cls];
         if (nit == 0) continue;
-        ProfScope prof(ctx, st);
+        st = user_st;
+        int my_side = -1;
+        if (fork && side < N_CLS - 1 && cls != 0 && ctx->cls_begin[cls] != 0) {   // not the first active class
+            my_side = side++;
+            st = ctx->side_stream[my_side];
+            CU(cudaStreamWaitEvent(st, ctx->ev_fork, 0));
+        }
         const ClassGeom &g = ctx->geom[cls];
         p.items = ctx->d_items + ctx->cls_begin[cls];
         p.frow_base = ctx->cls_begin[cls];
@@ -188,16 +205,21 @@ int launch_eval(afsat_ctx *ctx, const T *x, T *G, int64_t g_ld, int64_t g_b0, T 
                                  : (grad ? (Fn)k_eval_km<T, 9, 16, 1, true, 1> : (Fn)k_eval_km<T, 9, 16, 1, false, 1>);
             fn<<<grid, block, 0, st>>>(p);
         } else {
-            if (grad) {
-                CU(cudaFuncSetAttribute(k_eval_long<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem));
-                k_eval_long<T, true><<<grid, block, g.smem, st>>>(p, ctx->kmax_long);
-            } else {
-                CU(cudaFuncSetAttribute(k_eval_long<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem));
-                k_eval_long<T, false><<<grid, block, g.smem, st>>>(p, ctx->kmax_long);
-            }
+            using Fn = void (*)(EvalParams<T>);
+            Fn fn;
+            const int km = ctx->kmax_long <= 32 ? 32 : ctx->kmax_long <= 48 ? 48 : 64;
+            if (km == 32) fn = grad ? (Fn)k_eval_blk<T, 32, true> : (Fn)k_eval_blk<T, 32, false>;
+            else if (km == 48) fn = grad ? (Fn)k_eval_blk<T, 48, true> : (Fn)k_eval_blk<T, 48, false>;
+            else fn = grad ? (Fn)k_eval_blk<T, 64, true> : (Fn)k_eval_blk<T, 64, false>;
+            CU(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem));
+            fn<<<grid, block, g.smem, st>>>(p);
         }
         ++ctx->launches;
         CU(cudaPeekAtLastError());
+        if (my_side >= 0) {
+            CU(cudaEventRecord(ctx->ev_join[my_side], st));
+            CU(cudaStreamWaitEvent(user_st, ctx->ev_join[my_side], 0));
+        }
     }
     return AFSAT_OK;
 }
@@ -482,10 +504,9 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
         g.V = (cls == CLS_A && dtype == 32) ? AFSAT_A_V : 1;
         g.warps = CTA_WARPS;
         if (cls == CLS_LONG) {
-            const size_t fixed_b = (size_t)MAX_ROWS * 8 * esz + (size_t)LIT_CHUNK * 4 + (size_t)CTA_WARPS * 32 * esz;
-            const size_t per_warp = (size_t)4 * std::max(kmax_long, 1) * 32 * esz;
-            g.warps = pow2_floor(std::max<int64_t>(1, std::min<int64_t>(CTA_WARPS, (int64_t)((200 * 1024 - fixed_b) / per_warp))));
-            g.smem = fixed_b + per_warp * g.warps;
+            const int km = kmax_long <= 32 ? 32 : kmax_long <= 48 ? 48 : 64;
+            g.warps = LONG_THREADS / 32;
+            g.smem = (size_t)g.warps * km * 32 * esz;                  // literal values [warps][KMAX][32]
         }
         const int64_t cw = 32 * g.V;
         g.Wc = std::min(g.warps, pow2_floor(std::max<int64_t>(1, (tile_w + cw - 1) / cw)));
@@ -592,6 +613,11 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
     CREATE_FAIL(dev_alloc(ctx, &ctx->d_any, 2, true));
     {
         cudaError_t e = cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming);
+        for (int i = 0; i < N_CLS - 1 && e == cudaSuccess; ++i) {
+            e = cudaStreamCreateWithFlags(&ctx->side_stream[i], cudaStreamNonBlocking);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_join[i], cudaEventDisableTiming);
+        }
         if (e != cudaSuccess) { ctx->err = cudaGetErrorString(e); CREATE_FAIL(AFSAT_E_CUDA); }
     }
     *out = ctx;
@@ -616,6 +642,11 @@ void afsat_destroy(afsat_ctx *ctx)
     cudaFree(ctx->d_satacc); cudaFree(ctx->d_any);
     cudaFree(ctx->dh_x); cudaFree(ctx->dh_F); cudaFree(ctx->dh_sat); cudaFree(ctx->dh_first); cudaFree(ctx->dh_sol);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
+    for (int i = 0; i < N_CLS - 1; ++i) {
+        if (ctx->side_stream[i]) cudaStreamDestroy(ctx->side_stream[i]);
+        if (ctx->ev_join[i]) cudaEventDestroy(ctx->ev_join[i]);
+    }
+    if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
     delete ctx;
 }
 

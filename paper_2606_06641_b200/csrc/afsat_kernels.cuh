@@ -779,6 +779,185 @@ __global__ void __launch_bounds__(CTA_THREADS) k_eval_long(const EvalParams<T> p
     store_item_F<T, 1>(p, reinterpret_cast<T(*)[32]>(s_F), fe_acc, warp, lane, wk, b, active);
 }
 
+// ---- register-blocked kernel for long constraints (16 < k <= KMAX <= 64), one candidate per lane ------
+// The k partial gradients live in REGISTERS (the literal loop is unrolled to KMAX in blocks of LB, blocks
+// beyond k are skipped by a warp-uniform branch); the literal values are staged once per constraint in
+// shared memory as [i][lane] columns; per DFT point the forward pass keeps only the prefix product at
+// each block boundary and the backward pass rebuilds the LB prefixes of a block from its boundary value
+// before walking the suffix through it (leave-one-out = prefix x suffix, no division).  Shared-memory
+// traffic is 2 loads per literal and point instead of the 9 accesses of a fully staged scheme.
+constexpr int LB = 8;
+constexpr int LONG_THREADS = 128;
+
+template <typename T, bool CPLX, int NU>
+struct BlkOps {
+    // forward through one block of NU literals: run <- run * prod f_u
+    static __device__ __forceinline__ void fwd(const T *__restrict__ sy, T ar, T ai, T br, T bi, T &rr, T &ri)
+    {
+#pragma unroll
+        for (int u = 0; u < NU; ++u) {
+            const T yv = sy[u * 32];
+            const T fr = fma_(br, yv, ar);
+            if (CPLX) {
+                const T fi = fma_(bi, yv, ai);
+                const T nr = fma_(rr, fr, -(ri * fi));
+                const T ni = fma_(rr, fi, ri * fr);
+                rr = nr; ri = ni;
+            } else {
+                rr *= fr;
+            }
+        }
+    }
+    // backward through one block: prefixes rebuilt from the boundary value (pr0, pi0), then
+    // g_u += Re(prefix_u * suffix), suffix <- suffix * f_u for u = NU-1 .. 0
+    static __device__ __forceinline__ void bwd(const T *__restrict__ sy, T ar, T ai, T br, T bi, T pr0, T pi0, T &sr, T &si,
+                                               T *__restrict__ g)
+    {
+        T fr[NU], fi[CPLX ? NU : 1], pr[NU], pi[CPLX ? NU : 1];
+#pragma unroll
+        for (int u = 0; u < NU; ++u) {
+            const T yv = sy[u * 32];
+            fr[u] = fma_(br, yv, ar);
+            if (CPLX) fi[u] = fma_(bi, yv, ai);
+        }
+        pr[0] = pr0;
+        if (CPLX) pi[0] = pi0;
+#pragma unroll
+        for (int u = 1; u < NU; ++u) {
+            if (CPLX) {
+                pr[u] = fma_(pr[u - 1], fr[u - 1], -(pi[u - 1] * fi[u - 1]));
+                pi[u] = fma_(pr[u - 1], fi[u - 1], pi[u - 1] * fr[u - 1]);
+            } else {
+                pr[u] = pr[u - 1] * fr[u - 1];
+            }
+        }
+#pragma unroll
+        for (int u = NU - 1; u >= 0; --u) {
+            if (CPLX) {
+                g[u] = fma_(pr[u], sr, g[u]);
+                g[u] = fma_(-pi[u], si, g[u]);
+                const T nr = fma_(sr, fr[u], -(si * fi[u]));
+                const T ni = fma_(sr, fi[u], si * fr[u]);
+                sr = nr; si = ni;
+            } else {
+                g[u] = fma_(pr[u], sr, g[u]);
+                sr *= fr[u];
+            }
+        }
+    }
+};
+
+// dispatch on the (warp-uniform) number of literals nu in [1, LB] of the last, partial block
+template <typename T, bool CPLX>
+__device__ __forceinline__ void blk_fwd_n(int nu, const T *sy, T ar, T ai, T br, T bi, T &rr, T &ri)
+{
+    switch (nu) {
+    case 1: BlkOps<T, CPLX, 1>::fwd(sy, ar, ai, br, bi, rr, ri); break;
+    case 2: BlkOps<T, CPLX, 2>::fwd(sy, ar, ai, br, bi, rr, ri); break;
+    case 3: BlkOps<T, CPLX, 3>::fwd(sy, ar, ai, br, bi, rr, ri); break;
+    case 4: BlkOps<T, CPLX, 4>::fwd(sy, ar, ai, br, bi, rr, ri); break;
+    case 5: BlkOps<T, CPLX, 5>::fwd(sy, ar, ai, br, bi, rr, ri); break;
+    case 6: BlkOps<T, CPLX, 6>::fwd(sy, ar, ai, br, bi, rr, ri); break;
+    default: BlkOps<T, CPLX, 7>::fwd(sy, ar, ai, br, bi, rr, ri); break;
+    }
+}
+
+template <typename T, int KMAX, bool CPLX, bool GRAD>
+__device__ __forceinline__ void long_point(const T *__restrict__ sy, int k, const T *__restrict__ r, T &fe, T (&g)[KMAX])
+{
+    constexpr int NBLK = KMAX / LB;
+    const T ar = r[0], ai = r[1], br = r[2], bi = r[3];
+    T bnd_r[NBLK], bnd_i[CPLX ? NBLK : 1];
+    T rr = T(1), ri = T(0);
+    const int nfull = k / LB, tail = k % LB;
+#pragma unroll
+    for (int blk = 0; blk < NBLK; ++blk) {
+        if (blk < nfull) {
+            bnd_r[blk] = rr; if (CPLX) bnd_i[blk] = ri;
+            BlkOps<T, CPLX, LB>::fwd(sy + blk * LB * 32, ar, ai, br, bi, rr, ri);
+        } else if (blk == nfull && tail) {
+            bnd_r[blk] = rr; if (CPLX) bnd_i[blk] = ri;
+            blk_fwd_n<T, CPLX>(tail, sy + blk * LB * 32, ar, ai, br, bi, rr, ri);
+        }
+    }
+    fe = fma_(r[4], rr, fe);
+    if (CPLX) fe = fma_(-r[5], ri, fe);
+    if (GRAD) {
+        T sr = r[6], si = CPLX ? r[7] : T(0);                          // suffix seeded with w b
+#pragma unroll
+        for (int blk = NBLK - 1; blk >= 0; --blk) {
+            if (blk < nfull) {
+                BlkOps<T, CPLX, LB>::bwd(sy + blk * LB * 32, ar, ai, br, bi, bnd_r[blk], CPLX ? bnd_i[blk] : T(0), sr, si, &g[blk * LB]);
+            } else if (blk == nfull && tail) {
+                T *gb = &g[blk * LB];
+                const T *syb = sy + blk * LB * 32;
+                const T p0 = bnd_r[blk], p1 = CPLX ? bnd_i[blk] : T(0);
+                switch (tail) {
+                case 1: BlkOps<T, CPLX, 1>::bwd(syb, ar, ai, br, bi, p0, p1, sr, si, gb); break;
+                case 2: BlkOps<T, CPLX, 2>::bwd(syb, ar, ai, br, bi, p0, p1, sr, si, gb); break;
+                case 3: BlkOps<T, CPLX, 3>::bwd(syb, ar, ai, br, bi, p0, p1, sr, si, gb); break;
+                case 4: BlkOps<T, CPLX, 4>::bwd(syb, ar, ai, br, bi, p0, p1, sr, si, gb); break;
+                case 5: BlkOps<T, CPLX, 5>::bwd(syb, ar, ai, br, bi, p0, p1, sr, si, gb); break;
+                case 6: BlkOps<T, CPLX, 6>::bwd(syb, ar, ai, br, bi, p0, p1, sr, si, gb); break;
+                default: BlkOps<T, CPLX, 7>::bwd(syb, ar, ai, br, bi, p0, p1, sr, si, gb); break;
+                }
+            }
+        }
+    }
+}
+
+template <typename T, int KMAX, bool GRAD>
+__global__ void __launch_bounds__(LONG_THREADS) k_eval_blk(const EvalParams<T> p)
+{
+    constexpr int NW = LONG_THREADS / 32;
+    __shared__ __align__(16) T s_tab[MAX_ROWS * 8];
+    __shared__ int32_t s_lits[LIT_CHUNK];
+    __shared__ T s_F[NW][32];
+    extern __shared__ __align__(16) unsigned char s_dyn[];               // literal values [NW][KMAX][32]
+    T *s_y = reinterpret_cast<T *>(s_dyn);
+    const Item it = p.items[blockIdx.x];
+    const SigDev sgd = p.sigs[it.sig];
+    stage_item(p, it, sgd, s_tab, s_lits);
+    __syncthreads();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int wc = warp % p.Wc, wk = warp / p.Wc;
+    const int64_t b = p.b_begin + ((int64_t)blockIdx.y * p.Wc + wc) * 32 + lane;
+    const bool active = b < p.ldb && b < p.B;
+    T fe[1] = {T(0)};
+    if (active) {
+        T *sy = s_y + (size_t)warp * KMAX * 32 + lane;
+        const int k = it.k, nc = it.c_end - it.c_begin;
+        const char *xb = reinterpret_cast<const char *>(p.x + b);
+        char *gb = reinterpret_cast<char *>(p.G + (b - p.g_b0));
+        const uint32_t x_ld = (uint32_t)(p.ldb * (int64_t)sizeof(T)), g_ld = (uint32_t)(p.g_ld * (int64_t)sizeof(T));
+        for (int c = wk; c < nc; c += p.Wk) {
+            const int32_t *L = s_lits + c * k;
+            for (int i = 0; i < k; ++i) {                               // a1: gather, sign, stage
+                const int32_t lit = L[i];
+                const T v = (lit & LIT_FIXED) ? T(1) : __ldg(reinterpret_cast<const T *>(xb + (uint64_t)(uint32_t)(lit & LIT_VAR) * x_ld));
+                sy[i * 32] = flip_sign(v, lit);
+            }
+            T g[KMAX];
+#pragma unroll
+            for (int i = 0; i < KMAX; ++i) g[i] = T(0);
+            const T *r = s_tab;
+            for (int q = 0; q < sgd.n_real; ++q, r += 8) long_point<T, KMAX, false, GRAD>(sy, k, r, fe[0], g);
+            for (int q = 0; q < sgd.n_cplx; ++q, r += 8) long_point<T, KMAX, true, GRAD>(sy, k, r, fe[0], g);
+            if (GRAD) {
+#pragma unroll
+                for (int i = 0; i < KMAX; ++i) {
+                    if (i < k) {                                        // warp-uniform
+                        const int32_t lit = L[i];
+                        if (!(lit & LIT_FIXED))
+                            atomicAdd(reinterpret_cast<T *>(gb + (uint64_t)(uint32_t)(lit & LIT_VAR) * g_ld), flip_sign(g[i], lit));
+                    }
+                }
+            }
+        }
+    }
+    store_item_F<T, 1>(p, s_F, fe, warp, lane, wk, b, active);
+}
+
 // ---- a7: sign rounding as one bit per (variable, candidate): bits[v][b / 32] bit (b % 32) = (x < 0)
 template <typename T>
 __global__ void __launch_bounds__(CTA_THREADS) k_pack_signs(const T *__restrict__ x, uint32_t *__restrict__ bits, int n,
