@@ -506,7 +506,7 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
         if (cls == CLS_LONG) {
             const int km = kmax_long <= 32 ? 32 : kmax_long <= 48 ? 48 : 64;
             g.warps = LONG_THREADS / 32;
-            g.smem = (size_t)g.warps * km * 32 * esz;                  // literal values [warps][KMAX][32]
+            g.smem = (size_t)g.warps * (km + 2 * (km / LB)) * 32 * esz; // per warp: values [KMAX][32] + boundaries [2 KMAX/LB][32]
         }
         const int64_t cw = 32 * g.V;
         g.Wc = std::min(g.warps, pow2_floor(std::max<int64_t>(1, (tile_w + cw - 1) / cw)));
@@ -535,7 +535,7 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
             const int64_t cost_budget = std::max<int64_t>(1, total_cost / chunks_wanted);
             const int64_t cost1 = std::max<int64_t>(1, sig_cost[sg]);
             int64_t chunk = std::max<int64_t>(g.Wk, (cost_budget + cost1 - 1) / cost1);
-            chunk = std::min<int64_t>(chunk, LIT_CHUNK / k);
+            chunk = std::min<int64_t>(chunk, (cls == CLS_LONG ? LONG_LIT_CHUNK : LIT_CHUNK) / k);
             chunk = std::max<int64_t>(1, chunk);
             for (int32_t s = j; s < e; s += (int32_t)chunk) {
                 Item it;

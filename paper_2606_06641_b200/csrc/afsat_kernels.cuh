@@ -788,6 +788,7 @@ __global__ void __launch_bounds__(CTA_THREADS) k_eval_long(const EvalParams<T> p
 // traffic is 2 loads per literal and point instead of the 9 accesses of a fully staged scheme.
 constexpr int LB = 8;
 constexpr int LONG_THREADS = 128;
+constexpr int LONG_LIT_CHUNK = 1024;   // packed literals per work item of the long class (>= 16 constraints)
 
 template <typename T, bool CPLX, int NU>
 struct BlkOps {
@@ -847,60 +848,79 @@ struct BlkOps {
     }
 };
 
-// dispatch on the (warp-uniform) number of literals nu in [1, LB] of the last, partial block
+// backward through the LAST, partial block (nu < LB literals; the staged values beyond k are zeros):
+// same arithmetic, the updates of g and of the suffix predicated on u < nu
 template <typename T, bool CPLX>
-__device__ __forceinline__ void blk_fwd_n(int nu, const T *sy, T ar, T ai, T br, T bi, T &rr, T &ri)
+__device__ __forceinline__ void blk_bwd_partial(int nu, const T *__restrict__ sy, T ar, T ai, T br, T bi, T pr0, T pi0, T &sr,
+                                                T &si, T *__restrict__ g)
 {
-    switch (nu) {
-    case 1: BlkOps<T, CPLX, 1>::fwd(sy, ar, ai, br, bi, rr, ri); break;
-    case 2: BlkOps<T, CPLX, 2>::fwd(sy, ar, ai, br, bi, rr, ri); break;
-    case 3: BlkOps<T, CPLX, 3>::fwd(sy, ar, ai, br, bi, rr, ri); break;
-    case 4: BlkOps<T, CPLX, 4>::fwd(sy, ar, ai, br, bi, rr, ri); break;
-    case 5: BlkOps<T, CPLX, 5>::fwd(sy, ar, ai, br, bi, rr, ri); break;
-    case 6: BlkOps<T, CPLX, 6>::fwd(sy, ar, ai, br, bi, rr, ri); break;
-    default: BlkOps<T, CPLX, 7>::fwd(sy, ar, ai, br, bi, rr, ri); break;
+    T fr[LB], fi[CPLX ? LB : 1], pr[LB], pi[CPLX ? LB : 1];
+#pragma unroll
+    for (int u = 0; u < LB; ++u) {
+        const T yv = sy[u * 32];
+        fr[u] = fma_(br, yv, ar);
+        if (CPLX) fi[u] = fma_(bi, yv, ai);
+    }
+    pr[0] = pr0;
+    if (CPLX) pi[0] = pi0;
+#pragma unroll
+    for (int u = 1; u < LB; ++u) {
+        if (CPLX) {
+            pr[u] = fma_(pr[u - 1], fr[u - 1], -(pi[u - 1] * fi[u - 1]));
+            pi[u] = fma_(pr[u - 1], fi[u - 1], pi[u - 1] * fr[u - 1]);
+        } else {
+            pr[u] = pr[u - 1] * fr[u - 1];
+        }
+    }
+#pragma unroll
+    for (int u = LB - 1; u >= 0; --u) {
+        if (u < nu) {                                                 // warp-uniform
+            if (CPLX) {
+                g[u] = fma_(pr[u], sr, g[u]);
+                g[u] = fma_(-pi[u], si, g[u]);
+                const T nr = fma_(sr, fr[u], -(si * fi[u]));
+                const T ni = fma_(sr, fi[u], si * fr[u]);
+                sr = nr; si = ni;
+            } else {
+                g[u] = fma_(pr[u], sr, g[u]);
+                sr *= fr[u];
+            }
+        }
     }
 }
 
+// One DFT point of a long constraint.  sy: staged literal values [i][lane] (zeros up to the next
+// multiple of LB), sb: boundary prefixes [blk][re, im][lane] of this warp.
 template <typename T, int KMAX, bool CPLX, bool GRAD>
-__device__ __forceinline__ void long_point(const T *__restrict__ sy, int k, const T *__restrict__ r, T &fe, T (&g)[KMAX])
+__device__ __forceinline__ void long_point(const T *__restrict__ sy, T *__restrict__ sb, int k, const T *__restrict__ r, T &fe,
+                                           T (&g)[KMAX])
 {
     constexpr int NBLK = KMAX / LB;
     const T ar = r[0], ai = r[1], br = r[2], bi = r[3];
-    T bnd_r[NBLK], bnd_i[CPLX ? NBLK : 1];
     T rr = T(1), ri = T(0);
     const int nfull = k / LB, tail = k % LB;
-#pragma unroll
-    for (int blk = 0; blk < NBLK; ++blk) {
-        if (blk < nfull) {
-            bnd_r[blk] = rr; if (CPLX) bnd_i[blk] = ri;
-            BlkOps<T, CPLX, LB>::fwd(sy + blk * LB * 32, ar, ai, br, bi, rr, ri);
-        } else if (blk == nfull && tail) {
-            bnd_r[blk] = rr; if (CPLX) bnd_i[blk] = ri;
-            blk_fwd_n<T, CPLX>(tail, sy + blk * LB * 32, ar, ai, br, bi, rr, ri);
-        }
+    for (int blk = 0; blk < nfull; ++blk) {                           // forward: runtime loop, one body
+        sb[(2 * blk) * 32] = rr;
+        if (CPLX) sb[(2 * blk + 1) * 32] = ri;
+        BlkOps<T, CPLX, LB>::fwd(sy + blk * LB * 32, ar, ai, br, bi, rr, ri);
+    }
+    if (tail) {
+        sb[(2 * nfull) * 32] = rr;
+        if (CPLX) sb[(2 * nfull + 1) * 32] = ri;
+        for (int u = 0; u < tail; ++u) BlkOps<T, CPLX, 1>::fwd(sy + (nfull * LB + u) * 32, ar, ai, br, bi, rr, ri);
     }
     fe = fma_(r[4], rr, fe);
     if (CPLX) fe = fma_(-r[5], ri, fe);
     if (GRAD) {
         T sr = r[6], si = CPLX ? r[7] : T(0);                          // suffix seeded with w b
 #pragma unroll
-        for (int blk = NBLK - 1; blk >= 0; --blk) {
+        for (int blk = NBLK - 1; blk >= 0; --blk) {                    // backward: unrolled, g in registers
             if (blk < nfull) {
-                BlkOps<T, CPLX, LB>::bwd(sy + blk * LB * 32, ar, ai, br, bi, bnd_r[blk], CPLX ? bnd_i[blk] : T(0), sr, si, &g[blk * LB]);
+                BlkOps<T, CPLX, LB>::bwd(sy + blk * LB * 32, ar, ai, br, bi, sb[(2 * blk) * 32],
+                                         CPLX ? sb[(2 * blk + 1) * 32] : T(0), sr, si, &g[blk * LB]);
             } else if (blk == nfull && tail) {
-                T *gb = &g[blk * LB];
-                const T *syb = sy + blk * LB * 32;
-                const T p0 = bnd_r[blk], p1 = CPLX ? bnd_i[blk] : T(0);
-                switch (tail) {
-                case 1: BlkOps<T, CPLX, 1>::bwd(syb, ar, ai, br, bi, p0, p1, sr, si, gb); break;
-                case 2: BlkOps<T, CPLX, 2>::bwd(syb, ar, ai, br, bi, p0, p1, sr, si, gb); break;
-                case 3: BlkOps<T, CPLX, 3>::bwd(syb, ar, ai, br, bi, p0, p1, sr, si, gb); break;
-                case 4: BlkOps<T, CPLX, 4>::bwd(syb, ar, ai, br, bi, p0, p1, sr, si, gb); break;
-                case 5: BlkOps<T, CPLX, 5>::bwd(syb, ar, ai, br, bi, p0, p1, sr, si, gb); break;
-                case 6: BlkOps<T, CPLX, 6>::bwd(syb, ar, ai, br, bi, p0, p1, sr, si, gb); break;
-                default: BlkOps<T, CPLX, 7>::bwd(syb, ar, ai, br, bi, p0, p1, sr, si, gb); break;
-                }
+                blk_bwd_partial<T, CPLX>(tail, sy + blk * LB * 32, ar, ai, br, bi, sb[(2 * blk) * 32],
+                                         CPLX ? sb[(2 * blk + 1) * 32] : T(0), sr, si, &g[blk * LB]);
             }
         }
     }
@@ -911,9 +931,10 @@ __global__ void __launch_bounds__(LONG_THREADS) k_eval_blk(const EvalParams<T> p
 {
     constexpr int NW = LONG_THREADS / 32;
     __shared__ __align__(16) T s_tab[MAX_ROWS * 8];
-    __shared__ int32_t s_lits[LIT_CHUNK];
+    __shared__ int32_t s_lits[LONG_LIT_CHUNK];
     __shared__ T s_F[NW][32];
-    extern __shared__ __align__(16) unsigned char s_dyn[];               // literal values [NW][KMAX][32]
+    extern __shared__ __align__(16) unsigned char s_dyn[];               // per warp: values [KMAX][32], boundaries [2 NBLK][32]
+    constexpr int PER_WARP = (KMAX + 2 * (KMAX / LB)) * 32;
     T *s_y = reinterpret_cast<T *>(s_dyn);
     const Item it = p.items[blockIdx.x];
     const SigDev sgd = p.sigs[it.sig];
@@ -925,7 +946,8 @@ __global__ void __launch_bounds__(LONG_THREADS) k_eval_blk(const EvalParams<T> p
     const bool active = b < p.ldb && b < p.B;
     T fe[1] = {T(0)};
     if (active) {
-        T *sy = s_y + (size_t)warp * KMAX * 32 + lane;
+        T *sy = s_y + (size_t)warp * PER_WARP + lane;
+        T *sb = sy + KMAX * 32;
         const int k = it.k, nc = it.c_end - it.c_begin;
         const char *xb = reinterpret_cast<const char *>(p.x + b);
         char *gb = reinterpret_cast<char *>(p.G + (b - p.g_b0));
@@ -937,12 +959,13 @@ __global__ void __launch_bounds__(LONG_THREADS) k_eval_blk(const EvalParams<T> p
                 const T v = (lit & LIT_FIXED) ? T(1) : __ldg(reinterpret_cast<const T *>(xb + (uint64_t)(uint32_t)(lit & LIT_VAR) * x_ld));
                 sy[i * 32] = flip_sign(v, lit);
             }
+            for (int i = k; i < (k + LB - 1) / LB * LB; ++i) sy[i * 32] = T(0);   // finite padding of the last block
             T g[KMAX];
 #pragma unroll
             for (int i = 0; i < KMAX; ++i) g[i] = T(0);
             const T *r = s_tab;
-            for (int q = 0; q < sgd.n_real; ++q, r += 8) long_point<T, KMAX, false, GRAD>(sy, k, r, fe[0], g);
-            for (int q = 0; q < sgd.n_cplx; ++q, r += 8) long_point<T, KMAX, true, GRAD>(sy, k, r, fe[0], g);
+            for (int q = 0; q < sgd.n_real; ++q, r += 8) long_point<T, KMAX, false, GRAD>(sy, sb, k, r, fe[0], g);
+            for (int q = 0; q < sgd.n_cplx; ++q, r += 8) long_point<T, KMAX, true, GRAD>(sy, sb, k, r, fe[0], g);
             if (GRAD) {
 #pragma unroll
                 for (int i = 0; i < KMAX; ++i) {
