@@ -130,6 +130,27 @@ def oracle_sample(inst, x0, target_s=15.0, max_b=64):
                       f"{inst.batch} candidates x 1 step over all {inst.n_cons} constraints, {dt:.2f} s"}, dt, b_o
 
 
+def rank_x0_seed(cfg, rank):
+    """Replicas only: every rank draws its own batch of candidates."""
+    from paper_2606_06641_b200 import instances as I
+    return I.SEED_X0 + cfg + 1000 * rank
+
+
+def reduce_max(values, device="cpu"):
+    """Max over ranks of a list of per-rank timings (the only cross-rank datum of the benchmark)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return t.tolist()
+
+
+def whole_job_value(world, m, B, K, seconds):
+    """evals/s of the whole job: every rank processed m*B*K evaluations in `seconds` (max over ranks)."""
+    return world * m * B * K / seconds
+
+
 def run_reference(args):
     """--impl reference: the oracle, as it stands, on the host cores (rank 0 only)."""
     rank = int(os.environ.get("RANK", "0"))
@@ -190,7 +211,7 @@ def run_ours(args):
     m, B, n = inst.n_cons, inst.batch, inst.n_vars
     dtype = args.dtype
     npdt = np.float32 if dtype == 32 else np.float64
-    x0 = I.make_x0(inst, seed=I.SEED_X0 + args.config + 1000 * rank, dtype=npdt)
+    x0 = I.make_x0(inst, seed=rank_x0_seed(args.config, rank), dtype=npdt)
     ctx = Bd.Context.from_instance(inst, dtype=dtype, device=local)
     ldb = ctx.ldb
     stream = torch.cuda.current_stream()
@@ -263,16 +284,13 @@ def run_ours(args):
     h2d = n * ldb * esz
     d2h = n * ldb * esz + B * (esz + 4 + 1 + 4)
 
-    tt = torch.tensor([t_total, t_warm, t_e2e, kern_ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    t_total, t_warm, t_e2e, kern_ms = tt.tolist()
+    t_total, t_warm, t_e2e, kern_ms = reduce_max([t_total, t_warm, t_e2e, kern_ms], device="cuda")
     if rank == 0:
         peaks = load_peaks()
         sm = ctx.query(Bd.Q_SM_COUNT)
         flop_c, instr_c = flop_model(inst)
         evals = world * m * B * K
-        value = evals / t_total
+        value = whole_job_value(world, m, B, K, t_total)
         kern_s = kern_ms * 1e-3 / max(1, kern_launches)          # avg duration of one eval launch set
         launches_per_step = max(1, kern_launches // K)
         flop_per_step = flop_c * B

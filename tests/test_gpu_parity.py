@@ -348,3 +348,90 @@ def test_config3_small_both_precisions():
     # fp32 at k = 30..50: reported, bounded loosely (<= 2e-4 per constraint at x0)
     assert np.abs(F32 - Fo).max() <= 1e-4 * inst.n_cons + 1e-2
     assert np.abs(G32 - Go).max() <= 2e-2
+
+
+# ---- candidate tiling, n_steps = 0, full-size sampled parity ----------------------------------------
+
+def test_candidate_tiling_path(monkeypatch):
+    """Force the L2 candidate tiling: tile of 64 candidates, B = 200 (4 tiles, the last
+    one ragged).  eval_grad, check and teacher-forced steps must not depend on the tiling."""
+    monkeypatch.setenv("AFSAT_TILE_W", "64")
+    inst = I.make_mixed(n=70, m=400, kmin=1, kmax=24, seed=51, batch=200, with_fixed=True)
+    B = 200
+    x0 = I.make_x0(inst, seed=15, batch=B)
+    assert_eval_parity(inst, x0, B, 32, gtol=3e-4)
+    assert_eval_parity(inst, x0, B, 64)
+    ctx = Bd.Context.from_instance(inst, batch=B, ldb=x0.shape[1])
+    x = dev(x0)
+    state = None
+    for t in range(1, 5):
+        prev = x.cpu().numpy().astype(np.float64)
+        F, sat, sol, first = ctx.step(x, 0.1, 1, step_base=t - 1, state=state)
+        state = (sol, first)
+        now = x.cpu().numpy().astype(np.float64)
+        Xo, Fo, sato, solo, firsto = O.step(inst, prev, 0.1, 1, B)
+        assert np.abs(now[:, :B] - Xo[:, :B]).max() <= 0.1 * 3e-4
+        assert np.array_equal(sat.cpu().numpy(), O.check(inst, now, B)[0])
+        assert np.all(now[:, B:] == x0[:, B:])                      # X padding untouched
+
+
+def test_step_zero_steps_counts_only():
+    inst = I.make_config(0)
+    x0 = I.make_x0(inst)
+    ctx = Bd.Context.from_instance(inst)
+    x = dev(x0)
+    F, sat, sol, first = ctx.step(x, 0.1, 0)
+    so, lo = O.check(inst, x0.astype(np.float64), inst.batch)
+    assert np.array_equal(sat.cpu().numpy(), so)
+    assert np.all(sol.cpu().numpy() == 0) and np.all(first.cpu().numpy() == -1)   # X(0) is not marked (A11)
+    assert torch.equal(x, dev(x0))
+    Fo = O.eval_grad(inst, x0.astype(np.float64), inst.batch, grad=False)
+    assert np.all(np.abs(F.cpu().numpy() - Fo) <= tol_F(inst.n_cons, Fo, 32))
+
+
+def _sampled_full_size(cfg, dtype=32, n_sample=6, gtol=1e-4, ftol_extra=0.0):
+    """Full BASELINE size, the launch configuration bench.py times; the oracle recomputes a sample of
+    candidates (first 3 + random) over ALL constraints, one by one."""
+    inst = I.make_config(cfg)
+    B = inst.batch
+    x0 = I.make_x0(inst, dtype=np.float32 if dtype == 32 else np.float64)
+    ctx = Bd.Context.from_instance(inst, dtype=dtype)
+    x = dev(x0)
+    F, G = ctx.eval_grad(x)
+    sat, sol = ctx.check(x)
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(99 + cfg)
+    cols = np.unique(np.concatenate([np.arange(3), rng.integers(0, B, size=n_sample - 3), [B - 1]]))
+    xs = np.ascontiguousarray(x0[:, cols]).astype(np.float64)
+    xs_p = np.zeros((inst.n_vars, 32), dtype=np.float64)
+    xs_p[:, :cols.size] = xs
+    Fo, Go = O.eval_grad(inst, xs_p, cols.size)
+    so, lo = O.check(inst, xs_p, cols.size)
+    Fg = F.cpu().numpy().astype(np.float64)[cols]
+    Gg = G[:, torch.from_numpy(cols).cuda()].cpu().numpy().astype(np.float64)
+    assert np.array_equal(sat.cpu().numpy()[cols], so) and np.array_equal(sol.cpu().numpy()[cols], lo)
+    assert np.all(np.abs(Fg - Fo) <= tol_F(inst.n_cons, Fo, dtype) + ftol_extra), np.abs(Fg - Fo).max()
+    err = np.abs(Gg - Go[:, :cols.size]).max()
+    assert err <= gtol, err
+    # properties that hold at any size: |FE_C| <= 1 so |F| <= m; gradient rows of fixed variables are 0
+    assert np.all(np.abs(F.cpu().numpy()) <= inst.n_cons * (1 + 1e-3))
+    if inst.fixed is not None:
+        assert torch.all(G[torch.from_numpy(np.nonzero(inst.fixed != 0)[0]).cuda()] == 0)
+    return err
+
+
+def test_full_size_cfg1_sampled():
+    # 595 occurrences per variable: a component sums ~600 partials of k = 7 (each ~1e-6): 1e-4 holds
+    _sampled_full_size(1)
+
+
+def test_full_size_cfg2_sampled():
+    _sampled_full_size(2, gtol=3e-4)
+
+
+def test_full_size_cfg3_sampled_fp64():
+    _sampled_full_size(3, dtype=64, gtol=1e-10, ftol_extra=1e-9)
+
+
+def test_full_size_cfg4_sampled():
+    _sampled_full_size(4)
