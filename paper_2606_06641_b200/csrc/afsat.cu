@@ -170,7 +170,7 @@ int launch_eval(afsat_ctx *ctx, const T *x, T *G, int64_t g_ld, int64_t g_b0, T 
     EvalParams<T> p;
     p.x = x; p.G = G; p.g_ld = g_ld; p.g_b0 = g_b0; p.Fpart = Fpart;
     p.lits = ctx->d_lits; p.sigs = ctx->d_sigs; p.rows = (const T *)ctx->d_rows;
-    p.B = ctx->B; p.ldb = ctx->ldb; p.b_begin = b_begin;
+    p.B = ctx->B; p.ldb = ctx->ldb; p.b_begin = b_begin; p.b_end = std::min<int64_t>(b_begin + width, ctx->ldb);
     const bool grad = G != nullptr;
     constexpr int VA = sizeof(T) == 4 ? AFSAT_A_V : 1;
     // The length classes are independent (they only share the RED target), so their launches run

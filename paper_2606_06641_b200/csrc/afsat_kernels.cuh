@@ -63,7 +63,7 @@ struct EvalParams {
     int32_t frow_base;          // row of Fpart for (items[0], group 0)
     int32_t B;
     int64_t ldb;
-    int64_t b_begin;            // first candidate of this launch's tile
+    int64_t b_begin, b_end;     // candidate tile of this launch (b_end <= ldb)
     int32_t Wc, Wk;             // warps of a CTA: Wc candidate sub-tiles x Wk constraint groups
 };
 
@@ -420,38 +420,6 @@ __device__ __forceinline__ void store_item_F(const EvalParams<T> &p, T (*s_F)[32
     }
 }
 
-// Register kernel for constraints of length exactly K (one kernel per length: independent register
-// allocation and scheduling); the item's signature is CTA-uniform.
-template <typename T, int K, int V, bool GRAD, int MINB>
-__global__ void __launch_bounds__(CTA_THREADS, MINB) k_eval_k(const EvalParams<T> p)
-{
-    __shared__ __align__(16) T s_tab[((K + 1) / 2 + 1) * 8];    // H = floor((K+1)/2) + 1 DFT points
-    __shared__ int32_t s_lits[LIT_CHUNK];
-    __shared__ T s_F[CTA_WARPS][32 * V];
-    const Item it = p.items[blockIdx.x];
-    const SigDev sg = p.sigs[it.sig];
-    stage_item(p, it, sg, s_tab, s_lits);
-    __syncthreads();
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int wc = warp % p.Wc, wk = warp / p.Wc;
-    const int64_t b = p.b_begin + ((int64_t)blockIdx.y * p.Wc + wc) * (32 * V) + lane * V;
-    const bool active = b < p.ldb && b < p.B;
-    T fe[V];
-#pragma unroll
-    for (int v = 0; v < V; ++v) fe[v] = T(0);
-    if (active) {
-        const int nc = it.c_end - it.c_begin;
-        if (K <= 5) {
-            if (it.has_fixed) run_item_pf<T, K, V, GRAD, true>(p, s_lits, s_tab, sg.n_real, sg.n_cplx, nc, wk, b, fe);
-            else run_item_pf<T, K, V, GRAD, false>(p, s_lits, s_tab, sg.n_real, sg.n_cplx, nc, wk, b, fe);
-        } else {
-            if (it.has_fixed) run_item_reg<T, K, V, GRAD, true>(p, s_lits, s_tab, sg.n_real, sg.n_cplx, nc, wk, b, fe);
-            else run_item_reg<T, K, V, GRAD, false>(p, s_lits, s_tab, sg.n_real, sg.n_cplx, nc, wk, b, fe);
-        }
-    }
-    store_item_F<T, V>(p, s_F, fe, warp, lane, wk, b, active);
-}
-
 // ---- packed-pair register kernel (fp32, NP pairs = 2 NP candidates per lane, FFMA2), length K --------
 template <int NP> struct PairIO;
 template <> struct PairIO<1> {
@@ -532,53 +500,6 @@ __device__ __forceinline__ void run_item_f2(const EvalParams<float> &p, const in
     }
 }
 
-template <int K, int NP, bool GRAD, int MINB>
-__global__ void __launch_bounds__(CTA_THREADS, MINB) k_eval_f2(const EvalParams<float> p)
-{
-    constexpr int H = (K + 1) / 2 + 1;                                // DFT points floor((K+1)/2) + 1
-    constexpr int V = 2 * NP;
-    __shared__ __align__(16) f32x2 s_tab2[H * ROW2];
-    __shared__ int32_t s_lits[LIT_CHUNK];
-    __shared__ float s_F[CTA_WARPS][32 * V];
-    const Item it = p.items[blockIdx.x];
-    const SigDev sg = p.sigs[it.sig];
-    for (int i = threadIdx.x; i < (sg.n_real + sg.n_cplx) * ROW2; i += blockDim.x) {
-        const int q = i / ROW2, j = i % ROW2;
-        const float *r = p.rows + ((int64_t)sg.row_off + q) * 8;
-        float v = 0.f;
-        if (q < sg.n_real) { if (j < 4) v = r[2 * j]; }               // a, b, w, wb
-        else {
-            switch (j) {
-            case 0: v = r[0]; break;  case 1: v = r[1]; break;  case 2: v = -r[1]; break;
-            case 3: v = r[2]; break;  case 4: v = r[3]; break;  case 5: v = -r[3]; break;
-            case 6: v = r[4]; break;  case 7: v = -r[5]; break; case 8: v = r[6]; break;  case 9: v = -r[7]; break;
-            default: break;
-            }
-        }
-        s_tab2[i] = pk(v, v);
-    }
-    const int nl = (it.c_end - it.c_begin) * K;
-    for (int i = threadIdx.x; i < nl; i += blockDim.x) s_lits[i] = __ldg(p.lits + it.lit_base + i);
-    __syncthreads();
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int wc = warp % p.Wc, wk = warp / p.Wc;
-    const int64_t b = p.b_begin + ((int64_t)blockIdx.y * p.Wc + wc) * (32 * V) + lane * V;
-    const bool active = b < p.ldb && b < p.B;
-    f32x2 fe2[NP];
-#pragma unroll
-    for (int q = 0; q < NP; ++q) fe2[q] = 0ull;
-    if (active) {
-        const int nc = it.c_end - it.c_begin;
-        constexpr bool PF = K <= 5;
-        if (it.has_fixed) run_item_f2<K, NP, GRAD, true, PF>(p, s_lits, s_tab2, sg.n_real, sg.n_cplx, nc, wk, b, fe2);
-        else run_item_f2<K, NP, GRAD, false, PF>(p, s_lits, s_tab2, sg.n_real, sg.n_cplx, nc, wk, b, fe2);
-    }
-    float fe[V];
-#pragma unroll
-    for (int q = 0; q < NP; ++q) upk(fe2[q], fe[2 * q], fe[2 * q + 1]);
-    store_item_F<float, V>(p, s_F, fe, warp, lane, wk, b, active);
-}
-
 // ---- one launch for a RANGE of lengths [KLO, KHI]: the CTA's item picks its length-K body, which is a
 // separately compiled (noinline) function so that every length keeps its own schedule and register
 // allocation while all lengths share one grid (no per-length launch tails) ---------------------------
@@ -590,7 +511,7 @@ __device__ __noinline__ void item_body_f2(const EvalParams<float> &p, const int3
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int wc = warp % p.Wc, wk = warp / p.Wc;
     const int64_t b = p.b_begin + ((int64_t)blockIdx.y * p.Wc + wc) * (32 * V) + lane * V;
-    const bool active = b < p.ldb && b < p.B;
+    const bool active = b < p.b_end && b < p.B;            // this launch owns [b_begin, b_end)
     f32x2 fe2[NP];
 #pragma unroll
     for (int q = 0; q < NP; ++q) fe2[q] = 0ull;
@@ -652,7 +573,7 @@ __device__ __noinline__ void item_body_k(const EvalParams<T> &p, const int32_t *
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int wc = warp % p.Wc, wk = warp / p.Wc;
     const int64_t b = p.b_begin + ((int64_t)blockIdx.y * p.Wc + wc) * (32 * V) + lane * V;
-    const bool active = b < p.ldb && b < p.B;
+    const bool active = b < p.b_end && b < p.B;            // this launch owns [b_begin, b_end)
     T fe[V];
 #pragma unroll
     for (int v = 0; v < V; ++v) fe[v] = T(0);
@@ -689,94 +610,6 @@ __global__ void __launch_bounds__(CTA_THREADS, MINB) k_eval_km(const EvalParams<
     stage_item(p, it, sg, s_tab, s_lits);
     __syncthreads();
     SwitchK<T, KLO, KHI, V, GRAD>::go(it.k, p, s_lits, s_tab, s_F, sg.n_real, sg.n_cplx, it.c_end - it.c_begin, it.has_fixed != 0);
-}
-
-// ---- generic kernel for long constraints (runtime k <= 64), V = 1: literal values, prefix products
-// and partial gradients staged in shared memory as [i][lane] columns (conflict-free), suffix
-// running in registers ------------------------------------------------------------------------------
-template <typename T, bool GRAD>
-__global__ void __launch_bounds__(CTA_THREADS) k_eval_long(const EvalParams<T> p, int kmax)
-{
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    T *s_tab = reinterpret_cast<T *>(smem_raw);                       // [MAX_ROWS * 8]
-    int32_t *s_lits = reinterpret_cast<int32_t *>(s_tab + MAX_ROWS * 8);   // [LIT_CHUNK]
-    T *s_F = reinterpret_cast<T *>(s_lits + LIT_CHUNK);                // [CTA_WARPS][32]
-    T *s_work = s_F + CTA_WARPS * 32;                                  // [warps][4][kmax][32]
-    const Item it = p.items[blockIdx.x];
-    const SigDev sgd = p.sigs[it.sig];
-    stage_item(p, it, sgd, s_tab, s_lits);
-    __syncthreads();
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int wc = warp % p.Wc, wk = warp / p.Wc;
-    const int64_t b = p.b_begin + ((int64_t)blockIdx.y * p.Wc + wc) * 32 + lane;
-    const bool active = b < p.ldb && b < p.B;
-    T fe_acc[1] = {T(0)};
-    if (active) {
-        T *sy = s_work + (size_t)warp * 4 * kmax * 32 + lane;
-        T *spr = sy + (size_t)kmax * 32, *spi = spr + (size_t)kmax * 32, *sg = spi + (size_t)kmax * 32;
-        const int k = it.k, nc = it.c_end - it.c_begin;
-        for (int c = wk; c < nc; c += p.Wk) {
-            const int32_t *L = s_lits + c * k;
-            for (int i = 0; i < k; ++i) {
-                const int32_t lit = L[i];
-                T v = (lit & LIT_FIXED) ? T(1) : __ldg(p.x + (int64_t)(lit & LIT_VAR) * p.ldb + b);
-                sy[i * 32] = (lit < 0) ? -v : v;
-                sg[i * 32] = T(0);
-            }
-            const T *r = s_tab;
-            for (int q = 0; q < sgd.n_real; ++q, r += 8) {
-                const T a = r[0], bb = r[2], w = r[4], wb = r[6];
-                T run = T(1);
-                for (int i = 0; i < k; ++i) { spr[i * 32] = run; run *= fma_(bb, sy[i * 32], a); }
-                fe_acc[0] = fma_(w, run, fe_acc[0]);
-                if (GRAD) {
-                    T suf = wb;
-                    for (int i = k - 1; i >= 0; --i) {
-                        sg[i * 32] = fma_(spr[i * 32], suf, sg[i * 32]);
-                        suf *= fma_(bb, sy[i * 32], a);
-                    }
-                }
-            }
-            for (int q = 0; q < sgd.n_cplx; ++q, r += 8) {
-                const T ar = r[0], ai = r[1], br = r[2], bi = r[3], wr = r[4], wi = r[5];
-                T rr = T(1), ri = T(0);
-                for (int i = 0; i < k; ++i) {
-                    const T yi = sy[i * 32];
-                    const T f_r = fma_(br, yi, ar), f_i = fma_(bi, yi, ai);
-                    spr[i * 32] = rr; spi[i * 32] = ri;
-                    const T nr = fma_(rr, f_r, -(ri * f_i));
-                    const T ni = fma_(rr, f_i, ri * f_r);
-                    rr = nr; ri = ni;
-                }
-                fe_acc[0] = fma_(wr, rr, fe_acc[0]);
-                fe_acc[0] = fma_(-wi, ri, fe_acc[0]);
-                if (GRAD) {
-                    T sr = r[6], si = r[7];
-                    for (int i = k - 1; i >= 0; --i) {
-                        const T yi = sy[i * 32];
-                        T gi = sg[i * 32];
-                        gi = fma_(spr[i * 32], sr, gi);
-                        gi = fma_(-spi[i * 32], si, gi);
-                        sg[i * 32] = gi;
-                        const T f_r = fma_(br, yi, ar), f_i = fma_(bi, yi, ai);
-                        const T nr = fma_(sr, f_r, -(si * f_i));
-                        const T ni = fma_(sr, f_i, si * f_r);
-                        sr = nr; si = ni;
-                    }
-                }
-            }
-            if (GRAD) {
-                for (int i = 0; i < k; ++i) {
-                    const int32_t lit = L[i];
-                    if (!(lit & LIT_FIXED)) {
-                        const T gi = sg[i * 32];
-                        atomicAdd(p.G + (int64_t)(lit & LIT_VAR) * p.g_ld + (b - p.g_b0), (lit < 0) ? -gi : gi);
-                    }
-                }
-            }
-        }
-    }
-    store_item_F<T, 1>(p, reinterpret_cast<T(*)[32]>(s_F), fe_acc, warp, lane, wk, b, active);
 }
 
 // ---- register-blocked kernel for long constraints (16 < k <= KMAX <= 64), one candidate per lane ------
@@ -943,7 +776,7 @@ __global__ void __launch_bounds__(LONG_THREADS) k_eval_blk(const EvalParams<T> p
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int wc = warp % p.Wc, wk = warp / p.Wc;
     const int64_t b = p.b_begin + ((int64_t)blockIdx.y * p.Wc + wc) * 32 + lane;
-    const bool active = b < p.ldb && b < p.B;
+    const bool active = b < p.b_end && b < p.B;            // this launch owns [b_begin, b_end)
     T fe[1] = {T(0)};
     if (active) {
         T *sy = s_y + (size_t)warp * PER_WARP + lane;

@@ -356,7 +356,7 @@ def test_candidate_tiling_path(monkeypatch):
     """Force the L2 candidate tiling: tile of 64 candidates, B = 200 (4 tiles, the last
     one ragged).  eval_grad, check and teacher-forced steps must not depend on the tiling."""
     monkeypatch.setenv("AFSAT_TILE_W", "64")
-    inst = I.make_mixed(n=70, m=400, kmin=1, kmax=24, seed=51, batch=200, with_fixed=True)
+    inst = I.make_mixed(n=70, m=400, kmin=1, kmax=18, seed=51, batch=200, with_fixed=True)
     B = 200
     x0 = I.make_x0(inst, seed=15, batch=B)
     assert_eval_parity(inst, x0, B, 32, gtol=3e-4)
