@@ -41,6 +41,16 @@ def load_peaks():
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "source": "fallback"}
 
 
+def load_traffic(cfg):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu capture (profiles/), or None."""
+    p = os.path.join(ROOT, "profiles", "r1_traffic.json")
+    try:
+        with open(p) as f:
+            return json.load(f).get(f"cfg{cfg}", {}).get("bytes_per_launch")
+    except (OSError, ValueError):
+        return None
+
+
 def flop_model(inst):
     """Algorithmic work per candidate over all constraints:
     flop = k(19 C + 6 R) + 4 C + 2 R, FP32 instr = k(12 C + 4 R) + 2 C + R with R = 1 + [k odd]
@@ -304,7 +314,7 @@ def run_ours(args):
                 if kern_ms > 0 else 0.0,
                 "kernel_ms_per_step": kern_ms / K, "kernel_launches_per_step": launches_per_step,
                 "kernel_share_of_step": (kern_ms / K) / (1e3 * t_total / K),
-                "algorithmic_flop_per_step": flop_per_step, "traffic": None,
+                "algorithmic_flop_per_step": flop_per_step, "traffic": load_traffic(args.config),
                 "hbm_floor_bytes_per_step": 2 * n * B * esz, "hbm_peak_gbs": peaks["hbm_gbs"]}
         if clocks.get("sm_mhz"):
             roof["frac_at_observed_clock"] = roof["frac"] * peaks["sm_max_mhz"] / clocks["sm_mhz"]
