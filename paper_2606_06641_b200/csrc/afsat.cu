@@ -310,8 +310,11 @@ int step_t(afsat_ctx *ctx, T *x, double eta, int n_steps, int step_base, int res
                                                               ctx->n, B, ctx->ldb, b0, b0 + w, ucols);
             ++ctx->launches;
             CU(cudaPeekAtLastError());
-            // a8: exact count on X(t)
-            rc = launch_check_bits(ctx, b0 / 32, (b0 + w) / 32, st);
+        }
+        // a8: exact count on X(t), ONE launch over the whole batch: every constraint reads the full
+        // [ldb/32]-word bit rows of its variables (coalesced), 1 bit per literal and candidate
+        {
+            int rc = launch_check_bits(ctx, 0, ctx->ldb / 32, st);
             if (rc) return rc;
         }
         k_flags<<<gb, tb, 0, st>>>(ctx->d_satacc, B, ctx->m, 1, step_base + t, sat, sol, first, ctx->d_any, h_any_dev);
@@ -486,7 +489,7 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
     const size_t esz = dtype == 32 ? 4 : 8;
     int64_t tile_w = ldb;
     {
-        int64_t budget = (int64_t)48 << 20;                            // bytes of L2 for the X and G tiles
+        int64_t budget = (int64_t)104 << 20;                           // bytes of L2 for the X and G tiles (126 MB L2)
         if (const char *e = getenv("AFSAT_L2_TILE_BYTES")) { long long v = atoll(e); if (v > 0) budget = v; }
         const int64_t per_col = (int64_t)2 * n_vars * (int64_t)esz;
         if (per_col * ldb > budget) tile_w = std::max<int64_t>(64, budget / per_col / 64 * 64);
