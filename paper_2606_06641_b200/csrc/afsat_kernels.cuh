@@ -193,6 +193,13 @@ __device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b)
 {
     f32x2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d;
 }
+// pair (c, c) from entry j of a packed table, read as ONE scalar so that the compiler can use the
+// broadcast operand form
+__device__ __forceinline__ f32x2 bc(const f32x2 *tab, int j)
+{
+    const float c = reinterpret_cast<const float *>(tab)[2 * j];
+    return pk(c, c);
+}
 __device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b)
 {
     f32x2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d;
@@ -205,13 +212,92 @@ __device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b)
 // walk carries the suffix as (Re s, -Im s).
 constexpr int ROW2 = 12;
 
+#ifndef AFSAT_F2_PAIR_POINTS
+#define AFSAT_F2_PAIR_POINTS 0
+#endif
+#ifndef AFSAT_F2_NEG_BY_XOR
+#define AFSAT_F2_NEG_BY_XOR 1
+#endif
+
+// PP complex DFT points (consecutive table rows) for NP candidate pairs: prefix walk, contraction,
+// suffix walk with the leave-one-out accumulation.  All PP x NP chains are independent.
+template <int K, int NP, int PP, bool GRAD>
+__device__ __forceinline__ void cplx_points_f2(const f32x2 (&y)[K][NP], const f32x2 *__restrict__ r, f32x2 (&fe)[NP],
+                                               f32x2 (&g)[K][NP])
+{
+    f32x2 pr[PP][K][NP], pi[PP][K][NP], fr[PP][K][NP], fi[PP][K][NP], nfi[PP][K][NP], rr[PP][NP], ri[PP][NP];
+#pragma unroll
+    for (int t = 0; t < PP; ++t) {
+        const f32x2 *rt = r + t * ROW2;
+        // coefficients are the same for both candidates: read ONE float and let FFMA2 broadcast it
+        // (R.F32 operand) -- a true register pair would cost a third 64-bit register-file read
+        const f32x2 ar = bc(rt, 0), ai = bc(rt, 1), nai = bc(rt, 2), br = bc(rt, 3), bi = bc(rt, 4), nbi = bc(rt, 5);
+#pragma unroll
+        for (int i = 0; i < K; ++i)
+#pragma unroll
+            for (int q = 0; q < NP; ++q) {
+                fr[t][i][q] = fma2(br, y[i][q], ar); fi[t][i][q] = fma2(bi, y[i][q], ai);
+#if AFSAT_F2_NEG_BY_XOR
+                nfi[t][i][q] = fi[t][i][q] ^ 0x8000000080000000ull;   // -Im f on the ALU pipe (2 LOP3), not the FMA pipe
+#else
+                nfi[t][i][q] = fma2(nbi, y[i][q], nai);
+#endif
+            }
+    }
+#pragma unroll
+    for (int t = 0; t < PP; ++t)
+#pragma unroll
+        for (int q = 0; q < NP; ++q) { rr[t][q] = fr[t][0][q]; ri[t][q] = fi[t][0][q]; }
+#pragma unroll
+    for (int i = 1; i < K; ++i)
+#pragma unroll
+        for (int t = 0; t < PP; ++t)
+#pragma unroll
+            for (int q = 0; q < NP; ++q) {
+                pr[t][i][q] = rr[t][q]; pi[t][i][q] = ri[t][q];
+                const f32x2 nr = fma2(rr[t][q], fr[t][i][q], mul2(ri[t][q], nfi[t][i][q]));   // Re: rr fr - ri fi
+                const f32x2 ni = fma2(rr[t][q], fi[t][i][q], mul2(ri[t][q], fr[t][i][q]));    // Im: rr fi + ri fr
+                rr[t][q] = nr; ri[t][q] = ni;
+            }
+#pragma unroll
+    for (int t = 0; t < PP; ++t)
+#pragma unroll
+        for (int q = 0; q < NP; ++q) {
+            fe[q] = fma2(bc(r, t * ROW2 + 6), rr[t][q], fe[q]);       // + wr Re P
+            fe[q] = fma2(bc(r, t * ROW2 + 7), ri[t][q], fe[q]);       // - wi Im P
+        }
+    if (GRAD) {
+        f32x2 sr[PP][NP], nsi[PP][NP];                                // suffix (Re s, -Im s) seeded with w b
+#pragma unroll
+        for (int t = 0; t < PP; ++t)
+#pragma unroll
+            for (int q = 0; q < NP; ++q) { sr[t][q] = r[t * ROW2 + 8]; nsi[t][q] = r[t * ROW2 + 9]; }
+#pragma unroll
+        for (int i = K - 1; i >= 1; --i)
+#pragma unroll
+            for (int t = 0; t < PP; ++t)
+#pragma unroll
+                for (int q = 0; q < NP; ++q) {
+                    g[i][q] = fma2(pr[t][i][q], sr[t][q], g[i][q]);   // Re(pre * suf) = pr sr - pi si
+                    g[i][q] = fma2(pi[t][i][q], nsi[t][q], g[i][q]);
+                    const f32x2 t_r = fma2(nsi[t][q], fi[t][i][q], mul2(sr[t][q], fr[t][i][q]));    // Re: sr fr - si fi
+                    const f32x2 t_n = fma2(nsi[t][q], fr[t][i][q], mul2(sr[t][q], nfi[t][i][q]));   // -Im: -(sr fi + si fr)
+                    sr[t][q] = t_r; nsi[t][q] = t_n;
+                }
+#pragma unroll
+        for (int t = 0; t < PP; ++t)
+#pragma unroll
+            for (int q = 0; q < NP; ++q) g[0][q] = add2(g[0][q], sr[t][q]);       // prefix_0 = 1
+    }
+}
+
 template <int K, int NP, bool GRAD>
 __device__ __forceinline__ void eval_points_f2(const f32x2 (&y)[K][NP], const f32x2 *__restrict__ tab, int n_real,
                                                int n_cplx, f32x2 (&fe)[NP], f32x2 (&g)[K][NP])
 {
     const f32x2 *r = tab;
     for (int p = 0; p < n_real; ++p, r += ROW2) {                    // self-conjugate points
-        const f32x2 a = r[0], b = r[1], w = r[2], wb = r[3];
+        const f32x2 a = bc(r, 0), b = bc(r, 1), w = bc(r, 2), wb = bc(r, 3);
         f32x2 pre[K][NP], f[K][NP], run[NP], suf[NP];
 #pragma unroll
         for (int i = 0; i < K; ++i)
@@ -236,49 +322,11 @@ __device__ __forceinline__ void eval_points_f2(const f32x2 (&y)[K][NP], const f3
             for (int q = 0; q < NP; ++q) g[0][q] = add2(g[0][q], suf[q]);     // prefix_0 = 1
         }
     }
-    for (int p = 0; p < n_cplx; ++p, r += ROW2) {                    // one of each conjugate pair
-        const f32x2 ar = r[0], ai = r[1], nai = r[2], br = r[3], bi = r[4], nbi = r[5];
-        f32x2 pr[K][NP], pi[K][NP], fr[K][NP], fi[K][NP], nfi[K][NP], rr[NP], ri[NP];
-#pragma unroll
-        for (int i = 0; i < K; ++i)
-#pragma unroll
-            for (int q = 0; q < NP; ++q) {
-                fr[i][q] = fma2(br, y[i][q], ar); fi[i][q] = fma2(bi, y[i][q], ai); nfi[i][q] = fma2(nbi, y[i][q], nai);
-            }
-#pragma unroll
-        for (int q = 0; q < NP; ++q) { rr[q] = fr[0][q]; ri[q] = fi[0][q]; }
-#pragma unroll
-        for (int i = 1; i < K; ++i)
-#pragma unroll
-            for (int q = 0; q < NP; ++q) {
-                pr[i][q] = rr[q]; pi[i][q] = ri[q];
-                const f32x2 nr = fma2(rr[q], fr[i][q], mul2(ri[q], nfi[i][q]));   // Re: rr fr - ri fi
-                const f32x2 ni = fma2(rr[q], fi[i][q], mul2(ri[q], fr[i][q]));    // Im: rr fi + ri fr
-                rr[q] = nr; ri[q] = ni;
-            }
-#pragma unroll
-        for (int q = 0; q < NP; ++q) {
-            fe[q] = fma2(r[6], rr[q], fe[q]);                         // + wr Re P
-            fe[q] = fma2(r[7], ri[q], fe[q]);                         // - wi Im P
-        }
-        if (GRAD) {
-            f32x2 sr[NP], nsi[NP];                                    // suffix (Re s, -Im s) seeded with w b
-#pragma unroll
-            for (int q = 0; q < NP; ++q) { sr[q] = r[8]; nsi[q] = r[9]; }
-#pragma unroll
-            for (int i = K - 1; i >= 1; --i)
-#pragma unroll
-                for (int q = 0; q < NP; ++q) {
-                    g[i][q] = fma2(pr[i][q], sr[q], g[i][q]);         // Re(pre * suf) = pr sr - pi si
-                    g[i][q] = fma2(pi[i][q], nsi[q], g[i][q]);
-                    const f32x2 t_r = fma2(nsi[q], fi[i][q], mul2(sr[q], fr[i][q]));    // Re: sr fr - si fi
-                    const f32x2 t_n = fma2(nsi[q], fr[i][q], mul2(sr[q], nfi[i][q]));   // -Im: -(sr fi + si fr)
-                    sr[q] = t_r; nsi[q] = t_n;
-                }
-#pragma unroll
-            for (int q = 0; q < NP; ++q) g[0][q] = add2(g[0][q], sr[q]);          // prefix_0 = 1
-        }
+    int p = 0;
+    if (AFSAT_F2_PAIR_POINTS) {                                       // two conjugate-pair points per pass: 2 x the independent chains
+        for (; p + 1 < n_cplx; p += 2, r += 2 * ROW2) cplx_points_f2<K, NP, 2, GRAD>(y, r, fe, g);
     }
+    for (; p < n_cplx; ++p, r += ROW2) cplx_points_f2<K, NP, 1, GRAD>(y, r, fe, g);
 }
 
 // sign flip by the literal's polarity bit (bit 31 of the packed literal): one LOP3 per value
