@@ -162,6 +162,27 @@ void (*pick_a(bool grad))(EvalParams<T>)
         return grad ? (Fn)k_eval_km<T, 1, 8, VA, true, MB> : (Fn)k_eval_km<T, 1, 8, VA, false, MB>;
 }
 
+// k > 16: KMAX is the unroll bound of the register-blocked kernels; fp32 runs the packed two-candidate form
+inline int long_kmax(int kmax_long) { return kmax_long <= 32 ? 32 : kmax_long <= 40 ? 40 : kmax_long <= 48 ? 48 : kmax_long <= 56 ? 56 : 64; }
+#ifndef AFSAT_LONG_PACKED
+#define AFSAT_LONG_PACKED 1
+#endif
+template <typename T>
+void (*pick_long(int km, bool grad))(EvalParams<T>)
+{
+    using Fn = void (*)(EvalParams<T>);
+#define AFSAT_LONG_CASE(KM_)                                                                                  \
+    case KM_:                                                                                                 \
+        if constexpr (sizeof(T) == 4 && AFSAT_LONG_PACKED) return grad ? (Fn)k_eval_blk2<KM_, true> : (Fn)k_eval_blk2<KM_, false>; \
+        else return grad ? (Fn)k_eval_blk<T, KM_, true> : (Fn)k_eval_blk<T, KM_, false>;
+    switch (km) {
+        AFSAT_LONG_CASE(32) AFSAT_LONG_CASE(40) AFSAT_LONG_CASE(48) AFSAT_LONG_CASE(56)
+    default:
+        AFSAT_LONG_CASE(64)
+    }
+#undef AFSAT_LONG_CASE
+}
+
 // ---- launch of the evaluation kernels (a1-a5) for the candidate tile [b_begin, b_begin + width) ----
 template <typename T>
 int launch_eval(afsat_ctx *ctx, const T *x, T *G, int64_t g_ld, int64_t g_b0, T *Fpart, int64_t b_begin, int64_t width,
@@ -206,11 +227,7 @@ int launch_eval(afsat_ctx *ctx, const T *x, T *G, int64_t g_ld, int64_t g_b0, T 
             fn<<<grid, block, 0, st>>>(p);
         } else {
             using Fn = void (*)(EvalParams<T>);
-            Fn fn;
-            const int km = ctx->kmax_long <= 32 ? 32 : ctx->kmax_long <= 48 ? 48 : 64;
-            if (km == 32) fn = grad ? (Fn)k_eval_blk<T, 32, true> : (Fn)k_eval_blk<T, 32, false>;
-            else if (km == 48) fn = grad ? (Fn)k_eval_blk<T, 48, true> : (Fn)k_eval_blk<T, 48, false>;
-            else fn = grad ? (Fn)k_eval_blk<T, 64, true> : (Fn)k_eval_blk<T, 64, false>;
+            Fn fn = pick_long<T>(long_kmax(ctx->kmax_long), grad);
             CU(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem));
             fn<<<grid, block, g.smem, st>>>(p);
         }
@@ -507,9 +524,14 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
         g.V = (cls == CLS_A && dtype == 32) ? AFSAT_A_V : 1;
         g.warps = CTA_WARPS;
         if (cls == CLS_LONG) {
-            const int km = kmax_long <= 32 ? 32 : kmax_long <= 48 ? 48 : 64;
+            const int km = long_kmax(kmax_long);
             g.warps = LONG_THREADS / 32;
-            g.smem = (size_t)g.warps * (km + 2 * (km / LB)) * 32 * esz; // per warp: values [KMAX][32] + boundaries [2 KMAX/LB][32]
+            if (dtype == 32 && AFSAT_LONG_PACKED) {
+                g.V = 2;
+                g.smem = (size_t)g.warps * (km + 2 * (km / LB2)) * 32 * 8;  // per warp: value pairs [KMAX][32] + boundary pairs [2 KMAX/LB2][32]
+            } else {
+                g.smem = (size_t)g.warps * (km + 2 * (km / LB)) * 32 * esz; // per warp: values [KMAX][32] + boundaries [2 KMAX/LB][32]
+            }
         }
         const int64_t cw = 32 * g.V;
         g.Wc = std::min(g.warps, pow2_floor(std::max<int64_t>(1, (tile_w + cw - 1) / cw)));

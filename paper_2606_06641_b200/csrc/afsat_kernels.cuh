@@ -862,6 +862,171 @@ __global__ void __launch_bounds__(LONG_THREADS) k_eval_blk(const EvalParams<T> p
     store_item_F<T, 1>(p, s_F, fe, warp, lane, wk, b, active);
 }
 
+// ---- the same register-blocked scheme with TWO candidates per lane in packed f32x2 arithmetic (fp32) ----
+// A 3-pair-operand FFMA2 costs ~3 pipe cycles (register-file read bandwidth, profiles/r1_notes.md), so the
+// packed form tops out near 65 % of the FP32 peak -- but it halves the instruction count and is free of
+// the register-bank dispatch stalls that hold the scalar long kernel near 36 %.
+constexpr int LB2 = 4;
+constexpr f32x2 NEG2 = 0x8000000080000000ull;
+
+template <bool CPLX, int NU>
+struct BlkOps2 {
+    static __device__ __forceinline__ void fwd(const f32x2 *__restrict__ sy, f32x2 ar, f32x2 ai, f32x2 br, f32x2 bi, f32x2 &rr,
+                                               f32x2 &ri)
+    {
+#pragma unroll
+        for (int u = 0; u < NU; ++u) {
+            const f32x2 yv = sy[u * 32];
+            const f32x2 fr = fma2(br, yv, ar);
+            if (CPLX) {
+                const f32x2 fi = fma2(bi, yv, ai);
+                const f32x2 nr = fma2(rr, fr, mul2(ri, fi ^ NEG2));
+                const f32x2 ni = fma2(rr, fi, mul2(ri, fr));
+                rr = nr; ri = ni;
+            } else {
+                rr = mul2(rr, fr);
+            }
+        }
+    }
+    // nu <= NU literals are live (nu == NU for a full block); suffix carried as (Re s, -Im s)
+    static __device__ __forceinline__ void bwd(int nu, const f32x2 *__restrict__ sy, f32x2 ar, f32x2 ai, f32x2 br, f32x2 bi,
+                                               f32x2 pr0, f32x2 pi0, f32x2 &sr, f32x2 &nsi, f32x2 *__restrict__ g)
+    {
+        f32x2 fr[NU], fi[CPLX ? NU : 1], pr[NU], pi[CPLX ? NU : 1];
+#pragma unroll
+        for (int u = 0; u < NU; ++u) {
+            const f32x2 yv = sy[u * 32];
+            fr[u] = fma2(br, yv, ar);
+            if (CPLX) fi[u] = fma2(bi, yv, ai);
+        }
+        pr[0] = pr0;
+        if (CPLX) pi[0] = pi0;
+#pragma unroll
+        for (int u = 1; u < NU; ++u) {
+            if (CPLX) {
+                pr[u] = fma2(pr[u - 1], fr[u - 1], mul2(pi[u - 1], fi[u - 1] ^ NEG2));
+                pi[u] = fma2(pr[u - 1], fi[u - 1], mul2(pi[u - 1], fr[u - 1]));
+            } else {
+                pr[u] = mul2(pr[u - 1], fr[u - 1]);
+            }
+        }
+#pragma unroll
+        for (int u = NU - 1; u >= 0; --u) {
+            if (u < nu) {                                             // warp-uniform; always true for a full block
+                if (CPLX) {
+                    g[u] = fma2(pr[u], sr, g[u]);                     // Re(pre suf) = pr sr - pi si
+                    g[u] = fma2(pi[u], nsi, g[u]);
+                    const f32x2 t_r = fma2(nsi, fi[u], mul2(sr, fr[u]));              // Re: sr fr - si fi
+                    const f32x2 t_n = fma2(nsi, fr[u], mul2(sr, fi[u] ^ NEG2));       // -Im: -(sr fi + si fr)
+                    sr = t_r; nsi = t_n;
+                } else {
+                    g[u] = fma2(pr[u], sr, g[u]);
+                    sr = mul2(sr, fr[u]);
+                }
+            }
+        }
+    }
+};
+
+template <int KMAX, bool CPLX, bool GRAD>
+__device__ __forceinline__ void long_point2(const f32x2 *__restrict__ sy, f32x2 *__restrict__ sb, int k, const float *__restrict__ r,
+                                            f32x2 &fe, f32x2 (&g)[KMAX])
+{
+    constexpr int NBLK = KMAX / LB2;
+    const f32x2 ar = pk(r[0], r[0]), ai = pk(r[1], r[1]), br = pk(r[2], r[2]), bi = pk(r[3], r[3]);
+    f32x2 rr = pk(1.f, 1.f), ri = 0ull;
+    const int nfull = k / LB2, tail = k % LB2;
+    for (int blk = 0; blk < nfull; ++blk) {                           // forward: runtime loop, one body
+        sb[(2 * blk) * 32] = rr;
+        if (CPLX) sb[(2 * blk + 1) * 32] = ri;
+        BlkOps2<CPLX, LB2>::fwd(sy + blk * LB2 * 32, ar, ai, br, bi, rr, ri);
+    }
+    if (tail) {
+        sb[(2 * nfull) * 32] = rr;
+        if (CPLX) sb[(2 * nfull + 1) * 32] = ri;
+        for (int u = 0; u < tail; ++u) BlkOps2<CPLX, 1>::fwd(sy + (nfull * LB2 + u) * 32, ar, ai, br, bi, rr, ri);
+    }
+    fe = fma2(pk(r[4], r[4]), rr, fe);
+    if (CPLX) fe = fma2(pk(-r[5], -r[5]), ri, fe);
+    if (GRAD) {
+        f32x2 sr = pk(r[6], r[6]), nsi = CPLX ? pk(-r[7], -r[7]) : 0ull;   // suffix (Re, -Im) seeded with w b
+#pragma unroll
+        for (int blk = NBLK - 1; blk >= 0; --blk) {                    // backward: unrolled, g in registers
+            if (blk < nfull)
+                BlkOps2<CPLX, LB2>::bwd(LB2, sy + blk * LB2 * 32, ar, ai, br, bi, sb[(2 * blk) * 32],
+                                        CPLX ? sb[(2 * blk + 1) * 32] : 0ull, sr, nsi, &g[blk * LB2]);
+            else if (blk == nfull && tail)
+                BlkOps2<CPLX, LB2>::bwd(tail, sy + blk * LB2 * 32, ar, ai, br, bi, sb[(2 * blk) * 32],
+                                        CPLX ? sb[(2 * blk + 1) * 32] : 0ull, sr, nsi, &g[blk * LB2]);
+        }
+    }
+}
+
+template <int KMAX, bool GRAD>
+__global__ void __launch_bounds__(LONG_THREADS) k_eval_blk2(const EvalParams<float> p)
+{
+    constexpr int NW = LONG_THREADS / 32;
+    __shared__ __align__(16) float s_tab[MAX_ROWS * 8];
+    __shared__ int32_t s_lits[LONG_LIT_CHUNK];
+    __shared__ float s_F[NW][64];
+    extern __shared__ __align__(16) unsigned char s_dyn[];               // per warp: values [KMAX][32] pairs, boundaries [2 NBLK][32] pairs
+    constexpr int PER_WARP = (KMAX + 2 * (KMAX / LB2)) * 32;
+    f32x2 *s_y = reinterpret_cast<f32x2 *>(s_dyn);
+    const Item it = p.items[blockIdx.x];
+    const SigDev sgd = p.sigs[it.sig];
+    stage_item(p, it, sgd, s_tab, s_lits);
+    __syncthreads();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int wc = warp % p.Wc, wk = warp / p.Wc;
+    const int64_t b = p.b_begin + ((int64_t)blockIdx.y * p.Wc + wc) * 64 + lane * 2;
+    const bool active = b < p.b_end && b < p.B;            // this launch owns [b_begin, b_end)
+    f32x2 fe2 = 0ull;
+    if (active) {
+        f32x2 *sy = s_y + (size_t)warp * PER_WARP + lane;
+        f32x2 *sb = sy + KMAX * 32;
+        const int k = it.k, nc = it.c_end - it.c_begin;
+        const char *xb = reinterpret_cast<const char *>(p.x + b);
+        char *gb = reinterpret_cast<char *>(p.G + (b - p.g_b0));
+        const uint32_t x_ld = (uint32_t)(p.ldb * 4), g_ld = (uint32_t)(p.g_ld * 4);
+        for (int c = wk; c < nc; c += p.Wk) {
+            const int32_t *L = s_lits + c * k;
+            for (int i = 0; i < k; ++i) {                               // a1: gather, sign, stage
+                const int32_t lit = L[i];
+                const f32x2 v = (lit & LIT_FIXED) ? pk(1.f, 1.f)
+                                                  : __ldg(reinterpret_cast<const f32x2 *>(xb + (uint64_t)(uint32_t)(lit & LIT_VAR) * x_ld));
+                const uint32_t m = (uint32_t)(lit & LIT_NEG);
+                sy[i * 32] = v ^ (((f32x2)m << 32) | m);
+            }
+            for (int i = k; i < (k + LB2 - 1) / LB2 * LB2; ++i) sy[i * 32] = 0ull;   // finite padding of the last block
+            f32x2 g[KMAX];
+#pragma unroll
+            for (int i = 0; i < KMAX; ++i) g[i] = 0ull;
+            const float *r = s_tab;
+            for (int q = 0; q < sgd.n_real; ++q, r += 8) long_point2<KMAX, false, GRAD>(sy, sb, k, r, fe2, g);
+            for (int q = 0; q < sgd.n_cplx; ++q, r += 8) long_point2<KMAX, true, GRAD>(sy, sb, k, r, fe2, g);
+            if (GRAD) {
+#pragma unroll
+                for (int i = 0; i < KMAX; ++i) {
+                    if (i < k) {                                        // warp-uniform
+                        const int32_t lit = L[i];
+                        if (!(lit & LIT_FIXED)) {
+                            const uint32_t m = (uint32_t)(lit & LIT_NEG);
+                            float g0, g1;
+                            upk(g[i] ^ (((f32x2)m << 32) | m), g0, g1);
+                            asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(gb + (uint64_t)(uint32_t)(lit & LIT_VAR) * g_ld),
+                                         "f"(g0), "f"(g1)
+                                         : "memory");
+                        }
+                    }
+                }
+            }
+        }
+    }
+    float fe[2];
+    upk(fe2, fe[0], fe[1]);
+    store_item_F<float, 2>(p, s_F, fe, warp, lane, wk, b, active);
+}
+
 // ---- a7: sign rounding as one bit per (variable, candidate): bits[v][b / 32] bit (b % 32) = (x < 0)
 template <typename T>
 __global__ void __launch_bounds__(CTA_THREADS) k_pack_signs(const T *__restrict__ x, uint32_t *__restrict__ bits, int n,
