@@ -528,7 +528,7 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
             g.warps = LONG_THREADS / 32;
             if (dtype == 32 && AFSAT_LONG_PACKED) {
                 g.V = 2;
-                g.smem = (size_t)g.warps * (km + 2 * (km / LB2)) * 32 * 8;  // per warp: value pairs [KMAX][32] + boundary pairs [2 KMAX/LB2][32]
+                g.smem = (size_t)g.warps * (km + 2 * long_pp(km) * (km / LB2)) * 32 * 8;  // per warp: value pairs [KMAX][32] + boundary pairs
             } else {
                 g.smem = (size_t)g.warps * (km + 2 * (km / LB)) * 32 * esz; // per warp: values [KMAX][32] + boundaries [2 KMAX/LB][32]
             }

@@ -869,95 +869,130 @@ __global__ void __launch_bounds__(LONG_THREADS) k_eval_blk(const EvalParams<T> p
 constexpr int LB2 = 4;
 constexpr f32x2 NEG2 = 0x8000000080000000ull;
 
-template <bool CPLX, int NU>
+// DFT points evaluated at once by the packed long kernel: 2 while the boundary storage of two points
+// still leaves room for 3 CTAs per SM (KMAX <= 32), else 1
+__host__ __device__ constexpr int long_pp(int kmax) { return kmax <= 32 ? 2 : 1; }
+
+// PP DFT points at once (independent chains interleaved for instruction-level parallelism)
+template <bool CPLX, int NU, int PP>
 struct BlkOps2 {
-    static __device__ __forceinline__ void fwd(const f32x2 *__restrict__ sy, f32x2 ar, f32x2 ai, f32x2 br, f32x2 bi, f32x2 &rr,
-                                               f32x2 &ri)
+    static __device__ __forceinline__ void fwd(const f32x2 *__restrict__ sy, const f32x2 (&ar)[PP], const f32x2 (&ai)[PP],
+                                               const f32x2 (&br)[PP], const f32x2 (&bi)[PP], f32x2 (&rr)[PP], f32x2 (&ri)[PP])
     {
 #pragma unroll
         for (int u = 0; u < NU; ++u) {
             const f32x2 yv = sy[u * 32];
-            const f32x2 fr = fma2(br, yv, ar);
-            if (CPLX) {
-                const f32x2 fi = fma2(bi, yv, ai);
-                const f32x2 nr = fma2(rr, fr, mul2(ri, fi ^ NEG2));
-                const f32x2 ni = fma2(rr, fi, mul2(ri, fr));
-                rr = nr; ri = ni;
-            } else {
-                rr = mul2(rr, fr);
+#pragma unroll
+            for (int t = 0; t < PP; ++t) {
+                const f32x2 fr = fma2(br[t], yv, ar[t]);
+                if (CPLX) {
+                    const f32x2 fi = fma2(bi[t], yv, ai[t]);
+                    const f32x2 nr = fma2(rr[t], fr, mul2(ri[t], fi ^ NEG2));
+                    const f32x2 ni = fma2(rr[t], fi, mul2(ri[t], fr));
+                    rr[t] = nr; ri[t] = ni;
+                } else {
+                    rr[t] = mul2(rr[t], fr);
+                }
             }
         }
     }
     // nu <= NU literals are live (nu == NU for a full block); suffix carried as (Re s, -Im s)
-    static __device__ __forceinline__ void bwd(int nu, const f32x2 *__restrict__ sy, f32x2 ar, f32x2 ai, f32x2 br, f32x2 bi,
-                                               f32x2 pr0, f32x2 pi0, f32x2 &sr, f32x2 &nsi, f32x2 *__restrict__ g)
+    static __device__ __forceinline__ void bwd(int nu, const f32x2 *__restrict__ sy, const f32x2 (&ar)[PP], const f32x2 (&ai)[PP],
+                                               const f32x2 (&br)[PP], const f32x2 (&bi)[PP], const f32x2 (&pr0)[PP],
+                                               const f32x2 (&pi0)[PP], f32x2 (&sr)[PP], f32x2 (&nsi)[PP], f32x2 *__restrict__ g)
     {
-        f32x2 fr[NU], fi[CPLX ? NU : 1], pr[NU], pi[CPLX ? NU : 1];
+        f32x2 fr[PP][NU], fi[PP][CPLX ? NU : 1], pr[PP][NU], pi[PP][CPLX ? NU : 1];
 #pragma unroll
         for (int u = 0; u < NU; ++u) {
             const f32x2 yv = sy[u * 32];
-            fr[u] = fma2(br, yv, ar);
-            if (CPLX) fi[u] = fma2(bi, yv, ai);
-        }
-        pr[0] = pr0;
-        if (CPLX) pi[0] = pi0;
 #pragma unroll
-        for (int u = 1; u < NU; ++u) {
-            if (CPLX) {
-                pr[u] = fma2(pr[u - 1], fr[u - 1], mul2(pi[u - 1], fi[u - 1] ^ NEG2));
-                pi[u] = fma2(pr[u - 1], fi[u - 1], mul2(pi[u - 1], fr[u - 1]));
-            } else {
-                pr[u] = mul2(pr[u - 1], fr[u - 1]);
+            for (int t = 0; t < PP; ++t) {
+                fr[t][u] = fma2(br[t], yv, ar[t]);
+                if (CPLX) fi[t][u] = fma2(bi[t], yv, ai[t]);
             }
         }
 #pragma unroll
+        for (int t = 0; t < PP; ++t) { pr[t][0] = pr0[t]; if (CPLX) pi[t][0] = pi0[t]; }
+#pragma unroll
+        for (int u = 1; u < NU; ++u)
+#pragma unroll
+            for (int t = 0; t < PP; ++t) {
+                if (CPLX) {
+                    pr[t][u] = fma2(pr[t][u - 1], fr[t][u - 1], mul2(pi[t][u - 1], fi[t][u - 1] ^ NEG2));
+                    pi[t][u] = fma2(pr[t][u - 1], fi[t][u - 1], mul2(pi[t][u - 1], fr[t][u - 1]));
+                } else {
+                    pr[t][u] = mul2(pr[t][u - 1], fr[t][u - 1]);
+                }
+            }
+#pragma unroll
         for (int u = NU - 1; u >= 0; --u) {
             if (u < nu) {                                             // warp-uniform; always true for a full block
-                if (CPLX) {
-                    g[u] = fma2(pr[u], sr, g[u]);                     // Re(pre suf) = pr sr - pi si
-                    g[u] = fma2(pi[u], nsi, g[u]);
-                    const f32x2 t_r = fma2(nsi, fi[u], mul2(sr, fr[u]));              // Re: sr fr - si fi
-                    const f32x2 t_n = fma2(nsi, fr[u], mul2(sr, fi[u] ^ NEG2));       // -Im: -(sr fi + si fr)
-                    sr = t_r; nsi = t_n;
-                } else {
-                    g[u] = fma2(pr[u], sr, g[u]);
-                    sr = mul2(sr, fr[u]);
+#pragma unroll
+                for (int t = 0; t < PP; ++t) {
+                    if (CPLX) {
+                        g[u] = fma2(pr[t][u], sr[t], g[u]);           // Re(pre suf) = pr sr - pi si
+                        g[u] = fma2(pi[t][u], nsi[t], g[u]);
+                        const f32x2 t_r = fma2(nsi[t], fi[t][u], mul2(sr[t], fr[t][u]));            // Re: sr fr - si fi
+                        const f32x2 t_n = fma2(nsi[t], fr[t][u], mul2(sr[t], fi[t][u] ^ NEG2));     // -Im: -(sr fi + si fr)
+                        sr[t] = t_r; nsi[t] = t_n;
+                    } else {
+                        g[u] = fma2(pr[t][u], sr[t], g[u]);
+                        sr[t] = mul2(sr[t], fr[t][u]);
+                    }
                 }
             }
         }
     }
 };
 
-template <int KMAX, bool CPLX, bool GRAD>
+// PP consecutive table rows r, r+8, ... (all real or all complex).  sb: [blk][point][re, im][lane].
+template <int KMAX, bool CPLX, bool GRAD, int PP>
 __device__ __forceinline__ void long_point2(const f32x2 *__restrict__ sy, f32x2 *__restrict__ sb, int k, const float *__restrict__ r,
                                             f32x2 &fe, f32x2 (&g)[KMAX])
 {
     constexpr int NBLK = KMAX / LB2;
-    const f32x2 ar = pk(r[0], r[0]), ai = pk(r[1], r[1]), br = pk(r[2], r[2]), bi = pk(r[3], r[3]);
-    f32x2 rr = pk(1.f, 1.f), ri = 0ull;
+    f32x2 ar[PP], ai[PP], br[PP], bi[PP], rr[PP], ri[PP];
+#pragma unroll
+    for (int t = 0; t < PP; ++t) {
+        const float *rt = r + 8 * t;
+        ar[t] = pk(rt[0], rt[0]); ai[t] = pk(rt[1], rt[1]); br[t] = pk(rt[2], rt[2]); bi[t] = pk(rt[3], rt[3]);
+        rr[t] = pk(1.f, 1.f); ri[t] = 0ull;
+    }
     const int nfull = k / LB2, tail = k % LB2;
+    auto save = [&](int blk) {
+#pragma unroll
+        for (int t = 0; t < PP; ++t) {
+            sb[((2 * blk) * PP + t) * 32] = rr[t];
+            if (CPLX) sb[((2 * blk + 1) * PP + t) * 32] = ri[t];
+        }
+    };
     for (int blk = 0; blk < nfull; ++blk) {                           // forward: runtime loop, one body
-        sb[(2 * blk) * 32] = rr;
-        if (CPLX) sb[(2 * blk + 1) * 32] = ri;
-        BlkOps2<CPLX, LB2>::fwd(sy + blk * LB2 * 32, ar, ai, br, bi, rr, ri);
+        save(blk);
+        BlkOps2<CPLX, LB2, PP>::fwd(sy + blk * LB2 * 32, ar, ai, br, bi, rr, ri);
     }
     if (tail) {
-        sb[(2 * nfull) * 32] = rr;
-        if (CPLX) sb[(2 * nfull + 1) * 32] = ri;
-        for (int u = 0; u < tail; ++u) BlkOps2<CPLX, 1>::fwd(sy + (nfull * LB2 + u) * 32, ar, ai, br, bi, rr, ri);
+        save(nfull);
+        for (int u = 0; u < tail; ++u) BlkOps2<CPLX, 1, PP>::fwd(sy + (nfull * LB2 + u) * 32, ar, ai, br, bi, rr, ri);
     }
-    fe = fma2(pk(r[4], r[4]), rr, fe);
-    if (CPLX) fe = fma2(pk(-r[5], -r[5]), ri, fe);
+#pragma unroll
+    for (int t = 0; t < PP; ++t) {
+        fe = fma2(pk(r[8 * t + 4], r[8 * t + 4]), rr[t], fe);
+        if (CPLX) fe = fma2(pk(-r[8 * t + 5], -r[8 * t + 5]), ri[t], fe);
+    }
     if (GRAD) {
-        f32x2 sr = pk(r[6], r[6]), nsi = CPLX ? pk(-r[7], -r[7]) : 0ull;   // suffix (Re, -Im) seeded with w b
+        f32x2 sr[PP], nsi[PP], p0[PP], p1[PP];                        // suffix (Re, -Im) seeded with w b
+#pragma unroll
+        for (int t = 0; t < PP; ++t) { sr[t] = pk(r[8 * t + 6], r[8 * t + 6]); nsi[t] = CPLX ? pk(-r[8 * t + 7], -r[8 * t + 7]) : 0ull; }
 #pragma unroll
         for (int blk = NBLK - 1; blk >= 0; --blk) {                    // backward: unrolled, g in registers
-            if (blk < nfull)
-                BlkOps2<CPLX, LB2>::bwd(LB2, sy + blk * LB2 * 32, ar, ai, br, bi, sb[(2 * blk) * 32],
-                                        CPLX ? sb[(2 * blk + 1) * 32] : 0ull, sr, nsi, &g[blk * LB2]);
-            else if (blk == nfull && tail)
-                BlkOps2<CPLX, LB2>::bwd(tail, sy + blk * LB2 * 32, ar, ai, br, bi, sb[(2 * blk) * 32],
-                                        CPLX ? sb[(2 * blk + 1) * 32] : 0ull, sr, nsi, &g[blk * LB2]);
+            if (blk < nfull || (blk == nfull && tail)) {
+#pragma unroll
+                for (int t = 0; t < PP; ++t) {
+                    p0[t] = sb[((2 * blk) * PP + t) * 32];
+                    p1[t] = CPLX ? sb[((2 * blk + 1) * PP + t) * 32] : 0ull;
+                }
+                BlkOps2<CPLX, LB2, PP>::bwd(blk < nfull ? LB2 : tail, sy + blk * LB2 * 32, ar, ai, br, bi, p0, p1, sr, nsi, &g[blk * LB2]);
+            }
         }
     }
 }
@@ -970,7 +1005,8 @@ __global__ void __launch_bounds__(LONG_THREADS) k_eval_blk2(const EvalParams<flo
     __shared__ int32_t s_lits[LONG_LIT_CHUNK];
     __shared__ float s_F[NW][64];
     extern __shared__ __align__(16) unsigned char s_dyn[];               // per warp: values [KMAX][32] pairs, boundaries [2 NBLK][32] pairs
-    constexpr int PER_WARP = (KMAX + 2 * (KMAX / LB2)) * 32;
+    constexpr int PP = long_pp(KMAX);
+    constexpr int PER_WARP = (KMAX + 2 * PP * (KMAX / LB2)) * 32;
     f32x2 *s_y = reinterpret_cast<f32x2 *>(s_dyn);
     const Item it = p.items[blockIdx.x];
     const SigDev sgd = p.sigs[it.sig];
@@ -1002,8 +1038,11 @@ __global__ void __launch_bounds__(LONG_THREADS) k_eval_blk2(const EvalParams<flo
 #pragma unroll
             for (int i = 0; i < KMAX; ++i) g[i] = 0ull;
             const float *r = s_tab;
-            for (int q = 0; q < sgd.n_real; ++q, r += 8) long_point2<KMAX, false, GRAD>(sy, sb, k, r, fe2, g);
-            for (int q = 0; q < sgd.n_cplx; ++q, r += 8) long_point2<KMAX, true, GRAD>(sy, sb, k, r, fe2, g);
+            for (int q = 0; q < sgd.n_real; ++q, r += 8) long_point2<KMAX, false, GRAD, 1>(sy, sb, k, r, fe2, g);
+            int q = 0;
+            if (PP == 2)
+                for (; q + 1 < sgd.n_cplx; q += 2, r += 16) long_point2<KMAX, true, GRAD, 2>(sy, sb, k, r, fe2, g);
+            for (; q < sgd.n_cplx; ++q, r += 8) long_point2<KMAX, true, GRAD, 1>(sy, sb, k, r, fe2, g);
             if (GRAD) {
 #pragma unroll
                 for (int i = 0; i < KMAX; ++i) {
