@@ -215,6 +215,9 @@ constexpr int ROW2 = 12;
 #ifndef AFSAT_F2_PAIR_POINTS
 #define AFSAT_F2_PAIR_POINTS 0
 #endif
+#ifndef AFSAT_F2_UNIT_ROWS
+#define AFSAT_F2_UNIT_ROWS 1
+#endif
 #ifndef AFSAT_F2_NEG_BY_XOR
 #define AFSAT_F2_NEG_BY_XOR 1
 #endif
@@ -291,12 +294,100 @@ __device__ __forceinline__ void cplx_points_f2(const f32x2 (&y)[K][NP], const f3
     }
 }
 
-template <int K, int NP, bool GRAD>
+// ---- trivial twiddles (standard tables only: a = 1/2 exactly) ---------------------------------------
+// With the halving folded into the weights (w 2^-k, w b 2^-(k-1): exact power-of-two rescales done when
+// the row is staged) a factor is 1 + (b/a) y, and for the DFT points w^l in {1, -1, i} -- l = 0, N/2, N/4,
+// the twiddles every FFT treats as free -- the product needs no multiplication by a coefficient:
+//   real:  P <- P + P y'                      (y' = y or -y)                1 FFMA2 per literal
+//   w = i: P <- (Re P - y Im P) + i (Im P + y Re P)                         2 FFMA2 per literal
+constexpr f32x2 NEGP = 0x8000000080000000ull;
+
+// The unit rows of a signature are walked TOGETHER (HP: w = 1, HM: w = -1, HI: w = i): each is a serial
+// chain of dependent FFMA2s, so interleaving them is what keeps the FMA pipe fed at 4 warps per scheduler.
+template <int K, int NP, bool HP, bool HM, bool HI, bool GRAD>
+__device__ __forceinline__ void unit_rows_f2(const f32x2 (&y)[K][NP], const f32x2 *__restrict__ rP, const f32x2 *__restrict__ rM,
+                                             const f32x2 *__restrict__ rI, f32x2 (&fe)[NP], f32x2 (&g)[K][NP])
+{
+    const f32x2 one2 = pk(1.0f, 1.0f);
+    f32x2 ny[K][NP], preP[HP ? K : 1][NP], preM[HM ? K : 1][NP], pr[HI ? K : 1][NP], pi[HI ? K : 1][NP];
+    f32x2 runP[NP], runM[NP], rr[NP], ri[NP];
+#pragma unroll
+    for (int i = 0; i < K; ++i)
+#pragma unroll
+        for (int q = 0; q < NP; ++q) ny[i][q] = y[i][q] ^ NEGP;
+#pragma unroll
+    for (int q = 0; q < NP; ++q) {
+        if (HP) runP[q] = add2(y[0][q], one2);                                       // 1 + y_0
+        if (HM) runM[q] = add2(ny[0][q], one2);                                      // 1 - y_0
+        if (HI) { rr[q] = one2; ri[q] = y[0][q]; }                                   // 1 + i y_0
+    }
+#pragma unroll
+    for (int i = 1; i < K; ++i)
+#pragma unroll
+        for (int q = 0; q < NP; ++q) {
+            if (HP) { preP[i][q] = runP[q]; runP[q] = fma2(runP[q], y[i][q], runP[q]); }
+            if (HM) { preM[i][q] = runM[q]; runM[q] = fma2(runM[q], ny[i][q], runM[q]); }
+            if (HI) {
+                pr[i][q] = rr[q]; pi[i][q] = ri[q];
+                const f32x2 nr = fma2(ny[i][q], ri[q], rr[q]);                       // Re: rr - y ri
+                const f32x2 ni = fma2(y[i][q], rr[q], ri[q]);                        // Im: ri + y rr
+                rr[q] = nr; ri[q] = ni;
+            }
+        }
+#pragma unroll
+    for (int q = 0; q < NP; ++q) {
+        if (HP) fe[q] = fma2(bc(rP, 2), runP[q], fe[q]);
+        if (HM) fe[q] = fma2(bc(rM, 2), runM[q], fe[q]);
+        if (HI) { fe[q] = fma2(bc(rI, 6), rr[q], fe[q]); fe[q] = fma2(bc(rI, 7), ri[q], fe[q]); }   // + wr Re P - wi Im P
+    }
+    if (GRAD) {
+        f32x2 sufP[NP], sufM[NP], sr[NP], nsi[NP];                                   // suffixes seeded with w b; (Re s, -Im s)
+#pragma unroll
+        for (int q = 0; q < NP; ++q) {
+            if (HP) sufP[q] = bc(rP, 3);
+            if (HM) sufM[q] = bc(rM, 3);
+            if (HI) { sr[q] = rI[8]; nsi[q] = rI[9]; }
+        }
+#pragma unroll
+        for (int i = K - 1; i >= 1; --i)
+#pragma unroll
+            for (int q = 0; q < NP; ++q) {
+                if (HP) { g[i][q] = fma2(preP[i][q], sufP[q], g[i][q]); sufP[q] = fma2(sufP[q], y[i][q], sufP[q]); }
+                if (HM) { g[i][q] = fma2(preM[i][q], sufM[q], g[i][q]); sufM[q] = fma2(sufM[q], ny[i][q], sufM[q]); }
+                if (HI) {
+                    g[i][q] = fma2(pr[i][q], sr[q], g[i][q]);                        // Re(pre suf) = pr sr - pi si
+                    g[i][q] = fma2(pi[i][q], nsi[q], g[i][q]);
+                    const f32x2 t_r = fma2(y[i][q], nsi[q], sr[q]);                  // Re: sr - y si
+                    const f32x2 t_n = fma2(ny[i][q], sr[q], nsi[q]);                 // -Im: -(si + y sr)
+                    sr[q] = t_r; nsi[q] = t_n;
+                }
+            }
+#pragma unroll
+        for (int q = 0; q < NP; ++q) {                                               // prefix_0 = 1
+            if (HP) g[0][q] = add2(g[0][q], sufP[q]);
+            if (HM) g[0][q] = add2(g[0][q], sufM[q]);
+            if (HI) g[0][q] = add2(g[0][q], sr[q]);
+        }
+    }
+}
+
+// UV (unit variant, chosen once per work item when its table is staged): 0 = generic coefficients in
+// every row; 1 / 2 = standard table whose first rows are the trivial twiddles [w = 1 (UV 1 only)]
+// [w = -1 iff K odd] [w = i iff K = 3 mod 4] (n_real = their number), followed by n_cplx generic complex rows.
+template <int K, int NP, bool GRAD, int UV>
 __device__ __forceinline__ void eval_points_f2(const f32x2 (&y)[K][NP], const f32x2 *__restrict__ tab, int n_real,
                                                int n_cplx, f32x2 (&fe)[NP], f32x2 (&g)[K][NP])
 {
+    if (UV != 0) {
+        constexpr bool HP = UV == 1, HM = (K & 1) != 0, HI = (K & 3) == 3;
+        const f32x2 *rP = tab, *rM = tab + (HP ? ROW2 : 0), *rI = rM + (HM ? ROW2 : 0);
+        if (HP || HM || HI) unit_rows_f2<K, NP, HP, HM, HI, GRAD>(y, rP, rM, rI, fe, g);
+        const f32x2 *r = rI + (HI ? ROW2 : 0);
+        for (int p = 0; p < n_cplx; ++p, r += ROW2) cplx_points_f2<K, NP, 1, GRAD>(y, r, fe, g);
+        return;
+    }
     const f32x2 *r = tab;
-    for (int p = 0; p < n_real; ++p, r += ROW2) {                    // self-conjugate points
+    for (int p = 0; p < n_real; ++p, r += ROW2) {                    // self-conjugate points, generic coefficients
         const f32x2 a = bc(r, 0), b = bc(r, 1), w = bc(r, 2), wb = bc(r, 3);
         f32x2 pre[K][NP], f[K][NP], run[NP], suf[NP];
 #pragma unroll
@@ -322,11 +413,7 @@ __device__ __forceinline__ void eval_points_f2(const f32x2 (&y)[K][NP], const f3
             for (int q = 0; q < NP; ++q) g[0][q] = add2(g[0][q], suf[q]);     // prefix_0 = 1
         }
     }
-    int p = 0;
-    if (AFSAT_F2_PAIR_POINTS) {                                       // two conjugate-pair points per pass: 2 x the independent chains
-        for (; p + 1 < n_cplx; p += 2, r += 2 * ROW2) cplx_points_f2<K, NP, 2, GRAD>(y, r, fe, g);
-    }
-    for (; p < n_cplx; ++p, r += ROW2) cplx_points_f2<K, NP, 1, GRAD>(y, r, fe, g);
+    for (int p = 0; p < n_cplx; ++p, r += ROW2) cplx_points_f2<K, NP, 1, GRAD>(y, r, fe, g);   // one of each conjugate pair
 }
 
 // sign flip by the literal's polarity bit (bit 31 of the packed literal): one LOP3 per value
@@ -491,7 +578,7 @@ template <> struct PairIO<2> {
     }
 };
 
-template <int K, int NP, bool GRAD, bool FIXED, bool PF>
+template <int K, int NP, bool GRAD, bool FIXED, bool PF, int UV>
 __device__ __forceinline__ void run_item_f2(const EvalParams<float> &p, const int32_t *__restrict__ s_lits,
                                             const f32x2 *__restrict__ s_tab2, int n_real, int n_cplx, int nc, int wk,
                                             int64_t b, f32x2 (&fe)[NP])
@@ -530,7 +617,7 @@ __device__ __forceinline__ void run_item_f2(const EvalParams<float> &p, const in
             for (int q = 0; q < NP; ++q) { y[i][q] = y_n[i][q] ^ (((f32x2)m << 32) | m); g[i][q] = 0ull; }   // y = s x
         }
         if (PF && c + Wk < nc) fetch(c + Wk);
-        eval_points_f2<K, NP, GRAD>(y, s_tab2, n_real, n_cplx, fe, g);
+        eval_points_f2<K, NP, GRAD, UV>(y, s_tab2, n_real, n_cplx, fe, g);
         if (GRAD) {
 #pragma unroll
             for (int i = 0; i < K; ++i) {
@@ -553,7 +640,7 @@ __device__ __forceinline__ void run_item_f2(const EvalParams<float> &p, const in
 // allocation while all lengths share one grid (no per-length launch tails) ---------------------------
 template <int K, int NP, bool GRAD>
 __device__ __noinline__ void item_body_f2(const EvalParams<float> &p, const int32_t *s_lits, const f32x2 *s_tab2,
-                                          float (*s_F)[64 * NP], int n_real, int n_cplx, int nc, bool has_fixed)
+                                          float (*s_F)[64 * NP], int n_real, int n_cplx, int nc, bool has_fixed, int uv)
 {
     constexpr int V = 2 * NP;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -565,8 +652,15 @@ __device__ __noinline__ void item_body_f2(const EvalParams<float> &p, const int3
     for (int q = 0; q < NP; ++q) fe2[q] = 0ull;
     if (active) {
         constexpr bool PF = K <= 5;
-        if (has_fixed) run_item_f2<K, NP, GRAD, true, PF>(p, s_lits, s_tab2, n_real, n_cplx, nc, wk, b, fe2);
-        else run_item_f2<K, NP, GRAD, false, PF>(p, s_lits, s_tab2, n_real, n_cplx, nc, wk, b, fe2);
+        if (has_fixed) {                                      // rare (partial assignments): one generic-order body
+            if (uv == 1) run_item_f2<K, NP, GRAD, true, PF, 1>(p, s_lits, s_tab2, n_real, n_cplx, nc, wk, b, fe2);
+            else if (uv == 2) run_item_f2<K, NP, GRAD, true, PF, 2>(p, s_lits, s_tab2, n_real, n_cplx, nc, wk, b, fe2);
+            else run_item_f2<K, NP, GRAD, true, PF, 0>(p, s_lits, s_tab2, n_real, n_cplx, nc, wk, b, fe2);
+        } else {
+            if (uv == 1) run_item_f2<K, NP, GRAD, false, PF, 1>(p, s_lits, s_tab2, n_real, n_cplx, nc, wk, b, fe2);
+            else if (uv == 2) run_item_f2<K, NP, GRAD, false, PF, 2>(p, s_lits, s_tab2, n_real, n_cplx, nc, wk, b, fe2);
+            else run_item_f2<K, NP, GRAD, false, PF, 0>(p, s_lits, s_tab2, n_real, n_cplx, nc, wk, b, fe2);
+        }
     }
     float fe[V];
 #pragma unroll
@@ -577,10 +671,10 @@ __device__ __noinline__ void item_body_f2(const EvalParams<float> &p, const int3
 template <int K, int KHI, int NP, bool GRAD>
 struct SwitchF2 {
     static __device__ __forceinline__ void go(int k, const EvalParams<float> &p, const int32_t *s_lits, const f32x2 *s_tab2,
-                                              float (*s_F)[64 * NP], int n_real, int n_cplx, int nc, bool has_fixed)
+                                              float (*s_F)[64 * NP], int n_real, int n_cplx, int nc, bool has_fixed, int uv)
     {
-        if (k == K) item_body_f2<K, NP, GRAD>(p, s_lits, s_tab2, s_F, n_real, n_cplx, nc, has_fixed);
-        else if (K < KHI) SwitchF2<(K < KHI ? K + 1 : K), KHI, NP, GRAD>::go(k, p, s_lits, s_tab2, s_F, n_real, n_cplx, nc, has_fixed);
+        if (k == K) item_body_f2<K, NP, GRAD>(p, s_lits, s_tab2, s_F, n_real, n_cplx, nc, has_fixed, uv);
+        else if (K < KHI) SwitchF2<(K < KHI ? K + 1 : K), KHI, NP, GRAD>::go(k, p, s_lits, s_tab2, s_F, n_real, n_cplx, nc, has_fixed, uv);
     }
 };
 
@@ -588,22 +682,61 @@ template <int KLO, int KHI, int NP, bool GRAD, int MINB>
 __global__ void __launch_bounds__(CTA_THREADS, MINB) k_eval_f2m(const EvalParams<float> p)
 {
     constexpr int H = (KHI + 1) / 2 + 1;
-    __shared__ __align__(16) f32x2 s_tab2[H * ROW2];
+    __shared__ __align__(16) f32x2 s_tab2[(H + 2) * ROW2];
     __shared__ int32_t s_lits[LIT_CHUNK];
     __shared__ float s_F[CTA_WARPS][64 * NP];
     const Item it = p.items[blockIdx.x];
     const SigDev sg = p.sigs[it.sig];
-    for (int i = threadIdx.x; i < (sg.n_real + sg.n_cplx) * ROW2; i += blockDim.x) {
-        const int q = i / ROW2, j = i % ROW2;
-        const float *r = p.rows + ((int64_t)sg.row_off + q) * 8;
+    // Row order of the staged table.  Standard tables (a = 1/2 exactly in every row): the trivial twiddles
+    // first, at fixed positions (a missing one -- its weight was exactly zero -- is staged with weight 0),
+    // halvings folded into their weights (2^-k, 2^-(k-1): exact rescales); then the generic complex rows.
+    __shared__ int s_src[H + 3], s_hdr[3];                            // source row (or -1) per staged row; {uv, n_unit, n_gen}
+    if (threadIdx.x == 0) {
+        const int nr = sg.n_real + sg.n_cplx;
+        const float *r0 = p.rows + (int64_t)sg.row_off * 8;
+        int uv = 0, n_unit = sg.n_real, n_gen = sg.n_cplx;
+        bool std_tab = AFSAT_F2_UNIT_ROWS != 0;
+        for (int q = 0; q < nr; ++q) std_tab = std_tab && r0[8 * q] == 0.5f && r0[8 * q + 1] == 0.f;
+        if (std_tab) {
+            int iP = -1, iM = -1, iI = -1;
+            for (int q = 0; q < nr; ++q) {
+                const float br = r0[8 * q + 2], bi = r0[8 * q + 3];
+                if (q < sg.n_real) { if (br == 0.5f) iP = q; else if (br == -0.5f) iM = q; }
+                else if (br == 0.f && bi == 0.5f) iI = q;
+            }
+            uv = iP >= 0 ? 1 : 2;
+            int n = 0;
+            if (iP >= 0) s_src[n++] = iP;
+            if (it.k & 1) s_src[n++] = iM;
+            if ((it.k & 3) == 3) s_src[n++] = iI;
+            n_unit = n;
+            for (int q = sg.n_real; q < nr; ++q) if (q != iI) s_src[n++] = q;
+            n_gen = n - n_unit;
+        } else {
+            for (int q = 0; q < nr; ++q) s_src[q] = q;
+        }
+        s_hdr[0] = uv; s_hdr[1] = n_unit; s_hdr[2] = n_gen;
+    }
+    __syncthreads();
+    const int uv = s_hdr[0], n_unit = s_hdr[1], n_gen = s_hdr[2];
+    const float sc_w = __int_as_float((127 - it.k) << 23), sc_wb = 2.0f * sc_w;   // 2^-k, 2^-(k-1)
+    for (int i = threadIdx.x; i < (n_unit + n_gen) * ROW2; i += blockDim.x) {
+        const int q = i / ROW2, j = i % ROW2, src = s_src[q];
         float v = 0.f;
-        if (q < sg.n_real) { if (j < 4) v = r[2 * j]; }               // a, b, w, wb
-        else {
-            switch (j) {
-            case 0: v = r[0]; break;  case 1: v = r[1]; break;  case 2: v = -r[1]; break;
-            case 3: v = r[2]; break;  case 4: v = r[3]; break;  case 5: v = -r[3]; break;
-            case 6: v = r[4]; break;  case 7: v = -r[5]; break; case 8: v = r[6]; break;  case 9: v = -r[7]; break;
-            default: break;
+        if (src >= 0) {
+            const float *r = p.rows + ((int64_t)sg.row_off + src) * 8;
+            const bool unit = uv != 0 && q < n_unit;
+            const float fw = unit ? sc_w : 1.f, fwb = unit ? sc_wb : 1.f;
+            if (src < sg.n_real) {                                    // a, b, w, wb
+                if (j < 2) v = r[2 * j]; else if (j == 2) v = r[4] * fw; else if (j == 3) v = r[6] * fwb;
+            } else {
+                switch (j) {
+                case 0: v = r[0]; break;  case 1: v = r[1]; break;  case 2: v = -r[1]; break;
+                case 3: v = r[2]; break;  case 4: v = r[3]; break;  case 5: v = -r[3]; break;
+                case 6: v = r[4] * fw; break;  case 7: v = -r[5] * fw; break;
+                case 8: v = r[6] * fwb; break;  case 9: v = -r[7] * fwb; break;
+                default: break;
+                }
             }
         }
         s_tab2[i] = pk(v, v);
@@ -611,7 +744,7 @@ __global__ void __launch_bounds__(CTA_THREADS, MINB) k_eval_f2m(const EvalParams
     const int nl = (it.c_end - it.c_begin) * it.k;
     for (int i = threadIdx.x; i < nl; i += blockDim.x) s_lits[i] = __ldg(p.lits + it.lit_base + i);
     __syncthreads();
-    SwitchF2<KLO, KHI, NP, GRAD>::go(it.k, p, s_lits, s_tab2, s_F, sg.n_real, sg.n_cplx, it.c_end - it.c_begin, it.has_fixed != 0);
+    SwitchF2<KLO, KHI, NP, GRAD>::go(it.k, p, s_lits, s_tab2, s_F, n_unit, n_gen, it.c_end - it.c_begin, it.has_fixed != 0, uv);
 }
 
 template <typename T, int K, int V, bool GRAD>
