@@ -294,13 +294,14 @@ __device__ __forceinline__ void cplx_points_f2(const f32x2 (&y)[K][NP], const f3
     }
 }
 
+constexpr f32x2 NEGP = 0x8000000080000000ull;
+
 // ---- trivial twiddles (standard tables only: a = 1/2 exactly) ---------------------------------------
 // With the halving folded into the weights (w 2^-k, w b 2^-(k-1): exact power-of-two rescales done when
 // the row is staged) a factor is 1 + (b/a) y, and for the DFT points w^l in {1, -1, i} -- l = 0, N/2, N/4,
 // the twiddles every FFT treats as free -- the product needs no multiplication by a coefficient:
 //   real:  P <- P + P y'                      (y' = y or -y)                1 FFMA2 per literal
 //   w = i: P <- (Re P - y Im P) + i (Im P + y Re P)                         2 FFMA2 per literal
-constexpr f32x2 NEGP = 0x8000000080000000ull;
 
 // The unit rows of a signature are walked TOGETHER (HP: w = 1, HM: w = -1, HI: w = i): each is a serial
 // chain of dependent FFMA2s, so interleaving them is what keeps the FMA pipe fed at 4 warps per scheduler.
