@@ -125,6 +125,32 @@ int afsat_step(afsat_ctx *ctx, void *d_x, double eta, int32_t n_steps, int32_t s
                int32_t *d_first_step, int32_t *h_any_solved, void *stream);
 
 /*
+ * afsat_step_ls -- Alg. 1 WITH its line search and convergence test ("eta <-
+ * lineSearch(FE, grad FE, s)", :125 "if eta < delta", :103).  The paper
+ * names no method; reading B5 fixes backtracking with the Armijo rule along the projection
+ * arc, independently per candidate (the candidates of a batch are independent searches):
+ *     G = grad F(X);  eta = s_max;
+ *     repeat at most max_trials times:
+ *         X' = clamp(X - eta G, -1, +1) on free variables;   D = <G, X - X'>;
+ *         if F(X') <= F(X) - c1 D: accept, stop;   else eta <- beta eta;
+ *         if eta < delta: the candidate has CONVERGED (d_converged = 1): it keeps X and is frozen;
+ *     accepted: X <- X';  round;  count;  solved candidates are frozen as in afsat_step.
+ *   A candidate that exhausts max_trials without acceptance keeps X for this step and is not flagged.
+ *   Every trial costs one objective-only evaluation (a1-a3, no suffix walk) of the candidates
+ *   still searching; the others are skipped warp by warp.
+ *   d_x [n][ldb] in/out.  d_F [B] (may be NULL): F at the final X.  d_eta [B] (may be NULL): the step
+ *   length of the last iteration (accepted, or the one that fell below delta / was rejected last).
+ *   d_converged [B]; d_sat_count, d_is_solution, d_first_step, resume, step_base, h_any_solved as in
+ *   afsat_step (resume != 0 also reads d_converged).  0 < beta < 1, 0 <= c1 < 1, s_max > 0,
+ *   delta >= 0, max_trials >= 1; otherwise AFSAT_E_INVALID.
+ *   Workspace: a full gradient and a trial copy of X ([n][ldb] each), allocated on first use.
+ */
+int afsat_step_ls(afsat_ctx *ctx, void *d_x, double s_max, double beta, double c1, double delta,
+                  int32_t max_trials, int32_t n_steps, int32_t step_base, int32_t resume,
+                  void *d_F, void *d_eta, int32_t *d_sat_count, uint8_t *d_is_solution,
+                  int32_t *d_first_step, uint8_t *d_converged, int32_t *h_any_solved, void *stream);
+
+/*
  * afsat_step_host -- the same as afsat_step (resume = 0, step_base = 0) for HOST buffers: copies
  * h_x [n][ldb] to the device, runs n_steps, copies X, F, sat_count, is_solution, first_step back
  * (any output pointer may be NULL) and synchronises.  Pinned host memory makes the copies

@@ -27,6 +27,8 @@
  *   O9  x <- min(1, max(-1, x - eta * G))                      -- Alg. 1
  *   O10 T_v = (x_v < 0); tau = #true literals; integer satisfied count; first solved step;
  *       solved candidates are frozen (Alg. 1 :124-127).
+ *   O11 Alg. 1 with its line search (method not given by the paper: DESIGN.md
+ *       reading B5 = per-candidate backtracking, Armijo rule along the projection arc): oracle_step_ls.
  * No DFT, no prefix/suffix products, no blocking, no reordering.
  *
  * Pins (tests/test_oracle_pins.py, `-m "not gpu"`): brute force of Eq. (1) over all 2^k subsets
@@ -36,7 +38,9 @@
  * types, monotone-gradient closed forms, an independent integer recount for the discrete check,
  * and the worked k=3 values of tests/golden/worked_k3.txt.
  * Parity unpinned by the PAPER (pinned only by DESIGN.md readings): the step size eta, the
- * rounding of x = 0 (reading A9: True iff x < 0), "no-op" semantics of frozen candidates (A12).
+ * rounding of x = 0 (reading A9: True iff x < 0), "no-op" semantics of frozen candidates (A12), and
+ * the whole of oracle_step_ls (the paper names neither the line-search method nor its constants;
+ * its pins check the textbook properties of the rule in reading B5, not the paper).
  *
  * Layout: X, G are variable-major, candidate-minor: x[v*ldb + b].  All arrays are caller-owned.
  * Every function returns 0 on success, a negative number on invalid input.
@@ -343,6 +347,86 @@ int oracle_step(int32_t n, int32_t m, const int64_t *row_ptr, const int32_t *lit
             if (F) F[b] = (double)eval_candidate(&I, x, ldb, NULL);
         }
         free(g);
+    }
+    inst_free(&I);
+    return 0;
+}
+
+/*
+ * O11 -- Alg. 1 WITH line search and convergence test ("eta <- lineSearch(FE, grad FE, s)",
+ * :120-122 step and projection, :125 "if eta < delta").  Reading B5 (the paper gives no method):
+ * per candidate, backtracking with the Armijo rule along the projection arc,
+ *     eta = s_max;  repeat at most max_trials times:
+ *         X' = clamp(X - eta G) on free variables;  D = <G, X - X'>;
+ *         if F(X') <= F(X) - c1 D: accept;  else eta <- beta eta;  if eta < delta: converged.
+ * An accepted candidate moves to X'; a converged one keeps X and is frozen (like a solved one);
+ * one that exhausts max_trials keeps X for this step.  margin[b] (may be NULL) = the smallest
+ * |F(X') - (F(X) - c1 D)| met in the LAST iteration: how close the accept/reject decisions were
+ * to a tie (the parity tests compare decisions only where it exceeds the kernel's rounding).
+ */
+int oracle_step_ls(int32_t n, int32_t m, const int64_t *row_ptr, const int32_t *lit_var,
+                   const int8_t *lit_sign, const uint8_t *type, const int32_t *param,
+                   const int8_t *fixed, int32_t B, int64_t ldb, double *X /* in/out */,
+                   double s_max, double beta, double c1, double delta, int32_t max_trials,
+                   int32_t n_steps, int32_t step_base, int32_t resume,
+                   double *F /* [B] or NULL */, double *eta_out /* [B] or NULL */, int32_t *sat_count,
+                   uint8_t *is_solution, int32_t *first_step, uint8_t *converged,
+                   double *margin /* [B] or NULL */)
+{
+    inst_t I;
+    int rc = inst_init(&I, n, m, row_ptr, lit_var, lit_sign, type, param, fixed, 1);
+    if (rc) return rc;
+    if (!(s_max > 0) || !(beta > 0 && beta < 1) || !(c1 >= 0 && c1 < 1) || !(delta >= 0) || max_trials < 1) {
+        inst_free(&I);
+        return -1;
+    }
+#pragma omp parallel
+    {
+        real *g = (real *)malloc(sizeof(real) * (size_t)n);
+        double *xt = (double *)malloc(sizeof(double) * (size_t)n);   /* trial point, one column, stride 1 */
+        double *x0 = (double *)malloc(sizeof(double) * (size_t)n);
+#pragma omp for schedule(dynamic, 1)
+        for (int32_t b = 0; b < B; ++b) {
+            double *x = X + b;
+            int solved = resume ? (is_solution[b] != 0) : 0;
+            int conv = resume ? (converged[b] != 0) : 0;
+            int32_t first = resume ? first_step[b] : -1;
+            real eta = (real)s_max, mg = INFINITY;
+            for (int32_t t = 1; t <= n_steps && !solved && !conv; ++t) {
+                real F0 = eval_candidate(&I, x, ldb, g);
+                int accepted = 0;
+                eta = (real)s_max; mg = INFINITY;
+                for (int32_t v = 0; v < n; ++v) x0[v] = x[(int64_t)v * ldb];
+                for (int32_t j = 0; j < max_trials && !accepted && !conv; ++j) {
+                    real D = 0.0L;
+                    for (int32_t v = 0; v < n; ++v) {
+                        real nx = (real)x0[v];
+                        if (!(fixed && fixed[v] != 0)) {
+                            nx = (real)x0[v] - eta * g[v];
+                            if (nx > 1.0L) nx = 1.0L;
+                            if (nx < -1.0L) nx = -1.0L;
+                            D += g[v] * ((real)x0[v] - nx);
+                        }
+                        xt[v] = (double)nx;
+                    }
+                    real F1 = eval_candidate(&I, xt, 1, NULL);
+                    real gap = fabsl(F1 - (F0 - (real)c1 * D));
+                    if (gap < mg) mg = gap;
+                    if (F1 <= F0 - (real)c1 * D) accepted = 1;
+                    else { eta *= (real)beta; if (eta < (real)delta) conv = 1; }
+                }
+                if (accepted) for (int32_t v = 0; v < n; ++v) x[(int64_t)v * ldb] = xt[v];
+                if (check_candidate(&I, x, ldb) == m) { solved = 1; first = step_base + t; }
+            }
+            sat_count[b] = check_candidate(&I, x, ldb);
+            is_solution[b] = (uint8_t)solved;
+            converged[b] = (uint8_t)conv;
+            first_step[b] = first;
+            if (eta_out) eta_out[b] = (double)eta;
+            if (margin) margin[b] = (double)mg;
+            if (F) F[b] = (double)eval_candidate(&I, x, ldb, NULL);
+        }
+        free(g); free(xt); free(x0);
     }
     inst_free(&I);
     return 0;

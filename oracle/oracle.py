@@ -43,7 +43,7 @@ def lib():
         L = C.CDLL(str(_LIB))
         L.oracle_num_threads.restype = C.c_int
         for name in ("oracle_truth_table", "oracle_coeffs", "oracle_fe_single",
-                     "oracle_eval_grad", "oracle_check", "oracle_step"):
+                     "oracle_eval_grad", "oracle_check", "oracle_step", "oracle_step_ls"):
             getattr(L, name).restype = C.c_int
         _lib = L
     return _lib
@@ -154,3 +154,35 @@ def step(inst, X, eta: float, n_steps: int, B=None, *, step_base: int = 0, state
     if rc:
         raise ValueError(f"oracle_step rc={rc}")
     return X, F, sat, sol, first
+
+
+def step_ls(inst, X, n_steps: int, B=None, *, s_max: float = 1.0, beta: float = 0.5, c1: float = 1e-4,
+            delta: float = 1e-6, max_trials: int = 8, step_base: int = 0, state=None, want_F: bool = True):
+    """Alg. 1 with the backtracking line search of reading B5 (oracle_step_ls).
+    Returns (X_new, F, eta, sat_count, is_solution, first_step, converged, margin)."""
+    B = int(X.shape[1] if B is None else B)
+    X = _check_x(inst, X, B).copy()
+    F = np.zeros(B, dtype=np.float64) if want_F else None
+    eta = np.zeros(B, dtype=np.float64)
+    margin = np.zeros(B, dtype=np.float64)
+    sat = np.zeros(B, dtype=np.int32)
+    if state is None:
+        sol = np.zeros(B, dtype=np.uint8)
+        first = np.full(B, -1, dtype=np.int32)
+        conv = np.zeros(B, dtype=np.uint8)
+        resume = 0
+    else:
+        sol = np.ascontiguousarray(state[0], dtype=np.uint8).copy()
+        first = np.ascontiguousarray(state[1], dtype=np.int32).copy()
+        conv = np.ascontiguousarray(state[2], dtype=np.uint8).copy()
+        resume = 1
+    args, keep = _inst_args(inst)
+    rc = lib().oracle_step_ls(*args, C.c_int32(B), C.c_int64(X.shape[1]), _p(X, C.c_double),
+                              C.c_double(s_max), C.c_double(beta), C.c_double(c1), C.c_double(delta),
+                              C.c_int32(max_trials), C.c_int32(n_steps), C.c_int32(step_base),
+                              C.c_int32(resume), _p(F, C.c_double), _p(eta, C.c_double),
+                              _p(sat, C.c_int32), _p(sol, C.c_uint8), _p(first, C.c_int32),
+                              _p(conv, C.c_uint8), _p(margin, C.c_double))
+    if rc:
+        raise ValueError(f"oracle_step_ls rc={rc}")
+    return X, F, eta, sat, sol, first, conv, margin

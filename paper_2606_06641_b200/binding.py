@@ -28,7 +28,7 @@ ERROR_NAMES = {0: "AFSAT_OK", -1: "AFSAT_E_INVALID", -2: "AFSAT_E_LENGTH", -3: "
 
 EXPORTS = ["afsat_create", "afsat_destroy", "afsat_last_error", "afsat_eval_grad", "afsat_check",
            "afsat_step", "afsat_step_host", "afsat_host_tables", "afsat_query", "afsat_version",
-           "afsat_set_profiling"]
+           "afsat_set_profiling", "afsat_step_ls"]
 
 
 class AfsatError(RuntimeError):
@@ -59,6 +59,8 @@ def load_library():
     L.afsat_check.argtypes = [vp, vp, vp, vp, vp]
     L.afsat_step.restype = C.c_int
     L.afsat_step.argtypes = [vp, vp, dbl, i32, i32, i32, vp, vp, vp, vp, vp, vp]
+    L.afsat_step_ls.restype = C.c_int
+    L.afsat_step_ls.argtypes = [vp, vp, dbl, dbl, dbl, dbl, i32, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp]
     L.afsat_step_host.restype = C.c_int
     L.afsat_step_host.argtypes = [vp, vp, dbl, i32, vp, vp, vp, vp]
     L.afsat_host_tables.restype = C.c_int
@@ -209,6 +211,35 @@ class Context:
                                 first.data_ptr(), hp, _stream_ptr(stream))
         self._raise(rc)
         return F, sat, sol, first
+
+    def step_ls(self, x, n_steps, *, s_max=1.0, beta=0.5, c1=1e-4, delta=1e-6, max_trials=8, step_base=0,
+                state=None, want_F=True, h_any_solved=None, stream=None):
+        """In-place n_steps of Alg. 1 with the backtracking line search (afsat_step_ls).
+        Returns (F, eta, sat_count, is_solution, first_step, converged)."""
+        import torch
+        self._check_x(x)
+        dev = x.device
+        F = torch.empty(self.B, dtype=x.dtype, device=dev) if want_F else None
+        eta = torch.empty(self.B, dtype=x.dtype, device=dev)
+        sat = torch.empty(self.B, dtype=torch.int32, device=dev)
+        if state is None:
+            sol = torch.empty(self.B, dtype=torch.uint8, device=dev)
+            first = torch.empty(self.B, dtype=torch.int32, device=dev)
+            conv = torch.empty(self.B, dtype=torch.uint8, device=dev)
+            resume = 0
+        else:
+            sol, first, conv = state
+            resume = 1
+        hp = None
+        if h_any_solved is not None:
+            assert h_any_solved.is_pinned() and h_any_solved.dtype == torch.int32 and h_any_solved.numel() >= 2
+            hp = h_any_solved.data_ptr()
+        rc = self._L.afsat_step_ls(self._h, x.data_ptr(), float(s_max), float(beta), float(c1), float(delta),
+                                   int(max_trials), int(n_steps), int(step_base), resume,
+                                   F.data_ptr() if F is not None else None, eta.data_ptr(), sat.data_ptr(),
+                                   sol.data_ptr(), first.data_ptr(), conv.data_ptr(), hp, _stream_ptr(stream))
+        self._raise(rc)
+        return F, eta, sat, sol, first, conv
 
     def step_host(self, h_x, eta, n_steps, *, want_F=True):
         """End-to-end call on HOST buffers (numpy or pinned torch CPU tensors), synchronous.

@@ -69,6 +69,11 @@ struct afsat_ctx {
     void *dh_x = nullptr, *dh_F = nullptr;
     int32_t *dh_sat = nullptr, *dh_first = nullptr;
     uint8_t *dh_sol = nullptr;
+    // workspace of afsat_step_ls (lazy): full gradient, trial X', reduction partials, per-candidate state
+    void *ls_G = nullptr, *ls_xt = nullptr, *ls_F0 = nullptr, *ls_F1 = nullptr;
+    double *ls_Dpart = nullptr, *ls_eta = nullptr;
+    uint8_t *ls_state = nullptr;
+    const uint8_t *cur_skip = nullptr;             // candidate mask of the evaluation launches (line-search trials)
     cudaStream_t own_stream = nullptr;
     cudaStream_t side_stream[N_CLS - 1] = {nullptr, nullptr};       // concurrent launches of the length classes
     cudaEvent_t ev_fork = nullptr, ev_join[N_CLS - 1] = {nullptr, nullptr};
@@ -191,6 +196,7 @@ int launch_eval(afsat_ctx *ctx, const T *x, T *G, int64_t g_ld, int64_t g_b0, T 
     EvalParams<T> p;
     p.x = x; p.G = G; p.g_ld = g_ld; p.g_b0 = g_b0; p.Fpart = Fpart;
     p.lits = ctx->d_lits; p.sigs = ctx->d_sigs; p.rows = (const T *)ctx->d_rows;
+    p.skip = ctx->cur_skip;
     p.B = ctx->B; p.ldb = ctx->ldb; p.b_begin = b_begin; p.b_end = std::min<int64_t>(b_begin + width, ctx->ldb);
     const bool grad = G != nullptr;
     constexpr int VA = sizeof(T) == 4 ? AFSAT_A_V : 1;
@@ -275,7 +281,7 @@ int launch_pack(afsat_ctx *ctx, const T *x, cudaStream_t st)
 template <typename T>
 int reduce_F(afsat_ctx *ctx, T *F, cudaStream_t st)
 {
-    k_reduce_F<T><<<(ctx->B + 127) / 128, 128, 0, st>>>((const T *)ctx->d_Fpart, ctx->n_items, ctx->ldb, ctx->B, F);
+    k_reduce_F<T><<<(ctx->B + 127) / 128, 128, 0, st>>>((const T *)ctx->d_Fpart, ctx->n_items, ctx->ldb, ctx->B, F, ctx->cur_skip);
     ++ctx->launches;
     CU(cudaPeekAtLastError());
     return AFSAT_OK;
@@ -353,6 +359,89 @@ int step_t(afsat_ctx *ctx, T *x, double eta, int n_steps, int step_base, int res
         }
         return reduce_F<T>(ctx, F, st);
     }
+    return AFSAT_OK;
+}
+
+// Alg. 1 with the per-candidate backtracking line search of afsat_step_ls (include/afsat.h)
+template <typename T>
+int step_ls_t(afsat_ctx *ctx, T *x, double s_max, double beta, double c1, double delta, int max_trials, int n_steps,
+              int step_base, int resume, T *F, void *eta_out, int32_t *sat, uint8_t *sol, int32_t *first, uint8_t *conv,
+              int32_t *h_any_dev, cudaStream_t st)
+{
+    const int B = ctx->B, tb = 128, gb = (B + tb - 1) / tb;
+    const int64_t ldb = ctx->ldb;
+    const size_t nb = (size_t)ctx->n * ldb;
+    if (!ctx->ls_G) {
+        int rc;
+        char *pg = nullptr, *px = nullptr, *p0 = nullptr, *p1 = nullptr;
+        if ((rc = dev_alloc(ctx, &pg, nb * sizeof(T)))) return rc;
+        ctx->ls_G = pg;
+        if ((rc = dev_alloc(ctx, &px, nb * sizeof(T)))) return rc;
+        ctx->ls_xt = px;
+        if ((rc = dev_alloc(ctx, &p0, (size_t)ldb * sizeof(T), true))) return rc;
+        ctx->ls_F0 = p0;
+        if ((rc = dev_alloc(ctx, &p1, (size_t)ldb * sizeof(T), true))) return rc;
+        ctx->ls_F1 = p1;
+        if ((rc = dev_alloc(ctx, &ctx->ls_Dpart, (size_t)LS_CHUNKS * ldb, true))) return rc;
+        if ((rc = dev_alloc(ctx, &ctx->ls_eta, (size_t)ldb, true))) return rc;
+        if ((rc = dev_alloc(ctx, &ctx->ls_state, (size_t)ldb, true))) return rc;
+    }
+    T *G = (T *)ctx->ls_G, *xt = (T *)ctx->ls_xt, *F0 = (T *)ctx->ls_F0, *F1 = (T *)ctx->ls_F1;
+    if (!resume) {
+        k_reset_state<<<gb, tb, 0, st>>>(B, sol, first);
+        ++ctx->launches;
+        CU(cudaMemsetAsync(conv, 0, (size_t)B, st));
+    }
+    CU(cudaMemsetAsync(ctx->d_any, 0, 2 * sizeof(int32_t), st));
+    const unsigned gl = (unsigned)((ldb + CTA_THREADS - 1) / CTA_THREADS);
+    const unsigned gyc = (unsigned)std::min<int64_t>(ctx->n, std::max<int64_t>(1, (int64_t)ctx->sm_count * 8 / gl));
+    if (n_steps == 0) {                                               // no step: F, counts on X as it is
+        k_ls_begin<<<gl, CTA_THREADS, 0, st>>>(B, ldb, sol, conv, ctx->ls_state, s_max, ctx->ls_eta);
+        ++ctx->launches;
+        int rc = eval_grad_t<T>(ctx, x, F0, (T *)nullptr, st);
+        if (!rc) rc = launch_pack<T>(ctx, x, st);
+        if (!rc) rc = launch_check_bits(ctx, 0, ldb / 32, st);
+        if (rc) return rc;
+        k_flags<<<gb, tb, 0, st>>>(ctx->d_satacc, B, ctx->m, 0, step_base, sat, sol, first, ctx->d_any, h_any_dev);
+        ++ctx->launches;
+    }
+    for (int t = 1; t <= n_steps; ++t) {
+        k_ls_begin<<<gl, CTA_THREADS, 0, st>>>(B, ldb, sol, conv, ctx->ls_state, s_max, ctx->ls_eta);
+        ++ctx->launches;
+        // a1-a5 at X(t-1): objective and full gradient (frozen candidates are skipped)
+        ctx->cur_skip = ctx->ls_state;
+        int rc = eval_grad_t<T>(ctx, x, F0, G, st);
+        ctx->cur_skip = nullptr;
+        if (rc) return rc;
+        for (int j = 0; j < max_trials; ++j) {
+            k_ls_trial<T><<<dim3(gl, LS_CHUNKS), CTA_THREADS, 0, st>>>(x, G, xt, ctx->d_fixed, ctx->ls_state, ctx->ls_eta,
+                                                                        ctx->ls_Dpart, ctx->n, ldb, j == 0);
+            ++ctx->launches;
+            CU(cudaPeekAtLastError());
+            ctx->cur_skip = ctx->ls_state;                            // objective only, candidates still searching
+            rc = eval_grad_t<T>(ctx, xt, F1, (T *)nullptr, st);
+            ctx->cur_skip = nullptr;
+            if (rc) return rc;
+            k_ls_decide<T><<<gb, tb, 0, st>>>(B, ldb, F0, F1, ctx->ls_Dpart, ctx->ls_state, ctx->ls_eta, conv, c1, beta, delta);
+            ++ctx->launches;
+            CU(cudaPeekAtLastError());
+        }
+        k_ls_commit<T><<<dim3(gl, gyc), CTA_THREADS, 0, st>>>(x, xt, ctx->ls_state, ctx->d_bits, ctx->n, B, ldb);
+        ++ctx->launches;
+        CU(cudaPeekAtLastError());
+        rc = launch_check_bits(ctx, 0, ldb / 32, st);
+        if (rc) return rc;
+        k_flags<<<gb, tb, 0, st>>>(ctx->d_satacc, B, ctx->m, 1, step_base + t, sat, sol, first, ctx->d_any, h_any_dev);
+        ++ctx->launches;
+        CU(cudaPeekAtLastError());
+    }
+    if (eta_out) {
+        k_ls_report<T><<<gb, tb, 0, st>>>(B, ctx->ls_eta, (T *)eta_out);
+        ++ctx->launches;
+        CU(cudaPeekAtLastError());
+    }
+    if (F && n_steps > 0) return eval_grad_t<T>(ctx, x, F, (T *)nullptr, st);   // objective at the final X, every candidate
+    if (F) CU(cudaMemcpyAsync(F, F0, (size_t)B * sizeof(T), cudaMemcpyDeviceToDevice, st));
     return AFSAT_OK;
 }
 
@@ -665,6 +754,8 @@ void afsat_destroy(afsat_ctx *ctx)
     cudaFree(ctx->d_lits); cudaFree(ctx->d_bits); cudaFree(ctx->d_sigs); cudaFree(ctx->d_rows);
     cudaFree(ctx->d_fixed); cudaFree(ctx->d_items); cudaFree(ctx->d_G); cudaFree(ctx->d_Fpart);
     cudaFree(ctx->d_satacc); cudaFree(ctx->d_any);
+    cudaFree(ctx->ls_G); cudaFree(ctx->ls_xt); cudaFree(ctx->ls_F0); cudaFree(ctx->ls_F1); cudaFree(ctx->ls_Dpart);
+    cudaFree(ctx->ls_eta); cudaFree(ctx->ls_state);
     cudaFree(ctx->dh_x); cudaFree(ctx->dh_F); cudaFree(ctx->dh_sat); cudaFree(ctx->dh_first); cudaFree(ctx->dh_sol);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
     for (int i = 0; i < N_CLS - 1; ++i) {
@@ -720,6 +811,32 @@ int afsat_step(afsat_ctx *ctx, void *d_x, double eta, int32_t n_steps, int32_t s
     return ctx->dtype == 32
                ? step_t<float>(ctx, (float *)d_x, eta, n_steps, step_base, resume, (float *)d_F, d_sat_count, d_is_solution, d_first_step, h_dev, st)
                : step_t<double>(ctx, (double *)d_x, eta, n_steps, step_base, resume, (double *)d_F, d_sat_count, d_is_solution, d_first_step, h_dev, st);
+}
+
+int afsat_step_ls(afsat_ctx *ctx, void *d_x, double s_max, double beta, double c1, double delta, int32_t max_trials,
+                  int32_t n_steps, int32_t step_base, int32_t resume, void *d_F, void *d_eta, int32_t *d_sat_count,
+                  uint8_t *d_is_solution, int32_t *d_first_step, uint8_t *d_converged, int32_t *h_any_solved, void *stream)
+{
+    if (!ctx) return AFSAT_E_INVALID;
+    if (!d_x || !d_sat_count || !d_is_solution || !d_first_step || !d_converged)
+        return fail(ctx, AFSAT_E_INVALID, "afsat_step_ls: NULL pointer");
+    if (n_steps < 0 || max_trials < 1) return fail(ctx, AFSAT_E_INVALID, "afsat_step_ls: n_steps < 0 or max_trials < 1");
+    if (!(s_max > 0.0) || !(beta > 0.0 && beta < 1.0) || !(c1 >= 0.0 && c1 < 1.0) || !(delta >= 0.0))
+        return fail(ctx, AFSAT_E_INVALID, "afsat_step_ls: need s_max > 0, 0 < beta < 1, 0 <= c1 < 1, delta >= 0");
+    int rc = set_device(ctx);
+    if (rc) return rc;
+    int32_t *h_dev = nullptr;
+    if (h_any_solved) {
+        CU(cudaHostGetDevicePointer((void **)&h_dev, h_any_solved, 0));
+        h_any_solved[0] = 0;
+        h_any_solved[1] = -1;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    return ctx->dtype == 32
+               ? step_ls_t<float>(ctx, (float *)d_x, s_max, beta, c1, delta, max_trials, n_steps, step_base, resume, (float *)d_F,
+                                  d_eta, d_sat_count, d_is_solution, d_first_step, d_converged, h_dev, st)
+               : step_ls_t<double>(ctx, (double *)d_x, s_max, beta, c1, delta, max_trials, n_steps, step_base, resume, (double *)d_F,
+                                   d_eta, d_sat_count, d_is_solution, d_first_step, d_converged, h_dev, st);
 }
 
 int afsat_step_host(afsat_ctx *ctx, void *h_x, double eta, int32_t n_steps, void *h_F, int32_t *h_sat_count,

@@ -65,7 +65,18 @@ struct EvalParams {
     int64_t ldb;
     int64_t b_begin, b_end;     // candidate tile of this launch (b_end <= ldb)
     int32_t Wc, Wk;             // warps of a CTA: Wc candidate sub-tiles x Wk constraint groups
+    const uint8_t *skip;        // [ldb] or null: candidates with skip[b] != 0 are not evaluated (line search)
 };
+
+// lane-level test of the skip mask for the V candidates b .. b+V-1 of a lane (all must be skipped)
+template <typename T>
+__device__ __forceinline__ bool lane_skipped(const EvalParams<T> &p, int64_t b, int V)
+{
+    if (!p.skip) return false;
+    bool all = true;
+    for (int v = 0; v < V; ++v) all = all && (b + v >= p.ldb || p.skip[b + v] != 0);
+    return all;
+}
 
 template <typename T> __device__ __forceinline__ T fma_(T a, T b, T c);
 template <> __device__ __forceinline__ float fma_<float>(float a, float b, float c) { return fmaf(a, b, c); }
@@ -647,7 +658,7 @@ __device__ __noinline__ void item_body_f2(const EvalParams<float> &p, const int3
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int wc = warp % p.Wc, wk = warp / p.Wc;
     const int64_t b = p.b_begin + ((int64_t)blockIdx.y * p.Wc + wc) * (32 * V) + lane * V;
-    const bool active = b < p.b_end && b < p.B;            // this launch owns [b_begin, b_end)
+    const bool active = b < p.b_end && b < p.B && !lane_skipped(p, b, V);   // this launch owns [b_begin, b_end)
     f32x2 fe2[NP];
 #pragma unroll
     for (int q = 0; q < NP; ++q) fe2[q] = 0ull;
@@ -755,7 +766,7 @@ __device__ __noinline__ void item_body_k(const EvalParams<T> &p, const int32_t *
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int wc = warp % p.Wc, wk = warp / p.Wc;
     const int64_t b = p.b_begin + ((int64_t)blockIdx.y * p.Wc + wc) * (32 * V) + lane * V;
-    const bool active = b < p.b_end && b < p.B;            // this launch owns [b_begin, b_end)
+    const bool active = b < p.b_end && b < p.B && !lane_skipped(p, b, V);   // this launch owns [b_begin, b_end)
     T fe[V];
 #pragma unroll
     for (int v = 0; v < V; ++v) fe[v] = T(0);
@@ -958,7 +969,7 @@ __global__ void __launch_bounds__(LONG_THREADS) k_eval_blk(const EvalParams<T> p
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int wc = warp % p.Wc, wk = warp / p.Wc;
     const int64_t b = p.b_begin + ((int64_t)blockIdx.y * p.Wc + wc) * 32 + lane;
-    const bool active = b < p.b_end && b < p.B;            // this launch owns [b_begin, b_end)
+    const bool active = b < p.b_end && b < p.B && !lane_skipped(p, b, 1);   // this launch owns [b_begin, b_end)
     T fe[1] = {T(0)};
     if (active) {
         T *sy = s_y + (size_t)warp * PER_WARP + lane;
@@ -1149,7 +1160,7 @@ __global__ void __launch_bounds__(LONG_THREADS) k_eval_blk2(const EvalParams<flo
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int wc = warp % p.Wc, wk = warp / p.Wc;
     const int64_t b = p.b_begin + ((int64_t)blockIdx.y * p.Wc + wc) * 64 + lane * 2;
-    const bool active = b < p.b_end && b < p.B;            // this launch owns [b_begin, b_end)
+    const bool active = b < p.b_end && b < p.B && !lane_skipped(p, b, 2);   // this launch owns [b_begin, b_end)
     f32x2 fe2 = 0ull;
     if (active) {
         f32x2 *sy = s_y + (size_t)warp * PER_WARP + lane;
@@ -1353,6 +1364,95 @@ __global__ void __launch_bounds__(CTA_THREADS) k_check_bits(const CheckParams p)
     }
 }
 
+// ---- line search (afsat_step_ls; reading B5): per-candidate backtracking along the projection arc ----
+// ls_state[b]: 0 = still searching, 1 = step accepted, 2 = frozen (solved or converged)
+constexpr int LS_CHUNKS = 32;         // row chunks of the <G, X - X'> reduction (fixed-order two-stage sum)
+
+__global__ void k_ls_begin(int B, int64_t ldb, const uint8_t *__restrict__ is_solution, const uint8_t *__restrict__ converged,
+                           uint8_t *__restrict__ ls_state, double s_max, double *__restrict__ eta)
+{
+    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= ldb) return;
+    ls_state[b] = (b >= B || is_solution[b] || converged[b]) ? 2 : 0;
+    eta[b] = s_max;
+}
+
+// X' = clamp(X - eta_b G) for the candidates still searching (first trial: every candidate gets a valid X'),
+// Dpart[chunk][b] = sum over the chunk's rows of G (X - X')
+template <typename T>
+__global__ void __launch_bounds__(CTA_THREADS) k_ls_trial(const T *__restrict__ x, const T *__restrict__ G, T *__restrict__ xt,
+                                                         const int8_t *__restrict__ fixed, const uint8_t *__restrict__ ls_state,
+                                                         const double *__restrict__ eta, double *__restrict__ Dpart, int n,
+                                                         int64_t ldb, int first_trial)
+{
+    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= ldb) return;
+    const int st = ls_state[b];
+    const int rows = (n + LS_CHUNKS - 1) / LS_CHUNKS, v0 = blockIdx.y * rows, v1 = min(n, v0 + rows);
+    if (st != 0) {
+        if (first_trial) for (int v = v0; v < v1; ++v) xt[(int64_t)v * ldb + b] = x[(int64_t)v * ldb + b];
+        return;
+    }
+    const T e = (T)eta[b];
+    double D = 0.0;
+    for (int v = v0; v < v1; ++v) {
+        const T xv = x[(int64_t)v * ldb + b];
+        T nx = xv;
+        if (!fixed[v]) {
+            const T g = G[(int64_t)v * ldb + b];
+            nx = fma_(-e, g, xv);
+            nx = nx > T(1) ? T(1) : nx;
+            nx = nx < T(-1) ? T(-1) : nx;
+            D += (double)g * (double)(xv - nx);
+        }
+        xt[(int64_t)v * ldb + b] = nx;
+    }
+    Dpart[(int64_t)blockIdx.y * ldb + b] = D;
+}
+
+// Armijo test of the trial; backtrack or give up (eta < delta: converged)
+template <typename T>
+__global__ void k_ls_decide(int B, int64_t ldb, const T *__restrict__ F0, const T *__restrict__ F1, const double *__restrict__ Dpart,
+                            uint8_t *__restrict__ ls_state, double *__restrict__ eta, uint8_t *__restrict__ converged, double c1,
+                            double beta, double delta)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= B || ls_state[b] != 0) return;
+    double D = 0.0;
+    for (int c = 0; c < LS_CHUNKS; ++c) D += Dpart[(int64_t)c * ldb + b];
+    if ((double)F1[b] <= (double)F0[b] - c1 * D) { ls_state[b] = 1; return; }
+    const double e = eta[b] * beta;
+    eta[b] = e;
+    if (e < delta) { ls_state[b] = 2; converged[b] = 1; }
+}
+
+// accepted candidates take X', sign bits of the resulting X for everyone
+template <typename T>
+__global__ void __launch_bounds__(CTA_THREADS) k_ls_commit(T *__restrict__ x, const T *__restrict__ xt, const uint8_t *__restrict__ ls_state,
+                                                          uint32_t *__restrict__ bits, int n, int B, int64_t ldb)
+{
+    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= ldb) return;                                             // whole warps (ldb % 32 == 0)
+    const bool live = b < B, take = live && ls_state[b] == 1;
+    const int64_t ldw = ldb >> 5;
+    for (int v = blockIdx.y; v < n; v += gridDim.y) {
+        T xv = T(0);
+        if (live) {
+            xv = take ? xt[(int64_t)v * ldb + b] : x[(int64_t)v * ldb + b];
+            if (take) x[(int64_t)v * ldb + b] = xv;
+        }
+        const uint32_t w = __ballot_sync(0xffffffffu, live && xv < T(0));
+        if ((threadIdx.x & 31) == 0) bits[(int64_t)v * ldw + (b >> 5)] = w;
+    }
+}
+
+template <typename T>
+__global__ void k_ls_report(int B, const double *__restrict__ eta, T *__restrict__ eta_out)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b < B) eta_out[b] = (T)eta[b];
+}
+
 // zero the padding columns [B, ldb) of a caller-owned gradient (vector REDs of a lane pair that
 // straddles B spill into them)
 template <typename T>
@@ -1365,10 +1465,11 @@ __global__ void k_zero_pad(T *__restrict__ G, int n, int B, int64_t ldb)
 
 // ---- F[b] = sum over items of Fpart[item][b], fixed order, accumulated in double ------------
 template <typename T>
-__global__ void k_reduce_F(const T *__restrict__ Fpart, int n_rows, int64_t ldb, int B, T *__restrict__ F)
+__global__ void k_reduce_F(const T *__restrict__ Fpart, int n_rows, int64_t ldb, int B, T *__restrict__ F,
+                           const uint8_t *__restrict__ skip)
 {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= B) return;
+    if (b >= B || (skip && skip[b])) return;                           // skipped candidates keep their F
     double s = 0.0;
     for (int i = 0; i < n_rows; ++i) s += (double)Fpart[(int64_t)i * ldb + b];
     F[b] = (T)s;

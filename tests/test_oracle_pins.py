@@ -371,6 +371,101 @@ def test_step_composition_and_freeze(with_fixed):
     assert np.array_equal(Xb, Xo) and np.array_equal(solb, solo) and np.array_equal(firstb, firsto)
 
 
+# ---------------------------------------------------------------- O11: Alg. 1 with line search (reading B5)
+def _ls_recompose(inst, X0, B, T, s_max, beta, c1, delta, J):
+    """oracle.step_ls recomposed from eval_grad / check and numpy long doubles."""
+    X = X0.copy()
+    sol = np.zeros(B, dtype=bool); conv = np.zeros(B, dtype=bool)
+    first = np.full(B, -1); eta_last = np.full(B, s_max, dtype=np.longdouble)
+    free = np.ones(inst.n_vars, dtype=bool) if inst.fixed is None else (inst.fixed == 0)
+    accepted_etas = [[] for _ in range(B)]
+    for t in range(1, T + 1):
+        F0, G = O.eval_grad(inst, X, B)
+        for b in range(B):
+            if sol[b] or conv[b]:
+                continue
+            eta = np.longdouble(s_max)
+            x0 = X[:, b].astype(np.longdouble); g = G[:, b].astype(np.longdouble)
+            for _ in range(J):
+                xt = np.where(free, np.clip(x0 - eta * g, -1, 1), x0)
+                D = np.sum(g * (x0 - xt))
+                Xt = X[:, b:b + 1].copy(); Xt[:, 0] = xt.astype(np.float64)
+                F1 = O.eval_grad(inst, np.ascontiguousarray(Xt), 1, grad=False)[0]
+                if F1 <= F0[b] - c1 * D:
+                    X[:, b] = xt.astype(np.float64); accepted_etas[b].append(float(eta))
+                    break
+                eta = eta * beta
+                if eta < delta:
+                    conv[b] = True
+                    break
+            eta_last[b] = eta
+        sat, _ = O.check(inst, X, B)
+        newly = (sat == inst.n_cons) & ~sol & ~conv
+        # a candidate that converged in this very step is still checked (Alg. 1 checks X(t) every step)
+        newly |= (sat == inst.n_cons) & ~sol
+        first[newly] = t
+        sol |= newly
+    return X, sol, conv, first, eta_last, accepted_etas
+
+
+@pytest.mark.parametrize("with_fixed", [False, True])
+def test_step_ls_composition(with_fixed):
+    """oracle.step_ls == Alg. 1 with backtracking (reading B5) recomposed from eval_grad / check."""
+    base = I.make_mixed(n=20, m=26, kmin=2, kmax=4, seed=41, batch=12, with_fixed=with_fixed,
+                        types=[R.OR, R.XOR, R.NAE])
+    base.meta["admissible"] = [R.admissible_taus(int(t), int(k), int(p))
+                               for t, k, p in zip(base.ctype, base.lengths(), base.param)]
+    inst, _ = I.plant_solution(base, seed=5)
+    B, T = 12, 12
+    kw = dict(s_max=2.0, beta=0.5, c1=1e-4, delta=1e-3, max_trials=6)
+    X0 = I.make_x0(inst, seed=3, batch=B, dtype=np.float64)
+    Xo, Fo, etao, sato, solo, firsto, convo, margin = O.step_ls(inst, X0, T, B, **kw)
+    X, sol, conv, first, eta_last, _ = _ls_recompose(inst, X0, B, T, kw["s_max"], kw["beta"], kw["c1"], kw["delta"],
+                                                     kw["max_trials"])
+    assert np.array_equal(solo.astype(bool), sol) and np.array_equal(firsto, first)
+    assert np.array_equal(convo.astype(bool), conv)
+    assert np.max(np.abs(Xo - X)) < 1e-13
+    assert np.array_equal(sato, O.check(inst, Xo, B)[0])
+    assert np.max(np.abs(Fo - O.eval_grad(inst, Xo, B, grad=False))) < 1e-12
+    assert np.all(np.abs(Xo[:, :B]) <= 1.0)
+    # resume: T steps == 5 steps + (T - 5) resumed steps
+    Xa, _, _, _, sola, firsta, conva, _ = O.step_ls(inst, X0, 5, B, **kw)
+    Xb, _, _, _, solb, firstb, convb, _ = O.step_ls(inst, Xa, T - 5, B, step_base=5, state=(sola, firsta, conva), **kw)
+    assert np.array_equal(Xb, Xo) and np.array_equal(solb, solo) and np.array_equal(firstb, firsto)
+    assert np.array_equal(convb, convo)
+
+
+def test_step_ls_textbook_properties():
+    """What the Armijo rule along the projection arc guarantees, whatever the constants:
+    F never increases, every accepted step satisfies the sufficient-decrease inequality, eta is on the
+    ladder s_max beta^j, a huge delta freezes everything at once, and with beta-ladder exhausted (one
+    trial, absurd s_max) X stays put when the single trial is rejected."""
+    inst = I.make_mixed(n=30, m=60, kmin=2, kmax=6, seed=77, batch=16, types=[R.OR, R.XOR, R.ATLEAST, R.NAE])
+    B = 16
+    X0 = I.make_x0(inst, seed=8, batch=B, dtype=np.float64)
+    F_prev = O.eval_grad(inst, X0, B, grad=False)
+    X = X0
+    state = None
+    for t in range(6):
+        Xn, F, eta, sat, sol, first, conv, margin = O.step_ls(inst, X, 1, B, s_max=4.0, beta=0.5, c1=1e-3, delta=1e-9,
+                                                              max_trials=40, step_base=t, state=state)
+        assert np.all(F <= F_prev + 1e-15)                            # monotone descent
+        ladder = np.log2(4.0 / eta)
+        assert np.all(np.abs(ladder - np.round(ladder)) < 1e-12) and np.all(eta <= 4.0)
+        moved = np.any(Xn != X, axis=0)[:B]
+        _, G = O.eval_grad(inst, X, B)
+        D = np.sum(G[:, :B] * (X[:, :B] - Xn[:, :B]), axis=0)
+        assert np.all(F[moved] <= F_prev[moved] - 1e-3 * D[moved] + 1e-15)   # sufficient decrease where it moved
+        assert np.all(D[moved] >= 0)
+        X, F_prev, state = Xn, F, (sol, first, conv)
+    # delta above s_max * beta: the first rejection converges the candidate; accepted ones still move
+    Xn, F, eta, sat, sol, first, conv, _ = O.step_ls(inst, X0, 3, B, s_max=64.0, beta=0.5, c1=0.5, delta=40.0, max_trials=5)
+    assert np.all(conv[np.all(Xn == X0, axis=0)[:B] & (sol == 0)] == 1)
+    assert np.all(np.abs(Xn) <= 1.0)
+    with pytest.raises(ValueError):
+        O.step_ls(inst, X0, 1, B, beta=1.5)
+
+
 def test_rejects_bad_input():
     inst = I.make_mixed(n=10, m=5, kmin=2, kmax=4, seed=1, batch=2)
     X = I.make_x0(inst, batch=2, dtype=np.float64)
