@@ -290,6 +290,24 @@ def run_ours(args):
         ctx.step_host(hx, inst.eta, 1, want_F=True)
     barrier()
     t_e2e = time.perf_counter() - w0
+    # ---- optional: Alg. 1 with the line search (afsat_step_ls), reported beside the headline ---------
+    t_ls = None
+    if args.line_search:
+        xl = torch.from_numpy(x0).cuda()
+        ls_kw = dict(s_max=1.0, beta=0.5, c1=1e-4, delta=1e-6, max_trials=args.ls_trials)
+        ls_state = None
+        for t in range(max(W, 1)):
+            *_, s_, f_, c_ = ctx.step_ls(xl, 1, step_base=t, state=ls_state, want_F=False, **ls_kw)
+            ls_state = (s_, f_, c_)
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for t in range(K):
+            *_, s_, f_, c_ = ctx.step_ls(xl, 1, step_base=W + t, state=ls_state, want_F=False, **ls_kw)
+            ls_state = (s_, f_, c_)
+        e1.record(stream)
+        barrier()
+        t_ls = e0.elapsed_time(e1) * 1e-3
     esz = 4 if dtype == 32 else 8
     h2d = n * ldb * esz
     d2h = n * ldb * esz + B * (esz + 4 + 1 + 4)
@@ -330,6 +348,10 @@ def run_ours(args):
                 "roofline": roof, "cpu_baseline": cb,
                 "value_l2_warm": world * m * B * K / t_warm, "ms_per_step_l2_warm": 1e3 * t_warm / K,
                 "solved_candidates": int(sol.sum().item()), "wall_s_timed_region": wall}
+        if t_ls is not None:
+            line["line_search"] = {"ms_per_step": 1e3 * t_ls / K, "max_trials": args.ls_trials,
+                                   "note": "afsat_step_ls: 1 FE+grad evaluation + max_trials objective-only "
+                                           "evaluations of the candidates still searching, per step (L2 warm)"}
         print(json.dumps(line), flush=True)
     ctx.close()
     if world > 1:
@@ -348,6 +370,8 @@ def main():
     ap.add_argument("--dtype", type=int, default=32, choices=[32, 64])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--oracle-seconds", type=float, default=15.0)
+    ap.add_argument("--line-search", action="store_true", help="also time afsat_step_ls (Alg. 1 with line search)")
+    ap.add_argument("--ls-trials", type=int, default=4)
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
