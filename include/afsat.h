@@ -56,7 +56,9 @@ enum afsat_error {
     AFSAT_E_DUPLICATE   = -5,  /* the same variable twice in one constraint (FE is multilinear)   */
     AFSAT_E_PARAM       = -6,  /* ATLEAST/ATMOST/EXACTLY with param < 0 or > k; XOR param not 0/1 */
     AFSAT_E_NOMEM       = -7,
-    AFSAT_E_CUDA        = -8   /* no device / CUDA runtime error (text in afsat_last_error)       */
+    AFSAT_E_CUDA        = -8,  /* no device / CUDA runtime error (text in afsat_last_error)       */
+    AFSAT_E_UNSAT       = -9   /* afsat_parse: the file is unsatisfiable on its face (contradictory
+                                  unit assignments, a threshold no assignment can meet)           */
 };
 
 #define AFSAT_MAX_LEN 64       /* the paper's practical ceiling is ~50 literals    */
@@ -196,6 +198,40 @@ int64_t afsat_query(const afsat_ctx *ctx, int32_t key);
  * records per launch, so it is off by default and off in every timed headline region.
  */
 int afsat_set_profiling(afsat_ctx *ctx, int32_t on);
+
+/*
+ * Problem ingestion (HOST ONLY; App. A, simplifications :300-309 A.1; SURVEY.md §8(f)
+ * NEXT #2).  afsat_parse reads a DIMACS CNF file or the paper's DIMACS-like hybrid PB format from
+ * memory (text[0..len), need not be NUL-terminated) and returns an opaque afsat_problem holding what
+ * afsat_create consumes.  Grammar: comment lines start with 'c' or '*'; 'p cnf <vars> <constraints>';
+ * a constraint is  ['h'] [<id> [<threshold>]] <lit>+ 0  with <id> in { (none): disjunction,
+ * x|xor: odd parity, n|nae: not all equal, a|amo: at most one, e|eo: exactly one, k|ek <int>: exactly
+ * k, d|card [<|<=|>|>=]<int>: cardinality; a bare card threshold k means >= k if k > 0, < |k| if k < 0 }.
+ * A literal l is variable |l| (1-based in the file, 0-based in the arrays) and is true iff that
+ * variable is True (l > 0) or False (l < 0): lit_sign = +1 / -1.
+ * Simplifications applied while reading (A.1): unit disjunction / unit eo -> prefix assignment; unit amo
+ * discarded; card >= 1 -> disjunction; ek 1 = eo; card >= n and ek n -> all literals assigned true;
+ * card >= 0 discarded; ek 0 -> all literals assigned false.  Also (reading B6): a literal
+ * repeated in a disjunction is kept once, a disjunction with l and -l is discarded, a repeated variable
+ * elsewhere is AFSAT_E_DUPLICATE; at-most thresholds >= the length are discarded, at-most 0 assigns all
+ * literals false; contradictory assignments and unmeetable thresholds are AFSAT_E_UNSAT.
+ * n_vars = max(declared <vars>, largest variable used).  The prefix assignments come back as
+ * fixed[v] in {0 free, -1 True, +1 False} (the partial-assignment mask of afsat_create).
+ *   afsat_problem_sizes: stats (may be NULL) receives 5 values {constraints read, variables assigned
+ *     by unit extraction, constraints discarded, declared vars, declared constraints (summed over p lines)}.
+ *   afsat_problem_fill: copies into caller-owned HOST arrays row_ptr[m+1], lit_var[nnz], lit_sign[nnz],
+ *     type[m], param[m], fixed[n_vars].
+ *   afsat_parse_error: message of the last failing afsat_parse / afsat_parse_file on this thread.
+ */
+typedef struct afsat_problem afsat_problem;
+#define AFSAT_PARSE_MAX_VARS 0x3FFFFFFF
+int afsat_parse(const char *text, int64_t len, afsat_problem **out);
+int afsat_parse_file(const char *path, afsat_problem **out);
+const char *afsat_parse_error(void);
+int afsat_problem_sizes(const afsat_problem *p, int32_t *n_vars, int32_t *n_cons, int64_t *nnz, int64_t *stats);
+int afsat_problem_fill(const afsat_problem *p, int64_t *row_ptr, int32_t *lit_var, int8_t *lit_sign,
+                       uint8_t *type, int32_t *param, int8_t *fixed);
+void afsat_problem_free(afsat_problem *p);
 
 const char *afsat_version(void);
 

@@ -24,11 +24,12 @@ Q_KERNEL_LAUNCHES, Q_NUM_SIGNATURES, Q_NUM_BUCKETS, Q_NNZ, Q_WORKSPACE_BYTES, Q_
 
 ERROR_NAMES = {0: "AFSAT_OK", -1: "AFSAT_E_INVALID", -2: "AFSAT_E_LENGTH", -3: "AFSAT_E_VARIABLE",
                -4: "AFSAT_E_SIGN", -5: "AFSAT_E_DUPLICATE", -6: "AFSAT_E_PARAM",
-               -7: "AFSAT_E_NOMEM", -8: "AFSAT_E_CUDA"}
+               -7: "AFSAT_E_NOMEM", -8: "AFSAT_E_CUDA", -9: "AFSAT_E_UNSAT"}
 
 EXPORTS = ["afsat_create", "afsat_destroy", "afsat_last_error", "afsat_eval_grad", "afsat_check",
            "afsat_step", "afsat_step_host", "afsat_host_tables", "afsat_query", "afsat_version",
-           "afsat_set_profiling", "afsat_step_ls"]
+           "afsat_set_profiling", "afsat_step_ls", "afsat_parse", "afsat_parse_file", "afsat_parse_error",
+           "afsat_problem_sizes", "afsat_problem_fill", "afsat_problem_free"]
 
 
 class AfsatError(RuntimeError):
@@ -69,6 +70,18 @@ def load_library():
     L.afsat_query.argtypes = [vp, i32]
     L.afsat_set_profiling.restype = C.c_int
     L.afsat_set_profiling.argtypes = [vp, i32]
+    L.afsat_parse.restype = C.c_int
+    L.afsat_parse.argtypes = [C.c_char_p, i64, C.POINTER(vp)]
+    L.afsat_parse_file.restype = C.c_int
+    L.afsat_parse_file.argtypes = [C.c_char_p, C.POINTER(vp)]
+    L.afsat_parse_error.restype = C.c_char_p
+    L.afsat_parse_error.argtypes = []
+    L.afsat_problem_sizes.restype = C.c_int
+    L.afsat_problem_sizes.argtypes = [vp, vp, vp, vp, vp]
+    L.afsat_problem_fill.restype = C.c_int
+    L.afsat_problem_fill.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+    L.afsat_problem_free.restype = None
+    L.afsat_problem_free.argtypes = [vp]
     L.afsat_version.restype = C.c_char_p
     L.afsat_version.argtypes = []
     _lib = L
@@ -88,6 +101,60 @@ def host_tables(ctype: int, k: int, param: int, flags: int = 0):
     if rc < 0:
         raise AfsatError(rc, "afsat_host_tables")
     return tab[:rc].copy(), int(n_real.value)
+
+
+class Problem:
+    """What afsat_parse produced: the CSR constraint table and the partial-assignment mask (numpy)."""
+
+    def __init__(self, n_vars, row_ptr, lit_var, lit_sign, ctype, param, fixed, stats):
+        self.n_vars, self.row_ptr, self.lit_var, self.lit_sign = n_vars, row_ptr, lit_var, lit_sign
+        self.ctype, self.param, self.fixed, self.stats = ctype, param, fixed, stats
+        self.n_cons = int(row_ptr.shape[0] - 1)
+
+    def context(self, *, batch, dtype=32, device=0, flags=0, ldb=None):
+        return Context(self.n_vars, self.row_ptr, self.lit_var, self.lit_sign, self.ctype, self.param,
+                       self.fixed, batch=batch, ldb=ldb, dtype=dtype, device=device, flags=flags)
+
+
+def _take_problem(L, rc, h):
+    if rc != 0:
+        raise AfsatError(rc, L.afsat_parse_error().decode())
+    try:
+        n, m, nnz = C.c_int32(0), C.c_int32(0), C.c_int64(0)
+        stats = np.zeros(5, dtype=np.int64)
+        L.afsat_problem_sizes(h, C.addressof(n), C.addressof(m), C.addressof(nnz), stats.ctypes.data)
+        row_ptr = np.zeros(m.value + 1, dtype=np.int64)
+        lit_var = np.zeros(nnz.value, dtype=np.int32)
+        lit_sign = np.zeros(nnz.value, dtype=np.int8)
+        ctype = np.zeros(m.value, dtype=np.uint8)
+        param = np.zeros(m.value, dtype=np.int32)
+        fixed = np.zeros(n.value, dtype=np.int8)
+        rc = L.afsat_problem_fill(h, row_ptr.ctypes.data, lit_var.ctypes.data if nnz.value else None,
+                                  lit_sign.ctypes.data if nnz.value else None,
+                                  ctype.ctypes.data if m.value else None, param.ctypes.data if m.value else None,
+                                  fixed.ctypes.data)
+        if rc != 0:
+            raise AfsatError(rc, "afsat_problem_fill")
+        names = ("constraints_read", "variables_assigned", "constraints_discarded", "declared_vars", "declared_constraints")
+        return Problem(int(n.value), row_ptr, lit_var, lit_sign, ctype, param, fixed, dict(zip(names, stats.tolist())))
+    finally:
+        L.afsat_problem_free(h)
+
+
+def parse(text) -> Problem:
+    """afsat_parse: DIMACS CNF / hybrid PB text (str or bytes) -> Problem.  Host only."""
+    L = load_library()
+    data = text.encode() if isinstance(text, str) else bytes(text)
+    h = C.c_void_p(None)
+    rc = L.afsat_parse(data, len(data), C.byref(h))
+    return _take_problem(L, rc, h)
+
+
+def parse_file(path) -> Problem:
+    L = load_library()
+    h = C.c_void_p(None)
+    rc = L.afsat_parse_file(str(path).encode(), C.byref(h))
+    return _take_problem(L, rc, h)
 
 
 def _np_ptr(a):

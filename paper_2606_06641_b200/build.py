@@ -17,7 +17,7 @@ LIB = PKG / "libafsat_b200.so"
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 
 SOURCES_CU = [CSRC / "afsat.cu"]
-SOURCES_CPP = [CSRC / "precompute.cpp"]
+SOURCES_CPP = [CSRC / "precompute.cpp", CSRC / "parser.cpp"]
 DEPS = [CSRC / "afsat_kernels.cuh", CSRC / "afsat_internal.h", PKG.parent / "include" / "afsat.h"]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
