@@ -33,8 +33,21 @@ thread_local std::string g_create_error;
 
 // length classes: register kernels for k in [1,8] and [9,16] (one launch each, one separately compiled
 // body per length), shared-memory kernel for [17,64]
-enum { CLS_A = 0, CLS_B = 1, CLS_LONG = 2, N_CLS = 3 };
-inline int class_of(int k) { return k <= 8 ? CLS_A : k <= 16 ? CLS_B : CLS_LONG; }
+// fp32 only: the shortest constraints (k <= AFSAT_S_KMAX) run FOUR candidates per lane (two packed pairs): their
+// launches are issue-bound on per-constraint overhead (literal and table loads, addresses, sign masks), which
+// a lane then pays once per four candidates; their bodies are small enough for it at 128 registers
+#ifndef AFSAT_S_KMAX
+#define AFSAT_S_KMAX 4
+#endif
+#if defined(AFSAT_NO_FFMA2) || AFSAT_A_V < 2
+#undef AFSAT_S_KMAX
+#define AFSAT_S_KMAX 0
+#endif
+enum { CLS_S = 0, CLS_A = 1, CLS_B = 2, CLS_LONG = 3, N_CLS = 4 };
+inline int class_of(int k, int dtype)
+{
+    return (dtype == 32 && k <= AFSAT_S_KMAX) ? CLS_S : k <= 8 ? CLS_A : k <= 16 ? CLS_B : CLS_LONG;
+}
 
 struct ClassGeom {              // how one length class maps candidates onto a CTA
     int V = 1;                  // candidates per lane
@@ -75,8 +88,8 @@ struct afsat_ctx {
     uint8_t *ls_state = nullptr;
     const uint8_t *cur_skip = nullptr;             // candidate mask of the evaluation launches (line-search trials)
     cudaStream_t own_stream = nullptr;
-    cudaStream_t side_stream[N_CLS - 1] = {nullptr, nullptr};       // concurrent launches of the length classes
-    cudaEvent_t ev_fork = nullptr, ev_join[N_CLS - 1] = {nullptr, nullptr};
+    cudaStream_t side_stream[N_CLS - 1] = {};                       // concurrent launches of the length classes
+    cudaEvent_t ev_fork = nullptr, ev_join[N_CLS - 1] = {};
     size_t ws_bytes = 0;
     int64_t launches = 0;
     // afsat_set_profiling: event pairs around the evaluation-kernel launches
@@ -167,6 +180,18 @@ void (*pick_a(bool grad))(EvalParams<T>)
         return grad ? (Fn)k_eval_km<T, 1, 8, VA, true, MB> : (Fn)k_eval_km<T, 1, 8, VA, false, MB>;
 }
 
+// k <= AFSAT_S_KMAX, fp32: the packed kernel with two pairs (four candidates) per lane
+template <typename T, int MB>
+void (*pick_s(bool grad))(EvalParams<T>)
+{
+    using Fn = void (*)(EvalParams<T>);
+#if AFSAT_S_KMAX > 0
+    if constexpr (sizeof(T) == 4) return grad ? (Fn)k_eval_f2m<1, AFSAT_S_KMAX, 2, true, MB> : (Fn)k_eval_f2m<1, AFSAT_S_KMAX, 2, false, MB>;
+    else
+#endif
+        return nullptr;                                                // class S is empty for this dtype / build
+}
+
 // k > 16: KMAX is the unroll bound of the register-blocked kernels; fp32 runs the packed two-candidate form
 inline int long_kmax(int kmax_long) { return kmax_long <= 32 ? 32 : kmax_long <= 40 ? 40 : kmax_long <= 48 ? 48 : kmax_long <= 56 ? 56 : 64; }
 #ifndef AFSAT_LONG_PACKED
@@ -228,7 +253,8 @@ int launch_eval(afsat_ctx *ctx, const T *x, T *G, int64_t g_ld, int64_t g_b0, T 
         if (cls != CLS_LONG) {
             using Fn = void (*)(EvalParams<T>);
             constexpr int MB = sizeof(T) == 4 ? AFSAT_A_MINB : 1;
-            Fn fn = cls == CLS_A ? pick_a<T, VA, MB>(grad)
+            Fn fn = cls == CLS_S ? pick_s<T, MB>(grad)
+                  : cls == CLS_A ? pick_a<T, VA, MB>(grad)
                                  : (grad ? (Fn)k_eval_km<T, 9, 16, 1, true, 1> : (Fn)k_eval_km<T, 9, 16, 1, false, 1>);
             fn<<<grid, block, 0, st>>>(p);
         } else {
@@ -296,7 +322,7 @@ int eval_grad_t(afsat_ctx *ctx, const T *x, T *F, T *G, cudaStream_t st)
         int rc = launch_eval<T>(ctx, x, G, ctx->ldb, 0, F ? (T *)ctx->d_Fpart : nullptr, b0, w, st);
         if (rc) return rc;
     }
-    if (G && ctx->B < ctx->ldb && (ctx->B & 1)) {                     // a lane pair straddles B: clear the spill
+    if (G && ctx->B < ctx->ldb && (ctx->B & 3)) {                     // a lane's candidates straddle B: clear the spill
         k_zero_pad<T><<<std::min(1024, ctx->n), 128, 0, st>>>(G, ctx->n, ctx->B, ctx->ldb);
         ++ctx->launches;
         CU(cudaPeekAtLastError());
@@ -607,10 +633,10 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
     int sm_count = 148;
     ClassGeom geom[N_CLS];
     int kmax_long = 0;
-    for (int32_t j = 0; j < n_cons; ++j) { const int k = sig_k[cons_sig[j]]; if (class_of(k) == CLS_LONG) kmax_long = std::max(kmax_long, k); }
+    for (int32_t j = 0; j < n_cons; ++j) { const int k = sig_k[cons_sig[j]]; if (class_of(k, dtype) == CLS_LONG) kmax_long = std::max(kmax_long, k); }
     for (int cls = 0; cls < N_CLS; ++cls) {
         ClassGeom &g = geom[cls];
-        g.V = (cls == CLS_A && dtype == 32) ? AFSAT_A_V : 1;
+        g.V = (cls == CLS_S) ? 4 : (cls == CLS_A && dtype == 32) ? AFSAT_A_V : 1;
         g.warps = CTA_WARPS;
         if (cls == CLS_LONG) {
             const int km = long_kmax(kmax_long);
@@ -641,7 +667,7 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
             int32_t e = j;
             while (e < n_cons && cons_sig[e] == sg) ++e;
             if (k != last_k) { ++n_buckets; last_k = k; }
-            const int cls = class_of(k);
+            const int cls = class_of(k, dtype);
             while (cur_cls < cls) cls_begin[++cur_cls] = (int32_t)items.size();
             const ClassGeom &g = geom[cls];
             const int64_t tiles_y = (tile_w + (int64_t)32 * g.V * g.Wc - 1) / ((int64_t)32 * g.V * g.Wc);
