@@ -37,7 +37,7 @@ thread_local std::string g_create_error;
 // launches are issue-bound on per-constraint overhead (literal and table loads, addresses, sign masks), which
 // a lane then pays once per four candidates; their bodies are small enough for it at 128 registers
 #ifndef AFSAT_S_KMAX
-#define AFSAT_S_KMAX 4
+#define AFSAT_S_KMAX 5
 #endif
 #if defined(AFSAT_NO_FFMA2) || AFSAT_A_V < 2
 #undef AFSAT_S_KMAX

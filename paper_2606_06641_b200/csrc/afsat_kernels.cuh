@@ -383,6 +383,31 @@ __device__ __forceinline__ void unit_rows_f2(const f32x2 (&y)[K][NP], const f32x
     }
 }
 
+// One generic complex DFT point for all NP pairs of a lane.  With two pairs and k >= AFSAT_F2_SEQ_MINK the
+// pairs are walked one after the other (each keeps 5 k register pairs of factors and prefixes alive).
+#ifndef AFSAT_F2_SEQ_MINK
+#define AFSAT_F2_SEQ_MINK 5
+#endif
+template <int K, int NP, bool GRAD>
+__device__ __forceinline__ void cplx_row_f2(const f32x2 (&y)[K][NP], const f32x2 *__restrict__ r, f32x2 (&fe)[NP], f32x2 (&g)[K][NP])
+{
+    if constexpr (NP == 1 || K < AFSAT_F2_SEQ_MINK) {
+        cplx_points_f2<K, NP, 1, GRAD>(y, r, fe, g);
+    } else {
+#pragma unroll
+        for (int q = 0; q < NP; ++q) {
+            f32x2 y1[K][1], g1[K][1], fe1[1];
+#pragma unroll
+            for (int i = 0; i < K; ++i) { y1[i][0] = y[i][q]; g1[i][0] = g[i][q]; }
+            fe1[0] = fe[q];
+            cplx_points_f2<K, 1, 1, GRAD>(y1, r, fe1, g1);
+#pragma unroll
+            for (int i = 0; i < K; ++i) g[i][q] = g1[i][0];
+            fe[q] = fe1[0];
+        }
+    }
+}
+
 // UV (unit variant, chosen once per work item when its table is staged): 0 = generic coefficients in
 // every row; 1 / 2 = standard table whose first rows are the trivial twiddles [w = 1 (UV 1 only)]
 // [w = -1 iff K odd] [w = i iff K = 3 mod 4] (n_real = their number), followed by n_cplx generic complex rows.
@@ -395,7 +420,7 @@ __device__ __forceinline__ void eval_points_f2(const f32x2 (&y)[K][NP], const f3
         const f32x2 *rP = tab, *rM = tab + (HP ? ROW2 : 0), *rI = rM + (HM ? ROW2 : 0);
         if (HP || HM || HI) unit_rows_f2<K, NP, HP, HM, HI, GRAD>(y, rP, rM, rI, fe, g);
         const f32x2 *r = rI + (HI ? ROW2 : 0);
-        for (int p = 0; p < n_cplx; ++p, r += ROW2) cplx_points_f2<K, NP, 1, GRAD>(y, r, fe, g);
+        for (int p = 0; p < n_cplx; ++p, r += ROW2) cplx_row_f2<K, NP, GRAD>(y, r, fe, g);
         return;
     }
     const f32x2 *r = tab;
@@ -425,7 +450,7 @@ __device__ __forceinline__ void eval_points_f2(const f32x2 (&y)[K][NP], const f3
             for (int q = 0; q < NP; ++q) g[0][q] = add2(g[0][q], suf[q]);     // prefix_0 = 1
         }
     }
-    for (int p = 0; p < n_cplx; ++p, r += ROW2) cplx_points_f2<K, NP, 1, GRAD>(y, r, fe, g);   // one of each conjugate pair
+    for (int p = 0; p < n_cplx; ++p, r += ROW2) cplx_row_f2<K, NP, GRAD>(y, r, fe, g);   // one of each conjugate pair
 }
 
 // sign flip by the literal's polarity bit (bit 31 of the packed literal): one LOP3 per value
