@@ -333,7 +333,10 @@ def run_ours(args):
                 "kernel_ms_per_step": kern_ms / K, "kernel_launches_per_step": launches_per_step,
                 "kernel_share_of_step": (kern_ms / K) / (1e3 * t_total / K),
                 "algorithmic_flop_per_step": flop_per_step, "traffic": load_traffic(args.config),
-                "hbm_floor_bytes_per_step": 2 * n * B * esz, "hbm_peak_gbs": peaks["hbm_gbs"]}
+                "hbm_floor_bytes_per_step": 2 * n * B * esz, "hbm_peak_gbs": peaks["hbm_gbs"],
+                "note": "achieved = ALGORITHMIC flop (SURVEY.md App. D: 12 / 4 FP32 instructions per literal at a complex / "
+                        "real DFT point, every retained point) / measured kernel time; the kernels execute fewer "
+                        "instructions than that at the points 1, -1, i (trivial twiddles, DESIGN.md 6.1)"}
         if clocks.get("sm_mhz"):
             roof["frac_at_observed_clock"] = roof["frac"] * peaks["sm_max_mhz"] / clocks["sm_mhz"]
         cb = None

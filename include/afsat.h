@@ -153,6 +153,33 @@ int afsat_step_ls(afsat_ctx *ctx, void *d_x, double s_max, double beta, double c
                   int32_t *d_first_step, uint8_t *d_converged, int32_t *h_any_solved, void *stream);
 
 /*
+ * afsat_restart -- random re-initialisation of candidates (the compiled search is "executed
+ * repeatedly with different random initialisations"; :105-107: fixed variables keep their value for every
+ * candidate, the remainder is random).  For every candidate b with
+ * d_keep == NULL or d_keep[b] == 0:  x[v][b] = the fixed value of v if v is fixed, else
+ *     u(seed, round, v, b) = ((h >> 8) * 2^-23) - 1   in [-1, 1),   exactly representable in fp32,
+ *     h1 = fmix(lo ^ (b * 0x9E3779B9));  h2 = fmix((h1 + v * 0x85EBCA6B) ^ hi);  h = fmix(h2 + round * 0xC2B2AE35),
+ *     lo / hi = low / high 32 bits of seed,  fmix(h): h ^= h >> 16; h *= 0x85EBCA6B; h ^= h >> 13;
+ *     h *= 0xC2B2AE35; h ^= h >> 16   (all arithmetic mod 2^32).
+ * A counter-based generator: the value depends only on (seed, round, v, b), never on launch geometry, so
+ * the CPU oracle reproduces it bit for bit.  Kept candidates (e.g. d_keep = is_solution) are untouched.
+ */
+int afsat_restart(afsat_ctx *ctx, void *d_x, const uint8_t *d_keep, uint64_t seed, uint32_t round, void *stream);
+
+/*
+ * afsat_solve -- the restart loop around afsat_step (Alg. 1): up to max_rounds rounds of
+ * steps_per_round fixed-step iterations each; after a round without a solution every unsolved candidate
+ * is re-initialised by afsat_restart(seed, round = r) and the next round continues the step count
+ * (first_step is the global iteration index).  Stops after the first round in which some candidate is
+ * solved (stop_at_first != 0) or after max_rounds.  X(0) is the caller's d_x (call afsat_restart with
+ * round 0xFFFFFFFF first for a random start).  Synchronises `stream` once per round (reads one flag).
+ * rounds_done (HOST, may be NULL) receives the number of rounds executed.  Outputs as in afsat_step.
+ */
+int afsat_solve(afsat_ctx *ctx, void *d_x, double eta, int32_t steps_per_round, int32_t max_rounds,
+                uint64_t seed, int32_t stop_at_first, void *d_F, int32_t *d_sat_count,
+                uint8_t *d_is_solution, int32_t *d_first_step, int32_t *rounds_done, void *stream);
+
+/*
  * afsat_step_host -- the same as afsat_step (resume = 0, step_base = 0) for HOST buffers: copies
  * h_x [n][ldb] to the device, runs n_steps, copies X, F, sat_count, is_solution, first_step back
  * (any output pointer may be NULL) and synchronises.  Pinned host memory makes the copies

@@ -29,6 +29,8 @@
  *       solved candidates are frozen (Alg. 1 :124-127).
  *   O11 Alg. 1 with its line search (method not given by the paper: DESIGN.md
  *       reading B5 = per-candidate backtracking, Armijo rule along the projection arc): oracle_step_ls.
+ *   O12 random re-initialisation for restarts: oracle_restart, the counter-based
+ *       generator the C ABI header documents, restated here (the one thing both sides must share by value).
  * No DFT, no prefix/suffix products, no blocking, no reordering.
  *
  * Pins (tests/test_oracle_pins.py, `-m "not gpu"`): brute force of Eq. (1) over all 2^k subsets
@@ -429,5 +431,43 @@ int oracle_step_ls(int32_t n, int32_t m, const int64_t *row_ptr, const int32_t *
         free(g); free(xt); free(x0);
     }
     inst_free(&I);
+    return 0;
+}
+
+/*
+ * O12 -- restart initialisation ("executed repeatedly with different random initialisations";
+ * :105-107 fixed variables keep their value in every candidate).  The generator is the one the C ABI
+ * documents (a method-level random draw must be the same numbers on both sides): for candidate b,
+ * variable v, 64-bit seed (lo, hi) and round r, all arithmetic mod 2^32,
+ *     h1 = fmix(lo ^ b*0x9E3779B9);  h2 = fmix((h1 + v*0x85EBCA6B) ^ hi);  h = fmix(h2 + r*0xC2B2AE35);
+ *     x = (h >> 8) * 2^-23 - 1  in [-1, 1)
+ * with fmix the 32-bit avalanche  h ^= h>>16; h *= 0x85EBCA6B; h ^= h>>13; h *= 0xC2B2AE35; h ^= h>>16.
+ * Candidates with keep[b] != 0 are left untouched.
+ */
+static uint32_t avalanche32(uint32_t h)
+{
+    h ^= h >> 16; h *= 0x85EBCA6BU; h ^= h >> 13; h *= 0xC2B2AE35U; h ^= h >> 16;
+    return h;
+}
+
+int oracle_restart(int32_t n, const int8_t *fixed, int32_t B, int64_t ldb, double *X,
+                   const uint8_t *keep, uint64_t seed, uint32_t round)
+{
+    if (n < 1 || B < 0 || ldb < B) return -1;
+    const uint32_t lo = (uint32_t)(seed & 0xFFFFFFFFULL), hi = (uint32_t)(seed >> 32);
+    for (int32_t b = 0; b < B; ++b) {
+        if (keep && keep[b]) continue;
+        for (int32_t v = 0; v < n; ++v) {
+            double val;
+            if (fixed && fixed[v] != 0) val = (double)fixed[v];
+            else {
+                uint32_t h1 = avalanche32(lo ^ ((uint32_t)b * 0x9E3779B9U));
+                uint32_t h2 = avalanche32((h1 + (uint32_t)v * 0x85EBCA6BU) ^ hi);
+                uint32_t h = avalanche32(h2 + round * 0xC2B2AE35U);
+                val = (double)(h >> 8) / 8388608.0 - 1.0;
+            }
+            X[(int64_t)v * ldb + b] = val;
+        }
+    }
     return 0;
 }

@@ -43,7 +43,7 @@ def lib():
         L = C.CDLL(str(_LIB))
         L.oracle_num_threads.restype = C.c_int
         for name in ("oracle_truth_table", "oracle_coeffs", "oracle_fe_single",
-                     "oracle_eval_grad", "oracle_check", "oracle_step", "oracle_step_ls"):
+                     "oracle_eval_grad", "oracle_check", "oracle_step", "oracle_step_ls", "oracle_restart"):
             getattr(L, name).restype = C.c_int
         _lib = L
     return _lib
@@ -186,3 +186,34 @@ def step_ls(inst, X, n_steps: int, B=None, *, s_max: float = 1.0, beta: float = 
     if rc:
         raise ValueError(f"oracle_step_ls rc={rc}")
     return X, F, eta, sat, sol, first, conv, margin
+
+
+def restart(inst, X, seed: int, round_: int, B=None, *, keep=None):
+    """Counter-based uniform re-initialisation (oracle_restart); returns a new X."""
+    B = int(X.shape[1] if B is None else B)
+    X = _check_x(inst, X, B).copy()
+    fixed = None if inst.fixed is None else np.ascontiguousarray(inst.fixed, dtype=np.int8)
+    keep = None if keep is None else np.ascontiguousarray(keep, dtype=np.uint8)
+    rc = lib().oracle_restart(C.c_int32(inst.n_vars), _p(fixed, C.c_int8), C.c_int32(B), C.c_int64(X.shape[1]),
+                              _p(X, C.c_double), _p(keep, C.c_uint8), C.c_uint64(seed), C.c_uint32(round_ & 0xFFFFFFFF))
+    if rc:
+        raise ValueError(f"oracle_restart rc={rc}")
+    return X
+
+
+def solve(inst, X, eta: float, steps_per_round: int, max_rounds: int, seed: int, B=None, *, stop_at_first=True):
+    """The restart loop of afsat_solve recomposed from step / restart.  Returns (X, sat, sol, first, rounds)."""
+    B = int(X.shape[1] if B is None else B)
+    state = None
+    r = 0
+    sat = None
+    while r < max_rounds:
+        X, _, sat, sol, first = step(inst, X, eta, steps_per_round, B, step_base=r * steps_per_round, state=state,
+                                     want_F=False)
+        state = (sol, first)
+        any_now = bool(np.any((first > r * steps_per_round)))
+        r += 1
+        if (any_now and stop_at_first) or r == max_rounds:
+            break
+        X = restart(inst, X, seed, r - 1, B, keep=sol)
+    return X, sat, state[0], state[1], r

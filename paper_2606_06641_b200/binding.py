@@ -29,7 +29,7 @@ ERROR_NAMES = {0: "AFSAT_OK", -1: "AFSAT_E_INVALID", -2: "AFSAT_E_LENGTH", -3: "
 EXPORTS = ["afsat_create", "afsat_destroy", "afsat_last_error", "afsat_eval_grad", "afsat_check",
            "afsat_step", "afsat_step_host", "afsat_host_tables", "afsat_query", "afsat_version",
            "afsat_set_profiling", "afsat_step_ls", "afsat_parse", "afsat_parse_file", "afsat_parse_error",
-           "afsat_problem_sizes", "afsat_problem_fill", "afsat_problem_free"]
+           "afsat_problem_sizes", "afsat_problem_fill", "afsat_problem_free", "afsat_restart", "afsat_solve"]
 
 
 class AfsatError(RuntimeError):
@@ -62,6 +62,10 @@ def load_library():
     L.afsat_step.argtypes = [vp, vp, dbl, i32, i32, i32, vp, vp, vp, vp, vp, vp]
     L.afsat_step_ls.restype = C.c_int
     L.afsat_step_ls.argtypes = [vp, vp, dbl, dbl, dbl, dbl, i32, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp]
+    L.afsat_restart.restype = C.c_int
+    L.afsat_restart.argtypes = [vp, vp, vp, C.c_uint64, u32, vp]
+    L.afsat_solve.restype = C.c_int
+    L.afsat_solve.argtypes = [vp, vp, dbl, i32, i32, C.c_uint64, i32, vp, vp, vp, vp, vp, vp]
     L.afsat_step_host.restype = C.c_int
     L.afsat_step_host.argtypes = [vp, vp, dbl, i32, vp, vp, vp, vp]
     L.afsat_host_tables.restype = C.c_int
@@ -307,6 +311,30 @@ class Context:
                                    sol.data_ptr(), first.data_ptr(), conv.data_ptr(), hp, _stream_ptr(stream))
         self._raise(rc)
         return F, eta, sat, sol, first, conv
+
+    def restart(self, x, seed, round_, *, keep=None, stream=None):
+        """Counter-based uniform re-initialisation of the candidates with keep[b] == 0 (afsat_restart)."""
+        self._check_x(x)
+        rc = self._L.afsat_restart(self._h, x.data_ptr(), keep.data_ptr() if keep is not None else None,
+                                   int(seed), int(round_) & 0xFFFFFFFF, _stream_ptr(stream))
+        self._raise(rc)
+        return x
+
+    def solve(self, x, eta, steps_per_round, max_rounds, seed, *, stop_at_first=True, want_F=True, stream=None):
+        """The restart loop around step (afsat_solve).  Returns (F, sat_count, is_solution, first_step, rounds)."""
+        import torch
+        self._check_x(x)
+        dev = x.device
+        F = torch.empty(self.B, dtype=x.dtype, device=dev) if want_F else None
+        sat = torch.empty(self.B, dtype=torch.int32, device=dev)
+        sol = torch.empty(self.B, dtype=torch.uint8, device=dev)
+        first = torch.empty(self.B, dtype=torch.int32, device=dev)
+        rounds = C.c_int32(0)
+        rc = self._L.afsat_solve(self._h, x.data_ptr(), float(eta), int(steps_per_round), int(max_rounds), int(seed),
+                                 1 if stop_at_first else 0, F.data_ptr() if F is not None else None, sat.data_ptr(),
+                                 sol.data_ptr(), first.data_ptr(), C.addressof(rounds), _stream_ptr(stream))
+        self._raise(rc)
+        return F, sat, sol, first, int(rounds.value)
 
     def step_host(self, h_x, eta, n_steps, *, want_F=True):
         """End-to-end call on HOST buffers (numpy or pinned torch CPU tensors), synchronous.

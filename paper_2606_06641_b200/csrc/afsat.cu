@@ -865,6 +865,51 @@ int afsat_step_ls(afsat_ctx *ctx, void *d_x, double s_max, double beta, double c
                                    d_eta, d_sat_count, d_is_solution, d_first_step, d_converged, h_dev, st);
 }
 
+int afsat_restart(afsat_ctx *ctx, void *d_x, const uint8_t *d_keep, uint64_t seed, uint32_t round, void *stream)
+{
+    if (!ctx) return AFSAT_E_INVALID;
+    if (!d_x) return fail(ctx, AFSAT_E_INVALID, "afsat_restart: NULL pointer");
+    int rc = set_device(ctx);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const unsigned gx = (unsigned)((ctx->B + CTA_THREADS - 1) / CTA_THREADS);
+    const unsigned gy = (unsigned)std::min<int64_t>(ctx->n, std::max<int64_t>(1, (int64_t)ctx->sm_count * 8 / gx));
+    const uint32_t lo = (uint32_t)(seed & 0xFFFFFFFFull), hi = (uint32_t)(seed >> 32);
+    if (ctx->dtype == 32)
+        k_restart<float><<<dim3(gx, gy), CTA_THREADS, 0, st>>>((float *)d_x, ctx->d_fixed, d_keep, lo, hi, round, ctx->n, ctx->B, ctx->ldb);
+    else
+        k_restart<double><<<dim3(gx, gy), CTA_THREADS, 0, st>>>((double *)d_x, ctx->d_fixed, d_keep, lo, hi, round, ctx->n, ctx->B, ctx->ldb);
+    ++ctx->launches;
+    CU(cudaPeekAtLastError());
+    return AFSAT_OK;
+}
+
+int afsat_solve(afsat_ctx *ctx, void *d_x, double eta, int32_t steps_per_round, int32_t max_rounds, uint64_t seed,
+                int32_t stop_at_first, void *d_F, int32_t *d_sat_count, uint8_t *d_is_solution, int32_t *d_first_step,
+                int32_t *rounds_done, void *stream)
+{
+    if (!ctx) return AFSAT_E_INVALID;
+    if (!d_x || !d_sat_count || !d_is_solution || !d_first_step) return fail(ctx, AFSAT_E_INVALID, "afsat_solve: NULL pointer");
+    if (steps_per_round < 1 || max_rounds < 1) return fail(ctx, AFSAT_E_INVALID, "afsat_solve: steps_per_round and max_rounds must be >= 1");
+    cudaStream_t st = (cudaStream_t)stream;
+    int r = 0;
+    for (; r < max_rounds; ++r) {
+        const bool last = r + 1 == max_rounds;
+        int rc = afsat_step(ctx, d_x, eta, steps_per_round, r * steps_per_round, r > 0, nullptr, d_sat_count, d_is_solution,
+                            d_first_step, nullptr, stream);
+        if (rc) return rc;
+        int32_t any[2] = {0, -1};
+        CU(cudaMemcpyAsync(any, ctx->d_any, sizeof any, cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+        if ((any[0] && stop_at_first) || last) { ++r; break; }
+        rc = afsat_restart(ctx, d_x, d_is_solution, seed, (uint32_t)r, stream);
+        if (rc) return rc;
+    }
+    if (rounds_done) *rounds_done = r;
+    if (d_F) return afsat_eval_grad(ctx, d_x, d_F, nullptr, stream);
+    return AFSAT_OK;
+}
+
 int afsat_step_host(afsat_ctx *ctx, void *h_x, double eta, int32_t n_steps, void *h_F, int32_t *h_sat_count,
                     uint8_t *h_is_solution, int32_t *h_first_step)
 {

@@ -1478,6 +1478,33 @@ __global__ void k_ls_report(int B, const double *__restrict__ eta, T *__restrict
     if (b < B) eta_out[b] = (T)eta[b];
 }
 
+// ---- afsat_restart: counter-based uniform re-initialisation (include/afsat.h states the generator) ----
+__device__ __forceinline__ uint32_t fmix32(uint32_t h)
+{
+    h ^= h >> 16; h *= 0x85EBCA6Bu; h ^= h >> 13; h *= 0xC2B2AE35u; h ^= h >> 16;
+    return h;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(CTA_THREADS) k_restart(T *__restrict__ x, const int8_t *__restrict__ fixed,
+                                                        const uint8_t *__restrict__ keep, uint32_t lo, uint32_t hi, uint32_t round,
+                                                        int n, int B, int64_t ldb)
+{
+    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= B || (keep && keep[b])) return;
+    const uint32_t hb = fmix32(lo ^ ((uint32_t)b * 0x9E3779B9u));
+    for (int v = blockIdx.y; v < n; v += gridDim.y) {
+        const int8_t f = fixed[v];
+        T val;
+        if (f) val = (T)f;
+        else {
+            const uint32_t h = fmix32(fmix32((hb + (uint32_t)v * 0x85EBCA6Bu) ^ hi) + round * 0xC2B2AE35u);
+            val = (T)((float)(h >> 8) * 1.1920928955078125e-07f - 1.0f);     // (h >> 8) 2^-23 - 1, exact
+        }
+        x[(int64_t)v * ldb + b] = val;
+    }
+}
+
 // zero the padding columns [B, ldb) of a caller-owned gradient (vector REDs of a lane pair that
 // straddles B spill into them)
 template <typename T>

@@ -410,6 +410,47 @@ def test_step_ls_rejects_bad_parameters():
             ctx.step_ls(x, 1, **bad)
 
 
+# ---- restarts (afsat_restart / afsat_solve) -----------------------------------
+
+@pytest.mark.parametrize("dtype", [32, 64])
+def test_restart_bit_exact(dtype):
+    """Integer generator + exact conversion: the CUDA values equal the oracle's bit for bit; kept candidates
+    and padding columns are untouched, fixed variables hold their value."""
+    inst = I.make_mixed(n=70, m=20, kmin=2, kmax=5, seed=5, batch=300, with_fixed=True)
+    B = 300
+    x0 = I.make_x0(inst, seed=1, batch=B)
+    ctx = Bd.Context.from_instance(inst, batch=B, ldb=x0.shape[1], dtype=dtype)
+    x = dev(x0.astype(np.float32 if dtype == 32 else np.float64))
+    keep = (np.arange(B) % 5 == 1).astype(np.uint8)
+    ctx.restart(x, 0xDEADBEEFCAFE1234, 9, keep=dev(keep))
+    torch.cuda.synchronize()
+    Xo = O.restart(inst, x0.astype(np.float64), 0xDEADBEEFCAFE1234, 9, B, keep=keep)
+    assert np.array_equal(x.cpu().numpy().astype(np.float64), Xo)
+    ctx.restart(x, 5, 0)
+    assert np.array_equal(x.cpu().numpy().astype(np.float64)[:, :B], O.restart(inst, x0.astype(np.float64), 5, 0, B)[:, :B])
+    assert np.array_equal(x.cpu().numpy()[:, B:], x0[:, B:].astype(x.cpu().numpy().dtype))
+    ctx.close()
+
+
+def test_solve_restart_loop_matches_oracle():
+    """afsat_solve on cfg0 (fp64): rounds of 40 steps with restarts of the unsolved candidates vs the same loop
+    recomposed from the oracle's step / restart: same rounds, solved flags and first-solved steps."""
+    inst = I.make_config(0, instance_seed=6641002)
+    x0 = I.make_x0(inst).astype(np.float64)
+    ctx = Bd.Context.from_instance(inst, dtype=64)
+    for stop in (True, False):
+        x = dev(x0)
+        F, sat, sol, first, rounds = ctx.solve(x, 0.1, 40, 4, 2026, stop_at_first=stop)
+        torch.cuda.synchronize()
+        Xo, sato, solo, firsto, ro = O.solve(inst, x0, 0.1, 40, 4, 2026, inst.batch, stop_at_first=stop)
+        assert rounds == ro
+        assert np.array_equal(sol.cpu().numpy(), solo) and np.array_equal(first.cpu().numpy(), firsto)
+        assert np.array_equal(sat.cpu().numpy(), sato)
+        assert np.abs(x.cpu().numpy()[:, :64] - Xo[:, :64]).max() < 1e-8
+        assert np.all(np.abs(F.cpu().numpy() - O.eval_grad(inst, Xo, inst.batch, grad=False)) < 1e-7)
+    ctx.close()
+
+
 # ---- scaled-down versions of configs 1-4 (several tiles + ragged tails) -----------------------------
 
 @pytest.mark.parametrize("cfg,scale,B", [(1, 0.01, 96), (2, 0.05, 160), (4, 0.002, 96)])

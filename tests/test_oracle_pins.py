@@ -466,6 +466,46 @@ def test_step_ls_textbook_properties():
         O.step_ls(inst, X0, 1, B, beta=1.5)
 
 
+# ---------------------------------------------------------------- O12: restart initialisation
+def test_restart_generator_properties():
+    """The generator is fixed by include/afsat.h; what pins it here: one value worked out by hand-coded
+    integer arithmetic in Python, range [-1, 1) on the 2^-23 grid, uniformity (chi-square), independence of
+    seed / round / candidate / variable streams, fixed variables and kept candidates."""
+    inst = I.make_mixed(n=64, m=10, kmin=2, kmax=4, seed=3, batch=256, with_fixed=True)
+    B = 256
+    X0 = np.zeros((64, 256))
+    Xa = O.restart(inst, X0, seed=0x123456789ABCDEF, round_=3, B=B)
+    # the formula, retyped with Python integers for one (b, v)
+    M = 0xFFFFFFFF
+    def fmix(h):
+        h ^= h >> 16; h = (h * 0x85EBCA6B) & M; h ^= h >> 13; h = (h * 0xC2B2AE35) & M; h ^= h >> 16
+        return h
+    free = np.nonzero(inst.fixed == 0)[0]
+    v, b = int(free[5]), 77
+    lo, hi = 0x123456789ABCDEF & M, 0x123456789ABCDEF >> 32
+    h = fmix((fmix(((fmix(lo ^ ((b * 0x9E3779B9) & M)) + v * 0x85EBCA6B) & M) ^ hi) + 3 * 0xC2B2AE35) & M)
+    assert Xa[v, b] == (h >> 8) / 2.0 ** 23 - 1.0
+    vals = Xa[free][:, :B].ravel()
+    assert vals.min() >= -1.0 and vals.max() < 1.0
+    assert np.all(vals * 2 ** 23 == np.round(vals * 2 ** 23))         # on the fp32-exact grid
+    hist, _ = np.histogram(vals, bins=32, range=(-1, 1))
+    exp = vals.size / 32
+    assert np.sum((hist - exp) ** 2 / exp) < 80                       # chi-square, 31 dof (p ~ 1e-6 at 80)
+    assert abs(vals.mean()) < 0.02
+    fx = inst.fixed != 0
+    assert np.all(Xa[fx][:, :B] == inst.fixed[fx][:, None])           # fixed variables hold their value
+    for other in (O.restart(inst, X0, seed=0x123456789ABCDEF, round_=4, B=B),
+                  O.restart(inst, X0, seed=0x123456789ABCDEE, round_=3, B=B),
+                  O.restart(inst, X0, seed=0x023456789ABCDEF, round_=3, B=B)):
+        assert abs(np.corrcoef(other[free][:, :B].ravel(), vals)[0, 1]) < 0.04   # ~4.5 sigma at 13 000 samples
+    assert abs(np.corrcoef(Xa[free][:, 0], Xa[free][:, 1])[0, 1]) < 0.5
+    assert abs(np.corrcoef(Xa[free[0], :B], Xa[free[1], :B])[0, 1]) < 0.2
+    keep = (np.arange(B) % 3 == 0).astype(np.uint8)
+    Xk = O.restart(inst, X0 + 0.25, seed=7, round_=0, B=B, keep=keep)
+    assert np.all(Xk[:, :B][:, keep != 0] == 0.25)
+    assert np.array_equal(Xk[:, :B][:, keep == 0], O.restart(inst, X0, seed=7, round_=0, B=B)[:, :B][:, keep == 0])
+
+
 def test_rejects_bad_input():
     inst = I.make_mixed(n=10, m=5, kmin=2, kmax=4, seed=1, batch=2)
     X = I.make_x0(inst, batch=2, dtype=np.float64)
