@@ -43,10 +43,15 @@ thread_local std::string g_create_error;
 #undef AFSAT_S_KMAX
 #define AFSAT_S_KMAX 0
 #endif
+// fp32: the scalar register kernel (one candidate per lane, every intermediate in registers, the compiler
+// spilling what does not fit) up to this length; it beats the shared-memory-staged kernel at every length
+#ifndef AFSAT_B_KMAX32
+#define AFSAT_B_KMAX32 64
+#endif
 enum { CLS_S = 0, CLS_A = 1, CLS_B = 2, CLS_LONG = 3, N_CLS = 4 };
 inline int class_of(int k, int dtype)
 {
-    return (dtype == 32 && k <= AFSAT_S_KMAX) ? CLS_S : k <= 8 ? CLS_A : k <= 16 ? CLS_B : CLS_LONG;
+    return (dtype == 32 && k <= AFSAT_S_KMAX) ? CLS_S : k <= 8 ? CLS_A : k <= (dtype == 32 ? AFSAT_B_KMAX32 : 16) ? CLS_B : CLS_LONG;
 }
 
 struct ClassGeom {              // how one length class maps candidates onto a CTA
@@ -192,6 +197,14 @@ void (*pick_s(bool grad))(EvalParams<T>)
         return nullptr;                                                // class S is empty for this dtype / build
 }
 
+template <typename T>
+void (*pick_b(bool grad))(EvalParams<T>)
+{
+    using Fn = void (*)(EvalParams<T>);
+    constexpr int KHI = sizeof(T) == 4 ? AFSAT_B_KMAX32 : 16;
+    return grad ? (Fn)k_eval_km<T, 9, KHI, 1, true, 1> : (Fn)k_eval_km<T, 9, KHI, 1, false, 1>;
+}
+
 // k > 16: KMAX is the unroll bound of the register-blocked kernels; fp32 runs the packed two-candidate form
 inline int long_kmax(int kmax_long) { return kmax_long <= 32 ? 32 : kmax_long <= 40 ? 40 : kmax_long <= 48 ? 48 : kmax_long <= 56 ? 56 : 64; }
 #ifndef AFSAT_LONG_PACKED
@@ -201,6 +214,8 @@ template <typename T>
 void (*pick_long(int km, bool grad))(EvalParams<T>)
 {
     using Fn = void (*)(EvalParams<T>);
+    if constexpr (sizeof(T) == 4 && AFSAT_B_KMAX32 >= AFSAT_MAX_LEN) return nullptr;   // the class is empty for fp32
+    else {
 #define AFSAT_LONG_CASE(KM_)                                                                                  \
     case KM_:                                                                                                 \
         if constexpr (sizeof(T) == 4 && AFSAT_LONG_PACKED) return grad ? (Fn)k_eval_blk2<KM_, true> : (Fn)k_eval_blk2<KM_, false>; \
@@ -211,6 +226,7 @@ void (*pick_long(int km, bool grad))(EvalParams<T>)
         AFSAT_LONG_CASE(64)
     }
 #undef AFSAT_LONG_CASE
+    }
 }
 
 // ---- launch of the evaluation kernels (a1-a5) for the candidate tile [b_begin, b_begin + width) ----
@@ -255,7 +271,7 @@ int launch_eval(afsat_ctx *ctx, const T *x, T *G, int64_t g_ld, int64_t g_b0, T 
             constexpr int MB = sizeof(T) == 4 ? AFSAT_A_MINB : 1;
             Fn fn = cls == CLS_S ? pick_s<T, MB>(grad)
                   : cls == CLS_A ? pick_a<T, VA, MB>(grad)
-                                 : (grad ? (Fn)k_eval_km<T, 9, 16, 1, true, 1> : (Fn)k_eval_km<T, 9, 16, 1, false, 1>);
+                                 : pick_b<T>(grad);
             fn<<<grid, block, 0, st>>>(p);
         } else {
             using Fn = void (*)(EvalParams<T>);
