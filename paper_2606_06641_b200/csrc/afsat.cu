@@ -48,10 +48,13 @@ thread_local std::string g_create_error;
 #ifndef AFSAT_B_KMAX32
 #define AFSAT_B_KMAX32 64
 #endif
+#ifndef AFSAT_B_KMAX64
+#define AFSAT_B_KMAX64 20
+#endif
 enum { CLS_S = 0, CLS_A = 1, CLS_B = 2, CLS_LONG = 3, N_CLS = 4 };
 inline int class_of(int k, int dtype)
 {
-    return (dtype == 32 && k <= AFSAT_S_KMAX) ? CLS_S : k <= 8 ? CLS_A : k <= (dtype == 32 ? AFSAT_B_KMAX32 : 16) ? CLS_B : CLS_LONG;
+    return (dtype == 32 && k <= AFSAT_S_KMAX) ? CLS_S : k <= 8 ? CLS_A : k <= (dtype == 32 ? AFSAT_B_KMAX32 : AFSAT_B_KMAX64) ? CLS_B : CLS_LONG;
 }
 
 struct ClassGeom {              // how one length class maps candidates onto a CTA
@@ -201,15 +204,12 @@ template <typename T>
 void (*pick_b(bool grad))(EvalParams<T>)
 {
     using Fn = void (*)(EvalParams<T>);
-    constexpr int KHI = sizeof(T) == 4 ? AFSAT_B_KMAX32 : 16;
+    constexpr int KHI = sizeof(T) == 4 ? AFSAT_B_KMAX32 : AFSAT_B_KMAX64;
     return grad ? (Fn)k_eval_km<T, 9, KHI, 1, true, 1> : (Fn)k_eval_km<T, 9, KHI, 1, false, 1>;
 }
 
 // k > 16: KMAX is the unroll bound of the register-blocked kernels; fp32 runs the packed two-candidate form
 inline int long_kmax(int kmax_long) { return kmax_long <= 32 ? 32 : kmax_long <= 40 ? 40 : kmax_long <= 48 ? 48 : kmax_long <= 56 ? 56 : 64; }
-#ifndef AFSAT_LONG_PACKED
-#define AFSAT_LONG_PACKED 1
-#endif
 template <typename T>
 void (*pick_long(int km, bool grad))(EvalParams<T>)
 {
@@ -218,8 +218,7 @@ void (*pick_long(int km, bool grad))(EvalParams<T>)
     else {
 #define AFSAT_LONG_CASE(KM_)                                                                                  \
     case KM_:                                                                                                 \
-        if constexpr (sizeof(T) == 4 && AFSAT_LONG_PACKED) return grad ? (Fn)k_eval_blk2<KM_, true> : (Fn)k_eval_blk2<KM_, false>; \
-        else return grad ? (Fn)k_eval_blk<T, KM_, true> : (Fn)k_eval_blk<T, KM_, false>;
+        return grad ? (Fn)k_eval_blk<T, KM_, true> : (Fn)k_eval_blk<T, KM_, false>;
     switch (km) {
         AFSAT_LONG_CASE(32) AFSAT_LONG_CASE(40) AFSAT_LONG_CASE(48) AFSAT_LONG_CASE(56)
     default:
@@ -657,12 +656,7 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
         if (cls == CLS_LONG) {
             const int km = long_kmax(kmax_long);
             g.warps = LONG_THREADS / 32;
-            if (dtype == 32 && AFSAT_LONG_PACKED) {
-                g.V = 2;
-                g.smem = (size_t)g.warps * (km + 2 * long_pp(km) * (km / LB2)) * 32 * 8;  // per warp: value pairs [KMAX][32] + boundary pairs
-            } else {
-                g.smem = (size_t)g.warps * (km + 2 * (km / LB)) * 32 * esz; // per warp: values [KMAX][32] + boundaries [2 KMAX/LB][32]
-            }
+            g.smem = (size_t)g.warps * (km + 2 * (km / LB)) * 32 * esz; // per warp: values [KMAX][32] + boundaries [2 KMAX/LB][32]
         }
         const int64_t cw = 32 * g.V;
         g.Wc = std::min(g.warps, pow2_floor(std::max<int64_t>(1, (tile_w + cw - 1) / cw)));

@@ -1045,210 +1045,6 @@ __global__ void __launch_bounds__(LONG_THREADS) k_eval_blk(const EvalParams<T> p
     store_item_F<T, 1>(p, s_F, fe, warp, lane, wk, b, active);
 }
 
-// ---- the same register-blocked scheme with TWO candidates per lane in packed f32x2 arithmetic (fp32) ----
-// A 3-pair-operand FFMA2 costs ~3 pipe cycles (register-file read bandwidth, profiles/r1_notes.md), so the
-// packed form tops out near 65 % of the FP32 peak -- but it halves the instruction count and is free of
-// the register-bank dispatch stalls that hold the scalar long kernel near 36 %.
-constexpr int LB2 = 4;
-constexpr f32x2 NEG2 = 0x8000000080000000ull;
-
-// DFT points evaluated at once by the packed long kernel: 2 while the boundary storage of two points
-// still leaves room for 3 CTAs per SM (KMAX <= 32), else 1
-__host__ __device__ constexpr int long_pp(int kmax) { return kmax <= 32 ? 2 : 1; }
-
-// PP DFT points at once (independent chains interleaved for instruction-level parallelism)
-template <bool CPLX, int NU, int PP>
-struct BlkOps2 {
-    static __device__ __forceinline__ void fwd(const f32x2 *__restrict__ sy, const f32x2 (&ar)[PP], const f32x2 (&ai)[PP],
-                                               const f32x2 (&br)[PP], const f32x2 (&bi)[PP], f32x2 (&rr)[PP], f32x2 (&ri)[PP])
-    {
-#pragma unroll
-        for (int u = 0; u < NU; ++u) {
-            const f32x2 yv = sy[u * 32];
-#pragma unroll
-            for (int t = 0; t < PP; ++t) {
-                const f32x2 fr = fma2(br[t], yv, ar[t]);
-                if (CPLX) {
-                    const f32x2 fi = fma2(bi[t], yv, ai[t]);
-                    const f32x2 nr = fma2(rr[t], fr, mul2(ri[t], fi ^ NEG2));
-                    const f32x2 ni = fma2(rr[t], fi, mul2(ri[t], fr));
-                    rr[t] = nr; ri[t] = ni;
-                } else {
-                    rr[t] = mul2(rr[t], fr);
-                }
-            }
-        }
-    }
-    // nu <= NU literals are live (nu == NU for a full block); suffix carried as (Re s, -Im s)
-    static __device__ __forceinline__ void bwd(int nu, const f32x2 *__restrict__ sy, const f32x2 (&ar)[PP], const f32x2 (&ai)[PP],
-                                               const f32x2 (&br)[PP], const f32x2 (&bi)[PP], const f32x2 (&pr0)[PP],
-                                               const f32x2 (&pi0)[PP], f32x2 (&sr)[PP], f32x2 (&nsi)[PP], f32x2 *__restrict__ g)
-    {
-        f32x2 fr[PP][NU], fi[PP][CPLX ? NU : 1], pr[PP][NU], pi[PP][CPLX ? NU : 1];
-#pragma unroll
-        for (int u = 0; u < NU; ++u) {
-            const f32x2 yv = sy[u * 32];
-#pragma unroll
-            for (int t = 0; t < PP; ++t) {
-                fr[t][u] = fma2(br[t], yv, ar[t]);
-                if (CPLX) fi[t][u] = fma2(bi[t], yv, ai[t]);
-            }
-        }
-#pragma unroll
-        for (int t = 0; t < PP; ++t) { pr[t][0] = pr0[t]; if (CPLX) pi[t][0] = pi0[t]; }
-#pragma unroll
-        for (int u = 1; u < NU; ++u)
-#pragma unroll
-            for (int t = 0; t < PP; ++t) {
-                if (CPLX) {
-                    pr[t][u] = fma2(pr[t][u - 1], fr[t][u - 1], mul2(pi[t][u - 1], fi[t][u - 1] ^ NEG2));
-                    pi[t][u] = fma2(pr[t][u - 1], fi[t][u - 1], mul2(pi[t][u - 1], fr[t][u - 1]));
-                } else {
-                    pr[t][u] = mul2(pr[t][u - 1], fr[t][u - 1]);
-                }
-            }
-#pragma unroll
-        for (int u = NU - 1; u >= 0; --u) {
-            if (u < nu) {                                             // warp-uniform; always true for a full block
-#pragma unroll
-                for (int t = 0; t < PP; ++t) {
-                    if (CPLX) {
-                        g[u] = fma2(pr[t][u], sr[t], g[u]);           // Re(pre suf) = pr sr - pi si
-                        g[u] = fma2(pi[t][u], nsi[t], g[u]);
-                        const f32x2 t_r = fma2(nsi[t], fi[t][u], mul2(sr[t], fr[t][u]));            // Re: sr fr - si fi
-                        const f32x2 t_n = fma2(nsi[t], fr[t][u], mul2(sr[t], fi[t][u] ^ NEG2));     // -Im: -(sr fi + si fr)
-                        sr[t] = t_r; nsi[t] = t_n;
-                    } else {
-                        g[u] = fma2(pr[t][u], sr[t], g[u]);
-                        sr[t] = mul2(sr[t], fr[t][u]);
-                    }
-                }
-            }
-        }
-    }
-};
-
-// PP consecutive table rows r, r+8, ... (all real or all complex).  sb: [blk][point][re, im][lane].
-template <int KMAX, bool CPLX, bool GRAD, int PP>
-__device__ __forceinline__ void long_point2(const f32x2 *__restrict__ sy, f32x2 *__restrict__ sb, int k, const float *__restrict__ r,
-                                            f32x2 &fe, f32x2 (&g)[KMAX])
-{
-    constexpr int NBLK = KMAX / LB2;
-    f32x2 ar[PP], ai[PP], br[PP], bi[PP], rr[PP], ri[PP];
-#pragma unroll
-    for (int t = 0; t < PP; ++t) {
-        const float *rt = r + 8 * t;
-        ar[t] = pk(rt[0], rt[0]); ai[t] = pk(rt[1], rt[1]); br[t] = pk(rt[2], rt[2]); bi[t] = pk(rt[3], rt[3]);
-        rr[t] = pk(1.f, 1.f); ri[t] = 0ull;
-    }
-    const int nfull = k / LB2, tail = k % LB2;
-    auto save = [&](int blk) {
-#pragma unroll
-        for (int t = 0; t < PP; ++t) {
-            sb[((2 * blk) * PP + t) * 32] = rr[t];
-            if (CPLX) sb[((2 * blk + 1) * PP + t) * 32] = ri[t];
-        }
-    };
-    for (int blk = 0; blk < nfull; ++blk) {                           // forward: runtime loop, one body
-        save(blk);
-        BlkOps2<CPLX, LB2, PP>::fwd(sy + blk * LB2 * 32, ar, ai, br, bi, rr, ri);
-    }
-    if (tail) {
-        save(nfull);
-        for (int u = 0; u < tail; ++u) BlkOps2<CPLX, 1, PP>::fwd(sy + (nfull * LB2 + u) * 32, ar, ai, br, bi, rr, ri);
-    }
-#pragma unroll
-    for (int t = 0; t < PP; ++t) {
-        fe = fma2(pk(r[8 * t + 4], r[8 * t + 4]), rr[t], fe);
-        if (CPLX) fe = fma2(pk(-r[8 * t + 5], -r[8 * t + 5]), ri[t], fe);
-    }
-    if (GRAD) {
-        f32x2 sr[PP], nsi[PP], p0[PP], p1[PP];                        // suffix (Re, -Im) seeded with w b
-#pragma unroll
-        for (int t = 0; t < PP; ++t) { sr[t] = pk(r[8 * t + 6], r[8 * t + 6]); nsi[t] = CPLX ? pk(-r[8 * t + 7], -r[8 * t + 7]) : 0ull; }
-#pragma unroll
-        for (int blk = NBLK - 1; blk >= 0; --blk) {                    // backward: unrolled, g in registers
-            if (blk < nfull || (blk == nfull && tail)) {
-#pragma unroll
-                for (int t = 0; t < PP; ++t) {
-                    p0[t] = sb[((2 * blk) * PP + t) * 32];
-                    p1[t] = CPLX ? sb[((2 * blk + 1) * PP + t) * 32] : 0ull;
-                }
-                BlkOps2<CPLX, LB2, PP>::bwd(blk < nfull ? LB2 : tail, sy + blk * LB2 * 32, ar, ai, br, bi, p0, p1, sr, nsi, &g[blk * LB2]);
-            }
-        }
-    }
-}
-
-template <int KMAX, bool GRAD>
-__global__ void __launch_bounds__(LONG_THREADS) k_eval_blk2(const EvalParams<float> p)
-{
-    constexpr int NW = LONG_THREADS / 32;
-    __shared__ __align__(16) float s_tab[MAX_ROWS * 8];
-    __shared__ int32_t s_lits[LONG_LIT_CHUNK];
-    __shared__ float s_F[NW][64];
-    extern __shared__ __align__(16) unsigned char s_dyn[];               // per warp: values [KMAX][32] pairs, boundaries [2 NBLK][32] pairs
-    constexpr int PP = long_pp(KMAX);
-    constexpr int PER_WARP = (KMAX + 2 * PP * (KMAX / LB2)) * 32;
-    f32x2 *s_y = reinterpret_cast<f32x2 *>(s_dyn);
-    const Item it = p.items[blockIdx.x];
-    const SigDev sgd = p.sigs[it.sig];
-    stage_item(p, it, sgd, s_tab, s_lits);
-    __syncthreads();
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int wc = warp % p.Wc, wk = warp / p.Wc;
-    const int64_t b = p.b_begin + ((int64_t)blockIdx.y * p.Wc + wc) * 64 + lane * 2;
-    const bool active = b < p.b_end && b < p.B && !lane_skipped(p, b, 2);   // this launch owns [b_begin, b_end)
-    f32x2 fe2 = 0ull;
-    if (active) {
-        f32x2 *sy = s_y + (size_t)warp * PER_WARP + lane;
-        f32x2 *sb = sy + KMAX * 32;
-        const int k = it.k, nc = it.c_end - it.c_begin;
-        const char *xb = reinterpret_cast<const char *>(p.x + b);
-        char *gb = reinterpret_cast<char *>(p.G + (b - p.g_b0));
-        const uint32_t x_ld = (uint32_t)(p.ldb * 4), g_ld = (uint32_t)(p.g_ld * 4);
-        for (int c = wk; c < nc; c += p.Wk) {
-            const int32_t *L = s_lits + c * k;
-            for (int i = 0; i < k; ++i) {                               // a1: gather, sign, stage
-                const int32_t lit = L[i];
-                const f32x2 v = (lit & LIT_FIXED) ? pk(1.f, 1.f)
-                                                  : __ldg(reinterpret_cast<const f32x2 *>(xb + (uint64_t)(uint32_t)(lit & LIT_VAR) * x_ld));
-                const uint32_t m = (uint32_t)(lit & LIT_NEG);
-                sy[i * 32] = v ^ (((f32x2)m << 32) | m);
-            }
-            for (int i = k; i < (k + LB2 - 1) / LB2 * LB2; ++i) sy[i * 32] = 0ull;   // finite padding of the last block
-            f32x2 g[KMAX];
-#pragma unroll
-            for (int i = 0; i < KMAX; ++i) g[i] = 0ull;
-            const float *r = s_tab;
-            for (int q = 0; q < sgd.n_real; ++q, r += 8) long_point2<KMAX, false, GRAD, 1>(sy, sb, k, r, fe2, g);
-            int q = 0;
-            if (PP == 2)
-                for (; q + 1 < sgd.n_cplx; q += 2, r += 16) long_point2<KMAX, true, GRAD, 2>(sy, sb, k, r, fe2, g);
-            for (; q < sgd.n_cplx; ++q, r += 8) long_point2<KMAX, true, GRAD, 1>(sy, sb, k, r, fe2, g);
-            if (GRAD) {
-#pragma unroll
-                for (int i = 0; i < KMAX; ++i) {
-                    if (i < k) {                                        // warp-uniform
-                        const int32_t lit = L[i];
-                        if (!(lit & LIT_FIXED)) {
-                            const uint32_t m = (uint32_t)(lit & LIT_NEG);
-                            float g0, g1;
-                            upk(g[i] ^ (((f32x2)m << 32) | m), g0, g1);
-                            asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(gb + (uint64_t)(uint32_t)(lit & LIT_VAR) * g_ld),
-                                         "f"(g0), "f"(g1)
-                                         : "memory");
-                        }
-                    }
-                }
-            }
-        }
-    }
-    float fe[2];
-    upk(fe2, fe[0], fe[1]);
-    store_item_F<float, 2>(p, s_F, fe, warp, lane, wk, b, active);
-}
-
 // ---- a7: sign rounding as one bit per (variable, candidate): bits[v][b / 32] bit (b % 32) = (x < 0)
 template <typename T>
 __global__ void __launch_bounds__(CTA_THREADS) k_pack_signs(const T *__restrict__ x, uint32_t *__restrict__ bits, int n,
