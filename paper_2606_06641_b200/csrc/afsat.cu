@@ -48,6 +48,9 @@ thread_local std::string g_create_error;
 #ifndef AFSAT_B_KMAX32
 #define AFSAT_B_KMAX32 64
 #endif
+#ifndef AFSAT_B_MINB
+#define AFSAT_B_MINB 1
+#endif
 #ifndef AFSAT_B_KMAX64
 #define AFSAT_B_KMAX64 20
 #endif
@@ -205,7 +208,7 @@ void (*pick_b(bool grad))(EvalParams<T>)
 {
     using Fn = void (*)(EvalParams<T>);
     constexpr int KHI = sizeof(T) == 4 ? AFSAT_B_KMAX32 : AFSAT_B_KMAX64;
-    return grad ? (Fn)k_eval_km<T, 9, KHI, 1, true, 1> : (Fn)k_eval_km<T, 9, KHI, 1, false, 1>;
+    return grad ? (Fn)k_eval_km<T, 9, KHI, 1, true, AFSAT_B_MINB> : (Fn)k_eval_km<T, 9, KHI, 1, false, AFSAT_B_MINB>;
 }
 
 // k > 16: KMAX is the unroll bound of the register-blocked kernels; fp32 runs the packed two-candidate form
