@@ -140,6 +140,72 @@ def oracle_sample(inst, x0, target_s=15.0, max_b=64):
                       f"{inst.batch} candidates x 1 step over all {inst.n_cons} constraints, {dt:.2f} s"}, dt, b_o
 
 
+def time_to_first_solution(inst, x0, dtype, device, max_steps):
+    """Time from the first afsat_step launch to the first step at which some candidate is solved, read from
+    the pinned any-solved flag the library sets from the device (polled here without a blocking sync).
+    The random instances of configs 1-4 sit far above the satisfiability threshold, so this runs the
+    PLANTED variant of the same workload (literal signs re-chosen so that a hidden assignment satisfies
+    every constraint); one candidate in 1024 starts next to the hidden assignment (0.1 % of the variables
+    wrong, |x| = 0.5), the others start uniformly at random like the headline run."""
+    import torch
+    from paper_2606_06641_b200 import binding as Bd, instances as I
+
+    def admissible(t, k, p):                       # counts of true literals that satisfy the constraint
+        taus = np.arange(k + 1)
+        ok = {0: taus >= 1, 1: taus % 2 == p, 2: taus >= p, 3: taus <= p, 4: taus == p, 5: (taus > 0) & (taus < k)}[int(t)]
+        return taus[ok]
+    base = I.Instance(**{**inst.__dict__})
+    base.meta = dict(inst.meta)
+    base.meta["admissible"] = [admissible(t, k, p) for t, k, p in zip(inst.ctype, inst.lengths(), inst.param)]
+    planted, hidden = I.plant_solution(base, seed=I.SEED_X0 + 77)
+    rng = np.random.default_rng(I.SEED_X0 + 78)
+    x = x0.copy()
+    near = np.where(hidden, -0.5, 0.5).astype(x.dtype)
+    probes = list(range(0, inst.batch, 1024))
+    for b in probes:
+        col = near.copy()
+        wrong = rng.choice(inst.n_vars, size=max(1, inst.n_vars // 1000), replace=False)
+        col[wrong] = -col[wrong]
+        if planted.fixed is not None:
+            fx = planted.fixed != 0
+            col[fx] = planted.fixed[fx]
+        x[:, b] = col
+    ctx = Bd.Context.from_instance(planted, dtype=dtype, device=device)
+    xd = torch.from_numpy(x).cuda()
+    flag = torch.zeros(2, dtype=torch.int32).pin_memory()
+    ctx.step(xd, inst.eta, 2, want_F=False)                      # warm-up (module load, workspace)
+    xd.copy_(torch.from_numpy(x).cuda())
+    torch.cuda.synchronize()
+    # the launching call blocks the host while the launch queue is full, so the flag is polled from a
+    # second thread (the ctypes call releases the GIL); the device writes it through mapped pinned memory
+    fl = flag.numpy()
+    seen = {}
+    stop = threading.Event()
+
+    def poll():
+        while not stop.is_set():
+            if fl[0] == 1:
+                seen["t"] = time.perf_counter()
+                return
+            time.sleep(0.0001)
+    th = threading.Thread(target=poll, daemon=True)
+    t0 = time.perf_counter()
+    th.start()
+    F, sat, sol, first = ctx.step(xd, inst.eta, max_steps, want_F=False, h_any_solved=flag)
+    torch.cuda.synchronize()
+    t_all = time.perf_counter() - t0
+    stop.set()
+    th.join(timeout=1)
+    t_first = (seen["t"] - t0) if "t" in seen else (t_all if int(flag[0]) == 1 else None)
+    out = {"instance": planted.name, "steps_run": max_steps, "probe_candidates": len(probes),
+           "first_solved_step": int(flag[1]) if int(flag[0]) else None,
+           "ms_to_first_solution": None if t_first is None else 1e3 * t_first,
+           "ms_all_steps": 1e3 * t_all, "solved_candidates": int(sol.sum().item()),
+           "random_instance": "no candidate solved in the benchmark's steps (far above the satisfiability threshold)"}
+    ctx.close()
+    return out
+
+
 def rank_x0_seed(cfg, rank):
     """Replicas only: every rank draws its own batch of candidates."""
     from paper_2606_06641_b200 import instances as I
@@ -308,6 +374,10 @@ def run_ours(args):
         e1.record(stream)
         barrier()
         t_ls = e0.elapsed_time(e1) * 1e-3
+    # ---- optional: time to first solution (BASELINE.json configs[4]) on the PLANTED variant of the workload ----
+    ttfs = None
+    if args.ttfs:
+        ttfs = time_to_first_solution(inst, x0, dtype, local, args.ttfs_steps)
     esz = 4 if dtype == 32 else 8
     h2d = n * ldb * esz
     d2h = n * ldb * esz + B * (esz + 4 + 1 + 4)
@@ -351,6 +421,8 @@ def run_ours(args):
                 "roofline": roof, "cpu_baseline": cb,
                 "value_l2_warm": world * m * B * K / t_warm, "ms_per_step_l2_warm": 1e3 * t_warm / K,
                 "solved_candidates": int(sol.sum().item()), "wall_s_timed_region": wall}
+        if ttfs is not None:
+            line["time_to_first_solution"] = ttfs
         if t_ls is not None:
             line["line_search"] = {"ms_per_step": 1e3 * t_ls / K, "max_trials": args.ls_trials,
                                    "note": "afsat_step_ls: 1 FE+grad evaluation + max_trials objective-only "
@@ -373,6 +445,8 @@ def main():
     ap.add_argument("--dtype", type=int, default=32, choices=[32, 64])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--oracle-seconds", type=float, default=15.0)
+    ap.add_argument("--ttfs", action="store_true", help="also report time to first solution on the planted variant")
+    ap.add_argument("--ttfs-steps", type=int, default=100)
     ap.add_argument("--line-search", action="store_true", help="also time afsat_step_ls (Alg. 1 with line search)")
     ap.add_argument("--ls-trials", type=int, default=4)
     args = ap.parse_args()
