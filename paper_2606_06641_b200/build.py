@@ -20,8 +20,9 @@ SOURCES_CU = [CSRC / "afsat.cu"]
 SOURCES_CPP = [CSRC / "precompute.cpp", CSRC / "parser.cpp"]
 DEPS = [CSRC / "afsat_kernels.cuh", CSRC / "afsat_internal.h", PKG.parent / "include" / "afsat.h"]
 
+# -split-compile=0: the optimiser works on the (many, independent) per-length bodies with all host threads
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "-Xcompiler", "-fPIC"]
+              "-split-compile=0", "-Xcompiler", "-fPIC"]
 
 
 def needs_build() -> bool:
