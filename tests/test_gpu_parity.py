@@ -129,6 +129,44 @@ def test_long_constraints_uniform_x(dtype):
         assert np.abs(G - Go).max() <= 1e-10
 
 
+@pytest.mark.parametrize("with_fixed", [False, True])
+def test_every_length_9_to_64(with_fixed):
+    """One constraint of EVERY length 9..64 (every exact body, every ragged body at each of its four lengths,
+    with and without fixed literals), fp32, robust tables (tight at any length): F and G against the oracle at
+    1e-4, and the paper's tables within the loose long-constraint bound."""
+    rng = np.random.default_rng(909)
+    n = 72
+    row_ptr, lit_var, lit_sign, ctype, param = [0], [], [], [], []
+    types = [I.ATLEAST, I.ATMOST, I.EXACTLY, I.OR, I.NAE, I.XOR]
+    for k in range(9, 65):
+        vs = rng.choice(n, size=k, replace=False)
+        lit_var += vs.tolist()
+        lit_sign += (rng.integers(0, 2, size=k) * 2 - 1).tolist()
+        row_ptr.append(len(lit_var))
+        t = types[k % 6]
+        ctype.append(t)
+        param.append(int(rng.integers(0, 2)) if t == I.XOR else (k // 2 if t in (I.ATLEAST, I.ATMOST, I.EXACTLY) else 0))
+    fixed = None
+    if with_fixed:
+        fixed = np.zeros(n, dtype=np.int8)
+        which = rng.choice(n, size=12, replace=False)
+        fixed[which] = (rng.integers(0, 2, size=12) * 2 - 1).astype(np.int8)
+    inst = I.Instance(name="every_length", n_vars=n, row_ptr=np.asarray(row_ptr, dtype=np.int64),
+                      lit_var=np.asarray(lit_var, dtype=np.int32), lit_sign=np.asarray(lit_sign, dtype=np.int8),
+                      ctype=np.asarray(ctype, dtype=np.uint8), param=np.asarray(param, dtype=np.int32), fixed=fixed,
+                      batch=70, eta=0.1, steps=1, meta={})
+    x = I.make_x0(inst, seed=910, batch=70)
+    Fo, Go = O.eval_grad(inst, x.astype(np.float64), 70)
+    Fr, Gr = run_eval(inst, x, 70, 32, flags=Bd.FLAG_ROBUST)
+    assert np.abs(Fr - Fo).max() <= 1e-4 * inst.n_cons and np.abs(Gr[:, :70] - Go[:, :70]).max() <= 1e-4
+    F, G = run_eval(inst, x, 70, 32)
+    assert np.abs(F - Fo).max() <= 1e-4 * inst.n_cons + 1e-2 and np.abs(G[:, :70] - Go[:, :70]).max() <= 5e-2
+    if fixed is not None:
+        assert np.all(G[fixed != 0] == 0) and np.all(Gr[fixed != 0] == 0)
+    Fd, Gd = run_eval(inst, x, 70, 64, flags=Bd.FLAG_ROBUST)
+    assert np.abs(Fd - Fo).max() <= 1e-10 and np.abs(Gd[:, :70] - Go[:, :70]).max() <= 1e-10
+
+
 @pytest.mark.parametrize("dtype", [32, 64])
 def test_corners_and_zero(dtype):
     """x exactly +-1 (where PGD parks variables: factors vanish, division-based leave-one-out is
