@@ -78,6 +78,7 @@ struct afsat_ctx {
     int32_t *d_lits = nullptr;
     SigDev *d_sigs = nullptr;
     void *d_rows = nullptr;
+    float *d_rows2 = nullptr;                      // staged tables of the packed fp32 kernel
     int8_t *d_fixed = nullptr;
     Item *d_items = nullptr;
     int32_t n_items = 0, cls_begin[N_CLS + 1] = {0};
@@ -238,7 +239,7 @@ int launch_eval(afsat_ctx *ctx, const T *x, T *G, int64_t g_ld, int64_t g_b0, T 
 {
     EvalParams<T> p;
     p.x = x; p.G = G; p.g_ld = g_ld; p.g_b0 = g_b0; p.Fpart = Fpart;
-    p.lits = ctx->d_lits; p.sigs = ctx->d_sigs; p.rows = (const T *)ctx->d_rows;
+    p.lits = ctx->d_lits; p.sigs = ctx->d_sigs; p.rows = (const T *)ctx->d_rows; p.rows2 = ctx->d_rows2;
     p.skip = ctx->cur_skip;
     p.B = ctx->B; p.ldb = ctx->ldb; p.b_begin = b_begin; p.b_end = std::min<int64_t>(b_begin + width, ctx->ldb);
     const bool grad = G != nullptr;
@@ -586,6 +587,7 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
     const int n_sigs = (int)sig_id.size();
     std::vector<SigDev> sigs(n_sigs);
     std::vector<double> rows;
+    std::vector<float> rows2;
     std::vector<int> sig_k(n_sigs), sig_cost(n_sigs);
     for (auto &kv : sig_id) {
         AfsatSigHost hs;
@@ -605,6 +607,15 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
             d.k = kk;
         }
         rows.insert(rows.end(), hs.rows, hs.rows + 8 * (hs.n_real + hs.n_cplx));
+        if (dtype == 32 && hs.k <= 8) {                                // staged table of the packed kernel (k <= 8)
+            float r32[8 * AFSAT_MAX_POINTS], packed[AFSAT_PACK_MAX_ROWS * ROW2];
+            for (int i = 0; i < 8 * (hs.n_real + hs.n_cplx); ++i) r32[i] = (float)hs.rows[i];
+            int uv = 0, nu = 0, ng = 0;
+            const int nrows2 = pack_rows_f2(r32, hs.n_real, hs.n_cplx, hs.k, packed, &uv, &nu, &ng);
+            d.row2_off = (int32_t)(rows2.size() / ROW2);
+            d.uv = (int8_t)uv; d.n_unit = (int8_t)nu; d.n_gen = (int8_t)ng;
+            rows2.insert(rows2.end(), packed, packed + (size_t)nrows2 * ROW2);
+        }
         sig_k[kv.second] = hs.k;
         sig_cost[kv.second] = (int)cost_of(hs.k, hs.n_real, hs.n_cplx);
     }
@@ -744,6 +755,7 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
         float *p = nullptr;
         CREATE_FAIL(upload(ctx, &p, r32));
         ctx->d_rows = p;
+        CREATE_FAIL(upload(ctx, &ctx->d_rows2, rows2));
     } else {
         double *p = nullptr;
         CREATE_FAIL(upload(ctx, &p, rows));
@@ -790,7 +802,7 @@ void afsat_destroy(afsat_ctx *ctx)
 {
     if (!ctx) return;
     prof_drain(ctx, false);
-    cudaFree(ctx->d_lits); cudaFree(ctx->d_bits); cudaFree(ctx->d_sigs); cudaFree(ctx->d_rows);
+    cudaFree(ctx->d_lits); cudaFree(ctx->d_bits); cudaFree(ctx->d_sigs); cudaFree(ctx->d_rows); cudaFree(ctx->d_rows2);
     cudaFree(ctx->d_fixed); cudaFree(ctx->d_items); cudaFree(ctx->d_G); cudaFree(ctx->d_Fpart);
     cudaFree(ctx->d_satacc); cudaFree(ctx->d_any);
     cudaFree(ctx->ls_G); cudaFree(ctx->ls_xt); cudaFree(ctx->ls_F0); cudaFree(ctx->ls_F1); cudaFree(ctx->ls_Dpart);

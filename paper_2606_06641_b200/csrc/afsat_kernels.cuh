@@ -34,12 +34,14 @@ constexpr int CTA_THREADS = AFSAT_CTA_THREADS;
 constexpr int CTA_WARPS = CTA_THREADS / 32;
 constexpr int MAX_ROWS = 33;          // retained DFT points per signature: H <= 64/2 + 1
 
-struct SigDev {                 // 32 bytes, one per signature (type, k, param)
+struct SigDev {                 // 40 bytes, one per signature (type, k, param)
     int32_t row_off;            // first row in the weight table (8 scalars per row)
     int16_t n_real, n_cplx;     // real rows first, then complex rows
     uint64_t scan_lo, scan_hi;  // bit tau set: tau is in the SCANNED set of the discrete check
     int32_t scan_is_sat;        // 1: scanned set = satisfied counts; 0: = violated counts (smaller)
     int32_t k;
+    int32_t row2_off;           // packed fp32 kernel: first row of the STAGED table (ROW2 scalars per row, pack_rows_f2)
+    int8_t uv, n_unit, n_gen, pad;   // its unit variant, number of trivial-twiddle rows, number of generic complex rows
 };
 
 struct Item {                   // one CTA-sized chunk of constraints of a single signature
@@ -59,6 +61,7 @@ struct EvalParams {
     const int32_t *lits;        // packed literals, bucket order
     const SigDev *sigs;
     const T *rows;              // weight table
+    const float *rows2;         // staged table of the packed fp32 kernel (fp32 contexts), else null
     const Item *items;          // items of this launch
     int32_t frow_base;          // row of Fpart for (items[0], group 0)
     int32_t B;
@@ -220,6 +223,10 @@ __device__ __forceinline__ f32x2 bc(const f32x2 *tab, int j)
     const float c = reinterpret_cast<const float *>(tab)[2 * j];
     return pk(c, c);
 }
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b)
+{
+    f32x2 d; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d;   // FADD2 with a negated operand
+}
 __device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b)
 {
     f32x2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d;
@@ -231,9 +238,13 @@ __device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b)
 // FFMA2 has no negated operands, so the negated imaginary parts are tabulated and the backward
 // walk carries the suffix as (Re s, -Im s).
 constexpr int ROW2 = 12;
+#define AFSAT_PACK_MAX_ROWS 40              // >= MAX_ROWS + the zero-weight unit rows a table may get
 
 #ifndef AFSAT_F2_PAIR_POINTS
 #define AFSAT_F2_PAIR_POINTS 0
+#endif
+#ifndef AFSAT_F2_OCT_ROWS
+#define AFSAT_F2_OCT_ROWS 1
 #endif
 #ifndef AFSAT_F2_UNIT_ROWS
 #define AFSAT_F2_UNIT_ROWS 1
@@ -241,6 +252,60 @@ constexpr int ROW2 = 12;
 #ifndef AFSAT_F2_NEG_BY_XOR
 #define AFSAT_F2_NEG_BY_XOR 1
 #endif
+
+// HOST: the staged table of one signature for the packed kernel, from its fp32 rows {Re a, Im a, Re b, Im b,
+// Re w, Im w, Re(wb), Im(wb)} (real rows first).  Standard tables (a = 1/2 exactly in every row): the
+// trivial twiddles first, at fixed positions -- [w = 1 (absent: uv = 2)] [w = -1 iff k odd] [w = i iff k = 3 mod 4]
+// [w = (1+i)/sqrt 2, then its partner (-1+i)/sqrt 2 with CONJUGATED weights, iff k = 7 mod 8] -- a missing one
+// (its weight was exactly zero) staged with weight 0, the halvings folded into their weights (2^-k, 2^-(k-1):
+// exact rescales); then the generic complex rows.  Other tables: rows as they are, uv = 0.
+// Returns the number of staged rows; out gets ROW2 scalars per row.
+inline int pack_rows_f2(const float *r0, int n_real, int n_cplx, int k, float *out, int *uv_out, int *n_unit_out, int *n_gen_out)
+{
+    const int nr = n_real + n_cplx;
+    int src[AFSAT_PACK_MAX_ROWS], n = 0, uv = 0, n_unit = n_real, n_gen = n_cplx, q_conj = -1;
+    bool std_tab = AFSAT_F2_UNIT_ROWS != 0;
+    for (int q = 0; q < nr; ++q) std_tab = std_tab && r0[8 * q] == 0.5f && r0[8 * q + 1] == 0.f;
+    if (std_tab) {
+        int iP = -1, iM = -1, iI = -1, iA = -1, iB = -1;
+        const bool oct = AFSAT_F2_OCT_ROWS && (k & 7) == 7;
+        for (int q = 0; q < nr; ++q) {
+            const float br = r0[8 * q + 2], bi = r0[8 * q + 3];
+            if (q < n_real) { if (br == 0.5f) iP = q; else if (br == -0.5f) iM = q; }
+            else if (br == 0.f && bi == 0.5f) iI = q;
+            else if (oct && bi > 0.35f && bi < 0.36f && br == bi) iA = q;        // w = (1 + i)/sqrt 2
+            else if (oct && bi > 0.35f && bi < 0.36f && br == -bi) iB = q;       // w = (-1 + i)/sqrt 2
+        }
+        uv = iP >= 0 ? 1 : 2;
+        if (iP >= 0) src[n++] = iP;
+        if (k & 1) src[n++] = iM;
+        if ((k & 3) == 3) src[n++] = iI;
+        if (oct) { src[n++] = iA; q_conj = n; src[n++] = iB; }
+        n_unit = n;
+        for (int q = n_real; q < nr; ++q) if (q != iI && q != iA && q != iB) src[n++] = q;
+        n_gen = n - n_unit;
+    } else {
+        for (int q = 0; q < nr; ++q) src[n++] = q;
+    }
+    float sc_w = 1.f;
+    for (int i = 0; i < k; ++i) sc_w *= 0.5f;                                   // 2^-k
+    const float sc_wb = 2.0f * sc_w;                                            // 2^-(k-1)
+    for (int q = 0; q < n; ++q) {
+        float *o = out + (size_t)q * ROW2;
+        for (int j = 0; j < ROW2; ++j) o[j] = 0.f;
+        if (src[q] < 0) continue;
+        const float *r = r0 + 8 * src[q];
+        const bool unit = uv != 0 && q < n_unit;
+        const float fw = unit ? sc_w : 1.f, fwb = unit ? sc_wb : 1.f, cj = q == q_conj ? -1.f : 1.f;
+        if (src[q] < n_real) { o[0] = r[0]; o[1] = r[2]; o[2] = r[4] * fw; o[3] = r[6] * fwb; }   // a, b, w, wb
+        else {
+            o[0] = r[0]; o[1] = r[1]; o[2] = -r[1]; o[3] = r[2]; o[4] = r[3]; o[5] = -r[3];
+            o[6] = r[4] * fw; o[7] = -cj * r[5] * fw; o[8] = r[6] * fwb; o[9] = -cj * r[7] * fwb;
+        }
+    }
+    *uv_out = uv; *n_unit_out = n_unit; *n_gen_out = n_gen;
+    return n;
+}
 
 // PP complex DFT points (consecutive table rows) for NP candidate pairs: prefix walk, contraction,
 // suffix walk with the leave-one-out accumulation.  All PP x NP chains are independent.
@@ -392,6 +457,53 @@ __device__ __forceinline__ void unit_rows_f2(const f32x2 (&y)[K][NP], const f32x
     }
 }
 
+// The eighth roots of unity (k = 7 mod 8): at the DFT point w = (1 + i)/sqrt 2 a factor is (1 + z) + i z with
+// z = y/sqrt 2, and multiplying by it needs two adds and two FMAs instead of four multiplies and two FMAs,
+// no stored factors and no negation at all (the suffix is carried CONJUGATED, T = conj(S), T <- T conj(f)):
+//   P <- (Re P + z (Re P - Im P)) + i (Im P + z (Re P + Im P))
+//   T <- (Re T + z (Re T + Im T)) + i (Im T + z (Im T - Re T)),      g_i += Re P_i Re T_i + Im P_i Im T_i
+// Its partner w' = (-1 + i)/sqrt 2 = -conj(w) is the same walk at -y with conjugated weights (the row is staged
+// that way): prod (1 + w' y_j) = conj( prod (1 + w (-y_j)) ).  cz = +-1/sqrt 2 selects the row.
+template <int K, int NP, bool GRAD>
+__device__ __forceinline__ void oct_row_f2(const f32x2 (&y)[K][NP], const f32x2 *__restrict__ r, float cz, f32x2 (&fe)[NP],
+                                           f32x2 (&g)[K][NP])
+{
+    const f32x2 one2 = pk(1.0f, 1.0f), c2 = pk(cz, cz);
+    f32x2 z[K][NP], pr[K][NP], pi[K][NP], rr[NP], ri[NP];
+#pragma unroll
+    for (int i = 0; i < K; ++i)
+#pragma unroll
+        for (int q = 0; q < NP; ++q) z[i][q] = mul2(c2, y[i][q]);
+#pragma unroll
+    for (int q = 0; q < NP; ++q) { rr[q] = add2(z[0][q], one2); ri[q] = z[0][q]; }    // (1 + z_0) + i z_0
+#pragma unroll
+    for (int i = 1; i < K; ++i)
+#pragma unroll
+        for (int q = 0; q < NP; ++q) {
+            pr[i][q] = rr[q]; pi[i][q] = ri[q];
+            const f32x2 d = sub2(rr[q], ri[q]), s = add2(rr[q], ri[q]);
+            rr[q] = fma2(z[i][q], d, rr[q]); ri[q] = fma2(z[i][q], s, ri[q]);
+        }
+#pragma unroll
+    for (int q = 0; q < NP; ++q) { fe[q] = fma2(bc(r, 6), rr[q], fe[q]); fe[q] = fma2(bc(r, 7), ri[q], fe[q]); }
+    if (GRAD) {
+        f32x2 tr[NP], ti[NP];                                                         // conjugated suffix, seeded from the row
+#pragma unroll
+        for (int q = 0; q < NP; ++q) { tr[q] = r[8]; ti[q] = r[9]; }
+#pragma unroll
+        for (int i = K - 1; i >= 1; --i)
+#pragma unroll
+            for (int q = 0; q < NP; ++q) {
+                g[i][q] = fma2(pr[i][q], tr[q], g[i][q]);
+                g[i][q] = fma2(pi[i][q], ti[q], g[i][q]);
+                const f32x2 u = add2(tr[q], ti[q]), v = sub2(ti[q], tr[q]);
+                tr[q] = fma2(z[i][q], u, tr[q]); ti[q] = fma2(z[i][q], v, ti[q]);
+            }
+#pragma unroll
+        for (int q = 0; q < NP; ++q) g[0][q] = add2(g[0][q], tr[q]);                  // prefix_0 = 1
+    }
+}
+
 // One generic complex DFT point for all NP pairs of a lane.  With two pairs and k >= AFSAT_F2_SEQ_MINK the
 // pairs are walked one after the other (each keeps 5 k register pairs of factors and prefixes alive).
 #ifndef AFSAT_F2_SEQ_MINK
@@ -428,7 +540,13 @@ __device__ __forceinline__ void eval_points_f2(const f32x2 (&y)[K][NP], const f3
         constexpr bool HP = UV == 1, HM = (K & 1) != 0, HI = (K & 3) == 3;
         const f32x2 *rP = tab, *rM = tab + (HP ? ROW2 : 0), *rI = rM + (HM ? ROW2 : 0);
         if (HP || HM || HI) unit_rows_f2<K, NP, HP, HM, HI, GRAD>(y, rP, rM, rI, fe, g);
-        const f32x2 *r = rI + (HI ? ROW2 : 0);
+        constexpr bool HO = AFSAT_F2_OCT_ROWS && (K & 7) == 7;       // the pair of eighth roots, next in the staged order
+        const f32x2 *rO = rI + (HI ? ROW2 : 0);
+        if (HO) {
+            oct_row_f2<K, NP, GRAD>(y, rO, 0.70710678118654752f, fe, g);             // = 2 Re b of the row, bit for bit
+            oct_row_f2<K, NP, GRAD>(y, rO + ROW2, -0.70710678118654752f, fe, g);
+        }
+        const f32x2 *r = rO + (HO ? 2 * ROW2 : 0);
         for (int p = 0; p < n_cplx; ++p, r += ROW2) cplx_row_f2<K, NP, GRAD>(y, r, fe, g);
         return;
     }
@@ -733,58 +851,10 @@ __global__ void __launch_bounds__(CTA_THREADS, MINB) k_eval_f2m(const EvalParams
     __shared__ float s_F[CTA_WARPS][64 * NP];
     const Item it = p.items[blockIdx.x];
     const SigDev sg = p.sigs[it.sig];
-    // Row order of the staged table.  Standard tables (a = 1/2 exactly in every row): the trivial twiddles
-    // first, at fixed positions (a missing one -- its weight was exactly zero -- is staged with weight 0),
-    // halvings folded into their weights (2^-k, 2^-(k-1): exact rescales); then the generic complex rows.
-    __shared__ int s_src[H + 3], s_hdr[3];                            // source row (or -1) per staged row; {uv, n_unit, n_gen}
-    if (threadIdx.x == 0) {
-        const int nr = sg.n_real + sg.n_cplx;
-        const float *r0 = p.rows + (int64_t)sg.row_off * 8;
-        int uv = 0, n_unit = sg.n_real, n_gen = sg.n_cplx;
-        bool std_tab = AFSAT_F2_UNIT_ROWS != 0;
-        for (int q = 0; q < nr; ++q) std_tab = std_tab && r0[8 * q] == 0.5f && r0[8 * q + 1] == 0.f;
-        if (std_tab) {
-            int iP = -1, iM = -1, iI = -1;
-            for (int q = 0; q < nr; ++q) {
-                const float br = r0[8 * q + 2], bi = r0[8 * q + 3];
-                if (q < sg.n_real) { if (br == 0.5f) iP = q; else if (br == -0.5f) iM = q; }
-                else if (br == 0.f && bi == 0.5f) iI = q;
-            }
-            uv = iP >= 0 ? 1 : 2;
-            int n = 0;
-            if (iP >= 0) s_src[n++] = iP;
-            if (it.k & 1) s_src[n++] = iM;
-            if ((it.k & 3) == 3) s_src[n++] = iI;
-            n_unit = n;
-            for (int q = sg.n_real; q < nr; ++q) if (q != iI) s_src[n++] = q;
-            n_gen = n - n_unit;
-        } else {
-            for (int q = 0; q < nr; ++q) s_src[q] = q;
-        }
-        s_hdr[0] = uv; s_hdr[1] = n_unit; s_hdr[2] = n_gen;
-    }
-    __syncthreads();
-    const int uv = s_hdr[0], n_unit = s_hdr[1], n_gen = s_hdr[2];
-    const float sc_w = __int_as_float((127 - it.k) << 23), sc_wb = 2.0f * sc_w;   // 2^-k, 2^-(k-1)
+    // the staged table (row order, folded weights: pack_rows_f2, built once per signature at create time)
+    const int uv = sg.uv, n_unit = sg.n_unit, n_gen = sg.n_gen;
     for (int i = threadIdx.x; i < (n_unit + n_gen) * ROW2; i += blockDim.x) {
-        const int q = i / ROW2, j = i % ROW2, src = s_src[q];
-        float v = 0.f;
-        if (src >= 0) {
-            const float *r = p.rows + ((int64_t)sg.row_off + src) * 8;
-            const bool unit = uv != 0 && q < n_unit;
-            const float fw = unit ? sc_w : 1.f, fwb = unit ? sc_wb : 1.f;
-            if (src < sg.n_real) {                                    // a, b, w, wb
-                if (j < 2) v = r[2 * j]; else if (j == 2) v = r[4] * fw; else if (j == 3) v = r[6] * fwb;
-            } else {
-                switch (j) {
-                case 0: v = r[0]; break;  case 1: v = r[1]; break;  case 2: v = -r[1]; break;
-                case 3: v = r[2]; break;  case 4: v = r[3]; break;  case 5: v = -r[3]; break;
-                case 6: v = r[4] * fw; break;  case 7: v = -r[5] * fw; break;
-                case 8: v = r[6] * fwb; break;  case 9: v = -r[7] * fwb; break;
-                default: break;
-                }
-            }
-        }
+        const float v = __ldg(p.rows2 + (int64_t)sg.row2_off * ROW2 + i);
         s_tab2[i] = pk(v, v);
     }
     const int nl = (it.c_end - it.c_begin) * it.k;
