@@ -16,13 +16,15 @@ CSRC = PKG / "csrc"
 LIB = PKG / "libafsat_b200.so"
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 
-SOURCES_CU = [CSRC / "afsat.cu"]
+SOURCES_CU = [CSRC / "afsat.cu", CSRC / "afsat_km32.cu"]
 SOURCES_CPP = [CSRC / "precompute.cpp", CSRC / "parser.cpp"]
 DEPS = [CSRC / "afsat_kernels.cuh", CSRC / "afsat_internal.h", PKG.parent / "include" / "afsat.h"]
 
-# -split-compile=0: the optimiser works on the (many, independent) per-length bodies with all host threads
+# (nvcc -split-compile=0 halves the build time but costs the fp64 register-blocked kernel 17 %: not used; the two
+# CUDA translation units are compiled in parallel instead)
+# -static-global-template-stub=false: a kernel template instantiated in one unit is launched from the other
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "-split-compile=0", "-Xcompiler", "-fPIC"]
+              "-static-global-template-stub=false", "-Xcompiler", "-fPIC"]
 
 
 def needs_build() -> bool:
@@ -45,14 +47,18 @@ def build(force: bool = False, verbose: bool = False) -> Path:
             print(" ".join(cmd), flush=True)
         subprocess.check_call(cmd)
         objs.append(obj)
-    for src in SOURCES_CU:
+    procs = []
+    for src in SOURCES_CU:                                            # the CUDA translation units in parallel
         obj = objdir / (src.stem + ".o")
         cmd = [NVCC, *NVCC_FLAGS, *os.environ.get("AFSAT_NVCC_FLAGS", "").split(), "-c", str(src), "-o", str(obj)]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
             print(" ".join(cmd), flush=True)
-        subprocess.check_call(cmd)
+        procs.append((cmd, subprocess.Popen(cmd)))
         objs.append(obj)
+    for cmd, pr in procs:
+        if pr.wait() != 0:
+            raise subprocess.CalledProcessError(pr.returncode, cmd)
     tmp = LIB.with_suffix(f".so.tmp{os.getpid()}")
     cmd = [NVCC, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", str(tmp),
            *map(str, objs), "-lquadmath", "-cudart", "static"]

@@ -45,12 +45,6 @@ thread_local std::string g_create_error;
 #endif
 // fp32: the scalar register kernel (one candidate per lane, every intermediate in registers, the compiler
 // spilling what does not fit) up to this length; it beats the shared-memory-staged kernel at every length
-#ifndef AFSAT_B_KMAX32
-#define AFSAT_B_KMAX32 64
-#endif
-#ifndef AFSAT_B_MINB
-#define AFSAT_B_MINB 1
-#endif
 #ifndef AFSAT_B_KMAX64
 #define AFSAT_B_KMAX64 20
 #endif

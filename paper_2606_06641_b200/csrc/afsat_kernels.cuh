@@ -1197,6 +1197,7 @@ struct CheckParams {
     int32_t n_items;
 };
 
+#ifndef AFSAT_KM32_TU   // non-template kernel: defined in ONE translation unit only
 __global__ void __launch_bounds__(CTA_THREADS) k_check_bits(const CheckParams p)
 {
     __shared__ int32_t s_lits[LIT_CHUNK];
@@ -1267,11 +1268,13 @@ __global__ void __launch_bounds__(CTA_THREADS) k_check_bits(const CheckParams p)
         if (b < p.B && b < (int64_t)p.w_end * 32 && s_cnt[i]) atomicAdd(p.satacc + b, s_cnt[i]);
     }
 }
+#endif
 
 // ---- line search (afsat_step_ls; reading B5): per-candidate backtracking along the projection arc ----
 // ls_state[b]: 0 = still searching, 1 = step accepted, 2 = frozen (solved or converged)
 constexpr int LS_CHUNKS = 32;         // row chunks of the <G, X - X'> reduction (fixed-order two-stage sum)
 
+#ifndef AFSAT_KM32_TU   // non-template kernel: defined in ONE translation unit only
 __global__ void k_ls_begin(int B, int64_t ldb, const uint8_t *__restrict__ is_solution, const uint8_t *__restrict__ converged,
                            uint8_t *__restrict__ ls_state, double s_max, double *__restrict__ eta)
 {
@@ -1280,6 +1283,7 @@ __global__ void k_ls_begin(int B, int64_t ldb, const uint8_t *__restrict__ is_so
     ls_state[b] = (b >= B || is_solution[b] || converged[b]) ? 2 : 0;
     eta[b] = s_max;
 }
+#endif
 
 // X' = clamp(X - eta_b G) for the candidates still searching (first trial: every candidate gets a valid X'),
 // Dpart[chunk][b] = sum over the chunk's rows of G (X - X')
@@ -1407,6 +1411,7 @@ __global__ void k_reduce_F(const T *__restrict__ Fpart, int n_rows, int64_t ldb,
 }
 
 // ---- per-candidate state machine of Alg. 1 (a8, a9): satacc holds the count on the current X ----
+#ifndef AFSAT_KM32_TU   // non-template kernel: defined in ONE translation unit only
 __global__ void k_flags(int32_t *__restrict__ satacc, int B, int m, int mark_solved, int step_value,
                         int32_t *__restrict__ sat_count, uint8_t *__restrict__ is_solution,
                         int32_t *__restrict__ first_step, int32_t *__restrict__ d_any, volatile int32_t *h_any)
@@ -1425,8 +1430,10 @@ __global__ void k_flags(int32_t *__restrict__ satacc, int B, int m, int mark_sol
         }
     }
 }
+#endif
 
 // afsat_check epilogue: counts out, is_solution = (count == m), accumulator reset.
+#ifndef AFSAT_KM32_TU   // non-template kernel: defined in ONE translation unit only
 __global__ void k_check_finish(int32_t *__restrict__ satacc, int B, int m, int32_t *__restrict__ sat_count,
                                uint8_t *__restrict__ is_solution)
 {
@@ -1437,11 +1444,27 @@ __global__ void k_check_finish(int32_t *__restrict__ satacc, int B, int m, int32
     sat_count[b] = s;
     is_solution[b] = (uint8_t)(s == m);
 }
+#endif
 
+#ifndef AFSAT_KM32_TU   // non-template kernel: defined in ONE translation unit only
 __global__ void k_reset_state(int B, uint8_t *is_solution, int32_t *first_step)
 {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b < B) { is_solution[b] = 0; first_step[b] = -1; }
 }
+#endif
+
+// The fp32 instantiation of the scalar register kernel (bodies for 56 lengths) is compiled in its own translation
+// unit (afsat_km32.cu) so that the two halves of the build run in parallel; everyone else only declares it.
+#ifndef AFSAT_B_KMAX32
+#define AFSAT_B_KMAX32 64             // fp32: the scalar register kernel up to this length
+#endif
+#ifndef AFSAT_B_MINB
+#define AFSAT_B_MINB 1
+#endif
+#ifndef AFSAT_KM32_TU
+extern template __global__ void k_eval_km<float, 9, AFSAT_B_KMAX32, 1, true, AFSAT_B_MINB>(const EvalParams<float>);
+extern template __global__ void k_eval_km<float, 9, AFSAT_B_KMAX32, 1, false, AFSAT_B_MINB>(const EvalParams<float>);
+#endif
 
 }  // namespace afsat
