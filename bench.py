@@ -394,7 +394,7 @@ def run_ours(args):
         flop_per_step = flop_c * B
         peak_tf = sm * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
         ach_tf = flop_per_step / (kern_ms * 1e-3 / K) / 1e12 if kern_ms > 0 else 0.0
-        roof = {"bound": "alu", "kernel": "evaluation kernels, a1-a5 (k_eval_f2m fp32 k<=8 | k_eval_km | k_eval_blk): all launches of one step", "achieved": ach_tf, "peak": peak_tf,
+        roof = {"bound": "alu", "kernel": "evaluation kernels, a1-a5 (k_eval_f2m fp32 k<=8 | k_eval_km 9..20 | k_eval_split fp32 k>20 | k_eval_blk fp64 k>20): all launches of one step", "achieved": ach_tf, "peak": peak_tf,
                 "unit": "TFLOP/s", "frac": ach_tf / peak_tf,
                 "peak_source": f"{sm} SMs x 128 FP32 lanes x 2 flop x {peaks['sm_max_mhz']:.0f} MHz "
                                f"({peaks['source']} sm_max_mhz; DESIGN.md 'Roofline')",

@@ -15,6 +15,7 @@
 
 #include "afsat_internal.h"
 #include "afsat_kernels.cuh"
+#include "afsat_split.cuh"
 
 using namespace afsat;
 
@@ -56,6 +57,7 @@ inline int class_of(int k, int dtype)
 
 struct ClassGeom {              // how one length class maps candidates onto a CTA
     int V = 1;                  // candidates per lane
+    int cw = 32;                // candidates per warp (32 V; 32 / NS in the lane-split kernel)
     int warps = CTA_WARPS;      // warps per CTA
     int Wc = 1, Wk = CTA_WARPS; // candidate sub-tiles x constraint groups
     size_t smem = 0;            // dynamic shared memory (long kernel only)
@@ -212,8 +214,10 @@ template <typename T>
 void (*pick_long(int km, bool grad))(EvalParams<T>)
 {
     using Fn = void (*)(EvalParams<T>);
-    if constexpr (sizeof(T) == 4 && AFSAT_B_KMAX32 >= AFSAT_MAX_LEN) return nullptr;   // the class is empty for fp32
-    else {
+    if constexpr (sizeof(T) == 4) {                                    // fp32: the lane-split register kernel
+        return grad ? (Fn)k_eval_split<AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, true, AFSAT_L32_THREADS, AFSAT_L32_MINB>
+                    : (Fn)k_eval_split<AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, false, AFSAT_L32_THREADS, AFSAT_L32_MINB>;
+    } else {
 #define AFSAT_LONG_CASE(KM_)                                                                                  \
     case KM_:                                                                                                 \
         return grad ? (Fn)k_eval_blk<T, KM_, true> : (Fn)k_eval_blk<T, KM_, false>;
@@ -261,7 +265,7 @@ int launch_eval(afsat_ctx *ctx, const T *x, T *G, int64_t g_ld, int64_t g_b0, T 
         p.items = ctx->d_items + ctx->cls_begin[cls];
         p.frow_base = ctx->cls_begin[cls];
         p.Wc = g.Wc; p.Wk = g.Wk;
-        const int64_t per_cta = (int64_t)32 * g.V * g.Wc;
+        const int64_t per_cta = (int64_t)g.cw * g.Wc;
         dim3 block(32 * g.warps), grid(nit, (unsigned)((width + per_cta - 1) / per_cta));
         if (cls != CLS_LONG) {
             using Fn = void (*)(EvalParams<T>);
@@ -273,7 +277,7 @@ int launch_eval(afsat_ctx *ctx, const T *x, T *G, int64_t g_ld, int64_t g_b0, T 
         } else {
             using Fn = void (*)(EvalParams<T>);
             Fn fn = pick_long<T>(long_kmax(ctx->kmax_long), grad);
-            CU(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem));
+            if (g.smem) CU(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem));
             fn<<<grid, block, g.smem, st>>>(p);
         }
         ++ctx->launches;
@@ -661,12 +665,16 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
         ClassGeom &g = geom[cls];
         g.V = (cls == CLS_S) ? 4 : (cls == CLS_A && dtype == 32) ? AFSAT_A_V : 1;
         g.warps = CTA_WARPS;
-        if (cls == CLS_LONG) {
+        g.cw = 32 * g.V;
+        if (cls == CLS_LONG && dtype == 32) {                          // lane-split kernel: NS lanes per candidate
+            g.warps = AFSAT_L32_THREADS / 32;
+            g.cw = 32 / AFSAT_L32_NS;
+        } else if (cls == CLS_LONG) {
             const int km = long_kmax(kmax_long);
             g.warps = LONG_THREADS / 32;
             g.smem = (size_t)g.warps * (km + 2 * (km / LB)) * 32 * esz; // per warp: values [KMAX][32] + boundaries [2 KMAX/LB][32]
         }
-        const int64_t cw = 32 * g.V;
+        const int64_t cw = g.cw;
         g.Wc = std::min(g.warps, pow2_floor(std::max<int64_t>(1, (tile_w + cw - 1) / cw)));
         if ((int64_t)g.Wc * cw < tile_w && g.Wc < g.warps && (int64_t)g.Wc * cw * 2 <= tile_w + cw - 1) g.Wc *= 2;
         g.Wk = g.warps / g.Wc;
@@ -688,12 +696,12 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
             const int cls = class_of(k, dtype);
             while (cur_cls < cls) cls_begin[++cur_cls] = (int32_t)items.size();
             const ClassGeom &g = geom[cls];
-            const int64_t tiles_y = (tile_w + (int64_t)32 * g.V * g.Wc - 1) / ((int64_t)32 * g.V * g.Wc);
+            const int64_t tiles_y = (tile_w + (int64_t)g.cw * g.Wc - 1) / ((int64_t)g.cw * g.Wc);
             const int64_t chunks_wanted = std::max<int64_t>(1, (int64_t)148 * 16 / tiles_y);
             const int64_t cost_budget = std::max<int64_t>(1, total_cost / chunks_wanted);
             const int64_t cost1 = std::max<int64_t>(1, sig_cost[sg]);
             int64_t chunk = std::max<int64_t>(g.Wk, (cost_budget + cost1 - 1) / cost1);
-            chunk = std::min<int64_t>(chunk, (cls == CLS_LONG ? LONG_LIT_CHUNK : LIT_CHUNK) / k);
+            chunk = std::min<int64_t>(chunk, (cls == CLS_LONG && dtype == 64 ? LONG_LIT_CHUNK : LIT_CHUNK) / k);
             chunk = std::max<int64_t>(1, chunk);
             for (int32_t s = j; s < e; s += (int32_t)chunk) {
                 Item it;

@@ -86,10 +86,14 @@ template <> __device__ __forceinline__ float fma_<float>(float a, float b, float
 template <> __device__ __forceinline__ double fma_<double>(double a, double b, double c) { return fma(a, b, c); }
 
 // ---- vector gather / vector RED ------------------------------------------------------------------
+// scalar RED as inline PTX: atomicAdd on a pointer the compiler cannot prove global compiles to ATOM plus a
+// shared-window test with a CAS fallback
+__device__ __forceinline__ void red_add(float *p, float v) { asm volatile("red.global.add.f32 [%0], %1;" ::"l"(p), "f"(v) : "memory"); }
+__device__ __forceinline__ void red_add(double *p, double v) { asm volatile("red.global.add.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory"); }
 template <typename T, int V> struct VecIO;
 template <> struct VecIO<float, 1> {
     static __device__ __forceinline__ void load(const float *p, float (&v)[1]) { v[0] = __ldg(p); }
-    static __device__ __forceinline__ void red(float *p, const float (&v)[1]) { atomicAdd(p, v[0]); }
+    static __device__ __forceinline__ void red(float *p, const float (&v)[1]) { red_add(p, v[0]); }
 };
 template <> struct VecIO<float, 2> {
     static __device__ __forceinline__ void load(const float *p, float (&v)[2])
@@ -116,7 +120,7 @@ template <> struct VecIO<float, 4> {
 };
 template <> struct VecIO<double, 1> {
     static __device__ __forceinline__ void load(const double *p, double (&v)[1]) { v[0] = __ldg(p); }
-    static __device__ __forceinline__ void red(double *p, const double (&v)[1]) { atomicAdd(p, v[0]); }
+    static __device__ __forceinline__ void red(double *p, const double (&v)[1]) { red_add(p, v[0]); }
 };
 template <> struct VecIO<double, 2> {
     static __device__ __forceinline__ void load(const double *p, double (&v)[2])
@@ -126,7 +130,7 @@ template <> struct VecIO<double, 2> {
     }
     static __device__ __forceinline__ void red(double *p, const double (&v)[2])
     {
-        atomicAdd(p, v[0]); atomicAdd(p + 1, v[1]);
+        red_add(p, v[0]); red_add(p + 1, v[1]);
     }
 };
 
@@ -1106,7 +1110,7 @@ __global__ void __launch_bounds__(LONG_THREADS) k_eval_blk(const EvalParams<T> p
                     if (i < k) {                                        // warp-uniform
                         const int32_t lit = L[i];
                         if (!(lit & LIT_FIXED))
-                            atomicAdd(reinterpret_cast<T *>(gb + (uint64_t)(uint32_t)(lit & LIT_VAR) * g_ld), flip_sign(g[i], lit));
+                            red_add(reinterpret_cast<T *>(gb + (uint64_t)(uint32_t)(lit & LIT_VAR) * g_ld), flip_sign(g[i], lit));
                     }
                 }
             }
@@ -1454,10 +1458,10 @@ __global__ void k_reset_state(int B, uint8_t *is_solution, int32_t *first_step)
 }
 #endif
 
-// The fp32 instantiation of the scalar register kernel (bodies for 56 lengths) is compiled in its own translation
-// unit (afsat_km32.cu) so that the two halves of the build run in parallel; everyone else only declares it.
+// The fp32 instantiation of the scalar register kernel is compiled in its own translation unit (afsat_km32.cu) so
+// that the parts of the build run in parallel; everyone else only declares it.
 #ifndef AFSAT_B_KMAX32
-#define AFSAT_B_KMAX32 64             // fp32: the scalar register kernel up to this length
+#define AFSAT_B_KMAX32 20             // fp32: the scalar register kernel up to this length (beyond: afsat_split.cuh)
 #endif
 #ifndef AFSAT_B_MINB
 #define AFSAT_B_MINB 1

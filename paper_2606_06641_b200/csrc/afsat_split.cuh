@@ -1,0 +1,256 @@
+// afsat_split.cuh -- lane-split register kernel for LONG fp32 constraints (k > AFSAT_B_KMAX32;
+// DESIGN.md 6.2b).  Internal to the library.
+//
+// One (constraint, candidate) evaluation is shared by NS lanes of a warp: lane (h, c) -- h = lane / (32 / NS),
+// c = lane % (32 / NS) -- owns the literals j = i NS + h, i < KS = ceil(k / NS), of candidate c.  Per DFT point
+// every lane walks ITS literals forward (prefixes of its own partial product), the NS partial
+// products are exchanged with warp shuffles, and the backward walk is seeded with  w b x (product of the OTHER
+// lanes' partial products):  the leave-one-out product of literal i in lane h is
+//     prefix_h(i) x suffix_h(i) x prod_{h' != h} P_h',
+// still a product of factors, never a division (north_star).  Every intermediate of a point -- the KS literal values,
+// factors, prefixes and partial gradients of the lane -- then fits in registers WITHOUT spills at k = 64, at twice the
+// warps per SM of the one-lane-per-candidate kernel (k_eval_km: 255 registers, spills beyond k ~ 36); the arithmetic
+// per literal and point is the same 12 instructions, plus one exchange (2 (NS - 1) shuffles, NS - 1 + 2 complex
+// multiplies) per point.  Literals missing from the last row (j >= k) are unit factors.
+#pragma once
+#include "afsat_internal.h"
+#include "afsat_kernels.cuh"
+
+namespace afsat {
+
+#ifndef AFSAT_L32_NS
+#define AFSAT_L32_NS 2                 // lanes per (constraint, candidate)
+#endif
+#ifndef AFSAT_L32_THREADS
+#define AFSAT_L32_THREADS 384             // 12 warps per SM at 168 registers (measured: 256 / 255 regs 5 % slower)
+#endif
+#ifndef AFSAT_L32_MINB
+#define AFSAT_L32_MINB 1
+#endif
+#ifndef AFSAT_L32_CHAINS
+#define AFSAT_L32_CHAINS 2             // independent product chains per thread at a complex point
+#endif
+#ifndef AFSAT_L32_PREFETCH
+#define AFSAT_L32_PREFETCH 1
+#endif
+#ifndef AFSAT_L32_KMIN
+#define AFSAT_L32_KMIN (AFSAT_B_KMAX32 + 1)
+#endif
+
+// product of the OTHER lanes' values (NS = 2: the partner's; NS = 4: butterfly over lane bits log2(CW), log2(CW) + 1)
+template <int NS>
+__device__ __forceinline__ float others_real(unsigned mask, float v)
+{
+    constexpr int CW = 32 / NS;
+    if (NS == 2) return __shfl_xor_sync(mask, v, CW);
+    const float n1 = __shfl_xor_sync(mask, v, CW);
+    const float po = __shfl_xor_sync(mask, v * n1, 2 * CW);
+    return n1 * po;
+}
+template <int NS>
+__device__ __forceinline__ void others_cplx(unsigned mask, float vr, float vi, float &orr, float &oi)
+{
+    constexpr int CW = 32 / NS;
+    const float n1r = __shfl_xor_sync(mask, vr, CW), n1i = __shfl_xor_sync(mask, vi, CW);
+    if (NS == 2) { orr = n1r; oi = n1i; return; }
+    const float ppr = fmaf(vr, n1r, -(vi * n1i)), ppi = fmaf(vr, n1i, vi * n1r);
+    const float por = __shfl_xor_sync(mask, ppr, 2 * CW), poi = __shfl_xor_sync(mask, ppi, 2 * CW);
+    orr = fmaf(n1r, por, -(n1i * poi)); oi = fmaf(n1r, poi, n1i * por);
+}
+
+// a2-a4 for the lane's KS literals of one constraint; tab rows as in eval_points_reg ({Re a, Im a, Re b, Im b,
+// Re w, Im w, Re(w b), Im(w b)}, real rows first).  miss: the lane's LAST literal does not exist (unit factor).
+template <int KS, int NS, bool GRAD>
+__device__ __forceinline__ void eval_points_split(unsigned mask, const float (&y)[KS], bool miss,
+                                                  const float *__restrict__ tab, int n_real, int n_cplx, float &fe,
+                                                  float (&g)[KS])
+{
+    const float *r = tab;
+    for (int p = 0; p < n_real; ++p, r += 8) {                       // self-conjugate points
+        const float a = r[0], b = r[2], w = r[4], wb = r[6];
+        float pre[KS], f[KS];
+#pragma unroll
+        for (int i = 0; i < KS; ++i) f[i] = fmaf(b, y[i], a);
+        if (miss) f[KS - 1] = 1.0f;
+        float run = f[0];
+#pragma unroll
+        for (int i = 1; i < KS; ++i) { pre[i] = run; run *= f[i]; }
+        const float oth = others_real<NS>(mask, run);
+        fe = fmaf(w, run * oth, fe);
+        if (GRAD) {
+            float suf = wb * oth;
+#pragma unroll
+            for (int i = KS - 1; i >= 1; --i) { g[i] = fmaf(pre[i], suf, g[i]); suf *= f[i]; }
+            g[0] += suf;                                              // prefix_0 = 1
+        }
+    }
+    // complex points: the lane's literals are walked as TWO independent chains, A = [0, KA) and B = [KA, KS) -- the
+    // same leave-one-out identity one level down (LOO_i = prefix_A(i) suffix_A(i) P_B others) -- so that a thread
+    // always has two dependent FMUL -> FFMA sequences in flight (with 3 warps per scheduler one chain per thread
+    // leaves the issue slots idle on fixed-latency waits: profiles/r1_eval_split_cfg3.md)
+    constexpr int KA = AFSAT_L32_CHAINS == 2 ? KS / 2 : KS, KB = KS - KA;
+    for (int p = 0; p < n_cplx; ++p, r += 8) {                       // one of each conjugate pair
+        const float ar = r[0], ai = r[1], br = r[2], bi = r[3], wr = r[4], wi = r[5], wbr = r[6], wbi = r[7];
+        float pr[KS], pi[KS], fr[KS], fi[KS];
+#pragma unroll
+        for (int i = 0; i < KS; ++i) { fr[i] = fmaf(br, y[i], ar); fi[i] = fmaf(bi, y[i], ai); }
+        if (miss) { fr[KS - 1] = 1.0f; fi[KS - 1] = 0.0f; }
+        float rr = fr[0], ri = fi[0], qr = 1.0f, qi = 0.0f;
+        if (KB > 0) { qr = fr[KA]; qi = fi[KA]; }
+#pragma unroll
+        for (int i = 1; i < (KA > KB ? KA : KB); ++i) {
+            if (i < KA) {
+                pr[i] = rr; pi[i] = ri;
+                const float nr = fmaf(rr, fr[i], -(ri * fi[i]));
+                const float ni = fmaf(rr, fi[i], ri * fr[i]);
+                rr = nr; ri = ni;
+            }
+            if (i < KB) {
+                pr[KA + i] = qr; pi[KA + i] = qi;
+                const float nr = fmaf(qr, fr[KA + i], -(qi * fi[KA + i]));
+                const float ni = fmaf(qr, fi[KA + i], qi * fr[KA + i]);
+                qr = nr; qi = ni;
+            }
+        }
+        float lr = rr, li = ri;                                       // the lane's partial product P_A P_B
+        if (KB > 0) { lr = fmaf(rr, qr, -(ri * qi)); li = fmaf(rr, qi, ri * qr); }
+        float orr, oi;
+        others_cplx<NS>(mask, lr, li, orr, oi);
+        const float tr = fmaf(lr, orr, -(li * oi)), ti = fmaf(lr, oi, li * orr);   // P_l, the whole product
+        fe = fmaf(wr, tr, fe);
+        fe = fmaf(-wi, ti, fe);
+        if (GRAD) {
+            const float zr = fmaf(wbr, orr, -(wbi * oi)), zi = fmaf(wbr, oi, wbi * orr);   // w b x others
+            float sr = zr, si = zi, ur = zr, ui = zi;                 // suffix of chain A seeded with z P_B, of B with z P_A
+            if (KB > 0) {
+                sr = fmaf(zr, qr, -(zi * qi)); si = fmaf(zr, qi, zi * qr);
+                ur = fmaf(zr, rr, -(zi * ri)); ui = fmaf(zr, ri, zi * rr);
+            }
+#pragma unroll
+            for (int i = (KA > KB ? KA : KB) - 1; i >= 1; --i) {
+                if (i < KA) {
+                    g[i] = fmaf(pr[i], sr, g[i]);
+                    g[i] = fmaf(-pi[i], si, g[i]);
+                    const float nr = fmaf(sr, fr[i], -(si * fi[i]));
+                    const float ni = fmaf(sr, fi[i], si * fr[i]);
+                    sr = nr; si = ni;
+                }
+                if (i < KB) {
+                    g[KA + i] = fmaf(pr[KA + i], ur, g[KA + i]);
+                    g[KA + i] = fmaf(-pi[KA + i], ui, g[KA + i]);
+                    const float nr = fmaf(ur, fr[KA + i], -(ui * fi[KA + i]));
+                    const float ni = fmaf(ur, fi[KA + i], ui * fr[KA + i]);
+                    ur = nr; ui = ni;
+                }
+            }
+            g[0] += sr;                                               // prefix_0 = 1 in both chains
+            if (KB > 0) g[KA] += ur;
+        }
+    }
+}
+
+template <int KS, int NS, bool GRAD, bool FIXED>
+__device__ __forceinline__ void run_item_split(const EvalParams<float> &p, unsigned mask, const int32_t *__restrict__ s_lits,
+                                               const float *__restrict__ s_tab, int n_real, int n_cplx, int nc, int wk,
+                                               int h, int64_t b, float &fe, int k)
+{
+    const char *xb = reinterpret_cast<const char *>(p.x + b);
+    char *gb = reinterpret_cast<char *>(p.G + (b - p.g_b0));
+    const uint32_t x_ld = (uint32_t)(p.ldb * 4), g_ld = (uint32_t)(p.g_ld * 4);
+    const int Wk = p.Wk;
+    const bool miss = (KS - 1) * NS + h >= k;
+    for (int c = wk; c < nc; c += Wk) {
+        const int32_t *L = s_lits + c * k + h;
+        int32_t lit[KS];
+        float y[KS], g[KS];
+#pragma unroll
+        for (int i = 0; i < KS - 1; ++i) lit[i] = L[i * NS];
+        lit[KS - 1] = miss ? LIT_FIXED : L[(KS - 1) * NS];            // missing literal: constant, no gather, no RED
+#pragma unroll
+        for (int i = 0; i < KS; ++i) {
+            if ((FIXED || i == KS - 1) && (lit[i] & LIT_FIXED)) y[i] = 1.0f;
+            else y[i] = __ldg(reinterpret_cast<const float *>(xb + (uint64_t)(uint32_t)(lit[i] & LIT_VAR) * x_ld));
+            y[i] = flip_sign(y[i], lit[i]);
+            g[i] = 0.0f;
+        }
+#if AFSAT_L32_PREFETCH
+        if (c + Wk < nc) {                                            // the NEXT constraint's row segments into L1: with 2-3
+            const int32_t *Ln = L + Wk * k;                           // warps per scheduler nothing else hides its gathers
+#pragma unroll
+            for (int i = 0; i < KS; ++i) {
+                if (i == KS - 1 && miss) continue;
+                const int32_t ln = Ln[i * NS];
+                if (FIXED && (ln & LIT_FIXED)) continue;
+                asm volatile("prefetch.global.L1 [%0];" ::"l"(xb + (uint64_t)(uint32_t)(ln & LIT_VAR) * x_ld));
+            }
+        }
+#endif
+        eval_points_split<KS, NS, GRAD>(mask, y, miss, s_tab, n_real, n_cplx, fe, g);
+        if (GRAD) {
+#pragma unroll
+            for (int i = 0; i < KS; ++i) {
+                if ((FIXED || i == KS - 1) && (lit[i] & LIT_FIXED)) continue;   // masked gradient
+                const float gi[1] = {flip_sign(g[i], lit[i])};
+                VecIO<float, 1>::red(reinterpret_cast<float *>(gb + (uint64_t)(uint32_t)(lit[i] & LIT_VAR) * g_ld), gi);
+            }
+        }
+    }
+}
+
+template <int KS, int NS, bool GRAD>
+__device__ __noinline__ void item_body_split(const EvalParams<float> &p, const int32_t *s_lits, const float *s_tab,
+                                             float (*s_F)[32], int n_real, int n_cplx, int nc, bool has_fixed, int k)
+{
+    constexpr int CW = 32 / NS;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int h = lane / CW, cl = lane % CW;
+    const int wc = warp % p.Wc, wk = warp / p.Wc;
+    const int64_t b = p.b_begin + ((int64_t)blockIdx.y * p.Wc + wc) * CW + cl;
+    const bool active = b < p.b_end && b < p.B && !lane_skipped(p, b, 1);   // the NS lanes of a candidate agree
+    const unsigned mask = __ballot_sync(0xffffffffu, active);
+    float fe = 0.0f;
+    if (active) {
+        if (has_fixed) run_item_split<KS, NS, GRAD, true>(p, mask, s_lits, s_tab, n_real, n_cplx, nc, wk, h, b, fe, k);
+        else run_item_split<KS, NS, GRAD, false>(p, mask, s_lits, s_tab, n_real, n_cplx, nc, wk, h, b, fe, k);
+    }
+    if (!p.Fpart) return;
+    s_F[warp][lane] = fe;
+    __syncthreads();
+    if (wk == 0 && h == 0 && active) {                                // fixed order over the Wk constraint groups
+        float s = 0.0f;
+        for (int g = 0; g < p.Wk; ++g) s += s_F[warp + g * p.Wc][lane];
+        p.Fpart[(int64_t)(p.frow_base + blockIdx.x) * p.ldb + b] = s;
+    }
+}
+
+template <int KS, int KSHI, int NS, bool GRAD>
+struct SwitchSplit {
+    static __device__ __forceinline__ void go(int ks, const EvalParams<float> &p, const int32_t *s_lits, const float *s_tab,
+                                              float (*s_F)[32], int n_real, int n_cplx, int nc, bool has_fixed, int k)
+    {
+        if (ks == KS) item_body_split<KS, NS, GRAD>(p, s_lits, s_tab, s_F, n_real, n_cplx, nc, has_fixed, k);
+        else if (KS < KSHI) SwitchSplit<(KS < KSHI ? KS + 1 : KS), KSHI, NS, GRAD>::go(ks, p, s_lits, s_tab, s_F, n_real, n_cplx, nc, has_fixed, k);
+    }
+};
+
+// one launch for every length in [KLO, KHI]: the CTA's item picks the body compiled for ceil(k / NS) literals per lane
+template <int KLO, int KHI, int NS, bool GRAD, int THREADS, int MINB>
+__global__ void __launch_bounds__(THREADS, MINB) k_eval_split(const EvalParams<float> p)
+{
+    __shared__ __align__(16) float s_tab[((KHI + 1) / 2 + 1) * 8];
+    __shared__ int32_t s_lits[LIT_CHUNK];
+    __shared__ float s_F[THREADS / 32][32];
+    const Item it = p.items[blockIdx.x];
+    const SigDev sg = p.sigs[it.sig];
+    stage_item(p, it, sg, s_tab, s_lits);
+    __syncthreads();
+    SwitchSplit<(KLO + NS - 1) / NS, (KHI + NS - 1) / NS, NS, GRAD>::go((it.k + NS - 1) / NS, p, s_lits, s_tab, s_F, sg.n_real,
+                                                                        sg.n_cplx, it.c_end - it.c_begin, it.has_fixed != 0, it.k);
+}
+
+#ifndef AFSAT_KS32_TU   // instantiated in afsat_ks32.cu
+extern template __global__ void k_eval_split<AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, true, AFSAT_L32_THREADS, AFSAT_L32_MINB>(const EvalParams<float>);
+extern template __global__ void k_eval_split<AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, false, AFSAT_L32_THREADS, AFSAT_L32_MINB>(const EvalParams<float>);
+#endif
+
+}  // namespace afsat
