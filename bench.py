@@ -133,8 +133,9 @@ def oracle_sample(inst, x0, target_s=15.0, max_b=64):
     waves = int(max(1, min(target_s / per_wave, max(1, max_b * 8 // max(cores, 1)))))
     b_o = int(min(inst.batch, max(probe_b, waves * cores)))
     t0 = time.perf_counter()
-    O.step(inst, x0[:, :b_o].astype(np.float64), inst.eta, 1, b_o, want_F=False)
+    X1, _, sat1, _, _ = O.step(inst, x0[:, :b_o].astype(np.float64), inst.eta, 1, b_o, want_F=False)
     dt = time.perf_counter() - t0
+    oracle_sample.last = (X1[:, :b_o], sat1[:b_o])          # X(1) and the counts on X(1), for the deviation report
     return {"value": inst.n_cons * b_o * 1 / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": f"oracle_step (long double, gcc -O2, OpenMP over candidates) on the first {b_o} of "
                       f"{inst.batch} candidates x 1 step over all {inst.n_cons} constraints, {dt:.2f} s"}, dt, b_o
@@ -409,16 +410,27 @@ def run_ours(args):
                         "instructions than that at the points 1, -1, i (trivial twiddles, DESIGN.md 6.1)"}
         if clocks.get("sm_mhz"):
             roof["frac_at_observed_clock"] = roof["frac"] * peaks["sm_max_mhz"] / clocks["sm_mhz"]
-        cb = None
+        cb = dev_rep = None
         if world == 1 or rank == 0:
-            cb, _, _ = oracle_sample(inst, x0.astype(np.float64), target_s=args.oracle_seconds)
+            cb, _, b_o = oracle_sample(inst, x0.astype(np.float64), target_s=args.oracle_seconds)
+            # deviation vs the oracle (BASELINE.json configs[3]: "report deviation vs oracle"): ONE step from x0
+            # on the GPU against the oracle's step on the sampled candidates -- X(1) = clamp(x0 - eta G), so
+            # max|dX| / eta is the gradient deviation where the clamp is inactive; counts are bit-exact or not
+            X1o, sat1o = oracle_sample.last
+            xd = torch.from_numpy(np.ascontiguousarray(x0)).cuda()
+            _, sat_d, _, _ = ctx.step(xd, inst.eta, 1, step_base=0, state=None, want_F=False)
+            torch.cuda.synchronize()
+            dX = np.abs(xd[:, :b_o].double().cpu().numpy() - X1o)
+            dev_rep = {"candidates": int(b_o), "max_abs_dX_after_one_step": float(dX.max()),
+                       "max_abs_dG_implied": float(dX.max() / inst.eta),
+                       "sat_count_bit_exact": bool(np.array_equal(sat_d[:b_o].cpu().numpy(), sat1o))}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
                 "ms_per_step": 1e3 * t_total / K, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f32" if dtype == 32 else "f64", "data": "synthetic",
                 "config": config_dict(inst, args), "clocks": clocks, "gpu_launches": int(launches),
                 "e2e": {"value": world * m * B * K / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d,
                         "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * t_e2e / K},
-                "roofline": roof, "cpu_baseline": cb,
+                "roofline": roof, "cpu_baseline": cb, "deviation_vs_oracle": dev_rep,
                 "value_l2_warm": world * m * B * K / t_warm, "ms_per_step_l2_warm": 1e3 * t_warm / K,
                 "solved_candidates": int(sol.sum().item()), "wall_s_timed_region": wall}
         if ttfs is not None:

@@ -599,3 +599,31 @@ def test_full_size_cfg3_sampled_fp64():
 
 def test_full_size_cfg4_sampled():
     _sampled_full_size(4)
+
+
+def test_full_size_cfg3_sampled_fp32():
+    """cfg3 at full size in fp32 -- the launch configuration bench.py times for `--config 3` (the lane-split
+    kernel, k = 30..50): robust tables (B4) at the tight bound; the paper's tables at the loose long-constraint
+    bound of DESIGN.md §8 (the product form loses precision with k; at uniform x0 SURVEY.md
+    App. C measures <= 2e-4 per constraint, a gradient component sums ~80 partials)."""
+    inst = I.make_config(3)
+    B = inst.batch
+    x0 = I.make_x0(inst, dtype=np.float32)
+    rng = np.random.default_rng(99 + 3)
+    cols = np.unique(np.concatenate([np.arange(3), rng.integers(0, B, size=3), [B - 1]]))
+    xs_p = np.zeros((inst.n_vars, 32), dtype=np.float64)
+    xs_p[:, :cols.size] = x0[:, cols]
+    Fo, Go = O.eval_grad(inst, xs_p, cols.size)
+    so, lo = O.check(inst, xs_p, cols.size)
+    for flags, ftol, gtol in ((Bd.FLAG_ROBUST, 1e-4 * inst.n_cons, 1e-4), (0, 1e-4 * inst.n_cons + 1e-2, 2e-2)):
+        ctx = Bd.Context.from_instance(inst, dtype=32, flags=flags)
+        x = dev(x0)
+        F, G = ctx.eval_grad(x)
+        sat, sol = ctx.check(x)
+        torch.cuda.synchronize()
+        Fg = F.cpu().numpy().astype(np.float64)[cols]
+        Gg = G[:, torch.from_numpy(cols).cuda()].cpu().numpy().astype(np.float64)
+        assert np.array_equal(sat.cpu().numpy()[cols], so) and np.array_equal(sol.cpu().numpy()[cols], lo)
+        assert np.abs(Fg - Fo).max() <= ftol, (flags, np.abs(Fg - Fo).max())
+        assert np.abs(Gg - Go[:, :cols.size]).max() <= gtol, (flags, np.abs(Gg - Go[:, :cols.size]).max())
+        ctx.close()
