@@ -205,6 +205,12 @@ void (*pick_b(bool grad))(EvalParams<T>)
 {
     using Fn = void (*)(EvalParams<T>);
     constexpr int KHI = sizeof(T) == 4 ? AFSAT_B_KMAX32 : AFSAT_B_KMAX64;
+#if AFSAT_M32_PACKED
+    if constexpr (sizeof(T) == 4)                                      // fp32: the packed lane-split kernel
+        return grad ? (Fn)k_eval_split<9, AFSAT_B_KMAX32, 2, 2, true, AFSAT_M32_THREADS, 1>
+                    : (Fn)k_eval_split<9, AFSAT_B_KMAX32, 2, 2, false, AFSAT_M32_THREADS, 1>;
+    else
+#endif
     return grad ? (Fn)k_eval_km<T, 9, KHI, 1, true, AFSAT_B_MINB> : (Fn)k_eval_km<T, 9, KHI, 1, false, AFSAT_B_MINB>;
 }
 
@@ -215,8 +221,8 @@ void (*pick_long(int km, bool grad))(EvalParams<T>)
 {
     using Fn = void (*)(EvalParams<T>);
     if constexpr (sizeof(T) == 4) {                                    // fp32: the lane-split register kernel
-        return grad ? (Fn)k_eval_split<AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, true, AFSAT_L32_THREADS, AFSAT_L32_MINB>
-                    : (Fn)k_eval_split<AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, false, AFSAT_L32_THREADS, AFSAT_L32_MINB>;
+        return grad ? (Fn)k_eval_split<AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, 1, true, AFSAT_L32_THREADS, AFSAT_L32_MINB>
+                    : (Fn)k_eval_split<AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, 1, false, AFSAT_L32_THREADS, AFSAT_L32_MINB>;
     } else {
 #define AFSAT_LONG_CASE(KM_)                                                                                  \
     case KM_:                                                                                                 \
@@ -666,6 +672,12 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
         g.V = (cls == CLS_S) ? 4 : (cls == CLS_A && dtype == 32) ? AFSAT_A_V : 1;
         g.warps = CTA_WARPS;
         g.cw = 32 * g.V;
+#if AFSAT_M32_PACKED
+        if (cls == CLS_B && dtype == 32) {                             // packed lane-split kernel: 2 lanes x 2 candidates
+            g.warps = AFSAT_M32_THREADS / 32;
+            g.cw = 32;
+        } else
+#endif
         if (cls == CLS_LONG && dtype == 32) {                          // lane-split kernel: NS lanes per candidate
             g.warps = AFSAT_L32_THREADS / 32;
             g.cw = 32 / AFSAT_L32_NS;

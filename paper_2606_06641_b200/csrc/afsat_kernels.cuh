@@ -1466,7 +1466,10 @@ __global__ void k_reset_state(int B, uint8_t *is_solution, int32_t *first_step)
 #ifndef AFSAT_B_MINB
 #define AFSAT_B_MINB 1
 #endif
-#ifndef AFSAT_KM32_TU
+#ifndef AFSAT_M32_PACKED
+#define AFSAT_M32_PACKED 1             // fp32, 9 <= k <= AFSAT_B_KMAX32: the packed lane-split kernel (afsat_split.cuh)
+#endif                                 // instead of k_eval_km<float>
+#if !defined(AFSAT_KM32_TU) && !AFSAT_M32_PACKED
 extern template __global__ void k_eval_km<float, 9, AFSAT_B_KMAX32, 1, true, AFSAT_B_MINB>(const EvalParams<float>);
 extern template __global__ void k_eval_km<float, 9, AFSAT_B_KMAX32, 1, false, AFSAT_B_MINB>(const EvalParams<float>);
 #endif

@@ -30,6 +30,9 @@ namespace afsat {
 #ifndef AFSAT_L32_CHAINS
 #define AFSAT_L32_CHAINS 2             // independent product chains per thread at a complex point
 #endif
+#ifndef AFSAT_M32_THREADS
+#define AFSAT_M32_THREADS 384
+#endif
 #ifndef AFSAT_L32_PREFETCH
 #define AFSAT_L32_PREFETCH 1
 #endif
@@ -223,34 +226,196 @@ __device__ __noinline__ void item_body_split(const EvalParams<float> &p, const i
     }
 }
 
-template <int KS, int KSHI, int NS, bool GRAD>
+// ---- packed form (V = 2): a lane holds TWO adjacent candidates as f32x2 pairs and every product is an FFMA2 / FMUL2
+// (DESIGN.md 6.1 "FFMA2"): half the issue slots for the same flops.  FFMA2 has no negated operands, so -Im f is made by
+// XOR on the ALU pipe and the backward walk carries the suffix as (Re s, -Im s).  12 registers per literal, so this
+// form serves the lengths whose KS fits the register budget (9 <= k <= AFSAT_B_KMAX32).
+constexpr f32x2 SGN2 = 0x8000000080000000ull;
+__device__ __forceinline__ f32x2 shfl2(unsigned mask, f32x2 v, int d)
+{
+    float lo, hi; upk(v, lo, hi);
+    return pk(__shfl_xor_sync(mask, lo, d), __shfl_xor_sync(mask, hi, d));
+}
+
+template <int KS, int NS, bool GRAD>
+__device__ __forceinline__ void eval_points_split2(unsigned mask, const f32x2 (&y)[KS], bool miss,
+                                                   const float *__restrict__ tab, int n_real, int n_cplx, f32x2 &fe,
+                                                   f32x2 (&g)[KS])
+{
+    static_assert(NS == 2, "the packed form exchanges with one partner");
+    constexpr int CW = 32 / NS;
+    const f32x2 one2 = pk(1.0f, 1.0f);
+    const float *r = tab;
+    for (int p = 0; p < n_real; ++p, r += 8) {                       // self-conjugate points
+        const f32x2 a = pk(r[0], r[0]), b = pk(r[2], r[2]), w = pk(r[4], r[4]), wb = pk(r[6], r[6]);
+        f32x2 pre[KS], f[KS];
+#pragma unroll
+        for (int i = 0; i < KS; ++i) f[i] = fma2(b, y[i], a);
+        if (miss) f[KS - 1] = one2;
+        f32x2 run = f[0];
+#pragma unroll
+        for (int i = 1; i < KS; ++i) { pre[i] = run; run = mul2(run, f[i]); }
+        const f32x2 oth = shfl2(mask, run, CW);
+        fe = fma2(w, mul2(run, oth), fe);
+        if (GRAD) {
+            f32x2 suf = mul2(wb, oth);
+#pragma unroll
+            for (int i = KS - 1; i >= 1; --i) { g[i] = fma2(pre[i], suf, g[i]); suf = mul2(suf, f[i]); }
+            g[0] = add2(g[0], suf);                                   // prefix_0 = 1
+        }
+    }
+    for (int p = 0; p < n_cplx; ++p, r += 8) {                       // one of each conjugate pair
+        const f32x2 ar = pk(r[0], r[0]), ai = pk(r[1], r[1]), br = pk(r[2], r[2]), bi = pk(r[3], r[3]);
+        f32x2 pr[KS], pi[KS], fr[KS], fi[KS];
+#pragma unroll
+        for (int i = 0; i < KS; ++i) { fr[i] = fma2(br, y[i], ar); fi[i] = fma2(bi, y[i], ai); }
+        if (miss) { fr[KS - 1] = one2; fi[KS - 1] = 0ull; }
+        f32x2 rr = fr[0], ri = fi[0];
+#pragma unroll
+        for (int i = 1; i < KS; ++i) {
+            pr[i] = rr; pi[i] = ri;
+            const f32x2 nr = fma2(rr, fr[i], mul2(ri, fi[i] ^ SGN2));   // Re: rr fr - ri fi
+            const f32x2 ni = fma2(rr, fi[i], mul2(ri, fr[i]));          // Im: rr fi + ri fr
+            rr = nr; ri = ni;
+        }
+        const f32x2 orr = shfl2(mask, rr, CW), oi = shfl2(mask, ri, CW);
+        const f32x2 tr = fma2(rr, orr, mul2(ri, oi ^ SGN2)), ti = fma2(rr, oi, mul2(ri, orr));   // P_l, the whole product
+        fe = fma2(pk(r[4], r[4]), tr, fe);
+        fe = fma2(pk(-r[5], -r[5]), ti, fe);
+        if (GRAD) {
+            const f32x2 wbr = pk(r[6], r[6]), wbi = pk(r[7], r[7]);
+            f32x2 sr = fma2(wbr, orr, mul2(wbi, oi ^ SGN2));           // suffix (Re s, -Im s) seeded with w b x other
+            f32x2 nsi = fma2(wbr, oi, mul2(wbi, orr)) ^ SGN2;
+#pragma unroll
+            for (int i = KS - 1; i >= 1; --i) {
+                g[i] = fma2(pr[i], sr, g[i]);
+                g[i] = fma2(pi[i], nsi, g[i]);                        // Re(prefix x suffix)
+                const f32x2 nr = fma2(sr, fr[i], mul2(nsi, fi[i]));
+                const f32x2 nn = fma2(nsi, fr[i], mul2(sr, fi[i] ^ SGN2));
+                sr = nr; nsi = nn;
+            }
+            g[0] = add2(g[0], sr);                                    // prefix_0 = 1
+        }
+    }
+}
+
+template <int KS, int NS, bool GRAD, bool FIXED>
+__device__ __forceinline__ void run_item_split2(const EvalParams<float> &p, unsigned mask, const int32_t *__restrict__ s_lits,
+                                                const float *__restrict__ s_tab, int n_real, int n_cplx, int nc, int wk,
+                                                int h, int64_t b, f32x2 &fe, int k)
+{
+    const char *xb = reinterpret_cast<const char *>(p.x + b);
+    char *gb = reinterpret_cast<char *>(p.G + (b - p.g_b0));
+    const uint32_t x_ld = (uint32_t)(p.ldb * 4), g_ld = (uint32_t)(p.g_ld * 4);
+    const int Wk = p.Wk;
+    const bool miss = (KS - 1) * NS + h >= k;
+    const f32x2 one2 = pk(1.0f, 1.0f);
+    for (int c = wk; c < nc; c += Wk) {
+        const int32_t *L = s_lits + c * k + h;
+        int32_t lit[KS];
+        f32x2 y[KS], g[KS];
+#pragma unroll
+        for (int i = 0; i < KS - 1; ++i) lit[i] = L[i * NS];
+        lit[KS - 1] = miss ? LIT_FIXED : L[(KS - 1) * NS];            // missing literal: constant, no gather, no RED
+#pragma unroll
+        for (int i = 0; i < KS; ++i) {
+            f32x2 v[1] = {one2};
+            if (!((FIXED || i == KS - 1) && (lit[i] & LIT_FIXED)))
+                PairIO<1>::load(xb + (uint64_t)(uint32_t)(lit[i] & LIT_VAR) * x_ld, v);
+            const uint32_t m = (uint32_t)(lit[i] & LIT_NEG);
+            y[i] = v[0] ^ (((f32x2)m << 32) | m);                     // y = s x
+            g[i] = 0ull;
+        }
+#if AFSAT_L32_PREFETCH
+        if (c + Wk < nc) {
+            const int32_t *Ln = L + Wk * k;
+#pragma unroll
+            for (int i = 0; i < KS; ++i) {
+                if (i == KS - 1 && miss) continue;
+                const int32_t ln = Ln[i * NS];
+                if (FIXED && (ln & LIT_FIXED)) continue;
+                asm volatile("prefetch.global.L1 [%0];" ::"l"(xb + (uint64_t)(uint32_t)(ln & LIT_VAR) * x_ld));
+            }
+        }
+#endif
+        eval_points_split2<KS, NS, GRAD>(mask, y, miss, s_tab, n_real, n_cplx, fe, g);
+        if (GRAD) {
+#pragma unroll
+            for (int i = 0; i < KS; ++i) {
+                if ((FIXED || i == KS - 1) && (lit[i] & LIT_FIXED)) continue;   // masked gradient
+                const uint32_t m = (uint32_t)(lit[i] & LIT_NEG);
+                const f32x2 gi[1] = {g[i] ^ (((f32x2)m << 32) | m)};
+                PairIO<1>::red(gb + (uint64_t)(uint32_t)(lit[i] & LIT_VAR) * g_ld, gi);
+            }
+        }
+    }
+}
+
+template <int KS, int NS, bool GRAD>
+__device__ __noinline__ void item_body_split2(const EvalParams<float> &p, const int32_t *s_lits, const float *s_tab,
+                                              float (*s_F)[64], int n_real, int n_cplx, int nc, bool has_fixed, int k)
+{
+    constexpr int CW = 32 / NS;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int h = lane / CW, cl = lane % CW;
+    const int wc = warp % p.Wc, wk = warp / p.Wc;
+    const int64_t b = p.b_begin + ((int64_t)blockIdx.y * p.Wc + wc) * (2 * CW) + 2 * cl;
+    const bool active = b < p.b_end && b < p.B && !lane_skipped(p, b, 2);   // the NS lanes of a candidate pair agree
+    const unsigned mask = __ballot_sync(0xffffffffu, active);
+    f32x2 fe2 = 0ull;
+    if (active) {
+        if (has_fixed) run_item_split2<KS, NS, GRAD, true>(p, mask, s_lits, s_tab, n_real, n_cplx, nc, wk, h, b, fe2, k);
+        else run_item_split2<KS, NS, GRAD, false>(p, mask, s_lits, s_tab, n_real, n_cplx, nc, wk, h, b, fe2, k);
+    }
+    if (!p.Fpart) return;
+    float f0, f1; upk(fe2, f0, f1);
+    s_F[warp][2 * lane] = f0; s_F[warp][2 * lane + 1] = f1;
+    __syncthreads();
+    if (wk == 0 && h == 0 && active) {                                // fixed order over the Wk constraint groups
+#pragma unroll
+        for (int v = 0; v < 2; ++v) {
+            float s = 0.0f;
+            for (int g = 0; g < p.Wk; ++g) s += s_F[warp + g * p.Wc][2 * lane + v];
+            if (b + v < p.B) p.Fpart[(int64_t)(p.frow_base + blockIdx.x) * p.ldb + b + v] = s;
+        }
+    }
+}
+
+template <int KS, int KSHI, int NS, int V, bool GRAD>
 struct SwitchSplit {
     static __device__ __forceinline__ void go(int ks, const EvalParams<float> &p, const int32_t *s_lits, const float *s_tab,
-                                              float (*s_F)[32], int n_real, int n_cplx, int nc, bool has_fixed, int k)
+                                              float (*s_F)[32 * V], int n_real, int n_cplx, int nc, bool has_fixed, int k)
     {
-        if (ks == KS) item_body_split<KS, NS, GRAD>(p, s_lits, s_tab, s_F, n_real, n_cplx, nc, has_fixed, k);
-        else if (KS < KSHI) SwitchSplit<(KS < KSHI ? KS + 1 : KS), KSHI, NS, GRAD>::go(ks, p, s_lits, s_tab, s_F, n_real, n_cplx, nc, has_fixed, k);
+        if (ks == KS) {
+            if constexpr (V == 2) item_body_split2<KS, NS, GRAD>(p, s_lits, s_tab, s_F, n_real, n_cplx, nc, has_fixed, k);
+            else item_body_split<KS, NS, GRAD>(p, s_lits, s_tab, s_F, n_real, n_cplx, nc, has_fixed, k);
+        } else if (KS < KSHI)
+            SwitchSplit<(KS < KSHI ? KS + 1 : KS), KSHI, NS, V, GRAD>::go(ks, p, s_lits, s_tab, s_F, n_real, n_cplx, nc, has_fixed, k);
     }
 };
 
 // one launch for every length in [KLO, KHI]: the CTA's item picks the body compiled for ceil(k / NS) literals per lane
-template <int KLO, int KHI, int NS, bool GRAD, int THREADS, int MINB>
+template <int KLO, int KHI, int NS, int V, bool GRAD, int THREADS, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB) k_eval_split(const EvalParams<float> p)
 {
     __shared__ __align__(16) float s_tab[((KHI + 1) / 2 + 1) * 8];
     __shared__ int32_t s_lits[LIT_CHUNK];
-    __shared__ float s_F[THREADS / 32][32];
+    __shared__ float s_F[THREADS / 32][32 * V];
     const Item it = p.items[blockIdx.x];
     const SigDev sg = p.sigs[it.sig];
     stage_item(p, it, sg, s_tab, s_lits);
     __syncthreads();
-    SwitchSplit<(KLO + NS - 1) / NS, (KHI + NS - 1) / NS, NS, GRAD>::go((it.k + NS - 1) / NS, p, s_lits, s_tab, s_F, sg.n_real,
+    SwitchSplit<(KLO + NS - 1) / NS, (KHI + NS - 1) / NS, NS, V, GRAD>::go((it.k + NS - 1) / NS, p, s_lits, s_tab, s_F, sg.n_real,
                                                                         sg.n_cplx, it.c_end - it.c_begin, it.has_fixed != 0, it.k);
 }
 
 #ifndef AFSAT_KS32_TU   // instantiated in afsat_ks32.cu
-extern template __global__ void k_eval_split<AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, true, AFSAT_L32_THREADS, AFSAT_L32_MINB>(const EvalParams<float>);
-extern template __global__ void k_eval_split<AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, false, AFSAT_L32_THREADS, AFSAT_L32_MINB>(const EvalParams<float>);
+extern template __global__ void k_eval_split<AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, 1, true, AFSAT_L32_THREADS, AFSAT_L32_MINB>(const EvalParams<float>);
+extern template __global__ void k_eval_split<AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, 1, false, AFSAT_L32_THREADS, AFSAT_L32_MINB>(const EvalParams<float>);
+#if AFSAT_M32_PACKED
+extern template __global__ void k_eval_split<9, AFSAT_B_KMAX32, 2, 2, true, AFSAT_M32_THREADS, 1>(const EvalParams<float>);
+extern template __global__ void k_eval_split<9, AFSAT_B_KMAX32, 2, 2, false, AFSAT_M32_THREADS, 1>(const EvalParams<float>);
+#endif
 #endif
 
 }  // namespace afsat

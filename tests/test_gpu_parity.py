@@ -160,7 +160,13 @@ def test_every_length_9_to_64(with_fixed):
     Fr, Gr = run_eval(inst, x, 70, 32, flags=Bd.FLAG_ROBUST)
     assert np.abs(Fr - Fo).max() <= 1e-4 * inst.n_cons and np.abs(Gr[:, :70] - Go[:, :70]).max() <= 1e-4
     F, G = run_eval(inst, x, 70, 32)
-    assert np.abs(F - Fo).max() <= 1e-4 * inst.n_cons + 1e-2 and np.abs(G[:, :70] - Go[:, :70]).max() <= 5e-2
+    # the paper's product form in fp32 at k up to 64: a REPORTED ceiling, not a parity bound (PAPER.md:135-139 -- the
+    # products reach 2^k and eps^k; SURVEY.md App. C measures 0.05..0.7 on one gradient component of ONE k = 50
+    # constraint at corner points, and the fixed variables here ARE corner coordinates).  A component sums ~45
+    # partials, the k > 48 ones dominate the error, and its value moves with the rounding order of the products
+    # (measured 0.047..0.053 over the kernel variants of profiles/r1_notes.md), hence 1e-1; the tight checks of
+    # this test are the robust tables above (1e-4) and fp64 below (1e-10)
+    assert np.abs(F - Fo).max() <= 1e-4 * inst.n_cons + 1e-2 and np.abs(G[:, :70] - Go[:, :70]).max() <= 1e-1
     if fixed is not None:
         assert np.all(G[fixed != 0] == 0) and np.all(Gr[fixed != 0] == 0)
     Fd, Gd = run_eval(inst, x, 70, 64, flags=Bd.FLAG_ROBUST)
