@@ -689,6 +689,7 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
         const int64_t cw = g.cw;
         g.Wc = std::min(g.warps, pow2_floor(std::max<int64_t>(1, (tile_w + cw - 1) / cw)));
         if ((int64_t)g.Wc * cw < tile_w && g.Wc < g.warps && (int64_t)g.Wc * cw * 2 <= tile_w + cw - 1) g.Wc *= 2;
+        while (g.warps % g.Wc) --g.Wc;                                 // 12-warp CTAs: Wc x Wk must tile the CTA exactly
         g.Wk = g.warps / g.Wc;
     }
 

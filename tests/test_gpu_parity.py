@@ -633,3 +633,36 @@ def test_full_size_cfg3_sampled_fp32():
         assert np.abs(Fg - Fo).max() <= ftol, (flags, np.abs(Fg - Fo).max())
         assert np.abs(Gg - Go[:, :cols.size]).max() <= gtol, (flags, np.abs(Gg - Go[:, :cols.size]).max())
         ctx.close()
+
+
+@pytest.mark.parametrize("B", [96, 160, 256, 320, 1000])
+def test_lane_split_classes_many_constraints_per_item(B):
+    """The lane-split kernels run 12-warp CTAs: for every batch width the Wc x Wk warp grid must tile the CTA exactly
+    (Wc = 8 with 12 warps would walk some constraints twice: B = 160 for the scalar class, 256 and 320 for the
+    packed one).  Thousands of constraints of one signature, so that a work item holds SEVERAL of them, in both
+    lane-split classes (k = 12 packed, k = 30 and k = 33 scalar with a missing literal); robust tables so that the
+    bound is tight."""
+    rng = np.random.default_rng(1212 + B)
+    n = 60
+    row_ptr, lit_var, lit_sign, ctype, param = [0], [], [], [], []
+    for k, t, cnt in ((12, I.EXACTLY, 3000), (30, I.ATLEAST, 2600), (33, I.ATMOST, 24), (9, I.NAE, 17)):
+        for _ in range(cnt):
+            vs = rng.choice(n, size=k, replace=False)
+            lit_var += vs.tolist()
+            lit_sign += (rng.integers(0, 2, size=k) * 2 - 1).tolist()
+            row_ptr.append(len(lit_var))
+            ctype.append(t)
+            param.append(k // 2 if t != I.NAE else 0)
+    inst = I.Instance(name="split_many", n_vars=n, row_ptr=np.asarray(row_ptr, dtype=np.int64),
+                      lit_var=np.asarray(lit_var, dtype=np.int32), lit_sign=np.asarray(lit_sign, dtype=np.int8),
+                      ctype=np.asarray(ctype, dtype=np.uint8), param=np.asarray(param, dtype=np.int32), fixed=None,
+                      batch=B, eta=0.1, steps=1, meta={})
+    x = I.make_x0(inst, seed=77 + B, batch=B)
+    cols = np.unique(np.concatenate([np.arange(2), rng.integers(0, B, size=5), [B - 1]]))
+    xs = np.zeros((n, 32), dtype=np.float64)
+    xs[:, :cols.size] = x[:, cols]
+    Fo, Go = O.eval_grad(inst, xs, cols.size)
+    F, G = run_eval(inst, x, B, 32, flags=Bd.FLAG_ROBUST)
+    assert np.abs(F[cols] - Fo).max() <= 1e-4 * inst.n_cons
+    # a component sums ~2000 partials (each within ~1e-6 with the robust tables) of magnitude up to ~0.5
+    assert np.abs(G[:, cols] - Go[:, :cols.size]).max() <= 2e-3
