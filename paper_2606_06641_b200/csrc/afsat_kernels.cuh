@@ -137,12 +137,9 @@ template <> struct VecIO<double, 2> {
 // ---- a2-a4 for one constraint of compile-time length K and V candidates, all in registers --------
 // tab: the signature's rows in shared memory, 8 scalars per row {Re a, Im a, Re b, Im b, Re w, Im w,
 // Re(w b), Im(w b)}, real rows first.
-// RAG (ragged): the body is compiled for K literals but the constraint has k in (K - RAG_STEP, K]; the
-// factors of the missing literals i >= k are set to exactly 1, which leaves every product unchanged.
-constexpr int RAG_STEP = 4;
-template <typename T, int K, int V, bool GRAD, bool RAG>
+template <typename T, int K, int V, bool GRAD>
 __device__ __forceinline__ void eval_points_reg(const T (&y)[K][V], const T *__restrict__ tab, int n_real,
-                                                int n_cplx, T (&fe)[V], T (&g)[K][V], int k)
+                                                int n_cplx, T (&fe)[V], T (&g)[K][V])
 {
     const T *r = tab;
     for (int p = 0; p < n_real; ++p, r += 8) {                       // self-conjugate points
@@ -151,10 +148,7 @@ __device__ __forceinline__ void eval_points_reg(const T (&y)[K][V], const T *__r
         for (int v = 0; v < V; ++v) {
             T pre[K], f[K];
 #pragma unroll
-            for (int i = 0; i < K; ++i) {
-                f[i] = fma_(b, y[i][v], a);
-                if (RAG && i > K - RAG_STEP && i >= k) f[i] = T(1);
-            }
+            for (int i = 0; i < K; ++i) f[i] = fma_(b, y[i][v], a);
             T run = f[0];
 #pragma unroll
             for (int i = 1; i < K; ++i) { pre[i] = run; run *= f[i]; }
@@ -173,10 +167,7 @@ __device__ __forceinline__ void eval_points_reg(const T (&y)[K][V], const T *__r
         for (int v = 0; v < V; ++v) {
             T pr[K], pi[K], fr[K], fi[K];
 #pragma unroll
-            for (int i = 0; i < K; ++i) {
-                fr[i] = fma_(br, y[i][v], ar); fi[i] = fma_(bi, y[i][v], ai);
-                if (RAG && i > K - RAG_STEP && i >= k) { fr[i] = T(1); fi[i] = T(0); }
-            }
+            for (int i = 0; i < K; ++i) { fr[i] = fma_(br, y[i][v], ar); fi[i] = fma_(bi, y[i][v], ai); }
             T rr = fr[0], ri = fi[0];
 #pragma unroll
             for (int i = 1; i < K; ++i) {
@@ -598,24 +589,24 @@ __device__ __forceinline__ double flip_sign(double v, int32_t lit)
 // FIXED = the item contains fixed literals (constant y = +-1, no gather, no gradient).
 // Padding candidates (b >= B inside a live lane pair) are computed and scattered like live ones:
 // G's padding columns are scratch here and are reset by the caller.
-template <typename T, int K, int V, bool GRAD, bool FIXED, bool RAG>
+template <typename T, int K, int V, bool GRAD, bool FIXED>
 __device__ __forceinline__ void run_item_reg(const EvalParams<T> &p, const int32_t *__restrict__ s_lits,
                                              const T *__restrict__ s_tab, int n_real, int n_cplx, int nc, int wk,
-                                             int64_t b, T (&fe)[V], int k)
+                                             int64_t b, T (&fe)[V])
 {
     const char *xb = reinterpret_cast<const char *>(p.x + b);
     char *gb = reinterpret_cast<char *>(p.G + (b - p.g_b0));
     const uint32_t x_ld = (uint32_t)(p.ldb * (int64_t)sizeof(T)), g_ld = (uint32_t)(p.g_ld * (int64_t)sizeof(T));
     const int Wk = p.Wk;
     for (int c = wk; c < nc; c += Wk) {
-        const int32_t *L = s_lits + c * (RAG ? k : K);
+        const int32_t *L = s_lits + c * K;
         int32_t lit[K];
         T y[K][V], g[K][V];
 #pragma unroll
-        for (int i = 0; i < K; ++i) lit[i] = (RAG && i > K - RAG_STEP && i >= k) ? LIT_FIXED : L[i];   // missing literal: constant, no gather
+        for (int i = 0; i < K; ++i) lit[i] = L[i];
 #pragma unroll
         for (int i = 0; i < K; ++i) {
-            if ((FIXED || (RAG && i > K - RAG_STEP)) && (lit[i] & LIT_FIXED)) {   // warp-uniform branch
+            if (FIXED && (lit[i] & LIT_FIXED)) {                      // warp-uniform branch
 #pragma unroll
                 for (int v = 0; v < V; ++v) y[i][v] = T(1);
             } else {
@@ -624,11 +615,11 @@ __device__ __forceinline__ void run_item_reg(const EvalParams<T> &p, const int32
 #pragma unroll
             for (int v = 0; v < V; ++v) { y[i][v] = flip_sign(y[i][v], lit[i]); g[i][v] = T(0); }
         }
-        eval_points_reg<T, K, V, GRAD, RAG>(y, s_tab, n_real, n_cplx, fe, g, k);
+        eval_points_reg<T, K, V, GRAD>(y, s_tab, n_real, n_cplx, fe, g);
         if (GRAD) {
 #pragma unroll
             for (int i = 0; i < K; ++i) {
-                if ((FIXED || (RAG && i > K - RAG_STEP)) && (lit[i] & LIT_FIXED)) continue;   // masked gradient
+                if (FIXED && (lit[i] & LIT_FIXED)) continue;          // masked gradient
                 T gi[V];
 #pragma unroll
                 for (int v = 0; v < V; ++v) gi[v] = flip_sign(g[i][v], lit[i]);
@@ -679,7 +670,7 @@ __device__ __forceinline__ void run_item_pf(const EvalParams<T> &p, const int32_
             for (int v = 0; v < V; ++v) { y[i][v] = flip_sign(y_n[i][v], lit[i]); g[i][v] = T(0); }
         }
         if (c + Wk < nc) fetch(c + Wk);
-        eval_points_reg<T, K, V, GRAD, false>(y, s_tab, n_real, n_cplx, fe, g, K);
+        eval_points_reg<T, K, V, GRAD>(y, s_tab, n_real, n_cplx, fe, g);
         if (GRAD) {
 #pragma unroll
             for (int i = 0; i < K; ++i) {
@@ -867,13 +858,11 @@ __global__ void __launch_bounds__(CTA_THREADS, MINB) k_eval_f2m(const EvalParams
     SwitchF2<KLO, KHI, NP, GRAD>::go(it.k, p, s_lits, s_tab2, s_F, n_unit, n_gen, it.c_end - it.c_begin, it.has_fixed != 0, uv);
 }
 
-// bodies are compiled for every length up to K_EXACT and for every RAG_STEP-th length beyond (ragged bodies)
-constexpr int K_EXACT = 20;
+// one body per length: KHI <= 20 for both instantiations (fp32 beyond k = 8 runs the lane-split kernels of afsat_split.cuh)
 template <typename T, int K, int V, bool GRAD>
 __device__ __noinline__ void item_body_k(const EvalParams<T> &p, const int32_t *s_lits, const T *s_tab, T (*s_F)[32 * V],
-                                         int n_real, int n_cplx, int nc, bool has_fixed, int k)
+                                         int n_real, int n_cplx, int nc, bool has_fixed)
 {
-    constexpr bool RAG = K > K_EXACT;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int wc = warp % p.Wc, wk = warp / p.Wc;
     const int64_t b = p.b_begin + ((int64_t)blockIdx.y * p.Wc + wc) * (32 * V) + lane * V;
@@ -886,8 +875,8 @@ __device__ __noinline__ void item_body_k(const EvalParams<T> &p, const int32_t *
             if (has_fixed) run_item_pf<T, K, V, GRAD, true>(p, s_lits, s_tab, n_real, n_cplx, nc, wk, b, fe);
             else run_item_pf<T, K, V, GRAD, false>(p, s_lits, s_tab, n_real, n_cplx, nc, wk, b, fe);
         } else {
-            if (has_fixed) run_item_reg<T, K, V, GRAD, true, RAG>(p, s_lits, s_tab, n_real, n_cplx, nc, wk, b, fe, k);
-            else run_item_reg<T, K, V, GRAD, false, RAG>(p, s_lits, s_tab, n_real, n_cplx, nc, wk, b, fe, k);
+            if (has_fixed) run_item_reg<T, K, V, GRAD, true>(p, s_lits, s_tab, n_real, n_cplx, nc, wk, b, fe);
+            else run_item_reg<T, K, V, GRAD, false>(p, s_lits, s_tab, n_real, n_cplx, nc, wk, b, fe);
         }
     }
     store_item_F<T, V>(p, s_F, fe, warp, lane, wk, b, active);
@@ -898,9 +887,8 @@ struct SwitchK {
     static __device__ __forceinline__ void go(int k, const EvalParams<T> &p, const int32_t *s_lits, const T *s_tab,
                                               T (*s_F)[32 * V], int n_real, int n_cplx, int nc, bool has_fixed)
     {
-        constexpr int KN = K < K_EXACT ? K + 1 : K + RAG_STEP;        // next compiled length
-        if (k <= K) item_body_k<T, K, V, GRAD>(p, s_lits, s_tab, s_F, n_real, n_cplx, nc, has_fixed, k);
-        else if (K < KHI) SwitchK<T, (KN < KHI ? KN : KHI), KHI, V, GRAD>::go(k, p, s_lits, s_tab, s_F, n_real, n_cplx, nc, has_fixed);
+        if (k == K) item_body_k<T, K, V, GRAD>(p, s_lits, s_tab, s_F, n_real, n_cplx, nc, has_fixed);
+        else if (K < KHI) SwitchK<T, (K < KHI ? K + 1 : K), KHI, V, GRAD>::go(k, p, s_lits, s_tab, s_F, n_real, n_cplx, nc, has_fixed);
     }
 };
 

@@ -1,6 +1,6 @@
-// afsat_km32.cu -- the fp32 instantiation of the scalar register kernel k_eval_km (SURVEY.md §8(a) a1-a5 for
-// constraints of 9..64 literals), in a translation unit of its own: its per-length bodies are most
-// of the build, and this way they compile in parallel with everything else (build.py).
+// afsat_km32.cu -- the fp32 instantiation of the scalar register kernel k_eval_km for 9 <= k <= AFSAT_B_KMAX32
+// (DESIGN.md 6.2), in a translation unit of its own so that it compiles in parallel with the
+// rest (build.py).  Only built with -DAFSAT_M32_PACKED=0: by default those lengths run the packed lane-split kernel.
 #define AFSAT_KM32_TU
 #include "afsat_kernels.cuh"
 

@@ -131,9 +131,10 @@ def test_long_constraints_uniform_x(dtype):
 
 @pytest.mark.parametrize("with_fixed", [False, True])
 def test_every_length_9_to_64(with_fixed):
-    """One constraint of EVERY length 9..64 (every exact body, every ragged body at each of its four lengths,
-    with and without fixed literals), fp32, robust tables (tight at any length): F and G against the oracle at
-    1e-4, and the paper's tables within the loose long-constraint bound."""
+    """One constraint of EVERY length 9..64 (every per-length body of the packed and of the scalar lane-split kernel,
+    odd lengths with their missing literal, with and without fixed literals; fp64: every body of the register and
+    the register-blocked kernel), robust tables (tight at any length): F and G against the oracle at 1e-4 / 1e-10,
+    and the paper's tables in fp32 within the loose long-constraint bound."""
     rng = np.random.default_rng(909)
     n = 72
     row_ptr, lit_var, lit_sign, ctype, param = [0], [], [], [], []
