@@ -207,8 +207,8 @@ void (*pick_b(bool grad))(EvalParams<T>)
     constexpr int KHI = sizeof(T) == 4 ? AFSAT_B_KMAX32 : AFSAT_B_KMAX64;
 #if AFSAT_M32_PACKED
     if constexpr (sizeof(T) == 4)                                      // fp32: the packed lane-split kernel
-        return grad ? (Fn)k_eval_split<9, AFSAT_B_KMAX32, 2, 2, true, AFSAT_M32_THREADS, 1>
-                    : (Fn)k_eval_split<9, AFSAT_B_KMAX32, 2, 2, false, AFSAT_M32_THREADS, 1>;
+        return grad ? (Fn)k_eval_split<float, 9, AFSAT_B_KMAX32, 2, 2, true, AFSAT_M32_THREADS, 1>
+                    : (Fn)k_eval_split<float, 9, AFSAT_B_KMAX32, 2, 2, false, AFSAT_M32_THREADS, 1>;
     else
 #endif
     return grad ? (Fn)k_eval_km<T, 9, KHI, 1, true, AFSAT_B_MINB> : (Fn)k_eval_km<T, 9, KHI, 1, false, AFSAT_B_MINB>;
@@ -221,9 +221,13 @@ void (*pick_long(int km, bool grad))(EvalParams<T>)
 {
     using Fn = void (*)(EvalParams<T>);
     if constexpr (sizeof(T) == 4) {                                    // fp32: the lane-split register kernel
-        return grad ? (Fn)k_eval_split<AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, 1, true, AFSAT_L32_THREADS, AFSAT_L32_MINB>
-                    : (Fn)k_eval_split<AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, 1, false, AFSAT_L32_THREADS, AFSAT_L32_MINB>;
+        return grad ? (Fn)k_eval_split<float, AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, 1, true, AFSAT_L32_THREADS, AFSAT_L32_MINB>
+                    : (Fn)k_eval_split<float, AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, 1, false, AFSAT_L32_THREADS, AFSAT_L32_MINB>;
     } else {
+#if AFSAT_L64_SPLIT
+        return grad ? (Fn)k_eval_split<double, AFSAT_L64_KMIN, AFSAT_MAX_LEN, 4, 1, true, AFSAT_L64_THREADS, 1>
+                    : (Fn)k_eval_split<double, AFSAT_L64_KMIN, AFSAT_MAX_LEN, 4, 1, false, AFSAT_L64_THREADS, 1>;
+#endif
 #define AFSAT_LONG_CASE(KM_)                                                                                  \
     case KM_:                                                                                                 \
         return grad ? (Fn)k_eval_blk<T, KM_, true> : (Fn)k_eval_blk<T, KM_, false>;
@@ -681,6 +685,11 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
         if (cls == CLS_LONG && dtype == 32) {                          // lane-split kernel: NS lanes per candidate
             g.warps = AFSAT_L32_THREADS / 32;
             g.cw = 32 / AFSAT_L32_NS;
+#if AFSAT_L64_SPLIT
+        } else if (cls == CLS_LONG) {                                  // fp64: four lanes per candidate
+            g.warps = AFSAT_L64_THREADS / 32;
+            g.cw = 8;
+#endif
         } else if (cls == CLS_LONG) {
             const int km = long_kmax(kmax_long);
             g.warps = LONG_THREADS / 32;

@@ -6,10 +6,14 @@
 #include "afsat_split.cuh"
 
 namespace afsat {
-template __global__ void k_eval_split<AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, 1, true, AFSAT_L32_THREADS, AFSAT_L32_MINB>(const EvalParams<float>);
-template __global__ void k_eval_split<AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, 1, false, AFSAT_L32_THREADS, AFSAT_L32_MINB>(const EvalParams<float>);
+template __global__ void k_eval_split<float, AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, 1, true, AFSAT_L32_THREADS, AFSAT_L32_MINB>(const EvalParams<float>);
+template __global__ void k_eval_split<float, AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, 1, false, AFSAT_L32_THREADS, AFSAT_L32_MINB>(const EvalParams<float>);
+#if AFSAT_L64_SPLIT
+template __global__ void k_eval_split<double, AFSAT_L64_KMIN, AFSAT_MAX_LEN, 4, 1, true, AFSAT_L64_THREADS, 1>(const EvalParams<double>);
+template __global__ void k_eval_split<double, AFSAT_L64_KMIN, AFSAT_MAX_LEN, 4, 1, false, AFSAT_L64_THREADS, 1>(const EvalParams<double>);
+#endif
 #if AFSAT_M32_PACKED
-template __global__ void k_eval_split<9, AFSAT_B_KMAX32, 2, 2, true, AFSAT_M32_THREADS, 1>(const EvalParams<float>);
-template __global__ void k_eval_split<9, AFSAT_B_KMAX32, 2, 2, false, AFSAT_M32_THREADS, 1>(const EvalParams<float>);
+template __global__ void k_eval_split<float, 9, AFSAT_B_KMAX32, 2, 2, true, AFSAT_M32_THREADS, 1>(const EvalParams<float>);
+template __global__ void k_eval_split<float, 9, AFSAT_B_KMAX32, 2, 2, false, AFSAT_M32_THREADS, 1>(const EvalParams<float>);
 #endif
 }  // namespace afsat

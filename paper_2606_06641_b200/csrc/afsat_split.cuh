@@ -33,6 +33,13 @@ namespace afsat {
 #ifndef AFSAT_M32_THREADS
 #define AFSAT_M32_THREADS 384
 #endif
+#ifndef AFSAT_L64_SPLIT
+#define AFSAT_L64_SPLIT 1              // fp64, k > 20: FOUR lanes per candidate (a double takes two registers)
+#endif
+#ifndef AFSAT_L64_THREADS
+#define AFSAT_L64_THREADS 384             // 168 registers, 12 warps per SM (256 x 255 registers: 4.25 vs 4.07 ms on cfg3)
+#endif
+#define AFSAT_L64_KMIN 21              // = AFSAT_B_KMAX64 + 1 (afsat.cu)
 #ifndef AFSAT_L32_PREFETCH
 #define AFSAT_L32_PREFETCH 1
 #endif
@@ -41,49 +48,49 @@ namespace afsat {
 #endif
 
 // product of the OTHER lanes' values (NS = 2: the partner's; NS = 4: butterfly over lane bits log2(CW), log2(CW) + 1)
-template <int NS>
-__device__ __forceinline__ float others_real(unsigned mask, float v)
+template <typename T, int NS>
+__device__ __forceinline__ T others_real(unsigned mask, T v)
 {
     constexpr int CW = 32 / NS;
     if (NS == 2) return __shfl_xor_sync(mask, v, CW);
-    const float n1 = __shfl_xor_sync(mask, v, CW);
-    const float po = __shfl_xor_sync(mask, v * n1, 2 * CW);
+    const T n1 = __shfl_xor_sync(mask, v, CW);
+    const T po = __shfl_xor_sync(mask, v * n1, 2 * CW);
     return n1 * po;
 }
-template <int NS>
-__device__ __forceinline__ void others_cplx(unsigned mask, float vr, float vi, float &orr, float &oi)
+template <typename T, int NS>
+__device__ __forceinline__ void others_cplx(unsigned mask, T vr, T vi, T &orr, T &oi)
 {
     constexpr int CW = 32 / NS;
-    const float n1r = __shfl_xor_sync(mask, vr, CW), n1i = __shfl_xor_sync(mask, vi, CW);
+    const T n1r = __shfl_xor_sync(mask, vr, CW), n1i = __shfl_xor_sync(mask, vi, CW);
     if (NS == 2) { orr = n1r; oi = n1i; return; }
-    const float ppr = fmaf(vr, n1r, -(vi * n1i)), ppi = fmaf(vr, n1i, vi * n1r);
-    const float por = __shfl_xor_sync(mask, ppr, 2 * CW), poi = __shfl_xor_sync(mask, ppi, 2 * CW);
-    orr = fmaf(n1r, por, -(n1i * poi)); oi = fmaf(n1r, poi, n1i * por);
+    const T ppr = fma_(vr, n1r, -(vi * n1i)), ppi = fma_(vr, n1i, vi * n1r);
+    const T por = __shfl_xor_sync(mask, ppr, 2 * CW), poi = __shfl_xor_sync(mask, ppi, 2 * CW);
+    orr = fma_(n1r, por, -(n1i * poi)); oi = fma_(n1r, poi, n1i * por);
 }
 
 // a2-a4 for the lane's KS literals of one constraint; tab rows as in eval_points_reg ({Re a, Im a, Re b, Im b,
 // Re w, Im w, Re(w b), Im(w b)}, real rows first).  miss: the lane's LAST literal does not exist (unit factor).
-template <int KS, int NS, bool GRAD>
-__device__ __forceinline__ void eval_points_split(unsigned mask, const float (&y)[KS], bool miss,
-                                                  const float *__restrict__ tab, int n_real, int n_cplx, float &fe,
-                                                  float (&g)[KS])
+template <typename T, int KS, int NS, bool GRAD>
+__device__ __forceinline__ void eval_points_split(unsigned mask, const T (&y)[KS], bool miss,
+                                                  const T *__restrict__ tab, int n_real, int n_cplx, T &fe,
+                                                  T (&g)[KS])
 {
-    const float *r = tab;
+    const T *r = tab;
     for (int p = 0; p < n_real; ++p, r += 8) {                       // self-conjugate points
-        const float a = r[0], b = r[2], w = r[4], wb = r[6];
-        float pre[KS], f[KS];
+        const T a = r[0], b = r[2], w = r[4], wb = r[6];
+        T pre[KS], f[KS];
 #pragma unroll
-        for (int i = 0; i < KS; ++i) f[i] = fmaf(b, y[i], a);
-        if (miss) f[KS - 1] = 1.0f;
-        float run = f[0];
+        for (int i = 0; i < KS; ++i) f[i] = fma_(b, y[i], a);
+        if (miss) f[KS - 1] = T(1);
+        T run = f[0];
 #pragma unroll
         for (int i = 1; i < KS; ++i) { pre[i] = run; run *= f[i]; }
-        const float oth = others_real<NS>(mask, run);
-        fe = fmaf(w, run * oth, fe);
+        const T oth = others_real<T, NS>(mask, run);
+        fe = fma_(w, run * oth, fe);
         if (GRAD) {
-            float suf = wb * oth;
+            T suf = wb * oth;
 #pragma unroll
-            for (int i = KS - 1; i >= 1; --i) { g[i] = fmaf(pre[i], suf, g[i]); suf *= f[i]; }
+            for (int i = KS - 1; i >= 1; --i) { g[i] = fma_(pre[i], suf, g[i]); suf *= f[i]; }
             g[0] += suf;                                              // prefix_0 = 1
         }
     }
@@ -93,56 +100,56 @@ __device__ __forceinline__ void eval_points_split(unsigned mask, const float (&y
     // leaves the issue slots idle on fixed-latency waits: profiles/r1_eval_split_cfg3.md)
     constexpr int KA = AFSAT_L32_CHAINS == 2 ? KS / 2 : KS, KB = KS - KA;
     for (int p = 0; p < n_cplx; ++p, r += 8) {                       // one of each conjugate pair
-        const float ar = r[0], ai = r[1], br = r[2], bi = r[3], wr = r[4], wi = r[5], wbr = r[6], wbi = r[7];
-        float pr[KS], pi[KS], fr[KS], fi[KS];
+        const T ar = r[0], ai = r[1], br = r[2], bi = r[3], wr = r[4], wi = r[5], wbr = r[6], wbi = r[7];
+        T pr[KS], pi[KS], fr[KS], fi[KS];
 #pragma unroll
-        for (int i = 0; i < KS; ++i) { fr[i] = fmaf(br, y[i], ar); fi[i] = fmaf(bi, y[i], ai); }
-        if (miss) { fr[KS - 1] = 1.0f; fi[KS - 1] = 0.0f; }
-        float rr = fr[0], ri = fi[0], qr = 1.0f, qi = 0.0f;
+        for (int i = 0; i < KS; ++i) { fr[i] = fma_(br, y[i], ar); fi[i] = fma_(bi, y[i], ai); }
+        if (miss) { fr[KS - 1] = T(1); fi[KS - 1] = T(0); }
+        T rr = fr[0], ri = fi[0], qr = T(1), qi = T(0);
         if (KB > 0) { qr = fr[KA]; qi = fi[KA]; }
 #pragma unroll
         for (int i = 1; i < (KA > KB ? KA : KB); ++i) {
             if (i < KA) {
                 pr[i] = rr; pi[i] = ri;
-                const float nr = fmaf(rr, fr[i], -(ri * fi[i]));
-                const float ni = fmaf(rr, fi[i], ri * fr[i]);
+                const T nr = fma_(rr, fr[i], -(ri * fi[i]));
+                const T ni = fma_(rr, fi[i], ri * fr[i]);
                 rr = nr; ri = ni;
             }
             if (i < KB) {
                 pr[KA + i] = qr; pi[KA + i] = qi;
-                const float nr = fmaf(qr, fr[KA + i], -(qi * fi[KA + i]));
-                const float ni = fmaf(qr, fi[KA + i], qi * fr[KA + i]);
+                const T nr = fma_(qr, fr[KA + i], -(qi * fi[KA + i]));
+                const T ni = fma_(qr, fi[KA + i], qi * fr[KA + i]);
                 qr = nr; qi = ni;
             }
         }
-        float lr = rr, li = ri;                                       // the lane's partial product P_A P_B
-        if (KB > 0) { lr = fmaf(rr, qr, -(ri * qi)); li = fmaf(rr, qi, ri * qr); }
-        float orr, oi;
-        others_cplx<NS>(mask, lr, li, orr, oi);
-        const float tr = fmaf(lr, orr, -(li * oi)), ti = fmaf(lr, oi, li * orr);   // P_l, the whole product
-        fe = fmaf(wr, tr, fe);
-        fe = fmaf(-wi, ti, fe);
+        T lr = rr, li = ri;                                       // the lane's partial product P_A P_B
+        if (KB > 0) { lr = fma_(rr, qr, -(ri * qi)); li = fma_(rr, qi, ri * qr); }
+        T orr, oi;
+        others_cplx<T, NS>(mask, lr, li, orr, oi);
+        const T tr = fma_(lr, orr, -(li * oi)), ti = fma_(lr, oi, li * orr);   // P_l, the whole product
+        fe = fma_(wr, tr, fe);
+        fe = fma_(-wi, ti, fe);
         if (GRAD) {
-            const float zr = fmaf(wbr, orr, -(wbi * oi)), zi = fmaf(wbr, oi, wbi * orr);   // w b x others
-            float sr = zr, si = zi, ur = zr, ui = zi;                 // suffix of chain A seeded with z P_B, of B with z P_A
+            const T zr = fma_(wbr, orr, -(wbi * oi)), zi = fma_(wbr, oi, wbi * orr);   // w b x others
+            T sr = zr, si = zi, ur = zr, ui = zi;                 // suffix of chain A seeded with z P_B, of B with z P_A
             if (KB > 0) {
-                sr = fmaf(zr, qr, -(zi * qi)); si = fmaf(zr, qi, zi * qr);
-                ur = fmaf(zr, rr, -(zi * ri)); ui = fmaf(zr, ri, zi * rr);
+                sr = fma_(zr, qr, -(zi * qi)); si = fma_(zr, qi, zi * qr);
+                ur = fma_(zr, rr, -(zi * ri)); ui = fma_(zr, ri, zi * rr);
             }
 #pragma unroll
             for (int i = (KA > KB ? KA : KB) - 1; i >= 1; --i) {
                 if (i < KA) {
-                    g[i] = fmaf(pr[i], sr, g[i]);
-                    g[i] = fmaf(-pi[i], si, g[i]);
-                    const float nr = fmaf(sr, fr[i], -(si * fi[i]));
-                    const float ni = fmaf(sr, fi[i], si * fr[i]);
+                    g[i] = fma_(pr[i], sr, g[i]);
+                    g[i] = fma_(-pi[i], si, g[i]);
+                    const T nr = fma_(sr, fr[i], -(si * fi[i]));
+                    const T ni = fma_(sr, fi[i], si * fr[i]);
                     sr = nr; si = ni;
                 }
                 if (i < KB) {
-                    g[KA + i] = fmaf(pr[KA + i], ur, g[KA + i]);
-                    g[KA + i] = fmaf(-pi[KA + i], ui, g[KA + i]);
-                    const float nr = fmaf(ur, fr[KA + i], -(ui * fi[KA + i]));
-                    const float ni = fmaf(ur, fi[KA + i], ui * fr[KA + i]);
+                    g[KA + i] = fma_(pr[KA + i], ur, g[KA + i]);
+                    g[KA + i] = fma_(-pi[KA + i], ui, g[KA + i]);
+                    const T nr = fma_(ur, fr[KA + i], -(ui * fi[KA + i]));
+                    const T ni = fma_(ur, fi[KA + i], ui * fr[KA + i]);
                     ur = nr; ui = ni;
                 }
             }
@@ -152,29 +159,29 @@ __device__ __forceinline__ void eval_points_split(unsigned mask, const float (&y
     }
 }
 
-template <int KS, int NS, bool GRAD, bool FIXED>
-__device__ __forceinline__ void run_item_split(const EvalParams<float> &p, unsigned mask, const int32_t *__restrict__ s_lits,
-                                               const float *__restrict__ s_tab, int n_real, int n_cplx, int nc, int wk,
-                                               int h, int64_t b, float &fe, int k)
+template <typename T, int KS, int NS, bool GRAD, bool FIXED>
+__device__ __forceinline__ void run_item_split(const EvalParams<T> &p, unsigned mask, const int32_t *__restrict__ s_lits,
+                                               const T *__restrict__ s_tab, int n_real, int n_cplx, int nc, int wk,
+                                               int h, int64_t b, T &fe, int k)
 {
     const char *xb = reinterpret_cast<const char *>(p.x + b);
     char *gb = reinterpret_cast<char *>(p.G + (b - p.g_b0));
-    const uint32_t x_ld = (uint32_t)(p.ldb * 4), g_ld = (uint32_t)(p.g_ld * 4);
+    const uint32_t x_ld = (uint32_t)(p.ldb * (int64_t)sizeof(T)), g_ld = (uint32_t)(p.g_ld * (int64_t)sizeof(T));
     const int Wk = p.Wk;
     const bool miss = (KS - 1) * NS + h >= k;
     for (int c = wk; c < nc; c += Wk) {
         const int32_t *L = s_lits + c * k + h;
         int32_t lit[KS];
-        float y[KS], g[KS];
+        T y[KS], g[KS];
 #pragma unroll
         for (int i = 0; i < KS - 1; ++i) lit[i] = L[i * NS];
         lit[KS - 1] = miss ? LIT_FIXED : L[(KS - 1) * NS];            // missing literal: constant, no gather, no RED
 #pragma unroll
         for (int i = 0; i < KS; ++i) {
-            if ((FIXED || i == KS - 1) && (lit[i] & LIT_FIXED)) y[i] = 1.0f;
-            else y[i] = __ldg(reinterpret_cast<const float *>(xb + (uint64_t)(uint32_t)(lit[i] & LIT_VAR) * x_ld));
+            if ((FIXED || i == KS - 1) && (lit[i] & LIT_FIXED)) y[i] = T(1);
+            else y[i] = __ldg(reinterpret_cast<const T *>(xb + (uint64_t)(uint32_t)(lit[i] & LIT_VAR) * x_ld));
             y[i] = flip_sign(y[i], lit[i]);
-            g[i] = 0.0f;
+            g[i] = T(0);
         }
 #if AFSAT_L32_PREFETCH
         if (c + Wk < nc) {                                            // the NEXT constraint's row segments into L1: with 2-3
@@ -188,21 +195,21 @@ __device__ __forceinline__ void run_item_split(const EvalParams<float> &p, unsig
             }
         }
 #endif
-        eval_points_split<KS, NS, GRAD>(mask, y, miss, s_tab, n_real, n_cplx, fe, g);
+        eval_points_split<T, KS, NS, GRAD>(mask, y, miss, s_tab, n_real, n_cplx, fe, g);
         if (GRAD) {
 #pragma unroll
             for (int i = 0; i < KS; ++i) {
                 if ((FIXED || i == KS - 1) && (lit[i] & LIT_FIXED)) continue;   // masked gradient
-                const float gi[1] = {flip_sign(g[i], lit[i])};
-                VecIO<float, 1>::red(reinterpret_cast<float *>(gb + (uint64_t)(uint32_t)(lit[i] & LIT_VAR) * g_ld), gi);
+                const T gi[1] = {flip_sign(g[i], lit[i])};
+                VecIO<T, 1>::red(reinterpret_cast<T *>(gb + (uint64_t)(uint32_t)(lit[i] & LIT_VAR) * g_ld), gi);
             }
         }
     }
 }
 
-template <int KS, int NS, bool GRAD>
-__device__ __noinline__ void item_body_split(const EvalParams<float> &p, const int32_t *s_lits, const float *s_tab,
-                                             float (*s_F)[32], int n_real, int n_cplx, int nc, bool has_fixed, int k)
+template <typename T, int KS, int NS, bool GRAD>
+__device__ __noinline__ void item_body_split(const EvalParams<T> &p, const int32_t *s_lits, const T *s_tab,
+                                             T (*s_F)[32], int n_real, int n_cplx, int nc, bool has_fixed, int k)
 {
     constexpr int CW = 32 / NS;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -211,16 +218,16 @@ __device__ __noinline__ void item_body_split(const EvalParams<float> &p, const i
     const int64_t b = p.b_begin + ((int64_t)blockIdx.y * p.Wc + wc) * CW + cl;
     const bool active = b < p.b_end && b < p.B && !lane_skipped(p, b, 1);   // the NS lanes of a candidate agree
     const unsigned mask = __ballot_sync(0xffffffffu, active);
-    float fe = 0.0f;
+    T fe = T(0);
     if (active) {
-        if (has_fixed) run_item_split<KS, NS, GRAD, true>(p, mask, s_lits, s_tab, n_real, n_cplx, nc, wk, h, b, fe, k);
-        else run_item_split<KS, NS, GRAD, false>(p, mask, s_lits, s_tab, n_real, n_cplx, nc, wk, h, b, fe, k);
+        if (has_fixed) run_item_split<T, KS, NS, GRAD, true>(p, mask, s_lits, s_tab, n_real, n_cplx, nc, wk, h, b, fe, k);
+        else run_item_split<T, KS, NS, GRAD, false>(p, mask, s_lits, s_tab, n_real, n_cplx, nc, wk, h, b, fe, k);
     }
     if (!p.Fpart) return;
     s_F[warp][lane] = fe;
     __syncthreads();
     if (wk == 0 && h == 0 && active) {                                // fixed order over the Wk constraint groups
-        float s = 0.0f;
+        T s = T(0);
         for (int g = 0; g < p.Wk; ++g) s += s_F[warp + g * p.Wc][lane];
         p.Fpart[(int64_t)(p.frow_base + blockIdx.x) * p.ldb + b] = s;
     }
@@ -381,40 +388,44 @@ __device__ __noinline__ void item_body_split2(const EvalParams<float> &p, const 
     }
 }
 
-template <int KS, int KSHI, int NS, int V, bool GRAD>
+template <typename T, int KS, int KSHI, int NS, int V, bool GRAD>
 struct SwitchSplit {
-    static __device__ __forceinline__ void go(int ks, const EvalParams<float> &p, const int32_t *s_lits, const float *s_tab,
-                                              float (*s_F)[32 * V], int n_real, int n_cplx, int nc, bool has_fixed, int k)
+    static __device__ __forceinline__ void go(int ks, const EvalParams<T> &p, const int32_t *s_lits, const T *s_tab,
+                                              T (*s_F)[32 * V], int n_real, int n_cplx, int nc, bool has_fixed, int k)
     {
         if (ks == KS) {
             if constexpr (V == 2) item_body_split2<KS, NS, GRAD>(p, s_lits, s_tab, s_F, n_real, n_cplx, nc, has_fixed, k);
-            else item_body_split<KS, NS, GRAD>(p, s_lits, s_tab, s_F, n_real, n_cplx, nc, has_fixed, k);
+            else item_body_split<T, KS, NS, GRAD>(p, s_lits, s_tab, s_F, n_real, n_cplx, nc, has_fixed, k);
         } else if (KS < KSHI)
-            SwitchSplit<(KS < KSHI ? KS + 1 : KS), KSHI, NS, V, GRAD>::go(ks, p, s_lits, s_tab, s_F, n_real, n_cplx, nc, has_fixed, k);
+            SwitchSplit<T, (KS < KSHI ? KS + 1 : KS), KSHI, NS, V, GRAD>::go(ks, p, s_lits, s_tab, s_F, n_real, n_cplx, nc, has_fixed, k);
     }
 };
 
 // one launch for every length in [KLO, KHI]: the CTA's item picks the body compiled for ceil(k / NS) literals per lane
-template <int KLO, int KHI, int NS, int V, bool GRAD, int THREADS, int MINB>
-__global__ void __launch_bounds__(THREADS, MINB) k_eval_split(const EvalParams<float> p)
+template <typename T, int KLO, int KHI, int NS, int V, bool GRAD, int THREADS, int MINB>
+__global__ void __launch_bounds__(THREADS, MINB) k_eval_split(const EvalParams<T> p)
 {
-    __shared__ __align__(16) float s_tab[((KHI + 1) / 2 + 1) * 8];
+    __shared__ __align__(16) T s_tab[((KHI + 1) / 2 + 1) * 8];
     __shared__ int32_t s_lits[LIT_CHUNK];
-    __shared__ float s_F[THREADS / 32][32 * V];
+    __shared__ T s_F[THREADS / 32][32 * V];
     const Item it = p.items[blockIdx.x];
     const SigDev sg = p.sigs[it.sig];
     stage_item(p, it, sg, s_tab, s_lits);
     __syncthreads();
-    SwitchSplit<(KLO + NS - 1) / NS, (KHI + NS - 1) / NS, NS, V, GRAD>::go((it.k + NS - 1) / NS, p, s_lits, s_tab, s_F, sg.n_real,
+    SwitchSplit<T, (KLO + NS - 1) / NS, (KHI + NS - 1) / NS, NS, V, GRAD>::go((it.k + NS - 1) / NS, p, s_lits, s_tab, s_F, sg.n_real,
                                                                         sg.n_cplx, it.c_end - it.c_begin, it.has_fixed != 0, it.k);
 }
 
 #ifndef AFSAT_KS32_TU   // instantiated in afsat_ks32.cu
-extern template __global__ void k_eval_split<AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, 1, true, AFSAT_L32_THREADS, AFSAT_L32_MINB>(const EvalParams<float>);
-extern template __global__ void k_eval_split<AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, 1, false, AFSAT_L32_THREADS, AFSAT_L32_MINB>(const EvalParams<float>);
+extern template __global__ void k_eval_split<float, AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, 1, true, AFSAT_L32_THREADS, AFSAT_L32_MINB>(const EvalParams<float>);
+extern template __global__ void k_eval_split<float, AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, 1, false, AFSAT_L32_THREADS, AFSAT_L32_MINB>(const EvalParams<float>);
+#if AFSAT_L64_SPLIT
+extern template __global__ void k_eval_split<double, AFSAT_L64_KMIN, AFSAT_MAX_LEN, 4, 1, true, AFSAT_L64_THREADS, 1>(const EvalParams<double>);
+extern template __global__ void k_eval_split<double, AFSAT_L64_KMIN, AFSAT_MAX_LEN, 4, 1, false, AFSAT_L64_THREADS, 1>(const EvalParams<double>);
+#endif
 #if AFSAT_M32_PACKED
-extern template __global__ void k_eval_split<9, AFSAT_B_KMAX32, 2, 2, true, AFSAT_M32_THREADS, 1>(const EvalParams<float>);
-extern template __global__ void k_eval_split<9, AFSAT_B_KMAX32, 2, 2, false, AFSAT_M32_THREADS, 1>(const EvalParams<float>);
+extern template __global__ void k_eval_split<float, 9, AFSAT_B_KMAX32, 2, 2, true, AFSAT_M32_THREADS, 1>(const EvalParams<float>);
+extern template __global__ void k_eval_split<float, 9, AFSAT_B_KMAX32, 2, 2, false, AFSAT_M32_THREADS, 1>(const EvalParams<float>);
 #endif
 #endif
 
