@@ -395,7 +395,7 @@ def run_ours(args):
         flop_per_step = flop_c * B
         peak_tf = sm * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
         ach_tf = flop_per_step / (kern_ms * 1e-3 / K) / 1e12 if kern_ms > 0 else 0.0
-        roof = {"bound": "alu", "kernel": "evaluation kernels, a1-a5 (k_eval_f2m fp32 k<=8 | k_eval_km 9..20 | k_eval_split fp32 k>20 | k_eval_blk fp64 k>20): all launches of one step", "achieved": ach_tf, "peak": peak_tf,
+        roof = {"bound": "alu", "kernel": "evaluation kernels, a1-a5 (fp32: k_eval_f2m k<=8 | k_eval_split k>=9; fp64: k_eval_km k<=20 | k_eval_split k>20): all launches of one step", "achieved": ach_tf, "peak": peak_tf,
                 "unit": "TFLOP/s", "frac": ach_tf / peak_tf,
                 "peak_source": f"{sm} SMs x 128 FP32 lanes x 2 flop x {peaks['sm_max_mhz']:.0f} MHz "
                                f"({peaks['source']} sm_max_mhz; DESIGN.md 'Roofline')",
@@ -408,6 +408,11 @@ def run_ours(args):
                 "note": "achieved = ALGORITHMIC flop (SURVEY.md App. D: 12 / 4 FP32 instructions per literal at a complex / "
                         "real DFT point, every retained point) / measured kernel time; the kernels execute fewer "
                         "instructions than that at the points 1, -1, i (trivial twiddles, DESIGN.md 6.1)"}
+        if dtype == 64:
+            # the DFMA pipe issues 64 lanes per SM per clock on this part (ncu: sm__pipe_fp64_cycles_active 61.7 % for
+            # 1.3e9 FP64 warp instructions in 4.0 ms, profiles/r1_eval_split_cfg3_f64.md): half the FP32 rate
+            roof["fp64_peak"] = peak_tf / 2
+            roof["frac_of_fp64_peak"] = ach_tf / (peak_tf / 2)
         if clocks.get("sm_mhz"):
             roof["frac_at_observed_clock"] = roof["frac"] * peaks["sm_max_mhz"] / clocks["sm_mhz"]
         cb = dev_rep = None
