@@ -68,7 +68,7 @@ def flop_model(inst):
 class ClockSampler(threading.Thread):
     """Samples SM clock and throttle reasons through NVML during the timed region."""
 
-    def __init__(self, index, period=0.1):
+    def __init__(self, index, period=0.005):   # the default timed region is ~40 ms
         super().__init__(daemon=True)
         self.index, self.period = index, period
         self.samples, self.reasons, self.max_mhz = [], set(), None
