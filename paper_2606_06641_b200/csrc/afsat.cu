@@ -661,9 +661,14 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
         int64_t budget = (int64_t)104 << 20;                           // bytes of L2 for the X and G tiles (126 MB L2)
         if (const char *e = getenv("AFSAT_L2_TILE_BYTES")) { long long v = atoll(e); if (v > 0) budget = v; }
         const int64_t per_col = (int64_t)2 * n_vars * (int64_t)esz;
-        // a working set that overflows the budget only modestly is better left whole (cfg2, 1.58 x: 1.23 ms un-tiled,
-        // 1.25 in two equal tiles, 1.31 in the 2624 + 1472 split this rule used to make)
-        if (per_col * ldb > budget + budget * 3 / 4) tile_w = std::max<int64_t>(64, budget / per_col / 64 * 64);
+        // a working set within a few budgets is better left whole: the L2 misses hide behind the arithmetic, the small
+        // grids of the tiles do not (cfg2 fp32, 1.58 x: 1.23 ms un-tiled vs 1.31; cfg2 fp64, 3.15 x: 2.75 vs 3.13;
+        // DESIGN.md 6.5).  Beyond: equal tiles (no small remainder tile) of at most budget / per_col columns.
+        if (per_col * ldb > 4 * budget) {
+            const int64_t tile_max = std::max<int64_t>(64, budget / per_col / 64 * 64);
+            const int64_t n_tiles = (ldb + tile_max - 1) / tile_max;
+            tile_w = ((ldb + n_tiles - 1) / n_tiles + 63) / 64 * 64;
+        }
         if (const char *e = getenv("AFSAT_TILE_W")) { long long v = atoll(e); if (v >= 32 && v % 32 == 0) tile_w = v; }
         tile_w = std::min<int64_t>(tile_w, ldb);
     }
