@@ -63,13 +63,20 @@ enum afsat_error {
 
 #define AFSAT_MAX_LEN 64       /* the paper's practical ceiling is ~50 literals    */
 
-/* afsat_create flags */
+/* afsat_create flags: which host tables a signature gets (same kernels either way).
+ *   paper tables : prod_i (1 + w^l y_i)/2 contracted with the tailored DFT of the integer Fourier coefficients
+ *                  (PAPER.md:59-67, :141-147).  Its weights reach 2^k/N, so fp32 loses the north_star's 1e-4 on
+ *                  gradients beyond k ~ 20 (the floating-point ceiling of PAPER.md:135-139).
+ *   robust tables: prod_i ((1 + w^l)/2 + y_i (1 - w^l)/2) contracted with the DFT of the truth table itself
+ *                  (reading B4): every factor has modulus <= 1, same FE, holds 1e-4 in fp32 up to k = 64.
+ * AFSAT_FLAG_DEFAULT (automatic, SURVEY.md §8(f) NEXT #3 "per-bucket choice"): fp32 contexts use the paper tables
+ * for lengths k <= 20 and the robust tables for k > 20; fp64 contexts use the paper tables at every length.
+ * AFSAT_FLAG_ROBUST: robust tables for every signature.  AFSAT_FLAG_PAPER: paper tables for every signature
+ * (the comparison mode BASELINE.json configs[3] "report deviation" asks for).  Lengths are those AFTER the
+ * partial assignment has been substituted (see afsat_create).                                                  */
 #define AFSAT_FLAG_DEFAULT      0u
-/* Numerically robust variant of the same contraction: the product is
- * taken over (1 + w^l)/2 + y_i (1 - w^l)/2 and contracted with the DFT of the truth table, so all
- * factors have modulus <= 1.  Same FE, same kernels, different host tables.  Off by default: the
- * default is the paper's prod_i (1 + w^l y_i).                                                   */
 #define AFSAT_FLAG_ROBUST       1u
+#define AFSAT_FLAG_PAPER        2u
 
 /*
  * afsat_create -- build a context for one instance.
@@ -79,15 +86,48 @@ enum afsat_error {
  *   assignment of PAPER.md:105-107; fixed variables use that value whatever X holds, receive zero
  *   gradient and are never updated.
  *   batch = B >= 1, ldb >= B with ldb % 32 == 0, dtype = 32 or 64, device = CUDA ordinal.
- * Validates everything (see afsat_error), groups constraints by signature (type, k, param) and
- * by length, precomputes per signature the exact integer coefficients, the conjugate-symmetric
- * root table and the contracted weights (division deferred to the end), uploads the tables.
+ * Validates everything (see afsat_error); SUBSTITUTES the partial assignment into the constraints (PAPER.md:133:
+ * a symmetric constraint restricted by fixed literals is again symmetric -- with f_T fixed-true literals its truth
+ * table is the original one shifted by f_T on the remaining literals; constraints it decides outright become
+ * constants of F and of the satisfied count); groups the resulting constraints by signature (length, truth table);
+ * precomputes per signature the exact integer coefficients, the conjugate-symmetric root table and the contracted
+ * weights (division deferred to the end); uploads the tables.
  * Validation happens before the device is touched, so invalid input is reported even without a GPU.
  */
 int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t *row_ptr,
                  const int32_t *lit_var, const int8_t *lit_sign, const uint8_t *type,
                  const int32_t *param, const int8_t *fixed, int32_t batch, int64_t ldb,
                  int32_t dtype, int32_t device, uint32_t flags);
+
+/*
+ * afsat_create_ex -- afsat_create with explicit options (every field 0 = the automatic choice).
+ *   n_groups > 1: SEVERAL partial assignments ("AFSAT evenly divides up a given batch of candidate
+ *     assignment amongst multiple partial assignment"): fixed is then [n_groups][n_vars] and candidates
+ *     [g B / n_groups, (g + 1) B / n_groups) run under mask g.  Requires batch % (32 n_groups) == 0.
+ *   tile_w: width of the candidate tiles of a step (a multiple of 32); l2_budget_bytes: bytes of L2
+ *     the X and G tiles may take when the library picks the width itself (default: 13/16 of the device's L2).
+ *   step_path: AFSAT_STEP_AUTO, or force AFSAT_STEP_LAUNCHES / AFSAT_STEP_PERSISTENT / AFSAT_STEP_GRAPH for afsat_step
+ *     (PERSISTENT is refused with AFSAT_E_INVALID when the instance does not fit: every length <= 8, one group,
+ *     X and G of 32 candidates in shared memory).
+ */
+enum afsat_step_path {
+    AFSAT_STEP_AUTO = 0,
+    AFSAT_STEP_LAUNCHES = 1,    /* one set of launches per iteration and candidate tile                               */
+    AFSAT_STEP_PERSISTENT = 2,  /* the whole n_steps loop in ONE launch, X and G in shared memory (small instances)   */
+    AFSAT_STEP_GRAPH = 3        /* one iteration captured into a CUDA graph, replayed n_steps times                   */
+};
+typedef struct afsat_options {
+    uint32_t struct_size;       /* sizeof(afsat_options) */
+    uint32_t flags;             /* AFSAT_FLAG_* */
+    int32_t  n_groups;          /* 0 or 1: one partial assignment */
+    int32_t  step_path;         /* enum afsat_step_path */
+    int64_t  tile_w;
+    int64_t  l2_budget_bytes;
+} afsat_options;
+int afsat_create_ex(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t *row_ptr,
+                    const int32_t *lit_var, const int8_t *lit_sign, const uint8_t *type,
+                    const int32_t *param, const int8_t *fixed, int32_t batch, int64_t ldb,
+                    int32_t dtype, int32_t device, const afsat_options *opt);
 
 void afsat_destroy(afsat_ctx *ctx);
 
@@ -99,6 +139,8 @@ const char *afsat_last_error(const afsat_ctx *ctx);
  *   d_x [n][ldb] (read), d_F [B] (written; may be NULL), d_G [n][ldb] (OVERWRITTEN, not
  *   accumulated; rows of fixed variables and padding columns are 0; may be NULL for F only).
  *   The gradient is the analytic leave-one-out product (prefix x suffix), never a division.
+ *   Every d_x / d_G of this header must be 16-byte aligned (the kernels use 16-byte vector accesses; a torch
+ *   tensor is 256-byte aligned); a misaligned pointer is AFSAT_E_INVALID, not a fault.
  */
 int afsat_eval_grad(afsat_ctx *ctx, const void *d_x, void *d_F, void *d_G, void *stream);
 
@@ -116,14 +158,20 @@ int afsat_check(afsat_ctx *ctx, const void *d_x, int32_t *d_sat_count, uint8_t *
  *     candidates;  round;  count on X(t);  if all m satisfied: is_solution = 1,
  *     first_step = step_base + t, and the candidate is frozen (executes no-ops).
  *   X(0) itself is not checked (Alg. 1 checks after each step).
- *   d_x [n][ldb] in/out.  d_F [B] (may be NULL): F at the final X.  d_sat_count [B]: satisfied
- *   count at the final X.  d_is_solution [B], d_first_step [B] (-1 = none): if resume != 0 they
- *   are read as the state left by an earlier call (frozen candidates stay frozen), else reset.
+ *   d_x [n][ldb] in/out.  d_F [B] (may be NULL): F at the final X (Alg. 1's output FE(X_bar); costs one more
+ *   objective-only pass).  d_F_pre [B] (may be NULL): F(X(n_steps - 1)), the objective at the point where the LAST
+ *   gradient was taken -- a by-product of the fused pass (the contraction a3 of the same products), so it is free;
+ *   a caller that steps repeatedly sees Alg. 1's FE(X(t)) one iteration late.  Not written when n_steps = 0.
+ *   d_sat_count [B]: satisfied count at the final X.  d_is_solution [B], d_first_step [B] (-1 = none): if
+ *   resume != 0 they are read as the state left by an earlier call (frozen candidates stay frozen), else reset.
  *   h_any_solved (may be NULL): 2 x int32 in PINNED, device-mapped host memory; [0] is set to 1
- *   and [1] to the step index as soon as the first candidate is solved (poll without syncing).
+ *   and [1] to the step index as soon as the first candidate is solved (poll without syncing); both are reset
+ *   ({0, -1}) ON THE STREAM at the start of the call, after earlier work of the stream.
+ *   How the loop runs (afsat_query AFSAT_Q_STEP_PATH): small instances run all n_steps in ONE persistent launch;
+ *   others launch per iteration, or replay one captured iteration as a CUDA graph.
  */
 int afsat_step(afsat_ctx *ctx, void *d_x, double eta, int32_t n_steps, int32_t step_base,
-               int32_t resume, void *d_F, int32_t *d_sat_count, uint8_t *d_is_solution,
+               int32_t resume, void *d_F, void *d_F_pre, int32_t *d_sat_count, uint8_t *d_is_solution,
                int32_t *d_first_step, int32_t *h_any_solved, void *stream);
 
 /*
@@ -181,11 +229,12 @@ int afsat_solve(afsat_ctx *ctx, void *d_x, double eta, int32_t steps_per_round, 
 
 /*
  * afsat_step_host -- the same as afsat_step (resume = 0, step_base = 0) for HOST buffers: copies
- * h_x [n][ldb] to the device, runs n_steps, copies X, F, sat_count, is_solution, first_step back
+ * h_x [n][ldb] to the device, runs n_steps, copies X, F, F_pre, sat_count, is_solution, first_step back
  * (any output pointer may be NULL) and synchronises.  Pinned host memory makes the copies
- * asynchronous; pageable memory works too.  This is the end-to-end call bench.py times.
+ * asynchronous; pageable memory works too.  When the step runs tile by tile the copies are pipelined by candidate
+ * tile behind the evaluation.  This is the end-to-end call bench.py times.
  */
-int afsat_step_host(afsat_ctx *ctx, void *h_x, double eta, int32_t n_steps, void *h_F,
+int afsat_step_host(afsat_ctx *ctx, void *h_x, double eta, int32_t n_steps, void *h_F, void *h_F_pre,
                     int32_t *h_sat_count, uint8_t *h_is_solution, int32_t *h_first_step);
 
 /*
@@ -214,7 +263,16 @@ enum afsat_query_key {
     AFSAT_Q_PROFILED_EVAL_NS = 7,       /* afsat_set_profiling: device time of the evaluation kernels
                                            (a1-a5, a7-a8) since profiling was switched on, in ns;
                                            SYNCHRONISES with the recorded events                  */
-    AFSAT_Q_PROFILED_EVAL_LAUNCHES = 8  /* number of evaluation-kernel launches in that time       */
+    AFSAT_Q_PROFILED_EVAL_LAUNCHES = 8, /* number of evaluation-kernel launches in that time       */
+    AFSAT_Q_FLOP_PER_CANDIDATE = 9,     /* model flop count, same scope as key 6; both are counted on the
+                                           constraint table AFTER the partial assignment was substituted */
+    AFSAT_Q_NUM_GROUPS = 10,            /* partial assignments                                     */
+    AFSAT_Q_STEP_PATH = 11,             /* enum afsat_step_path actually used by afsat_step        */
+    AFSAT_Q_TILE_W = 12,                /* candidate tile width of a step                          */
+    AFSAT_Q_LIVE_CONSTRAINTS = 13,      /* constraints that reach a kernel (group 0)               */
+    AFSAT_Q_LIVE_NNZ = 14,              /* their literals (group 0)                                */
+    AFSAT_Q_DECIDED_SATISFIED = 15,     /* constraints group 0's partial assignment satisfies outright */
+    AFSAT_Q_L2_BYTES = 16               /* cudaDeviceProp::l2CacheSize                             */
 };
 int64_t afsat_query(const afsat_ctx *ctx, int32_t key);
 
@@ -259,6 +317,13 @@ int afsat_problem_sizes(const afsat_problem *p, int32_t *n_vars, int32_t *n_cons
 int afsat_problem_fill(const afsat_problem *p, int64_t *row_ptr, int32_t *lit_var, int8_t *lit_sign,
                        uint8_t *type, int32_t *param, int8_t *fixed);
 void afsat_problem_free(afsat_problem *p);
+
+/*
+ * afsat_probe_peak -- measured issue rate of the FP pipes the path is bound by (the `alu` roofline denominator of
+ * bench.py): kind 0 = scalar FFMA, 1 = packed FFMA2 (fma.rn.f32x2), 2 = DFMA; independent chains, nothing else,
+ * timed with CUDA events on `device`.  *tflops receives the best of 5 runs (FMA = 2 flop).  SYNCHRONISES.
+ */
+int afsat_probe_peak(int32_t device, int32_t kind, double *tflops);
 
 const char *afsat_version(void);
 

@@ -17,19 +17,28 @@ _lib = None
 
 FLAG_DEFAULT = 0
 FLAG_ROBUST = 1
+FLAG_PAPER = 2
 MAX_LEN = 64
+STEP_AUTO, STEP_LAUNCHES, STEP_PERSISTENT, STEP_GRAPH = range(4)
 
 Q_KERNEL_LAUNCHES, Q_NUM_SIGNATURES, Q_NUM_BUCKETS, Q_NNZ, Q_WORKSPACE_BYTES, Q_SM_COUNT, \
-    Q_FP_INSTR_PER_CANDIDATE, Q_PROFILED_EVAL_NS, Q_PROFILED_EVAL_LAUNCHES = range(9)
+    Q_FP_INSTR_PER_CANDIDATE, Q_PROFILED_EVAL_NS, Q_PROFILED_EVAL_LAUNCHES, Q_FLOP_PER_CANDIDATE, Q_NUM_GROUPS, \
+    Q_STEP_PATH, Q_TILE_W, Q_LIVE_CONSTRAINTS, Q_LIVE_NNZ, Q_DECIDED_SATISFIED, Q_L2_BYTES = range(17)
 
 ERROR_NAMES = {0: "AFSAT_OK", -1: "AFSAT_E_INVALID", -2: "AFSAT_E_LENGTH", -3: "AFSAT_E_VARIABLE",
                -4: "AFSAT_E_SIGN", -5: "AFSAT_E_DUPLICATE", -6: "AFSAT_E_PARAM",
                -7: "AFSAT_E_NOMEM", -8: "AFSAT_E_CUDA", -9: "AFSAT_E_UNSAT"}
 
-EXPORTS = ["afsat_create", "afsat_destroy", "afsat_last_error", "afsat_eval_grad", "afsat_check",
+EXPORTS = ["afsat_create", "afsat_create_ex", "afsat_probe_peak", "afsat_destroy", "afsat_last_error", "afsat_eval_grad", "afsat_check",
            "afsat_step", "afsat_step_host", "afsat_host_tables", "afsat_query", "afsat_version",
            "afsat_set_profiling", "afsat_step_ls", "afsat_parse", "afsat_parse_file", "afsat_parse_error",
            "afsat_problem_sizes", "afsat_problem_fill", "afsat_problem_free", "afsat_restart", "afsat_solve"]
+
+
+class Options(C.Structure):
+    """struct afsat_options of include/afsat.h."""
+    _fields_ = [("struct_size", C.c_uint32), ("flags", C.c_uint32), ("n_groups", C.c_int32), ("step_path", C.c_int32),
+                ("tile_w", C.c_int64), ("l2_budget_bytes", C.c_int64)]
 
 
 class AfsatError(RuntimeError):
@@ -50,6 +59,10 @@ def load_library():
     vp, i32, i64, u32, dbl = C.c_void_p, C.c_int32, C.c_int64, C.c_uint32, C.c_double
     L.afsat_create.restype = C.c_int
     L.afsat_create.argtypes = [C.POINTER(vp), i32, i32, vp, vp, vp, vp, vp, vp, i32, i64, i32, i32, u32]
+    L.afsat_create_ex.restype = C.c_int
+    L.afsat_create_ex.argtypes = [C.POINTER(vp), i32, i32, vp, vp, vp, vp, vp, vp, i32, i64, i32, i32, C.POINTER(Options)]
+    L.afsat_probe_peak.restype = C.c_int
+    L.afsat_probe_peak.argtypes = [i32, i32, C.POINTER(dbl)]
     L.afsat_destroy.restype = None
     L.afsat_destroy.argtypes = [vp]
     L.afsat_last_error.restype = C.c_char_p
@@ -59,7 +72,7 @@ def load_library():
     L.afsat_check.restype = C.c_int
     L.afsat_check.argtypes = [vp, vp, vp, vp, vp]
     L.afsat_step.restype = C.c_int
-    L.afsat_step.argtypes = [vp, vp, dbl, i32, i32, i32, vp, vp, vp, vp, vp, vp]
+    L.afsat_step.argtypes = [vp, vp, dbl, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp]
     L.afsat_step_ls.restype = C.c_int
     L.afsat_step_ls.argtypes = [vp, vp, dbl, dbl, dbl, dbl, i32, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp]
     L.afsat_restart.restype = C.c_int
@@ -67,7 +80,7 @@ def load_library():
     L.afsat_solve.restype = C.c_int
     L.afsat_solve.argtypes = [vp, vp, dbl, i32, i32, C.c_uint64, i32, vp, vp, vp, vp, vp, vp]
     L.afsat_step_host.restype = C.c_int
-    L.afsat_step_host.argtypes = [vp, vp, dbl, i32, vp, vp, vp, vp]
+    L.afsat_step_host.argtypes = [vp, vp, dbl, i32, vp, vp, vp, vp, vp]
     L.afsat_host_tables.restype = C.c_int
     L.afsat_host_tables.argtypes = [i32, i32, i32, u32, vp, vp]
     L.afsat_query.restype = i64
@@ -96,6 +109,16 @@ def version() -> str:
     return load_library().afsat_version().decode()
 
 
+def probe_peak(kind: int, device: int = 0) -> float:
+    """afsat_probe_peak: measured TFLOP/s of independent FMA chains; kind 0 = FFMA, 1 = FFMA2, 2 = DFMA."""
+    L = load_library()
+    out = C.c_double(0.0)
+    rc = L.afsat_probe_peak(int(device), int(kind), C.byref(out))
+    if rc != 0:
+        raise AfsatError(rc, L.afsat_last_error(None).decode())
+    return float(out.value)
+
+
 def host_tables(ctype: int, k: int, param: int, flags: int = 0):
     """(rows [P,8] float64, n_real) -- see afsat_host_tables in include/afsat.h.  Host only."""
     L = load_library()
@@ -115,9 +138,9 @@ class Problem:
         self.ctype, self.param, self.fixed, self.stats = ctype, param, fixed, stats
         self.n_cons = int(row_ptr.shape[0] - 1)
 
-    def context(self, *, batch, dtype=32, device=0, flags=0, ldb=None):
+    def context(self, *, batch, dtype=32, device=0, flags=0, ldb=None, **opts):
         return Context(self.n_vars, self.row_ptr, self.lit_var, self.lit_sign, self.ctype, self.param,
-                       self.fixed, batch=batch, ldb=ldb, dtype=dtype, device=device, flags=flags)
+                       self.fixed, batch=batch, ldb=ldb, dtype=dtype, device=device, flags=flags, **opts)
 
 
 def _take_problem(L, rc, h):
@@ -176,7 +199,8 @@ class Context:
     """An afsat_ctx for one instance.  Tensors are torch CUDA tensors, variable-major [n, ldb]."""
 
     def __init__(self, n_vars, row_ptr, lit_var, lit_sign, ctype, param, fixed=None, *, batch,
-                 ldb=None, dtype=32, device=0, flags=0):
+                 ldb=None, dtype=32, device=0, flags=0, tile_w=0, l2_budget_bytes=0, step_path=STEP_AUTO):
+        """fixed: None, [n] (one partial assignment) or [n_groups, n] (several; afsat_create_ex)."""
         L = load_library()
         self._L = L
         self._h = C.c_void_p(None)
@@ -186,25 +210,33 @@ class Context:
         ctype = np.ascontiguousarray(ctype, dtype=np.uint8)
         param = np.ascontiguousarray(param, dtype=np.int32)
         fixed = None if fixed is None else np.ascontiguousarray(fixed, dtype=np.int8)
+        self.n_groups = 1 if fixed is None or fixed.ndim == 1 else int(fixed.shape[0])
         self.n = int(n_vars)
         self.m = int(row_ptr.shape[0] - 1)
         self.B = int(batch)
         self.ldb = int(ldb) if ldb is not None else (self.B + 31) // 32 * 32
         self.dtype = int(dtype)
         self.device = int(device)
-        rc = L.afsat_create(C.byref(self._h), self.n, self.m, _np_ptr(row_ptr), _np_ptr(lit_var),
-                            _np_ptr(lit_sign), _np_ptr(ctype), _np_ptr(param), _np_ptr(fixed),
-                            self.B, self.ldb, self.dtype, self.device, int(flags))
+        if self.n_groups == 1 and not tile_w and not l2_budget_bytes and step_path == STEP_AUTO:
+            rc = L.afsat_create(C.byref(self._h), self.n, self.m, _np_ptr(row_ptr), _np_ptr(lit_var),
+                                _np_ptr(lit_sign), _np_ptr(ctype), _np_ptr(param), _np_ptr(fixed),
+                                self.B, self.ldb, self.dtype, self.device, int(flags))
+        else:
+            opt = Options(C.sizeof(Options), int(flags), self.n_groups, int(step_path), int(tile_w), int(l2_budget_bytes))
+            rc = L.afsat_create_ex(C.byref(self._h), self.n, self.m, _np_ptr(row_ptr), _np_ptr(lit_var),
+                                   _np_ptr(lit_sign), _np_ptr(ctype), _np_ptr(param), _np_ptr(fixed),
+                                   self.B, self.ldb, self.dtype, self.device, C.byref(opt))
         if rc != 0:
             msg = L.afsat_last_error(None).decode()
             self._h = C.c_void_p(None)
             raise AfsatError(rc, msg)
 
     @classmethod
-    def from_instance(cls, inst, *, batch=None, dtype=32, device=0, flags=0, ldb=None):
+    def from_instance(cls, inst, *, batch=None, dtype=32, device=0, flags=0, ldb=None, fixed="instance", **opts):
         return cls(inst.n_vars, inst.row_ptr, inst.lit_var, inst.lit_sign, inst.ctype, inst.param,
-                   inst.fixed, batch=int(batch if batch is not None else inst.batch), ldb=ldb,
-                   dtype=dtype, device=device, flags=flags)
+                   inst.fixed if isinstance(fixed, str) else fixed,
+                   batch=int(batch if batch is not None else inst.batch), ldb=ldb,
+                   dtype=dtype, device=device, flags=flags, **opts)
 
     # ---- helpers -------------------------------------------------------------------------
     def _torch_dtype(self):
@@ -218,8 +250,6 @@ class Context:
                 and x.device.index == self.device):
             raise ValueError(f"expected a contiguous CUDA tensor [{self.n},{self.ldb}] "
                              f"{self._torch_dtype()} on device {self.device}")
-        if x.data_ptr() % 128:
-            raise ValueError("X must be 128-byte aligned")
 
     def _raise(self, rc):
         if rc != 0:
@@ -257,9 +287,10 @@ class Context:
         self._raise(rc)
         return sat_count, is_solution
 
-    def step(self, x, eta, n_steps, *, step_base=0, state=None, want_F=True, F=None,
+    def step(self, x, eta, n_steps, *, step_base=0, state=None, want_F=True, F=None, F_pre=None,
              h_any_solved=None, stream=None):
-        """In-place n_steps of PGD on x.  Returns (F, sat_count, is_solution, first_step)."""
+        """In-place n_steps of PGD on x.  Returns (F, sat_count, is_solution, first_step); F_pre (a [B] tensor, optional)
+        receives F(X(n_steps - 1)), the by-product of the last fused gradient pass."""
         import torch
         self._check_x(x)
         dev = x.device
@@ -278,7 +309,8 @@ class Context:
             assert h_any_solved.is_pinned() and h_any_solved.dtype == torch.int32 and h_any_solved.numel() >= 2
             hp = h_any_solved.data_ptr()
         rc = self._L.afsat_step(self._h, x.data_ptr(), float(eta), int(n_steps), int(step_base), resume,
-                                F.data_ptr() if F is not None else None, sat.data_ptr(), sol.data_ptr(),
+                                F.data_ptr() if F is not None else None,
+                                F_pre.data_ptr() if F_pre is not None else None, sat.data_ptr(), sol.data_ptr(),
                                 first.data_ptr(), hp, _stream_ptr(stream))
         self._raise(rc)
         return F, sat, sol, first
@@ -336,9 +368,10 @@ class Context:
         self._raise(rc)
         return F, sat, sol, first, int(rounds.value)
 
-    def step_host(self, h_x, eta, n_steps, *, want_F=True):
+    def step_host(self, h_x, eta, n_steps, *, want_F=True, F_pre=None):
         """End-to-end call on HOST buffers (numpy or pinned torch CPU tensors), synchronous.
-        h_x [n, ldb] is updated in place.  Returns (F, sat_count, is_solution, first_step) numpy."""
+        h_x [n, ldb] is updated in place.  Returns (F, sat_count, is_solution, first_step) numpy; F_pre (numpy [B],
+        optional) receives F(X(n_steps - 1))."""
         np_dtype = np.float32 if self.dtype == 32 else np.float64
         xp = h_x.data_ptr() if hasattr(h_x, "data_ptr") else h_x.ctypes.data
         assert tuple(h_x.shape) == (self.n, self.ldb)
@@ -346,7 +379,7 @@ class Context:
         sat = np.empty(self.B, dtype=np.int32)
         sol = np.empty(self.B, dtype=np.uint8)
         first = np.empty(self.B, dtype=np.int32)
-        rc = self._L.afsat_step_host(self._h, xp, float(eta), int(n_steps), _np_ptr(F), sat.ctypes.data,
+        rc = self._L.afsat_step_host(self._h, xp, float(eta), int(n_steps), _np_ptr(F), _np_ptr(F_pre), sat.ctypes.data,
                                      sol.ctypes.data, first.ctypes.data)
         self._raise(rc)
         return F, sat, sol, first

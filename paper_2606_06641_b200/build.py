@@ -16,12 +16,12 @@ CSRC = PKG / "csrc"
 LIB = PKG / "libafsat_b200.so"
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 
-SOURCES_CU = [CSRC / "afsat.cu", CSRC / "afsat_km32.cu", CSRC / "afsat_ks32.cu"]
+SOURCES_CU = [CSRC / "afsat.cu", CSRC / "afsat_ks32.cu"]
 SOURCES_CPP = [CSRC / "precompute.cpp", CSRC / "parser.cpp"]
-DEPS = [CSRC / "afsat_kernels.cuh", CSRC / "afsat_split.cuh", CSRC / "afsat_internal.h", PKG.parent / "include" / "afsat.h"]
+DEPS = [CSRC / "afsat_kernels.cuh", CSRC / "afsat_split.cuh", CSRC / "afsat_step.cuh", CSRC / "afsat_internal.h",
+        PKG.parent / "include" / "afsat.h"]
 
-# (nvcc -split-compile=0 halves the build time but costs the fp64 register-blocked kernel 17 %: not used; the two
-# CUDA translation units are compiled in parallel instead)
+# the two CUDA translation units are compiled in parallel
 # -static-global-template-stub=false: a kernel template instantiated in one unit is launched from the other
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-static-global-template-stub=false", "-Xcompiler", "-fPIC"]

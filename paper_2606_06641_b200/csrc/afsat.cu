@@ -1,7 +1,8 @@
-// afsat.cu -- C ABI (include/afsat.h) of the B200-native AFSAT hot path: context construction
-// (validation, bucketing by signature and length, table upload) and the launch sequences of
-// afsat_eval_grad / afsat_check / afsat_step.  All arithmetic of the path runs in the kernels of
-// afsat_kernels.cuh; the host tables come from precompute.cpp.  No CPU fallback exists.
+// afsat.cu -- C ABI (include/afsat.h) of the B200-native AFSAT hot path: context construction (validation,
+// substitution of the partial assignments, bucketing by signature and length, table upload) and the launch sequences
+// of afsat_eval_grad / afsat_check / afsat_step / afsat_step_ls / afsat_restart / afsat_solve / afsat_step_host.
+// All arithmetic of the path runs in the kernels of afsat_kernels.cuh, afsat_split.cuh and afsat_step.cuh; the host
+// tables come from precompute.cpp.  No CPU fallback exists.
 #include <cuda_runtime.h>
 #include <algorithm>
 #include <map>
@@ -16,80 +17,83 @@
 #include "afsat_internal.h"
 #include "afsat_kernels.cuh"
 #include "afsat_split.cuh"
+#include "afsat_step.cuh"
 
 using namespace afsat;
-
-// tuning knobs of the k <= 8 fp32 register kernel: candidates per lane and
-// the occupancy the register allocator is held to
-#ifndef AFSAT_A_V
-#define AFSAT_A_V 2
-#endif
-#ifndef AFSAT_A_MINB
-#define AFSAT_A_MINB 2
-#endif
 
 namespace {
 
 thread_local std::string g_create_error;
 
-// length classes: register kernels for k in [1,8] and [9,16] (one launch each, one separately compiled
-// body per length), shared-memory kernel for [17,64]
-// fp32 only: the shortest constraints (k <= AFSAT_S_KMAX) run FOUR candidates per lane (two packed pairs): their
-// launches are issue-bound on per-constraint overhead (literal and table loads, addresses, sign masks), which
-// a lane then pays once per four candidates; their bodies are small enough for it at 128 registers
-#ifndef AFSAT_S_KMAX
-#define AFSAT_S_KMAX 5
-#endif
-#if defined(AFSAT_NO_FFMA2) || AFSAT_A_V < 2
-#undef AFSAT_S_KMAX
-#define AFSAT_S_KMAX 0
-#endif
-// fp32: the scalar register kernel (one candidate per lane, every intermediate in registers, the compiler
-// spilling what does not fit) up to this length; it beats the shared-memory-staged kernel at every length
-#ifndef AFSAT_B_KMAX64
-#define AFSAT_B_KMAX64 20
-#endif
+// Length classes (one launch each per candidate tile, concurrent; one separately compiled body per length):
+//   fp32: S  k <= 5   k_eval_f2m, FOUR candidates per lane (two packed pairs) -- the shortest constraints are issue-bound
+//                     on per-constraint overhead (literal and table loads, addresses, sign masks), which a lane then
+//                     pays once per four candidates
+//         A  6..8     k_eval_f2m, two candidates per lane
+//         B  9..20    packed lane-split kernel (two lanes x two candidates)
+//         L  21..64   scalar lane-split kernel (two lanes per candidate)
+//   fp64: A  k <= 8 and B 9..20  k_eval_km (one candidate per lane);  L  21..64  lane-split kernel, four lanes per candidate
 enum { CLS_S = 0, CLS_A = 1, CLS_B = 2, CLS_LONG = 3, N_CLS = 4 };
 inline int class_of(int k, int dtype)
 {
-    return (dtype == 32 && k <= AFSAT_S_KMAX) ? CLS_S : k <= 8 ? CLS_A : k <= (dtype == 32 ? AFSAT_B_KMAX32 : AFSAT_B_KMAX64) ? CLS_B : CLS_LONG;
+    return (dtype == 32 && k <= AFSAT_S_KMAX) ? CLS_S : k <= AFSAT_A_KMAX ? CLS_A : k <= AFSAT_B_KMAX ? CLS_B : CLS_LONG;
 }
+constexpr int ROBUST_FROM_K32 = 21;     // AFSAT_FLAG_DEFAULT, fp32: robust tables from this length on (include/afsat.h)
 
 struct ClassGeom {              // how one length class maps candidates onto a CTA
     int V = 1;                  // candidates per lane
-    int cw = 32;                // candidates per warp (32 V; 32 / NS in the lane-split kernel)
+    int cw = 32;                // candidates per warp (32 V; 32 V / NS in the lane-split kernels)
     int warps = CTA_WARPS;      // warps per CTA
     int Wc = 1, Wk = CTA_WARPS; // candidate sub-tiles x constraint groups
-    size_t smem = 0;            // dynamic shared memory (long kernel only)
+};
+
+// One partial assignment and the constraint table it leaves: literals of fixed variables are gone,
+// constraints it decides are constants.
+struct GroupPlan {
+    int64_t b0 = 0, b1 = 0;     // candidates [b0, b1) (the last group also owns the padding columns up to ldb)
+    int32_t *d_lits = nullptr;
+    Item *d_items = nullptr;
+    int32_t n_items = 0, cls_begin[N_CLS + 1] = {0};
+    int64_t nnz = 0;            // literals that reach a kernel
+    int32_t m_live = 0;         // constraints that reach a kernel
+    int32_t sat_const = 0;      // constraints the assignment satisfies outright
+    double F_const = 0.0;       // decided constraints' share of F: -1 each satisfied, +1 each violated
+    int64_t fp_instr = 0, flop = 0;   // cost model on the substituted table
+    int32_t kmax = 0;
+};
+
+struct StepGraph {              // one captured iteration of afsat_step and what its nodes were built for
+    cudaGraphExec_t exec = nullptr;
+    void *x = nullptr, *sat = nullptr, *sol = nullptr, *first = nullptr, *h_any = nullptr;
+    double eta = 0.0;
 };
 
 }  // namespace
 
 struct afsat_ctx {
     int32_t n = 0, m = 0, B = 0, dtype = 32, device = 0, sm_count = 148;
-    int64_t ldb = 0, nnz = 0, tile_w = 0;
+    int64_t ldb = 0, nnz = 0, tile_w = 0, group_w = 0, l2_bytes = 0;
     uint32_t flags = 0;
     size_t esz = 4;
-    // device tables
-    int32_t *d_lits = nullptr;
+    // device tables shared by the groups
     SigDev *d_sigs = nullptr;
     void *d_rows = nullptr;
     float *d_rows2 = nullptr;                      // staged tables of the packed fp32 kernel
-    int8_t *d_fixed = nullptr;
-    Item *d_items = nullptr;
-    int32_t n_items = 0, cls_begin[N_CLS + 1] = {0};
+    int8_t *d_fixed = nullptr;                     // [n_groups][n]
+    int32_t *d_sat_const = nullptr;                // [n_groups]
+    std::vector<GroupPlan> groups;
     ClassGeom geom[N_CLS];
-    int32_t kmax_long = 0;
-    int32_t n_sigs = 0, n_buckets = 0;
-    int64_t fp_instr_per_candidate = 0;
+    int32_t n_sigs = 0, n_buckets = 0, max_items = 0;
     // workspace
-    void *d_G = nullptr, *d_Fpart = nullptr;      // G scratch [n][tile_w]; Fpart [n_items][ldb]
+    void *d_G = nullptr, *d_Fpart = nullptr;      // G scratch [n][tile_w]; Fpart [max_items][ldb]
     uint32_t *d_bits = nullptr;                    // sign bits [n][ldb/32]
-    int32_t *d_satacc = nullptr, *d_any = nullptr;
+    int32_t *d_satacc = nullptr, *d_any = nullptr; // d_any: {flag, first step, finished CTAs, step counter}
     // buffers of afsat_step_host (lazy)
-    void *dh_x = nullptr, *dh_F = nullptr;
+    void *dh_x = nullptr, *dh_F = nullptr, *dh_Fpre = nullptr;
     int32_t *dh_sat = nullptr, *dh_first = nullptr;
     uint8_t *dh_sol = nullptr;
+    cudaStream_t in_stream = nullptr, out_stream = nullptr;
+    std::vector<cudaEvent_t> chunk_in, chunk_done;
     // workspace of afsat_step_ls (lazy): full gradient, trial X', reduction partials, per-candidate state
     void *ls_G = nullptr, *ls_xt = nullptr, *ls_F0 = nullptr, *ls_F1 = nullptr;
     double *ls_Dpart = nullptr, *ls_eta = nullptr;
@@ -100,6 +104,11 @@ struct afsat_ctx {
     cudaEvent_t ev_fork = nullptr, ev_join[N_CLS - 1] = {};
     size_t ws_bytes = 0;
     int64_t launches = 0;
+    // how afsat_step runs its loop
+    int32_t step_path = AFSAT_STEP_LAUNCHES;
+    size_t small_smem = 0;
+    StepGraph graph;
+    bool capturing = false;
     // afsat_set_profiling: event pairs around the evaluation-kernel launches
     bool profiling = false;
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_events;
@@ -123,6 +132,8 @@ int fail(afsat_ctx *c, int code, const std::string &msg)
             return fail(ctx, AFSAT_E_CUDA, std::string(#call) + ": " + cudaGetErrorString(e_)); \
     } while (0)
 
+inline bool misaligned(const void *p) { return ((uintptr_t)p & 15u) != 0; }
+
 template <typename U>
 int dev_alloc(afsat_ctx *ctx, U **p, size_t count, bool zero = false)
 {
@@ -142,17 +153,18 @@ int upload(afsat_ctx *ctx, U **p, const std::vector<U> &h)
     return AFSAT_OK;
 }
 
-// model count of FP instructions for one (constraint, candidate): DESIGN.md cost model
+// model counts for one (constraint, candidate): DESIGN.md cost model
 inline int64_t cost_of(int k, int n_real, int n_cplx) { return (int64_t)k * (12 * n_cplx + 4 * n_real) + 2 * n_cplx + n_real; }
+inline int64_t flop_of(int k, int n_real, int n_cplx) { return (int64_t)k * (19 * n_cplx + 6 * n_real) + 4 * n_cplx + 2 * n_real; }
 
 inline int pow2_floor(int64_t v) { int p = 1; while ((int64_t)p * 2 <= v) p *= 2; return p; }
 
-// brackets one evaluation-kernel launch with events when profiling is on
+// brackets one evaluation-kernel launch set with events when profiling is on
 struct ProfScope {
     afsat_ctx *c; cudaStream_t st; cudaEvent_t e0 = nullptr, e1 = nullptr;
     ProfScope(afsat_ctx *c_, cudaStream_t st_) : c(c_), st(st_)
     {
-        if (!c->profiling) return;
+        if (!c->profiling || c->capturing) return;
         if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) { e0 = e1 = nullptr; return; }
         cudaEventRecord(e0, st);
     }
@@ -176,120 +188,70 @@ void prof_drain(afsat_ctx *c, bool keep)
     c->prof_events.clear();
 }
 
-// k <= 8: fp32 with >= 2 candidates per lane runs the packed FFMA2 kernel, everything else the scalar one
-template <typename T, int VA, int MB>
-void (*pick_a(bool grad))(EvalParams<T>)
-{
-    using Fn = void (*)(EvalParams<T>);
-#ifndef AFSAT_NO_FFMA2
-    if constexpr (sizeof(T) == 4 && VA >= 2) return grad ? (Fn)k_eval_f2m<1, 8, VA / 2, true, MB> : (Fn)k_eval_f2m<1, 8, VA / 2, false, MB>;
-    else
-#endif
-        return grad ? (Fn)k_eval_km<T, 1, 8, VA, true, MB> : (Fn)k_eval_km<T, 1, 8, VA, false, MB>;
-}
-
-// k <= AFSAT_S_KMAX, fp32: the packed kernel with two pairs (four candidates) per lane
-template <typename T, int MB>
-void (*pick_s(bool grad))(EvalParams<T>)
-{
-    using Fn = void (*)(EvalParams<T>);
-#if AFSAT_S_KMAX > 0
-    if constexpr (sizeof(T) == 4) return grad ? (Fn)k_eval_f2m<1, AFSAT_S_KMAX, 2, true, MB> : (Fn)k_eval_f2m<1, AFSAT_S_KMAX, 2, false, MB>;
-    else
-#endif
-        return nullptr;                                                // class S is empty for this dtype / build
-}
-
+// ---- kernel selection per length class ------------------------------------------------------------------------------
 template <typename T>
-void (*pick_b(bool grad))(EvalParams<T>)
+void (*pick_kernel(int cls, bool grad))(EvalParams<T>)
 {
     using Fn = void (*)(EvalParams<T>);
-    constexpr int KHI = sizeof(T) == 4 ? AFSAT_B_KMAX32 : AFSAT_B_KMAX64;
-#if AFSAT_M32_PACKED
-    if constexpr (sizeof(T) == 4)                                      // fp32: the packed lane-split kernel
-        return grad ? (Fn)k_eval_split<float, 9, AFSAT_B_KMAX32, 2, 2, true, AFSAT_M32_THREADS, 1>
-                    : (Fn)k_eval_split<float, 9, AFSAT_B_KMAX32, 2, 2, false, AFSAT_M32_THREADS, 1>;
-    else
-#endif
-    return grad ? (Fn)k_eval_km<T, 9, KHI, 1, true, AFSAT_B_MINB> : (Fn)k_eval_km<T, 9, KHI, 1, false, AFSAT_B_MINB>;
-}
-
-// k > 16: KMAX is the unroll bound of the register-blocked kernels; fp32 runs the packed two-candidate form
-inline int long_kmax(int kmax_long) { return kmax_long <= 32 ? 32 : kmax_long <= 40 ? 40 : kmax_long <= 48 ? 48 : kmax_long <= 56 ? 56 : 64; }
-template <typename T>
-void (*pick_long(int km, bool grad))(EvalParams<T>)
-{
-    using Fn = void (*)(EvalParams<T>);
-    if constexpr (sizeof(T) == 4) {                                    // fp32: the lane-split register kernel
-        return grad ? (Fn)k_eval_split<float, AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, 1, true, AFSAT_L32_THREADS, AFSAT_L32_MINB>
-                    : (Fn)k_eval_split<float, AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, 1, false, AFSAT_L32_THREADS, AFSAT_L32_MINB>;
+    if constexpr (sizeof(T) == 4) {
+        switch (cls) {
+        case CLS_S: return grad ? (Fn)k_eval_f2m<1, AFSAT_S_KMAX, 2, true, 2> : (Fn)k_eval_f2m<1, AFSAT_S_KMAX, 2, false, 2>;
+        case CLS_A: return grad ? (Fn)k_eval_f2m<AFSAT_S_KMAX + 1, AFSAT_A_KMAX, 1, true, 2> : (Fn)k_eval_f2m<AFSAT_S_KMAX + 1, AFSAT_A_KMAX, 1, false, 2>;
+        case CLS_B: return grad ? (Fn)k_eval_split<float, AFSAT_A_KMAX + 1, AFSAT_B_KMAX, 2, 2, true, AFSAT_M32_THREADS, 1>
+                                : (Fn)k_eval_split<float, AFSAT_A_KMAX + 1, AFSAT_B_KMAX, 2, 2, false, AFSAT_M32_THREADS, 1>;
+        default:    return grad ? (Fn)k_eval_split<float, AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, 1, true, AFSAT_L32_THREADS, AFSAT_L32_MINB>
+                                : (Fn)k_eval_split<float, AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, 1, false, AFSAT_L32_THREADS, AFSAT_L32_MINB>;
+        }
     } else {
-#if AFSAT_L64_SPLIT
-        return grad ? (Fn)k_eval_split<double, AFSAT_L64_KMIN, AFSAT_MAX_LEN, 4, 1, true, AFSAT_L64_THREADS, 1>
-                    : (Fn)k_eval_split<double, AFSAT_L64_KMIN, AFSAT_MAX_LEN, 4, 1, false, AFSAT_L64_THREADS, 1>;
-#endif
-#define AFSAT_LONG_CASE(KM_)                                                                                  \
-    case KM_:                                                                                                 \
-        return grad ? (Fn)k_eval_blk<T, KM_, true> : (Fn)k_eval_blk<T, KM_, false>;
-    switch (km) {
-        AFSAT_LONG_CASE(32) AFSAT_LONG_CASE(40) AFSAT_LONG_CASE(48) AFSAT_LONG_CASE(56)
-    default:
-        AFSAT_LONG_CASE(64)
-    }
-#undef AFSAT_LONG_CASE
+        switch (cls) {
+        case CLS_S: return nullptr;                                    // empty for fp64
+        case CLS_A: return grad ? (Fn)k_eval_km<T, 1, AFSAT_A_KMAX, 1, true, 1> : (Fn)k_eval_km<T, 1, AFSAT_A_KMAX, 1, false, 1>;
+        case CLS_B: return grad ? (Fn)k_eval_km<T, AFSAT_A_KMAX + 1, AFSAT_B_KMAX, 1, true, 1> : (Fn)k_eval_km<T, AFSAT_A_KMAX + 1, AFSAT_B_KMAX, 1, false, 1>;
+        default:    return grad ? (Fn)k_eval_split<double, AFSAT_L64_KMIN, AFSAT_MAX_LEN, 4, 1, true, AFSAT_L64_THREADS, 1>
+                                : (Fn)k_eval_split<double, AFSAT_L64_KMIN, AFSAT_MAX_LEN, 4, 1, false, AFSAT_L64_THREADS, 1>;
+        }
     }
 }
 
-// ---- launch of the evaluation kernels (a1-a5) for the candidate tile [b_begin, b_begin + width) ----
+// ---- launch of the evaluation kernels (a1-a5) of group gp for the candidate tile [b_begin, b_begin + width) ----
 template <typename T>
-int launch_eval(afsat_ctx *ctx, const T *x, T *G, int64_t g_ld, int64_t g_b0, T *Fpart, int64_t b_begin, int64_t width,
-                cudaStream_t st)
+int launch_eval(afsat_ctx *ctx, const GroupPlan &gp, const T *x, T *G, int64_t g_ld, int64_t g_b0, T *Fpart, int64_t b_begin,
+                int64_t width, cudaStream_t st)
 {
     EvalParams<T> p;
     p.x = x; p.G = G; p.g_ld = g_ld; p.g_b0 = g_b0; p.Fpart = Fpart;
-    p.lits = ctx->d_lits; p.sigs = ctx->d_sigs; p.rows = (const T *)ctx->d_rows; p.rows2 = ctx->d_rows2;
+    p.lits = gp.d_lits; p.sigs = ctx->d_sigs; p.rows = (const T *)ctx->d_rows; p.rows2 = ctx->d_rows2;
     p.skip = ctx->cur_skip;
     p.B = ctx->B; p.ldb = ctx->ldb; p.b_begin = b_begin; p.b_end = std::min<int64_t>(b_begin + width, ctx->ldb);
     const bool grad = G != nullptr;
-    constexpr int VA = sizeof(T) == 4 ? AFSAT_A_V : 1;
     // The length classes are independent (they only share the RED target), so their launches run
-    // CONCURRENTLY: class 0 on the caller's stream, the others on forked side streams that join back.
+    // CONCURRENTLY: the first active class on the caller's stream, the others on forked side streams that join back.
     int n_active = 0;
-    for (int cls = 0; cls < N_CLS; ++cls) n_active += ctx->cls_begin[cls + 1] > ctx->cls_begin[cls];
+    for (int cls = 0; cls < N_CLS; ++cls) n_active += gp.cls_begin[cls + 1] > gp.cls_begin[cls];
     ProfScope prof(ctx, st);                                          // brackets the whole launch set
     const bool fork = n_active > 1;
     if (fork) CU(cudaEventRecord(ctx->ev_fork, st));
     int side = 0;
+    bool first_active = true;
     cudaStream_t user_st = st;
     for (int cls = 0; cls < N_CLS; ++cls) {
-        const int nit = ctx->cls_begin[cls + 1] - ctx->cls_begin[cls];
+        const int nit = gp.cls_begin[cls + 1] - gp.cls_begin[cls];
         if (nit == 0) continue;
         st = user_st;
         int my_side = -1;
-        if (fork && side < N_CLS - 1 && cls != 0 && ctx->cls_begin[cls] != 0) {   // not the first active class
+        if (fork && !first_active && side < N_CLS - 1) {
             my_side = side++;
             st = ctx->side_stream[my_side];
             CU(cudaStreamWaitEvent(st, ctx->ev_fork, 0));
         }
+        first_active = false;
         const ClassGeom &g = ctx->geom[cls];
-        p.items = ctx->d_items + ctx->cls_begin[cls];
-        p.frow_base = ctx->cls_begin[cls];
+        p.items = gp.d_items + gp.cls_begin[cls];
+        p.frow_base = gp.cls_begin[cls];
         p.Wc = g.Wc; p.Wk = g.Wk;
         const int64_t per_cta = (int64_t)g.cw * g.Wc;
         dim3 block(32 * g.warps), grid(nit, (unsigned)((width + per_cta - 1) / per_cta));
-        if (cls != CLS_LONG) {
-            using Fn = void (*)(EvalParams<T>);
-            constexpr int MB = sizeof(T) == 4 ? AFSAT_A_MINB : 1;
-            Fn fn = cls == CLS_S ? pick_s<T, MB>(grad)
-                  : cls == CLS_A ? pick_a<T, VA, MB>(grad)
-                                 : pick_b<T>(grad);
-            fn<<<grid, block, 0, st>>>(p);
-        } else {
-            using Fn = void (*)(EvalParams<T>);
-            Fn fn = pick_long<T>(long_kmax(ctx->kmax_long), grad);
-            if (g.smem) CU(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem));
-            fn<<<grid, block, g.smem, st>>>(p);
-        }
+        pick_kernel<T>(cls, grad)<<<grid, block, 0, st>>>(p);
         ++ctx->launches;
         CU(cudaPeekAtLastError());
         if (my_side >= 0) {
@@ -300,23 +262,36 @@ int launch_eval(afsat_ctx *ctx, const T *x, T *G, int64_t g_ld, int64_t g_b0, T 
     return AFSAT_OK;
 }
 
-// a8 on the words [w_begin, w_end) of the sign-bit array
-int launch_check_bits(afsat_ctx *ctx, int64_t w_begin, int64_t w_end, cudaStream_t st)
+// a8 for group gp on the words [w_begin, w_end) of the sign-bit array
+int launch_check_bits(afsat_ctx *ctx, const GroupPlan &gp, int64_t w_begin, int64_t w_end, int32_t *step_ctr, cudaStream_t st)
 {
-    if (ctx->n_items == 0 || w_end <= w_begin) return AFSAT_OK;
+    if (w_end <= w_begin) return AFSAT_OK;
     CheckParams p;
-    p.bits = ctx->d_bits; p.ldw = ctx->ldb / 32; p.lits = ctx->d_lits; p.sigs = ctx->d_sigs; p.items = ctx->d_items;
+    p.bits = ctx->d_bits; p.ldw = ctx->ldb / 32; p.lits = gp.d_lits; p.sigs = ctx->d_sigs; p.items = gp.d_items;
     p.satacc = ctx->d_satacc; p.B = ctx->B; p.w_begin = (int32_t)w_begin; p.w_end = (int32_t)w_end;
+    p.step_ctr = step_ctr;
     const int64_t nw = w_end - w_begin;
     p.wpb = std::min(32, pow2_floor(nw));
     if (p.wpb < nw && p.wpb < 32) p.wpb *= 2;                         // cover a ragged word count in one CTA row
     p.wpb = std::min(p.wpb, 32);
-    p.n_items = ctx->n_items;
+    p.n_items = gp.n_items;
     const unsigned gy = (unsigned)((nw + p.wpb - 1) / p.wpb);
-    dim3 grid((unsigned)std::max<int64_t>(1, std::min<int64_t>(ctx->n_items, (int64_t)ctx->sm_count * 4 / gy)), gy);
+    dim3 grid((unsigned)std::max<int64_t>(1, std::min<int64_t>(std::max(1, gp.n_items), (int64_t)ctx->sm_count * 8 / gy)), gy);
     k_check_bits<<<grid, CTA_THREADS, 0, st>>>(p);
     ++ctx->launches;
     CU(cudaPeekAtLastError());
+    return AFSAT_OK;
+}
+
+// a8 over the whole batch: one launch per partial-assignment group
+int check_all(afsat_ctx *ctx, bool count_step, cudaStream_t st)
+{
+    for (size_t g = 0; g < ctx->groups.size(); ++g) {
+        const GroupPlan &gp = ctx->groups[g];
+        const int64_t w1 = (g + 1 == ctx->groups.size()) ? ctx->ldb / 32 : gp.b1 / 32;
+        int rc = launch_check_bits(ctx, gp, gp.b0 / 32, w1, (count_step && g == 0) ? ctx->d_any + 3 : nullptr, st);
+        if (rc) return rc;
+    }
     return AFSAT_OK;
 }
 
@@ -334,9 +309,29 @@ int launch_pack(afsat_ctx *ctx, const T *x, cudaStream_t st)
 template <typename T>
 int reduce_F(afsat_ctx *ctx, T *F, cudaStream_t st)
 {
-    k_reduce_F<T><<<(ctx->B + 127) / 128, 128, 0, st>>>((const T *)ctx->d_Fpart, ctx->n_items, ctx->ldb, ctx->B, F, ctx->cur_skip);
-    ++ctx->launches;
-    CU(cudaPeekAtLastError());
+    for (const GroupPlan &gp : ctx->groups) {
+        const int64_t b1 = std::min<int64_t>(gp.b1, ctx->B);
+        if (b1 <= gp.b0) continue;
+        k_reduce_F<T><<<(unsigned)((b1 - gp.b0 + 127) / 128), 128, 0, st>>>((const T *)ctx->d_Fpart, gp.n_items, ctx->ldb, gp.b0, b1,
+                                                                           gp.F_const, F, ctx->cur_skip);
+        ++ctx->launches;
+        CU(cudaPeekAtLastError());
+    }
+    return AFSAT_OK;
+}
+
+// the candidate tiles of a step: for every group, [b, b + w) with w <= tile_w inside the group's columns
+template <typename Fn>
+int for_tiles(afsat_ctx *ctx, Fn &&fn)
+{
+    for (size_t g = 0; g < ctx->groups.size(); ++g) {
+        const GroupPlan &gp = ctx->groups[g];
+        const int64_t end = (g + 1 == ctx->groups.size()) ? ctx->ldb : gp.b1;   // the last group owns the padding columns
+        for (int64_t b0 = gp.b0; b0 < end && b0 < ctx->B; b0 += ctx->tile_w) {
+            int rc = fn(gp, b0, std::min<int64_t>(ctx->tile_w, end - b0));
+            if (rc) return rc;
+        }
+    }
     return AFSAT_OK;
 }
 
@@ -344,11 +339,10 @@ template <typename T>
 int eval_grad_t(afsat_ctx *ctx, const T *x, T *F, T *G, cudaStream_t st)
 {
     if (G) CU(cudaMemsetAsync(G, 0, (size_t)ctx->n * ctx->ldb * sizeof(T), st));
-    for (int64_t b0 = 0; b0 < ctx->B; b0 += ctx->tile_w) {            // candidate tiles keep X/G tiles L2-resident
-        const int64_t w = std::min<int64_t>(ctx->tile_w, ctx->ldb - b0);
-        int rc = launch_eval<T>(ctx, x, G, ctx->ldb, 0, F ? (T *)ctx->d_Fpart : nullptr, b0, w, st);
-        if (rc) return rc;
-    }
+    int rc = for_tiles(ctx, [&](const GroupPlan &gp, int64_t b0, int64_t w) {   // candidate tiles keep X/G tiles L2-resident
+        return launch_eval<T>(ctx, gp, x, G, ctx->ldb, 0, F ? (T *)ctx->d_Fpart : nullptr, b0, w, st);
+    });
+    if (rc) return rc;
     if (G && ctx->B < ctx->ldb && (ctx->B & 3)) {                     // a lane's candidates straddle B: clear the spill
         k_zero_pad<T><<<std::min(1024, ctx->n), 128, 0, st>>>(G, ctx->n, ctx->B, ctx->ldb);
         ++ctx->launches;
@@ -358,58 +352,145 @@ int eval_grad_t(afsat_ctx *ctx, const T *x, T *F, T *G, cudaStream_t st)
     return AFSAT_OK;
 }
 
+// a6, a7, a9 on the candidate columns [b0, b0 + w) of group gp; G is the gradient array with leading dimension g_ld whose
+// column 0 is candidate g_b0
 template <typename T>
-int step_t(afsat_ctx *ctx, T *x, double eta, int n_steps, int step_base, int resume, T *F, int32_t *sat,
+int launch_update(afsat_ctx *ctx, const GroupPlan &gp, T *x, T *G, int64_t g_ld, int64_t g_b0, const uint8_t *sol, double eta,
+                  int64_t b0, int64_t w, cudaStream_t st)
+{
+    constexpr int VW = Vec16<T>::VW;
+    const int tpr = std::min<int>(CTA_THREADS, pow2_floor(w / VW));   // w is a multiple of 32: tpr >= 32 / VW lanes = whole words
+    const unsigned gx = (unsigned)((w / VW + tpr - 1) / tpr);
+    const int rpp = CTA_THREADS / tpr;
+    const unsigned gy = (unsigned)std::max<int64_t>(1, std::min<int64_t>((ctx->n + rpp * UPD_UNROLL - 1) / (rpp * UPD_UNROLL),
+                                                                           (int64_t)ctx->sm_count * 8 / gx));
+    const size_t gi = &gp - ctx->groups.data();
+    k_update<T><<<dim3(gx, gy), CTA_THREADS, 0, st>>>(x, G, g_ld, g_b0, ctx->d_fixed + gi * (size_t)ctx->n, sol, ctx->d_bits, (T)eta,
+                                                      ctx->n, ctx->B, ctx->ldb, b0, b0 + w, tpr);
+    ++ctx->launches;
+    CU(cudaPeekAtLastError());
+    return AFSAT_OK;
+}
+
+// one iteration of Alg. 1 over the whole batch (a1-a9); step_value < 0: the step index comes from the device counter
+template <typename T>
+int one_iteration(afsat_ctx *ctx, T *x, double eta, int step_value, bool want_pre, int32_t *sat, uint8_t *sol, int32_t *first,
+                  int32_t *h_any_dev, cudaStream_t st)
+{
+    const int B = ctx->B, tb = 128, gb = (B + tb - 1) / tb;
+    const int64_t tw = ctx->tile_w;
+    int rc = for_tiles(ctx, [&](const GroupPlan &gp, int64_t b0, int64_t w) {
+        // a1-a5: gradient at X(t-1) into the (zeroed) tile scratch
+        int r = launch_eval<T>(ctx, gp, x, (T *)ctx->d_G, tw, b0, want_pre ? (T *)ctx->d_Fpart : nullptr, b0, w, st);
+        if (r) return r;
+        // a6, a7, a9: X(t) = clamp(X(t-1) - eta G) on free variables of unsolved candidates, sign bits, G reset
+        return launch_update<T>(ctx, gp, x, (T *)ctx->d_G, tw, b0, sol, eta, b0, w, st);
+    });
+    if (rc) return rc;
+    // a8: exact count on X(t), one launch per group over its whole batch: every constraint reads the full bit rows of its
+    // variables (coalesced), 1 bit per literal and candidate
+    rc = check_all(ctx, step_value < 0, st);
+    if (rc) return rc;
+    k_flags<<<gb, tb, 0, st>>>(ctx->d_satacc, B, ctx->m, 1, step_value, step_value < 0 ? ctx->d_any + 3 : nullptr, ctx->d_sat_const,
+                               ctx->group_w, (int)ctx->groups.size(), sat, sol, first, ctx->d_any, h_any_dev);
+    ++ctx->launches;
+    CU(cudaPeekAtLastError());
+    return AFSAT_OK;
+}
+
+// the whole loop in ONE launch (k_step_small)
+template <typename T>
+int step_small(afsat_ctx *ctx, T *x, double eta, int n_steps, int step_base, int32_t *sat, uint8_t *sol, int32_t *first,
+               int32_t *h_any_dev, cudaStream_t st)
+{
+    const GroupPlan &gp = ctx->groups[0];
+    SmallParams<T> p;
+    p.x = x; p.ldb = ctx->ldb; p.n = ctx->n; p.B = ctx->B; p.m = ctx->m; p.n_items = gp.n_items;
+    p.lits = gp.d_lits; p.items = gp.d_items; p.sigs = ctx->d_sigs; p.rows = (const T *)ctx->d_rows; p.fixed = ctx->d_fixed;
+    p.eta = (T)eta; p.n_steps = n_steps; p.step_base = step_base; p.sat_const = gp.sat_const;
+    p.n_ctas = (ctx->B + 31) / 32;
+    p.sat_count = sat; p.is_solution = sol; p.first_step = first; p.d_any = ctx->d_any; p.h_any = h_any_dev;
+    k_step_small<T><<<p.n_ctas, SMALL_THREADS, ctx->small_smem, st>>>(p);
+    ++ctx->launches;
+    CU(cudaPeekAtLastError());
+    return AFSAT_OK;
+}
+
+template <typename T>
+int step_t(afsat_ctx *ctx, T *x, double eta, int n_steps, int step_base, int resume, T *F, T *F_pre, int32_t *sat,
            uint8_t *sol, int32_t *first, int32_t *h_any_dev, cudaStream_t st)
 {
     const int B = ctx->B, tb = 128, gb = (B + tb - 1) / tb;
-    if (!resume) {
-        k_reset_state<<<gb, tb, 0, st>>>(B, sol, first);
-        ++ctx->launches;
-    }
-    CU(cudaMemsetAsync(ctx->d_any, 0, 2 * sizeof(int32_t), st));
-    const int64_t tw = ctx->tile_w;
-    for (int t = 1; t <= n_steps; ++t) {
-        for (int64_t b0 = 0; b0 < B; b0 += tw) {
-            const int64_t w = std::min<int64_t>(tw, ctx->ldb - b0);
-            // a1-a5: gradient at X(t-1) into the (zeroed) tile scratch
-            int rc = launch_eval<T>(ctx, x, (T *)ctx->d_G, tw, b0, nullptr, b0, w, st);
-            if (rc) return rc;
-            // a6, a7, a9: X(t) = clamp(X(t-1) - eta G) on free variables of unsolved candidates, sign bits, G reset
-            const int cols = (int)std::min<int64_t>(CTA_THREADS, w);                 // w is a multiple of 32
-            const int ucols = CTA_THREADS % cols == 0 ? cols : 32;
-            const unsigned gx = (unsigned)((w + ucols - 1) / ucols);
-            const int rpp = CTA_THREADS / ucols;
-            const unsigned gy = (unsigned)std::max<int64_t>(1, std::min<int64_t>((ctx->n + rpp * UPD_UNROLL - 1) / (rpp * UPD_UNROLL),
-                                                                                   (int64_t)ctx->sm_count * 8 / gx));
-            k_update<T><<<dim3(gx, gy), CTA_THREADS, 0, st>>>(x, (T *)ctx->d_G, tw, b0, ctx->d_fixed, sol, ctx->d_bits, (T)eta,
-                                                              ctx->n, B, ctx->ldb, b0, b0 + w, ucols);
-            ++ctx->launches;
-            CU(cudaPeekAtLastError());
-        }
-        // a8: exact count on X(t), ONE launch over the whole batch: every constraint reads the full
-        // [ldb/32]-word bit rows of its variables (coalesced), 1 bit per literal and candidate
-        {
-            int rc = launch_check_bits(ctx, 0, ctx->ldb / 32, st);
-            if (rc) return rc;
-        }
-        k_flags<<<gb, tb, 0, st>>>(ctx->d_satacc, B, ctx->m, 1, step_base + t, sat, sol, first, ctx->d_any, h_any_dev);
-        ++ctx->launches;
-        CU(cudaPeekAtLastError());
-    }
-    if (n_steps == 0) {                                               // no step: count on X as it is, mark nothing
-        int rc = launch_pack<T>(ctx, x, st);
-        if (!rc) rc = launch_check_bits(ctx, 0, ctx->ldb / 32, st);
+    k_reset_state<<<gb, tb, 0, st>>>(B, !resume, sol, first, ctx->d_any, h_any_dev, step_base);
+    ++ctx->launches;
+    CU(cudaPeekAtLastError());
+    int path = ctx->step_path;
+    if (path == AFSAT_STEP_PERSISTENT && (F_pre || ctx->profiling)) path = AFSAT_STEP_LAUNCHES;   // F_pre is a by-product of the big kernels
+    if (path == AFSAT_STEP_GRAPH && (ctx->profiling || n_steps < 3)) path = AFSAT_STEP_LAUNCHES;
+    if (path == AFSAT_STEP_PERSISTENT) {
+        int rc = step_small<T>(ctx, x, eta, n_steps, step_base, sat, sol, first, h_any_dev, st);
         if (rc) return rc;
-        k_flags<<<gb, tb, 0, st>>>(ctx->d_satacc, B, ctx->m, 0, step_base, sat, sol, first, ctx->d_any, h_any_dev);
+    } else if (n_steps == 0) {                                        // no step: count on X as it is, mark nothing
+        int rc = launch_pack<T>(ctx, x, st);
+        if (!rc) rc = check_all(ctx, false, st);
+        if (rc) return rc;
+        k_flags<<<gb, tb, 0, st>>>(ctx->d_satacc, B, ctx->m, 0, step_base, nullptr, ctx->d_sat_const, ctx->group_w,
+                                   (int)ctx->groups.size(), sat, sol, first, ctx->d_any, h_any_dev);
         ++ctx->launches;
         CU(cudaPeekAtLastError());
+    } else {
+        int t = 1;
+        if (path == AFSAT_STEP_GRAPH) {                               // iterations 1 .. n_steps - 1 (or all): graph replays
+            StepGraph &sg = ctx->graph;
+            const bool stale = !sg.exec || sg.x != x || sg.sat != sat || sg.sol != sol || sg.first != first ||
+                               sg.h_any != h_any_dev || sg.eta != eta;
+            bool ok = true;
+            if (stale) {
+                if (sg.exec) { cudaGraphExecDestroy(sg.exec); sg.exec = nullptr; }
+                cudaGraph_t graph = nullptr;
+                const int64_t l0 = ctx->launches;
+                ok = cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+                if (ok) {
+                    ctx->capturing = true;
+                    const int rc = one_iteration<T>(ctx, x, eta, -1, false, sat, sol, first, h_any_dev, st);
+                    ctx->capturing = false;
+                    const cudaError_t e = cudaStreamEndCapture(st, &graph);
+                    ok = rc == AFSAT_OK && e == cudaSuccess && graph &&
+                         cudaGraphInstantiate(&sg.exec, graph, 0) == cudaSuccess;
+                    if (graph) cudaGraphDestroy(graph);
+                }
+                ctx->launches = l0;                                   // captured, not launched
+                if (ok) { sg.x = x; sg.sat = sat; sg.sol = sol; sg.first = first; sg.h_any = h_any_dev; sg.eta = eta; }
+                else { cudaGetLastError(); sg.exec = nullptr; }
+            }
+            if (ok) {
+                const int n_replay = F_pre ? n_steps - 1 : n_steps;
+                int per_iter = 2;                                      // k_check_bits per group + k_flags
+                for (const GroupPlan &gp : ctx->groups) {
+                    int act = 0;
+                    for (int cls = 0; cls < N_CLS; ++cls) act += gp.cls_begin[cls + 1] > gp.cls_begin[cls];
+                    const int64_t end = (&gp == &ctx->groups.back()) ? ctx->ldb : gp.b1;
+                    per_iter += (int)((std::min<int64_t>(end, ctx->B) - gp.b0 + ctx->tile_w - 1) / ctx->tile_w) * (act + 1);
+                }
+                per_iter += (int)ctx->groups.size() - 1;
+                for (; t <= n_replay; ++t) {
+                    CU(cudaGraphLaunch(sg.exec, st));
+                    ctx->launches += per_iter;
+                }
+            }
+        }
+        for (; t <= n_steps; ++t) {
+            int rc = one_iteration<T>(ctx, x, eta, path == AFSAT_STEP_GRAPH ? -1 : step_base + t, F_pre && t == n_steps, sat, sol,
+                                      first, h_any_dev, st);
+            if (rc) return rc;
+        }
+        if (F_pre) { int rc = reduce_F<T>(ctx, F_pre, st); if (rc) return rc; }
     }
     if (F) {                                                          // objective at the final X
-        for (int64_t b0 = 0; b0 < B; b0 += tw) {
-            int rc = launch_eval<T>(ctx, x, nullptr, 0, 0, (T *)ctx->d_Fpart, b0, std::min<int64_t>(tw, ctx->ldb - b0), st);
-            if (rc) return rc;
-        }
+        int rc = for_tiles(ctx, [&](const GroupPlan &gp, int64_t b0, int64_t w) {
+            return launch_eval<T>(ctx, gp, x, (T *)nullptr, 0, 0, (T *)ctx->d_Fpart, b0, w, st);
+        });
+        if (rc) return rc;
         return reduce_F<T>(ctx, F, st);
     }
     return AFSAT_OK;
@@ -424,6 +505,7 @@ int step_ls_t(afsat_ctx *ctx, T *x, double s_max, double beta, double c1, double
     const int B = ctx->B, tb = 128, gb = (B + tb - 1) / tb;
     const int64_t ldb = ctx->ldb;
     const size_t nb = (size_t)ctx->n * ldb;
+    const int ng = (int)ctx->groups.size();
     if (!ctx->ls_G) {
         int rc;
         char *pg = nullptr, *px = nullptr, *p0 = nullptr, *p1 = nullptr;
@@ -440,12 +522,9 @@ int step_ls_t(afsat_ctx *ctx, T *x, double s_max, double beta, double c1, double
         if ((rc = dev_alloc(ctx, &ctx->ls_state, (size_t)ldb, true))) return rc;
     }
     T *G = (T *)ctx->ls_G, *xt = (T *)ctx->ls_xt, *F0 = (T *)ctx->ls_F0, *F1 = (T *)ctx->ls_F1;
-    if (!resume) {
-        k_reset_state<<<gb, tb, 0, st>>>(B, sol, first);
-        ++ctx->launches;
-        CU(cudaMemsetAsync(conv, 0, (size_t)B, st));
-    }
-    CU(cudaMemsetAsync(ctx->d_any, 0, 2 * sizeof(int32_t), st));
+    k_reset_state<<<gb, tb, 0, st>>>(B, !resume, sol, first, ctx->d_any, h_any_dev, step_base);
+    ++ctx->launches;
+    if (!resume) CU(cudaMemsetAsync(conv, 0, (size_t)B, st));
     const unsigned gl = (unsigned)((ldb + CTA_THREADS - 1) / CTA_THREADS);
     const unsigned gyc = (unsigned)std::min<int64_t>(ctx->n, std::max<int64_t>(1, (int64_t)ctx->sm_count * 8 / gl));
     if (n_steps == 0) {                                               // no step: F, counts on X as it is
@@ -453,9 +532,10 @@ int step_ls_t(afsat_ctx *ctx, T *x, double s_max, double beta, double c1, double
         ++ctx->launches;
         int rc = eval_grad_t<T>(ctx, x, F0, (T *)nullptr, st);
         if (!rc) rc = launch_pack<T>(ctx, x, st);
-        if (!rc) rc = launch_check_bits(ctx, 0, ldb / 32, st);
+        if (!rc) rc = check_all(ctx, false, st);
         if (rc) return rc;
-        k_flags<<<gb, tb, 0, st>>>(ctx->d_satacc, B, ctx->m, 0, step_base, sat, sol, first, ctx->d_any, h_any_dev);
+        k_flags<<<gb, tb, 0, st>>>(ctx->d_satacc, B, ctx->m, 0, step_base, nullptr, ctx->d_sat_const, ctx->group_w, ng, sat, sol,
+                                   first, ctx->d_any, h_any_dev);
         ++ctx->launches;
     }
     for (int t = 1; t <= n_steps; ++t) {
@@ -467,8 +547,8 @@ int step_ls_t(afsat_ctx *ctx, T *x, double s_max, double beta, double c1, double
         ctx->cur_skip = nullptr;
         if (rc) return rc;
         for (int j = 0; j < max_trials; ++j) {
-            k_ls_trial<T><<<dim3(gl, LS_CHUNKS), CTA_THREADS, 0, st>>>(x, G, xt, ctx->d_fixed, ctx->ls_state, ctx->ls_eta,
-                                                                        ctx->ls_Dpart, ctx->n, ldb, j == 0);
+            k_ls_trial<T><<<dim3(gl, LS_CHUNKS), CTA_THREADS, 0, st>>>(x, G, xt, ctx->d_fixed, ctx->group_w, ng, ctx->ls_state,
+                                                                        ctx->ls_eta, ctx->ls_Dpart, ctx->n, ldb, j == 0);
             ++ctx->launches;
             CU(cudaPeekAtLastError());
             ctx->cur_skip = ctx->ls_state;                            // objective only, candidates still searching
@@ -482,9 +562,10 @@ int step_ls_t(afsat_ctx *ctx, T *x, double s_max, double beta, double c1, double
         k_ls_commit<T><<<dim3(gl, gyc), CTA_THREADS, 0, st>>>(x, xt, ctx->ls_state, ctx->d_bits, ctx->n, B, ldb);
         ++ctx->launches;
         CU(cudaPeekAtLastError());
-        rc = launch_check_bits(ctx, 0, ldb / 32, st);
+        rc = check_all(ctx, false, st);
         if (rc) return rc;
-        k_flags<<<gb, tb, 0, st>>>(ctx->d_satacc, B, ctx->m, 1, step_base + t, sat, sol, first, ctx->d_any, h_any_dev);
+        k_flags<<<gb, tb, 0, st>>>(ctx->d_satacc, B, ctx->m, 1, step_base + t, nullptr, ctx->d_sat_const, ctx->group_w, ng, sat,
+                                   sol, first, ctx->d_any, h_any_dev);
         ++ctx->launches;
         CU(cudaPeekAtLastError());
     }
@@ -504,12 +585,83 @@ int set_device(afsat_ctx *ctx)
     return AFSAT_OK;
 }
 
+// One fixed-step iteration on host buffers with the copies pipelined behind the evaluation: the batch is cut into
+// candidate chunks (the tiles of a tiled step, else four), chunk c + 1 is uploaded and chunk c - 1 downloaded while
+// chunk c is evaluated and updated; the count and the flags follow once for the whole batch.
+template <typename T>
+int step_host_pipelined(afsat_ctx *ctx, T *h_x, double eta, T *h_F_pre)
+{
+    cudaStream_t st = ctx->own_stream;
+    const int B = ctx->B, tb = 128, gb = (B + tb - 1) / tb;
+    const int64_t ldb = ctx->ldb;
+    const bool tiled = ctx->tile_w < (ctx->groups.size() > 1 ? ctx->group_w : ldb);
+    T *x = (T *)ctx->dh_x;
+    struct Chunk { const GroupPlan *gp; int64_t b0, w; };
+    std::vector<Chunk> chunks;
+    if (tiled) {
+        for_tiles(ctx, [&](const GroupPlan &gp, int64_t b0, int64_t w) { chunks.push_back({&gp, b0, w}); return 0; });
+    } else {
+        for (size_t g = 0; g < ctx->groups.size(); ++g) {
+            const GroupPlan &gp = ctx->groups[g];
+            const int64_t end = (g + 1 == ctx->groups.size()) ? ldb : gp.b1;
+            const int64_t cw = std::max<int64_t>(128, ((end - gp.b0 + 3) / 4 + 127) / 128 * 128);
+            for (int64_t b0 = gp.b0; b0 < end && b0 < B; b0 += cw) chunks.push_back({&gp, b0, std::min(cw, end - b0)});
+        }
+    }
+    while (ctx->chunk_in.size() < chunks.size()) {
+        cudaEvent_t a, b;
+        CU(cudaEventCreateWithFlags(&a, cudaEventDisableTiming));
+        CU(cudaEventCreateWithFlags(&b, cudaEventDisableTiming));
+        ctx->chunk_in.push_back(a); ctx->chunk_done.push_back(b);
+    }
+    k_reset_state<<<gb, tb, 0, st>>>(B, 1, ctx->dh_sol, ctx->dh_first, ctx->d_any, nullptr, 0);
+    ++ctx->launches;
+    T *G = tiled ? (T *)ctx->d_G : (T *)ctx->ls_G;                     // un-tiled: a full-width gradient (the line-search buffer)
+    if (!tiled) CU(cudaMemsetAsync(G, 0, (size_t)ctx->n * ldb * sizeof(T), st));
+    CU(cudaEventRecord(ctx->ev_fork, st));
+    CU(cudaStreamWaitEvent(ctx->in_stream, ctx->ev_fork, 0));          // uploads start after earlier work on the buffers
+    CU(cudaStreamWaitEvent(ctx->out_stream, ctx->ev_fork, 0));
+    for (size_t c = 0; c < chunks.size(); ++c) {
+        const Chunk &ch = chunks[c];
+        CU(cudaMemcpy2DAsync(x + ch.b0, ldb * sizeof(T), h_x + ch.b0, ldb * sizeof(T), ch.w * sizeof(T), ctx->n,
+                             cudaMemcpyHostToDevice, ctx->in_stream));
+        CU(cudaEventRecord(ctx->chunk_in[c], ctx->in_stream));
+    }
+    for (size_t c = 0; c < chunks.size(); ++c) {
+        const Chunk &ch = chunks[c];
+        CU(cudaStreamWaitEvent(st, ctx->chunk_in[c], 0));
+        int rc = launch_eval<T>(ctx, *ch.gp, x, G, tiled ? ctx->tile_w : ldb, tiled ? ch.b0 : 0, h_F_pre ? (T *)ctx->d_Fpart : nullptr,
+                                ch.b0, ch.w, st);
+        if (!rc) rc = launch_update<T>(ctx, *ch.gp, x, G, tiled ? ctx->tile_w : ldb, tiled ? ch.b0 : 0, ctx->dh_sol, eta, ch.b0, ch.w, st);
+        if (rc) return rc;
+        CU(cudaEventRecord(ctx->chunk_done[c], st));
+        CU(cudaStreamWaitEvent(ctx->out_stream, ctx->chunk_done[c], 0));
+        CU(cudaMemcpy2DAsync(h_x + ch.b0, ldb * sizeof(T), x + ch.b0, ldb * sizeof(T), ch.w * sizeof(T), ctx->n,
+                             cudaMemcpyDeviceToHost, ctx->out_stream));
+    }
+    int rc = check_all(ctx, false, st);
+    if (rc) return rc;
+    k_flags<<<gb, tb, 0, st>>>(ctx->d_satacc, B, ctx->m, 1, 1, nullptr, ctx->d_sat_const, ctx->group_w, (int)ctx->groups.size(),
+                               ctx->dh_sat, ctx->dh_sol, ctx->dh_first, ctx->d_any, nullptr);
+    ++ctx->launches;
+    CU(cudaPeekAtLastError());
+    if (h_F_pre) { rc = reduce_F<T>(ctx, (T *)ctx->dh_Fpre, st); if (rc) return rc; }
+    return AFSAT_OK;
+}
+
+// A constraint under a partial assignment: f_T of its literals are fixed true, the k' free ones keep a
+// symmetric constraint whose truth table is the original one shifted by f_T.
+struct SigKey {
+    int k; uint64_t lo, hi;
+    bool operator<(const SigKey &o) const { return std::tie(k, lo, hi) < std::tie(o.k, o.lo, o.hi); }
+};
+
 }  // namespace
 
 // ============================================================================================
 extern "C" {
 
-const char *afsat_version(void) { return "afsat-b200 0.1 (sm_100a)"; }
+const char *afsat_version(void) { return "afsat-b200 0.2 (sm_100a)"; }
 
 const char *afsat_last_error(const afsat_ctx *ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
 
@@ -529,26 +681,50 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
                  const int8_t *lit_sign, const uint8_t *type, const int32_t *param, const int8_t *fixed,
                  int32_t batch, int64_t ldb, int32_t dtype, int32_t device, uint32_t flags)
 {
+    afsat_options opt;
+    memset(&opt, 0, sizeof opt);
+    opt.struct_size = sizeof opt;
+    opt.flags = flags;
+    return afsat_create_ex(out, n_vars, n_cons, row_ptr, lit_var, lit_sign, type, param, fixed, batch, ldb, dtype, device, &opt);
+}
+
+int afsat_create_ex(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t *row_ptr, const int32_t *lit_var,
+                    const int8_t *lit_sign, const uint8_t *type, const int32_t *param, const int8_t *fixed,
+                    int32_t batch, int64_t ldb, int32_t dtype, int32_t device, const afsat_options *opt_in)
+{
     afsat_ctx *ctx = nullptr;   // errors before allocation go to the thread-local message
     if (!out) return fail(ctx, AFSAT_E_INVALID, "out is NULL");
     *out = nullptr;
+    afsat_options opt;
+    memset(&opt, 0, sizeof opt);
+    if (opt_in) {
+        if (opt_in->struct_size < 8 || opt_in->struct_size > sizeof opt) return fail(ctx, AFSAT_E_INVALID, "afsat_options.struct_size");
+        memcpy(&opt, opt_in, opt_in->struct_size);
+    }
+    const uint32_t flags = opt.flags;
+    const int G = opt.n_groups <= 0 ? 1 : opt.n_groups;
     if (n_vars < 1 || n_vars > LIT_VAR) return fail(ctx, AFSAT_E_INVALID, "n_vars out of range");
     if (n_cons < 0) return fail(ctx, AFSAT_E_INVALID, "n_cons < 0");
     if (!row_ptr || (n_cons > 0 && (!type || !param))) return fail(ctx, AFSAT_E_INVALID, "NULL constraint arrays");
     if (batch < 1) return fail(ctx, AFSAT_E_INVALID, "batch must be >= 1");
     if (ldb < batch || ldb % 32 != 0) return fail(ctx, AFSAT_E_INVALID, "ldb must be >= batch and a multiple of 32");
     if (dtype != 32 && dtype != 64) return fail(ctx, AFSAT_E_INVALID, "dtype must be 32 or 64");
-    if (flags & ~(uint32_t)AFSAT_FLAG_ROBUST) return fail(ctx, AFSAT_E_INVALID, "unknown flags");
+    if (flags & ~(uint32_t)(AFSAT_FLAG_ROBUST | AFSAT_FLAG_PAPER)) return fail(ctx, AFSAT_E_INVALID, "unknown flags");
+    if ((flags & AFSAT_FLAG_ROBUST) && (flags & AFSAT_FLAG_PAPER)) return fail(ctx, AFSAT_E_INVALID, "AFSAT_FLAG_ROBUST and AFSAT_FLAG_PAPER exclude each other");
+    if (G > 1 && (!fixed || batch % (32 * G) != 0))
+        return fail(ctx, AFSAT_E_INVALID, "n_groups > 1 needs fixed[n_groups][n_vars] and batch % (32 n_groups) == 0");
+    if (opt.tile_w < 0 || opt.tile_w % 32 != 0) return fail(ctx, AFSAT_E_INVALID, "tile_w must be a multiple of 32");
+    if (opt.l2_budget_bytes < 0) return fail(ctx, AFSAT_E_INVALID, "l2_budget_bytes < 0");
+    if (opt.step_path < AFSAT_STEP_AUTO || opt.step_path > AFSAT_STEP_GRAPH) return fail(ctx, AFSAT_E_INVALID, "unknown step_path");
     if (row_ptr[0] != 0) return fail(ctx, AFSAT_E_INVALID, "row_ptr[0] != 0");
     const int64_t nnz = row_ptr[n_cons];
     if (nnz > 0 && (!lit_var || !lit_sign)) return fail(ctx, AFSAT_E_INVALID, "NULL literal arrays");
     if (fixed)
-        for (int32_t v = 0; v < n_vars; ++v)
+        for (int64_t v = 0; v < (int64_t)G * n_vars; ++v)
             if (fixed[v] < -1 || fixed[v] > 1) return fail(ctx, AFSAT_E_SIGN, "fixed[] must be -1, 0 or +1");
 
-    // ---- validate constraints, assign signatures -------------------------------------------
-    std::map<std::tuple<int, int, int>, int> sig_id;            // (k, type, param) -> id, ordered by k
-    std::vector<int32_t> csig(n_cons);
+    // ---- validate constraints ------------------------------------------------------------------
+    std::vector<int32_t> cprm(n_cons);
     std::vector<int32_t> scratch;
     for (int32_t c = 0; c < n_cons; ++c) {
         const int64_t lo = row_ptr[c], hi = row_ptr[c + 1];
@@ -566,6 +742,7 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
             snprintf(buf, sizeof buf, "constraint %d: parameter %d outside [0,%lld]", c, prm, (long long)k);
             return fail(ctx, AFSAT_E_PARAM, buf);
         }
+        cprm[c] = prm;
         scratch.assign(lit_var + lo, lit_var + hi);
         for (int64_t q = lo; q < hi; ++q) {
             if (lit_var[q] < 0 || lit_var[q] >= n_vars) { snprintf(buf, sizeof buf, "constraint %d: variable %d out of range", c, lit_var[q]); return fail(ctx, AFSAT_E_VARIABLE, buf); }
@@ -576,19 +753,65 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
             snprintf(buf, sizeof buf, "constraint %d repeats a variable", c);
             return fail(ctx, AFSAT_E_DUPLICATE, buf);
         }
-        auto key = std::make_tuple((int)k, (int)type[c], prm);
-        auto it = sig_id.find(key);
-        if (it == sig_id.end()) it = sig_id.emplace(key, 0).first;
-        (void)it;
     }
-    {   // ids in (k, type, param) order so that a bucket's signatures are contiguous
+
+    // ---- device (everything above is reported even without one) ----------------------------------------
+    int sm_count = 148;
+    int64_t l2_bytes = (int64_t)126 << 20;
+    {
+        int ndev = 0;
+        cudaError_t e = cudaGetDeviceCount(&ndev);
+        if (e != cudaSuccess || ndev <= 0 || device < 0 || device >= ndev)
+            return fail(nullptr, AFSAT_E_CUDA, std::string("no usable CUDA device ") + std::to_string(device) + " (" +
+                        (e != cudaSuccess ? cudaGetErrorString(e) : "device count 0 or ordinal out of range") +
+                        "); this library has no CPU fallback");
+        cudaDeviceProp prop;
+        e = cudaSetDevice(device);
+        if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, device);
+        if (e != cudaSuccess) return fail(nullptr, AFSAT_E_CUDA, std::string("cudaGetDeviceProperties: ") + cudaGetErrorString(e));
+        sm_count = prop.multiProcessorCount;
+        if (prop.l2CacheSize > 0) l2_bytes = prop.l2CacheSize;
+    }
+
+    // ---- substitute every partial assignment: constraint -> (k', truth table on the free literals) or a constant ----
+    const int64_t group_w = G > 1 ? batch / G : ldb;
+    std::map<SigKey, int> sig_id;                                // ordered by k' so that a length's signatures are contiguous
+    struct Sub { SigKey key; bool live; };
+    std::vector<std::vector<Sub>> subs(G, std::vector<Sub>(n_cons));
+    std::vector<GroupPlan> groups(G);
+    for (int g = 0; g < G; ++g) {
+        const int8_t *fx = fixed ? fixed + (size_t)g * n_vars : nullptr;
+        GroupPlan &gp = groups[g];
+        gp.b0 = g * group_w; gp.b1 = G > 1 ? (g + 1) * group_w : batch;
+        for (int32_t c = 0; c < n_cons; ++c) {
+            const int k = (int)(row_ptr[c + 1] - row_ptr[c]);
+            int fT = 0, kf = 0;                                        // fixed-true literals, free literals
+            for (int64_t q = row_ptr[c]; q < row_ptr[c + 1]; ++q) {
+                const int f = fx ? fx[lit_var[q]] : 0;
+                if (!f) ++kf;
+                else if ((f < 0) == (lit_sign[q] > 0)) ++fT;          // variable True and literal positive, or False and negated
+            }
+            SigKey key{kf, 0, 0};
+            int nsat = 0;
+            for (int tau = 0; tau <= kf; ++tau)
+                if (afsat_sig_satisfied(type[c], k, cprm[c], tau + fT)) {
+                    ++nsat;
+                    if (tau < 64) key.lo |= 1ull << tau; else key.hi |= 1ull << (tau - 64);
+                }
+            Sub &s = subs[g][c];
+            s.key = key;
+            s.live = nsat != 0 && nsat != kf + 1;
+            if (!s.live) {                                             // decided by the partial assignment (or trivial): FE = -1 / +1
+                if (nsat) { ++gp.sat_const; gp.F_const -= 1.0; } else gp.F_const += 1.0;
+            } else {
+                sig_id.emplace(key, 0);
+                ++gp.m_live; gp.nnz += kf; gp.kmax = std::max(gp.kmax, kf);
+            }
+        }
+    }
+    {
         int id = 0;
         for (auto &kv : sig_id) kv.second = id++;
-    }
-    for (int32_t c = 0; c < n_cons; ++c) {
-        const int k = (int)(row_ptr[c + 1] - row_ptr[c]);
-        int prm = (type[c] == AFSAT_OR || type[c] == AFSAT_NAE) ? 0 : param[c];
-        csig[c] = sig_id[std::make_tuple(k, (int)type[c], prm)];
     }
 
     // ---- host tables per signature -----------------------------------------------------------
@@ -596,17 +819,19 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
     std::vector<SigDev> sigs(n_sigs);
     std::vector<double> rows;
     std::vector<float> rows2;
-    std::vector<int> sig_k(n_sigs), sig_cost(n_sigs);
+    std::vector<int> sig_k(n_sigs);
+    std::vector<int64_t> sig_cost(n_sigs), sig_flop(n_sigs);
     for (auto &kv : sig_id) {
         AfsatSigHost hs;
-        int rc = afsat_sig_build(std::get<1>(kv.first), std::get<0>(kv.first), std::get<2>(kv.first), flags, &hs);
+        const int kk = kv.first.k;
+        const bool robust = (flags & AFSAT_FLAG_ROBUST) || (!(flags & AFSAT_FLAG_PAPER) && dtype == 32 && kk >= ROBUST_FROM_K32);
+        int rc = afsat_sig_build_mask(kk, kv.first.lo, kv.first.hi, robust ? AFSAT_FLAG_ROBUST : 0u, &hs);
         if (rc) return fail(ctx, rc, "signature table construction failed");
         SigDev &d = sigs[kv.second];
         memset(&d, 0, sizeof d);
         d.row_off = (int32_t)(rows.size() / 8);
         d.n_real = (int16_t)hs.n_real; d.n_cplx = (int16_t)hs.n_cplx;
         {   // discrete check scans the smaller of {satisfied, violated} counts (k_check_bits)
-            const int kk = hs.k;
             auto mask_upto = [](int nbits) { return nbits >= 64 ? ~0ull : ((1ull << nbits) - 1ull); };
             const uint64_t full_lo = mask_upto(std::min(kk + 1, 64)), full_hi = kk + 1 > 64 ? mask_upto(kk + 1 - 64) : 0ull;
             const int nsat = __builtin_popcountll(hs.satmask_lo) + __builtin_popcountll(hs.satmask_hi);
@@ -615,93 +840,51 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
             d.k = kk;
         }
         rows.insert(rows.end(), hs.rows, hs.rows + 8 * (hs.n_real + hs.n_cplx));
-        if (dtype == 32 && hs.k <= 8) {                                // staged table of the packed kernel (k <= 8)
+        if (dtype == 32 && kk <= AFSAT_A_KMAX) {                       // staged table of the packed kernel (k <= 8)
             float r32[8 * AFSAT_MAX_POINTS], packed[AFSAT_PACK_MAX_ROWS * ROW2];
             for (int i = 0; i < 8 * (hs.n_real + hs.n_cplx); ++i) r32[i] = (float)hs.rows[i];
             int uv = 0, nu = 0, ng = 0;
-            const int nrows2 = pack_rows_f2(r32, hs.n_real, hs.n_cplx, hs.k, packed, &uv, &nu, &ng);
+            const int nrows2 = pack_rows_f2(r32, hs.n_real, hs.n_cplx, kk, packed, &uv, &nu, &ng);
             d.row2_off = (int32_t)(rows2.size() / ROW2);
             d.uv = (int8_t)uv; d.n_unit = (int8_t)nu; d.n_gen = (int8_t)ng;
             rows2.insert(rows2.end(), packed, packed + (size_t)nrows2 * ROW2);
         }
-        sig_k[kv.second] = hs.k;
-        sig_cost[kv.second] = (int)cost_of(hs.k, hs.n_real, hs.n_cplx);
-    }
-
-    // ---- bucket order: constraints sorted by (k, signature), stable ----------------------------
-    std::vector<int32_t> order(n_cons);
-    for (int32_t c = 0; c < n_cons; ++c) order[c] = c;
-    std::stable_sort(order.begin(), order.end(), [&](int32_t a, int32_t b) { return csig[a] < csig[b]; });
-    std::vector<int32_t> lits((size_t)nnz), cons_sig(n_cons);
-    std::vector<int64_t> lit_off(n_cons + 1, 0);
-    int64_t total_cost = 0;
-    {
-        int64_t w = 0;
-        for (int32_t j = 0; j < n_cons; ++j) {
-            const int32_t c = order[j];
-            cons_sig[j] = csig[c];
-            lit_off[j] = w;
-            total_cost += sig_cost[csig[c]];
-            for (int64_t q = row_ptr[c]; q < row_ptr[c + 1]; ++q) {
-                int32_t v = lit_var[q];
-                int neg = lit_sign[q] < 0;
-                int32_t packed = v;
-                if (fixed && fixed[v] != 0) { packed |= LIT_FIXED; neg ^= (fixed[v] < 0); }   // y = sign * (+-1)
-                if (neg) packed |= LIT_NEG;
-                lits[w++] = packed;
-            }
-        }
-        lit_off[n_cons] = w;
+        sig_k[kv.second] = kk;
+        // the model counts every DFT point l < H of the constraint as it stands after substitution (R = 1 + [k odd] real)
+        const int R = 1 + (kk & 1), Cc = (kk + 1) / 2 + 1 - R;
+        sig_cost[kv.second] = cost_of(kk, R, Cc);
+        sig_flop[kv.second] = flop_of(kk, R, Cc);
     }
 
     // ---- candidate tile: X tile + G tile must stay L2-resident ------------
     const size_t esz = dtype == 32 ? 4 : 8;
-    int64_t tile_w = ldb;
+    const int64_t span = G > 1 ? group_w : ldb;                        // columns a tile sequence has to cover
+    int64_t tile_w = span;
     {
-        int64_t budget = (int64_t)104 << 20;                           // bytes of L2 for the X and G tiles (126 MB L2)
-        if (const char *e = getenv("AFSAT_L2_TILE_BYTES")) { long long v = atoll(e); if (v > 0) budget = v; }
+        const int64_t budget = opt.l2_budget_bytes > 0 ? opt.l2_budget_bytes : l2_bytes / 16 * 13;   // X and G tiles: 13/16 of L2
         const int64_t per_col = (int64_t)2 * n_vars * (int64_t)esz;
         // a working set within a few budgets is better left whole: the L2 misses hide behind the arithmetic, the small
         // grids of the tiles do not (cfg2 fp32, 1.58 x: 1.23 ms un-tiled vs 1.31; cfg2 fp64, 3.15 x: 2.75 vs 3.13;
         // DESIGN.md 6.5).  Beyond: equal tiles (no small remainder tile) of at most budget / per_col columns.
         if (per_col * ldb > 4 * budget) {
             const int64_t tile_max = std::max<int64_t>(64, budget / per_col / 64 * 64);
-            const int64_t n_tiles = (ldb + tile_max - 1) / tile_max;
-            tile_w = ((ldb + n_tiles - 1) / n_tiles + 63) / 64 * 64;
+            const int64_t n_tiles = (span + tile_max - 1) / tile_max;
+            tile_w = ((span + n_tiles - 1) / n_tiles + 63) / 64 * 64;
         }
-        if (const char *e = getenv("AFSAT_TILE_W")) { long long v = atoll(e); if (v >= 32 && v % 32 == 0) tile_w = v; }
-        tile_w = std::min<int64_t>(tile_w, ldb);
+        if (opt.tile_w > 0) tile_w = opt.tile_w;
+        tile_w = std::max<int64_t>(32, std::min<int64_t>(tile_w, span));
     }
 
     // ---- class geometry ---------------------------------------------------------------------------------
-    int sm_count = 148;
     ClassGeom geom[N_CLS];
-    int kmax_long = 0;
-    for (int32_t j = 0; j < n_cons; ++j) { const int k = sig_k[cons_sig[j]]; if (class_of(k, dtype) == CLS_LONG) kmax_long = std::max(kmax_long, k); }
     for (int cls = 0; cls < N_CLS; ++cls) {
         ClassGeom &g = geom[cls];
-        g.V = (cls == CLS_S) ? 4 : (cls == CLS_A && dtype == 32) ? AFSAT_A_V : 1;
+        g.V = (cls == CLS_S) ? 4 : (cls == CLS_A && dtype == 32) ? 2 : 1;
         g.warps = CTA_WARPS;
         g.cw = 32 * g.V;
-#if AFSAT_M32_PACKED
-        if (cls == CLS_B && dtype == 32) {                             // packed lane-split kernel: 2 lanes x 2 candidates
-            g.warps = AFSAT_M32_THREADS / 32;
-            g.cw = 32;
-        } else
-#endif
-        if (cls == CLS_LONG && dtype == 32) {                          // lane-split kernel: NS lanes per candidate
-            g.warps = AFSAT_L32_THREADS / 32;
-            g.cw = 32 / AFSAT_L32_NS;
-#if AFSAT_L64_SPLIT
-        } else if (cls == CLS_LONG) {                                  // fp64: four lanes per candidate
-            g.warps = AFSAT_L64_THREADS / 32;
-            g.cw = 8;
-#endif
-        } else if (cls == CLS_LONG) {
-            const int km = long_kmax(kmax_long);
-            g.warps = LONG_THREADS / 32;
-            g.smem = (size_t)g.warps * (km + 2 * (km / LB)) * 32 * esz; // per warp: values [KMAX][32] + boundaries [2 KMAX/LB][32]
-        }
+        if (cls == CLS_B && dtype == 32) { g.warps = AFSAT_M32_THREADS / 32; g.cw = 32; }                 // 2 lanes x 2 candidates
+        else if (cls == CLS_LONG && dtype == 32) { g.warps = AFSAT_L32_THREADS / 32; g.cw = 32 / AFSAT_L32_NS; }
+        else if (cls == CLS_LONG) { g.warps = AFSAT_L64_THREADS / 32; g.cw = 8; }                         // fp64: four lanes per candidate
         const int64_t cw = g.cw;
         g.Wc = std::min(g.warps, pow2_floor(std::max<int64_t>(1, (tile_w + cw - 1) / cw)));
         if ((int64_t)g.Wc * cw < tile_w && g.Wc < g.warps && (int64_t)g.Wc * cw * 2 <= tile_w + cw - 1) g.Wc *= 2;
@@ -709,50 +892,78 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
         g.Wk = g.warps / g.Wc;
     }
 
-    // ---- work items: chunks of ONE signature, sized by the cost model and by the literal staging buffer ----
-    std::vector<Item> items;
-    int32_t cls_begin[N_CLS + 1] = {0};
-    int n_buckets = 0;
-    {
+    // ---- per group: bucket order, packed literals, work items ------------------------------------------------------
+    std::vector<std::vector<int32_t>> g_lits(G);
+    std::vector<std::vector<Item>> g_items(G);
+    int n_buckets = 0, max_items = 1;
+    for (int g = 0; g < G; ++g) {
+        const int8_t *fx = fixed ? fixed + (size_t)g * n_vars : nullptr;
+        GroupPlan &gp = groups[g];
+        std::vector<int32_t> order;
+        order.reserve(gp.m_live);
+        std::vector<int32_t> csig(n_cons, -1);
+        for (int32_t c = 0; c < n_cons; ++c)
+            if (subs[g][c].live) { csig[c] = sig_id[subs[g][c].key]; order.push_back(c); }
+        std::stable_sort(order.begin(), order.end(), [&](int32_t a, int32_t b) { return csig[a] < csig[b]; });
+        std::vector<int32_t> &lits = g_lits[g];
+        lits.resize((size_t)gp.nnz);
+        std::vector<int64_t> lit_off(order.size() + 1, 0);
+        std::vector<int32_t> cons_sig(order.size());
+        int64_t w = 0;
+        for (size_t j = 0; j < order.size(); ++j) {
+            const int32_t c = order[j];
+            cons_sig[j] = csig[c];
+            lit_off[j] = w;
+            gp.fp_instr += sig_cost[csig[c]]; gp.flop += sig_flop[csig[c]];
+            for (int64_t q = row_ptr[c]; q < row_ptr[c + 1]; ++q) {
+                const int32_t v = lit_var[q];
+                if (fx && fx[v]) continue;                             // substituted
+                lits[w++] = v | (lit_sign[q] < 0 ? LIT_NEG : 0);
+            }
+        }
+        lit_off[order.size()] = w;
+        // work items: chunks of ONE signature, sized by the cost model and by the literal staging buffer
+        std::vector<Item> &items = g_items[g];
+        const int32_t nc = (int32_t)order.size();
         int32_t j = 0;
         int cur_cls = 0, last_k = -1;
-        while (j < n_cons) {
+        while (j < nc) {
             const int sg = cons_sig[j];
             const int k = sig_k[sg];
             int32_t e = j;
-            while (e < n_cons && cons_sig[e] == sg) ++e;
-            if (k != last_k) { ++n_buckets; last_k = k; }
+            while (e < nc && cons_sig[e] == sg) ++e;
+            if (g == 0 && k != last_k) { ++n_buckets; last_k = k; }
             const int cls = class_of(k, dtype);
-            while (cur_cls < cls) cls_begin[++cur_cls] = (int32_t)items.size();
-            const ClassGeom &g = geom[cls];
-            const int64_t tiles_y = (tile_w + (int64_t)g.cw * g.Wc - 1) / ((int64_t)g.cw * g.Wc);
-            const int64_t chunks_wanted = std::max<int64_t>(1, (int64_t)148 * 16 / tiles_y);
-            const int64_t cost_budget = std::max<int64_t>(1, total_cost / chunks_wanted);
+            while (cur_cls < cls) gp.cls_begin[++cur_cls] = (int32_t)items.size();
+            const ClassGeom &cg = geom[cls];
+            const int64_t tiles_y = (tile_w + (int64_t)cg.cw * cg.Wc - 1) / ((int64_t)cg.cw * cg.Wc);
+            const int64_t chunks_wanted = std::max<int64_t>(1, (int64_t)sm_count * 16 / tiles_y);
+            const int64_t cost_budget = std::max<int64_t>(1, gp.fp_instr / chunks_wanted);
             const int64_t cost1 = std::max<int64_t>(1, sig_cost[sg]);
-            int64_t chunk = std::max<int64_t>(g.Wk, (cost_budget + cost1 - 1) / cost1);
-            chunk = std::min<int64_t>(chunk, (cls == CLS_LONG && dtype == 64 ? LONG_LIT_CHUNK : LIT_CHUNK) / k);
+            int64_t chunk = std::max<int64_t>(cg.Wk, (cost_budget + cost1 - 1) / cost1);
+            chunk = std::min<int64_t>(chunk, LIT_CHUNK / k);
             chunk = std::max<int64_t>(1, chunk);
-            for (int32_t s = j; s < e; s += (int32_t)chunk) {
+            for (int32_t s0 = j; s0 < e; s0 += (int32_t)chunk) {
                 Item it;
-                it.k = k; it.sig = sg; it.c_begin = s; it.c_end = (int32_t)std::min<int64_t>(e, s + chunk);
-                it.lit_base = lit_off[s];
-                it.has_fixed = 0; it.pad = 0;
-                for (int64_t q = lit_off[s]; q < lit_off[it.c_end]; ++q) if (lits[q] & LIT_FIXED) { it.has_fixed = 1; break; }
+                it.k = k; it.sig = sg; it.c_begin = s0; it.c_end = (int32_t)std::min<int64_t>(e, s0 + chunk);
+                it.lit_base = lit_off[s0];
+                it.pad0 = it.pad1 = 0;
                 items.push_back(it);
             }
             j = e;
         }
-        while (cur_cls < N_CLS) cls_begin[++cur_cls] = (int32_t)items.size();
+        while (cur_cls < N_CLS) gp.cls_begin[++cur_cls] = (int32_t)items.size();
+        gp.n_items = (int32_t)items.size();
+        max_items = std::max(max_items, gp.n_items);
     }
 
     // ---- device ----------------------------------------------------------------------------------
     ctx = new (std::nothrow) afsat_ctx;
     if (!ctx) return fail(nullptr, AFSAT_E_NOMEM, "out of host memory");
     ctx->n = n_vars; ctx->m = n_cons; ctx->B = batch; ctx->ldb = ldb; ctx->dtype = dtype; ctx->device = device;
-    ctx->flags = flags; ctx->esz = dtype == 32 ? 4 : 8; ctx->nnz = nnz; ctx->n_sigs = n_sigs; ctx->n_buckets = n_buckets;
-    ctx->n_items = (int32_t)items.size(); ctx->kmax_long = kmax_long; ctx->fp_instr_per_candidate = total_cost;
-    ctx->tile_w = tile_w;
-    memcpy(ctx->cls_begin, cls_begin, sizeof cls_begin);
+    ctx->flags = flags; ctx->esz = esz; ctx->nnz = nnz; ctx->n_sigs = n_sigs; ctx->n_buckets = n_buckets;
+    ctx->tile_w = tile_w; ctx->group_w = group_w; ctx->sm_count = sm_count; ctx->l2_bytes = l2_bytes; ctx->max_items = max_items;
+    ctx->groups = groups;
     for (int cls = 0; cls < N_CLS; ++cls) ctx->geom[cls] = geom[cls];
 
 #define CREATE_FAIL(rc_)                                   \
@@ -761,26 +972,12 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
         if (r2_) { g_create_error = ctx->err; afsat_destroy(ctx); return r2_; } \
     } while (0)
 
-    {
-        int ndev = 0;
-        cudaError_t e = cudaGetDeviceCount(&ndev);
-        if (e != cudaSuccess || ndev <= 0 || device < 0 || device >= ndev) {
-            std::string msg = std::string("no usable CUDA device ") + std::to_string(device) + " (" +
-                              (e != cudaSuccess ? cudaGetErrorString(e) : "device count 0 or ordinal out of range") +
-                              "); this library has no CPU fallback";
-            ctx->err = msg;
-            CREATE_FAIL(AFSAT_E_CUDA);
-        }
-    }
     CREATE_FAIL(set_device(ctx));
-    {
-        cudaDeviceProp prop;
-        if (cudaGetDeviceProperties(&prop, device) == cudaSuccess) sm_count = prop.multiProcessorCount;
-        ctx->sm_count = sm_count;
+    for (int g = 0; g < G; ++g) {
+        CREATE_FAIL(upload(ctx, &ctx->groups[g].d_lits, g_lits[g]));
+        CREATE_FAIL(upload(ctx, &ctx->groups[g].d_items, g_items[g]));
     }
-    CREATE_FAIL(upload(ctx, &ctx->d_lits, lits));
     CREATE_FAIL(upload(ctx, &ctx->d_sigs, sigs));
-    CREATE_FAIL(upload(ctx, &ctx->d_items, items));
     if (dtype == 32) {
         std::vector<float> r32(rows.begin(), rows.end());
         float *p = nullptr;
@@ -793,20 +990,23 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
         ctx->d_rows = p;
     }
     {
-        std::vector<int8_t> fx(n_vars, 0);
-        if (fixed) memcpy(fx.data(), fixed, n_vars);
+        std::vector<int8_t> fx((size_t)G * n_vars, 0);
+        if (fixed) memcpy(fx.data(), fixed, fx.size());
         CREATE_FAIL(upload(ctx, &ctx->d_fixed, fx));
+        std::vector<int32_t> sc(G);
+        for (int g = 0; g < G; ++g) sc[g] = groups[g].sat_const;
+        CREATE_FAIL(upload(ctx, &ctx->d_sat_const, sc));
     }
     {
         char *g = nullptr, *fp = nullptr;
-        CREATE_FAIL(dev_alloc(ctx, &g, (size_t)n_vars * tile_w * ctx->esz, true));
+        CREATE_FAIL(dev_alloc(ctx, &g, (size_t)n_vars * tile_w * esz, true));
         ctx->d_G = g;
-        CREATE_FAIL(dev_alloc(ctx, &fp, (size_t)std::max<int>(1, ctx->n_items) * ldb * ctx->esz, true));
+        CREATE_FAIL(dev_alloc(ctx, &fp, (size_t)max_items * ldb * esz, true));
         ctx->d_Fpart = fp;
     }
     CREATE_FAIL(dev_alloc(ctx, &ctx->d_bits, (size_t)n_vars * (size_t)(ldb / 32), true));
     CREATE_FAIL(dev_alloc(ctx, &ctx->d_satacc, (size_t)ldb, true));
-    CREATE_FAIL(dev_alloc(ctx, &ctx->d_any, 2, true));
+    CREATE_FAIL(dev_alloc(ctx, &ctx->d_any, 4, true));
     {
         cudaError_t e = cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking);
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming);
@@ -815,6 +1015,37 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
             if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_join[i], cudaEventDisableTiming);
         }
         if (e != cudaSuccess) { ctx->err = cudaGetErrorString(e); CREATE_FAIL(AFSAT_E_CUDA); }
+    }
+
+    // ---- how afsat_step runs its loop ------------------------------------------------------------------------------------
+    {
+        // PERSISTENT needs: one group, every length <= 8, X and G of 32 candidates in shared memory
+        const size_t smem = (size_t)2 * n_vars * 32 * esz;
+        int dev_smem = 0;
+        cudaDeviceGetAttribute(&dev_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
+        const bool fits = G == 1 && groups[0].kmax <= AFSAT_A_KMAX && smem + 1024 <= (size_t)dev_smem;
+        // launch-bound when one iteration's arithmetic is shorter than its launches (~2.5 us each): model instructions
+        // over the FP32 issue rate of the whole chip at ~1.9 GHz
+        const double est_us = (double)groups[0].fp_instr * batch / ((double)sm_count * 128 * 1.9e3);
+        int path = opt.step_path;
+        if (path == AFSAT_STEP_PERSISTENT && !fits) {
+            ctx->err = "AFSAT_STEP_PERSISTENT: the instance does not fit (one group, every length <= 8, 2 n 32 elements of shared memory)";
+            CREATE_FAIL(AFSAT_E_INVALID);
+        }
+        if (path == AFSAT_STEP_AUTO) {
+            const int64_t tiles = (span + tile_w - 1) / tile_w * G;
+            path = (fits && est_us < 8.0 && batch <= 32 * sm_count) ? AFSAT_STEP_PERSISTENT
+                 : (est_us < 60.0 && tiles <= 8)                      ? AFSAT_STEP_GRAPH
+                                                                      : AFSAT_STEP_LAUNCHES;
+        }
+        ctx->step_path = path;
+        if (fits) {
+            ctx->small_smem = smem;
+            cudaError_t e = dtype == 32
+                ? cudaFuncSetAttribute(k_step_small<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)
+                : cudaFuncSetAttribute(k_step_small<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) { ctx->err = std::string("cudaFuncSetAttribute(k_step_small): ") + cudaGetErrorString(e); CREATE_FAIL(AFSAT_E_CUDA); }
+        }
     }
     *out = ctx;
     return AFSAT_OK;
@@ -833,12 +1064,18 @@ void afsat_destroy(afsat_ctx *ctx)
 {
     if (!ctx) return;
     prof_drain(ctx, false);
-    cudaFree(ctx->d_lits); cudaFree(ctx->d_bits); cudaFree(ctx->d_sigs); cudaFree(ctx->d_rows); cudaFree(ctx->d_rows2);
-    cudaFree(ctx->d_fixed); cudaFree(ctx->d_items); cudaFree(ctx->d_G); cudaFree(ctx->d_Fpart);
+    if (ctx->graph.exec) cudaGraphExecDestroy(ctx->graph.exec);
+    for (GroupPlan &gp : ctx->groups) { cudaFree(gp.d_lits); cudaFree(gp.d_items); }
+    cudaFree(ctx->d_bits); cudaFree(ctx->d_sigs); cudaFree(ctx->d_rows); cudaFree(ctx->d_rows2);
+    cudaFree(ctx->d_fixed); cudaFree(ctx->d_sat_const); cudaFree(ctx->d_G); cudaFree(ctx->d_Fpart);
     cudaFree(ctx->d_satacc); cudaFree(ctx->d_any);
     cudaFree(ctx->ls_G); cudaFree(ctx->ls_xt); cudaFree(ctx->ls_F0); cudaFree(ctx->ls_F1); cudaFree(ctx->ls_Dpart);
     cudaFree(ctx->ls_eta); cudaFree(ctx->ls_state);
-    cudaFree(ctx->dh_x); cudaFree(ctx->dh_F); cudaFree(ctx->dh_sat); cudaFree(ctx->dh_first); cudaFree(ctx->dh_sol);
+    cudaFree(ctx->dh_x); cudaFree(ctx->dh_F); cudaFree(ctx->dh_Fpre); cudaFree(ctx->dh_sat); cudaFree(ctx->dh_first); cudaFree(ctx->dh_sol);
+    for (cudaEvent_t e : ctx->chunk_in) cudaEventDestroy(e);
+    for (cudaEvent_t e : ctx->chunk_done) cudaEventDestroy(e);
+    if (ctx->in_stream) cudaStreamDestroy(ctx->in_stream);
+    if (ctx->out_stream) cudaStreamDestroy(ctx->out_stream);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
     for (int i = 0; i < N_CLS - 1; ++i) {
         if (ctx->side_stream[i]) cudaStreamDestroy(ctx->side_stream[i]);
@@ -852,6 +1089,7 @@ int afsat_eval_grad(afsat_ctx *ctx, const void *d_x, void *d_F, void *d_G, void 
 {
     if (!ctx) return AFSAT_E_INVALID;
     if (!d_x || (!d_F && !d_G)) return fail(ctx, AFSAT_E_INVALID, "afsat_eval_grad: NULL pointer");
+    if (misaligned(d_x) || misaligned(d_G)) return fail(ctx, AFSAT_E_INVALID, "afsat_eval_grad: d_x / d_G must be 16-byte aligned");
     int rc = set_device(ctx);
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
@@ -863,36 +1101,35 @@ int afsat_check(afsat_ctx *ctx, const void *d_x, int32_t *d_sat_count, uint8_t *
 {
     if (!ctx) return AFSAT_E_INVALID;
     if (!d_x || !d_sat_count || !d_is_solution) return fail(ctx, AFSAT_E_INVALID, "afsat_check: NULL pointer");
+    if (misaligned(d_x)) return fail(ctx, AFSAT_E_INVALID, "afsat_check: d_x must be 16-byte aligned");
     int rc = set_device(ctx);
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     rc = ctx->dtype == 32 ? launch_pack<float>(ctx, (const float *)d_x, st) : launch_pack<double>(ctx, (const double *)d_x, st);
-    if (!rc) rc = launch_check_bits(ctx, 0, ctx->ldb / 32, st);
+    if (!rc) rc = check_all(ctx, false, st);
     if (rc) return rc;
-    k_check_finish<<<(ctx->B + 127) / 128, 128, 0, st>>>(ctx->d_satacc, ctx->B, ctx->m, d_sat_count, d_is_solution);
+    k_check_finish<<<(ctx->B + 127) / 128, 128, 0, st>>>(ctx->d_satacc, ctx->B, ctx->m, ctx->d_sat_const, ctx->group_w,
+                                                         (int)ctx->groups.size(), d_sat_count, d_is_solution);
     ++ctx->launches;
     CU(cudaPeekAtLastError());
     return AFSAT_OK;
 }
 
-int afsat_step(afsat_ctx *ctx, void *d_x, double eta, int32_t n_steps, int32_t step_base, int32_t resume, void *d_F,
+int afsat_step(afsat_ctx *ctx, void *d_x, double eta, int32_t n_steps, int32_t step_base, int32_t resume, void *d_F, void *d_F_pre,
                int32_t *d_sat_count, uint8_t *d_is_solution, int32_t *d_first_step, int32_t *h_any_solved, void *stream)
 {
     if (!ctx) return AFSAT_E_INVALID;
     if (!d_x || !d_sat_count || !d_is_solution || !d_first_step) return fail(ctx, AFSAT_E_INVALID, "afsat_step: NULL pointer");
+    if (misaligned(d_x)) return fail(ctx, AFSAT_E_INVALID, "afsat_step: d_x must be 16-byte aligned");
     if (n_steps < 0) return fail(ctx, AFSAT_E_INVALID, "afsat_step: n_steps < 0");
     int rc = set_device(ctx);
     if (rc) return rc;
     int32_t *h_dev = nullptr;
-    if (h_any_solved) {
-        CU(cudaHostGetDevicePointer((void **)&h_dev, h_any_solved, 0));
-        h_any_solved[0] = 0;
-        h_any_solved[1] = -1;
-    }
+    if (h_any_solved) CU(cudaHostGetDevicePointer((void **)&h_dev, h_any_solved, 0));   // reset on the stream (k_reset_state)
     cudaStream_t st = (cudaStream_t)stream;
     return ctx->dtype == 32
-               ? step_t<float>(ctx, (float *)d_x, eta, n_steps, step_base, resume, (float *)d_F, d_sat_count, d_is_solution, d_first_step, h_dev, st)
-               : step_t<double>(ctx, (double *)d_x, eta, n_steps, step_base, resume, (double *)d_F, d_sat_count, d_is_solution, d_first_step, h_dev, st);
+               ? step_t<float>(ctx, (float *)d_x, eta, n_steps, step_base, resume, (float *)d_F, (float *)d_F_pre, d_sat_count, d_is_solution, d_first_step, h_dev, st)
+               : step_t<double>(ctx, (double *)d_x, eta, n_steps, step_base, resume, (double *)d_F, (double *)d_F_pre, d_sat_count, d_is_solution, d_first_step, h_dev, st);
 }
 
 int afsat_step_ls(afsat_ctx *ctx, void *d_x, double s_max, double beta, double c1, double delta, int32_t max_trials,
@@ -902,17 +1139,14 @@ int afsat_step_ls(afsat_ctx *ctx, void *d_x, double s_max, double beta, double c
     if (!ctx) return AFSAT_E_INVALID;
     if (!d_x || !d_sat_count || !d_is_solution || !d_first_step || !d_converged)
         return fail(ctx, AFSAT_E_INVALID, "afsat_step_ls: NULL pointer");
+    if (misaligned(d_x)) return fail(ctx, AFSAT_E_INVALID, "afsat_step_ls: d_x must be 16-byte aligned");
     if (n_steps < 0 || max_trials < 1) return fail(ctx, AFSAT_E_INVALID, "afsat_step_ls: n_steps < 0 or max_trials < 1");
     if (!(s_max > 0.0) || !(beta > 0.0 && beta < 1.0) || !(c1 >= 0.0 && c1 < 1.0) || !(delta >= 0.0))
         return fail(ctx, AFSAT_E_INVALID, "afsat_step_ls: need s_max > 0, 0 < beta < 1, 0 <= c1 < 1, delta >= 0");
     int rc = set_device(ctx);
     if (rc) return rc;
     int32_t *h_dev = nullptr;
-    if (h_any_solved) {
-        CU(cudaHostGetDevicePointer((void **)&h_dev, h_any_solved, 0));
-        h_any_solved[0] = 0;
-        h_any_solved[1] = -1;
-    }
+    if (h_any_solved) CU(cudaHostGetDevicePointer((void **)&h_dev, h_any_solved, 0));
     cudaStream_t st = (cudaStream_t)stream;
     return ctx->dtype == 32
                ? step_ls_t<float>(ctx, (float *)d_x, s_max, beta, c1, delta, max_trials, n_steps, step_base, resume, (float *)d_F,
@@ -925,16 +1159,18 @@ int afsat_restart(afsat_ctx *ctx, void *d_x, const uint8_t *d_keep, uint64_t see
 {
     if (!ctx) return AFSAT_E_INVALID;
     if (!d_x) return fail(ctx, AFSAT_E_INVALID, "afsat_restart: NULL pointer");
+    if (misaligned(d_x)) return fail(ctx, AFSAT_E_INVALID, "afsat_restart: d_x must be 16-byte aligned");
     int rc = set_device(ctx);
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     const unsigned gx = (unsigned)((ctx->B + CTA_THREADS - 1) / CTA_THREADS);
     const unsigned gy = (unsigned)std::min<int64_t>(ctx->n, std::max<int64_t>(1, (int64_t)ctx->sm_count * 8 / gx));
     const uint32_t lo = (uint32_t)(seed & 0xFFFFFFFFull), hi = (uint32_t)(seed >> 32);
+    const int ng = (int)ctx->groups.size();
     if (ctx->dtype == 32)
-        k_restart<float><<<dim3(gx, gy), CTA_THREADS, 0, st>>>((float *)d_x, ctx->d_fixed, d_keep, lo, hi, round, ctx->n, ctx->B, ctx->ldb);
+        k_restart<float><<<dim3(gx, gy), CTA_THREADS, 0, st>>>((float *)d_x, ctx->d_fixed, ctx->group_w, ng, d_keep, lo, hi, round, ctx->n, ctx->B, ctx->ldb);
     else
-        k_restart<double><<<dim3(gx, gy), CTA_THREADS, 0, st>>>((double *)d_x, ctx->d_fixed, d_keep, lo, hi, round, ctx->n, ctx->B, ctx->ldb);
+        k_restart<double><<<dim3(gx, gy), CTA_THREADS, 0, st>>>((double *)d_x, ctx->d_fixed, ctx->group_w, ng, d_keep, lo, hi, round, ctx->n, ctx->B, ctx->ldb);
     ++ctx->launches;
     CU(cudaPeekAtLastError());
     return AFSAT_OK;
@@ -951,7 +1187,7 @@ int afsat_solve(afsat_ctx *ctx, void *d_x, double eta, int32_t steps_per_round, 
     int r = 0;
     for (; r < max_rounds; ++r) {
         const bool last = r + 1 == max_rounds;
-        int rc = afsat_step(ctx, d_x, eta, steps_per_round, r * steps_per_round, r > 0, nullptr, d_sat_count, d_is_solution,
+        int rc = afsat_step(ctx, d_x, eta, steps_per_round, r * steps_per_round, r > 0, nullptr, nullptr, d_sat_count, d_is_solution,
                             d_first_step, nullptr, stream);
         if (rc) return rc;
         int32_t any[2] = {0, -1};
@@ -966,7 +1202,7 @@ int afsat_solve(afsat_ctx *ctx, void *d_x, double eta, int32_t steps_per_round, 
     return AFSAT_OK;
 }
 
-int afsat_step_host(afsat_ctx *ctx, void *h_x, double eta, int32_t n_steps, void *h_F, int32_t *h_sat_count,
+int afsat_step_host(afsat_ctx *ctx, void *h_x, double eta, int32_t n_steps, void *h_F, void *h_F_pre, int32_t *h_sat_count,
                     uint8_t *h_is_solution, int32_t *h_first_step)
 {
     if (!ctx) return AFSAT_E_INVALID;
@@ -976,26 +1212,47 @@ int afsat_step_host(afsat_ctx *ctx, void *h_x, double eta, int32_t n_steps, void
     if (rc) return rc;
     const size_t xb = (size_t)ctx->n * ctx->ldb * ctx->esz;
     if (!ctx->dh_x) {
-        char *px = nullptr, *pf = nullptr;
+        char *px = nullptr, *pf = nullptr, *pp = nullptr;
         if ((rc = dev_alloc(ctx, &px, xb))) return rc;
         ctx->dh_x = px;
         if ((rc = dev_alloc(ctx, &pf, (size_t)ctx->ldb * ctx->esz))) return rc;
         ctx->dh_F = pf;
+        if ((rc = dev_alloc(ctx, &pp, (size_t)ctx->ldb * ctx->esz))) return rc;
+        ctx->dh_Fpre = pp;
         if ((rc = dev_alloc(ctx, &ctx->dh_sat, (size_t)ctx->ldb))) return rc;
         if ((rc = dev_alloc(ctx, &ctx->dh_first, (size_t)ctx->ldb))) return rc;
         if ((rc = dev_alloc(ctx, &ctx->dh_sol, (size_t)ctx->ldb))) return rc;
+        CU(cudaStreamCreateWithFlags(&ctx->in_stream, cudaStreamNonBlocking));
+        CU(cudaStreamCreateWithFlags(&ctx->out_stream, cudaStreamNonBlocking));
     }
     cudaStream_t st = ctx->own_stream;
-    CU(cudaMemcpyAsync(ctx->dh_x, h_x, xb, cudaMemcpyHostToDevice, st));
-    rc = afsat_step(ctx, ctx->dh_x, eta, n_steps, 0, 0, h_F ? ctx->dh_F : nullptr, ctx->dh_sat, ctx->dh_sol, ctx->dh_first,
-                    nullptr, (void *)st);
-    if (rc) return rc;
-    CU(cudaMemcpyAsync(h_x, ctx->dh_x, xb, cudaMemcpyDeviceToHost, st));
+    const bool tiled = ctx->tile_w < (ctx->groups.size() > 1 ? ctx->group_w : ctx->ldb);
+    // one iteration, a batch wide enough to cut: copies pipelined behind the evaluation, chunk by chunk
+    const bool pipelined = n_steps == 1 && !h_F && !ctx->profiling && ctx->step_path != AFSAT_STEP_PERSISTENT &&
+                           (tiled || ctx->B >= 512);
+    if (pipelined && !tiled && !ctx->ls_G) {                          // un-tiled: a full-width gradient buffer
+        char *pg = nullptr;
+        if ((rc = dev_alloc(ctx, &pg, xb))) return rc;
+        ctx->ls_G = pg;
+    }
+    if (pipelined) {
+        rc = ctx->dtype == 32 ? step_host_pipelined<float>(ctx, (float *)h_x, eta, (float *)h_F_pre)
+                              : step_host_pipelined<double>(ctx, (double *)h_x, eta, (double *)h_F_pre);
+        if (rc) return rc;
+    } else {
+        CU(cudaMemcpyAsync(ctx->dh_x, h_x, xb, cudaMemcpyHostToDevice, st));
+        rc = afsat_step(ctx, ctx->dh_x, eta, n_steps, 0, 0, h_F ? ctx->dh_F : nullptr, (h_F_pre && n_steps > 0) ? ctx->dh_Fpre : nullptr,
+                        ctx->dh_sat, ctx->dh_sol, ctx->dh_first, nullptr, (void *)st);
+        if (rc) return rc;
+        CU(cudaMemcpyAsync(h_x, ctx->dh_x, xb, cudaMemcpyDeviceToHost, st));
+    }
     if (h_F) CU(cudaMemcpyAsync(h_F, ctx->dh_F, (size_t)ctx->B * ctx->esz, cudaMemcpyDeviceToHost, st));
+    if (h_F_pre && n_steps > 0) CU(cudaMemcpyAsync(h_F_pre, ctx->dh_Fpre, (size_t)ctx->B * ctx->esz, cudaMemcpyDeviceToHost, st));
     if (h_sat_count) CU(cudaMemcpyAsync(h_sat_count, ctx->dh_sat, (size_t)ctx->B * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
     if (h_is_solution) CU(cudaMemcpyAsync(h_is_solution, ctx->dh_sol, (size_t)ctx->B, cudaMemcpyDeviceToHost, st));
     if (h_first_step) CU(cudaMemcpyAsync(h_first_step, ctx->dh_first, (size_t)ctx->B * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
+    if (pipelined) CU(cudaStreamSynchronize(ctx->out_stream));
     return AFSAT_OK;
 }
 
@@ -1006,6 +1263,7 @@ int64_t afsat_query(const afsat_ctx *ctx, int32_t key)
         prof_drain(const_cast<afsat_ctx *>(ctx), true);
         return key == AFSAT_Q_PROFILED_EVAL_NS ? (int64_t)ctx->prof_ns : ctx->prof_launches;
     }
+    const GroupPlan &g0 = ctx->groups[0];
     switch (key) {
     case AFSAT_Q_KERNEL_LAUNCHES: return ctx->launches;
     case AFSAT_Q_NUM_SIGNATURES:  return ctx->n_sigs;
@@ -1013,9 +1271,50 @@ int64_t afsat_query(const afsat_ctx *ctx, int32_t key)
     case AFSAT_Q_NNZ:             return ctx->nnz;
     case AFSAT_Q_WORKSPACE_BYTES: return (int64_t)ctx->ws_bytes;
     case AFSAT_Q_SM_COUNT:        return ctx->sm_count;
-    case AFSAT_Q_FP_INSTR_PER_CANDIDATE: return ctx->fp_instr_per_candidate;
+    case AFSAT_Q_FP_INSTR_PER_CANDIDATE: return g0.fp_instr;
+    case AFSAT_Q_FLOP_PER_CANDIDATE: return g0.flop;
+    case AFSAT_Q_NUM_GROUPS:      return (int64_t)ctx->groups.size();
+    case AFSAT_Q_STEP_PATH:       return ctx->step_path;
+    case AFSAT_Q_TILE_W:          return ctx->tile_w;
+    case AFSAT_Q_LIVE_CONSTRAINTS: return g0.m_live;
+    case AFSAT_Q_LIVE_NNZ:        return g0.nnz;
+    case AFSAT_Q_DECIDED_SATISFIED: return g0.sat_const;
+    case AFSAT_Q_L2_BYTES:        return ctx->l2_bytes;
     default: return -1;
     }
+}
+
+int afsat_probe_peak(int32_t device, int32_t kind, double *tflops)
+{
+    afsat_ctx *ctx = nullptr;
+    if (!tflops || kind < 0 || kind > 2) return fail(ctx, AFSAT_E_INVALID, "afsat_probe_peak: bad arguments");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev)
+        return fail(ctx, AFSAT_E_CUDA, "afsat_probe_peak: no usable CUDA device (no CPU fallback)");
+    CU(cudaSetDevice(device));
+    cudaDeviceProp prop;
+    CU(cudaGetDeviceProperties(&prop, device));
+    float *d_out = nullptr;
+    CU(cudaMalloc((void **)&d_out, 64));
+    cudaEvent_t e0, e1;
+    CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1));
+    const int iters = 1 << 14, blocks = prop.multiProcessorCount * 8, threads = 256;
+    double best = 0.0;
+    for (int rep = 0; rep < 6; ++rep) {
+        CU(cudaEventRecord(e0, 0));
+        if (kind == 0) k_probe<0><<<blocks, threads>>>(d_out, iters, 1.0001f);
+        else if (kind == 1) k_probe<1><<<blocks, threads>>>(d_out, iters, 1.0001f);
+        else k_probe<2><<<blocks, threads>>>(d_out, iters, 1.0001f);
+        CU(cudaEventRecord(e1, 0));
+        CU(cudaEventSynchronize(e1));
+        float ms = 0.f;
+        CU(cudaEventElapsedTime(&ms, e0, e1));
+        const double fma = (double)blocks * threads * iters * 8.0 * (kind == 1 ? 2.0 : 1.0);
+        if (rep > 0 && ms > 0.f) best = std::max(best, 2.0 * fma / (ms * 1e-3) / 1e12);
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d_out);
+    *tflops = best;
+    return AFSAT_OK;
 }
 
 }  // extern "C"

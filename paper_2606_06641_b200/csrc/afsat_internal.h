@@ -18,5 +18,8 @@ struct AfsatSigHost {
 // Returns AFSAT_OK or AFSAT_E_*; never touches a device.
 int afsat_sig_build(int32_t type, int32_t k, int32_t param, uint32_t flags, AfsatSigHost *out);
 
+// The same for any symmetric constraint on k literals: bit tau of the mask set <=> satisfied with tau true literals.
+int afsat_sig_build_mask(int32_t k, uint64_t satmask_lo, uint64_t satmask_hi, uint32_t flags, AfsatSigHost *out);
+
 // Is the constraint satisfied with tau true literals?  (Table 1 / Table 2 semantics.)
 bool afsat_sig_satisfied(int32_t type, int32_t k, int32_t param, int32_t tau);

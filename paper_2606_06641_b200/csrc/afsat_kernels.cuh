@@ -22,9 +22,12 @@
 
 namespace afsat {
 
-constexpr int32_t LIT_NEG   = (int32_t)0x80000000u;  // y = -x (or the constant -1 when fixed)
-constexpr int32_t LIT_FIXED = 0x40000000;            // y is the constant +-1, no gradient
-constexpr int32_t LIT_VAR   = 0x3FFFFFFF;
+// packed literal: bits 0-29 variable, bit 31 negation (y = -x).  Fixed variables never reach a kernel: afsat_create
+// substitutes them into the constraints.  LIT_NONE marks a literal slot a lane does not have
+// (lane-split kernels, afsat_split.cuh).
+constexpr int32_t LIT_NEG  = (int32_t)0x80000000u;
+constexpr int32_t LIT_NONE = 0x40000000;
+constexpr int32_t LIT_VAR  = 0x3FFFFFFF;
 
 constexpr int LIT_CHUNK = 4096;       // packed literals staged in shared memory per work item
 #ifndef AFSAT_CTA_THREADS
@@ -48,7 +51,7 @@ struct Item {                   // one CTA-sized chunk of constraints of a singl
     int32_t k, sig;
     int32_t c_begin, c_end;     // constraint range in bucket order
     int64_t lit_base;           // offset of c_begin's first packed literal
-    int32_t has_fixed, pad;     // some literal of the chunk is a fixed variable
+    int32_t pad0, pad1;
 };
 
 template <typename T>
@@ -235,18 +238,6 @@ __device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b)
 constexpr int ROW2 = 12;
 #define AFSAT_PACK_MAX_ROWS 40              // >= MAX_ROWS + the zero-weight unit rows a table may get
 
-#ifndef AFSAT_F2_PAIR_POINTS
-#define AFSAT_F2_PAIR_POINTS 0
-#endif
-#ifndef AFSAT_F2_OCT_ROWS
-#define AFSAT_F2_OCT_ROWS 1
-#endif
-#ifndef AFSAT_F2_UNIT_ROWS
-#define AFSAT_F2_UNIT_ROWS 1
-#endif
-#ifndef AFSAT_F2_NEG_BY_XOR
-#define AFSAT_F2_NEG_BY_XOR 1
-#endif
 
 // HOST: the staged table of one signature for the packed kernel, from its fp32 rows {Re a, Im a, Re b, Im b,
 // Re w, Im w, Re(wb), Im(wb)} (real rows first).  Standard tables (a = 1/2 exactly in every row): the
@@ -259,11 +250,11 @@ inline int pack_rows_f2(const float *r0, int n_real, int n_cplx, int k, float *o
 {
     const int nr = n_real + n_cplx;
     int src[AFSAT_PACK_MAX_ROWS], n = 0, uv = 0, n_unit = n_real, n_gen = n_cplx, q_conj = -1;
-    bool std_tab = AFSAT_F2_UNIT_ROWS != 0;
+    bool std_tab = true;
     for (int q = 0; q < nr; ++q) std_tab = std_tab && r0[8 * q] == 0.5f && r0[8 * q + 1] == 0.f;
     if (std_tab) {
         int iP = -1, iM = -1, iI = -1, iA = -1, iB = -1;
-        const bool oct = AFSAT_F2_OCT_ROWS && (k & 7) == 7;
+        const bool oct = (k & 7) == 7;
         for (int q = 0; q < nr; ++q) {
             const float br = r0[8 * q + 2], bi = r0[8 * q + 3];
             if (q < n_real) { if (br == 0.5f) iP = q; else if (br == -0.5f) iM = q; }
@@ -302,75 +293,55 @@ inline int pack_rows_f2(const float *r0, int n_real, int n_cplx, int k, float *o
     return n;
 }
 
-// PP complex DFT points (consecutive table rows) for NP candidate pairs: prefix walk, contraction,
-// suffix walk with the leave-one-out accumulation.  All PP x NP chains are independent.
-template <int K, int NP, int PP, bool GRAD>
+// One generic complex DFT point (table row r) for NP candidate pairs: prefix walk, contraction, suffix walk with
+// the leave-one-out accumulation.  The NP chains are independent.
+template <int K, int NP, bool GRAD>
 __device__ __forceinline__ void cplx_points_f2(const f32x2 (&y)[K][NP], const f32x2 *__restrict__ r, f32x2 (&fe)[NP],
                                                f32x2 (&g)[K][NP])
 {
-    f32x2 pr[PP][K][NP], pi[PP][K][NP], fr[PP][K][NP], fi[PP][K][NP], nfi[PP][K][NP], rr[PP][NP], ri[PP][NP];
+    f32x2 pr[K][NP], pi[K][NP], fr[K][NP], fi[K][NP], nfi[K][NP], rr[NP], ri[NP];
+    // coefficients are the same for both candidates: read ONE float and let FFMA2 broadcast it
+    // (R.F32 operand) -- a true register pair would cost a third 64-bit register-file read
+    const f32x2 ar = bc(r, 0), ai = bc(r, 1), br = bc(r, 3), bi = bc(r, 4);
 #pragma unroll
-    for (int t = 0; t < PP; ++t) {
-        const f32x2 *rt = r + t * ROW2;
-        // coefficients are the same for both candidates: read ONE float and let FFMA2 broadcast it
-        // (R.F32 operand) -- a true register pair would cost a third 64-bit register-file read
-        const f32x2 ar = bc(rt, 0), ai = bc(rt, 1), nai = bc(rt, 2), br = bc(rt, 3), bi = bc(rt, 4), nbi = bc(rt, 5);
+    for (int i = 0; i < K; ++i)
 #pragma unroll
-        for (int i = 0; i < K; ++i)
+        for (int q = 0; q < NP; ++q) {
+            fr[i][q] = fma2(br, y[i][q], ar); fi[i][q] = fma2(bi, y[i][q], ai);
+            nfi[i][q] = fi[i][q] ^ 0x8000000080000000ull;             // -Im f on the ALU pipe (2 LOP3), not the FMA pipe
+        }
 #pragma unroll
-            for (int q = 0; q < NP; ++q) {
-                fr[t][i][q] = fma2(br, y[i][q], ar); fi[t][i][q] = fma2(bi, y[i][q], ai);
-#if AFSAT_F2_NEG_BY_XOR
-                nfi[t][i][q] = fi[t][i][q] ^ 0x8000000080000000ull;   // -Im f on the ALU pipe (2 LOP3), not the FMA pipe
-#else
-                nfi[t][i][q] = fma2(nbi, y[i][q], nai);
-#endif
-            }
-    }
-#pragma unroll
-    for (int t = 0; t < PP; ++t)
-#pragma unroll
-        for (int q = 0; q < NP; ++q) { rr[t][q] = fr[t][0][q]; ri[t][q] = fi[t][0][q]; }
+    for (int q = 0; q < NP; ++q) { rr[q] = fr[0][q]; ri[q] = fi[0][q]; }
 #pragma unroll
     for (int i = 1; i < K; ++i)
 #pragma unroll
-        for (int t = 0; t < PP; ++t)
-#pragma unroll
-            for (int q = 0; q < NP; ++q) {
-                pr[t][i][q] = rr[t][q]; pi[t][i][q] = ri[t][q];
-                const f32x2 nr = fma2(rr[t][q], fr[t][i][q], mul2(ri[t][q], nfi[t][i][q]));   // Re: rr fr - ri fi
-                const f32x2 ni = fma2(rr[t][q], fi[t][i][q], mul2(ri[t][q], fr[t][i][q]));    // Im: rr fi + ri fr
-                rr[t][q] = nr; ri[t][q] = ni;
-            }
-#pragma unroll
-    for (int t = 0; t < PP; ++t)
-#pragma unroll
         for (int q = 0; q < NP; ++q) {
-            fe[q] = fma2(bc(r, t * ROW2 + 6), rr[t][q], fe[q]);       // + wr Re P
-            fe[q] = fma2(bc(r, t * ROW2 + 7), ri[t][q], fe[q]);       // - wi Im P
+            pr[i][q] = rr[q]; pi[i][q] = ri[q];
+            const f32x2 nr = fma2(rr[q], fr[i][q], mul2(ri[q], nfi[i][q]));   // Re: rr fr - ri fi
+            const f32x2 ni = fma2(rr[q], fi[i][q], mul2(ri[q], fr[i][q]));    // Im: rr fi + ri fr
+            rr[q] = nr; ri[q] = ni;
         }
+#pragma unroll
+    for (int q = 0; q < NP; ++q) {
+        fe[q] = fma2(bc(r, 6), rr[q], fe[q]);                         // + wr Re P
+        fe[q] = fma2(bc(r, 7), ri[q], fe[q]);                         // - wi Im P
+    }
     if (GRAD) {
-        f32x2 sr[PP][NP], nsi[PP][NP];                                // suffix (Re s, -Im s) seeded with w b
+        f32x2 sr[NP], nsi[NP];                                        // suffix (Re s, -Im s) seeded with w b
 #pragma unroll
-        for (int t = 0; t < PP; ++t)
-#pragma unroll
-            for (int q = 0; q < NP; ++q) { sr[t][q] = r[t * ROW2 + 8]; nsi[t][q] = r[t * ROW2 + 9]; }
+        for (int q = 0; q < NP; ++q) { sr[q] = r[8]; nsi[q] = r[9]; }
 #pragma unroll
         for (int i = K - 1; i >= 1; --i)
 #pragma unroll
-            for (int t = 0; t < PP; ++t)
+            for (int q = 0; q < NP; ++q) {
+                g[i][q] = fma2(pr[i][q], sr[q], g[i][q]);             // Re(pre * suf) = pr sr - pi si
+                g[i][q] = fma2(pi[i][q], nsi[q], g[i][q]);
+                const f32x2 t_r = fma2(nsi[q], fi[i][q], mul2(sr[q], fr[i][q]));    // Re: sr fr - si fi
+                const f32x2 t_n = fma2(nsi[q], fr[i][q], mul2(sr[q], nfi[i][q]));   // -Im: -(sr fi + si fr)
+                sr[q] = t_r; nsi[q] = t_n;
+            }
 #pragma unroll
-                for (int q = 0; q < NP; ++q) {
-                    g[i][q] = fma2(pr[t][i][q], sr[t][q], g[i][q]);   // Re(pre * suf) = pr sr - pi si
-                    g[i][q] = fma2(pi[t][i][q], nsi[t][q], g[i][q]);
-                    const f32x2 t_r = fma2(nsi[t][q], fi[t][i][q], mul2(sr[t][q], fr[t][i][q]));    // Re: sr fr - si fi
-                    const f32x2 t_n = fma2(nsi[t][q], fr[t][i][q], mul2(sr[t][q], nfi[t][i][q]));   // -Im: -(sr fi + si fr)
-                    sr[t][q] = t_r; nsi[t][q] = t_n;
-                }
-#pragma unroll
-        for (int t = 0; t < PP; ++t)
-#pragma unroll
-            for (int q = 0; q < NP; ++q) g[0][q] = add2(g[0][q], sr[t][q]);       // prefix_0 = 1
+        for (int q = 0; q < NP; ++q) g[0][q] = add2(g[0][q], sr[q]);  // prefix_0 = 1
     }
 }
 
@@ -508,7 +479,7 @@ template <int K, int NP, bool GRAD>
 __device__ __forceinline__ void cplx_row_f2(const f32x2 (&y)[K][NP], const f32x2 *__restrict__ r, f32x2 (&fe)[NP], f32x2 (&g)[K][NP])
 {
     if constexpr (NP == 1 || K < AFSAT_F2_SEQ_MINK) {
-        cplx_points_f2<K, NP, 1, GRAD>(y, r, fe, g);
+        cplx_points_f2<K, NP, GRAD>(y, r, fe, g);
     } else {
 #pragma unroll
         for (int q = 0; q < NP; ++q) {
@@ -516,7 +487,7 @@ __device__ __forceinline__ void cplx_row_f2(const f32x2 (&y)[K][NP], const f32x2
 #pragma unroll
             for (int i = 0; i < K; ++i) { y1[i][0] = y[i][q]; g1[i][0] = g[i][q]; }
             fe1[0] = fe[q];
-            cplx_points_f2<K, 1, 1, GRAD>(y1, r, fe1, g1);
+            cplx_points_f2<K, 1, GRAD>(y1, r, fe1, g1);
 #pragma unroll
             for (int i = 0; i < K; ++i) g[i][q] = g1[i][0];
             fe[q] = fe1[0];
@@ -535,7 +506,7 @@ __device__ __forceinline__ void eval_points_f2(const f32x2 (&y)[K][NP], const f3
         constexpr bool HP = UV == 1, HM = (K & 1) != 0, HI = (K & 3) == 3;
         const f32x2 *rP = tab, *rM = tab + (HP ? ROW2 : 0), *rI = rM + (HM ? ROW2 : 0);
         if (HP || HM || HI) unit_rows_f2<K, NP, HP, HM, HI, GRAD>(y, rP, rM, rI, fe, g);
-        constexpr bool HO = AFSAT_F2_OCT_ROWS && (K & 7) == 7;       // the pair of eighth roots, next in the staged order
+        constexpr bool HO = (K & 7) == 7;       // the pair of eighth roots, next in the staged order
         const f32x2 *rO = rI + (HI ? ROW2 : 0);
         if (HO) {
             oct_row_f2<K, NP, GRAD>(y, rO, 0.70710678118654752f, fe, g);             // = 2 Re b of the row, bit for bit
@@ -586,10 +557,9 @@ __device__ __forceinline__ double flip_sign(double v, int32_t lit)
 }
 
 // One work item for this thread's V candidates; returns the item's partial objective in fe.
-// FIXED = the item contains fixed literals (constant y = +-1, no gather, no gradient).
 // Padding candidates (b >= B inside a live lane pair) are computed and scattered like live ones:
 // G's padding columns are scratch here and are reset by the caller.
-template <typename T, int K, int V, bool GRAD, bool FIXED>
+template <typename T, int K, int V, bool GRAD>
 __device__ __forceinline__ void run_item_reg(const EvalParams<T> &p, const int32_t *__restrict__ s_lits,
                                              const T *__restrict__ s_tab, int n_real, int n_cplx, int nc, int wk,
                                              int64_t b, T (&fe)[V])
@@ -606,12 +576,7 @@ __device__ __forceinline__ void run_item_reg(const EvalParams<T> &p, const int32
         for (int i = 0; i < K; ++i) lit[i] = L[i];
 #pragma unroll
         for (int i = 0; i < K; ++i) {
-            if (FIXED && (lit[i] & LIT_FIXED)) {                      // warp-uniform branch
-#pragma unroll
-                for (int v = 0; v < V; ++v) y[i][v] = T(1);
-            } else {
-                VecIO<T, V>::load(reinterpret_cast<const T *>(xb + (uint64_t)(uint32_t)(lit[i] & LIT_VAR) * x_ld), y[i]);
-            }
+            VecIO<T, V>::load(reinterpret_cast<const T *>(xb + (uint64_t)(uint32_t)(lit[i] & LIT_VAR) * x_ld), y[i]);
 #pragma unroll
             for (int v = 0; v < V; ++v) { y[i][v] = flip_sign(y[i][v], lit[i]); g[i][v] = T(0); }
         }
@@ -619,7 +584,6 @@ __device__ __forceinline__ void run_item_reg(const EvalParams<T> &p, const int32
         if (GRAD) {
 #pragma unroll
             for (int i = 0; i < K; ++i) {
-                if (FIXED && (lit[i] & LIT_FIXED)) continue;          // masked gradient
                 T gi[V];
 #pragma unroll
                 for (int v = 0; v < V; ++v) gi[v] = flip_sign(g[i][v], lit[i]);
@@ -631,10 +595,9 @@ __device__ __forceinline__ void run_item_reg(const EvalParams<T> &p, const int32
 
 // The same for SHORT constraints, which are latency-bound on the gathers: the NEXT constraint's
 // literals and row segments are requested before the current one is evaluated (software pipelining).
-// FIXED = the item contains fixed literals (constant y = +-1, no gather, no gradient).
 // Padding candidates (b >= B inside a live lane pair) are computed and scattered like live ones:
 // G's padding columns are scratch here and are reset by the caller.
-template <typename T, int K, int V, bool GRAD, bool FIXED>
+template <typename T, int K, int V, bool GRAD>
 __device__ __forceinline__ void run_item_pf(const EvalParams<T> &p, const int32_t *__restrict__ s_lits,
                                              const T *__restrict__ s_tab, int n_real, int n_cplx, int nc, int wk,
                                              int64_t b, T (&fe)[V])
@@ -650,14 +613,8 @@ __device__ __forceinline__ void run_item_pf(const EvalParams<T> &p, const int32_
 #pragma unroll
         for (int i = 0; i < K; ++i) lit_n[i] = L[i];
 #pragma unroll
-        for (int i = 0; i < K; ++i) {
-            if (FIXED && (lit_n[i] & LIT_FIXED)) {                    // warp-uniform branch
-#pragma unroll
-                for (int v = 0; v < V; ++v) y_n[i][v] = T(1);
-            } else {
-                VecIO<T, V>::load(reinterpret_cast<const T *>(xb + (uint64_t)(uint32_t)(lit_n[i] & LIT_VAR) * x_ld), y_n[i]);
-            }
-        }
+        for (int i = 0; i < K; ++i)
+            VecIO<T, V>::load(reinterpret_cast<const T *>(xb + (uint64_t)(uint32_t)(lit_n[i] & LIT_VAR) * x_ld), y_n[i]);
     };
     if (wk < nc) fetch(wk);
     for (int c = wk; c < nc; c += Wk) {
@@ -674,7 +631,6 @@ __device__ __forceinline__ void run_item_pf(const EvalParams<T> &p, const int32_
         if (GRAD) {
 #pragma unroll
             for (int i = 0; i < K; ++i) {
-                if (FIXED && (lit[i] & LIT_FIXED)) continue;          // masked gradient
                 T gi[V];
 #pragma unroll
                 for (int v = 0; v < V; ++v) gi[v] = flip_sign(g[i][v], lit[i]);
@@ -737,7 +693,7 @@ template <> struct PairIO<2> {
     }
 };
 
-template <int K, int NP, bool GRAD, bool FIXED, bool PF, int UV>
+template <int K, int NP, bool GRAD, bool PF, int UV>
 __device__ __forceinline__ void run_item_f2(const EvalParams<float> &p, const int32_t *__restrict__ s_lits,
                                             const f32x2 *__restrict__ s_tab2, int n_real, int n_cplx, int nc, int wk,
                                             int64_t b, f32x2 (&fe)[NP])
@@ -746,7 +702,6 @@ __device__ __forceinline__ void run_item_f2(const EvalParams<float> &p, const in
     char *gb = reinterpret_cast<char *>(p.G + (b - p.g_b0));
     const uint32_t x_ld = (uint32_t)(p.ldb * 4), g_ld = (uint32_t)(p.g_ld * 4);
     const int Wk = p.Wk;
-    const f32x2 one2 = pk(1.0f, 1.0f);
     int32_t lit_n[K];
     f32x2 y_n[K][NP];
     auto fetch = [&](int c) {
@@ -754,14 +709,7 @@ __device__ __forceinline__ void run_item_f2(const EvalParams<float> &p, const in
 #pragma unroll
         for (int i = 0; i < K; ++i) lit_n[i] = L[i];
 #pragma unroll
-        for (int i = 0; i < K; ++i) {
-            if (FIXED && (lit_n[i] & LIT_FIXED)) {                    // warp-uniform branch
-#pragma unroll
-                for (int q = 0; q < NP; ++q) y_n[i][q] = one2;
-            } else {
-                PairIO<NP>::load(xb + (uint64_t)(uint32_t)(lit_n[i] & LIT_VAR) * x_ld, y_n[i]);
-            }
-        }
+        for (int i = 0; i < K; ++i) PairIO<NP>::load(xb + (uint64_t)(uint32_t)(lit_n[i] & LIT_VAR) * x_ld, y_n[i]);
     };
     if (PF && wk < nc) fetch(wk);
     for (int c = wk; c < nc; c += Wk) {
@@ -780,14 +728,10 @@ __device__ __forceinline__ void run_item_f2(const EvalParams<float> &p, const in
         if (GRAD) {
 #pragma unroll
             for (int i = 0; i < K; ++i) {
-                if (FIXED && (lit[i] & LIT_FIXED)) continue;          // masked gradient
                 const uint32_t m = (uint32_t)(lit[i] & LIT_NEG);
                 f32x2 gi[NP];
 #pragma unroll
                 for (int q = 0; q < NP; ++q) gi[q] = g[i][q] ^ (((f32x2)m << 32) | m);
-#ifdef AFSAT_EXP_NORED
-                if (gi[0] == 0x123456789ull)
-#endif
                 PairIO<NP>::red(gb + (uint64_t)(uint32_t)(lit[i] & LIT_VAR) * g_ld, gi);
             }
         }
@@ -799,7 +743,7 @@ __device__ __forceinline__ void run_item_f2(const EvalParams<float> &p, const in
 // allocation while all lengths share one grid (no per-length launch tails) ---------------------------
 template <int K, int NP, bool GRAD>
 __device__ __noinline__ void item_body_f2(const EvalParams<float> &p, const int32_t *s_lits, const f32x2 *s_tab2,
-                                          float (*s_F)[64 * NP], int n_real, int n_cplx, int nc, bool has_fixed, int uv)
+                                          float (*s_F)[64 * NP], int n_real, int n_cplx, int nc, int uv)
 {
     constexpr int V = 2 * NP;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -811,15 +755,9 @@ __device__ __noinline__ void item_body_f2(const EvalParams<float> &p, const int3
     for (int q = 0; q < NP; ++q) fe2[q] = 0ull;
     if (active) {
         constexpr bool PF = K <= 5;
-        if (has_fixed) {                                      // rare (partial assignments): one generic-order body
-            if (uv == 1) run_item_f2<K, NP, GRAD, true, PF, 1>(p, s_lits, s_tab2, n_real, n_cplx, nc, wk, b, fe2);
-            else if (uv == 2) run_item_f2<K, NP, GRAD, true, PF, 2>(p, s_lits, s_tab2, n_real, n_cplx, nc, wk, b, fe2);
-            else run_item_f2<K, NP, GRAD, true, PF, 0>(p, s_lits, s_tab2, n_real, n_cplx, nc, wk, b, fe2);
-        } else {
-            if (uv == 1) run_item_f2<K, NP, GRAD, false, PF, 1>(p, s_lits, s_tab2, n_real, n_cplx, nc, wk, b, fe2);
-            else if (uv == 2) run_item_f2<K, NP, GRAD, false, PF, 2>(p, s_lits, s_tab2, n_real, n_cplx, nc, wk, b, fe2);
-            else run_item_f2<K, NP, GRAD, false, PF, 0>(p, s_lits, s_tab2, n_real, n_cplx, nc, wk, b, fe2);
-        }
+        if (uv == 1) run_item_f2<K, NP, GRAD, PF, 1>(p, s_lits, s_tab2, n_real, n_cplx, nc, wk, b, fe2);
+        else if (uv == 2) run_item_f2<K, NP, GRAD, PF, 2>(p, s_lits, s_tab2, n_real, n_cplx, nc, wk, b, fe2);
+        else run_item_f2<K, NP, GRAD, PF, 0>(p, s_lits, s_tab2, n_real, n_cplx, nc, wk, b, fe2);
     }
     float fe[V];
 #pragma unroll
@@ -830,10 +768,10 @@ __device__ __noinline__ void item_body_f2(const EvalParams<float> &p, const int3
 template <int K, int KHI, int NP, bool GRAD>
 struct SwitchF2 {
     static __device__ __forceinline__ void go(int k, const EvalParams<float> &p, const int32_t *s_lits, const f32x2 *s_tab2,
-                                              float (*s_F)[64 * NP], int n_real, int n_cplx, int nc, bool has_fixed, int uv)
+                                              float (*s_F)[64 * NP], int n_real, int n_cplx, int nc, int uv)
     {
-        if (k == K) item_body_f2<K, NP, GRAD>(p, s_lits, s_tab2, s_F, n_real, n_cplx, nc, has_fixed, uv);
-        else if (K < KHI) SwitchF2<(K < KHI ? K + 1 : K), KHI, NP, GRAD>::go(k, p, s_lits, s_tab2, s_F, n_real, n_cplx, nc, has_fixed, uv);
+        if (k == K) item_body_f2<K, NP, GRAD>(p, s_lits, s_tab2, s_F, n_real, n_cplx, nc, uv);
+        else if (K < KHI) SwitchF2<(K < KHI ? K + 1 : K), KHI, NP, GRAD>::go(k, p, s_lits, s_tab2, s_F, n_real, n_cplx, nc, uv);
     }
 };
 
@@ -855,13 +793,13 @@ __global__ void __launch_bounds__(CTA_THREADS, MINB) k_eval_f2m(const EvalParams
     const int nl = (it.c_end - it.c_begin) * it.k;
     for (int i = threadIdx.x; i < nl; i += blockDim.x) s_lits[i] = __ldg(p.lits + it.lit_base + i);
     __syncthreads();
-    SwitchF2<KLO, KHI, NP, GRAD>::go(it.k, p, s_lits, s_tab2, s_F, n_unit, n_gen, it.c_end - it.c_begin, it.has_fixed != 0, uv);
+    SwitchF2<KLO, KHI, NP, GRAD>::go(it.k, p, s_lits, s_tab2, s_F, n_unit, n_gen, it.c_end - it.c_begin, uv);
 }
 
 // one body per length: KHI <= 20 for both instantiations (fp32 beyond k = 8 runs the lane-split kernels of afsat_split.cuh)
 template <typename T, int K, int V, bool GRAD>
 __device__ __noinline__ void item_body_k(const EvalParams<T> &p, const int32_t *s_lits, const T *s_tab, T (*s_F)[32 * V],
-                                         int n_real, int n_cplx, int nc, bool has_fixed)
+                                         int n_real, int n_cplx, int nc)
 {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int wc = warp % p.Wc, wk = warp / p.Wc;
@@ -871,13 +809,8 @@ __device__ __noinline__ void item_body_k(const EvalParams<T> &p, const int32_t *
 #pragma unroll
     for (int v = 0; v < V; ++v) fe[v] = T(0);
     if (active) {
-        if (K <= 5) {
-            if (has_fixed) run_item_pf<T, K, V, GRAD, true>(p, s_lits, s_tab, n_real, n_cplx, nc, wk, b, fe);
-            else run_item_pf<T, K, V, GRAD, false>(p, s_lits, s_tab, n_real, n_cplx, nc, wk, b, fe);
-        } else {
-            if (has_fixed) run_item_reg<T, K, V, GRAD, true>(p, s_lits, s_tab, n_real, n_cplx, nc, wk, b, fe);
-            else run_item_reg<T, K, V, GRAD, false>(p, s_lits, s_tab, n_real, n_cplx, nc, wk, b, fe);
-        }
+        if (K <= 5) run_item_pf<T, K, V, GRAD>(p, s_lits, s_tab, n_real, n_cplx, nc, wk, b, fe);
+        else run_item_reg<T, K, V, GRAD>(p, s_lits, s_tab, n_real, n_cplx, nc, wk, b, fe);
     }
     store_item_F<T, V>(p, s_F, fe, warp, lane, wk, b, active);
 }
@@ -885,10 +818,10 @@ __device__ __noinline__ void item_body_k(const EvalParams<T> &p, const int32_t *
 template <typename T, int K, int KHI, int V, bool GRAD>
 struct SwitchK {
     static __device__ __forceinline__ void go(int k, const EvalParams<T> &p, const int32_t *s_lits, const T *s_tab,
-                                              T (*s_F)[32 * V], int n_real, int n_cplx, int nc, bool has_fixed)
+                                              T (*s_F)[32 * V], int n_real, int n_cplx, int nc)
     {
-        if (k == K) item_body_k<T, K, V, GRAD>(p, s_lits, s_tab, s_F, n_real, n_cplx, nc, has_fixed);
-        else if (K < KHI) SwitchK<T, (K < KHI ? K + 1 : K), KHI, V, GRAD>::go(k, p, s_lits, s_tab, s_F, n_real, n_cplx, nc, has_fixed);
+        if (k == K) item_body_k<T, K, V, GRAD>(p, s_lits, s_tab, s_F, n_real, n_cplx, nc);
+        else if (K < KHI) SwitchK<T, (K < KHI ? K + 1 : K), KHI, V, GRAD>::go(k, p, s_lits, s_tab, s_F, n_real, n_cplx, nc);
     }
 };
 
@@ -902,564 +835,13 @@ __global__ void __launch_bounds__(CTA_THREADS, MINB) k_eval_km(const EvalParams<
     const SigDev sg = p.sigs[it.sig];
     stage_item(p, it, sg, s_tab, s_lits);
     __syncthreads();
-    SwitchK<T, KLO, KHI, V, GRAD>::go(it.k, p, s_lits, s_tab, s_F, sg.n_real, sg.n_cplx, it.c_end - it.c_begin, it.has_fixed != 0);
+    SwitchK<T, KLO, KHI, V, GRAD>::go(it.k, p, s_lits, s_tab, s_F, sg.n_real, sg.n_cplx, it.c_end - it.c_begin);
 }
 
-// ---- register-blocked kernel for long constraints (16 < k <= KMAX <= 64), one candidate per lane ------
-// The k partial gradients live in REGISTERS (the literal loop is unrolled to KMAX in blocks of LB, blocks
-// beyond k are skipped by a warp-uniform branch); the literal values are staged once per constraint in
-// shared memory as [i][lane] columns; per DFT point the forward pass keeps only the prefix product at
-// each block boundary and the backward pass rebuilds the LB prefixes of a block from its boundary value
-// before walking the suffix through it (leave-one-out = prefix x suffix, no division).  Shared-memory
-// traffic is 2 loads per literal and point instead of the 9 accesses of a fully staged scheme.
-constexpr int LB = 8;
-constexpr int LONG_THREADS = 128;
-constexpr int LONG_LIT_CHUNK = 1024;   // packed literals per work item of the long class (>= 16 constraints)
-
-template <typename T, bool CPLX, int NU>
-struct BlkOps {
-    // forward through one block of NU literals: run <- run * prod f_u
-    static __device__ __forceinline__ void fwd(const T *__restrict__ sy, T ar, T ai, T br, T bi, T &rr, T &ri)
-    {
-#pragma unroll
-        for (int u = 0; u < NU; ++u) {
-            const T yv = sy[u * 32];
-            const T fr = fma_(br, yv, ar);
-            if (CPLX) {
-                const T fi = fma_(bi, yv, ai);
-                const T nr = fma_(rr, fr, -(ri * fi));
-                const T ni = fma_(rr, fi, ri * fr);
-                rr = nr; ri = ni;
-            } else {
-                rr *= fr;
-            }
-        }
-    }
-    // backward through one block: prefixes rebuilt from the boundary value (pr0, pi0), then
-    // g_u += Re(prefix_u * suffix), suffix <- suffix * f_u for u = NU-1 .. 0
-    static __device__ __forceinline__ void bwd(const T *__restrict__ sy, T ar, T ai, T br, T bi, T pr0, T pi0, T &sr, T &si,
-                                               T *__restrict__ g)
-    {
-        T fr[NU], fi[CPLX ? NU : 1], pr[NU], pi[CPLX ? NU : 1];
-#pragma unroll
-        for (int u = 0; u < NU; ++u) {
-            const T yv = sy[u * 32];
-            fr[u] = fma_(br, yv, ar);
-            if (CPLX) fi[u] = fma_(bi, yv, ai);
-        }
-        pr[0] = pr0;
-        if (CPLX) pi[0] = pi0;
-#pragma unroll
-        for (int u = 1; u < NU; ++u) {
-            if (CPLX) {
-                pr[u] = fma_(pr[u - 1], fr[u - 1], -(pi[u - 1] * fi[u - 1]));
-                pi[u] = fma_(pr[u - 1], fi[u - 1], pi[u - 1] * fr[u - 1]);
-            } else {
-                pr[u] = pr[u - 1] * fr[u - 1];
-            }
-        }
-#pragma unroll
-        for (int u = NU - 1; u >= 0; --u) {
-            if (CPLX) {
-                g[u] = fma_(pr[u], sr, g[u]);
-                g[u] = fma_(-pi[u], si, g[u]);
-                const T nr = fma_(sr, fr[u], -(si * fi[u]));
-                const T ni = fma_(sr, fi[u], si * fr[u]);
-                sr = nr; si = ni;
-            } else {
-                g[u] = fma_(pr[u], sr, g[u]);
-                sr *= fr[u];
-            }
-        }
-    }
-};
-
-// backward through the LAST, partial block (nu < LB literals; the staged values beyond k are zeros):
-// same arithmetic, the updates of g and of the suffix predicated on u < nu
-template <typename T, bool CPLX>
-__device__ __forceinline__ void blk_bwd_partial(int nu, const T *__restrict__ sy, T ar, T ai, T br, T bi, T pr0, T pi0, T &sr,
-                                                T &si, T *__restrict__ g)
-{
-    T fr[LB], fi[CPLX ? LB : 1], pr[LB], pi[CPLX ? LB : 1];
-#pragma unroll
-    for (int u = 0; u < LB; ++u) {
-        const T yv = sy[u * 32];
-        fr[u] = fma_(br, yv, ar);
-        if (CPLX) fi[u] = fma_(bi, yv, ai);
-    }
-    pr[0] = pr0;
-    if (CPLX) pi[0] = pi0;
-#pragma unroll
-    for (int u = 1; u < LB; ++u) {
-        if (CPLX) {
-            pr[u] = fma_(pr[u - 1], fr[u - 1], -(pi[u - 1] * fi[u - 1]));
-            pi[u] = fma_(pr[u - 1], fi[u - 1], pi[u - 1] * fr[u - 1]);
-        } else {
-            pr[u] = pr[u - 1] * fr[u - 1];
-        }
-    }
-#pragma unroll
-    for (int u = LB - 1; u >= 0; --u) {
-        if (u < nu) {                                                 // warp-uniform
-            if (CPLX) {
-                g[u] = fma_(pr[u], sr, g[u]);
-                g[u] = fma_(-pi[u], si, g[u]);
-                const T nr = fma_(sr, fr[u], -(si * fi[u]));
-                const T ni = fma_(sr, fi[u], si * fr[u]);
-                sr = nr; si = ni;
-            } else {
-                g[u] = fma_(pr[u], sr, g[u]);
-                sr *= fr[u];
-            }
-        }
-    }
-}
-
-// One DFT point of a long constraint.  sy: staged literal values [i][lane] (zeros up to the next
-// multiple of LB), sb: boundary prefixes [blk][re, im][lane] of this warp.
-template <typename T, int KMAX, bool CPLX, bool GRAD>
-__device__ __forceinline__ void long_point(const T *__restrict__ sy, T *__restrict__ sb, int k, const T *__restrict__ r, T &fe,
-                                           T (&g)[KMAX])
-{
-    constexpr int NBLK = KMAX / LB;
-    const T ar = r[0], ai = r[1], br = r[2], bi = r[3];
-    T rr = T(1), ri = T(0);
-    const int nfull = k / LB, tail = k % LB;
-    for (int blk = 0; blk < nfull; ++blk) {                           // forward: runtime loop, one body
-        sb[(2 * blk) * 32] = rr;
-        if (CPLX) sb[(2 * blk + 1) * 32] = ri;
-        BlkOps<T, CPLX, LB>::fwd(sy + blk * LB * 32, ar, ai, br, bi, rr, ri);
-    }
-    if (tail) {
-        sb[(2 * nfull) * 32] = rr;
-        if (CPLX) sb[(2 * nfull + 1) * 32] = ri;
-        for (int u = 0; u < tail; ++u) BlkOps<T, CPLX, 1>::fwd(sy + (nfull * LB + u) * 32, ar, ai, br, bi, rr, ri);
-    }
-    fe = fma_(r[4], rr, fe);
-    if (CPLX) fe = fma_(-r[5], ri, fe);
-    if (GRAD) {
-        T sr = r[6], si = CPLX ? r[7] : T(0);                          // suffix seeded with w b
-#pragma unroll
-        for (int blk = NBLK - 1; blk >= 0; --blk) {                    // backward: unrolled, g in registers
-            if (blk < nfull) {
-                BlkOps<T, CPLX, LB>::bwd(sy + blk * LB * 32, ar, ai, br, bi, sb[(2 * blk) * 32],
-                                         CPLX ? sb[(2 * blk + 1) * 32] : T(0), sr, si, &g[blk * LB]);
-            } else if (blk == nfull && tail) {
-                blk_bwd_partial<T, CPLX>(tail, sy + blk * LB * 32, ar, ai, br, bi, sb[(2 * blk) * 32],
-                                         CPLX ? sb[(2 * blk + 1) * 32] : T(0), sr, si, &g[blk * LB]);
-            }
-        }
-    }
-}
-
-template <typename T, int KMAX, bool GRAD>
-__global__ void __launch_bounds__(LONG_THREADS) k_eval_blk(const EvalParams<T> p)
-{
-    constexpr int NW = LONG_THREADS / 32;
-    __shared__ __align__(16) T s_tab[MAX_ROWS * 8];
-    __shared__ int32_t s_lits[LONG_LIT_CHUNK];
-    __shared__ T s_F[NW][32];
-    extern __shared__ __align__(16) unsigned char s_dyn[];               // per warp: values [KMAX][32], boundaries [2 NBLK][32]
-    constexpr int PER_WARP = (KMAX + 2 * (KMAX / LB)) * 32;
-    T *s_y = reinterpret_cast<T *>(s_dyn);
-    const Item it = p.items[blockIdx.x];
-    const SigDev sgd = p.sigs[it.sig];
-    stage_item(p, it, sgd, s_tab, s_lits);
-    __syncthreads();
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int wc = warp % p.Wc, wk = warp / p.Wc;
-    const int64_t b = p.b_begin + ((int64_t)blockIdx.y * p.Wc + wc) * 32 + lane;
-    const bool active = b < p.b_end && b < p.B && !lane_skipped(p, b, 1);   // this launch owns [b_begin, b_end)
-    T fe[1] = {T(0)};
-    if (active) {
-        T *sy = s_y + (size_t)warp * PER_WARP + lane;
-        T *sb = sy + KMAX * 32;
-        const int k = it.k, nc = it.c_end - it.c_begin;
-        const char *xb = reinterpret_cast<const char *>(p.x + b);
-        char *gb = reinterpret_cast<char *>(p.G + (b - p.g_b0));
-        const uint32_t x_ld = (uint32_t)(p.ldb * (int64_t)sizeof(T)), g_ld = (uint32_t)(p.g_ld * (int64_t)sizeof(T));
-        for (int c = wk; c < nc; c += p.Wk) {
-            const int32_t *L = s_lits + c * k;
-            for (int i = 0; i < k; ++i) {                               // a1: gather, sign, stage
-                const int32_t lit = L[i];
-                const T v = (lit & LIT_FIXED) ? T(1) : __ldg(reinterpret_cast<const T *>(xb + (uint64_t)(uint32_t)(lit & LIT_VAR) * x_ld));
-                sy[i * 32] = flip_sign(v, lit);
-            }
-            for (int i = k; i < (k + LB - 1) / LB * LB; ++i) sy[i * 32] = T(0);   // finite padding of the last block
-            T g[KMAX];
-#pragma unroll
-            for (int i = 0; i < KMAX; ++i) g[i] = T(0);
-            const T *r = s_tab;
-            for (int q = 0; q < sgd.n_real; ++q, r += 8) long_point<T, KMAX, false, GRAD>(sy, sb, k, r, fe[0], g);
-            for (int q = 0; q < sgd.n_cplx; ++q, r += 8) long_point<T, KMAX, true, GRAD>(sy, sb, k, r, fe[0], g);
-            if (GRAD) {
-#pragma unroll
-                for (int i = 0; i < KMAX; ++i) {
-                    if (i < k) {                                        // warp-uniform
-                        const int32_t lit = L[i];
-                        if (!(lit & LIT_FIXED))
-                            red_add(reinterpret_cast<T *>(gb + (uint64_t)(uint32_t)(lit & LIT_VAR) * g_ld), flip_sign(g[i], lit));
-                    }
-                }
-            }
-        }
-    }
-    store_item_F<T, 1>(p, s_F, fe, warp, lane, wk, b, active);
-}
-
-// ---- a7: sign rounding as one bit per (variable, candidate): bits[v][b / 32] bit (b % 32) = (x < 0)
-template <typename T>
-__global__ void __launch_bounds__(CTA_THREADS) k_pack_signs(const T *__restrict__ x, uint32_t *__restrict__ bits, int n,
-                                                           int B, int64_t ldb)
-{
-    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= ldb) return;                                             // whole warps (ldb % 32 == 0)
-    const int64_t ldw = ldb >> 5;
-    for (int v = blockIdx.y; v < n; v += gridDim.y) {
-        const bool t = (b < B) && (x[(int64_t)v * ldb + b] < T(0));   // True iff x < 0 (0, -0.0 -> False)
-        const uint32_t w = __ballot_sync(0xffffffffu, t);
-        if ((threadIdx.x & 31) == 0) bits[(int64_t)v * ldw + (b >> 5)] = w;
-    }
-}
-
-// ---- a6 + a7 + a9: projected step on the candidate tile [b_begin, b_end), gradient scratch reset,
-// sign bits of the NEW x.  Frozen (solved) candidates and fixed variables keep their x.
-// Thread layout: cols = min(tile width, CTA_THREADS) adjacent candidates x (CTA_THREADS / cols)
-// variables per CTA pass, UPD_UNROLL independent rows in flight per thread.
-constexpr int UPD_UNROLL = 4;
-template <typename T>
-__global__ void __launch_bounds__(CTA_THREADS) k_update(T *__restrict__ x, T *__restrict__ G, int64_t g_ld, int64_t g_b0,
-                                                       const int8_t *__restrict__ fixed,
-                                                       const uint8_t *__restrict__ is_solution, uint32_t *__restrict__ bits,
-                                                       T eta, int n, int B, int64_t ldb, int64_t b_begin, int64_t b_end,
-                                                       int cols)
-{
-    const int col = threadIdx.x % cols, r = threadIdx.x / cols, rows_per_pass = blockDim.x / cols;
-    const int64_t b = b_begin + (int64_t)blockIdx.x * cols + col;
-    if (b >= b_end) return;                                           // tiles and cols are multiples of 32
-    const bool live = b < B;
-    const bool upd = live && !is_solution[b];
-    const int64_t ldw = ldb >> 5;
-    const int stride = gridDim.y * rows_per_pass;
-    for (int v0 = blockIdx.y * rows_per_pass + r; v0 < n; v0 += stride * UPD_UNROLL) {
-        T g[UPD_UNROLL], xv[UPD_UNROLL];
-        int8_t fx[UPD_UNROLL];
-#pragma unroll
-        for (int u = 0; u < UPD_UNROLL; ++u) {
-            const int v = v0 + u * stride;
-            if (v < n) {
-                g[u] = G[(int64_t)v * g_ld + (b - g_b0)];
-                xv[u] = x[(int64_t)v * ldb + b];
-                fx[u] = fixed[v];
-            }
-        }
-#pragma unroll
-        for (int u = 0; u < UPD_UNROLL; ++u) {
-            const int v = v0 + u * stride;
-            if (v < n) {                                              // warp-uniform (v depends on the warp's row only)
-                G[(int64_t)v * g_ld + (b - g_b0)] = T(0);
-                T nx = xv[u];
-                if (upd && !fx[u]) {
-                    nx = fma_(-eta, g[u], nx);
-                    nx = nx > T(1) ? T(1) : nx;
-                    nx = nx < T(-1) ? T(-1) : nx;
-                    x[(int64_t)v * ldb + b] = nx;
-                }
-                const uint32_t w = __ballot_sync(0xffffffffu, live && (nx < T(0)));
-                if ((threadIdx.x & 31) == 0) bits[(int64_t)v * ldw + (b >> 5)] = w;
-            }
-        }
-    }
-}
-
-// ---- a8: exact discrete count, integer only.  One thread = one 32-candidate word; the number tau
-// of true literals is kept BIT-SLICED (t[j] holds bit j of tau for 32 candidates), the predicate is
-// evaluated by scanning the smaller of {satisfied counts, violated counts}, and the per-candidate
-// number of satisfied constraints of the item is again a bit-sliced counter.
-struct CheckParams {
-    const uint32_t *bits;       // [n][ldw]
-    int64_t ldw;
-    const int32_t *lits;
-    const SigDev *sigs;
-    const Item *items;
-    int32_t *satacc;            // [ldb]
-    int32_t B;
-    int32_t w_begin, w_end;     // word range of this launch
-    int32_t wpb;                // words per CTA (power of two <= 32)
-    int32_t n_items;
-};
-
-#ifndef AFSAT_KM32_TU   // non-template kernel: defined in ONE translation unit only
-__global__ void __launch_bounds__(CTA_THREADS) k_check_bits(const CheckParams p)
-{
-    __shared__ int32_t s_lits[LIT_CHUNK];
-    __shared__ int32_t s_cnt[32 * 32];
-    for (int i = threadIdx.x; i < p.wpb * 32; i += blockDim.x) s_cnt[i] = 0;
-    const int wi = threadIdx.x % p.wpb, grp = threadIdx.x / p.wpb, ngrp = blockDim.x / p.wpb;
-    const int word = p.w_begin + blockIdx.y * p.wpb + wi;
-    const bool valid = word < p.w_end;
-    uint32_t cnt[13];
-#pragma unroll
-    for (int j = 0; j < 13; ++j) cnt[j] = 0u;
-    int nacc = 0;                                                     // constraints counted in cnt[] so far
-    auto flush = [&]() {                                              // bit-sliced counter -> per-candidate integers
-        for (int bit = 0; bit < 32; ++bit) {
-            int val = 0;
-#pragma unroll
-            for (int j = 0; j < 13; ++j) val |= (int)((cnt[j] >> bit) & 1u) << j;
-            if (val) atomicAdd(&s_cnt[wi * 32 + bit], val);
-        }
-#pragma unroll
-        for (int j = 0; j < 13; ++j) cnt[j] = 0u;
-        nacc = 0;
-    };
-    for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {   // persistent over work items
-        const Item it = p.items[item];
-        const SigDev sg = p.sigs[it.sig];
-        const int k = it.k, nc = it.c_end - it.c_begin;
-        __syncthreads();                                              // previous item's literals are consumed
-        for (int i = threadIdx.x; i < nc * k; i += blockDim.x) s_lits[i] = __ldg(p.lits + it.lit_base + i);
-        __syncthreads();
-        if (!valid) continue;
-        int nb = 1;
-        while ((1 << nb) <= k) ++nb;                                  // bits of tau in [0, k]
-        const int mine = (nc - grp + ngrp - 1) / ngrp;
-        if (nacc + mine > 8191) flush();
-        nacc += mine > 0 ? mine : 0;
-        for (int c = grp; c < nc; c += ngrp) {
-            uint32_t t[7] = {0u, 0u, 0u, 0u, 0u, 0u, 0u};
-            const int32_t *L = s_lits + c * k;
-            for (int i = 0; i < k; ++i) {
-                const int32_t lit = L[i];
-                uint32_t m = (lit & LIT_FIXED) ? 0u : __ldg(p.bits + (int64_t)(lit & LIT_VAR) * p.ldw + word);
-                if (lit < 0) m = ~m;                                  // literal true = variable true XOR negated
-#pragma unroll
-                for (int j = 0; j < 7; ++j)
-                    if (j < nb) { const uint32_t s = t[j] ^ m; m &= t[j]; t[j] = s; }
-            }
-            uint32_t acc = 0u;
-            for (int tau = 0; tau <= k; ++tau) {
-                const uint64_t bit = tau < 64 ? (sg.scan_lo >> tau) : (sg.scan_hi >> (tau - 64));
-                if (!(bit & 1ull)) continue;
-                uint32_t eq = 0xffffffffu;
-#pragma unroll
-                for (int j = 0; j < 7; ++j)
-                    if (j < nb) eq &= ((tau >> j) & 1) ? t[j] : ~t[j];
-                acc |= eq;
-            }
-            uint32_t carry = sg.scan_is_sat ? acc : ~acc;             // 1 = constraint satisfied
-#pragma unroll
-            for (int j = 0; j < 13; ++j) { const uint32_t s = cnt[j] ^ carry; carry &= cnt[j]; cnt[j] = s; }
-        }
-    }
-    if (valid && nacc) flush();
-    __syncthreads();
-    const int64_t b0 = ((int64_t)p.w_begin + (int64_t)blockIdx.y * p.wpb) * 32;
-    for (int i = threadIdx.x; i < p.wpb * 32; i += blockDim.x) {
-        const int64_t b = b0 + i;
-        if (b < p.B && b < (int64_t)p.w_end * 32 && s_cnt[i]) atomicAdd(p.satacc + b, s_cnt[i]);
-    }
-}
-#endif
-
-// ---- line search (afsat_step_ls; reading B5): per-candidate backtracking along the projection arc ----
-// ls_state[b]: 0 = still searching, 1 = step accepted, 2 = frozen (solved or converged)
-constexpr int LS_CHUNKS = 32;         // row chunks of the <G, X - X'> reduction (fixed-order two-stage sum)
-
-#ifndef AFSAT_KM32_TU   // non-template kernel: defined in ONE translation unit only
-__global__ void k_ls_begin(int B, int64_t ldb, const uint8_t *__restrict__ is_solution, const uint8_t *__restrict__ converged,
-                           uint8_t *__restrict__ ls_state, double s_max, double *__restrict__ eta)
-{
-    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= ldb) return;
-    ls_state[b] = (b >= B || is_solution[b] || converged[b]) ? 2 : 0;
-    eta[b] = s_max;
-}
-#endif
-
-// X' = clamp(X - eta_b G) for the candidates still searching (first trial: every candidate gets a valid X'),
-// Dpart[chunk][b] = sum over the chunk's rows of G (X - X')
-template <typename T>
-__global__ void __launch_bounds__(CTA_THREADS) k_ls_trial(const T *__restrict__ x, const T *__restrict__ G, T *__restrict__ xt,
-                                                         const int8_t *__restrict__ fixed, const uint8_t *__restrict__ ls_state,
-                                                         const double *__restrict__ eta, double *__restrict__ Dpart, int n,
-                                                         int64_t ldb, int first_trial)
-{
-    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= ldb) return;
-    const int st = ls_state[b];
-    const int rows = (n + LS_CHUNKS - 1) / LS_CHUNKS, v0 = blockIdx.y * rows, v1 = min(n, v0 + rows);
-    if (st != 0) {
-        if (first_trial) for (int v = v0; v < v1; ++v) xt[(int64_t)v * ldb + b] = x[(int64_t)v * ldb + b];
-        return;
-    }
-    const T e = (T)eta[b];
-    double D = 0.0;
-    for (int v = v0; v < v1; ++v) {
-        const T xv = x[(int64_t)v * ldb + b];
-        T nx = xv;
-        if (!fixed[v]) {
-            const T g = G[(int64_t)v * ldb + b];
-            nx = fma_(-e, g, xv);
-            nx = nx > T(1) ? T(1) : nx;
-            nx = nx < T(-1) ? T(-1) : nx;
-            D += (double)g * (double)(xv - nx);
-        }
-        xt[(int64_t)v * ldb + b] = nx;
-    }
-    Dpart[(int64_t)blockIdx.y * ldb + b] = D;
-}
-
-// Armijo test of the trial; backtrack or give up (eta < delta: converged)
-template <typename T>
-__global__ void k_ls_decide(int B, int64_t ldb, const T *__restrict__ F0, const T *__restrict__ F1, const double *__restrict__ Dpart,
-                            uint8_t *__restrict__ ls_state, double *__restrict__ eta, uint8_t *__restrict__ converged, double c1,
-                            double beta, double delta)
-{
-    const int b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= B || ls_state[b] != 0) return;
-    double D = 0.0;
-    for (int c = 0; c < LS_CHUNKS; ++c) D += Dpart[(int64_t)c * ldb + b];
-    if ((double)F1[b] <= (double)F0[b] - c1 * D) { ls_state[b] = 1; return; }
-    const double e = eta[b] * beta;
-    eta[b] = e;
-    if (e < delta) { ls_state[b] = 2; converged[b] = 1; }
-}
-
-// accepted candidates take X', sign bits of the resulting X for everyone
-template <typename T>
-__global__ void __launch_bounds__(CTA_THREADS) k_ls_commit(T *__restrict__ x, const T *__restrict__ xt, const uint8_t *__restrict__ ls_state,
-                                                          uint32_t *__restrict__ bits, int n, int B, int64_t ldb)
-{
-    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= ldb) return;                                             // whole warps (ldb % 32 == 0)
-    const bool live = b < B, take = live && ls_state[b] == 1;
-    const int64_t ldw = ldb >> 5;
-    for (int v = blockIdx.y; v < n; v += gridDim.y) {
-        T xv = T(0);
-        if (live) {
-            xv = take ? xt[(int64_t)v * ldb + b] : x[(int64_t)v * ldb + b];
-            if (take) x[(int64_t)v * ldb + b] = xv;
-        }
-        const uint32_t w = __ballot_sync(0xffffffffu, live && xv < T(0));
-        if ((threadIdx.x & 31) == 0) bits[(int64_t)v * ldw + (b >> 5)] = w;
-    }
-}
-
-template <typename T>
-__global__ void k_ls_report(int B, const double *__restrict__ eta, T *__restrict__ eta_out)
-{
-    const int b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b < B) eta_out[b] = (T)eta[b];
-}
-
-// ---- afsat_restart: counter-based uniform re-initialisation (include/afsat.h states the generator) ----
-__device__ __forceinline__ uint32_t fmix32(uint32_t h)
-{
-    h ^= h >> 16; h *= 0x85EBCA6Bu; h ^= h >> 13; h *= 0xC2B2AE35u; h ^= h >> 16;
-    return h;
-}
-
-template <typename T>
-__global__ void __launch_bounds__(CTA_THREADS) k_restart(T *__restrict__ x, const int8_t *__restrict__ fixed,
-                                                        const uint8_t *__restrict__ keep, uint32_t lo, uint32_t hi, uint32_t round,
-                                                        int n, int B, int64_t ldb)
-{
-    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= B || (keep && keep[b])) return;
-    const uint32_t hb = fmix32(lo ^ ((uint32_t)b * 0x9E3779B9u));
-    for (int v = blockIdx.y; v < n; v += gridDim.y) {
-        const int8_t f = fixed[v];
-        T val;
-        if (f) val = (T)f;
-        else {
-            const uint32_t h = fmix32(fmix32((hb + (uint32_t)v * 0x85EBCA6Bu) ^ hi) + round * 0xC2B2AE35u);
-            val = (T)((float)(h >> 8) * 1.1920928955078125e-07f - 1.0f);     // (h >> 8) 2^-23 - 1, exact
-        }
-        x[(int64_t)v * ldb + b] = val;
-    }
-}
-
-// zero the padding columns [B, ldb) of a caller-owned gradient (vector REDs of a lane pair that
-// straddles B spill into them)
-template <typename T>
-__global__ void k_zero_pad(T *__restrict__ G, int n, int B, int64_t ldb)
-{
-    const int64_t np = ldb - B;
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < (int64_t)n * np; i += (int64_t)gridDim.x * blockDim.x)
-        G[(i / np) * ldb + B + (i % np)] = T(0);
-}
-
-// ---- F[b] = sum over items of Fpart[item][b], fixed order, accumulated in double ------------
-template <typename T>
-__global__ void k_reduce_F(const T *__restrict__ Fpart, int n_rows, int64_t ldb, int B, T *__restrict__ F,
-                           const uint8_t *__restrict__ skip)
-{
-    const int b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= B || (skip && skip[b])) return;                           // skipped candidates keep their F
-    double s = 0.0;
-    for (int i = 0; i < n_rows; ++i) s += (double)Fpart[(int64_t)i * ldb + b];
-    F[b] = (T)s;
-}
-
-// ---- per-candidate state machine of Alg. 1 (a8, a9): satacc holds the count on the current X ----
-#ifndef AFSAT_KM32_TU   // non-template kernel: defined in ONE translation unit only
-__global__ void k_flags(int32_t *__restrict__ satacc, int B, int m, int mark_solved, int step_value,
-                        int32_t *__restrict__ sat_count, uint8_t *__restrict__ is_solution,
-                        int32_t *__restrict__ first_step, int32_t *__restrict__ d_any, volatile int32_t *h_any)
-{
-    const int b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= B) return;
-    const int s = satacc[b];
-    satacc[b] = 0;
-    sat_count[b] = s;
-    if (mark_solved && s == m && !is_solution[b]) {
-        is_solution[b] = 1;
-        first_step[b] = step_value;
-        if (atomicCAS(d_any, 0, 1) == 0) {
-            d_any[1] = step_value;
-            if (h_any) { h_any[1] = step_value; __threadfence_system(); h_any[0] = 1; }
-        }
-    }
-}
-#endif
-
-// afsat_check epilogue: counts out, is_solution = (count == m), accumulator reset.
-#ifndef AFSAT_KM32_TU   // non-template kernel: defined in ONE translation unit only
-__global__ void k_check_finish(int32_t *__restrict__ satacc, int B, int m, int32_t *__restrict__ sat_count,
-                               uint8_t *__restrict__ is_solution)
-{
-    const int b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= B) return;
-    const int s = satacc[b];
-    satacc[b] = 0;
-    sat_count[b] = s;
-    is_solution[b] = (uint8_t)(s == m);
-}
-#endif
-
-#ifndef AFSAT_KM32_TU   // non-template kernel: defined in ONE translation unit only
-__global__ void k_reset_state(int B, uint8_t *is_solution, int32_t *first_step)
-{
-    const int b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b < B) { is_solution[b] = 0; first_step[b] = -1; }
-}
-#endif
-
-// The fp32 instantiation of the scalar register kernel is compiled in its own translation unit (afsat_km32.cu) so
-// that the parts of the build run in parallel; everyone else only declares it.
-#ifndef AFSAT_B_KMAX32
-#define AFSAT_B_KMAX32 20             // fp32: the scalar register kernel up to this length (beyond: afsat_split.cuh)
-#endif
-#ifndef AFSAT_B_MINB
-#define AFSAT_B_MINB 1
-#endif
-#ifndef AFSAT_M32_PACKED
-#define AFSAT_M32_PACKED 1             // fp32, 9 <= k <= AFSAT_B_KMAX32: the packed lane-split kernel (afsat_split.cuh)
-#endif                                 // instead of k_eval_km<float>
-#if !defined(AFSAT_KM32_TU) && !AFSAT_M32_PACKED
-extern template __global__ void k_eval_km<float, 9, AFSAT_B_KMAX32, 1, true, AFSAT_B_MINB>(const EvalParams<float>);
-extern template __global__ void k_eval_km<float, 9, AFSAT_B_KMAX32, 1, false, AFSAT_B_MINB>(const EvalParams<float>);
-#endif
+// length classes (afsat.cu class_of): fp32  k <= 5: k_eval_f2m, four candidates per lane | 6..8: k_eval_f2m, two per lane |
+// 9..20: packed lane-split kernel | 21..64: scalar lane-split kernel;  fp64  k <= 8, 9..20: k_eval_km | 21..64: lane-split
+#define AFSAT_S_KMAX 5
+#define AFSAT_A_KMAX 8
+#define AFSAT_B_KMAX 20
 
 }  // namespace afsat

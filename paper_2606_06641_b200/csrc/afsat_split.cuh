@@ -33,18 +33,15 @@ namespace afsat {
 #ifndef AFSAT_M32_THREADS
 #define AFSAT_M32_THREADS 384
 #endif
-#ifndef AFSAT_L64_SPLIT
-#define AFSAT_L64_SPLIT 1              // fp64, k > 20: FOUR lanes per candidate (a double takes two registers)
-#endif
 #ifndef AFSAT_L64_THREADS
 #define AFSAT_L64_THREADS 384             // 168 registers, 12 warps per SM (256 x 255 registers: 4.25 vs 4.07 ms on cfg3)
 #endif
-#define AFSAT_L64_KMIN 21              // = AFSAT_B_KMAX64 + 1 (afsat.cu)
+#define AFSAT_L64_KMIN (AFSAT_B_KMAX + 1)   // fp64, k > 20: FOUR lanes per candidate (a double takes two registers)
 #ifndef AFSAT_L32_PREFETCH
 #define AFSAT_L32_PREFETCH 1
 #endif
 #ifndef AFSAT_L32_KMIN
-#define AFSAT_L32_KMIN (AFSAT_B_KMAX32 + 1)
+#define AFSAT_L32_KMIN (AFSAT_B_KMAX + 1)
 #endif
 
 // product of the OTHER lanes' values (NS = 2: the partner's; NS = 4: butterfly over lane bits log2(CW), log2(CW) + 1)
@@ -159,7 +156,7 @@ __device__ __forceinline__ void eval_points_split(unsigned mask, const T (&y)[KS
     }
 }
 
-template <typename T, int KS, int NS, bool GRAD, bool FIXED>
+template <typename T, int KS, int NS, bool GRAD>
 __device__ __forceinline__ void run_item_split(const EvalParams<T> &p, unsigned mask, const int32_t *__restrict__ s_lits,
                                                const T *__restrict__ s_tab, int n_real, int n_cplx, int nc, int wk,
                                                int h, int64_t b, T &fe, int k)
@@ -175,10 +172,10 @@ __device__ __forceinline__ void run_item_split(const EvalParams<T> &p, unsigned 
         T y[KS], g[KS];
 #pragma unroll
         for (int i = 0; i < KS - 1; ++i) lit[i] = L[i * NS];
-        lit[KS - 1] = miss ? LIT_FIXED : L[(KS - 1) * NS];            // missing literal: constant, no gather, no RED
+        lit[KS - 1] = miss ? LIT_NONE : L[(KS - 1) * NS];             // missing literal: constant, no gather, no RED
 #pragma unroll
         for (int i = 0; i < KS; ++i) {
-            if ((FIXED || i == KS - 1) && (lit[i] & LIT_FIXED)) y[i] = T(1);
+            if (i == KS - 1 && (lit[i] & LIT_NONE)) y[i] = T(1);
             else y[i] = __ldg(reinterpret_cast<const T *>(xb + (uint64_t)(uint32_t)(lit[i] & LIT_VAR) * x_ld));
             y[i] = flip_sign(y[i], lit[i]);
             g[i] = T(0);
@@ -190,7 +187,6 @@ __device__ __forceinline__ void run_item_split(const EvalParams<T> &p, unsigned 
             for (int i = 0; i < KS; ++i) {
                 if (i == KS - 1 && miss) continue;
                 const int32_t ln = Ln[i * NS];
-                if (FIXED && (ln & LIT_FIXED)) continue;
                 asm volatile("prefetch.global.L1 [%0];" ::"l"(xb + (uint64_t)(uint32_t)(ln & LIT_VAR) * x_ld));
             }
         }
@@ -199,7 +195,7 @@ __device__ __forceinline__ void run_item_split(const EvalParams<T> &p, unsigned 
         if (GRAD) {
 #pragma unroll
             for (int i = 0; i < KS; ++i) {
-                if ((FIXED || i == KS - 1) && (lit[i] & LIT_FIXED)) continue;   // masked gradient
+                if (i == KS - 1 && (lit[i] & LIT_NONE)) continue;
                 const T gi[1] = {flip_sign(g[i], lit[i])};
                 VecIO<T, 1>::red(reinterpret_cast<T *>(gb + (uint64_t)(uint32_t)(lit[i] & LIT_VAR) * g_ld), gi);
             }
@@ -209,7 +205,7 @@ __device__ __forceinline__ void run_item_split(const EvalParams<T> &p, unsigned 
 
 template <typename T, int KS, int NS, bool GRAD>
 __device__ __noinline__ void item_body_split(const EvalParams<T> &p, const int32_t *s_lits, const T *s_tab,
-                                             T (*s_F)[32], int n_real, int n_cplx, int nc, bool has_fixed, int k)
+                                             T (*s_F)[32], int n_real, int n_cplx, int nc, int k)
 {
     constexpr int CW = 32 / NS;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -220,8 +216,7 @@ __device__ __noinline__ void item_body_split(const EvalParams<T> &p, const int32
     const unsigned mask = __ballot_sync(0xffffffffu, active);
     T fe = T(0);
     if (active) {
-        if (has_fixed) run_item_split<T, KS, NS, GRAD, true>(p, mask, s_lits, s_tab, n_real, n_cplx, nc, wk, h, b, fe, k);
-        else run_item_split<T, KS, NS, GRAD, false>(p, mask, s_lits, s_tab, n_real, n_cplx, nc, wk, h, b, fe, k);
+        run_item_split<T, KS, NS, GRAD>(p, mask, s_lits, s_tab, n_real, n_cplx, nc, wk, h, b, fe, k);
     }
     if (!p.Fpart) return;
     s_F[warp][lane] = fe;
@@ -306,7 +301,7 @@ __device__ __forceinline__ void eval_points_split2(unsigned mask, const f32x2 (&
     }
 }
 
-template <int KS, int NS, bool GRAD, bool FIXED>
+template <int KS, int NS, bool GRAD>
 __device__ __forceinline__ void run_item_split2(const EvalParams<float> &p, unsigned mask, const int32_t *__restrict__ s_lits,
                                                 const float *__restrict__ s_tab, int n_real, int n_cplx, int nc, int wk,
                                                 int h, int64_t b, f32x2 &fe, int k)
@@ -323,11 +318,11 @@ __device__ __forceinline__ void run_item_split2(const EvalParams<float> &p, unsi
         f32x2 y[KS], g[KS];
 #pragma unroll
         for (int i = 0; i < KS - 1; ++i) lit[i] = L[i * NS];
-        lit[KS - 1] = miss ? LIT_FIXED : L[(KS - 1) * NS];            // missing literal: constant, no gather, no RED
+        lit[KS - 1] = miss ? LIT_NONE : L[(KS - 1) * NS];             // missing literal: constant, no gather, no RED
 #pragma unroll
         for (int i = 0; i < KS; ++i) {
             f32x2 v[1] = {one2};
-            if (!((FIXED || i == KS - 1) && (lit[i] & LIT_FIXED)))
+            if (!(i == KS - 1 && (lit[i] & LIT_NONE)))
                 PairIO<1>::load(xb + (uint64_t)(uint32_t)(lit[i] & LIT_VAR) * x_ld, v);
             const uint32_t m = (uint32_t)(lit[i] & LIT_NEG);
             y[i] = v[0] ^ (((f32x2)m << 32) | m);                     // y = s x
@@ -340,7 +335,6 @@ __device__ __forceinline__ void run_item_split2(const EvalParams<float> &p, unsi
             for (int i = 0; i < KS; ++i) {
                 if (i == KS - 1 && miss) continue;
                 const int32_t ln = Ln[i * NS];
-                if (FIXED && (ln & LIT_FIXED)) continue;
                 asm volatile("prefetch.global.L1 [%0];" ::"l"(xb + (uint64_t)(uint32_t)(ln & LIT_VAR) * x_ld));
             }
         }
@@ -349,7 +343,7 @@ __device__ __forceinline__ void run_item_split2(const EvalParams<float> &p, unsi
         if (GRAD) {
 #pragma unroll
             for (int i = 0; i < KS; ++i) {
-                if ((FIXED || i == KS - 1) && (lit[i] & LIT_FIXED)) continue;   // masked gradient
+                if (i == KS - 1 && (lit[i] & LIT_NONE)) continue;
                 const uint32_t m = (uint32_t)(lit[i] & LIT_NEG);
                 const f32x2 gi[1] = {g[i] ^ (((f32x2)m << 32) | m)};
                 PairIO<1>::red(gb + (uint64_t)(uint32_t)(lit[i] & LIT_VAR) * g_ld, gi);
@@ -360,7 +354,7 @@ __device__ __forceinline__ void run_item_split2(const EvalParams<float> &p, unsi
 
 template <int KS, int NS, bool GRAD>
 __device__ __noinline__ void item_body_split2(const EvalParams<float> &p, const int32_t *s_lits, const float *s_tab,
-                                              float (*s_F)[64], int n_real, int n_cplx, int nc, bool has_fixed, int k)
+                                              float (*s_F)[64], int n_real, int n_cplx, int nc, int k)
 {
     constexpr int CW = 32 / NS;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -371,8 +365,7 @@ __device__ __noinline__ void item_body_split2(const EvalParams<float> &p, const 
     const unsigned mask = __ballot_sync(0xffffffffu, active);
     f32x2 fe2 = 0ull;
     if (active) {
-        if (has_fixed) run_item_split2<KS, NS, GRAD, true>(p, mask, s_lits, s_tab, n_real, n_cplx, nc, wk, h, b, fe2, k);
-        else run_item_split2<KS, NS, GRAD, false>(p, mask, s_lits, s_tab, n_real, n_cplx, nc, wk, h, b, fe2, k);
+        run_item_split2<KS, NS, GRAD>(p, mask, s_lits, s_tab, n_real, n_cplx, nc, wk, h, b, fe2, k);
     }
     if (!p.Fpart) return;
     float f0, f1; upk(fe2, f0, f1);
@@ -391,13 +384,13 @@ __device__ __noinline__ void item_body_split2(const EvalParams<float> &p, const 
 template <typename T, int KS, int KSHI, int NS, int V, bool GRAD>
 struct SwitchSplit {
     static __device__ __forceinline__ void go(int ks, const EvalParams<T> &p, const int32_t *s_lits, const T *s_tab,
-                                              T (*s_F)[32 * V], int n_real, int n_cplx, int nc, bool has_fixed, int k)
+                                              T (*s_F)[32 * V], int n_real, int n_cplx, int nc, int k)
     {
         if (ks == KS) {
-            if constexpr (V == 2) item_body_split2<KS, NS, GRAD>(p, s_lits, s_tab, s_F, n_real, n_cplx, nc, has_fixed, k);
-            else item_body_split<T, KS, NS, GRAD>(p, s_lits, s_tab, s_F, n_real, n_cplx, nc, has_fixed, k);
+            if constexpr (V == 2) item_body_split2<KS, NS, GRAD>(p, s_lits, s_tab, s_F, n_real, n_cplx, nc, k);
+            else item_body_split<T, KS, NS, GRAD>(p, s_lits, s_tab, s_F, n_real, n_cplx, nc, k);
         } else if (KS < KSHI)
-            SwitchSplit<T, (KS < KSHI ? KS + 1 : KS), KSHI, NS, V, GRAD>::go(ks, p, s_lits, s_tab, s_F, n_real, n_cplx, nc, has_fixed, k);
+            SwitchSplit<T, (KS < KSHI ? KS + 1 : KS), KSHI, NS, V, GRAD>::go(ks, p, s_lits, s_tab, s_F, n_real, n_cplx, nc, k);
     }
 };
 
@@ -413,20 +406,16 @@ __global__ void __launch_bounds__(THREADS, MINB) k_eval_split(const EvalParams<T
     stage_item(p, it, sg, s_tab, s_lits);
     __syncthreads();
     SwitchSplit<T, (KLO + NS - 1) / NS, (KHI + NS - 1) / NS, NS, V, GRAD>::go((it.k + NS - 1) / NS, p, s_lits, s_tab, s_F, sg.n_real,
-                                                                        sg.n_cplx, it.c_end - it.c_begin, it.has_fixed != 0, it.k);
+                                                                        sg.n_cplx, it.c_end - it.c_begin, it.k);
 }
 
 #ifndef AFSAT_KS32_TU   // instantiated in afsat_ks32.cu
 extern template __global__ void k_eval_split<float, AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, 1, true, AFSAT_L32_THREADS, AFSAT_L32_MINB>(const EvalParams<float>);
 extern template __global__ void k_eval_split<float, AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, 1, false, AFSAT_L32_THREADS, AFSAT_L32_MINB>(const EvalParams<float>);
-#if AFSAT_L64_SPLIT
 extern template __global__ void k_eval_split<double, AFSAT_L64_KMIN, AFSAT_MAX_LEN, 4, 1, true, AFSAT_L64_THREADS, 1>(const EvalParams<double>);
 extern template __global__ void k_eval_split<double, AFSAT_L64_KMIN, AFSAT_MAX_LEN, 4, 1, false, AFSAT_L64_THREADS, 1>(const EvalParams<double>);
-#endif
-#if AFSAT_M32_PACKED
-extern template __global__ void k_eval_split<float, 9, AFSAT_B_KMAX32, 2, 2, true, AFSAT_M32_THREADS, 1>(const EvalParams<float>);
-extern template __global__ void k_eval_split<float, 9, AFSAT_B_KMAX32, 2, 2, false, AFSAT_M32_THREADS, 1>(const EvalParams<float>);
-#endif
+extern template __global__ void k_eval_split<float, AFSAT_A_KMAX + 1, AFSAT_B_KMAX, 2, 2, true, AFSAT_M32_THREADS, 1>(const EvalParams<float>);
+extern template __global__ void k_eval_split<float, AFSAT_A_KMAX + 1, AFSAT_B_KMAX, 2, 2, false, AFSAT_M32_THREADS, 1>(const EvalParams<float>);
 #endif
 
 }  // namespace afsat

@@ -1,0 +1,579 @@
+// afsat_step.cuh -- the non-evaluation kernels of the path: projected step, sign rounding,
+// exact discrete count, per-candidate state, line-search bookkeeping, restarts; plus the ONE-LAUNCH step loop for
+// small instances (k_step_small) and the FP-pipe peak probes.  Included by afsat.cu only.
+#pragma once
+#include "afsat_kernels.cuh"
+
+namespace afsat {
+
+// ---- a7: sign rounding as one bit per (variable, candidate): bits[v][b / 32] bit (b % 32) = (x < 0)
+template <typename T>
+__global__ void __launch_bounds__(CTA_THREADS) k_pack_signs(const T *__restrict__ x, uint32_t *__restrict__ bits, int n,
+                                                           int B, int64_t ldb)
+{
+    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= ldb) return;                                             // whole warps (ldb % 32 == 0)
+    const int64_t ldw = ldb >> 5;
+    for (int v = blockIdx.y; v < n; v += gridDim.y) {
+        const bool t = (b < B) && (x[(int64_t)v * ldb + b] < T(0));   // True iff x < 0 (0, -0.0 -> False)
+        const uint32_t w = __ballot_sync(0xffffffffu, t);
+        if ((threadIdx.x & 31) == 0) bits[(int64_t)v * ldw + (b >> 5)] = w;
+    }
+}
+
+// ---- a6 + a7 + a9: projected step on the candidate tile [b_begin, b_end), gradient scratch reset, sign bits of the
+// NEW x.  Frozen (solved) candidates and fixed variables keep their x.  A thread owns VW = 16 / sizeof(T) ADJACENT
+// candidates (one 16-byte load / store per array and row), tpr threads span a row of the tile, a CTA pass covers
+// CTA_THREADS / tpr rows and every thread keeps UPD_UNROLL rows in flight.  The sign bits of a 32-candidate word come
+// from the 32 / VW lanes that hold it (one REDUX.OR).
+constexpr int UPD_UNROLL = 4;
+template <typename T> struct Vec16;
+template <> struct Vec16<float>  { typedef float4 type;  static constexpr int VW = 4; };
+template <> struct Vec16<double> { typedef double2 type; static constexpr int VW = 2; };
+__device__ __forceinline__ void vec_get(const float4 &v, float (&a)[4]) { a[0] = v.x; a[1] = v.y; a[2] = v.z; a[3] = v.w; }
+__device__ __forceinline__ void vec_get(const double2 &v, double (&a)[2]) { a[0] = v.x; a[1] = v.y; }
+__device__ __forceinline__ float4 vec_make(const float (&a)[4]) { return make_float4(a[0], a[1], a[2], a[3]); }
+__device__ __forceinline__ double2 vec_make(const double (&a)[2]) { return make_double2(a[0], a[1]); }
+
+template <typename T>
+__global__ void __launch_bounds__(CTA_THREADS) k_update(T *__restrict__ x, T *__restrict__ G, int64_t g_ld, int64_t g_b0,
+                                                       const int8_t *__restrict__ fixed,
+                                                       const uint8_t *__restrict__ is_solution, uint32_t *__restrict__ bits,
+                                                       T eta, int n, int B, int64_t ldb, int64_t b_begin, int64_t b_end,
+                                                       int tpr)
+{
+    typedef typename Vec16<T>::type VT;
+    constexpr int VW = Vec16<T>::VW, LPW = 32 / VW;                   // lanes per 32-candidate word
+    const int col = threadIdx.x % tpr, r = threadIdx.x / tpr, rows_per_pass = blockDim.x / tpr;
+    const int64_t b = b_begin + ((int64_t)blockIdx.x * tpr + col) * VW;
+    if (b >= b_end) return;                                           // tiles are multiples of 32 candidates: whole word groups
+    bool live[VW], upd[VW], any_upd = false;
+#pragma unroll
+    for (int j = 0; j < VW; ++j) {
+        live[j] = b + j < B;
+        upd[j] = live[j] && !is_solution[b + j];
+        any_upd |= upd[j];
+    }
+    const int lane = threadIdx.x & 31;
+    const unsigned wmask = ((LPW == 32) ? 0xffffffffu : ((1u << LPW) - 1u)) << (lane / LPW * LPW);
+    const int sh = (lane % LPW) * VW;
+    const int64_t ldw = ldb >> 5;
+    const int stride = gridDim.y * rows_per_pass;
+    for (int v0 = blockIdx.y * rows_per_pass + r; v0 < n; v0 += stride * UPD_UNROLL) {
+        VT g[UPD_UNROLL], xv[UPD_UNROLL];
+        int8_t fx[UPD_UNROLL];
+#pragma unroll
+        for (int u = 0; u < UPD_UNROLL; ++u) {
+            const int v = v0 + u * stride;
+            if (v < n) {
+                g[u] = *reinterpret_cast<const VT *>(G + (int64_t)v * g_ld + (b - g_b0));
+                xv[u] = *reinterpret_cast<const VT *>(x + (int64_t)v * ldb + b);
+                fx[u] = fixed[v];
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < UPD_UNROLL; ++u) {
+            const int v = v0 + u * stride;
+            if (v < n) {                                              // uniform over the lanes of a word (same row)
+                T gv[VW], xs[VW];
+                vec_get(g[u], gv); vec_get(xv[u], xs);
+                T zero[VW];
+#pragma unroll
+                for (int j = 0; j < VW; ++j) zero[j] = T(0);
+                *reinterpret_cast<VT *>(G + (int64_t)v * g_ld + (b - g_b0)) = vec_make(zero);
+                uint32_t nib = 0u;
+#pragma unroll
+                for (int j = 0; j < VW; ++j) {
+                    T nx = xs[j];
+                    if (upd[j] && !fx[u]) {
+                        nx = fma_(-eta, gv[j], nx);
+                        nx = nx > T(1) ? T(1) : nx;
+                        nx = nx < T(-1) ? T(-1) : nx;
+                    }
+                    xs[j] = nx;
+                    nib |= (uint32_t)(live[j] && (nx < T(0))) << j;
+                }
+                if (any_upd && !fx[u]) *reinterpret_cast<VT *>(x + (int64_t)v * ldb + b) = vec_make(xs);
+                const uint32_t w = __reduce_or_sync(wmask, nib << sh);
+                if (lane % LPW == 0) bits[(int64_t)v * ldw + (b >> 5)] = w;
+            }
+        }
+    }
+}
+
+// ---- a8: exact discrete count, integer only.  One thread = one 32-candidate word; the number tau
+// of true literals is kept BIT-SLICED (t[j] holds bit j of tau for 32 candidates), the predicate is
+// evaluated by scanning the smaller of {satisfied counts, violated counts}, and the per-candidate
+// number of satisfied constraints of the item is again a bit-sliced counter.  The bit rows of a constraint's
+// literals are requested CHK_MLP at a time before any is consumed (the kernel is bound by the latency of those loads).
+struct CheckParams {
+    const uint32_t *bits;       // [n][ldw]
+    int64_t ldw;
+    const int32_t *lits;
+    const SigDev *sigs;
+    const Item *items;
+    int32_t *satacc;            // [ldb]
+    int32_t B;
+    int32_t w_begin, w_end;     // word range of this launch
+    int32_t wpb;                // words per CTA (power of two <= 32)
+    int32_t n_items;
+    int32_t *step_ctr;          // or null: incremented once per launch (the step index of a replayed CUDA graph)
+};
+constexpr int CHK_MLP = 8;
+
+__global__ void __launch_bounds__(CTA_THREADS) k_check_bits(const CheckParams p)
+{
+    __shared__ int32_t s_lits[LIT_CHUNK];
+    __shared__ int32_t s_cnt[32 * 32];
+    if (p.step_ctr && blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) ++p.step_ctr[0];
+    for (int i = threadIdx.x; i < p.wpb * 32; i += blockDim.x) s_cnt[i] = 0;
+    const int wi = threadIdx.x % p.wpb, grp = threadIdx.x / p.wpb, ngrp = blockDim.x / p.wpb;
+    const int word = p.w_begin + blockIdx.y * p.wpb + wi;
+    const bool valid = word < p.w_end;
+    const uint32_t *bw = p.bits + (valid ? word : p.w_begin);
+    uint32_t cnt[13];
+#pragma unroll
+    for (int j = 0; j < 13; ++j) cnt[j] = 0u;
+    int nacc = 0;                                                     // constraints counted in cnt[] so far
+    auto flush = [&]() {                                              // bit-sliced counter -> per-candidate integers
+        for (int bit = 0; bit < 32; ++bit) {
+            int val = 0;
+#pragma unroll
+            for (int j = 0; j < 13; ++j) val |= (int)((cnt[j] >> bit) & 1u) << j;
+            if (val) atomicAdd(&s_cnt[wi * 32 + bit], val);
+        }
+#pragma unroll
+        for (int j = 0; j < 13; ++j) cnt[j] = 0u;
+        nacc = 0;
+    };
+    for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {   // persistent over work items
+        const Item it = p.items[item];
+        const SigDev sg = p.sigs[it.sig];
+        const int k = it.k, nc = it.c_end - it.c_begin;
+        __syncthreads();                                              // previous item's literals are consumed
+        for (int i = threadIdx.x; i < nc * k; i += blockDim.x) s_lits[i] = __ldg(p.lits + it.lit_base + i);
+        __syncthreads();
+        if (!valid) continue;
+        int nb = 1;
+        while ((1 << nb) <= k) ++nb;                                  // bits of tau in [0, k]
+        const int mine = (nc - grp + ngrp - 1) / ngrp;
+        if (nacc + mine > 8191) flush();
+        nacc += mine > 0 ? mine : 0;
+        for (int c = grp; c < nc; c += ngrp) {
+            uint32_t t[7] = {0u, 0u, 0u, 0u, 0u, 0u, 0u};
+            const int32_t *L = s_lits + c * k;
+            for (int i0 = 0; i0 < k; i0 += CHK_MLP) {
+                uint32_t mm[CHK_MLP];
+#pragma unroll
+                for (int u = 0; u < CHK_MLP; ++u) {
+                    mm[u] = 0u;
+                    if (i0 + u < k) {
+                        const int32_t lit = L[i0 + u];
+                        const uint32_t w = __ldg(bw + (int64_t)(lit & LIT_VAR) * p.ldw);
+                        mm[u] = lit < 0 ? ~w : w;                     // literal true = variable true XOR negated
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < CHK_MLP; ++u) {
+                    uint32_t m = mm[u];
+#pragma unroll
+                    for (int j = 0; j < 7; ++j)
+                        if (j < nb) { const uint32_t s = t[j] ^ m; m &= t[j]; t[j] = s; }
+                }
+            }
+            uint32_t acc = 0u;
+            for (int tau = 0; tau <= k; ++tau) {
+                const uint64_t bit = tau < 64 ? (sg.scan_lo >> tau) : (sg.scan_hi >> (tau - 64));
+                if (!(bit & 1ull)) continue;
+                uint32_t eq = 0xffffffffu;
+#pragma unroll
+                for (int j = 0; j < 7; ++j)
+                    if (j < nb) eq &= ((tau >> j) & 1) ? t[j] : ~t[j];
+                acc |= eq;
+            }
+            uint32_t carry = sg.scan_is_sat ? acc : ~acc;             // 1 = constraint satisfied
+#pragma unroll
+            for (int j = 0; j < 13; ++j) { const uint32_t s = cnt[j] ^ carry; carry &= cnt[j]; cnt[j] = s; }
+        }
+    }
+    if (valid && nacc) flush();
+    __syncthreads();
+    const int64_t b0 = ((int64_t)p.w_begin + (int64_t)blockIdx.y * p.wpb) * 32;
+    for (int i = threadIdx.x; i < p.wpb * 32; i += blockDim.x) {
+        const int64_t b = b0 + i;
+        if (b < p.B && b < (int64_t)p.w_end * 32 && s_cnt[i]) atomicAdd(p.satacc + b, s_cnt[i]);
+    }
+}
+
+// ---- line search (afsat_step_ls; reading B5): per-candidate backtracking along the projection arc ----
+// ls_state[b]: 0 = still searching, 1 = step accepted, 2 = frozen (solved or converged)
+constexpr int LS_CHUNKS = 32;         // row chunks of the <G, X - X'> reduction (fixed-order two-stage sum)
+
+__global__ void k_ls_begin(int B, int64_t ldb, const uint8_t *__restrict__ is_solution, const uint8_t *__restrict__ converged,
+                           uint8_t *__restrict__ ls_state, double s_max, double *__restrict__ eta)
+{
+    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= ldb) return;
+    ls_state[b] = (b >= B || is_solution[b] || converged[b]) ? 2 : 0;
+    eta[b] = s_max;
+}
+
+// the partial assignment of candidate b: fixed[(b / group_w) * n + v]  (several partial assignments)
+__device__ __forceinline__ const int8_t *fixed_of(const int8_t *fixed, int64_t b, int64_t group_w, int n_groups, int n)
+{
+    int64_t g = b / group_w;
+    if (g >= n_groups) g = n_groups - 1;
+    return fixed + g * (int64_t)n;
+}
+
+// X' = clamp(X - eta_b G) for the candidates still searching (first trial: every candidate gets a valid X'),
+// Dpart[chunk][b] = sum over the chunk's rows of G (X - X')
+template <typename T>
+__global__ void __launch_bounds__(CTA_THREADS) k_ls_trial(const T *__restrict__ x, const T *__restrict__ G, T *__restrict__ xt,
+                                                         const int8_t *__restrict__ fixed_all, int64_t group_w, int n_groups,
+                                                         const uint8_t *__restrict__ ls_state,
+                                                         const double *__restrict__ eta, double *__restrict__ Dpart, int n,
+                                                         int64_t ldb, int first_trial)
+{
+    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= ldb) return;
+    const int st = ls_state[b];
+    const int rows = (n + LS_CHUNKS - 1) / LS_CHUNKS, v0 = blockIdx.y * rows, v1 = min(n, v0 + rows);
+    if (st != 0) {
+        if (first_trial) for (int v = v0; v < v1; ++v) xt[(int64_t)v * ldb + b] = x[(int64_t)v * ldb + b];
+        return;
+    }
+    const int8_t *fixed = fixed_of(fixed_all, b, group_w, n_groups, n);
+    const T e = (T)eta[b];
+    double D = 0.0;
+    for (int v = v0; v < v1; ++v) {
+        const T xv = x[(int64_t)v * ldb + b];
+        T nx = xv;
+        if (!fixed[v]) {
+            const T g = G[(int64_t)v * ldb + b];
+            nx = fma_(-e, g, xv);
+            nx = nx > T(1) ? T(1) : nx;
+            nx = nx < T(-1) ? T(-1) : nx;
+            D += (double)g * (double)(xv - nx);
+        }
+        xt[(int64_t)v * ldb + b] = nx;
+    }
+    Dpart[(int64_t)blockIdx.y * ldb + b] = D;
+}
+
+// Armijo test of the trial; backtrack or give up (eta < delta: converged)
+template <typename T>
+__global__ void k_ls_decide(int B, int64_t ldb, const T *__restrict__ F0, const T *__restrict__ F1, const double *__restrict__ Dpart,
+                            uint8_t *__restrict__ ls_state, double *__restrict__ eta, uint8_t *__restrict__ converged, double c1,
+                            double beta, double delta)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= B || ls_state[b] != 0) return;
+    double D = 0.0;
+    for (int c = 0; c < LS_CHUNKS; ++c) D += Dpart[(int64_t)c * ldb + b];
+    if ((double)F1[b] <= (double)F0[b] - c1 * D) { ls_state[b] = 1; return; }
+    const double e = eta[b] * beta;
+    eta[b] = e;
+    if (e < delta) { ls_state[b] = 2; converged[b] = 1; }
+}
+
+// accepted candidates take X', sign bits of the resulting X for everyone
+template <typename T>
+__global__ void __launch_bounds__(CTA_THREADS) k_ls_commit(T *__restrict__ x, const T *__restrict__ xt, const uint8_t *__restrict__ ls_state,
+                                                          uint32_t *__restrict__ bits, int n, int B, int64_t ldb)
+{
+    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= ldb) return;                                             // whole warps (ldb % 32 == 0)
+    const bool live = b < B, take = live && ls_state[b] == 1;
+    const int64_t ldw = ldb >> 5;
+    for (int v = blockIdx.y; v < n; v += gridDim.y) {
+        T xv = T(0);
+        if (live) {
+            xv = take ? xt[(int64_t)v * ldb + b] : x[(int64_t)v * ldb + b];
+            if (take) x[(int64_t)v * ldb + b] = xv;
+        }
+        const uint32_t w = __ballot_sync(0xffffffffu, live && xv < T(0));
+        if ((threadIdx.x & 31) == 0) bits[(int64_t)v * ldw + (b >> 5)] = w;
+    }
+}
+
+template <typename T>
+__global__ void k_ls_report(int B, const double *__restrict__ eta, T *__restrict__ eta_out)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b < B) eta_out[b] = (T)eta[b];
+}
+
+// ---- afsat_restart: counter-based uniform re-initialisation (include/afsat.h states the generator) ----
+__device__ __forceinline__ uint32_t fmix32(uint32_t h)
+{
+    h ^= h >> 16; h *= 0x85EBCA6Bu; h ^= h >> 13; h *= 0xC2B2AE35u; h ^= h >> 16;
+    return h;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(CTA_THREADS) k_restart(T *__restrict__ x, const int8_t *__restrict__ fixed_all, int64_t group_w,
+                                                        int n_groups, const uint8_t *__restrict__ keep, uint32_t lo, uint32_t hi,
+                                                        uint32_t round, int n, int B, int64_t ldb)
+{
+    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= B || (keep && keep[b])) return;
+    const int8_t *fixed = fixed_of(fixed_all, b, group_w, n_groups, n);
+    const uint32_t hb = fmix32(lo ^ ((uint32_t)b * 0x9E3779B9u));
+    for (int v = blockIdx.y; v < n; v += gridDim.y) {
+        const int8_t f = fixed[v];
+        T val;
+        if (f) val = (T)f;
+        else {
+            const uint32_t h = fmix32(fmix32((hb + (uint32_t)v * 0x85EBCA6Bu) ^ hi) + round * 0xC2B2AE35u);
+            val = (T)((float)(h >> 8) * 1.1920928955078125e-07f - 1.0f);     // (h >> 8) 2^-23 - 1, exact
+        }
+        x[(int64_t)v * ldb + b] = val;
+    }
+}
+
+// zero the padding columns [B, ldb) of a caller-owned gradient (vector REDs of a lane pair that
+// straddles B spill into them)
+template <typename T>
+__global__ void k_zero_pad(T *__restrict__ G, int n, int B, int64_t ldb)
+{
+    const int64_t np = ldb - B;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < (int64_t)n * np; i += (int64_t)gridDim.x * blockDim.x)
+        G[(i / np) * ldb + B + (i % np)] = T(0);
+}
+
+// ---- F[b] = F_const + sum over items of Fpart[item][b], fixed order, accumulated in double, for the candidates
+// [b0, b1) of one partial-assignment group (F_const: the constraints the partial assignment already decides) ----
+template <typename T>
+__global__ void k_reduce_F(const T *__restrict__ Fpart, int n_rows, int64_t ldb, int64_t b0, int64_t b1, double F_const,
+                           T *__restrict__ F, const uint8_t *__restrict__ skip)
+{
+    const int64_t b = b0 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= b1 || (skip && skip[b])) return;                          // skipped candidates keep their F
+    double s = F_const;
+    for (int i = 0; i < n_rows; ++i) s += (double)Fpart[(int64_t)i * ldb + b];
+    F[b] = (T)s;
+}
+
+// ---- per-candidate state machine of Alg. 1 (a8, a9): satacc holds the count on the current X over the constraints
+// that reach a kernel; sat_const[g] adds the ones group g's partial assignment satisfies outright ----
+// d_any: {flag, first step, -, step counter}
+__global__ void k_flags(int32_t *__restrict__ satacc, int B, int m, int mark_solved, int step_value, const int32_t *step_ctr,
+                        const int32_t *__restrict__ sat_const, int64_t group_w, int n_groups,
+                        int32_t *__restrict__ sat_count, uint8_t *__restrict__ is_solution,
+                        int32_t *__restrict__ first_step, int32_t *__restrict__ d_any, volatile int32_t *h_any)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= B) return;
+    if (step_ctr) step_value = step_ctr[0];
+    int64_t g = b / group_w;
+    if (g >= n_groups) g = n_groups - 1;
+    const int s = satacc[b] + sat_const[g];
+    satacc[b] = 0;
+    sat_count[b] = s;
+    if (mark_solved && s == m && !is_solution[b]) {
+        is_solution[b] = 1;
+        first_step[b] = step_value;
+        if (atomicCAS(d_any, 0, 1) == 0) {
+            d_any[1] = step_value;
+            if (h_any) { h_any[1] = step_value; __threadfence_system(); h_any[0] = 1; }
+        }
+    }
+}
+
+// afsat_check epilogue: counts out, is_solution = (count == m), accumulator reset.
+__global__ void k_check_finish(int32_t *__restrict__ satacc, int B, int m, const int32_t *__restrict__ sat_const, int64_t group_w,
+                               int n_groups, int32_t *__restrict__ sat_count, uint8_t *__restrict__ is_solution)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= B) return;
+    int64_t g = b / group_w;
+    if (g >= n_groups) g = n_groups - 1;
+    const int s = satacc[b] + sat_const[g];
+    satacc[b] = 0;
+    sat_count[b] = s;
+    is_solution[b] = (uint8_t)(s == m);
+}
+
+// start of a step call, ON THE STREAM: per-candidate state (unless resuming), the any-solved flag on the device and
+// in the caller's pinned host memory, the step counter of a replayed graph
+__global__ void k_reset_state(int B, int reset_candidates, uint8_t *is_solution, int32_t *first_step, int32_t *d_any,
+                              volatile int32_t *h_any, int step_base)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (reset_candidates && b < B) { is_solution[b] = 0; first_step[b] = -1; }
+    if (b == 0) {
+        d_any[0] = 0; d_any[1] = 0x7fffffff; d_any[2] = 0; d_any[3] = step_base;
+        if (h_any) { h_any[0] = 0; h_any[1] = -1; }
+    }
+}
+
+// ---- the whole step loop in ONE launch (small instances: PAPER.md:81 "compiled once and executed repeatedly", :103
+// the lock-step loop runs on the accelerator) ------------------------------------------------
+// A CTA owns 32 candidates (lane = candidate) for all n_steps iterations: X and G of those candidates live in shared
+// memory as [n][32] columns, the warps share out the constraints, partial gradients meet in shared-memory atomics, and
+// the gather of iteration t + 1 also yields the sign bits of X(t), so the exact count (a8) rides on the same pass.
+// Candidates never exchange data, so no CTA waits on another.  Lengths k <= 8 only (one register body per length).
+template <typename T>
+struct SmallParams {
+    T *x;                       // [n][ldb], in/out
+    int64_t ldb;
+    int32_t n, B, m, n_items;
+    const int32_t *lits;
+    const Item *items;
+    const SigDev *sigs;
+    const T *rows;
+    const int8_t *fixed;
+    T eta;
+    int32_t n_steps, step_base, sat_const, n_ctas;
+    int32_t *sat_count;
+    uint8_t *is_solution;
+    int32_t *first_step;
+    int32_t *d_any;             // {flag, first step (min), finished CTAs, -}
+    volatile int32_t *h_any;
+};
+constexpr int SMALL_THREADS = 512;
+
+template <typename T, int K, bool GRAD>
+__device__ __forceinline__ int small_constraint(const int32_t *__restrict__ L, const T *__restrict__ sx, T *__restrict__ sg,
+                                                const T *__restrict__ tab, const SigDev &sg_, int lane)
+{
+    int32_t lit[K];
+    T y[K][1], g[K][1], fe[1] = {T(0)};
+    int tau = 0;
+#pragma unroll
+    for (int i = 0; i < K; ++i) {
+        lit[i] = __ldg(L + i);
+        const T xv = sx[(lit[i] & LIT_VAR) * 32 + lane];
+        tau += (int)((xv < T(0)) != (lit[i] < 0));                    // literal true = variable true XOR negated (B2)
+        y[i][0] = flip_sign(xv, lit[i]);
+        g[i][0] = T(0);
+    }
+    if (GRAD) {
+        eval_points_reg<T, K, 1, true>(y, tab, sg_.n_real, sg_.n_cplx, fe, g);
+#pragma unroll
+        for (int i = 0; i < K; ++i) atomicAdd(sg + (lit[i] & LIT_VAR) * 32 + lane, flip_sign(g[i][0], lit[i]));
+    }
+    const uint64_t bit = tau < 64 ? (sg_.scan_lo >> tau) : (sg_.scan_hi >> (tau - 64));
+    return (int)(bit & 1ull) == sg_.scan_is_sat;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(SMALL_THREADS, 1) k_step_small(const SmallParams<T> p)
+{
+    extern __shared__ __align__(16) unsigned char s_raw[];
+    T *sx = reinterpret_cast<T *>(s_raw), *sg = sx + (size_t)p.n * 32;
+    __shared__ int s_cnt[32], s_frozen[32];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = blockDim.x >> 5;
+    const int64_t b0 = (int64_t)blockIdx.x * 32, b = b0 + lane;
+    const bool live = b < p.B;
+    for (int i = threadIdx.x; i < p.n * 32; i += blockDim.x) sx[i] = p.x[(int64_t)(i >> 5) * p.ldb + b0 + (i & 31)];
+    if (warp == 0) s_frozen[lane] = live ? (int)p.is_solution[b] : 1;
+    int last = 0;
+    for (int it = 0; it <= p.n_steps; ++it) {
+        const bool grad = it < p.n_steps;
+        if (grad) for (int i = threadIdx.x; i < p.n * 32; i += blockDim.x) sg[i] = T(0);
+        if (warp == 0) s_cnt[lane] = 0;
+        __syncthreads();
+        int cnt = 0;
+        for (int item = 0; item < p.n_items; ++item) {
+            const Item itm = p.items[item];
+            const SigDev sd = p.sigs[itm.sig];
+            const T *tab = p.rows + (int64_t)sd.row_off * 8;
+            const int nc = itm.c_end - itm.c_begin, k = itm.k;
+            int c = (warp - itm.c_begin % nw + nw) % nw;              // constraint (c_begin + c) belongs to warp (c_begin + c) % nw
+            for (; c < nc; c += nw) {
+                const int32_t *L = p.lits + itm.lit_base + (int64_t)c * k;
+#define AFSAT_SMALL_CASE(K_) case K_: cnt += grad ? small_constraint<T, K_, true>(L, sx, sg, tab, sd, lane) \
+                                                  : small_constraint<T, K_, false>(L, sx, sg, tab, sd, lane); break;
+                switch (k) {
+                    AFSAT_SMALL_CASE(1) AFSAT_SMALL_CASE(2) AFSAT_SMALL_CASE(3) AFSAT_SMALL_CASE(4)
+                    AFSAT_SMALL_CASE(5) AFSAT_SMALL_CASE(6) AFSAT_SMALL_CASE(7) AFSAT_SMALL_CASE(8)
+                }
+#undef AFSAT_SMALL_CASE
+            }
+        }
+        if (cnt) atomicAdd(&s_cnt[lane], cnt);
+        __syncthreads();
+        if (warp == 0) {                                              // a8, a9 on X(it): X(0) is counted but not marked (A11)
+            last = s_cnt[lane] + p.sat_const;
+            if (live && it >= 1 && last == p.m && !s_frozen[lane]) {
+                s_frozen[lane] = 1;
+                p.is_solution[b] = 1;
+                const int step = p.step_base + it;
+                p.first_step[b] = step;
+                atomicExch(p.d_any, 1);
+                const int prev = atomicMin(p.d_any + 1, step);
+                if (p.h_any && step < prev) { p.h_any[1] = step; __threadfence_system(); p.h_any[0] = 1; }
+            }
+        }
+        if (!grad) break;
+        __syncthreads();
+        for (int i = threadIdx.x; i < p.n * 32; i += blockDim.x) {    // a6: projected step in shared memory
+            const int v = i >> 5;
+            if (!s_frozen[i & 31] && !p.fixed[v]) {
+                T nx = fma_(-p.eta, sg[i], sx[i]);
+                nx = nx > T(1) ? T(1) : nx;
+                nx = nx < T(-1) ? T(-1) : nx;
+                sx[i] = nx;
+            }
+        }
+        __syncthreads();
+    }
+    if (warp == 0 && live) p.sat_count[b] = last;
+    __syncthreads();
+    for (int i = threadIdx.x; i < p.n * 32; i += blockDim.x)
+        if (b0 + (i & 31) < p.B) p.x[(int64_t)(i >> 5) * p.ldb + b0 + (i & 31)] = sx[i];
+    if (threadIdx.x == 0 && p.h_any) {                                // the last CTA settles the host copy of the first step
+        __threadfence();
+        if (atomicAdd(p.d_any + 2, 1) == p.n_ctas - 1 && p.d_any[0]) {
+            p.h_any[1] = atomicMin(p.d_any + 1, 0x7fffffff);
+            __threadfence_system();
+            p.h_any[0] = 1;
+        }
+    }
+}
+
+// ---- FP-pipe peak probes (afsat_probe_peak): independent FMA chains, nothing else ----------------------------------
+// kind 0: scalar FFMA, 1: packed FFMA2 (fma.rn.f32x2), 2: DFMA.  Every thread runs 8 independent chains.
+template <int KIND>
+__global__ void __launch_bounds__(256) k_probe(float *out, int iters, float seed)
+{
+    if (KIND == 0) {
+        float a[8], m = seed, c = 0.5f;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) a[j] = seed + j;
+        for (int i = 0; i < iters; ++i)
+#pragma unroll
+            for (int j = 0; j < 8; ++j) a[j] = fmaf(a[j], m, c);
+        float s = 0.f;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) s += a[j];
+        if (s == 12345.678f) out[0] = s;
+    } else if (KIND == 1) {
+        f32x2 a[8];
+        const f32x2 m = pk(seed, seed), c = pk(0.5f, 0.25f);
+#pragma unroll
+        for (int j = 0; j < 8; ++j) a[j] = pk(seed + j, seed - j);
+        for (int i = 0; i < iters; ++i)
+#pragma unroll
+            for (int j = 0; j < 8; ++j) a[j] = fma2(a[j], m, c);
+        f32x2 s = 0ull;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) s = add2(s, a[j]);
+        if (s == 0x123456789ull) out[0] = 1.f;
+    } else {
+        double a[8], m = seed, c = 0.5;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) a[j] = seed + j;
+        for (int i = 0; i < iters; ++i)
+#pragma unroll
+            for (int j = 0; j < 8; ++j) a[j] = fma(a[j], m, c);
+        double s = 0.;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) s += a[j];
+        if (s == 12345.678) out[0] = (float)s;
+    }
+}
+
+}  // namespace afsat

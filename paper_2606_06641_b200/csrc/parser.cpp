@@ -123,7 +123,13 @@ int add_constraint(afsat_problem *P, int type, long long t, std::vector<int32_t>
                 if (vars[i] == vars[j]) return fail(P, AFSAT_E_DUPLICATE, line, "variable repeated inside a constraint");
     }
     const int k = (int)vars.size();
-    if (k > AFSAT_MAX_LEN) return fail(P, AFSAT_E_LENGTH, line, "constraint longer than AFSAT_MAX_LEN");
+    // the length limit binds only what reaches a kernel: constraints that A.1 turns into prefix assignments or discards
+    // may be longer
+    auto emit_c = [&](int ty, int prm) {
+        if (k > AFSAT_MAX_LEN) return fail(P, AFSAT_E_LENGTH, line, "constraint longer than AFSAT_MAX_LEN");
+        emit(P, ty, prm, vars, signs);
+        return (int)AFSAT_OK;
+    };
     auto all = [&](bool lit_true) {
         for (int i = 0; i < k; ++i) { int rc = assign(P, vars[i], signs[i], lit_true, line); if (rc) return rc; }
         return (int)AFSAT_OK;
@@ -131,31 +137,26 @@ int add_constraint(afsat_problem *P, int type, long long t, std::vector<int32_t>
     switch (type) {
     case AFSAT_OR:
         if (k == 1) return all(true);                                  // unit CNF -> prefix assignment
-        emit(P, AFSAT_OR, 0, vars, signs);
-        return AFSAT_OK;
+        return emit_c(AFSAT_OR, 0);
     case AFSAT_XOR:
     case AFSAT_NAE:
-        emit(P, type, type == AFSAT_XOR ? 1 : 0, vars, signs);         // odd parity (Table 2)
-        return AFSAT_OK;
+        return emit_c(type, type == AFSAT_XOR ? 1 : 0);                // odd parity (Table 2)
     case AFSAT_ATLEAST:
         if (t <= 0) { ++P->n_discarded; return AFSAT_OK; }             // CARD-0: trivially satisfied
         if (t > k) return fail(P, AFSAT_E_UNSAT, line, "at-least threshold exceeds the number of literals");
         if (t == k) return all(true);                                  // CARD-n -> unit assignments
-        if (t == 1) { emit(P, AFSAT_OR, 0, vars, signs); return AFSAT_OK; }   // CARD-1 -> CNF
-        emit(P, AFSAT_ATLEAST, (int)t, vars, signs);
-        return AFSAT_OK;
+        if (t == 1) return emit_c(AFSAT_OR, 0);                        // CARD-1 -> CNF
+        return emit_c(AFSAT_ATLEAST, (int)t);
     case AFSAT_ATMOST:
         if (t < 0) return fail(P, AFSAT_E_UNSAT, line, "at-most threshold below zero");
         if (t >= k) { ++P->n_discarded; return AFSAT_OK; }             // includes the unit AMO
         if (t == 0) return all(false);
-        emit(P, AFSAT_ATMOST, (int)t, vars, signs);
-        return AFSAT_OK;
+        return emit_c(AFSAT_ATMOST, (int)t);
     case AFSAT_EXACTLY:
         if (t < 0 || t > k) return fail(P, AFSAT_E_UNSAT, line, "exactly-k with k outside [0, number of literals]");
         if (t == k) return all(true);                                  // EK-n, and the unit EO
         if (t == 0) return all(false);                                 // EK-0 -> negated assignments
-        emit(P, AFSAT_EXACTLY, (int)t, vars, signs);                   // EK-1 is EO = EXACTLY 1
-        return AFSAT_OK;
+        return emit_c(AFSAT_EXACTLY, (int)t);                          // EK-1 is EO = EXACTLY 1
     default:
         return fail(P, AFSAT_E_INVALID, line, "internal: unknown type");
     }

@@ -77,16 +77,31 @@ int afsat_sig_build(int32_t type, int32_t k, int32_t param, uint32_t flags, Afsa
     if ((type == AFSAT_ATLEAST || type == AFSAT_ATMOST || type == AFSAT_EXACTLY) &&
         (param < 0 || param > k))
         return AFSAT_E_PARAM;
+    uint64_t lo = 0, hi = 0;
+    for (int tau = 0; tau <= k; ++tau)
+        if (afsat_sig_satisfied(type, k, param, tau)) { if (tau < 64) lo |= 1ull << tau; else hi |= 1ull << (tau - 64); }
+    int rc = afsat_sig_build_mask(k, lo, hi, flags, out);
+    if (rc) return rc;
+    out->type = type; out->param = (type == AFSAT_OR || type == AFSAT_NAE) ? 0 : param;
+    return AFSAT_OK;
+}
+
+// The same for ANY symmetric constraint on k literals, given as the set of satisfying counts (bit tau of the mask):
+// what a Table 1 constraint becomes once a partial assignment has decided some of its literals.
+int afsat_sig_build_mask(int32_t k, uint64_t satmask_lo, uint64_t satmask_hi, uint32_t flags, AfsatSigHost *out)
+{
+    if (!out) return AFSAT_E_INVALID;
+    if (k < 1 || k > AFSAT_MAX_LEN) return AFSAT_E_LENGTH;
     memset(out, 0, sizeof *out);
-    out->type = type; out->k = k; out->param = (type == AFSAT_OR || type == AFSAT_NAE) ? 0 : param;
+    out->type = -1; out->k = k; out->param = 0;
+    out->satmask_lo = satmask_lo; out->satmask_hi = satmask_hi;
     const int N = k + 1, H = N / 2 + 1;
     const bool robust = (flags & AFSAT_FLAG_ROBUST) != 0;
 
     int g[AFSAT_MAX_LEN + 1];                                          // +-1 truth table
     for (int tau = 0; tau <= k; ++tau) {
-        bool sat = afsat_sig_satisfied(type, k, param, tau);
+        const bool sat = ((tau < 64 ? satmask_lo >> tau : satmask_hi >> (tau - 64)) & 1ull) != 0;
         g[tau] = sat ? -1 : +1;
-        if (sat) { if (tau < 64) out->satmask_lo |= 1ull << tau; else out->satmask_hi |= 1ull << (tau - 64); }
     }
 
     // the spectrum that multiplies the products: integer sequence s_j and its scale

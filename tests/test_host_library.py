@@ -126,6 +126,11 @@ def test_host_tables_rejects():
     assert L.afsat_host_tables(0, 3, 0, 0, None, None) == -1
 
 
+def _has_gpu():
+    import torch
+    return torch.cuda.is_available()
+
+
 def _create(inst, **kw):
     return Bd.Context.from_instance(inst, **kw)
 
@@ -166,6 +171,15 @@ def test_create_validation_codes():
     expect(-1, base, batch=40, ldb=32)                                 # ldb < B
     expect(-1, base, dtype=16)
     expect(-1, base, flags=8)
+    expect(-1, base, flags=Bd.FLAG_ROBUST | Bd.FLAG_PAPER)             # the two table modes exclude each other
+    # afsat_create_ex options (include/afsat.h): explicit tile width, step path, several partial assignments
+    expect(-1, base, tile_w=48)                                        # not a multiple of 32
+    expect(-1, base, step_path=7)
+    masks = np.zeros((2, 12), dtype=np.int8); masks[0, 1] = 1
+    expect(-1, base, batch=96, fixed=masks)                            # 96 % (32 * 2) != 0
+    expect(-8, base, batch=128, fixed=masks) if not _has_gpu() else None   # valid: fails only for want of a device
+    bad = masks.copy(); bad[1, 5] = 3
+    expect(-4, base, batch=128, fixed=bad)
     # constraint longer than AFSAT_MAX_LEN / empty constraint
     n = 80
     rp = np.array([0, 65], dtype=np.int64)

@@ -212,6 +212,22 @@ def test_errors():
     assert r["constraints"] == [(OR, 0, ((0, 1), (1, -1)))]
 
 
+def test_length_limit_binds_only_emitted_constraints():
+    """AFSAT_MAX_LEN (64) applies to what reaches a kernel: a 70-literal constraint that A.1 turns into prefix
+    assignments or discards parses; one that stays a constraint is AFSAT_E_LENGTH."""
+    lits = " ".join(str(i) for i in range(1, 71))
+    for head, fixed_val in (("card >=70", -1), ("ek 70", -1), ("ek 0", +1), ("card <1", +1)):
+        pr = Bd.parse(f"p cnf 70 1\n{head} {lits} 0\n")
+        assert pr.n_cons == 0 and np.all(pr.fixed == fixed_val), head
+    for head in ("card <=70", "card <71", "card <=71"):
+        pr = Bd.parse(f"p cnf 70 1\n{head} {lits} 0\n")
+        assert pr.n_cons == 0 and not np.any(pr.fixed), head
+    for head in ("", "x", "card >=3", "ek 2", "card <5"):
+        with pytest.raises(Bd.AfsatError) as ei:
+            Bd.parse(f"p cnf 70 1\n{head} {lits} 0\n")
+        assert ei.value.code == -2, head
+
+
 def test_parsed_arrays_are_accepted_by_afsat_create_validation():
     """No device here: afsat_create validates before touching CUDA, so a parsed problem must get past
     validation and fail only with AFSAT_E_CUDA (or succeed on a GPU box)."""
