@@ -1,7 +1,12 @@
 #!/usr/bin/env python
 """bench.py -- headline benchmark of the AFSAT hot path on B200 (contract in DESIGN.md "Measurement").
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--impl ours|reference]
+                    [--no-per-config] [--no-ttfs] [--sweep-batch] [--probe-peaks] [--line-search]
+
+The headline (top-level keys) is BASELINE.json configs[4], the largest single-GPU configuration; the default run also
+measures configs 0-3 and config 3 in fp64 (`per_config`) and the time to the first solution on the planted variant of
+the headline workload (`time_to_first_solution`).
 
 A "step" is one pass of the whole hot path (gather, DFT-point products,
 contraction, leave-one-out gradient, scatter-add, projected step, sign rounding, exact discrete
@@ -41,14 +46,16 @@ def load_peaks():
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "source": "fallback"}
 
 
-def load_traffic(cfg):
-    """DRAM bytes per launch of the dominant kernel from the committed ncu capture (profiles/), or None."""
-    p = os.path.join(ROOT, "profiles", "r1_traffic.json")
+def load_capture(cfg, dtype):
+    """What the committed ncu captures of this workload measured (profiles/r2_ncu_summary.json; the commands are in
+    profiles/r2_ncu_summary.md): DRAM bytes of the evaluation kernels per step with a WARM L2 (--cache-control none),
+    FMA-pipe and issue-slot utilisation of the dominant kernel.  {} when there is no capture."""
+    p = os.path.join(ROOT, "profiles", "r2_ncu_summary.json")
     try:
         with open(p) as f:
-            return json.load(f).get(f"cfg{cfg}", {}).get("bytes_per_launch")
+            return json.load(f).get(f"cfg{cfg}" + ("_f64" if dtype == 64 else ""), {})
     except (OSError, ValueError):
-        return None
+        return {}
 
 
 def flop_model(inst):
@@ -114,6 +121,17 @@ class ClockSampler(threading.Thread):
                 "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
 
 
+_PEAKS = {}
+
+
+def probed_peak(kind, device):
+    """afsat_probe_peak (FFMA / FFMA2 / DFMA chains, measured in this run), cached."""
+    from paper_2606_06641_b200 import binding as Bd
+    if (kind, device) not in _PEAKS:
+        _PEAKS[(kind, device)] = Bd.probe_peak(kind, device)
+    return _PEAKS[(kind, device)]
+
+
 def workload(cfg, batch=None, scale=1.0):
     from paper_2606_06641_b200 import instances as I
     inst = I.make_config(cfg, scale=scale, batch=batch)
@@ -138,7 +156,9 @@ def oracle_sample(inst, x0, target_s=15.0, max_b=64):
     oracle_sample.last = (X1[:, :b_o], sat1[:b_o])          # X(1) and the counts on X(1), for the deviation report
     return {"value": inst.n_cons * b_o * 1 / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": f"oracle_step (long double, gcc -O2, OpenMP over candidates) on the first {b_o} of "
-                      f"{inst.batch} candidates x 1 step over all {inst.n_cons} constraints, {dt:.2f} s"}, dt, b_o
+                      f"{inst.batch} candidates x 1 step over all {inst.n_cons} constraints, {dt:.2f} s",
+            "note": "the PRECISION oracle as it stands (x87 long double, a fresh O(k^2) leave-one-out DP per literal), "
+                    "not a tuned CPU implementation: a reported baseline, never the target"}, dt, b_o
 
 
 def time_to_first_solution(inst, x0, dtype, device, max_steps):
@@ -175,7 +195,7 @@ def time_to_first_solution(inst, x0, dtype, device, max_steps):
     xd = torch.from_numpy(x).cuda()
     flag = torch.zeros(2, dtype=torch.int32).pin_memory()
     ctx.step(xd, inst.eta, 2, want_F=False)                      # warm-up (module load, workspace)
-    xd.copy_(torch.from_numpy(x).cuda())
+    xd.copy_(torch.from_numpy(x))
     torch.cuda.synchronize()
     # the launching call blocks the host while the launch queue is full, so the flag is polled from a
     # second thread (the ctypes call releases the GIL); the device writes it through mapped pinned memory
@@ -249,52 +269,42 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sum(times) / len(times),
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f80 (x87 long double)",
-            "data": "synthetic", "config": config_dict(inst, args, extra={"sampled_candidates": b_o}),
+            "data": "synthetic", "config": config_dict(inst, args.config, args.scale, args.gpus, extra={"sampled_candidates": b_o}),
             "cpu_baseline": cb, "gpu_launches": 0,
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line), flush=True)
     return 0
 
 
-def config_dict(inst, args, extra=None):
+def config_dict(inst, cfg, scale, gpus, extra=None):
     ks = inst.lengths()
-    d = {"workload": f"BASELINE.json configs[{args.config}]: {inst.name}", "n_vars": inst.n_vars,
+    d = {"workload": f"BASELINE.json configs[{cfg}]: {inst.name}", "n_vars": inst.n_vars,
          "n_constraints": inst.n_cons, "nnz": inst.nnz, "k_min": int(ks.min()), "k_max": int(ks.max()),
-         "batch_per_gpu": inst.batch, "eta": inst.eta, "scale": args.scale,
-         "parallelism": "replicas (candidates sharded, no collective)" if args.gpus > 1 else "single GPU",
+         "batch_per_gpu": inst.batch, "eta": inst.eta, "scale": scale,
+         "parallelism": "replicas (candidates sharded, no collective)" if gpus > 1 else "single GPU",
          "l2": "flushed between timed steps (256 MiB write, untimed); per-step CUDA events summed"}
     d.update(extra or {})
     return d
 
 
-def run_ours(args):
+def measure(cfg, dtype, K, W, *, batch=None, scale=1.0, oracle_seconds=10.0, rank=0, world=1, local=0, full=True,
+            line_search=0, flags=0):
+    """One workload through the C ABI: K timed steps (L2 flushed between them), the same K steps in one call, the
+    evaluation / update / count kernels timed live with CUDA events, the end-to-end call on host buffers, and the
+    oracle on a bounded sample beside it.  Returns the per-rank measurement dict (times already max-reduced)."""
     import torch
     import torch.distributed as dist
-    from paper_2606_06641_b200 import binding as Bd, build as Build, instances as I
+    from paper_2606_06641_b200 import binding as Bd, instances as I
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    if rank == 0:
-        Build.build()
-    if world > 1:
-        dist.barrier()
-    inst = workload(args.config, args.batch, args.scale)
+    inst = workload(cfg, batch, scale)
     m, B, n = inst.n_cons, inst.batch, inst.n_vars
-    dtype = args.dtype
     npdt = np.float32 if dtype == 32 else np.float64
-    x0 = I.make_x0(inst, seed=rank_x0_seed(args.config, rank), dtype=npdt)
-    ctx = Bd.Context.from_instance(inst, dtype=dtype, device=local)
+    x0 = I.make_x0(inst, seed=rank_x0_seed(cfg, rank), dtype=npdt)
+    ctx = Bd.Context.from_instance(inst, dtype=dtype, device=local, flags=flags)
     ldb = ctx.ldb
     stream = torch.cuda.current_stream()
     x = torch.from_numpy(x0).cuda()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
-    K, W = args.steps, max(args.warmup, 0)
 
     def barrier():
         torch.cuda.synchronize()
@@ -303,11 +313,11 @@ def run_ours(args):
             torch.cuda.synchronize()
 
     state = None
-    F = sat = sol = first = None
+    sol = None
 
     def one_step(t):
-        nonlocal state, F, sat, sol, first
-        F, sat, sol, first = ctx.step(x, inst.eta, 1, step_base=t, state=state, want_F=False)
+        nonlocal state, sol
+        _, _, sol, first = ctx.step(x, inst.eta, 1, step_base=t, state=state, want_F=False)
         state = (sol, first)
 
     for t in range(W):
@@ -329,39 +339,51 @@ def run_ours(args):
     wall = time.perf_counter() - wall0
     launches = ctx.query(Bd.Q_KERNEL_LAUNCHES) - l0
     clocks = sampler.stop()
-    ms = [a.elapsed_time(b) for a, b in ev]
-    t_total = sum(ms) * 1e-3
-    # ---- back-to-back (L2-warm) variant: what a solver run sees; reported beside the headline -------
+    t_total = sum(a.elapsed_time(b) for a, b in ev) * 1e-3
+    # ---- back-to-back (L2-warm) variant: what a solver run sees (ONE call; cfg0: its own 200 steps) -------
+    K_warm = max(K, inst.steps) if cfg == 0 else K
+    ctx.step(x, inst.eta, min(K_warm, 3), step_base=W + K, state=state, want_F=False)
     barrier()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l1 = ctx.query(Bd.Q_KERNEL_LAUNCHES)
     e0.record(stream)
-    F, sat, sol, first = ctx.step(x, inst.eta, K, step_base=W + K, state=state, want_F=False)
+    ctx.step(x, inst.eta, K_warm, step_base=W + K + 3, state=state, want_F=False)
     e1.record(stream)
     barrier()
-    t_warm = e0.elapsed_time(e1) * 1e-3
-    # ---- dominant kernel: per-launch duration measured with events inside the library --------------
-    ctx.set_profiling(True)
-    for t in range(K):
-        one_step(W + 2 * K + t)
-        flush.fill_(t & 0xFF)
-    barrier()
-    kern_ms, kern_launches = ctx.profiled_eval_ms()
-    ctx.set_profiling(False)
+    t_warm = e0.elapsed_time(e1) * 1e-3 * K / K_warm
+    launches_warm_call = ctx.query(Bd.Q_KERNEL_LAUNCHES) - l1
+    # ---- kernels of a step, timed with events inside the library (a second pass of K flushed steps) ----
+    path = ctx.query(Bd.Q_STEP_PATH)
+    kern_ms = upd_ms = chk_ms = 0.0
+    kern_launches = 0
+    if path != Bd.STEP_PERSISTENT:
+        ctx.set_profiling(True)
+        for t in range(K):
+            one_step(W + 2 * K + t)
+            flush.fill_(t & 0xFF)
+        barrier()
+        kern_ms, kern_launches = ctx.profiled_eval_ms()
+        upd_ms = ctx.query(Bd.Q_PROFILED_UPDATE_NS) * 1e-6
+        chk_ms = ctx.query(Bd.Q_PROFILED_CHECK_NS) * 1e-6
+        ctx.set_profiling(False)
     # ---- end to end: HOST buffers, H2D + step + D2H inside the timed region ---------------------------
     hx = torch.from_numpy(x0.copy()).pin_memory()
-    for _ in range(min(W, 3)):
-        ctx.step_host(hx, inst.eta, 1, want_F=True)
+    F_pre = np.empty(B, dtype=npdt)
+    K_e2e = K if full else min(K, 5)
+    for _ in range(2):
+        ctx.step_host(hx, inst.eta, 1, want_F=False, F_pre=F_pre)
     barrier()
     w0 = time.perf_counter()
-    for _ in range(K):
-        ctx.step_host(hx, inst.eta, 1, want_F=True)
+    for _ in range(K_e2e):
+        ctx.step_host(hx, inst.eta, 1, want_F=False, F_pre=F_pre)
     barrier()
-    t_e2e = time.perf_counter() - w0
+    t_e2e = (time.perf_counter() - w0) * K / K_e2e
+    del hx
     # ---- optional: Alg. 1 with the line search (afsat_step_ls), reported beside the headline ---------
     t_ls = None
-    if args.line_search:
+    if line_search:
         xl = torch.from_numpy(x0).cuda()
-        ls_kw = dict(s_max=1.0, beta=0.5, c1=1e-4, delta=1e-6, max_trials=args.ls_trials)
+        ls_kw = dict(s_max=1.0, beta=0.5, c1=1e-4, delta=1e-6, max_trials=line_search)
         ls_state = None
         for t in range(max(W, 1)):
             *_, s_, f_, c_ = ctx.step_ls(xl, 1, step_base=t, state=ls_state, want_F=False, **ls_kw)
@@ -375,77 +397,205 @@ def run_ours(args):
         e1.record(stream)
         barrier()
         t_ls = e0.elapsed_time(e1) * 1e-3
-    # ---- optional: time to first solution (BASELINE.json configs[4]) on the PLANTED variant of the workload ----
-    ttfs = None
-    if args.ttfs:
-        ttfs = time_to_first_solution(inst, x0, dtype, local, args.ttfs_steps)
+        del xl
     esz = 4 if dtype == 32 else 8
-    h2d = n * ldb * esz
-    d2h = n * ldb * esz + B * (esz + 4 + 1 + 4)
+    t_total, t_warm, t_e2e, kern_ms, upd_ms, chk_ms = reduce_max([t_total, t_warm, t_e2e, kern_ms, upd_ms, chk_ms], device="cuda")
+    out = {"inst": inst, "x0": x0, "ctx": ctx, "K": K, "W": W, "dtype": dtype, "cfg": cfg, "t_total": t_total, "t_warm": t_warm,
+           "t_e2e": t_e2e, "kern_ms": kern_ms, "upd_ms": upd_ms, "chk_ms": chk_ms, "kern_launches": kern_launches,
+           "launches": launches, "launches_warm_call": launches_warm_call, "K_warm": K_warm, "clocks": clocks, "wall": wall,
+           "h2d": n * ldb * esz, "d2h": n * ldb * esz + B * (esz + 4 + 1 + 4), "t_ls": t_ls, "path": path,
+           "solved": int(sol.sum().item()), "scale": scale}
+    del x, flush
+    return out
 
-    t_total, t_warm, t_e2e, kern_ms = reduce_max([t_total, t_warm, t_e2e, kern_ms], device="cuda")
+
+def report(r, world, local, oracle_seconds, rank0_oracle=True):
+    """The JSON-able report of one measurement (rank 0)."""
+    import torch
+    from paper_2606_06641_b200 import binding as Bd
+    inst, ctx, K, dtype, cfg = r["inst"], r["ctx"], r["K"], r["dtype"], r["cfg"]
+    m, B, n = inst.n_cons, inst.batch, inst.n_vars
+    peaks = load_peaks()
+    sm = ctx.query(Bd.Q_SM_COUNT)
+    flop_c, instr_c = flop_model(inst)
+    flop_sub, instr_sub = ctx.query(Bd.Q_FLOP_PER_CANDIDATE), ctx.query(Bd.Q_FP_INSTR_PER_CANDIDATE)
+    value = whole_job_value(world, m, B, K, r["t_total"])
+    kern_ms = r["kern_ms"]
+    flop_per_step = flop_c * B
+    peak_tf = sm * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+    ach_tf = flop_per_step / (kern_ms * 1e-3 / K) / 1e12 if kern_ms > 0 else 0.0
+    esz = 4 if dtype == 32 else 8
+    cap = load_capture(cfg, dtype)
+    path_name = {1: "launches", 2: "persistent (one launch)", 3: "cuda graph"}.get(r["path"], str(r["path"]))
+    roof = {"bound": "alu",
+            "kernel": "evaluation kernels, a1-a5 (fp32: k_eval_f2m k<=8 | k_eval_split k>=9; fp64: k_eval_km k<=20 | "
+                      "k_eval_split k>20): all launches of one step",
+            "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach_tf / peak_tf,
+            "peak_source": f"{sm} SMs x 128 FP32 lanes x 2 flop x {peaks['sm_max_mhz']:.0f} MHz "
+                           f"({peaks['source']} sm_max_mhz; DESIGN.md 6); MEASURED_PEAKS.json has no FP32 figure, so the "
+                           f"probe below checks it",
+            "peak_measured": {"ffma_tflops": probed_peak(0, local), "ffma2_tflops": probed_peak(1, local),
+                              "dfma_tflops": probed_peak(2, local),
+                              "how": "afsat_probe_peak: 8 independent FMA chains per thread, CUDA events, best of 5"},
+            "model_instr_over_issue_peak": (instr_c * B / (kern_ms * 1e-3 / K)) / (sm * FP32_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6)
+            if kern_ms > 0 else 0.0,
+            "measured_pipe_utilisation": {k_: cap.get(k_) for k_ in ("sm__pipe_fma_cycles_active_pct", "smsp__issue_active_pct",
+                                                                      "sm__inst_executed_pipe_fma_per_eval", "capture")} if cap else None,
+            "kernel_ms_per_step": kern_ms / K, "kernel_launches_per_step": max(1, r["kern_launches"] // K) if r["kern_launches"] else 0,
+            "kernel_share_of_step": (kern_ms / K) / (1e3 * r["t_total"] / K),
+            "update_ms_per_step": r["upd_ms"] / K, "count_ms_per_step": r["chk_ms"] / K,
+            "algorithmic_flop_per_step": flop_per_step,
+            "algorithmic_flop_per_step_after_substitution": flop_sub * B,
+            "frac_after_substitution": (flop_sub * B / (kern_ms * 1e-3 / K) / 1e12) / peak_tf if kern_ms > 0 else 0.0,
+            "traffic": cap.get("dram_bytes_per_step_eval_kernels"),
+            "traffic_whole_step": cap.get("dram_bytes_per_step"),
+            "hbm_floor_bytes_per_step": 2 * n * B * esz, "hbm_peak_gbs": peaks["hbm_gbs"],
+            "note": "achieved = ALGORITHMIC flop of the instance as given (SURVEY.md App. D: 12 / 4 FP32 instructions per literal at a "
+                    "complex / real DFT point, every retained point) / measured kernel time.  The kernels execute fewer instructions: "
+                    "trivial twiddles at the points 1, -1, i and the eighth roots (k <= 8; cfg1's k = 7 has only such points), literal "
+                    "groups (k >= 21), and a partial assignment is substituted before anything is evaluated (frac_after_substitution "
+                    "counts the model on the substituted table); measured_pipe_utilisation is what ncu saw executed"}
+    if dtype == 64:
+        roof["fp64_peak"] = probed_peak(2, local)
+        roof["frac_of_fp64_peak"] = ach_tf / max(probed_peak(2, local), 1e-9)
+    if r["clocks"].get("sm_mhz"):
+        roof["frac_at_observed_clock"] = roof["frac"] * peaks["sm_max_mhz"] / r["clocks"]["sm_mhz"]
+    if r["path"] == Bd.STEP_PERSISTENT:
+        roof["note_small"] = "launch-latency-bound workload: the whole step loop is one launch; no per-kernel roofline"
+    cb = dev_rep = None
+    if rank0_oracle:
+        x0 = r["x0"]
+        cb, _, b_o = oracle_sample(inst, x0.astype(np.float64), target_s=oracle_seconds)
+        # deviation vs the oracle (BASELINE.json configs[3]: "report deviation vs oracle"): ONE step from x0
+        # on the GPU against the oracle's step on the sampled candidates -- X(1) = clamp(x0 - eta G), so
+        # max|dX| / eta is the gradient deviation where the clamp is inactive; counts are bit-exact or not
+        X1o, sat1o = oracle_sample.last
+        xd = torch.from_numpy(np.ascontiguousarray(x0)).cuda()
+        _, sat_d, _, _ = ctx.step(xd, inst.eta, 1, step_base=0, state=None, want_F=False)
+        torch.cuda.synchronize()
+        dX = np.abs(xd[:, :b_o].double().cpu().numpy() - X1o)
+        dev_rep = {"candidates": int(b_o), "max_abs_dX_after_one_step": float(dX.max()),
+                   "max_abs_dG_implied": float(dX.max() / inst.eta),
+                   "sat_count_bit_exact": bool(np.array_equal(sat_d[:b_o].cpu().numpy(), sat1o)),
+                   "tables": "default (fp32: paper tables to k = 20, robust beyond; fp64: paper tables)"}
+        del xd
+    out = {"value": value, "unit": UNIT, "ms_per_step": 1e3 * r["t_total"] / K, "dtype": "f32" if dtype == 32 else "f64",
+           "config": config_dict(inst, cfg, r["scale"], world), "clocks": r["clocks"], "gpu_launches": int(r["launches"]),
+           "step_path": path_name,
+           "e2e": {"value": world * m * B * K / r["t_e2e"], "unit": UNIT, "h2d_bytes_per_step": r["h2d"],
+                   "d2h_bytes_per_step": r["d2h"], "ms_per_step": 1e3 * r["t_e2e"] / K,
+                   "result_read_back": "X(t), F(X(t-1)) (by-product of the fused pass), sat_count, is_solution, first_step"},
+           "roofline": roof, "cpu_baseline": cb, "deviation_vs_oracle": dev_rep,
+           "value_l2_warm": world * m * B * K / r["t_warm"], "ms_per_step_l2_warm": 1e3 * r["t_warm"] / K,
+           "l2_warm_call": {"n_steps": r["K_warm"], "launches": int(r["launches_warm_call"])},
+           "solved_candidates": r["solved"], "wall_s_timed_region": r["wall"]}
+    if r["t_ls"] is not None:
+        out["line_search"] = {"ms_per_step": 1e3 * r["t_ls"] / K,
+                              "note": "afsat_step_ls: 1 FE+grad evaluation + max_trials objective-only "
+                                      "evaluations of the candidates still searching, per step (L2 warm)"}
+    return out
+
+
+def sweep_batch(cfg, dtype, local, K=5):
+    """Throughput against batch size (Fig. 2b: the paper's throughput peaks where the working set is
+    ~2x the device cache and decays beyond; candidate tiling is this build's answer)."""
+    import torch
+    from paper_2606_06641_b200 import binding as Bd, instances as I
+    rows = []
+    base = workload(cfg)
+    esz = 4 if dtype == 32 else 8
+    for B in (64, 128, 256, 512, 1024, 2048, 4096, 8192, 16384, 32768, 65536):
+        if 2 * base.n_vars * B * esz > 60e9:
+            break
+        inst = workload(cfg, B)
+        x0 = I.make_x0(inst, dtype=np.float32 if dtype == 32 else np.float64)
+        ctx = Bd.Context.from_instance(inst, dtype=dtype, device=local)
+        x = torch.from_numpy(x0).cuda()
+        ctx.step(x, inst.eta, 2, want_F=False)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        ctx.step(x, inst.eta, K, want_F=False)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / K
+        rows.append({"batch": B, "x_bytes": inst.n_vars * ctx.ldb * esz, "working_set_over_l2": 2 * inst.n_vars * ctx.ldb * esz / ctx.query(Bd.Q_L2_BYTES),
+                     "tile_w": ctx.query(Bd.Q_TILE_W), "ms_per_step": ms, "evals_per_s": inst.n_cons * B / (ms * 1e-3)})
+        ctx.close()
+        del x, x0
+        torch.cuda.empty_cache()
+    return rows
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_06641_b200 import binding as Bd, build as Build
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     if rank == 0:
-        peaks = load_peaks()
-        sm = ctx.query(Bd.Q_SM_COUNT)
-        flop_c, instr_c = flop_model(inst)
-        evals = world * m * B * K
-        value = whole_job_value(world, m, B, K, t_total)
-        kern_s = kern_ms * 1e-3 / max(1, kern_launches)          # avg duration of one eval launch set
-        launches_per_step = max(1, kern_launches // K)
-        flop_per_step = flop_c * B
-        peak_tf = sm * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
-        ach_tf = flop_per_step / (kern_ms * 1e-3 / K) / 1e12 if kern_ms > 0 else 0.0
-        roof = {"bound": "alu", "kernel": "evaluation kernels, a1-a5 (fp32: k_eval_f2m k<=8 | k_eval_split k>=9; fp64: k_eval_km k<=20 | k_eval_split k>20): all launches of one step", "achieved": ach_tf, "peak": peak_tf,
-                "unit": "TFLOP/s", "frac": ach_tf / peak_tf,
-                "peak_source": f"{sm} SMs x 128 FP32 lanes x 2 flop x {peaks['sm_max_mhz']:.0f} MHz "
-                               f"({peaks['source']} sm_max_mhz; DESIGN.md 'Roofline')",
-                "fp32_issue_frac": (instr_c * B / (kern_ms * 1e-3 / K)) / (sm * FP32_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6)
-                if kern_ms > 0 else 0.0,
-                "kernel_ms_per_step": kern_ms / K, "kernel_launches_per_step": launches_per_step,
-                "kernel_share_of_step": (kern_ms / K) / (1e3 * t_total / K),
-                "algorithmic_flop_per_step": flop_per_step, "traffic": load_traffic(args.config),
-                "hbm_floor_bytes_per_step": 2 * n * B * esz, "hbm_peak_gbs": peaks["hbm_gbs"],
-                "note": "achieved = ALGORITHMIC flop (SURVEY.md App. D: 12 / 4 FP32 instructions per literal at a complex / "
-                        "real DFT point, every retained point) / measured kernel time; the kernels execute fewer "
-                        "instructions than that at the points 1, -1, i (trivial twiddles, DESIGN.md 6.1)"}
-        if dtype == 64:
-            # the DFMA pipe issues 64 lanes per SM per clock on this part (ncu: sm__pipe_fp64_cycles_active 61.7 % for
-            # 1.3e9 FP64 warp instructions in 4.0 ms, profiles/r1_eval_split_cfg3_f64.md): half the FP32 rate
-            roof["fp64_peak"] = peak_tf / 2
-            roof["frac_of_fp64_peak"] = ach_tf / (peak_tf / 2)
-        if clocks.get("sm_mhz"):
-            roof["frac_at_observed_clock"] = roof["frac"] * peaks["sm_max_mhz"] / clocks["sm_mhz"]
-        cb = dev_rep = None
-        if world == 1 or rank == 0:
-            cb, _, b_o = oracle_sample(inst, x0.astype(np.float64), target_s=args.oracle_seconds)
-            # deviation vs the oracle (BASELINE.json configs[3]: "report deviation vs oracle"): ONE step from x0
-            # on the GPU against the oracle's step on the sampled candidates -- X(1) = clamp(x0 - eta G), so
-            # max|dX| / eta is the gradient deviation where the clamp is inactive; counts are bit-exact or not
-            X1o, sat1o = oracle_sample.last
-            xd = torch.from_numpy(np.ascontiguousarray(x0)).cuda()
-            _, sat_d, _, _ = ctx.step(xd, inst.eta, 1, step_base=0, state=None, want_F=False)
-            torch.cuda.synchronize()
-            dX = np.abs(xd[:, :b_o].double().cpu().numpy() - X1o)
-            dev_rep = {"candidates": int(b_o), "max_abs_dX_after_one_step": float(dX.max()),
-                       "max_abs_dG_implied": float(dX.max() / inst.eta),
-                       "sat_count_bit_exact": bool(np.array_equal(sat_d[:b_o].cpu().numpy(), sat1o))}
-        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-                "ms_per_step": 1e3 * t_total / K, "higher_is_better": True, "scaling": "weak",
-                "vs_baseline": None, "dtype": "f32" if dtype == 32 else "f64", "data": "synthetic",
-                "config": config_dict(inst, args), "clocks": clocks, "gpu_launches": int(launches),
-                "e2e": {"value": world * m * B * K / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d,
-                        "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * t_e2e / K},
-                "roofline": roof, "cpu_baseline": cb, "deviation_vs_oracle": dev_rep,
-                "value_l2_warm": world * m * B * K / t_warm, "ms_per_step_l2_warm": 1e3 * t_warm / K,
-                "solved_candidates": int(sol.sum().item()), "wall_s_timed_region": wall}
-        if ttfs is not None:
-            line["time_to_first_solution"] = ttfs
-        if t_ls is not None:
-            line["line_search"] = {"ms_per_step": 1e3 * t_ls / K, "max_trials": args.ls_trials,
-                                   "note": "afsat_step_ls: 1 FE+grad evaluation + max_trials objective-only "
-                                           "evaluations of the candidates still searching, per step (L2 warm)"}
+        Build.build()
+    if world > 1:
+        dist.barrier()
+    t_run0 = time.perf_counter()
+    K, W = args.steps, max(args.warmup, 0)
+    r = measure(args.config, args.dtype, K, W, batch=args.batch, scale=args.scale, rank=rank, world=world, local=local,
+                line_search=args.ls_trials if args.line_search else 0)
+    line = None
+    if rank == 0:
+        rep = report(r, world, local, args.oracle_seconds)
+        line = {"metric": METRIC, "value": rep.pop("value"), "unit": rep.pop("unit"), "n_gpus": world, "steps": K, "warmup": W,
+                "ms_per_step": rep.pop("ms_per_step"), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": rep.pop("dtype"), "data": "synthetic"}
+        line.update(rep)
+    # ---- time to first solution (BASELINE.json configs[4]) on the PLANTED variant of the headline workload ----
+    if rank == 0 and world == 1 and not args.no_ttfs:
+        line["time_to_first_solution"] = time_to_first_solution(r["inst"], r["x0"], args.dtype, local, args.ttfs_steps)
+    r["ctx"].close()
+    r.clear()
+    torch.cuda.empty_cache()
+    # ---- the other configurations of BASELINE.json (and cfg3 in fp64), single GPU only -------------------------
+    if rank == 0 and world == 1 and not args.no_per_config and args.batch is None and args.scale == 1.0:
+        per = {}
+        todo = [(c, 32) for c in range(5) if c != args.config or args.dtype != 32] + [(3, 64)]
+        for c, dt in todo:
+            Kc = 200 if c == 0 else max(5, min(K, 10))
+            rc = measure(c, dt, Kc, 3, local=local, full=False)
+            rp = report(rc, 1, local, args.per_config_oracle_seconds)
+            keep = {k_: rp[k_] for k_ in ("ms_per_step", "value", "ms_per_step_l2_warm", "value_l2_warm", "l2_warm_call", "step_path",
+                                          "gpu_launches", "deviation_vs_oracle", "clocks", "solved_candidates")}
+            keep["steps"] = Kc
+            keep["e2e"] = {k_: rp["e2e"][k_] for k_ in ("value", "ms_per_step")}
+            keep["cpu_baseline"] = {k_: rp["cpu_baseline"][k_] for k_ in ("value", "cores", "sample")}
+            keep["roofline"] = {k_: rp["roofline"].get(k_) for k_ in ("frac", "achieved", "peak", "frac_after_substitution",
+                                                                      "frac_of_fp64_peak", "model_instr_over_issue_peak",
+                                                                      "kernel_ms_per_step", "kernel_share_of_step",
+                                                                      "update_ms_per_step", "count_ms_per_step",
+                                                                      "measured_pipe_utilisation", "traffic", "note_small")}
+            if c == 3 and dt == 32:
+                # BASELINE.json configs[3]: "run in both fp32 and fp64 and report deviation vs oracle" -- also for the paper's
+                # own product form in fp32 (AFSAT_FLAG_PAPER), which the default context replaces beyond k = 20
+                rq = measure(c, dt, 5, 2, local=local, full=False, flags=Bd.FLAG_PAPER)
+                rq_rep = report(rq, 1, local, 2.0)
+                keep["paper_tables_fp32"] = {"ms_per_step": rq_rep["ms_per_step"], "deviation_vs_oracle": rq_rep["deviation_vs_oracle"]}
+                rq["ctx"].close()
+            per[f"cfg{c}" + ("_f64" if dt == 64 else "")] = keep
+            rc["ctx"].close()
+            rc.clear()
+            torch.cuda.empty_cache()
+        line["per_config"] = per
+    if rank == 0 and world == 1 and args.sweep_batch:
+        line["batch_sweep"] = {f"cfg{c}": sweep_batch(c, 32, local) for c in (1, 3)}
+    if rank == 0:
+        line["wall_s_whole_run"] = time.perf_counter() - t_run0
         print(json.dumps(line), flush=True)
-    ctx.close()
     if world > 1:
         dist.destroy_process_group()
     return 0
@@ -456,17 +606,26 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=5)
-    ap.add_argument("--config", type=int, default=1)
+    ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--batch", type=int, default=None)
     ap.add_argument("--scale", type=float, default=1.0)
     ap.add_argument("--dtype", type=int, default=32, choices=[32, 64])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--oracle-seconds", type=float, default=15.0)
-    ap.add_argument("--ttfs", action="store_true", help="also report time to first solution on the planted variant")
+    ap.add_argument("--oracle-seconds", type=float, default=10.0)
+    ap.add_argument("--per-config-oracle-seconds", type=float, default=2.5)
+    ap.add_argument("--no-per-config", action="store_true", help="headline workload only")
+    ap.add_argument("--no-ttfs", action="store_true", help="skip the time-to-first-solution run")
     ap.add_argument("--ttfs-steps", type=int, default=100)
+    ap.add_argument("--sweep-batch", action="store_true", help="also throughput vs batch size on cfg1 and cfg3 (PAPER.md Fig. 2b)")
+    ap.add_argument("--probe-peaks", action="store_true", help="print the measured FFMA / FFMA2 / DFMA peaks and exit")
     ap.add_argument("--line-search", action="store_true", help="also time afsat_step_ls (Alg. 1 with line search)")
     ap.add_argument("--ls-trials", type=int, default=4)
     args = ap.parse_args()
+    if args.probe_peaks:
+        from paper_2606_06641_b200 import build as Build
+        Build.build()
+        print(json.dumps({"ffma_tflops": probed_peak(0, 0), "ffma2_tflops": probed_peak(1, 0), "dfma_tflops": probed_peak(2, 0)}))
+        return 0
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

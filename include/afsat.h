@@ -108,12 +108,13 @@ int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t 
  *     the X and G tiles may take when the library picks the width itself (default: 13/16 of the device's L2).
  *   step_path: AFSAT_STEP_AUTO, or force AFSAT_STEP_LAUNCHES / AFSAT_STEP_PERSISTENT / AFSAT_STEP_GRAPH for afsat_step
  *     (PERSISTENT is refused with AFSAT_E_INVALID when the instance does not fit: every length <= 8, one group,
- *     X and G of 32 candidates in shared memory).
+ *     X and G of one candidate in shared memory).
  */
 enum afsat_step_path {
     AFSAT_STEP_AUTO = 0,
     AFSAT_STEP_LAUNCHES = 1,    /* one set of launches per iteration and candidate tile                               */
-    AFSAT_STEP_PERSISTENT = 2,  /* the whole n_steps loop in ONE launch, X and G in shared memory (small instances)   */
+    AFSAT_STEP_PERSISTENT = 2,  /* the whole n_steps loop in ONE launch: a CTA per candidate, a thread per constraint, X and
+                                   G in shared memory (small instances)                                               */
     AFSAT_STEP_GRAPH = 3        /* one iteration captured into a CUDA graph, replayed n_steps times                   */
 };
 typedef struct afsat_options {
@@ -261,7 +262,7 @@ enum afsat_query_key {
     AFSAT_Q_FP_INSTR_PER_CANDIDATE = 6, /* model count of FP instructions for one eval_grad of one
                                            candidate over all constraints (DESIGN.md cost model)  */
     AFSAT_Q_PROFILED_EVAL_NS = 7,       /* afsat_set_profiling: device time of the evaluation kernels
-                                           (a1-a5, a7-a8) since profiling was switched on, in ns;
+                                           (a1-a5) since profiling was switched on, in ns;
                                            SYNCHRONISES with the recorded events                  */
     AFSAT_Q_PROFILED_EVAL_LAUNCHES = 8, /* number of evaluation-kernel launches in that time       */
     AFSAT_Q_FLOP_PER_CANDIDATE = 9,     /* model flop count, same scope as key 6; both are counted on the
@@ -272,7 +273,9 @@ enum afsat_query_key {
     AFSAT_Q_LIVE_CONSTRAINTS = 13,      /* constraints that reach a kernel (group 0)               */
     AFSAT_Q_LIVE_NNZ = 14,              /* their literals (group 0)                                */
     AFSAT_Q_DECIDED_SATISFIED = 15,     /* constraints group 0's partial assignment satisfies outright */
-    AFSAT_Q_L2_BYTES = 16               /* cudaDeviceProp::l2CacheSize                             */
+    AFSAT_Q_L2_BYTES = 16,              /* cudaDeviceProp::l2CacheSize                             */
+    AFSAT_Q_PROFILED_UPDATE_NS = 17,    /* afsat_set_profiling: device time of the update kernels (a6, a7, a9) */
+    AFSAT_Q_PROFILED_CHECK_NS = 18      /* ... and of the exact count (a8); both SYNCHRONISE like key 7 */
 };
 int64_t afsat_query(const afsat_ctx *ctx, int32_t key);
 

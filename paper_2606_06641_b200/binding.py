@@ -23,7 +23,8 @@ STEP_AUTO, STEP_LAUNCHES, STEP_PERSISTENT, STEP_GRAPH = range(4)
 
 Q_KERNEL_LAUNCHES, Q_NUM_SIGNATURES, Q_NUM_BUCKETS, Q_NNZ, Q_WORKSPACE_BYTES, Q_SM_COUNT, \
     Q_FP_INSTR_PER_CANDIDATE, Q_PROFILED_EVAL_NS, Q_PROFILED_EVAL_LAUNCHES, Q_FLOP_PER_CANDIDATE, Q_NUM_GROUPS, \
-    Q_STEP_PATH, Q_TILE_W, Q_LIVE_CONSTRAINTS, Q_LIVE_NNZ, Q_DECIDED_SATISFIED, Q_L2_BYTES = range(17)
+    Q_STEP_PATH, Q_TILE_W, Q_LIVE_CONSTRAINTS, Q_LIVE_NNZ, Q_DECIDED_SATISFIED, Q_L2_BYTES, Q_PROFILED_UPDATE_NS, \
+    Q_PROFILED_CHECK_NS = range(19)
 
 ERROR_NAMES = {0: "AFSAT_OK", -1: "AFSAT_E_INVALID", -2: "AFSAT_E_LENGTH", -3: "AFSAT_E_VARIABLE",
                -4: "AFSAT_E_SIGN", -5: "AFSAT_E_DUPLICATE", -6: "AFSAT_E_PARAM",

@@ -53,6 +53,7 @@ struct GroupPlan {
     int64_t b0 = 0, b1 = 0;     // candidates [b0, b1) (the last group also owns the padding columns up to ldb)
     int32_t *d_lits = nullptr;
     Item *d_items = nullptr;
+    ConsDev *d_cons = nullptr;  // per-constraint view of the table (the one-launch step loop)
     int32_t n_items = 0, cls_begin[N_CLS + 1] = {0};
     int64_t nnz = 0;            // literals that reach a kernel
     int32_t m_live = 0;         // constraints that reach a kernel
@@ -79,6 +80,7 @@ struct afsat_ctx {
     SigDev *d_sigs = nullptr;
     void *d_rows = nullptr;
     float *d_rows2 = nullptr;                      // staged tables of the packed fp32 kernel
+    void *d_rowsg = nullptr;                       // staged tables of the grouped lane-split kernels
     int8_t *d_fixed = nullptr;                     // [n_groups][n]
     int32_t *d_sat_const = nullptr;                // [n_groups]
     std::vector<GroupPlan> groups;
@@ -111,9 +113,10 @@ struct afsat_ctx {
     bool capturing = false;
     // afsat_set_profiling: event pairs around the evaluation-kernel launches
     bool profiling = false;
-    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_events;
-    double prof_ns = 0.0;
-    int64_t prof_launches = 0;
+    struct ProfEv { cudaEvent_t e0, e1; int cat; };
+    std::vector<ProfEv> prof_events;                // cat 0: evaluation (a1-a5), 1: update (a6, a7, a9), 2: count (a8)
+    double prof_ns[3] = {0.0, 0.0, 0.0};
+    int64_t prof_launches[3] = {0, 0, 0};
     std::string err;
 };
 
@@ -161,8 +164,8 @@ inline int pow2_floor(int64_t v) { int p = 1; while ((int64_t)p * 2 <= v) p *= 2
 
 // brackets one evaluation-kernel launch set with events when profiling is on
 struct ProfScope {
-    afsat_ctx *c; cudaStream_t st; cudaEvent_t e0 = nullptr, e1 = nullptr;
-    ProfScope(afsat_ctx *c_, cudaStream_t st_) : c(c_), st(st_)
+    afsat_ctx *c; cudaStream_t st; int cat; cudaEvent_t e0 = nullptr, e1 = nullptr;
+    ProfScope(afsat_ctx *c_, cudaStream_t st_, int cat_ = 0) : c(c_), st(st_), cat(cat_)
     {
         if (!c->profiling || c->capturing) return;
         if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) { e0 = e1 = nullptr; return; }
@@ -172,18 +175,18 @@ struct ProfScope {
     {
         if (!e0) return;
         cudaEventRecord(e1, st);
-        c->prof_events.emplace_back(e0, e1);
+        c->prof_events.push_back({e0, e1, cat});
     }
 };
 
 void prof_drain(afsat_ctx *c, bool keep)
 {
     for (auto &pr : c->prof_events) {
-        if (keep && cudaEventSynchronize(pr.second) == cudaSuccess) {
+        if (keep && cudaEventSynchronize(pr.e1) == cudaSuccess) {
             float ms = 0.f;
-            if (cudaEventElapsedTime(&ms, pr.first, pr.second) == cudaSuccess) { c->prof_ns += (double)ms * 1e6; ++c->prof_launches; }
+            if (cudaEventElapsedTime(&ms, pr.e0, pr.e1) == cudaSuccess) { c->prof_ns[pr.cat] += (double)ms * 1e6; ++c->prof_launches[pr.cat]; }
         }
-        cudaEventDestroy(pr.first); cudaEventDestroy(pr.second);
+        cudaEventDestroy(pr.e0); cudaEventDestroy(pr.e1);
     }
     c->prof_events.clear();
 }
@@ -221,6 +224,7 @@ int launch_eval(afsat_ctx *ctx, const GroupPlan &gp, const T *x, T *G, int64_t g
     EvalParams<T> p;
     p.x = x; p.G = G; p.g_ld = g_ld; p.g_b0 = g_b0; p.Fpart = Fpart;
     p.lits = gp.d_lits; p.sigs = ctx->d_sigs; p.rows = (const T *)ctx->d_rows; p.rows2 = ctx->d_rows2;
+    p.rowsg = (const T *)ctx->d_rowsg;
     p.skip = ctx->cur_skip;
     p.B = ctx->B; p.ldb = ctx->ldb; p.b_begin = b_begin; p.b_end = std::min<int64_t>(b_begin + width, ctx->ldb);
     const bool grad = G != nullptr;
@@ -277,6 +281,7 @@ int launch_check_bits(afsat_ctx *ctx, const GroupPlan &gp, int64_t w_begin, int6
     p.n_items = gp.n_items;
     const unsigned gy = (unsigned)((nw + p.wpb - 1) / p.wpb);
     dim3 grid((unsigned)std::max<int64_t>(1, std::min<int64_t>(std::max(1, gp.n_items), (int64_t)ctx->sm_count * 8 / gy)), gy);
+    ProfScope prof(ctx, st, 2);
     k_check_bits<<<grid, CTA_THREADS, 0, st>>>(p);
     ++ctx->launches;
     CU(cudaPeekAtLastError());
@@ -365,6 +370,7 @@ int launch_update(afsat_ctx *ctx, const GroupPlan &gp, T *x, T *G, int64_t g_ld,
     const unsigned gy = (unsigned)std::max<int64_t>(1, std::min<int64_t>((ctx->n + rpp * UPD_UNROLL - 1) / (rpp * UPD_UNROLL),
                                                                            (int64_t)ctx->sm_count * 8 / gx));
     const size_t gi = &gp - ctx->groups.data();
+    ProfScope prof(ctx, st, 1);
     k_update<T><<<dim3(gx, gy), CTA_THREADS, 0, st>>>(x, G, g_ld, g_b0, ctx->d_fixed + gi * (size_t)ctx->n, sol, ctx->d_bits, (T)eta,
                                                       ctx->n, ctx->B, ctx->ldb, b0, b0 + w, tpr);
     ++ctx->launches;
@@ -405,12 +411,12 @@ int step_small(afsat_ctx *ctx, T *x, double eta, int n_steps, int step_base, int
 {
     const GroupPlan &gp = ctx->groups[0];
     SmallParams<T> p;
-    p.x = x; p.ldb = ctx->ldb; p.n = ctx->n; p.B = ctx->B; p.m = ctx->m; p.n_items = gp.n_items;
-    p.lits = gp.d_lits; p.items = gp.d_items; p.sigs = ctx->d_sigs; p.rows = (const T *)ctx->d_rows; p.fixed = ctx->d_fixed;
+    p.x = x; p.ldb = ctx->ldb; p.n = ctx->n; p.B = ctx->B; p.m = ctx->m; p.m_live = gp.m_live;
+    p.lits = gp.d_lits; p.cons = gp.d_cons; p.sigs = ctx->d_sigs; p.rows = (const T *)ctx->d_rows; p.fixed = ctx->d_fixed;
     p.eta = (T)eta; p.n_steps = n_steps; p.step_base = step_base; p.sat_const = gp.sat_const;
-    p.n_ctas = (ctx->B + 31) / 32;
     p.sat_count = sat; p.is_solution = sol; p.first_step = first; p.d_any = ctx->d_any; p.h_any = h_any_dev;
-    k_step_small<T><<<p.n_ctas, SMALL_THREADS, ctx->small_smem, st>>>(p);
+    const int threads = std::min(SMALL_THREADS, std::max(64, (gp.m_live + 31) / 32 * 32));   // thread = constraint
+    k_step_small<T><<<ctx->B, threads, ctx->small_smem, st>>>(p);
     ++ctx->launches;
     CU(cudaPeekAtLastError());
     return AFSAT_OK;
@@ -819,6 +825,7 @@ int afsat_create_ex(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64
     std::vector<SigDev> sigs(n_sigs);
     std::vector<double> rows;
     std::vector<float> rows2;
+    std::vector<double> rowsg;
     std::vector<int> sig_k(n_sigs);
     std::vector<int64_t> sig_cost(n_sigs), sig_flop(n_sigs);
     for (auto &kv : sig_id) {
@@ -848,6 +855,12 @@ int afsat_create_ex(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64
             d.row2_off = (int32_t)(rows2.size() / ROW2);
             d.uv = (int8_t)uv; d.n_unit = (int8_t)nu; d.n_gen = (int8_t)ng;
             rows2.insert(rows2.end(), packed, packed + (size_t)nrows2 * ROW2);
+        }
+        if (class_of(kk, dtype) == CLS_LONG) {                         // staged table of the grouped lane-split kernels
+            double packed[AFSAT_MAX_POINTS * ROWG];
+            d.pad = (int8_t)pack_rows_grp(hs.rows, hs.n_real + hs.n_cplx, kk, packed);
+            d.row2_off = (int32_t)(rowsg.size() / ROWG);
+            rowsg.insert(rowsg.end(), packed, packed + (size_t)(hs.n_real + hs.n_cplx) * ROWG);
         }
         sig_k[kv.second] = kk;
         // the model counts every DFT point l < H of the constraint as it stands after substitution (R = 1 + [k odd] real)
@@ -895,6 +908,7 @@ int afsat_create_ex(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64
     // ---- per group: bucket order, packed literals, work items ------------------------------------------------------
     std::vector<std::vector<int32_t>> g_lits(G);
     std::vector<std::vector<Item>> g_items(G);
+    std::vector<std::vector<ConsDev>> g_cons(G);
     int n_buckets = 0, max_items = 1;
     for (int g = 0; g < G; ++g) {
         const int8_t *fx = fixed ? fixed + (size_t)g * n_vars : nullptr;
@@ -922,6 +936,11 @@ int afsat_create_ex(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64
             }
         }
         lit_off[order.size()] = w;
+        if (lit_off[order.size()] < ((int64_t)1 << 31)) {
+            g_cons[g].resize(order.size());
+            for (size_t j = 0; j < order.size(); ++j)
+                g_cons[g][j] = ConsDev{(int32_t)lit_off[j], (int16_t)cons_sig[j], (int16_t)sig_k[cons_sig[j]]};
+        }
         // work items: chunks of ONE signature, sized by the cost model and by the literal staging buffer
         std::vector<Item> &items = g_items[g];
         const int32_t nc = (int32_t)order.size();
@@ -976,6 +995,7 @@ int afsat_create_ex(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64
     for (int g = 0; g < G; ++g) {
         CREATE_FAIL(upload(ctx, &ctx->groups[g].d_lits, g_lits[g]));
         CREATE_FAIL(upload(ctx, &ctx->groups[g].d_items, g_items[g]));
+        if (g == 0 && n_sigs < 32768) CREATE_FAIL(upload(ctx, &ctx->groups[g].d_cons, g_cons[g]));
     }
     CREATE_FAIL(upload(ctx, &ctx->d_sigs, sigs));
     if (dtype == 32) {
@@ -984,10 +1004,16 @@ int afsat_create_ex(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64
         CREATE_FAIL(upload(ctx, &p, r32));
         ctx->d_rows = p;
         CREATE_FAIL(upload(ctx, &ctx->d_rows2, rows2));
+        std::vector<float> g32(rowsg.begin(), rowsg.end());
+        float *pg = nullptr;
+        CREATE_FAIL(upload(ctx, &pg, g32));
+        ctx->d_rowsg = pg;
     } else {
-        double *p = nullptr;
+        double *p = nullptr, *pg = nullptr;
         CREATE_FAIL(upload(ctx, &p, rows));
         ctx->d_rows = p;
+        CREATE_FAIL(upload(ctx, &pg, rowsg));
+        ctx->d_rowsg = pg;
     }
     {
         std::vector<int8_t> fx((size_t)G * n_vars, 0);
@@ -1019,22 +1045,22 @@ int afsat_create_ex(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64
 
     // ---- how afsat_step runs its loop ------------------------------------------------------------------------------------
     {
-        // PERSISTENT needs: one group, every length <= 8, X and G of 32 candidates in shared memory
-        const size_t smem = (size_t)2 * n_vars * 32 * esz;
+        // PERSISTENT needs: one group, every length <= 8, X and G of one candidate in shared memory
+        const size_t smem = (size_t)2 * n_vars * esz;
         int dev_smem = 0;
         cudaDeviceGetAttribute(&dev_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
-        const bool fits = G == 1 && groups[0].kmax <= AFSAT_A_KMAX && smem + 1024 <= (size_t)dev_smem;
+        const bool fits = G == 1 && groups[0].kmax <= AFSAT_A_KMAX && smem + 1024 <= (size_t)dev_smem && ctx->groups[0].d_cons;
         // launch-bound when one iteration's arithmetic is shorter than its launches (~2.5 us each): model instructions
         // over the FP32 issue rate of the whole chip at ~1.9 GHz
         const double est_us = (double)groups[0].fp_instr * batch / ((double)sm_count * 128 * 1.9e3);
         int path = opt.step_path;
         if (path == AFSAT_STEP_PERSISTENT && !fits) {
-            ctx->err = "AFSAT_STEP_PERSISTENT: the instance does not fit (one group, every length <= 8, 2 n 32 elements of shared memory)";
+            ctx->err = "AFSAT_STEP_PERSISTENT: the instance does not fit (one group, every length <= 8, X and G of a candidate in shared memory)";
             CREATE_FAIL(AFSAT_E_INVALID);
         }
         if (path == AFSAT_STEP_AUTO) {
             const int64_t tiles = (span + tile_w - 1) / tile_w * G;
-            path = (fits && est_us < 8.0 && batch <= 32 * sm_count) ? AFSAT_STEP_PERSISTENT
+            path = (fits && est_us < 8.0 && batch <= 8 * sm_count) ? AFSAT_STEP_PERSISTENT
                  : (est_us < 60.0 && tiles <= 8)                      ? AFSAT_STEP_GRAPH
                                                                       : AFSAT_STEP_LAUNCHES;
         }
@@ -1055,7 +1081,7 @@ int afsat_set_profiling(afsat_ctx *ctx, int32_t on)
 {
     if (!ctx) return AFSAT_E_INVALID;
     prof_drain(ctx, false);
-    ctx->prof_ns = 0.0; ctx->prof_launches = 0;
+    for (int i = 0; i < 3; ++i) { ctx->prof_ns[i] = 0.0; ctx->prof_launches[i] = 0; }
     ctx->profiling = on != 0;
     return AFSAT_OK;
 }
@@ -1065,8 +1091,8 @@ void afsat_destroy(afsat_ctx *ctx)
     if (!ctx) return;
     prof_drain(ctx, false);
     if (ctx->graph.exec) cudaGraphExecDestroy(ctx->graph.exec);
-    for (GroupPlan &gp : ctx->groups) { cudaFree(gp.d_lits); cudaFree(gp.d_items); }
-    cudaFree(ctx->d_bits); cudaFree(ctx->d_sigs); cudaFree(ctx->d_rows); cudaFree(ctx->d_rows2);
+    for (GroupPlan &gp : ctx->groups) { cudaFree(gp.d_lits); cudaFree(gp.d_items); cudaFree(gp.d_cons); }
+    cudaFree(ctx->d_bits); cudaFree(ctx->d_sigs); cudaFree(ctx->d_rows); cudaFree(ctx->d_rows2); cudaFree(ctx->d_rowsg);
     cudaFree(ctx->d_fixed); cudaFree(ctx->d_sat_const); cudaFree(ctx->d_G); cudaFree(ctx->d_Fpart);
     cudaFree(ctx->d_satacc); cudaFree(ctx->d_any);
     cudaFree(ctx->ls_G); cudaFree(ctx->ls_xt); cudaFree(ctx->ls_F0); cudaFree(ctx->ls_F1); cudaFree(ctx->ls_Dpart);
@@ -1259,9 +1285,11 @@ int afsat_step_host(afsat_ctx *ctx, void *h_x, double eta, int32_t n_steps, void
 int64_t afsat_query(const afsat_ctx *ctx, int32_t key)
 {
     if (!ctx) return -1;
-    if (key == AFSAT_Q_PROFILED_EVAL_NS || key == AFSAT_Q_PROFILED_EVAL_LAUNCHES) {
+    if (key == AFSAT_Q_PROFILED_EVAL_NS || key == AFSAT_Q_PROFILED_EVAL_LAUNCHES || key == AFSAT_Q_PROFILED_UPDATE_NS ||
+        key == AFSAT_Q_PROFILED_CHECK_NS) {
         prof_drain(const_cast<afsat_ctx *>(ctx), true);
-        return key == AFSAT_Q_PROFILED_EVAL_NS ? (int64_t)ctx->prof_ns : ctx->prof_launches;
+        return key == AFSAT_Q_PROFILED_EVAL_NS ? (int64_t)ctx->prof_ns[0] : key == AFSAT_Q_PROFILED_UPDATE_NS ? (int64_t)ctx->prof_ns[1]
+             : key == AFSAT_Q_PROFILED_CHECK_NS ? (int64_t)ctx->prof_ns[2] : ctx->prof_launches[0];
     }
     const GroupPlan &g0 = ctx->groups[0];
     switch (key) {

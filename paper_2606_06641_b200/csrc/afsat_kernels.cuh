@@ -43,8 +43,10 @@ struct SigDev {                 // 40 bytes, one per signature (type, k, param)
     uint64_t scan_lo, scan_hi;  // bit tau set: tau is in the SCANNED set of the discrete check
     int32_t scan_is_sat;        // 1: scanned set = satisfied counts; 0: = violated counts (smaller)
     int32_t k;
-    int32_t row2_off;           // packed fp32 kernel: first row of the STAGED table (ROW2 scalars per row, pack_rows_f2)
-    int8_t uv, n_unit, n_gen, pad;   // its unit variant, number of trivial-twiddle rows, number of generic complex rows
+    int32_t row2_off;           // first row of the STAGED table of the kernel that runs this length: rows2 (fp32, k <= 8,
+                                // ROW2 scalars per row, pack_rows_f2) or rowsg (grouped lane-split kernels, pack_rows_grp)
+    int8_t uv, n_unit, n_gen;   // rows2: unit variant, number of trivial-twiddle rows, number of generic complex rows
+    int8_t pad;                 // rowsg: the literal value whose factor is exactly 1 (0 or 1)
 };
 
 struct Item {                   // one CTA-sized chunk of constraints of a single signature
@@ -65,6 +67,7 @@ struct EvalParams {
     const SigDev *sigs;
     const T *rows;              // weight table
     const float *rows2;         // staged table of the packed fp32 kernel (fp32 contexts), else null
+    const T *rowsg;             // staged table of the grouped lane-split kernels (afsat_split.cuh), ROWG scalars per row
     const Item *items;          // items of this launch
     int32_t frow_base;          // row of Fpart for (items[0], group 0)
     int32_t B;

@@ -1,17 +1,24 @@
-// afsat_split.cuh -- lane-split register kernel for LONG fp32 constraints (k > AFSAT_B_KMAX32;
-// DESIGN.md 6.2b).  Internal to the library.
+// afsat_split.cuh -- lane-split register kernels for constraints too long for one lane per candidate (SURVEY.md §8(a)
+// a1-a5: fp32 k > 8, fp64 k > 20).  Internal to the library.
 //
 // One (constraint, candidate) evaluation is shared by NS lanes of a warp: lane (h, c) -- h = lane / (32 / NS),
 // c = lane % (32 / NS) -- owns the literals j = i NS + h, i < KS = ceil(k / NS), of candidate c.  Per DFT point
-// every lane walks ITS literals forward (prefixes of its own partial product), the NS partial
-// products are exchanged with warp shuffles, and the backward walk is seeded with  w b x (product of the OTHER
-// lanes' partial products):  the leave-one-out product of literal i in lane h is
-//     prefix_h(i) x suffix_h(i) x prod_{h' != h} P_h',
-// still a product of factors, never a division (north_star).  Every intermediate of a point -- the KS literal values,
-// factors, prefixes and partial gradients of the lane -- then fits in registers WITHOUT spills at k = 64, at twice the
-// warps per SM of the one-lane-per-candidate kernel (k_eval_km: 255 registers, spills beyond k ~ 36); the arithmetic
-// per literal and point is the same 12 instructions, plus one exchange (2 (NS - 1) shuffles, NS - 1 + 2 complex
-// multiplies) per point.  Literals missing from the last row (j >= k) are unit factors.
+// every lane forms the partial product of ITS literals, the NS partial products are exchanged with warp
+// shuffles, and the backward walk is seeded with  w x (product of the OTHER lanes' partial products): a leave-one-out
+// product is always prefix x suffix x the others' products, still a product of factors, never a division (north_star).
+//
+// Literal GROUPS (scalar form).  Inside a lane the literals are taken M at a time: the product of a group's factors is
+// the polynomial  prod_{u<M} (a + b y_u) = sum_{j<=M} a^(M-j) b^j e_j(y_group)  in its M + 1 elementary symmetric
+// polynomials, which do not depend on the DFT point -- they are formed once per constraint -- so at every point a group
+// costs 2 M FMAs for its (complex) factor instead of M factors and M - 1 complex multiplies, the prefix / suffix walk
+// runs over ceil(KS / M) group factors instead of KS, and the partial gradients come out of M accumulators per group,
+//     A_j += Re( w a^(M-j) b^j x prefix_g x suffix_g x others ),     dFE/dy_u = sum_j A_j e_{j-1}(y_group without y_u),
+// expanded once per constraint.  Per literal and complex point that is 4 + 12 / M instructions instead of 12 (M = 4: 7);
+// the generating polynomial is still evaluated at every DFT point and contracted with the same weights -- the groups
+// only change the order in which its factors are multiplied.  A slot without a literal (k not a multiple of NS, KS not
+// a multiple of M) holds the value `pad` for which the factor is exactly 1 at every point: 0 for the paper's tables
+// (staged un-halved, a = 1, b = w^l, the 2^-k folded into the weights -- an exact rescale), 1 for the robust tables
+// (a + b = 1).
 #pragma once
 #include "afsat_internal.h"
 #include "afsat_kernels.cuh"
@@ -22,19 +29,16 @@ namespace afsat {
 #define AFSAT_L32_NS 2                 // lanes per (constraint, candidate)
 #endif
 #ifndef AFSAT_L32_THREADS
-#define AFSAT_L32_THREADS 384             // 12 warps per SM at 168 registers (measured: 256 / 255 regs 5 % slower)
+#define AFSAT_L32_THREADS 384             // 12 warps per SM at 168 registers
 #endif
 #ifndef AFSAT_L32_MINB
 #define AFSAT_L32_MINB 1
-#endif
-#ifndef AFSAT_L32_CHAINS
-#define AFSAT_L32_CHAINS 2             // independent product chains per thread at a complex point
 #endif
 #ifndef AFSAT_M32_THREADS
 #define AFSAT_M32_THREADS 384
 #endif
 #ifndef AFSAT_L64_THREADS
-#define AFSAT_L64_THREADS 384             // 168 registers, 12 warps per SM (256 x 255 registers: 4.25 vs 4.07 ms on cfg3)
+#define AFSAT_L64_THREADS 384
 #endif
 #define AFSAT_L64_KMIN (AFSAT_B_KMAX + 1)   // fp64, k > 20: FOUR lanes per candidate (a double takes two registers)
 #ifndef AFSAT_L32_PREFETCH
@@ -43,6 +47,40 @@ namespace afsat {
 #ifndef AFSAT_L32_KMIN
 #define AFSAT_L32_KMIN (AFSAT_B_KMAX + 1)
 #endif
+#ifndef AFSAT_GRP_M
+#define AFSAT_GRP_M 4                  // literals per group
+#endif
+constexpr int GRP_M = AFSAT_GRP_M;
+constexpr int ROWG = 2 * (GRP_M + 1) + 2;   // staged row of a grouped kernel: {Re c_0, Im c_0, ..., Re c_M, Im c_M, Re w, Im w}
+
+// HOST: the staged table of one signature for the grouped kernels, from its rows {Re a, Im a, Re b, Im b, Re w, Im w, ..}
+// (real rows first): c_j = a^(M-j) b^j.  The paper's tables (a = 1/2 in every row) are staged un-halved (see above).
+// Returns the pad value (0 or 1).
+inline int pack_rows_grp(const double *r0, int n_rows, int k, double *out)
+{
+    bool std_tab = true;
+    for (int q = 0; q < n_rows; ++q) std_tab = std_tab && r0[8 * q] == 0.5 && r0[8 * q + 1] == 0.0;
+    const double sc = std_tab ? 2.0 : 1.0;
+    double scw = 1.0;
+    if (std_tab) for (int i = 0; i < k; ++i) scw *= 0.5;
+    for (int q = 0; q < n_rows; ++q) {
+        const double *r = r0 + 8 * q;
+        double *o = out + (size_t)q * ROWG;
+        const double ar = sc * r[0], ai = sc * r[1], br = sc * r[2], bi = sc * r[3];
+        // a^(M-j) b^j by repeated multiplication of double-precision values (M <= 6: relative error ~1e-15)
+        for (int j = 0; j <= GRP_M; ++j) {
+            double cr = 1.0, ci = 0.0;
+            for (int t = 0; t < GRP_M; ++t) {
+                const double fr = t < j ? br : ar, fi = t < j ? bi : ai;
+                const double nr = cr * fr - ci * fi, ni = cr * fi + ci * fr;
+                cr = nr; ci = ni;
+            }
+            o[2 * j] = cr; o[2 * j + 1] = ci;
+        }
+        o[2 * GRP_M + 2] = r[4] * scw; o[2 * GRP_M + 3] = r[5] * scw;
+    }
+    return std_tab ? 0 : 1;
+}
 
 // product of the OTHER lanes' values (NS = 2: the partner's; NS = 4: butterfly over lane bits log2(CW), log2(CW) + 1)
 template <typename T, int NS>
@@ -65,101 +103,136 @@ __device__ __forceinline__ void others_cplx(unsigned mask, T vr, T vi, T &orr, T
     orr = fma_(n1r, por, -(n1i * poi)); oi = fma_(n1r, poi, n1i * por);
 }
 
-// a2-a4 for the lane's KS literals of one constraint; tab rows as in eval_points_reg ({Re a, Im a, Re b, Im b,
-// Re w, Im w, Re(w b), Im(w b)}, real rows first).  miss: the lane's LAST literal does not exist (unit factor).
+// a2-a4 for the lane's KS literal slots of one constraint (slots without a literal hold `pad`); tab: ROWG scalars per
+// retained DFT point, real points first.  Returns the lane's partial gradients dFE/dy_i in g.
 template <typename T, int KS, int NS, bool GRAD>
-__device__ __forceinline__ void eval_points_split(unsigned mask, const T (&y)[KS], bool miss,
-                                                  const T *__restrict__ tab, int n_real, int n_cplx, T &fe,
-                                                  T (&g)[KS])
+__device__ __forceinline__ void eval_points_grp(unsigned mask, const T (&y)[KS], T pad, const T *__restrict__ tab, int n_real,
+                                                int n_cplx, T &fe, T (&g)[KS])
 {
+    constexpr int M = GRP_M, NG = (KS + M - 1) / M;
+    T e[NG][M], A[NG][M];                                            // e[g][j-1] = e_j(group g); A[g][j-1] pairs with c_j
+#pragma unroll
+    for (int gq = 0; gq < NG; ++gq) {
+        T ee[M + 1];
+        ee[0] = T(1);
+#pragma unroll
+        for (int j = 1; j <= M; ++j) ee[j] = T(0);
+#pragma unroll
+        for (int u = 0; u < M; ++u) {
+            const T yv = (gq * M + u < KS) ? y[gq * M + u < KS ? gq * M + u : 0] : pad;
+#pragma unroll
+            for (int j = M; j >= 1; --j)
+                if (j <= u + 1) ee[j] = fma_(yv, ee[j - 1], ee[j]);
+        }
+#pragma unroll
+        for (int j = 0; j < M; ++j) { e[gq][j] = ee[j + 1]; A[gq][j] = T(0); }
+    }
     const T *r = tab;
-    for (int p = 0; p < n_real; ++p, r += 8) {                       // self-conjugate points
-        const T a = r[0], b = r[2], w = r[4], wb = r[6];
-        T pre[KS], f[KS];
+    for (int p = 0; p < n_real; ++p, r += ROWG) {                    // self-conjugate points
+        T c[M + 1];
 #pragma unroll
-        for (int i = 0; i < KS; ++i) f[i] = fma_(b, y[i], a);
-        if (miss) f[KS - 1] = T(1);
-        T run = f[0];
+        for (int j = 0; j <= M; ++j) c[j] = r[2 * j];
+        const T w = r[2 * M + 2];
+        T q[NG], pre[NG];
 #pragma unroll
-        for (int i = 1; i < KS; ++i) { pre[i] = run; run *= f[i]; }
+        for (int gq = 0; gq < NG; ++gq) {
+            T sacc = c[0];
+#pragma unroll
+            for (int j = 0; j < M; ++j) sacc = fma_(c[j + 1], e[gq][j], sacc);
+            q[gq] = sacc;
+        }
+        T run = q[0];
+#pragma unroll
+        for (int gq = 1; gq < NG; ++gq) { pre[gq] = run; run *= q[gq]; }
         const T oth = others_real<T, NS>(mask, run);
-        fe = fma_(w, run * oth, fe);
+        T suf = w * oth;
+        fe = fma_(suf, run, fe);
         if (GRAD) {
-            T suf = wb * oth;
 #pragma unroll
-            for (int i = KS - 1; i >= 1; --i) { g[i] = fma_(pre[i], suf, g[i]); suf *= f[i]; }
-            g[0] += suf;                                              // prefix_0 = 1
+            for (int gq = NG - 1; gq >= 0; --gq) {
+                const T t = gq > 0 ? pre[gq] * suf : suf;
+#pragma unroll
+                for (int j = 0; j < M; ++j) A[gq][j] = fma_(c[j + 1], t, A[gq][j]);
+                if (gq > 0) suf *= q[gq];
+            }
         }
     }
-    // complex points: the lane's literals are walked as TWO independent chains, A = [0, KA) and B = [KA, KS) -- the
-    // same leave-one-out identity one level down (LOO_i = prefix_A(i) suffix_A(i) P_B others) -- so that a thread
-    // always has two dependent FMUL -> FFMA sequences in flight (with 3 warps per scheduler one chain per thread
-    // leaves the issue slots idle on fixed-latency waits: profiles/r1_eval_split_cfg3.md)
-    constexpr int KA = AFSAT_L32_CHAINS == 2 ? KS / 2 : KS, KB = KS - KA;
-    for (int p = 0; p < n_cplx; ++p, r += 8) {                       // one of each conjugate pair
-        const T ar = r[0], ai = r[1], br = r[2], bi = r[3], wr = r[4], wi = r[5], wbr = r[6], wbi = r[7];
-        T pr[KS], pi[KS], fr[KS], fi[KS];
+    for (int p = 0; p < n_cplx; ++p, r += ROWG) {                    // one of each conjugate pair
+        T cr[M + 1], ci[M + 1];
 #pragma unroll
-        for (int i = 0; i < KS; ++i) { fr[i] = fma_(br, y[i], ar); fi[i] = fma_(bi, y[i], ai); }
-        if (miss) { fr[KS - 1] = T(1); fi[KS - 1] = T(0); }
-        T rr = fr[0], ri = fi[0], qr = T(1), qi = T(0);
-        if (KB > 0) { qr = fr[KA]; qi = fi[KA]; }
+        for (int j = 0; j <= M; ++j) { cr[j] = r[2 * j]; ci[j] = r[2 * j + 1]; }
+        const T wr = r[2 * M + 2], wi = r[2 * M + 3];
+        T qr[NG], qi[NG], pr[NG], pi[NG];
 #pragma unroll
-        for (int i = 1; i < (KA > KB ? KA : KB); ++i) {
-            if (i < KA) {
-                pr[i] = rr; pi[i] = ri;
-                const T nr = fma_(rr, fr[i], -(ri * fi[i]));
-                const T ni = fma_(rr, fi[i], ri * fr[i]);
-                rr = nr; ri = ni;
-            }
-            if (i < KB) {
-                pr[KA + i] = qr; pi[KA + i] = qi;
-                const T nr = fma_(qr, fr[KA + i], -(qi * fi[KA + i]));
-                const T ni = fma_(qr, fi[KA + i], qi * fr[KA + i]);
-                qr = nr; qi = ni;
-            }
+        for (int gq = 0; gq < NG; ++gq) {
+            T sr = cr[0], si = ci[0];
+#pragma unroll
+            for (int j = 0; j < M; ++j) { sr = fma_(cr[j + 1], e[gq][j], sr); si = fma_(ci[j + 1], e[gq][j], si); }
+            qr[gq] = sr; qi[gq] = si;
         }
-        T lr = rr, li = ri;                                       // the lane's partial product P_A P_B
-        if (KB > 0) { lr = fma_(rr, qr, -(ri * qi)); li = fma_(rr, qi, ri * qr); }
-        T orr, oi;
-        others_cplx<T, NS>(mask, lr, li, orr, oi);
-        const T tr = fma_(lr, orr, -(li * oi)), ti = fma_(lr, oi, li * orr);   // P_l, the whole product
-        fe = fma_(wr, tr, fe);
-        fe = fma_(-wi, ti, fe);
-        if (GRAD) {
-            const T zr = fma_(wbr, orr, -(wbi * oi)), zi = fma_(wbr, oi, wbi * orr);   // w b x others
-            T sr = zr, si = zi, ur = zr, ui = zi;                 // suffix of chain A seeded with z P_B, of B with z P_A
-            if (KB > 0) {
-                sr = fma_(zr, qr, -(zi * qi)); si = fma_(zr, qi, zi * qr);
-                ur = fma_(zr, rr, -(zi * ri)); ui = fma_(zr, ri, zi * rr);
-            }
+        T rr = qr[0], ri = qi[0];
 #pragma unroll
-            for (int i = (KA > KB ? KA : KB) - 1; i >= 1; --i) {
-                if (i < KA) {
-                    g[i] = fma_(pr[i], sr, g[i]);
-                    g[i] = fma_(-pi[i], si, g[i]);
-                    const T nr = fma_(sr, fr[i], -(si * fi[i]));
-                    const T ni = fma_(sr, fi[i], si * fr[i]);
+        for (int gq = 1; gq < NG; ++gq) {
+            pr[gq] = rr; pi[gq] = ri;
+            const T nr = fma_(rr, qr[gq], -(ri * qi[gq]));
+            const T ni = fma_(rr, qi[gq], ri * qr[gq]);
+            rr = nr; ri = ni;
+        }
+        T orr, oi;
+        others_cplx<T, NS>(mask, rr, ri, orr, oi);
+        T sr = fma_(wr, orr, -(wi * oi)), si = fma_(wr, oi, wi * orr);      // suffix seeded with w x others
+        fe = fma_(sr, rr, fe);
+        fe = fma_(-si, ri, fe);                                              // Re(w others P_lane)
+        if (GRAD) {
+#pragma unroll
+            for (int gq = NG - 1; gq >= 0; --gq) {
+                T tr = sr, ti = si;
+                if (gq > 0) { tr = fma_(pr[gq], sr, -(pi[gq] * si)); ti = fma_(pr[gq], si, pi[gq] * sr); }
+#pragma unroll
+                for (int j = 0; j < M; ++j) {
+                    A[gq][j] = fma_(cr[j + 1], tr, A[gq][j]);
+                    A[gq][j] = fma_(-ci[j + 1], ti, A[gq][j]);               // Re(c_j T)
+                }
+                if (gq > 0) {
+                    const T nr = fma_(sr, qr[gq], -(si * qi[gq]));
+                    const T ni = fma_(sr, qi[gq], si * qr[gq]);
                     sr = nr; si = ni;
                 }
-                if (i < KB) {
-                    g[KA + i] = fma_(pr[KA + i], ur, g[KA + i]);
-                    g[KA + i] = fma_(-pi[KA + i], ui, g[KA + i]);
-                    const T nr = fma_(ur, fr[KA + i], -(ui * fi[KA + i]));
-                    const T ni = fma_(ur, fi[KA + i], ui * fr[KA + i]);
-                    ur = nr; ui = ni;
-                }
             }
-            g[0] += sr;                                               // prefix_0 = 1 in both chains
-            if (KB > 0) g[KA] += ur;
         }
+    }
+    if (GRAD) {                                                       // dFE/dy_u = sum_j A_j e_{j-1}(group without y_u)
+#pragma unroll
+        for (int gq = 0; gq < NG; ++gq)
+#pragma unroll
+            for (int u = 0; u < M; ++u) {
+                if (gq * M + u >= KS) continue;
+                T ee[M];
+                ee[0] = T(1);
+#pragma unroll
+                for (int j = 1; j < M; ++j) ee[j] = T(0);
+                int cntv = 0;
+#pragma unroll
+                for (int v = 0; v < M; ++v) {
+                    if (v == u) continue;
+                    const T yv = (gq * M + v < KS) ? y[gq * M + v < KS ? gq * M + v : 0] : pad;
+#pragma unroll
+                    for (int j = M - 1; j >= 1; --j)
+                        if (j <= cntv + 1) ee[j] = fma_(yv, ee[j - 1], ee[j]);
+                    ++cntv;
+                }
+                T acc = A[gq][0];
+#pragma unroll
+                for (int j = 1; j < M; ++j) acc = fma_(A[gq][j], ee[j], acc);
+                g[gq * M + u] = acc;
+            }
     }
 }
 
 template <typename T, int KS, int NS, bool GRAD>
 __device__ __forceinline__ void run_item_split(const EvalParams<T> &p, unsigned mask, const int32_t *__restrict__ s_lits,
                                                const T *__restrict__ s_tab, int n_real, int n_cplx, int nc, int wk,
-                                               int h, int64_t b, T &fe, int k)
+                                               int h, int64_t b, T &fe, int k, T pad)
 {
     const char *xb = reinterpret_cast<const char *>(p.x + b);
     char *gb = reinterpret_cast<char *>(p.G + (b - p.g_b0));
@@ -172,12 +245,11 @@ __device__ __forceinline__ void run_item_split(const EvalParams<T> &p, unsigned 
         T y[KS], g[KS];
 #pragma unroll
         for (int i = 0; i < KS - 1; ++i) lit[i] = L[i * NS];
-        lit[KS - 1] = miss ? LIT_NONE : L[(KS - 1) * NS];             // missing literal: constant, no gather, no RED
+        lit[KS - 1] = miss ? LIT_NONE : L[(KS - 1) * NS];             // missing literal: the pad value, no gather, no RED
 #pragma unroll
         for (int i = 0; i < KS; ++i) {
-            if (i == KS - 1 && (lit[i] & LIT_NONE)) y[i] = T(1);
-            else y[i] = __ldg(reinterpret_cast<const T *>(xb + (uint64_t)(uint32_t)(lit[i] & LIT_VAR) * x_ld));
-            y[i] = flip_sign(y[i], lit[i]);
+            if (i == KS - 1 && (lit[i] & LIT_NONE)) y[i] = pad;
+            else y[i] = flip_sign(__ldg(reinterpret_cast<const T *>(xb + (uint64_t)(uint32_t)(lit[i] & LIT_VAR) * x_ld)), lit[i]);
             g[i] = T(0);
         }
 #if AFSAT_L32_PREFETCH
@@ -191,7 +263,7 @@ __device__ __forceinline__ void run_item_split(const EvalParams<T> &p, unsigned 
             }
         }
 #endif
-        eval_points_split<T, KS, NS, GRAD>(mask, y, miss, s_tab, n_real, n_cplx, fe, g);
+        eval_points_grp<T, KS, NS, GRAD>(mask, y, pad, s_tab, n_real, n_cplx, fe, g);
         if (GRAD) {
 #pragma unroll
             for (int i = 0; i < KS; ++i) {
@@ -205,7 +277,7 @@ __device__ __forceinline__ void run_item_split(const EvalParams<T> &p, unsigned 
 
 template <typename T, int KS, int NS, bool GRAD>
 __device__ __noinline__ void item_body_split(const EvalParams<T> &p, const int32_t *s_lits, const T *s_tab,
-                                             T (*s_F)[32], int n_real, int n_cplx, int nc, int k)
+                                             T (*s_F)[32], int n_real, int n_cplx, int nc, int k, T pad)
 {
     constexpr int CW = 32 / NS;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -215,9 +287,7 @@ __device__ __noinline__ void item_body_split(const EvalParams<T> &p, const int32
     const bool active = b < p.b_end && b < p.B && !lane_skipped(p, b, 1);   // the NS lanes of a candidate agree
     const unsigned mask = __ballot_sync(0xffffffffu, active);
     T fe = T(0);
-    if (active) {
-        run_item_split<T, KS, NS, GRAD>(p, mask, s_lits, s_tab, n_real, n_cplx, nc, wk, h, b, fe, k);
-    }
+    if (active) run_item_split<T, KS, NS, GRAD>(p, mask, s_lits, s_tab, n_real, n_cplx, nc, wk, h, b, fe, k, pad);
     if (!p.Fpart) return;
     s_F[warp][lane] = fe;
     __syncthreads();
@@ -384,29 +454,38 @@ __device__ __noinline__ void item_body_split2(const EvalParams<float> &p, const 
 template <typename T, int KS, int KSHI, int NS, int V, bool GRAD>
 struct SwitchSplit {
     static __device__ __forceinline__ void go(int ks, const EvalParams<T> &p, const int32_t *s_lits, const T *s_tab,
-                                              T (*s_F)[32 * V], int n_real, int n_cplx, int nc, int k)
+                                              T (*s_F)[32 * V], int n_real, int n_cplx, int nc, int k, T pad)
     {
         if (ks == KS) {
             if constexpr (V == 2) item_body_split2<KS, NS, GRAD>(p, s_lits, s_tab, s_F, n_real, n_cplx, nc, k);
-            else item_body_split<T, KS, NS, GRAD>(p, s_lits, s_tab, s_F, n_real, n_cplx, nc, k);
+            else item_body_split<T, KS, NS, GRAD>(p, s_lits, s_tab, s_F, n_real, n_cplx, nc, k, pad);
         } else if (KS < KSHI)
-            SwitchSplit<T, (KS < KSHI ? KS + 1 : KS), KSHI, NS, V, GRAD>::go(ks, p, s_lits, s_tab, s_F, n_real, n_cplx, nc, k);
+            SwitchSplit<T, (KS < KSHI ? KS + 1 : KS), KSHI, NS, V, GRAD>::go(ks, p, s_lits, s_tab, s_F, n_real, n_cplx, nc, k, pad);
     }
 };
 
-// one launch for every length in [KLO, KHI]: the CTA's item picks the body compiled for ceil(k / NS) literals per lane
+// one launch for every length in [KLO, KHI]: the CTA's item picks the body compiled for ceil(k / NS) literals per lane.
+// V = 1: grouped scalar form (staged table rowsg, ROWG scalars per point); V = 2: packed form (table rows, 8 per point).
 template <typename T, int KLO, int KHI, int NS, int V, bool GRAD, int THREADS, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB) k_eval_split(const EvalParams<T> p)
 {
-    __shared__ __align__(16) T s_tab[((KHI + 1) / 2 + 1) * 8];
+    constexpr int RW = V == 1 ? ROWG : 8;
+    __shared__ __align__(16) T s_tab[((KHI + 1) / 2 + 1) * RW];
     __shared__ int32_t s_lits[LIT_CHUNK];
     __shared__ T s_F[THREADS / 32][32 * V];
     const Item it = p.items[blockIdx.x];
     const SigDev sg = p.sigs[it.sig];
-    stage_item(p, it, sg, s_tab, s_lits);
+    if (V == 1) {
+        const int nsc = (sg.n_real + sg.n_cplx) * ROWG;
+        for (int i = threadIdx.x; i < nsc; i += blockDim.x) s_tab[i] = p.rowsg[(int64_t)sg.row2_off * ROWG + i];
+        const int nl = (it.c_end - it.c_begin) * it.k;
+        for (int i = threadIdx.x; i < nl; i += blockDim.x) s_lits[i] = __ldg(p.lits + it.lit_base + i);
+    } else {
+        stage_item(p, it, sg, s_tab, s_lits);
+    }
     __syncthreads();
     SwitchSplit<T, (KLO + NS - 1) / NS, (KHI + NS - 1) / NS, NS, V, GRAD>::go((it.k + NS - 1) / NS, p, s_lits, s_tab, s_F, sg.n_real,
-                                                                        sg.n_cplx, it.c_end - it.c_begin, it.k);
+                                                                        sg.n_cplx, it.c_end - it.c_begin, it.k, (T)sg.pad);
 }
 
 #ifndef AFSAT_KS32_TU   // instantiated in afsat_ks32.cu

@@ -410,22 +410,27 @@ __global__ void k_reset_state(int B, int reset_candidates, uint8_t *is_solution,
 
 // ---- the whole step loop in ONE launch (small instances: PAPER.md:81 "compiled once and executed repeatedly", :103
 // the lock-step loop runs on the accelerator) ------------------------------------------------
-// A CTA owns 32 candidates (lane = candidate) for all n_steps iterations: X and G of those candidates live in shared
-// memory as [n][32] columns, the warps share out the constraints, partial gradients meet in shared-memory atomics, and
-// the gather of iteration t + 1 also yields the sign bits of X(t), so the exact count (a8) rides on the same pass.
-// Candidates never exchange data, so no CTA waits on another.  Lengths k <= 8 only (one register body per length).
+// Such instances are bound by launch latency, not by arithmetic (cfg0: 1.4e4 evaluations per step), and a batch of a
+// few dozen candidates cannot fill the machine with lane = candidate.  So here a CTA owns ONE candidate for all n_steps
+// iterations and its THREADS share out the constraints (thread = constraint; bucket order keeps the constraints of a
+// warp on one signature, so the length switch rarely diverges): X and G of the candidate live in shared memory, partial
+// gradients meet in shared-memory atomics, and the gather of iteration t + 1 also yields the signs of X(t), so the
+// exact count (a8) rides on the same pass.  Candidates never exchange data: no CTA waits on another, and a solved
+// candidate's CTA simply ends.  Lengths k <= 8 only (one register body per length).
+struct ConsDev { int32_t lit_off; int16_t sig; int16_t k; };       // one constraint in bucket order
+
 template <typename T>
 struct SmallParams {
     T *x;                       // [n][ldb], in/out
     int64_t ldb;
-    int32_t n, B, m, n_items;
+    int32_t n, B, m, m_live;
     const int32_t *lits;
-    const Item *items;
+    const ConsDev *cons;
     const SigDev *sigs;
     const T *rows;
     const int8_t *fixed;
     T eta;
-    int32_t n_steps, step_base, sat_const, n_ctas;
+    int32_t n_steps, step_base, sat_const;
     int32_t *sat_count;
     uint8_t *is_solution;
     int32_t *first_step;
@@ -436,69 +441,68 @@ constexpr int SMALL_THREADS = 512;
 
 template <typename T, int K, bool GRAD>
 __device__ __forceinline__ int small_constraint(const int32_t *__restrict__ L, const T *__restrict__ sx, T *__restrict__ sg,
-                                                const T *__restrict__ tab, const SigDev &sg_, int lane)
+                                                const T *__restrict__ tab, int n_real, int n_cplx, uint64_t scan_lo, int scan_is_sat)
 {
     int32_t lit[K];
     T y[K][1], g[K][1], fe[1] = {T(0)};
     int tau = 0;
 #pragma unroll
+    for (int i = 0; i < K; ++i) lit[i] = __ldg(L + i);
+#pragma unroll
     for (int i = 0; i < K; ++i) {
-        lit[i] = __ldg(L + i);
-        const T xv = sx[(lit[i] & LIT_VAR) * 32 + lane];
+        const T xv = sx[lit[i] & LIT_VAR];
         tau += (int)((xv < T(0)) != (lit[i] < 0));                    // literal true = variable true XOR negated (B2)
         y[i][0] = flip_sign(xv, lit[i]);
         g[i][0] = T(0);
     }
     if (GRAD) {
-        eval_points_reg<T, K, 1, true>(y, tab, sg_.n_real, sg_.n_cplx, fe, g);
+        eval_points_reg<T, K, 1, true>(y, tab, n_real, n_cplx, fe, g);
 #pragma unroll
-        for (int i = 0; i < K; ++i) atomicAdd(sg + (lit[i] & LIT_VAR) * 32 + lane, flip_sign(g[i][0], lit[i]));
+        for (int i = 0; i < K; ++i) atomicAdd(sg + (lit[i] & LIT_VAR), flip_sign(g[i][0], lit[i]));
     }
-    const uint64_t bit = tau < 64 ? (sg_.scan_lo >> tau) : (sg_.scan_hi >> (tau - 64));
-    return (int)(bit & 1ull) == sg_.scan_is_sat;
+    return (int)((scan_lo >> tau) & 1ull) == scan_is_sat;             // k <= 8: tau < 64
 }
 
 template <typename T>
 __global__ void __launch_bounds__(SMALL_THREADS, 1) k_step_small(const SmallParams<T> p)
 {
     extern __shared__ __align__(16) unsigned char s_raw[];
-    T *sx = reinterpret_cast<T *>(s_raw), *sg = sx + (size_t)p.n * 32;
-    __shared__ int s_cnt[32], s_frozen[32];
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = blockDim.x >> 5;
-    const int64_t b0 = (int64_t)blockIdx.x * 32, b = b0 + lane;
-    const bool live = b < p.B;
-    for (int i = threadIdx.x; i < p.n * 32; i += blockDim.x) sx[i] = p.x[(int64_t)(i >> 5) * p.ldb + b0 + (i & 31)];
-    if (warp == 0) s_frozen[lane] = live ? (int)p.is_solution[b] : 1;
+    T *sx = reinterpret_cast<T *>(s_raw), *sg = sx + p.n;
+    __shared__ int s_cnt, s_frozen;
+    const int t = threadIdx.x, nt = blockDim.x;
+    const int64_t b = blockIdx.x;
+    for (int v = t; v < p.n; v += nt) sx[v] = p.x[(int64_t)v * p.ldb + b];
+    if (t == 0) { s_frozen = (int)p.is_solution[b]; s_cnt = 0; }
     int last = 0;
     for (int it = 0; it <= p.n_steps; ++it) {
         const bool grad = it < p.n_steps;
-        if (grad) for (int i = threadIdx.x; i < p.n * 32; i += blockDim.x) sg[i] = T(0);
-        if (warp == 0) s_cnt[lane] = 0;
+        if (grad) for (int v = t; v < p.n; v += nt) sg[v] = T(0);
         __syncthreads();
+        if (s_frozen && it > 0) break;                                // solved: X and its count no longer change (a9)
         int cnt = 0;
-        for (int item = 0; item < p.n_items; ++item) {
-            const Item itm = p.items[item];
-            const SigDev sd = p.sigs[itm.sig];
-            const T *tab = p.rows + (int64_t)sd.row_off * 8;
-            const int nc = itm.c_end - itm.c_begin, k = itm.k;
-            int c = (warp - itm.c_begin % nw + nw) % nw;              // constraint (c_begin + c) belongs to warp (c_begin + c) % nw
-            for (; c < nc; c += nw) {
-                const int32_t *L = p.lits + itm.lit_base + (int64_t)c * k;
-#define AFSAT_SMALL_CASE(K_) case K_: cnt += grad ? small_constraint<T, K_, true>(L, sx, sg, tab, sd, lane) \
-                                                  : small_constraint<T, K_, false>(L, sx, sg, tab, sd, lane); break;
-                switch (k) {
-                    AFSAT_SMALL_CASE(1) AFSAT_SMALL_CASE(2) AFSAT_SMALL_CASE(3) AFSAT_SMALL_CASE(4)
-                    AFSAT_SMALL_CASE(5) AFSAT_SMALL_CASE(6) AFSAT_SMALL_CASE(7) AFSAT_SMALL_CASE(8)
-                }
-#undef AFSAT_SMALL_CASE
+        for (int j = t; j < p.m_live; j += nt) {
+            const ConsDev c = p.cons[j];
+            const int32_t *L = p.lits + c.lit_off;
+            const SigDev *sd = p.sigs + c.sig;
+            const T *tab = p.rows + (int64_t)sd->row_off * 8;
+            const int n_real = sd->n_real, n_cplx = sd->n_cplx, sis = sd->scan_is_sat;
+            const uint64_t slo = sd->scan_lo;
+#define AFSAT_SMALL_CASE(K_) case K_: cnt += grad ? small_constraint<T, K_, true>(L, sx, sg, tab, n_real, n_cplx, slo, sis) \
+                                                  : small_constraint<T, K_, false>(L, sx, sg, tab, n_real, n_cplx, slo, sis); break;
+            switch (c.k) {
+                AFSAT_SMALL_CASE(1) AFSAT_SMALL_CASE(2) AFSAT_SMALL_CASE(3) AFSAT_SMALL_CASE(4)
+                AFSAT_SMALL_CASE(5) AFSAT_SMALL_CASE(6) AFSAT_SMALL_CASE(7) AFSAT_SMALL_CASE(8)
             }
+#undef AFSAT_SMALL_CASE
         }
-        if (cnt) atomicAdd(&s_cnt[lane], cnt);
+        cnt = __reduce_add_sync(0xffffffffu, cnt);
+        if ((t & 31) == 0 && cnt) atomicAdd(&s_cnt, cnt);
         __syncthreads();
-        if (warp == 0) {                                              // a8, a9 on X(it): X(0) is counted but not marked (A11)
-            last = s_cnt[lane] + p.sat_const;
-            if (live && it >= 1 && last == p.m && !s_frozen[lane]) {
-                s_frozen[lane] = 1;
+        if (t == 0) {                                                 // a8, a9 on X(it): X(0) is counted but not marked (A11)
+            last = s_cnt + p.sat_const;
+            s_cnt = 0;
+            if (it >= 1 && last == p.m && !s_frozen) {
+                s_frozen = 1;
                 p.is_solution[b] = 1;
                 const int step = p.step_base + it;
                 p.first_step[b] = step;
@@ -509,24 +513,21 @@ __global__ void __launch_bounds__(SMALL_THREADS, 1) k_step_small(const SmallPara
         }
         if (!grad) break;
         __syncthreads();
-        for (int i = threadIdx.x; i < p.n * 32; i += blockDim.x) {    // a6: projected step in shared memory
-            const int v = i >> 5;
-            if (!s_frozen[i & 31] && !p.fixed[v]) {
-                T nx = fma_(-p.eta, sg[i], sx[i]);
-                nx = nx > T(1) ? T(1) : nx;
-                nx = nx < T(-1) ? T(-1) : nx;
-                sx[i] = nx;
-            }
-        }
-        __syncthreads();
+        if (!s_frozen)
+            for (int v = t; v < p.n; v += nt)                         // a6: projected step in shared memory
+                if (!p.fixed[v]) {
+                    T nx = fma_(-p.eta, sg[v], sx[v]);
+                    nx = nx > T(1) ? T(1) : nx;
+                    nx = nx < T(-1) ? T(-1) : nx;
+                    sx[v] = nx;
+                }
     }
-    if (warp == 0 && live) p.sat_count[b] = last;
+    if (t == 0) p.sat_count[b] = last;
     __syncthreads();
-    for (int i = threadIdx.x; i < p.n * 32; i += blockDim.x)
-        if (b0 + (i & 31) < p.B) p.x[(int64_t)(i >> 5) * p.ldb + b0 + (i & 31)] = sx[i];
-    if (threadIdx.x == 0 && p.h_any) {                                // the last CTA settles the host copy of the first step
+    for (int v = t; v < p.n; v += nt) p.x[(int64_t)v * p.ldb + b] = sx[v];
+    if (t == 0 && p.h_any) {                                          // the last CTA settles the host copy of the first step
         __threadfence();
-        if (atomicAdd(p.d_any + 2, 1) == p.n_ctas - 1 && p.d_any[0]) {
+        if (atomicAdd(p.d_any + 2, 1) == (int)gridDim.x - 1 && p.d_any[0]) {
             p.h_any[1] = atomicMin(p.d_any + 1, 0x7fffffff);
             __threadfence_system();
             p.h_any[0] = 1;

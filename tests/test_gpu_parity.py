@@ -804,7 +804,7 @@ def test_partial_assignment_is_substituted():
     xg[inst.fixed != 0] = 0.123
     F1, G1 = run_eval(inst, x, 64, 64)
     F2, G2 = run_eval(inst, xg, 64, 64)
-    assert np.array_equal(F1, F2) and np.array_equal(G1, G2)
+    assert np.array_equal(F1, F2) and np.abs(G1 - G2).max() <= 1e-12          # G: the REDs arrive in any order
 
 
 # ---- several partial assignments, the batch divided evenly among them -----
@@ -879,14 +879,15 @@ def test_several_partial_assignments(dtype):
 def test_step_paths_agree(dtype):
     """The same 40 steps through the three loop forms (k <= 8, a partial assignment, B = 80: a ragged last CTA):
     identical discrete outputs, X within rounding (RED / atomic order), F_pre and the pinned flag included."""
-    inst = I.make_mixed(n=40, m=170, kmin=1, kmax=8, seed=171, batch=80, with_fixed=True)
     base = I.make_mixed(n=40, m=170, kmin=1, kmax=8, seed=171, batch=80, with_fixed=True)
     base.meta["admissible"] = [R.admissible_taus(int(t), int(k), int(p)) or [0]
                                for t, k, p in zip(base.ctype, base.lengths(), base.param)]
     inst, hidden = I.plant_solution(base, seed=5)
     npdt = np.float32 if dtype == 32 else np.float64
     x0 = I.make_x0(inst, seed=172, batch=80).astype(npdt)
-    x0[:, 3] = np.where(hidden, -0.4, 0.4)                             # a candidate next to the hidden solution
+    x0[:, 3] = np.where(hidden, -0.9, 0.9)                             # candidates at / next to the hidden solution
+    x0[:, 70] = np.where(hidden, -0.6, 0.6)
+    x0[:2, 70] *= -1
     x0[inst.fixed != 0] = inst.fixed[inst.fixed != 0].astype(npdt)[:, None]
     x0[:, 80:] = 0
     outs = {}
@@ -902,7 +903,7 @@ def test_step_paths_agree(dtype):
         ctx.close()
     ref = outs[Bd.STEP_LAUNCHES]
     Xo, _, sato, solo, firsto = O.step(inst, x0.astype(np.float64), 0.1, 40, 80, want_F=False)
-    assert solo[3] == 1
+    assert solo[3] == 1 and firsto[3] == 1                             # the planted candidate: solved by the first step
     for path, o in outs.items():
         assert np.array_equal(o[1], ref[1]) and np.array_equal(o[2], ref[2]) and np.array_equal(o[3], ref[3]), path
         assert np.abs(o[0] - ref[0]).max() <= (1e-4 if dtype == 32 else 1e-11), path
