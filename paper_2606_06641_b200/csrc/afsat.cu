@@ -79,7 +79,7 @@ struct afsat_ctx {
     // device tables shared by the groups
     SigDev *d_sigs = nullptr;
     void *d_rows = nullptr;
-    float *d_rows2 = nullptr;                      // staged tables of the packed fp32 kernel
+    float *d_rows2 = nullptr, *d_rows2g = nullptr; // staged tables of the packed fp32 kernel (unit rows | grouped generic rows)
     void *d_rowsg = nullptr;                       // staged tables of the grouped lane-split kernels
     int8_t *d_fixed = nullptr;                     // [n_groups][n]
     int32_t *d_sat_const = nullptr;                // [n_groups]
@@ -224,7 +224,7 @@ int launch_eval(afsat_ctx *ctx, const GroupPlan &gp, const T *x, T *G, int64_t g
     EvalParams<T> p;
     p.x = x; p.G = G; p.g_ld = g_ld; p.g_b0 = g_b0; p.Fpart = Fpart;
     p.lits = gp.d_lits; p.sigs = ctx->d_sigs; p.rows = (const T *)ctx->d_rows; p.rows2 = ctx->d_rows2;
-    p.rowsg = (const T *)ctx->d_rowsg;
+    p.rowsg = (const T *)ctx->d_rowsg; p.rows2g = ctx->d_rows2g;
     p.skip = ctx->cur_skip;
     p.B = ctx->B; p.ldb = ctx->ldb; p.b_begin = b_begin; p.b_end = std::min<int64_t>(b_begin + width, ctx->ldb);
     const bool grad = G != nullptr;
@@ -602,17 +602,17 @@ int step_host_pipelined(afsat_ctx *ctx, T *h_x, double eta, T *h_F_pre)
     const int64_t ldb = ctx->ldb;
     const bool tiled = ctx->tile_w < (ctx->groups.size() > 1 ? ctx->group_w : ldb);
     T *x = (T *)ctx->dh_x;
+    // a chunk = a run of candidate tiles of one group, wide enough that a row of the strided host <-> device copy is a
+    // few KB (512-byte rows -- one cfg4 tile -- cost the copy engines more than the pipelining gains)
     struct Chunk { const GroupPlan *gp; int64_t b0, w; };
     std::vector<Chunk> chunks;
-    if (tiled) {
-        for_tiles(ctx, [&](const GroupPlan &gp, int64_t b0, int64_t w) { chunks.push_back({&gp, b0, w}); return 0; });
-    } else {
-        for (size_t g = 0; g < ctx->groups.size(); ++g) {
-            const GroupPlan &gp = ctx->groups[g];
-            const int64_t end = (g + 1 == ctx->groups.size()) ? ldb : gp.b1;
-            const int64_t cw = std::max<int64_t>(128, ((end - gp.b0 + 3) / 4 + 127) / 128 * 128);
-            for (int64_t b0 = gp.b0; b0 < end && b0 < B; b0 += cw) chunks.push_back({&gp, b0, std::min(cw, end - b0)});
-        }
+    for (size_t g = 0; g < ctx->groups.size(); ++g) {
+        const GroupPlan &gp = ctx->groups[g];
+        const int64_t end = (g + 1 == ctx->groups.size()) ? ldb : gp.b1;
+        int64_t cw = std::max<int64_t>(128, ((end - gp.b0 + 7) / 8 + 127) / 128 * 128);
+        if (!tiled) cw = std::max<int64_t>(128, ((end - gp.b0 + 3) / 4 + 127) / 128 * 128);
+        else cw = (cw + ctx->tile_w - 1) / ctx->tile_w * ctx->tile_w;                 // whole tiles
+        for (int64_t b0 = gp.b0; b0 < end && b0 < B; b0 += cw) chunks.push_back({&gp, b0, std::min(cw, end - b0)});
     }
     while (ctx->chunk_in.size() < chunks.size()) {
         cudaEvent_t a, b;
@@ -636,10 +636,13 @@ int step_host_pipelined(afsat_ctx *ctx, T *h_x, double eta, T *h_F_pre)
     for (size_t c = 0; c < chunks.size(); ++c) {
         const Chunk &ch = chunks[c];
         CU(cudaStreamWaitEvent(st, ctx->chunk_in[c], 0));
-        int rc = launch_eval<T>(ctx, *ch.gp, x, G, tiled ? ctx->tile_w : ldb, tiled ? ch.b0 : 0, h_F_pre ? (T *)ctx->d_Fpart : nullptr,
-                                ch.b0, ch.w, st);
-        if (!rc) rc = launch_update<T>(ctx, *ch.gp, x, G, tiled ? ctx->tile_w : ldb, tiled ? ch.b0 : 0, ctx->dh_sol, eta, ch.b0, ch.w, st);
-        if (rc) return rc;
+        for (int64_t b0 = ch.b0; b0 < ch.b0 + ch.w; b0 += tiled ? ctx->tile_w : ch.w) {
+            const int64_t w = tiled ? std::min<int64_t>(ctx->tile_w, ch.b0 + ch.w - b0) : ch.w;
+            int rc = launch_eval<T>(ctx, *ch.gp, x, G, tiled ? ctx->tile_w : ldb, tiled ? b0 : 0, h_F_pre ? (T *)ctx->d_Fpart : nullptr,
+                                    b0, w, st);
+            if (!rc) rc = launch_update<T>(ctx, *ch.gp, x, G, tiled ? ctx->tile_w : ldb, tiled ? b0 : 0, ctx->dh_sol, eta, b0, w, st);
+            if (rc) return rc;
+        }
         CU(cudaEventRecord(ctx->chunk_done[c], st));
         CU(cudaStreamWaitEvent(ctx->out_stream, ctx->chunk_done[c], 0));
         CU(cudaMemcpy2DAsync(h_x + ch.b0, ldb * sizeof(T), x + ch.b0, ldb * sizeof(T), ch.w * sizeof(T), ctx->n,
@@ -824,7 +827,7 @@ int afsat_create_ex(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64
     const int n_sigs = (int)sig_id.size();
     std::vector<SigDev> sigs(n_sigs);
     std::vector<double> rows;
-    std::vector<float> rows2;
+    std::vector<float> rows2, rows2g;
     std::vector<double> rowsg;
     std::vector<int> sig_k(n_sigs);
     std::vector<int64_t> sig_cost(n_sigs), sig_flop(n_sigs);
@@ -845,18 +848,38 @@ int afsat_create_ex(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64
             if (2 * nsat <= kk + 1) { d.scan_lo = hs.satmask_lo; d.scan_hi = hs.satmask_hi; d.scan_is_sat = 1; }
             else { d.scan_lo = ~hs.satmask_lo & full_lo; d.scan_hi = ~hs.satmask_hi & full_hi; d.scan_is_sat = 0; }
             d.k = kk;
+            // predicates that need no counting (k_check_bits): functions of any / all / parity of the literals
+            const uint64_t slo = hs.satmask_lo, shi = hs.satmask_hi;
+            auto bit_of = [&](int tau) { return (int)((tau < 64 ? slo >> tau : shi >> (tau - 64)) & 1ull); };
+            bool mid_all = true, mid_none = true, odd = true, even = true;
+            for (int tau = 0; tau <= kk; ++tau) {
+                if (tau > 0 && tau < kk) { mid_all = mid_all && bit_of(tau); mid_none = mid_none && !bit_of(tau); }
+                odd = odd && bit_of(tau) == (tau & 1); even = even && bit_of(tau) == !(tau & 1);
+            }
+            const int s0 = bit_of(0), sk = bit_of(kk);
+            d.chk_kind = CHK_GENERAL;
+            if (kk >= 2 && odd) d.chk_kind = CHK_ODD;
+            else if (kk >= 2 && even) d.chk_kind = CHK_EVEN;
+            else if (mid_all && !s0 && sk) d.chk_kind = CHK_OR;
+            else if (mid_all && s0 && !sk) d.chk_kind = CHK_NAND;
+            else if (mid_all && !s0 && !sk) d.chk_kind = CHK_NAE;
+            else if (mid_none && s0 && !sk) d.chk_kind = CHK_NONE;
+            else if (mid_none && !s0 && sk) d.chk_kind = CHK_ALL;
+            else if (mid_none && s0 && sk && kk >= 2) d.chk_kind = CHK_EQ;
         }
         rows.insert(rows.end(), hs.rows, hs.rows + 8 * (hs.n_real + hs.n_cplx));
         if (dtype == 32 && kk <= AFSAT_A_KMAX) {                       // staged table of the packed kernel (k <= 8)
-            float r32[8 * AFSAT_MAX_POINTS], packed[AFSAT_PACK_MAX_ROWS * ROW2];
+            float r32[8 * AFSAT_MAX_POINTS], packed[AFSAT_PACK_MAX_ROWS * ROW2], packedg[AFSAT_PACK_MAX_ROWS * ROW2G];
             for (int i = 0; i < 8 * (hs.n_real + hs.n_cplx); ++i) r32[i] = (float)hs.rows[i];
             int uv = 0, nu = 0, ng = 0;
-            const int nrows2 = pack_rows_f2(r32, hs.n_real, hs.n_cplx, kk, packed, &uv, &nu, &ng);
+            const int nrows2 = pack_rows_f2(r32, hs.rows, hs.n_real, hs.n_cplx, kk, packed, packedg, &uv, &nu, &ng);
             d.row2_off = (int32_t)(rows2.size() / ROW2);
+            d.row2g_off = (int32_t)(rows2g.size() / ROW2G);
             d.uv = (int8_t)uv; d.n_unit = (int8_t)nu; d.n_gen = (int8_t)ng;
             rows2.insert(rows2.end(), packed, packed + (size_t)nrows2 * ROW2);
+            rows2g.insert(rows2g.end(), packedg, packedg + (size_t)ng * ROW2G);
         }
-        if (class_of(kk, dtype) == CLS_LONG) {                         // staged table of the grouped lane-split kernels
+        if (class_of(kk, dtype) == CLS_LONG || (dtype == 32 && class_of(kk, dtype) == CLS_B)) {   // grouped lane-split kernels
             double packed[AFSAT_MAX_POINTS * ROWG];
             d.pad = (int8_t)pack_rows_grp(hs.rows, hs.n_real + hs.n_cplx, kk, packed);
             d.row2_off = (int32_t)(rowsg.size() / ROWG);
@@ -1004,6 +1027,7 @@ int afsat_create_ex(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64
         CREATE_FAIL(upload(ctx, &p, r32));
         ctx->d_rows = p;
         CREATE_FAIL(upload(ctx, &ctx->d_rows2, rows2));
+        CREATE_FAIL(upload(ctx, &ctx->d_rows2g, rows2g));
         std::vector<float> g32(rowsg.begin(), rowsg.end());
         float *pg = nullptr;
         CREATE_FAIL(upload(ctx, &pg, g32));
@@ -1059,10 +1083,10 @@ int afsat_create_ex(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64
             CREATE_FAIL(AFSAT_E_INVALID);
         }
         if (path == AFSAT_STEP_AUTO) {
-            const int64_t tiles = (span + tile_w - 1) / tile_w * G;
-            path = (fits && est_us < 8.0 && batch <= 8 * sm_count) ? AFSAT_STEP_PERSISTENT
-                 : (est_us < 60.0 && tiles <= 8)                      ? AFSAT_STEP_GRAPH
-                                                                      : AFSAT_STEP_LAUNCHES;
+            // (a replayed CUDA graph of one iteration, AFSAT_STEP_GRAPH, measured no faster than plain launches on cfg0 --
+            // 21.0 vs 20.6 us per step: the time is kernel-to-kernel dependency latency, not host launch cost -- so it is
+            // never chosen automatically)
+            path = (fits && est_us < 8.0 && batch <= 8 * sm_count) ? AFSAT_STEP_PERSISTENT : AFSAT_STEP_LAUNCHES;
         }
         ctx->step_path = path;
         if (fits) {
@@ -1092,7 +1116,7 @@ void afsat_destroy(afsat_ctx *ctx)
     prof_drain(ctx, false);
     if (ctx->graph.exec) cudaGraphExecDestroy(ctx->graph.exec);
     for (GroupPlan &gp : ctx->groups) { cudaFree(gp.d_lits); cudaFree(gp.d_items); cudaFree(gp.d_cons); }
-    cudaFree(ctx->d_bits); cudaFree(ctx->d_sigs); cudaFree(ctx->d_rows); cudaFree(ctx->d_rows2); cudaFree(ctx->d_rowsg);
+    cudaFree(ctx->d_bits); cudaFree(ctx->d_sigs); cudaFree(ctx->d_rows); cudaFree(ctx->d_rows2); cudaFree(ctx->d_rows2g); cudaFree(ctx->d_rowsg);
     cudaFree(ctx->d_fixed); cudaFree(ctx->d_sat_const); cudaFree(ctx->d_G); cudaFree(ctx->d_Fpart);
     cudaFree(ctx->d_satacc); cudaFree(ctx->d_any);
     cudaFree(ctx->ls_G); cudaFree(ctx->ls_xt); cudaFree(ctx->ls_F0); cudaFree(ctx->ls_F1); cudaFree(ctx->ls_Dpart);

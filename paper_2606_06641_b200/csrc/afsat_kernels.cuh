@@ -41,12 +41,14 @@ struct SigDev {                 // 40 bytes, one per signature (type, k, param)
     int32_t row_off;            // first row in the weight table (8 scalars per row)
     int16_t n_real, n_cplx;     // real rows first, then complex rows
     uint64_t scan_lo, scan_hi;  // bit tau set: tau is in the SCANNED set of the discrete check
-    int32_t scan_is_sat;        // 1: scanned set = satisfied counts; 0: = violated counts (smaller)
+    int16_t scan_is_sat;        // 1: scanned set = satisfied counts; 0: = violated counts (smaller)
+    int16_t chk_kind;           // k_check_bits: the predicate as a function of any / all / parity of the literals, or 0
     int32_t k;
     int32_t row2_off;           // first row of the STAGED table of the kernel that runs this length: rows2 (fp32, k <= 8,
                                 // ROW2 scalars per row, pack_rows_f2) or rowsg (grouped lane-split kernels, pack_rows_grp)
     int8_t uv, n_unit, n_gen;   // rows2: unit variant, number of trivial-twiddle rows, number of generic complex rows
     int8_t pad;                 // rowsg: the literal value whose factor is exactly 1 (0 or 1)
+    int32_t row2g_off, pad2;    // rows2g: first grouped generic row
 };
 
 struct Item {                   // one CTA-sized chunk of constraints of a single signature
@@ -67,6 +69,7 @@ struct EvalParams {
     const SigDev *sigs;
     const T *rows;              // weight table
     const float *rows2;         // staged table of the packed fp32 kernel (fp32 contexts), else null
+    const float *rows2g;        // packed fp32 kernel: the generic complex rows staged for literal groups (ROW2G scalars per row)
     const T *rowsg;             // staged table of the grouped lane-split kernels (afsat_split.cuh), ROWG scalars per row
     const Item *items;          // items of this launch
     int32_t frow_base;          // row of Fpart for (items[0], group 0)
@@ -248,8 +251,13 @@ constexpr int ROW2 = 12;
 // [w = (1+i)/sqrt 2, then its partner (-1+i)/sqrt 2 with CONJUGATED weights, iff k = 7 mod 8] -- a missing one
 // (its weight was exactly zero) staged with weight 0, the halvings folded into their weights (2^-k, 2^-(k-1):
 // exact rescales); then the generic complex rows.  Other tables: rows as they are, uv = 0.
+// The generic complex rows are ALSO staged for literal groups (grp_rows_f2; outg gets ROW2G scalars per generic row, rd are
+// the same rows in double): c_j = a^(M-j) b^j for the two group sizes; for the standard tables un-halved (a = 1, b = w^l,
+// the 2^-k folded into the weight: exact rescales).
 // Returns the number of staged rows; out gets ROW2 scalars per row.
-inline int pack_rows_f2(const float *r0, int n_real, int n_cplx, int k, float *out, int *uv_out, int *n_unit_out, int *n_gen_out)
+constexpr int ROW2G_G1_H = 10, ROW2G_W_H = 20, ROW2G_H = 22;    // = ROW2G_G1, ROW2G_W, ROW2G below
+inline int pack_rows_f2(const float *r0, const double *rd, int n_real, int n_cplx, int k, float *out, float *outg, int *uv_out,
+                        int *n_unit_out, int *n_gen_out)
 {
     const int nr = n_real + n_cplx;
     int src[AFSAT_PACK_MAX_ROWS], n = 0, uv = 0, n_unit = n_real, n_gen = n_cplx, q_conj = -1;
@@ -292,60 +300,31 @@ inline int pack_rows_f2(const float *r0, int n_real, int n_cplx, int k, float *o
             o[6] = r[4] * fw; o[7] = -cj * r[5] * fw; o[8] = r[6] * fwb; o[9] = -cj * r[7] * fwb;
         }
     }
+    {
+        const int M[2] = {(k + 1) / 2, k / 2}, off[2] = {0, ROW2G_G1_H};
+        double scw = 1.0;
+        if (std_tab) for (int i = 0; i < k; ++i) scw *= 0.5;
+        const double sc = std_tab ? 2.0 : 1.0;
+        for (int q = n_unit; q < n; ++q) {
+            float *o = outg + (size_t)(q - n_unit) * ROW2G_H;
+            for (int j = 0; j < ROW2G_H; ++j) o[j] = 0.f;
+            const double *r = rd + 8 * src[q];
+            const double ar = sc * r[0], ai = sc * r[1], br = sc * r[2], bi = sc * r[3];
+            for (int gq = 0; gq < 2; ++gq)
+                for (int j = 0; j <= M[gq]; ++j) {
+                    double cr = 1.0, ci = 0.0;
+                    for (int t = 0; t < M[gq]; ++t) {
+                        const double fr = t < j ? br : ar, fi = t < j ? bi : ai;
+                        const double nr2 = cr * fr - ci * fi, ni2 = cr * fi + ci * fr;
+                        cr = nr2; ci = ni2;
+                    }
+                    o[off[gq] + 2 * j] = (float)cr; o[off[gq] + 2 * j + 1] = (float)ci;
+                }
+            o[ROW2G_W_H] = (float)(r[4] * scw); o[ROW2G_W_H + 1] = (float)(r[5] * scw);
+        }
+    }
     *uv_out = uv; *n_unit_out = n_unit; *n_gen_out = n_gen;
     return n;
-}
-
-// One generic complex DFT point (table row r) for NP candidate pairs: prefix walk, contraction, suffix walk with
-// the leave-one-out accumulation.  The NP chains are independent.
-template <int K, int NP, bool GRAD>
-__device__ __forceinline__ void cplx_points_f2(const f32x2 (&y)[K][NP], const f32x2 *__restrict__ r, f32x2 (&fe)[NP],
-                                               f32x2 (&g)[K][NP])
-{
-    f32x2 pr[K][NP], pi[K][NP], fr[K][NP], fi[K][NP], nfi[K][NP], rr[NP], ri[NP];
-    // coefficients are the same for both candidates: read ONE float and let FFMA2 broadcast it
-    // (R.F32 operand) -- a true register pair would cost a third 64-bit register-file read
-    const f32x2 ar = bc(r, 0), ai = bc(r, 1), br = bc(r, 3), bi = bc(r, 4);
-#pragma unroll
-    for (int i = 0; i < K; ++i)
-#pragma unroll
-        for (int q = 0; q < NP; ++q) {
-            fr[i][q] = fma2(br, y[i][q], ar); fi[i][q] = fma2(bi, y[i][q], ai);
-            nfi[i][q] = fi[i][q] ^ 0x8000000080000000ull;             // -Im f on the ALU pipe (2 LOP3), not the FMA pipe
-        }
-#pragma unroll
-    for (int q = 0; q < NP; ++q) { rr[q] = fr[0][q]; ri[q] = fi[0][q]; }
-#pragma unroll
-    for (int i = 1; i < K; ++i)
-#pragma unroll
-        for (int q = 0; q < NP; ++q) {
-            pr[i][q] = rr[q]; pi[i][q] = ri[q];
-            const f32x2 nr = fma2(rr[q], fr[i][q], mul2(ri[q], nfi[i][q]));   // Re: rr fr - ri fi
-            const f32x2 ni = fma2(rr[q], fi[i][q], mul2(ri[q], fr[i][q]));    // Im: rr fi + ri fr
-            rr[q] = nr; ri[q] = ni;
-        }
-#pragma unroll
-    for (int q = 0; q < NP; ++q) {
-        fe[q] = fma2(bc(r, 6), rr[q], fe[q]);                         // + wr Re P
-        fe[q] = fma2(bc(r, 7), ri[q], fe[q]);                         // - wi Im P
-    }
-    if (GRAD) {
-        f32x2 sr[NP], nsi[NP];                                        // suffix (Re s, -Im s) seeded with w b
-#pragma unroll
-        for (int q = 0; q < NP; ++q) { sr[q] = r[8]; nsi[q] = r[9]; }
-#pragma unroll
-        for (int i = K - 1; i >= 1; --i)
-#pragma unroll
-            for (int q = 0; q < NP; ++q) {
-                g[i][q] = fma2(pr[i][q], sr[q], g[i][q]);             // Re(pre * suf) = pr sr - pi si
-                g[i][q] = fma2(pi[i][q], nsi[q], g[i][q]);
-                const f32x2 t_r = fma2(nsi[q], fi[i][q], mul2(sr[q], fr[i][q]));    // Re: sr fr - si fi
-                const f32x2 t_n = fma2(nsi[q], fr[i][q], mul2(sr[q], nfi[i][q]));   // -Im: -(sr fi + si fr)
-                sr[q] = t_r; nsi[q] = t_n;
-            }
-#pragma unroll
-        for (int q = 0; q < NP; ++q) g[0][q] = add2(g[0][q], sr[q]);  // prefix_0 = 1
-    }
 }
 
 constexpr f32x2 NEGP = 0x8000000080000000ull;
@@ -473,16 +452,137 @@ __device__ __forceinline__ void oct_row_f2(const f32x2 (&y)[K][NP], const f32x2 
     }
 }
 
-// One generic complex DFT point for all NP pairs of a lane.  With two pairs and k >= AFSAT_F2_SEQ_MINK the
-// pairs are walked one after the other (each keeps 5 k register pairs of factors and prefixes alive).
+// ---- literal GROUPS at the generic complex DFT points (packed form) ---------------------------------------------------
+// The product of M factors is the polynomial  prod_{u<M} (a + b y_u) = sum_{j<=M} a^(M-j) b^j e_j(y_group)  in the group's
+// elementary symmetric polynomials, which do not depend on the DFT point: they are formed once per constraint, and at
+// every point a group costs 2 M FFMA2 for its complex factor (coefficients through the broadcast operand) instead of M
+// factors and M - 1 complex multiplies.  The partial gradients come out of M accumulators per group,
+//     A_j += Re( w a^(M-j) b^j x (product of the OTHER groups' factors) ),   dFE/dy_u = sum_j A_j e_{j-1}(group without y_u),
+// expanded once per constraint.  The generating polynomial is still evaluated at every DFT point and contracted with the
+// same weights; the groups only change the order in which its factors are multiplied.
+constexpr f32x2 SGNP = 0x8000000080000000ull;
+__device__ __forceinline__ f32x2 bcf(float c) { return pk(c, c); }
+
+// e[j-1] = e_j(y[0..M)), M <= 4
+template <int M, int NP>
+__device__ __forceinline__ void esp_f2(const f32x2 (*y)[NP], f32x2 (&e)[M][NP])
+{
+    static_assert(M >= 1 && M <= 4, "group size");
+#pragma unroll
+    for (int q = 0; q < NP; ++q) {
+        if (M == 1) { e[0][q] = y[0][q]; }
+        else if (M == 2) { e[0][q] = add2(y[0][q], y[1][q]); e[M > 1 ? 1 : 0][q] = mul2(y[0][q], y[M > 1 ? 1 : 0][q]); }
+        else if (M == 3) {
+            const f32x2 s01 = add2(y[0][q], y[1][q]), p01 = mul2(y[0][q], y[1][q]), y2 = y[M > 2 ? 2 : 0][q];
+            e[0][q] = add2(s01, y2); e[M > 1 ? 1 : 0][q] = fma2(s01, y2, p01); e[M > 2 ? 2 : 0][q] = mul2(p01, y2);
+        } else {
+            const f32x2 s01 = add2(y[0][q], y[1][q]), p01 = mul2(y[0][q], y[1][q]);
+            const f32x2 s23 = add2(y[M > 2 ? 2 : 0][q], y[M > 3 ? 3 : 0][q]), p23 = mul2(y[M > 2 ? 2 : 0][q], y[M > 3 ? 3 : 0][q]);
+            e[0][q] = add2(s01, s23);
+            e[M > 1 ? 1 : 0][q] = fma2(s01, s23, add2(p01, p23));
+            e[M > 2 ? 2 : 0][q] = fma2(p01, s23, mul2(p23, s01));
+            e[M > 3 ? 3 : 0][q] = mul2(p01, p23);
+        }
+    }
+}
+
+// g[u] += sum_j A[j] e_j(y without y_u), j = 0 .. M-1
+template <int M, int NP>
+__device__ __forceinline__ void loo_f2(const f32x2 (*y)[NP], const f32x2 (&A)[M][NP], f32x2 (*g)[NP])
+{
+#pragma unroll
+    for (int q = 0; q < NP; ++q) {
+        if (M == 1) { g[0][q] = add2(g[0][q], A[0][q]); }
+        else if (M == 2) {
+            g[0][q] = add2(g[0][q], fma2(A[M > 1 ? 1 : 0][q], y[M > 1 ? 1 : 0][q], A[0][q]));
+            g[M > 1 ? 1 : 0][q] = add2(g[M > 1 ? 1 : 0][q], fma2(A[M > 1 ? 1 : 0][q], y[0][q], A[0][q]));
+        } else if (M == 3) {
+            const f32x2 y0 = y[0][q], y1 = y[M > 1 ? 1 : 0][q], y2 = y[M > 2 ? 2 : 0][q];
+            const f32x2 a0 = A[0][q], a1 = A[M > 1 ? 1 : 0][q], a2 = A[M > 2 ? 2 : 0][q];
+            g[0][q] = add2(g[0][q], fma2(a2, mul2(y1, y2), fma2(a1, add2(y1, y2), a0)));
+            g[M > 1 ? 1 : 0][q] = add2(g[M > 1 ? 1 : 0][q], fma2(a2, mul2(y0, y2), fma2(a1, add2(y0, y2), a0)));
+            g[M > 2 ? 2 : 0][q] = add2(g[M > 2 ? 2 : 0][q], fma2(a2, mul2(y0, y1), fma2(a1, add2(y0, y1), a0)));
+        } else {
+            const f32x2 y0 = y[0][q], y1 = y[M > 1 ? 1 : 0][q], y2 = y[M > 2 ? 2 : 0][q], y3 = y[M > 3 ? 3 : 0][q];
+            const f32x2 a0 = A[0][q], a1 = A[M > 1 ? 1 : 0][q], a2 = A[M > 2 ? 2 : 0][q], a3 = A[M > 3 ? 3 : 0][q];
+            const f32x2 s01 = add2(y0, y1), p01 = mul2(y0, y1), s23 = add2(y2, y3), p23 = mul2(y2, y3);
+            // others of y0: {y1, y2, y3}: e1 = y1 + s23, e2 = y1 s23 + p23, e3 = y1 p23; and so on
+            g[0][q] = add2(g[0][q], fma2(a3, mul2(y1, p23), fma2(a2, fma2(y1, s23, p23), fma2(a1, add2(y1, s23), a0))));
+            g[M > 1 ? 1 : 0][q] = add2(g[M > 1 ? 1 : 0][q], fma2(a3, mul2(y0, p23), fma2(a2, fma2(y0, s23, p23), fma2(a1, add2(y0, s23), a0))));
+            g[M > 2 ? 2 : 0][q] = add2(g[M > 2 ? 2 : 0][q], fma2(a3, mul2(y3, p01), fma2(a2, fma2(y3, s01, p01), fma2(a1, add2(y3, s01), a0))));
+            g[M > 3 ? 3 : 0][q] = add2(g[M > 3 ? 3 : 0][q], fma2(a3, mul2(y2, p01), fma2(a2, fma2(y2, s01, p01), fma2(a1, add2(y2, s01), a0))));
+        }
+    }
+}
+
+// Staged row of a generic complex point for TWO groups (sizes M0 = ceil(K/2), M1 = floor(K/2) <= 4): {Re, Im of c0_0 ..
+// c0_M0 | Re, Im of c1_0 .. c1_M1 (from scalar ROW2G_G1) | Re w, Im w (at ROW2G_W)}, c_j = a^(M-j) b^j of the group.
+constexpr int ROW2G_G1 = ROW2G_G1_H, ROW2G_W = ROW2G_W_H, ROW2G = ROW2G_H;
+
+// all generic complex rows of a signature for the K literals of a lane (K >= 2), two groups
+template <int K, int NP, bool GRAD>
+__device__ __forceinline__ void grp_rows_f2_joint(const f32x2 (&y)[K][NP], const float *__restrict__ rg, int n_rows, f32x2 (&fe)[NP],
+                                            f32x2 (&g)[K][NP])
+{
+    constexpr int M0 = (K + 1) / 2, M1 = K / 2;
+    f32x2 e0[M0][NP], e1[M1][NP], A0[M0][NP], A1[M1][NP];
+    esp_f2<M0, NP>(&y[0], e0);
+    esp_f2<M1, NP>(&y[M0], e1);
+#pragma unroll
+    for (int q = 0; q < NP; ++q) {
+#pragma unroll
+        for (int j = 0; j < M0; ++j) A0[j][q] = 0ull;
+#pragma unroll
+        for (int j = 0; j < M1; ++j) A1[j][q] = 0ull;
+    }
+    for (int p = 0; p < n_rows; ++p, rg += ROW2G) {
+        const float wr = rg[ROW2G_W], wi = rg[ROW2G_W + 1];
+        const f32x2 bwr = bcf(wr), bwi = bcf(wi), bnwi = bcf(-wi);
+#pragma unroll
+        for (int q = 0; q < NP; ++q) {
+            f32x2 q0r = bcf(rg[0]), q0i = bcf(rg[1]), q1r = bcf(rg[ROW2G_G1]), q1i = bcf(rg[ROW2G_G1 + 1]);
+#pragma unroll
+            for (int j = 0; j < M0; ++j) { q0r = fma2(bcf(rg[2 + 2 * j]), e0[j][q], q0r); q0i = fma2(bcf(rg[3 + 2 * j]), e0[j][q], q0i); }
+#pragma unroll
+            for (int j = 0; j < M1; ++j) {
+                q1r = fma2(bcf(rg[ROW2G_G1 + 2 + 2 * j]), e1[j][q], q1r); q1i = fma2(bcf(rg[ROW2G_G1 + 3 + 2 * j]), e1[j][q], q1i);
+            }
+            const f32x2 Pr = fma2(q0r, q1r, mul2(q0i, q1i ^ SGNP)), Pi = fma2(q0r, q1i, mul2(q0i, q1r));   // P = q0 q1
+            fe[q] = fma2(bwr, Pr, fe[q]);
+            fe[q] = fma2(bnwi, Pi, fe[q]);                            // Re(w P)
+            if (GRAD) {
+                // T0 = w q1 (everything but group 0), T1 = w q0;  A_j += Re(c_j T) = Re c_j Re T - Im c_j Im T
+                const f32x2 t0r = fma2(bwr, q1r, mul2(bnwi, q1i)), nt0i = fma2(bwr, q1i, mul2(bwi, q1r)) ^ SGNP;
+                const f32x2 t1r = fma2(bwr, q0r, mul2(bnwi, q0i)), nt1i = fma2(bwr, q0i, mul2(bwi, q0r)) ^ SGNP;
+#pragma unroll
+                for (int j = 0; j < M0; ++j) {
+                    A0[j][q] = fma2(bcf(rg[2 + 2 * j]), t0r, A0[j][q]); A0[j][q] = fma2(bcf(rg[3 + 2 * j]), nt0i, A0[j][q]);
+                }
+#pragma unroll
+                for (int j = 0; j < M1; ++j) {
+                    A1[j][q] = fma2(bcf(rg[ROW2G_G1 + 2 + 2 * j]), t1r, A1[j][q]);
+                    A1[j][q] = fma2(bcf(rg[ROW2G_G1 + 3 + 2 * j]), nt1i, A1[j][q]);
+                }
+            }
+        }
+    }
+    if (GRAD) {
+        loo_f2<M0, NP>(&y[0], A0, &g[0]);
+        loo_f2<M1, NP>(&y[M0], A1, &g[M0]);
+    }
+}
+
+// With two pairs per lane and K >= AFSAT_F2_SEQ_MINK the pairs are walked one after the other (each keeps ~4 K register
+// pairs of symmetric polynomials, accumulators and literal values alive).
 #ifndef AFSAT_F2_SEQ_MINK
 #define AFSAT_F2_SEQ_MINK 5
 #endif
 template <int K, int NP, bool GRAD>
-__device__ __forceinline__ void cplx_row_f2(const f32x2 (&y)[K][NP], const f32x2 *__restrict__ r, f32x2 (&fe)[NP], f32x2 (&g)[K][NP])
+__device__ __forceinline__ void grp_rows_f2(const f32x2 (&y)[K][NP], const float *__restrict__ rg, int n_rows, f32x2 (&fe)[NP],
+                                            f32x2 (&g)[K][NP])
 {
     if constexpr (NP == 1 || K < AFSAT_F2_SEQ_MINK) {
-        cplx_points_f2<K, NP, GRAD>(y, r, fe, g);
+        grp_rows_f2_joint<K, NP, GRAD>(y, rg, n_rows, fe, g);
     } else {
 #pragma unroll
         for (int q = 0; q < NP; ++q) {
@@ -490,7 +590,7 @@ __device__ __forceinline__ void cplx_row_f2(const f32x2 (&y)[K][NP], const f32x2
 #pragma unroll
             for (int i = 0; i < K; ++i) { y1[i][0] = y[i][q]; g1[i][0] = g[i][q]; }
             fe1[0] = fe[q];
-            cplx_points_f2<K, 1, GRAD>(y1, r, fe1, g1);
+            grp_rows_f2_joint<K, 1, GRAD>(y1, rg, n_rows, fe1, g1);
 #pragma unroll
             for (int i = 0; i < K; ++i) g[i][q] = g1[i][0];
             fe[q] = fe1[0];
@@ -502,8 +602,8 @@ __device__ __forceinline__ void cplx_row_f2(const f32x2 (&y)[K][NP], const f32x2
 // every row; 1 / 2 = standard table whose first rows are the trivial twiddles [w = 1 (UV 1 only)]
 // [w = -1 iff K odd] [w = i iff K = 3 mod 4] (n_real = their number), followed by n_cplx generic complex rows.
 template <int K, int NP, bool GRAD, int UV>
-__device__ __forceinline__ void eval_points_f2(const f32x2 (&y)[K][NP], const f32x2 *__restrict__ tab, int n_real,
-                                               int n_cplx, f32x2 (&fe)[NP], f32x2 (&g)[K][NP])
+__device__ __forceinline__ void eval_points_f2(const f32x2 (&y)[K][NP], const f32x2 *__restrict__ tab, const float *__restrict__ tabg,
+                                               int n_real, int n_cplx, f32x2 (&fe)[NP], f32x2 (&g)[K][NP])
 {
     if (UV != 0) {
         constexpr bool HP = UV == 1, HM = (K & 1) != 0, HI = (K & 3) == 3;
@@ -515,8 +615,7 @@ __device__ __forceinline__ void eval_points_f2(const f32x2 (&y)[K][NP], const f3
             oct_row_f2<K, NP, GRAD>(y, rO, 0.70710678118654752f, fe, g);             // = 2 Re b of the row, bit for bit
             oct_row_f2<K, NP, GRAD>(y, rO + ROW2, -0.70710678118654752f, fe, g);
         }
-        const f32x2 *r = rO + (HO ? 2 * ROW2 : 0);
-        for (int p = 0; p < n_cplx; ++p, r += ROW2) cplx_row_f2<K, NP, GRAD>(y, r, fe, g);
+        if constexpr (K >= 2) grp_rows_f2<K, NP, GRAD>(y, tabg, n_cplx, fe, g);   // the generic complex points, grouped
         return;
     }
     const f32x2 *r = tab;
@@ -546,7 +645,7 @@ __device__ __forceinline__ void eval_points_f2(const f32x2 (&y)[K][NP], const f3
             for (int q = 0; q < NP; ++q) g[0][q] = add2(g[0][q], suf[q]);     // prefix_0 = 1
         }
     }
-    for (int p = 0; p < n_cplx; ++p, r += ROW2) cplx_row_f2<K, NP, GRAD>(y, r, fe, g);   // one of each conjugate pair
+    if constexpr (K >= 2) grp_rows_f2<K, NP, GRAD>(y, tabg, n_cplx, fe, g);       // one of each conjugate pair, grouped
 }
 
 // sign flip by the literal's polarity bit (bit 31 of the packed literal): one LOP3 per value
@@ -698,8 +797,8 @@ template <> struct PairIO<2> {
 
 template <int K, int NP, bool GRAD, bool PF, int UV>
 __device__ __forceinline__ void run_item_f2(const EvalParams<float> &p, const int32_t *__restrict__ s_lits,
-                                            const f32x2 *__restrict__ s_tab2, int n_real, int n_cplx, int nc, int wk,
-                                            int64_t b, f32x2 (&fe)[NP])
+                                            const f32x2 *__restrict__ s_tab2, const float *__restrict__ s_tabg, int n_real,
+                                            int n_cplx, int nc, int wk, int64_t b, f32x2 (&fe)[NP])
 {
     const char *xb = reinterpret_cast<const char *>(p.x + b);
     char *gb = reinterpret_cast<char *>(p.G + (b - p.g_b0));
@@ -727,7 +826,7 @@ __device__ __forceinline__ void run_item_f2(const EvalParams<float> &p, const in
             for (int q = 0; q < NP; ++q) { y[i][q] = y_n[i][q] ^ (((f32x2)m << 32) | m); g[i][q] = 0ull; }   // y = s x
         }
         if (PF && c + Wk < nc) fetch(c + Wk);
-        eval_points_f2<K, NP, GRAD, UV>(y, s_tab2, n_real, n_cplx, fe, g);
+        eval_points_f2<K, NP, GRAD, UV>(y, s_tab2, s_tabg, n_real, n_cplx, fe, g);
         if (GRAD) {
 #pragma unroll
             for (int i = 0; i < K; ++i) {
@@ -746,7 +845,7 @@ __device__ __forceinline__ void run_item_f2(const EvalParams<float> &p, const in
 // allocation while all lengths share one grid (no per-length launch tails) ---------------------------
 template <int K, int NP, bool GRAD>
 __device__ __noinline__ void item_body_f2(const EvalParams<float> &p, const int32_t *s_lits, const f32x2 *s_tab2,
-                                          float (*s_F)[64 * NP], int n_real, int n_cplx, int nc, int uv)
+                                          const float *s_tabg, float (*s_F)[64 * NP], int n_real, int n_cplx, int nc, int uv)
 {
     constexpr int V = 2 * NP;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -758,9 +857,9 @@ __device__ __noinline__ void item_body_f2(const EvalParams<float> &p, const int3
     for (int q = 0; q < NP; ++q) fe2[q] = 0ull;
     if (active) {
         constexpr bool PF = K <= 5;
-        if (uv == 1) run_item_f2<K, NP, GRAD, PF, 1>(p, s_lits, s_tab2, n_real, n_cplx, nc, wk, b, fe2);
-        else if (uv == 2) run_item_f2<K, NP, GRAD, PF, 2>(p, s_lits, s_tab2, n_real, n_cplx, nc, wk, b, fe2);
-        else run_item_f2<K, NP, GRAD, PF, 0>(p, s_lits, s_tab2, n_real, n_cplx, nc, wk, b, fe2);
+        if (uv == 1) run_item_f2<K, NP, GRAD, PF, 1>(p, s_lits, s_tab2, s_tabg, n_real, n_cplx, nc, wk, b, fe2);
+        else if (uv == 2) run_item_f2<K, NP, GRAD, PF, 2>(p, s_lits, s_tab2, s_tabg, n_real, n_cplx, nc, wk, b, fe2);
+        else run_item_f2<K, NP, GRAD, PF, 0>(p, s_lits, s_tab2, s_tabg, n_real, n_cplx, nc, wk, b, fe2);
     }
     float fe[V];
 #pragma unroll
@@ -771,10 +870,10 @@ __device__ __noinline__ void item_body_f2(const EvalParams<float> &p, const int3
 template <int K, int KHI, int NP, bool GRAD>
 struct SwitchF2 {
     static __device__ __forceinline__ void go(int k, const EvalParams<float> &p, const int32_t *s_lits, const f32x2 *s_tab2,
-                                              float (*s_F)[64 * NP], int n_real, int n_cplx, int nc, int uv)
+                                              const float *s_tabg, float (*s_F)[64 * NP], int n_real, int n_cplx, int nc, int uv)
     {
-        if (k == K) item_body_f2<K, NP, GRAD>(p, s_lits, s_tab2, s_F, n_real, n_cplx, nc, uv);
-        else if (K < KHI) SwitchF2<(K < KHI ? K + 1 : K), KHI, NP, GRAD>::go(k, p, s_lits, s_tab2, s_F, n_real, n_cplx, nc, uv);
+        if (k == K) item_body_f2<K, NP, GRAD>(p, s_lits, s_tab2, s_tabg, s_F, n_real, n_cplx, nc, uv);
+        else if (K < KHI) SwitchF2<(K < KHI ? K + 1 : K), KHI, NP, GRAD>::go(k, p, s_lits, s_tab2, s_tabg, s_F, n_real, n_cplx, nc, uv);
     }
 };
 
@@ -783,6 +882,7 @@ __global__ void __launch_bounds__(CTA_THREADS, MINB) k_eval_f2m(const EvalParams
 {
     constexpr int H = (KHI + 1) / 2 + 1;
     __shared__ __align__(16) f32x2 s_tab2[(H + 2) * ROW2];
+    __shared__ float s_tabg[H * ROW2G];
     __shared__ int32_t s_lits[LIT_CHUNK];
     __shared__ float s_F[CTA_WARPS][64 * NP];
     const Item it = p.items[blockIdx.x];
@@ -793,10 +893,11 @@ __global__ void __launch_bounds__(CTA_THREADS, MINB) k_eval_f2m(const EvalParams
         const float v = __ldg(p.rows2 + (int64_t)sg.row2_off * ROW2 + i);
         s_tab2[i] = pk(v, v);
     }
+    for (int i = threadIdx.x; i < n_gen * ROW2G; i += blockDim.x) s_tabg[i] = __ldg(p.rows2g + (int64_t)sg.row2g_off * ROW2G + i);
     const int nl = (it.c_end - it.c_begin) * it.k;
     for (int i = threadIdx.x; i < nl; i += blockDim.x) s_lits[i] = __ldg(p.lits + it.lit_base + i);
     __syncthreads();
-    SwitchF2<KLO, KHI, NP, GRAD>::go(it.k, p, s_lits, s_tab2, s_F, n_unit, n_gen, it.c_end - it.c_begin, uv);
+    SwitchF2<KLO, KHI, NP, GRAD>::go(it.k, p, s_lits, s_tab2, s_tabg, s_F, n_unit, n_gen, it.c_end - it.c_begin, uv);
 }
 
 // one body per length: KHI <= 20 for both instantiations (fp32 beyond k = 8 runs the lane-split kernels of afsat_split.cuh)

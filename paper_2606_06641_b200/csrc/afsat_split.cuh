@@ -299,9 +299,9 @@ __device__ __noinline__ void item_body_split(const EvalParams<T> &p, const int32
 }
 
 // ---- packed form (V = 2): a lane holds TWO adjacent candidates as f32x2 pairs and every product is an FFMA2 / FMUL2
-// (DESIGN.md 6.1 "FFMA2"): half the issue slots for the same flops.  FFMA2 has no negated operands, so -Im f is made by
-// XOR on the ALU pipe and the backward walk carries the suffix as (Re s, -Im s).  12 registers per literal, so this
-// form serves the lengths whose KS fits the register budget (9 <= k <= AFSAT_B_KMAX32).
+// (DESIGN.md 6.1 "FFMA2"): half the issue slots for the same flops.  The same literal groups as the scalar form, with the
+// group coefficients fed through FFMA2's broadcast operand; FFMA2 has no negated operands, so the three negations a
+// group needs per point (-Im q, -Im suffix, -Im T) are XORs on the ALU pipe.  Serves 9 <= k <= 20 in fp32.
 constexpr f32x2 SGN2 = 0x8000000080000000ull;
 __device__ __forceinline__ f32x2 shfl2(unsigned mask, f32x2 v, int d)
 {
@@ -310,78 +310,111 @@ __device__ __forceinline__ f32x2 shfl2(unsigned mask, f32x2 v, int d)
 }
 
 template <int KS, int NS, bool GRAD>
-__device__ __forceinline__ void eval_points_split2(unsigned mask, const f32x2 (&y)[KS], bool miss,
-                                                   const float *__restrict__ tab, int n_real, int n_cplx, f32x2 &fe,
-                                                   f32x2 (&g)[KS])
+__device__ __forceinline__ void eval_points_grp2(unsigned mask, const f32x2 (&y)[KS], f32x2 pad2, const float *__restrict__ tab,
+                                                 int n_real, int n_cplx, f32x2 &fe, f32x2 (&g)[KS])
 {
     static_assert(NS == 2, "the packed form exchanges with one partner");
-    constexpr int CW = 32 / NS;
-    const f32x2 one2 = pk(1.0f, 1.0f);
+    constexpr int M = GRP_M, NG = (KS + M - 1) / M, CW = 32 / NS;
+    f32x2 yy[NG * M][1], e[NG][M][1], A[NG][M][1];
+#pragma unroll
+    for (int i = 0; i < NG * M; ++i) yy[i][0] = i < KS ? y[i < KS ? i : 0] : pad2;
+#pragma unroll
+    for (int gq = 0; gq < NG; ++gq) {
+        esp_f2<M, 1>(&yy[gq * M], e[gq]);
+#pragma unroll
+        for (int j = 0; j < M; ++j) A[gq][j][0] = 0ull;
+    }
     const float *r = tab;
-    for (int p = 0; p < n_real; ++p, r += 8) {                       // self-conjugate points
-        const f32x2 a = pk(r[0], r[0]), b = pk(r[2], r[2]), w = pk(r[4], r[4]), wb = pk(r[6], r[6]);
-        f32x2 pre[KS], f[KS];
+    for (int p = 0; p < n_real; ++p, r += ROWG) {                    // self-conjugate points
+        f32x2 q[NG], pre[NG];
 #pragma unroll
-        for (int i = 0; i < KS; ++i) f[i] = fma2(b, y[i], a);
-        if (miss) f[KS - 1] = one2;
-        f32x2 run = f[0];
+        for (int gq = 0; gq < NG; ++gq) {
+            f32x2 sacc = bcf(r[0]);
 #pragma unroll
-        for (int i = 1; i < KS; ++i) { pre[i] = run; run = mul2(run, f[i]); }
+            for (int j = 0; j < M; ++j) sacc = fma2(bcf(r[2 * j + 2]), e[gq][j][0], sacc);
+            q[gq] = sacc;
+        }
+        f32x2 run = q[0];
+#pragma unroll
+        for (int gq = 1; gq < NG; ++gq) { pre[gq] = run; run = mul2(run, q[gq]); }
         const f32x2 oth = shfl2(mask, run, CW);
-        fe = fma2(w, mul2(run, oth), fe);
+        f32x2 suf = mul2(bcf(r[2 * M + 2]), oth);
+        fe = fma2(suf, run, fe);
         if (GRAD) {
-            f32x2 suf = mul2(wb, oth);
 #pragma unroll
-            for (int i = KS - 1; i >= 1; --i) { g[i] = fma2(pre[i], suf, g[i]); suf = mul2(suf, f[i]); }
-            g[0] = add2(g[0], suf);                                   // prefix_0 = 1
+            for (int gq = NG - 1; gq >= 0; --gq) {
+                const f32x2 t = gq > 0 ? mul2(pre[gq], suf) : suf;
+#pragma unroll
+                for (int j = 0; j < M; ++j) A[gq][j][0] = fma2(bcf(r[2 * j + 2]), t, A[gq][j][0]);
+                if (gq > 0) suf = mul2(suf, q[gq]);
+            }
         }
     }
-    for (int p = 0; p < n_cplx; ++p, r += 8) {                       // one of each conjugate pair
-        const f32x2 ar = pk(r[0], r[0]), ai = pk(r[1], r[1]), br = pk(r[2], r[2]), bi = pk(r[3], r[3]);
-        f32x2 pr[KS], pi[KS], fr[KS], fi[KS];
+    for (int p = 0; p < n_cplx; ++p, r += ROWG) {                    // one of each conjugate pair
+        f32x2 qr[NG], qi[NG], nqi[NG], pr[NG], pi[NG];
 #pragma unroll
-        for (int i = 0; i < KS; ++i) { fr[i] = fma2(br, y[i], ar); fi[i] = fma2(bi, y[i], ai); }
-        if (miss) { fr[KS - 1] = one2; fi[KS - 1] = 0ull; }
-        f32x2 rr = fr[0], ri = fi[0];
+        for (int gq = 0; gq < NG; ++gq) {
+            f32x2 sr = bcf(r[0]), si = bcf(r[1]);
 #pragma unroll
-        for (int i = 1; i < KS; ++i) {
-            pr[i] = rr; pi[i] = ri;
-            const f32x2 nr = fma2(rr, fr[i], mul2(ri, fi[i] ^ SGN2));   // Re: rr fr - ri fi
-            const f32x2 ni = fma2(rr, fi[i], mul2(ri, fr[i]));          // Im: rr fi + ri fr
+            for (int j = 0; j < M; ++j) { sr = fma2(bcf(r[2 * j + 2]), e[gq][j][0], sr); si = fma2(bcf(r[2 * j + 3]), e[gq][j][0], si); }
+            qr[gq] = sr; qi[gq] = si; nqi[gq] = si ^ SGN2;
+        }
+        f32x2 rr = qr[0], ri = qi[0];
+#pragma unroll
+        for (int gq = 1; gq < NG; ++gq) {
+            pr[gq] = rr; pi[gq] = ri;
+            const f32x2 nr = fma2(rr, qr[gq], mul2(ri, nqi[gq]));     // Re: rr qr - ri qi
+            const f32x2 ni = fma2(rr, qi[gq], mul2(ri, qr[gq]));      // Im: rr qi + ri qr
             rr = nr; ri = ni;
         }
         const f32x2 orr = shfl2(mask, rr, CW), oi = shfl2(mask, ri, CW);
-        const f32x2 tr = fma2(rr, orr, mul2(ri, oi ^ SGN2)), ti = fma2(rr, oi, mul2(ri, orr));   // P_l, the whole product
-        fe = fma2(pk(r[4], r[4]), tr, fe);
-        fe = fma2(pk(-r[5], -r[5]), ti, fe);
+        const float wr = r[2 * M + 2], wi = r[2 * M + 3];
+        f32x2 sr = fma2(bcf(wr), orr, mul2(bcf(-wi), oi)), si = fma2(bcf(wr), oi, mul2(bcf(wi), orr));   // suffix seeded with w x other
+        fe = fma2(sr, rr, fe);
+        fe = fma2(si ^ SGN2, ri, fe);                                 // Re(w other P_lane)
         if (GRAD) {
-            const f32x2 wbr = pk(r[6], r[6]), wbi = pk(r[7], r[7]);
-            f32x2 sr = fma2(wbr, orr, mul2(wbi, oi ^ SGN2));           // suffix (Re s, -Im s) seeded with w b x other
-            f32x2 nsi = fma2(wbr, oi, mul2(wbi, orr)) ^ SGN2;
 #pragma unroll
-            for (int i = KS - 1; i >= 1; --i) {
-                g[i] = fma2(pr[i], sr, g[i]);
-                g[i] = fma2(pi[i], nsi, g[i]);                        // Re(prefix x suffix)
-                const f32x2 nr = fma2(sr, fr[i], mul2(nsi, fi[i]));
-                const f32x2 nn = fma2(nsi, fr[i], mul2(sr, fi[i] ^ SGN2));
-                sr = nr; nsi = nn;
+            for (int gq = NG - 1; gq >= 0; --gq) {
+                f32x2 tr = sr, nti = si ^ SGN2;
+                if (gq > 0) {
+                    tr = fma2(pr[gq], sr, mul2(pi[gq], si ^ SGN2));   // Re: pr sr - pi si
+                    nti = fma2(pr[gq], si, mul2(pi[gq], sr)) ^ SGN2;  // -Im
+                }
+#pragma unroll
+                for (int j = 0; j < M; ++j) {
+                    A[gq][j][0] = fma2(bcf(r[2 * j + 2]), tr, A[gq][j][0]);
+                    A[gq][j][0] = fma2(bcf(r[2 * j + 3]), nti, A[gq][j][0]);          // Re(c_j T)
+                }
+                if (gq > 0) {
+                    const f32x2 nr = fma2(sr, qr[gq], mul2(si, nqi[gq]));
+                    const f32x2 ni = fma2(sr, qi[gq], mul2(si, qr[gq]));
+                    sr = nr; si = ni;
+                }
             }
-            g[0] = add2(g[0], sr);                                    // prefix_0 = 1
         }
+    }
+    if (GRAD) {
+        f32x2 gg[NG * M][1];
+#pragma unroll
+        for (int i = 0; i < NG * M; ++i) gg[i][0] = 0ull;
+#pragma unroll
+        for (int gq = 0; gq < NG; ++gq) loo_f2<M, 1>(&yy[gq * M], A[gq], &gg[gq * M]);
+#pragma unroll
+        for (int i = 0; i < KS; ++i) g[i] = gg[i][0];
     }
 }
 
 template <int KS, int NS, bool GRAD>
 __device__ __forceinline__ void run_item_split2(const EvalParams<float> &p, unsigned mask, const int32_t *__restrict__ s_lits,
                                                 const float *__restrict__ s_tab, int n_real, int n_cplx, int nc, int wk,
-                                                int h, int64_t b, f32x2 &fe, int k)
+                                                int h, int64_t b, f32x2 &fe, int k, float pad)
 {
     const char *xb = reinterpret_cast<const char *>(p.x + b);
     char *gb = reinterpret_cast<char *>(p.G + (b - p.g_b0));
     const uint32_t x_ld = (uint32_t)(p.ldb * 4), g_ld = (uint32_t)(p.g_ld * 4);
     const int Wk = p.Wk;
     const bool miss = (KS - 1) * NS + h >= k;
-    const f32x2 one2 = pk(1.0f, 1.0f);
+    const f32x2 pad2 = pk(pad, pad);
     for (int c = wk; c < nc; c += Wk) {
         const int32_t *L = s_lits + c * k + h;
         int32_t lit[KS];
@@ -391,11 +424,11 @@ __device__ __forceinline__ void run_item_split2(const EvalParams<float> &p, unsi
         lit[KS - 1] = miss ? LIT_NONE : L[(KS - 1) * NS];             // missing literal: constant, no gather, no RED
 #pragma unroll
         for (int i = 0; i < KS; ++i) {
-            f32x2 v[1] = {one2};
+            f32x2 v[1] = {pad2};
             if (!(i == KS - 1 && (lit[i] & LIT_NONE)))
                 PairIO<1>::load(xb + (uint64_t)(uint32_t)(lit[i] & LIT_VAR) * x_ld, v);
             const uint32_t m = (uint32_t)(lit[i] & LIT_NEG);
-            y[i] = v[0] ^ (((f32x2)m << 32) | m);                     // y = s x
+            y[i] = v[0] ^ (((f32x2)m << 32) | m);                     // y = s x (a missing slot: pad, its polarity bit is 0)
             g[i] = 0ull;
         }
 #if AFSAT_L32_PREFETCH
@@ -409,7 +442,7 @@ __device__ __forceinline__ void run_item_split2(const EvalParams<float> &p, unsi
             }
         }
 #endif
-        eval_points_split2<KS, NS, GRAD>(mask, y, miss, s_tab, n_real, n_cplx, fe, g);
+        eval_points_grp2<KS, NS, GRAD>(mask, y, pad2, s_tab, n_real, n_cplx, fe, g);
         if (GRAD) {
 #pragma unroll
             for (int i = 0; i < KS; ++i) {
@@ -424,7 +457,7 @@ __device__ __forceinline__ void run_item_split2(const EvalParams<float> &p, unsi
 
 template <int KS, int NS, bool GRAD>
 __device__ __noinline__ void item_body_split2(const EvalParams<float> &p, const int32_t *s_lits, const float *s_tab,
-                                              float (*s_F)[64], int n_real, int n_cplx, int nc, int k)
+                                              float (*s_F)[64], int n_real, int n_cplx, int nc, int k, float pad)
 {
     constexpr int CW = 32 / NS;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -435,7 +468,7 @@ __device__ __noinline__ void item_body_split2(const EvalParams<float> &p, const 
     const unsigned mask = __ballot_sync(0xffffffffu, active);
     f32x2 fe2 = 0ull;
     if (active) {
-        run_item_split2<KS, NS, GRAD>(p, mask, s_lits, s_tab, n_real, n_cplx, nc, wk, h, b, fe2, k);
+        run_item_split2<KS, NS, GRAD>(p, mask, s_lits, s_tab, n_real, n_cplx, nc, wk, h, b, fe2, k, pad);
     }
     if (!p.Fpart) return;
     float f0, f1; upk(fe2, f0, f1);
@@ -457,7 +490,7 @@ struct SwitchSplit {
                                               T (*s_F)[32 * V], int n_real, int n_cplx, int nc, int k, T pad)
     {
         if (ks == KS) {
-            if constexpr (V == 2) item_body_split2<KS, NS, GRAD>(p, s_lits, s_tab, s_F, n_real, n_cplx, nc, k);
+            if constexpr (V == 2) item_body_split2<KS, NS, GRAD>(p, s_lits, s_tab, s_F, n_real, n_cplx, nc, k, pad);
             else item_body_split<T, KS, NS, GRAD>(p, s_lits, s_tab, s_F, n_real, n_cplx, nc, k, pad);
         } else if (KS < KSHI)
             SwitchSplit<T, (KS < KSHI ? KS + 1 : KS), KSHI, NS, V, GRAD>::go(ks, p, s_lits, s_tab, s_F, n_real, n_cplx, nc, k, pad);
@@ -465,24 +498,19 @@ struct SwitchSplit {
 };
 
 // one launch for every length in [KLO, KHI]: the CTA's item picks the body compiled for ceil(k / NS) literals per lane.
-// V = 1: grouped scalar form (staged table rowsg, ROWG scalars per point); V = 2: packed form (table rows, 8 per point).
+// V = 1: scalar form; V = 2: packed form (fp32 only); both read the grouped staged table rowsg (ROWG scalars per point).
 template <typename T, int KLO, int KHI, int NS, int V, bool GRAD, int THREADS, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB) k_eval_split(const EvalParams<T> p)
 {
-    constexpr int RW = V == 1 ? ROWG : 8;
-    __shared__ __align__(16) T s_tab[((KHI + 1) / 2 + 1) * RW];
+    __shared__ __align__(16) T s_tab[((KHI + 1) / 2 + 1) * ROWG];
     __shared__ int32_t s_lits[LIT_CHUNK];
     __shared__ T s_F[THREADS / 32][32 * V];
     const Item it = p.items[blockIdx.x];
     const SigDev sg = p.sigs[it.sig];
-    if (V == 1) {
-        const int nsc = (sg.n_real + sg.n_cplx) * ROWG;
-        for (int i = threadIdx.x; i < nsc; i += blockDim.x) s_tab[i] = p.rowsg[(int64_t)sg.row2_off * ROWG + i];
-        const int nl = (it.c_end - it.c_begin) * it.k;
-        for (int i = threadIdx.x; i < nl; i += blockDim.x) s_lits[i] = __ldg(p.lits + it.lit_base + i);
-    } else {
-        stage_item(p, it, sg, s_tab, s_lits);
-    }
+    const int nsc = (sg.n_real + sg.n_cplx) * ROWG;
+    for (int i = threadIdx.x; i < nsc; i += blockDim.x) s_tab[i] = p.rowsg[(int64_t)sg.row2_off * ROWG + i];
+    const int nl = (it.c_end - it.c_begin) * it.k;
+    for (int i = threadIdx.x; i < nl; i += blockDim.x) s_lits[i] = __ldg(p.lits + it.lit_base + i);
     __syncthreads();
     SwitchSplit<T, (KLO + NS - 1) / NS, (KHI + NS - 1) / NS, NS, V, GRAD>::go((it.k + NS - 1) / NS, p, s_lits, s_tab, s_F, sg.n_real,
                                                                         sg.n_cplx, it.c_end - it.c_begin, it.k, (T)sg.pad);

@@ -120,6 +120,9 @@ struct CheckParams {
     int32_t *step_ctr;          // or null: incremented once per launch (the step index of a replayed CUDA graph)
 };
 constexpr int CHK_MLP = 8;
+// SigDev::chk_kind: predicates of the count tau of true literals that need no counting
+enum { CHK_GENERAL = 0, CHK_OR = 1 /* tau >= 1 */, CHK_NONE = 2 /* tau == 0 */, CHK_ALL = 3 /* tau == k */,
+       CHK_NAND = 4 /* tau < k */, CHK_NAE = 5 /* 0 < tau < k */, CHK_EQ = 6 /* tau in {0, k} */, CHK_ODD = 7, CHK_EVEN = 8 };
 
 __global__ void __launch_bounds__(CTA_THREADS) k_check_bits(const CheckParams p)
 {
@@ -131,11 +134,27 @@ __global__ void __launch_bounds__(CTA_THREADS) k_check_bits(const CheckParams p)
     const int word = p.w_begin + blockIdx.y * p.wpb + wi;
     const bool valid = word < p.w_end;
     const uint32_t *bw = p.bits + (valid ? word : p.w_begin);
-    uint32_t cnt[13];
+    // satisfied constraints per candidate, bit-sliced, in two levels: a 3-plane counter takes 7 constraints, then it is
+    // added into the 13-plane counter (a full 13-plane ripple per constraint was a third of this kernel's instructions)
+    uint32_t cnt[13], lo[3] = {0u, 0u, 0u};
 #pragma unroll
     for (int j = 0; j < 13; ++j) cnt[j] = 0u;
-    int nacc = 0;                                                     // constraints counted in cnt[] so far
+    int nlo = 0, nacc = 0;                                            // constraints in lo[] / in cnt[] + lo[] so far
+    auto fold = [&]() {                                               // cnt += lo (3-plane value), lo = 0
+        uint32_t carry = 0u;
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            const uint32_t a = cnt[j], bq = lo[j];
+            cnt[j] = a ^ bq ^ carry;
+            carry = (a & bq) | (carry & (a ^ bq));
+            lo[j] = 0u;
+        }
+#pragma unroll
+        for (int j = 3; j < 13; ++j) { const uint32_t sv = cnt[j] ^ carry; carry &= cnt[j]; cnt[j] = sv; }
+        nlo = 0;
+    };
     auto flush = [&]() {                                              // bit-sliced counter -> per-candidate integers
+        fold();
         for (int bit = 0; bit < 32; ++bit) {
             int val = 0;
 #pragma unroll
@@ -149,7 +168,7 @@ __global__ void __launch_bounds__(CTA_THREADS) k_check_bits(const CheckParams p)
     for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {   // persistent over work items
         const Item it = p.items[item];
         const SigDev sg = p.sigs[it.sig];
-        const int k = it.k, nc = it.c_end - it.c_begin;
+        const int k = it.k, nc = it.c_end - it.c_begin, kind = sg.chk_kind;
         __syncthreads();                                              // previous item's literals are consumed
         for (int i = threadIdx.x; i < nc * k; i += blockDim.x) s_lits[i] = __ldg(p.lits + it.lit_base + i);
         __syncthreads();
@@ -157,43 +176,65 @@ __global__ void __launch_bounds__(CTA_THREADS) k_check_bits(const CheckParams p)
         int nb = 1;
         while ((1 << nb) <= k) ++nb;                                  // bits of tau in [0, k]
         const int mine = (nc - grp + ngrp - 1) / ngrp;
-        if (nacc + mine > 8191) flush();
+        if (nacc + mine > 8000) flush();
         nacc += mine > 0 ? mine : 0;
         for (int c = grp; c < nc; c += ngrp) {
-            uint32_t t[7] = {0u, 0u, 0u, 0u, 0u, 0u, 0u};
             const int32_t *L = s_lits + c * k;
-            for (int i0 = 0; i0 < k; i0 += CHK_MLP) {
-                uint32_t mm[CHK_MLP];
+            uint32_t sat;
+            if (kind != CHK_GENERAL) {
+                // predicates that are a function of (any literal true, all literals true, parity): no counting at all
+                uint32_t any = 0u, all = 0xffffffffu, par = 0u;
+                for (int i0 = 0; i0 < k; i0 += CHK_MLP) {
+                    uint32_t mm[CHK_MLP];
 #pragma unroll
-                for (int u = 0; u < CHK_MLP; ++u) {
-                    mm[u] = 0u;
-                    if (i0 + u < k) {
-                        const int32_t lit = L[i0 + u];
-                        const uint32_t w = __ldg(bw + (int64_t)(lit & LIT_VAR) * p.ldw);
-                        mm[u] = lit < 0 ? ~w : w;                     // literal true = variable true XOR negated
-                    }
+                    for (int u = 0; u < CHK_MLP; ++u)
+                        if (i0 + u < k) {
+                            const int32_t lit = L[i0 + u];
+                            const uint32_t w = __ldg(bw + (int64_t)(lit & LIT_VAR) * p.ldw);
+                            mm[u] = lit < 0 ? ~w : w;                 // literal true = variable true XOR negated
+                        }
+#pragma unroll
+                    for (int u = 0; u < CHK_MLP; ++u)
+                        if (i0 + u < k) { any |= mm[u]; all &= mm[u]; par ^= mm[u]; }
                 }
+                sat = kind == CHK_OR ? any : kind == CHK_NONE ? ~any : kind == CHK_ALL ? all : kind == CHK_NAND ? ~all
+                    : kind == CHK_NAE ? (any & ~all) : kind == CHK_EQ ? (all | ~any) : kind == CHK_ODD ? par : ~par;
+            } else {
+                uint32_t t[7] = {0u, 0u, 0u, 0u, 0u, 0u, 0u};
+                for (int i0 = 0; i0 < k; i0 += CHK_MLP) {
+                    uint32_t mm[CHK_MLP];
 #pragma unroll
-                for (int u = 0; u < CHK_MLP; ++u) {
-                    uint32_t m = mm[u];
+                    for (int u = 0; u < CHK_MLP; ++u)
+                        if (i0 + u < k) {
+                            const int32_t lit = L[i0 + u];
+                            const uint32_t w = __ldg(bw + (int64_t)(lit & LIT_VAR) * p.ldw);
+                            mm[u] = lit < 0 ? ~w : w;
+                        }
+#pragma unroll
+                    for (int u = 0; u < CHK_MLP; ++u)
+                        if (i0 + u < k) {
+                            uint32_t m = mm[u];
+#pragma unroll
+                            for (int j = 0; j < 7; ++j)
+                                if (j < nb) { const uint32_t sv = t[j] ^ m; m &= t[j]; t[j] = sv; }
+                        }
+                }
+                uint32_t acc = 0u;
+                for (int tau = 0; tau <= k; ++tau) {
+                    const uint64_t bit = tau < 64 ? (sg.scan_lo >> tau) : (sg.scan_hi >> (tau - 64));
+                    if (!(bit & 1ull)) continue;
+                    uint32_t eq = 0xffffffffu;
 #pragma unroll
                     for (int j = 0; j < 7; ++j)
-                        if (j < nb) { const uint32_t s = t[j] ^ m; m &= t[j]; t[j] = s; }
+                        if (j < nb) eq &= ((tau >> j) & 1) ? t[j] : ~t[j];
+                    acc |= eq;
                 }
+                sat = sg.scan_is_sat ? acc : ~acc;                    // 1 = constraint satisfied
             }
-            uint32_t acc = 0u;
-            for (int tau = 0; tau <= k; ++tau) {
-                const uint64_t bit = tau < 64 ? (sg.scan_lo >> tau) : (sg.scan_hi >> (tau - 64));
-                if (!(bit & 1ull)) continue;
-                uint32_t eq = 0xffffffffu;
+            uint32_t carry = sat;
 #pragma unroll
-                for (int j = 0; j < 7; ++j)
-                    if (j < nb) eq &= ((tau >> j) & 1) ? t[j] : ~t[j];
-                acc |= eq;
-            }
-            uint32_t carry = sg.scan_is_sat ? acc : ~acc;             // 1 = constraint satisfied
-#pragma unroll
-            for (int j = 0; j < 13; ++j) { const uint32_t s = cnt[j] ^ carry; carry &= cnt[j]; cnt[j] = s; }
+            for (int j = 0; j < 3; ++j) { const uint32_t sv = lo[j] ^ carry; carry &= lo[j]; lo[j] = sv; }
+            if (++nlo == 7) fold();
         }
     }
     if (valid && nacc) flush();

@@ -885,7 +885,8 @@ def test_step_paths_agree(dtype):
     inst, hidden = I.plant_solution(base, seed=5)
     npdt = np.float32 if dtype == 32 else np.float64
     x0 = I.make_x0(inst, seed=172, batch=80).astype(npdt)
-    x0[:, 3] = np.where(hidden, -0.9, 0.9)                             # candidates at / next to the hidden solution
+    x0[:, 3] = np.where(hidden, -1.0, 1.0)                             # AT the hidden solution: a fixed point of PGD (F = -m
+    #                                                                    is the minimum over the cube), solved at step 1; and next to it
     x0[:, 70] = np.where(hidden, -0.6, 0.6)
     x0[:2, 70] *= -1
     x0[inst.fixed != 0] = inst.fixed[inst.fixed != 0].astype(npdt)[:, None]
