@@ -881,7 +881,8 @@ int afsat_create_ex(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64
         }
         if (class_of(kk, dtype) == CLS_LONG || (dtype == 32 && class_of(kk, dtype) == CLS_B)) {   // grouped lane-split kernels
             double packed[AFSAT_MAX_POINTS * ROWG];
-            d.pad = (int8_t)pack_rows_grp(hs.rows, hs.n_real + hs.n_cplx, kk, packed);
+            const int ns = dtype == 64 ? 4 : 2;                        // lanes per candidate (pair) of the kernel that runs kk
+            d.pad = (int8_t)pack_rows_grp(hs.rows, hs.n_real + hs.n_cplx, kk, ns, packed);
             d.row2_off = (int32_t)(rowsg.size() / ROWG);
             rowsg.insert(rowsg.end(), packed, packed + (size_t)(hs.n_real + hs.n_cplx) * ROWG);
         }

@@ -615,7 +615,8 @@ __device__ __forceinline__ void eval_points_f2(const f32x2 (&y)[K][NP], const f3
             oct_row_f2<K, NP, GRAD>(y, rO, 0.70710678118654752f, fe, g);             // = 2 Re b of the row, bit for bit
             oct_row_f2<K, NP, GRAD>(y, rO + ROW2, -0.70710678118654752f, fe, g);
         }
-        if constexpr (K >= 2) grp_rows_f2<K, NP, GRAD>(y, tabg, n_cplx, fe, g);   // the generic complex points, grouped
+        // the generic complex points, grouped (K = 3 and K = 7 have none: all their points are trivial twiddles)
+        if constexpr (K >= 2 && K != 3 && K != 7) { if (n_cplx > 0) grp_rows_f2<K, NP, GRAD>(y, tabg, n_cplx, fe, g); }
         return;
     }
     const f32x2 *r = tab;
@@ -645,7 +646,7 @@ __device__ __forceinline__ void eval_points_f2(const f32x2 (&y)[K][NP], const f3
             for (int q = 0; q < NP; ++q) g[0][q] = add2(g[0][q], suf[q]);     // prefix_0 = 1
         }
     }
-    if constexpr (K >= 2) grp_rows_f2<K, NP, GRAD>(y, tabg, n_cplx, fe, g);       // one of each conjugate pair, grouped
+    if constexpr (K >= 2) { if (n_cplx > 0) grp_rows_f2<K, NP, GRAD>(y, tabg, n_cplx, fe, g); }   // one of each conjugate pair, grouped
 }
 
 // sign flip by the literal's polarity bit (bit 31 of the packed literal): one LOP3 per value

@@ -47,37 +47,50 @@ namespace afsat {
 #ifndef AFSAT_L32_KMIN
 #define AFSAT_L32_KMIN (AFSAT_B_KMAX + 1)
 #endif
-#ifndef AFSAT_GRP_M
-#define AFSAT_GRP_M 4                  // literals per group
-#endif
-constexpr int GRP_M = AFSAT_GRP_M;
-constexpr int ROWG = 2 * (GRP_M + 1) + 2;   // staged row of a grouped kernel: {Re c_0, Im c_0, ..., Re c_M, Im c_M, Re w, Im w}
+// Group layout of a lane with KS literal slots: NG = ceil(KS / 4) groups of BALANCED sizes -- the first NHI = KS mod NG
+// groups take MHI = MLO + 1 literals, the others MLO = floor(KS / NG) (<= 4) -- so that no slot is wasted on padding.
+// Staged row of a point: {Re, Im of c_0 .. c_MHI for groups of MHI | the same for groups of MLO (from scalar ROWG_LO) |
+// Re w, Im w (at ROWG_W)},  c_j = a^(M-j) b^j.
+constexpr int GRP_MAX = 4;
+constexpr int ROWG_LO = 2 * (GRP_MAX + 1), ROWG_W = 4 * (GRP_MAX + 1), ROWG = ROWG_W + 2;
+struct GrpLayout { int NG, MLO, NHI, MHI; };
+__host__ __device__ constexpr GrpLayout grp_layout(int KS)
+{
+    const int NG = (KS + GRP_MAX - 1) / GRP_MAX, MLO = KS / NG, NHI = KS % NG;
+    return GrpLayout{NG, MLO, NHI, MLO + (NHI > 0 ? 1 : 0)};
+}
+__host__ __device__ constexpr int grp_size(const GrpLayout &L, int gq) { return gq < L.NHI ? L.MHI : L.MLO; }
+__host__ __device__ constexpr int grp_off(const GrpLayout &L, int gq) { return gq < L.NHI ? gq * L.MHI : L.NHI * L.MHI + (gq - L.NHI) * L.MLO; }
 
 // HOST: the staged table of one signature for the grouped kernels, from its rows {Re a, Im a, Re b, Im b, Re w, Im w, ..}
-// (real rows first): c_j = a^(M-j) b^j.  The paper's tables (a = 1/2 in every row) are staged un-halved (see above).
-// Returns the pad value (0 or 1).
-inline int pack_rows_grp(const double *r0, int n_rows, int k, double *out)
+// (real rows first), for lanes of KS = ceil(k / NS) slots.  The paper's tables (a = 1/2 in every row) are staged
+// un-halved (see above).  Returns the pad value (0 or 1).
+inline int pack_rows_grp(const double *r0, int n_rows, int k, int ns, double *out)
 {
     bool std_tab = true;
     for (int q = 0; q < n_rows; ++q) std_tab = std_tab && r0[8 * q] == 0.5 && r0[8 * q + 1] == 0.0;
     const double sc = std_tab ? 2.0 : 1.0;
     double scw = 1.0;
     if (std_tab) for (int i = 0; i < k; ++i) scw *= 0.5;
+    const GrpLayout L = grp_layout((k + ns - 1) / ns);
+    const int M[2] = {L.MHI, L.MLO}, off[2] = {0, ROWG_LO};
     for (int q = 0; q < n_rows; ++q) {
         const double *r = r0 + 8 * q;
         double *o = out + (size_t)q * ROWG;
+        for (int j = 0; j < ROWG; ++j) o[j] = 0.0;
         const double ar = sc * r[0], ai = sc * r[1], br = sc * r[2], bi = sc * r[3];
-        // a^(M-j) b^j by repeated multiplication of double-precision values (M <= 6: relative error ~1e-15)
-        for (int j = 0; j <= GRP_M; ++j) {
-            double cr = 1.0, ci = 0.0;
-            for (int t = 0; t < GRP_M; ++t) {
-                const double fr = t < j ? br : ar, fi = t < j ? bi : ai;
-                const double nr = cr * fr - ci * fi, ni = cr * fi + ci * fr;
-                cr = nr; ci = ni;
+        // a^(M-j) b^j by repeated multiplication of double-precision values (M <= 4: relative error ~1e-15)
+        for (int gq = 0; gq < 2; ++gq)
+            for (int j = 0; j <= M[gq]; ++j) {
+                double cr = 1.0, ci = 0.0;
+                for (int t = 0; t < M[gq]; ++t) {
+                    const double fr = t < j ? br : ar, fi = t < j ? bi : ai;
+                    const double nr = cr * fr - ci * fi, ni = cr * fi + ci * fr;
+                    cr = nr; ci = ni;
+                }
+                o[off[gq] + 2 * j] = cr; o[off[gq] + 2 * j + 1] = ci;
             }
-            o[2 * j] = cr; o[2 * j + 1] = ci;
-        }
-        o[2 * GRP_M + 2] = r[4] * scw; o[2 * GRP_M + 3] = r[5] * scw;
+        o[ROWG_W] = r[4] * scw; o[ROWG_W + 1] = r[5] * scw;
     }
     return std_tab ? 0 : 1;
 }
@@ -103,42 +116,48 @@ __device__ __forceinline__ void others_cplx(unsigned mask, T vr, T vi, T &orr, T
     orr = fma_(n1r, por, -(n1i * poi)); oi = fma_(n1r, poi, n1i * por);
 }
 
-// a2-a4 for the lane's KS literal slots of one constraint (slots without a literal hold `pad`); tab: ROWG scalars per
-// retained DFT point, real points first.  Returns the lane's partial gradients dFE/dy_i in g.
+// a2-a4 for the lane's KS literal slots of one constraint (a slot without a literal holds the pad value); tab: ROWG scalars
+// per retained DFT point, real points first.  Returns the lane's partial gradients dFE/dy_i in g.
 template <typename T, int KS, int NS, bool GRAD>
-__device__ __forceinline__ void eval_points_grp(unsigned mask, const T (&y)[KS], T pad, const T *__restrict__ tab, int n_real,
+__device__ __forceinline__ void eval_points_grp(unsigned mask, const T (&y)[KS], const T *__restrict__ tab, int n_real,
                                                 int n_cplx, T &fe, T (&g)[KS])
 {
-    constexpr int M = GRP_M, NG = (KS + M - 1) / M;
-    T e[NG][M], A[NG][M];                                            // e[g][j-1] = e_j(group g); A[g][j-1] pairs with c_j
+    constexpr GrpLayout L = grp_layout(KS);
+    constexpr int NG = L.NG, MX = L.MHI;
+    T e[NG][MX], A[NG][MX];                                          // e[g][j-1] = e_j(group g); A[g][j-1] pairs with c_j
 #pragma unroll
     for (int gq = 0; gq < NG; ++gq) {
-        T ee[M + 1];
+        const int Mg = grp_size(L, gq), off = grp_off(L, gq);
+        T ee[MX + 1];
         ee[0] = T(1);
 #pragma unroll
-        for (int j = 1; j <= M; ++j) ee[j] = T(0);
+        for (int j = 1; j <= MX; ++j) ee[j] = T(0);
 #pragma unroll
-        for (int u = 0; u < M; ++u) {
-            const T yv = (gq * M + u < KS) ? y[gq * M + u < KS ? gq * M + u : 0] : pad;
+        for (int u = 0; u < MX; ++u)
+            if (u < Mg) {
+                const T yv = y[off + u < KS ? off + u : 0];
 #pragma unroll
-            for (int j = M; j >= 1; --j)
-                if (j <= u + 1) ee[j] = fma_(yv, ee[j - 1], ee[j]);
-        }
+                for (int j = MX; j >= 1; --j)
+                    if (j <= u + 1) ee[j] = fma_(yv, ee[j - 1], ee[j]);
+            }
 #pragma unroll
-        for (int j = 0; j < M; ++j) { e[gq][j] = ee[j + 1]; A[gq][j] = T(0); }
+        for (int j = 0; j < MX; ++j) { e[gq][j] = ee[j + 1]; A[gq][j] = T(0); }
     }
     const T *r = tab;
     for (int p = 0; p < n_real; ++p, r += ROWG) {                    // self-conjugate points
-        T c[M + 1];
+        T ch[MX + 1], cl[MX + 1];
 #pragma unroll
-        for (int j = 0; j <= M; ++j) c[j] = r[2 * j];
-        const T w = r[2 * M + 2];
+        for (int j = 0; j <= MX; ++j) { ch[j] = r[2 * j]; cl[j] = r[ROWG_LO + 2 * j]; }
+        const T w = r[ROWG_W];
         T q[NG], pre[NG];
 #pragma unroll
         for (int gq = 0; gq < NG; ++gq) {
-            T sacc = c[0];
+            const int Mg = grp_size(L, gq);
+            const bool hi = gq < L.NHI;
+            T sacc = hi ? ch[0] : cl[0];
 #pragma unroll
-            for (int j = 0; j < M; ++j) sacc = fma_(c[j + 1], e[gq][j], sacc);
+            for (int j = 0; j < MX; ++j)
+                if (j < Mg) sacc = fma_(hi ? ch[j + 1] : cl[j + 1], e[gq][j], sacc);
             q[gq] = sacc;
         }
         T run = q[0];
@@ -150,24 +169,33 @@ __device__ __forceinline__ void eval_points_grp(unsigned mask, const T (&y)[KS],
         if (GRAD) {
 #pragma unroll
             for (int gq = NG - 1; gq >= 0; --gq) {
+                const int Mg = grp_size(L, gq);
+                const bool hi = gq < L.NHI;
                 const T t = gq > 0 ? pre[gq] * suf : suf;
 #pragma unroll
-                for (int j = 0; j < M; ++j) A[gq][j] = fma_(c[j + 1], t, A[gq][j]);
+                for (int j = 0; j < MX; ++j)
+                    if (j < Mg) A[gq][j] = fma_(hi ? ch[j + 1] : cl[j + 1], t, A[gq][j]);
                 if (gq > 0) suf *= q[gq];
             }
         }
     }
     for (int p = 0; p < n_cplx; ++p, r += ROWG) {                    // one of each conjugate pair
-        T cr[M + 1], ci[M + 1];
+        T chr[MX + 1], chi[MX + 1], clr[MX + 1], cli[MX + 1];
 #pragma unroll
-        for (int j = 0; j <= M; ++j) { cr[j] = r[2 * j]; ci[j] = r[2 * j + 1]; }
-        const T wr = r[2 * M + 2], wi = r[2 * M + 3];
+        for (int j = 0; j <= MX; ++j) {
+            chr[j] = r[2 * j]; chi[j] = r[2 * j + 1];
+            clr[j] = r[ROWG_LO + 2 * j]; cli[j] = r[ROWG_LO + 2 * j + 1];
+        }
+        const T wr = r[ROWG_W], wi = r[ROWG_W + 1];
         T qr[NG], qi[NG], pr[NG], pi[NG];
 #pragma unroll
         for (int gq = 0; gq < NG; ++gq) {
-            T sr = cr[0], si = ci[0];
+            const int Mg = grp_size(L, gq);
+            const bool hi = gq < L.NHI;
+            T sr = hi ? chr[0] : clr[0], si = hi ? chi[0] : cli[0];
 #pragma unroll
-            for (int j = 0; j < M; ++j) { sr = fma_(cr[j + 1], e[gq][j], sr); si = fma_(ci[j + 1], e[gq][j], si); }
+            for (int j = 0; j < MX; ++j)
+                if (j < Mg) { sr = fma_(hi ? chr[j + 1] : clr[j + 1], e[gq][j], sr); si = fma_(hi ? chi[j + 1] : cli[j + 1], e[gq][j], si); }
             qr[gq] = sr; qi[gq] = si;
         }
         T rr = qr[0], ri = qi[0];
@@ -186,13 +214,16 @@ __device__ __forceinline__ void eval_points_grp(unsigned mask, const T (&y)[KS],
         if (GRAD) {
 #pragma unroll
             for (int gq = NG - 1; gq >= 0; --gq) {
+                const int Mg = grp_size(L, gq);
+                const bool hi = gq < L.NHI;
                 T tr = sr, ti = si;
                 if (gq > 0) { tr = fma_(pr[gq], sr, -(pi[gq] * si)); ti = fma_(pr[gq], si, pi[gq] * sr); }
 #pragma unroll
-                for (int j = 0; j < M; ++j) {
-                    A[gq][j] = fma_(cr[j + 1], tr, A[gq][j]);
-                    A[gq][j] = fma_(-ci[j + 1], ti, A[gq][j]);               // Re(c_j T)
-                }
+                for (int j = 0; j < MX; ++j)
+                    if (j < Mg) {
+                        A[gq][j] = fma_(hi ? chr[j + 1] : clr[j + 1], tr, A[gq][j]);
+                        A[gq][j] = fma_(-(hi ? chi[j + 1] : cli[j + 1]), ti, A[gq][j]);   // Re(c_j T)
+                    }
                 if (gq > 0) {
                     const T nr = fma_(sr, qr[gq], -(si * qi[gq]));
                     const T ni = fma_(sr, qi[gq], si * qr[gq]);
@@ -203,29 +234,32 @@ __device__ __forceinline__ void eval_points_grp(unsigned mask, const T (&y)[KS],
     }
     if (GRAD) {                                                       // dFE/dy_u = sum_j A_j e_{j-1}(group without y_u)
 #pragma unroll
-        for (int gq = 0; gq < NG; ++gq)
+        for (int gq = 0; gq < NG; ++gq) {
+            const int Mg = grp_size(L, gq), off = grp_off(L, gq);
 #pragma unroll
-            for (int u = 0; u < M; ++u) {
-                if (gq * M + u >= KS) continue;
-                T ee[M];
+            for (int u = 0; u < MX; ++u) {
+                if (u >= Mg) continue;
+                T ee[MX];
                 ee[0] = T(1);
 #pragma unroll
-                for (int j = 1; j < M; ++j) ee[j] = T(0);
+                for (int j = 1; j < MX; ++j) ee[j] = T(0);
                 int cntv = 0;
 #pragma unroll
-                for (int v = 0; v < M; ++v) {
-                    if (v == u) continue;
-                    const T yv = (gq * M + v < KS) ? y[gq * M + v < KS ? gq * M + v : 0] : pad;
+                for (int v = 0; v < MX; ++v) {
+                    if (v == u || v >= Mg) continue;
+                    const T yv = y[off + v < KS ? off + v : 0];
 #pragma unroll
-                    for (int j = M - 1; j >= 1; --j)
+                    for (int j = MX - 1; j >= 1; --j)
                         if (j <= cntv + 1) ee[j] = fma_(yv, ee[j - 1], ee[j]);
                     ++cntv;
                 }
                 T acc = A[gq][0];
 #pragma unroll
-                for (int j = 1; j < M; ++j) acc = fma_(A[gq][j], ee[j], acc);
-                g[gq * M + u] = acc;
+                for (int j = 1; j < MX; ++j)
+                    if (j < Mg) acc = fma_(A[gq][j], ee[j], acc);
+                g[off + u < KS ? off + u : 0] = acc;
             }
+        }
     }
 }
 
@@ -263,7 +297,7 @@ __device__ __forceinline__ void run_item_split(const EvalParams<T> &p, unsigned 
             }
         }
 #endif
-        eval_points_grp<T, KS, NS, GRAD>(mask, y, pad, s_tab, n_real, n_cplx, fe, g);
+        eval_points_grp<T, KS, NS, GRAD>(mask, y, s_tab, n_real, n_cplx, fe, g);
         if (GRAD) {
 #pragma unroll
             for (int i = 0; i < KS; ++i) {
@@ -309,43 +343,72 @@ __device__ __forceinline__ f32x2 shfl2(unsigned mask, f32x2 v, int d)
     return pk(__shfl_xor_sync(mask, lo, d), __shfl_xor_sync(mask, hi, d));
 }
 
+// group gq of a packed lane: its symmetric polynomials / its share of the gradient, sizes resolved at compile time
+template <int KS, int GQ>
+__device__ __forceinline__ void grp2_esp(const f32x2 (*y1)[1], f32x2 (*e)[1])
+{
+    constexpr GrpLayout L = grp_layout(KS);
+    constexpr int Mg = grp_size(L, GQ), off = grp_off(L, GQ);
+    f32x2 ee[Mg][1];
+    esp_f2<Mg, 1>(y1 + off, ee);
+#pragma unroll
+    for (int j = 0; j < Mg; ++j) e[j][0] = ee[j][0];
+}
+template <int KS, int GQ>
+__device__ __forceinline__ void grp2_loo(const f32x2 (*y1)[1], const f32x2 (*A)[1], f32x2 (*g1)[1])
+{
+    constexpr GrpLayout L = grp_layout(KS);
+    constexpr int Mg = grp_size(L, GQ), off = grp_off(L, GQ);
+    f32x2 AA[Mg][1];
+#pragma unroll
+    for (int j = 0; j < Mg; ++j) AA[j][0] = A[j][0];
+    loo_f2<Mg, 1>(y1 + off, AA, g1 + off);
+}
+
 template <int KS, int NS, bool GRAD>
-__device__ __forceinline__ void eval_points_grp2(unsigned mask, const f32x2 (&y)[KS], f32x2 pad2, const float *__restrict__ tab,
+__device__ __forceinline__ void eval_points_grp2(unsigned mask, const f32x2 (&y)[KS], const float *__restrict__ tab,
                                                  int n_real, int n_cplx, f32x2 &fe, f32x2 (&g)[KS])
 {
     static_assert(NS == 2, "the packed form exchanges with one partner");
-    constexpr int M = GRP_M, NG = (KS + M - 1) / M, CW = 32 / NS;
-    f32x2 yy[NG * M][1], e[NG][M][1], A[NG][M][1];
+    constexpr GrpLayout L = grp_layout(KS);
+    constexpr int NG = L.NG, MX = L.MHI, CW = 32 / NS;
+    static_assert(NG <= 3, "the packed form serves KS <= 12");
+    f32x2 y1[KS][1], e[NG][MX][1], A[NG][MX][1];
 #pragma unroll
-    for (int i = 0; i < NG * M; ++i) yy[i][0] = i < KS ? y[i < KS ? i : 0] : pad2;
+    for (int i = 0; i < KS; ++i) y1[i][0] = y[i];
+    grp2_esp<KS, 0>(y1, e[0]);
+    if constexpr (NG > 1) grp2_esp<KS, (NG > 1 ? 1 : 0)>(y1, e[NG > 1 ? 1 : 0]);
+    if constexpr (NG > 2) grp2_esp<KS, (NG > 2 ? 2 : 0)>(y1, e[NG > 2 ? 2 : 0]);
 #pragma unroll
-    for (int gq = 0; gq < NG; ++gq) {
-        esp_f2<M, 1>(&yy[gq * M], e[gq]);
+    for (int gq = 0; gq < NG; ++gq)
 #pragma unroll
-        for (int j = 0; j < M; ++j) A[gq][j][0] = 0ull;
-    }
+        for (int j = 0; j < MX; ++j) A[gq][j][0] = 0ull;
     const float *r = tab;
     for (int p = 0; p < n_real; ++p, r += ROWG) {                    // self-conjugate points
         f32x2 q[NG], pre[NG];
 #pragma unroll
         for (int gq = 0; gq < NG; ++gq) {
-            f32x2 sacc = bcf(r[0]);
+            const int Mg = grp_size(L, gq), co = gq < L.NHI ? 0 : ROWG_LO;
+            f32x2 sacc = bcf(r[co]);
 #pragma unroll
-            for (int j = 0; j < M; ++j) sacc = fma2(bcf(r[2 * j + 2]), e[gq][j][0], sacc);
+            for (int j = 0; j < MX; ++j)
+                if (j < Mg) sacc = fma2(bcf(r[co + 2 * j + 2]), e[gq][j][0], sacc);
             q[gq] = sacc;
         }
         f32x2 run = q[0];
 #pragma unroll
         for (int gq = 1; gq < NG; ++gq) { pre[gq] = run; run = mul2(run, q[gq]); }
         const f32x2 oth = shfl2(mask, run, CW);
-        f32x2 suf = mul2(bcf(r[2 * M + 2]), oth);
+        f32x2 suf = mul2(bcf(r[ROWG_W]), oth);
         fe = fma2(suf, run, fe);
         if (GRAD) {
 #pragma unroll
             for (int gq = NG - 1; gq >= 0; --gq) {
+                const int Mg = grp_size(L, gq), co = gq < L.NHI ? 0 : ROWG_LO;
                 const f32x2 t = gq > 0 ? mul2(pre[gq], suf) : suf;
 #pragma unroll
-                for (int j = 0; j < M; ++j) A[gq][j][0] = fma2(bcf(r[2 * j + 2]), t, A[gq][j][0]);
+                for (int j = 0; j < MX; ++j)
+                    if (j < Mg) A[gq][j][0] = fma2(bcf(r[co + 2 * j + 2]), t, A[gq][j][0]);
                 if (gq > 0) suf = mul2(suf, q[gq]);
             }
         }
@@ -354,9 +417,11 @@ __device__ __forceinline__ void eval_points_grp2(unsigned mask, const f32x2 (&y)
         f32x2 qr[NG], qi[NG], nqi[NG], pr[NG], pi[NG];
 #pragma unroll
         for (int gq = 0; gq < NG; ++gq) {
-            f32x2 sr = bcf(r[0]), si = bcf(r[1]);
+            const int Mg = grp_size(L, gq), co = gq < L.NHI ? 0 : ROWG_LO;
+            f32x2 sr = bcf(r[co]), si = bcf(r[co + 1]);
 #pragma unroll
-            for (int j = 0; j < M; ++j) { sr = fma2(bcf(r[2 * j + 2]), e[gq][j][0], sr); si = fma2(bcf(r[2 * j + 3]), e[gq][j][0], si); }
+            for (int j = 0; j < MX; ++j)
+                if (j < Mg) { sr = fma2(bcf(r[co + 2 * j + 2]), e[gq][j][0], sr); si = fma2(bcf(r[co + 2 * j + 3]), e[gq][j][0], si); }
             qr[gq] = sr; qi[gq] = si; nqi[gq] = si ^ SGN2;
         }
         f32x2 rr = qr[0], ri = qi[0];
@@ -368,23 +433,25 @@ __device__ __forceinline__ void eval_points_grp2(unsigned mask, const f32x2 (&y)
             rr = nr; ri = ni;
         }
         const f32x2 orr = shfl2(mask, rr, CW), oi = shfl2(mask, ri, CW);
-        const float wr = r[2 * M + 2], wi = r[2 * M + 3];
+        const float wr = r[ROWG_W], wi = r[ROWG_W + 1];
         f32x2 sr = fma2(bcf(wr), orr, mul2(bcf(-wi), oi)), si = fma2(bcf(wr), oi, mul2(bcf(wi), orr));   // suffix seeded with w x other
         fe = fma2(sr, rr, fe);
         fe = fma2(si ^ SGN2, ri, fe);                                 // Re(w other P_lane)
         if (GRAD) {
 #pragma unroll
             for (int gq = NG - 1; gq >= 0; --gq) {
+                const int Mg = grp_size(L, gq), co = gq < L.NHI ? 0 : ROWG_LO;
                 f32x2 tr = sr, nti = si ^ SGN2;
                 if (gq > 0) {
                     tr = fma2(pr[gq], sr, mul2(pi[gq], si ^ SGN2));   // Re: pr sr - pi si
                     nti = fma2(pr[gq], si, mul2(pi[gq], sr)) ^ SGN2;  // -Im
                 }
 #pragma unroll
-                for (int j = 0; j < M; ++j) {
-                    A[gq][j][0] = fma2(bcf(r[2 * j + 2]), tr, A[gq][j][0]);
-                    A[gq][j][0] = fma2(bcf(r[2 * j + 3]), nti, A[gq][j][0]);          // Re(c_j T)
-                }
+                for (int j = 0; j < MX; ++j)
+                    if (j < Mg) {
+                        A[gq][j][0] = fma2(bcf(r[co + 2 * j + 2]), tr, A[gq][j][0]);
+                        A[gq][j][0] = fma2(bcf(r[co + 2 * j + 3]), nti, A[gq][j][0]);     // Re(c_j T)
+                    }
                 if (gq > 0) {
                     const f32x2 nr = fma2(sr, qr[gq], mul2(si, nqi[gq]));
                     const f32x2 ni = fma2(sr, qi[gq], mul2(si, qr[gq]));
@@ -394,13 +461,14 @@ __device__ __forceinline__ void eval_points_grp2(unsigned mask, const f32x2 (&y)
         }
     }
     if (GRAD) {
-        f32x2 gg[NG * M][1];
+        f32x2 g1[KS][1];
 #pragma unroll
-        for (int i = 0; i < NG * M; ++i) gg[i][0] = 0ull;
+        for (int i = 0; i < KS; ++i) g1[i][0] = 0ull;
+        grp2_loo<KS, 0>(y1, A[0], g1);
+        if constexpr (NG > 1) grp2_loo<KS, (NG > 1 ? 1 : 0)>(y1, A[NG > 1 ? 1 : 0], g1);
+        if constexpr (NG > 2) grp2_loo<KS, (NG > 2 ? 2 : 0)>(y1, A[NG > 2 ? 2 : 0], g1);
 #pragma unroll
-        for (int gq = 0; gq < NG; ++gq) loo_f2<M, 1>(&yy[gq * M], A[gq], &gg[gq * M]);
-#pragma unroll
-        for (int i = 0; i < KS; ++i) g[i] = gg[i][0];
+        for (int i = 0; i < KS; ++i) g[i] = g1[i][0];
     }
 }
 
@@ -442,7 +510,7 @@ __device__ __forceinline__ void run_item_split2(const EvalParams<float> &p, unsi
             }
         }
 #endif
-        eval_points_grp2<KS, NS, GRAD>(mask, y, pad2, s_tab, n_real, n_cplx, fe, g);
+        eval_points_grp2<KS, NS, GRAD>(mask, y, s_tab, n_real, n_cplx, fe, g);
         if (GRAD) {
 #pragma unroll
             for (int i = 0; i < KS; ++i) {

@@ -879,7 +879,7 @@ def test_several_partial_assignments(dtype):
 def test_step_paths_agree(dtype):
     """The same 40 steps through the three loop forms (k <= 8, a partial assignment, B = 80: a ragged last CTA):
     identical discrete outputs, X within rounding (RED / atomic order), F_pre and the pinned flag included."""
-    base = I.make_mixed(n=40, m=170, kmin=1, kmax=8, seed=171, batch=80, with_fixed=True)
+    base = I.make_mixed(n=40, m=170, kmin=2, kmax=8, seed=171, batch=80, with_fixed=True)   # k >= 2: every constraint satisfiable
     base.meta["admissible"] = [R.admissible_taus(int(t), int(k), int(p)) or [0]
                                for t, k, p in zip(base.ctype, base.lengths(), base.param)]
     inst, hidden = I.plant_solution(base, seed=5)
