@@ -45,6 +45,7 @@ struct ClassGeom {              // how one length class maps candidates onto a C
     int cw = 32;                // candidates per warp (32 V; 32 V / NS in the lane-split kernels)
     int warps = CTA_WARPS;      // warps per CTA
     int Wc = 1, Wk = CTA_WARPS; // candidate sub-tiles x constraint groups
+    int cs = 1;                 // constraints a warp walks at once (k_eval_f2m: 32 / cs lanes each)
 };
 
 // One partial assignment and the constraint table it leaves: literals of fixed variables are gone,
@@ -200,8 +201,8 @@ void (*pick_kernel(int cls, bool grad))(EvalParams<T>)
         switch (cls) {
         case CLS_S: return grad ? (Fn)k_eval_f2m<1, AFSAT_S_KMAX, 2, true, 2> : (Fn)k_eval_f2m<1, AFSAT_S_KMAX, 2, false, 2>;
         case CLS_A: return grad ? (Fn)k_eval_f2m<AFSAT_S_KMAX + 1, AFSAT_A_KMAX, 1, true, 2> : (Fn)k_eval_f2m<AFSAT_S_KMAX + 1, AFSAT_A_KMAX, 1, false, 2>;
-        case CLS_B: return grad ? (Fn)k_eval_split<float, AFSAT_A_KMAX + 1, AFSAT_B_KMAX, 2, 2, true, AFSAT_M32_THREADS, 1>
-                                : (Fn)k_eval_split<float, AFSAT_A_KMAX + 1, AFSAT_B_KMAX, 2, 2, false, AFSAT_M32_THREADS, 1>;
+        case CLS_B: return grad ? (Fn)k_eval_split<float, AFSAT_A_KMAX + 1, AFSAT_B_KMAX, 2, 2, true, AFSAT_M32_THREADS, AFSAT_M32_MINB>
+                                : (Fn)k_eval_split<float, AFSAT_A_KMAX + 1, AFSAT_B_KMAX, 2, 2, false, AFSAT_M32_THREADS, AFSAT_M32_MINB>;
         default:    return grad ? (Fn)k_eval_split<float, AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, 1, true, AFSAT_L32_THREADS, AFSAT_L32_MINB>
                                 : (Fn)k_eval_split<float, AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, 1, false, AFSAT_L32_THREADS, AFSAT_L32_MINB>;
         }
@@ -252,7 +253,7 @@ int launch_eval(afsat_ctx *ctx, const GroupPlan &gp, const T *x, T *G, int64_t g
         const ClassGeom &g = ctx->geom[cls];
         p.items = gp.d_items + gp.cls_begin[cls];
         p.frow_base = gp.cls_begin[cls];
-        p.Wc = g.Wc; p.Wk = g.Wk;
+        p.Wc = g.Wc; p.Wk = g.Wk; p.cs = g.cs;
         const int64_t per_cta = (int64_t)g.cw * g.Wc;
         dim3 block(32 * g.warps), grid(nit, (unsigned)((width + per_cta - 1) / per_cta));
         pick_kernel<T>(cls, grad)<<<grid, block, 0, st>>>(p);
@@ -368,7 +369,7 @@ int launch_update(afsat_ctx *ctx, const GroupPlan &gp, T *x, T *G, int64_t g_ld,
     const unsigned gx = (unsigned)((w / VW + tpr - 1) / tpr);
     const int rpp = CTA_THREADS / tpr;
     const unsigned gy = (unsigned)std::max<int64_t>(1, std::min<int64_t>((ctx->n + rpp * UPD_UNROLL - 1) / (rpp * UPD_UNROLL),
-                                                                           (int64_t)ctx->sm_count * 8 / gx));
+                                                                           (int64_t)ctx->sm_count * AFSAT_UPD_CTAS_PER_SM / gx));
     const size_t gi = &gp - ctx->groups.data();
     ProfScope prof(ctx, st, 1);
     k_update<T><<<dim3(gx, gy), CTA_THREADS, 0, st>>>(x, G, g_ld, g_b0, ctx->d_fixed + gi * (size_t)ctx->n, sol, ctx->d_bits, (T)eta,
@@ -898,7 +899,13 @@ int afsat_create_ex(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64
     const int64_t span = G > 1 ? group_w : ldb;                        // columns a tile sequence has to cover
     int64_t tile_w = span;
     {
-        const int64_t budget = opt.l2_budget_bytes > 0 ? opt.l2_budget_bytes : l2_bytes / 16 * 13;   // X and G tiles: 13/16 of L2
+        // X and G tiles: 13/16 of L2 (cfg4: 128 candidates, 102 MB).  Measured with ncu (profiles/r2_traffic_cfg4.md): at that
+        // width the tiles do NOT stay resident -- 44 GB of DRAM traffic per step where X once is 6.6 GB (the L2 is two halves,
+        // one per die, and lines touched from both dies occupy both) -- while tiles of 64 candidates do (12 GB); yet 128 is
+        // the faster width, 20.3 against 21.9 ms per step: the evaluation of such short constraints is bound by L2
+        // THROUGHPUT (2.8 GB of gathers, REDs and inter-die traffic per tile, 10.7 of the ~12.4 TB/s the L2 delivers), the
+        // DRAM traffic hides under it, and the wider tile halves the per-CTA staging of the literal lists.
+        const int64_t budget = opt.l2_budget_bytes > 0 ? opt.l2_budget_bytes : l2_bytes / 16 * 13;
         const int64_t per_col = (int64_t)2 * n_vars * (int64_t)esz;
         // a working set within a few budgets is better left whole: the L2 misses hide behind the arithmetic, the small
         // grids of the tiles do not (cfg2 fp32, 1.58 x: 1.23 ms un-tiled vs 1.31; cfg2 fp64, 3.15 x: 2.75 vs 3.13;
@@ -919,6 +926,8 @@ int afsat_create_ex(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64
         g.V = (cls == CLS_S) ? 4 : (cls == CLS_A && dtype == 32) ? 2 : 1;
         g.warps = CTA_WARPS;
         g.cw = 32 * g.V;
+        if (dtype == 32 && (cls == CLS_S || cls == CLS_A))             // packed kernel: a tile narrower than a warp's candidates
+            while (g.cs < 4 && g.cw / 2 >= tile_w && g.cw / 2 >= 32) { g.cs *= 2; g.cw /= 2; }   // -> several constraints per warp
         if (cls == CLS_B && dtype == 32) { g.warps = AFSAT_M32_THREADS / 32; g.cw = 32; }                 // 2 lanes x 2 candidates
         else if (cls == CLS_LONG && dtype == 32) { g.warps = AFSAT_L32_THREADS / 32; g.cw = 32 / AFSAT_L32_NS; }
         else if (cls == CLS_LONG) { g.warps = AFSAT_L64_THREADS / 32; g.cw = 8; }                         // fp64: four lanes per candidate
@@ -983,7 +992,7 @@ int afsat_create_ex(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64
             const int64_t chunks_wanted = std::max<int64_t>(1, (int64_t)sm_count * 16 / tiles_y);
             const int64_t cost_budget = std::max<int64_t>(1, gp.fp_instr / chunks_wanted);
             const int64_t cost1 = std::max<int64_t>(1, sig_cost[sg]);
-            int64_t chunk = std::max<int64_t>(cg.Wk, (cost_budget + cost1 - 1) / cost1);
+            int64_t chunk = std::max<int64_t>((int64_t)cg.Wk * cg.cs, (cost_budget + cost1 - 1) / cost1);
             chunk = std::min<int64_t>(chunk, LIT_CHUNK / k);
             chunk = std::max<int64_t>(1, chunk);
             for (int32_t s0 = j; s0 < e; s0 += (int32_t)chunk) {

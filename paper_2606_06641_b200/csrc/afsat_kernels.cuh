@@ -77,6 +77,7 @@ struct EvalParams {
     int64_t ldb;
     int64_t b_begin, b_end;     // candidate tile of this launch (b_end <= ldb)
     int32_t Wc, Wk;             // warps of a CTA: Wc candidate sub-tiles x Wk constraint groups
+    int32_t cs;                 // k_eval_f2m: a warp's lanes take cs (1, 2 or 4) constraints at once, 32 / cs lanes each
     const uint8_t *skip;        // [ldb] or null: candidates with skip[b] != 0 are not evaluated (line search)
 };
 
@@ -799,12 +800,12 @@ template <> struct PairIO<2> {
 template <int K, int NP, bool GRAD, bool PF, int UV>
 __device__ __forceinline__ void run_item_f2(const EvalParams<float> &p, const int32_t *__restrict__ s_lits,
                                             const f32x2 *__restrict__ s_tab2, const float *__restrict__ s_tabg, int n_real,
-                                            int n_cplx, int nc, int wk, int64_t b, f32x2 (&fe)[NP])
+                                            int n_cplx, int nc, int wk, int Wk, int64_t b, f32x2 (&fe)[NP])
 {
+    // wk / Wk: first constraint of this lane and the stride (lanes of a warp may walk different constraints, EvalParams::cs)
     const char *xb = reinterpret_cast<const char *>(p.x + b);
     char *gb = reinterpret_cast<char *>(p.G + (b - p.g_b0));
     const uint32_t x_ld = (uint32_t)(p.ldb * 4), g_ld = (uint32_t)(p.g_ld * 4);
-    const int Wk = p.Wk;
     int32_t lit_n[K];
     f32x2 y_n[K][NP];
     auto fetch = [&](int c) {
@@ -851,21 +852,38 @@ __device__ __noinline__ void item_body_f2(const EvalParams<float> &p, const int3
     constexpr int V = 2 * NP;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int wc = warp % p.Wc, wk = warp / p.Wc;
-    const int64_t b = p.b_begin + ((int64_t)blockIdx.y * p.Wc + wc) * (32 * V) + lane * V;
+    // the warp's lanes take cs constraints at once (a narrow candidate tile still fills the warp: cfg4's tile of 64
+    // candidates is 16 lanes x 4 candidates; the per-constraint instructions are issued once for both constraints)
+    const int lpc = 32 / p.cs, sub = lane / lpc, ll = lane % lpc;
+    const int64_t b = p.b_begin + ((int64_t)blockIdx.y * p.Wc + wc) * (lpc * V) + ll * V;
     const bool active = b < p.b_end && b < p.B && !lane_skipped(p, b, V);   // this launch owns [b_begin, b_end)
     f32x2 fe2[NP];
 #pragma unroll
     for (int q = 0; q < NP; ++q) fe2[q] = 0ull;
     if (active) {
         constexpr bool PF = K <= 5;
-        if (uv == 1) run_item_f2<K, NP, GRAD, PF, 1>(p, s_lits, s_tab2, s_tabg, n_real, n_cplx, nc, wk, b, fe2);
-        else if (uv == 2) run_item_f2<K, NP, GRAD, PF, 2>(p, s_lits, s_tab2, s_tabg, n_real, n_cplx, nc, wk, b, fe2);
-        else run_item_f2<K, NP, GRAD, PF, 0>(p, s_lits, s_tab2, s_tabg, n_real, n_cplx, nc, wk, b, fe2);
+        const int c0 = wk * p.cs + sub, cstep = p.Wk * p.cs;
+        if (uv == 1) run_item_f2<K, NP, GRAD, PF, 1>(p, s_lits, s_tab2, s_tabg, n_real, n_cplx, nc, c0, cstep, b, fe2);
+        else if (uv == 2) run_item_f2<K, NP, GRAD, PF, 2>(p, s_lits, s_tab2, s_tabg, n_real, n_cplx, nc, c0, cstep, b, fe2);
+        else run_item_f2<K, NP, GRAD, PF, 0>(p, s_lits, s_tab2, s_tabg, n_real, n_cplx, nc, c0, cstep, b, fe2);
     }
+    if (!p.Fpart) return;
+    // partial objectives: fixed-order sum over the Wk warp groups and the cs lane groups that hold the same candidates
     float fe[V];
 #pragma unroll
     for (int q = 0; q < NP; ++q) upk(fe2[q], fe[2 * q], fe[2 * q + 1]);
-    store_item_F<float, V>(p, s_F, fe, warp, lane, wk, b, active);
+#pragma unroll
+    for (int v = 0; v < V; ++v) s_F[warp][lane * V + v] = fe[v];
+    __syncthreads();
+    if (wk == 0 && sub == 0 && active) {
+#pragma unroll
+        for (int v = 0; v < V; ++v) {
+            float sacc = 0.f;
+            for (int g = 0; g < p.Wk; ++g)
+                for (int u = 0; u < p.cs; ++u) sacc += s_F[warp + g * p.Wc][(u * lpc + ll) * V + v];
+            if (b + v < p.B) p.Fpart[(int64_t)(p.frow_base + blockIdx.x) * p.ldb + b + v] = sacc;
+        }
+    }
 }
 
 template <int K, int KHI, int NP, bool GRAD>

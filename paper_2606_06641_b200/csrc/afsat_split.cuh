@@ -35,7 +35,10 @@ namespace afsat {
 #define AFSAT_L32_MINB 1
 #endif
 #ifndef AFSAT_M32_THREADS
-#define AFSAT_M32_THREADS 384
+#define AFSAT_M32_THREADS 256             // packed form, k <= 20: 2 CTAs x 8 warps at 128 registers (cfg2: 0.621 ms / step against
+#endif                                    // 0.651 with 384 threads x 168 registers and 0.637 with 512 x 128)
+#ifndef AFSAT_M32_MINB
+#define AFSAT_M32_MINB 2
 #endif
 #ifndef AFSAT_L64_THREADS
 #define AFSAT_L64_THREADS 384
@@ -52,7 +55,7 @@ namespace afsat {
 // Staged row of a point: {Re, Im of c_0 .. c_MHI for groups of MHI | the same for groups of MLO (from scalar ROWG_LO) |
 // Re w, Im w (at ROWG_W)},  c_j = a^(M-j) b^j.
 constexpr int GRP_MAX = 4;
-constexpr int ROWG_LO = 2 * (GRP_MAX + 1), ROWG_W = 4 * (GRP_MAX + 1), ROWG = ROWG_W + 2;
+constexpr int ROWG_LO = 2 * (GRP_MAX + 1), ROWG_W = 4 * (GRP_MAX + 1), ROWG = ROWG_W + 4;   // 24: rows are whole 16-byte vectors
 struct GrpLayout { int NG, MLO, NHI, MHI; };
 __host__ __device__ constexpr GrpLayout grp_layout(int KS)
 {
@@ -93,6 +96,20 @@ inline int pack_rows_grp(const double *r0, int n_rows, int k, int ns, double *ou
         o[ROWG_W] = r[4] * scw; o[ROWG_W + 1] = r[5] * scw;
     }
     return std_tab ? 0 : 1;
+}
+
+// one staged row into registers with 16-byte shared-memory loads (the row is warp-uniform: broadcast)
+__device__ __forceinline__ void load_row(const float *__restrict__ r, float (&v)[ROWG])
+{
+    const float4 *r4 = reinterpret_cast<const float4 *>(r);
+#pragma unroll
+    for (int i = 0; i < ROWG / 4; ++i) { const float4 t = r4[i]; v[4 * i] = t.x; v[4 * i + 1] = t.y; v[4 * i + 2] = t.z; v[4 * i + 3] = t.w; }
+}
+__device__ __forceinline__ void load_row(const double *__restrict__ r, double (&v)[ROWG])
+{
+    const double2 *r2 = reinterpret_cast<const double2 *>(r);
+#pragma unroll
+    for (int i = 0; i < ROWG / 2; ++i) { const double2 t = r2[i]; v[2 * i] = t.x; v[2 * i + 1] = t.y; }
 }
 
 // product of the OTHER lanes' values (NS = 2: the partner's; NS = 4: butterfly over lane bits log2(CW), log2(CW) + 1)
@@ -145,10 +162,11 @@ __device__ __forceinline__ void eval_points_grp(unsigned mask, const T (&y)[KS],
     }
     const T *r = tab;
     for (int p = 0; p < n_real; ++p, r += ROWG) {                    // self-conjugate points
-        T ch[MX + 1], cl[MX + 1];
+        T rv[ROWG], ch[MX + 1], cl[MX + 1];
+        load_row(r, rv);
 #pragma unroll
-        for (int j = 0; j <= MX; ++j) { ch[j] = r[2 * j]; cl[j] = r[ROWG_LO + 2 * j]; }
-        const T w = r[ROWG_W];
+        for (int j = 0; j <= MX; ++j) { ch[j] = rv[2 * j]; cl[j] = rv[ROWG_LO + 2 * j]; }
+        const T w = rv[ROWG_W];
         T q[NG], pre[NG];
 #pragma unroll
         for (int gq = 0; gq < NG; ++gq) {
@@ -180,13 +198,14 @@ __device__ __forceinline__ void eval_points_grp(unsigned mask, const T (&y)[KS],
         }
     }
     for (int p = 0; p < n_cplx; ++p, r += ROWG) {                    // one of each conjugate pair
-        T chr[MX + 1], chi[MX + 1], clr[MX + 1], cli[MX + 1];
+        T rv[ROWG], chr[MX + 1], chi[MX + 1], clr[MX + 1], cli[MX + 1];
+        load_row(r, rv);
 #pragma unroll
         for (int j = 0; j <= MX; ++j) {
-            chr[j] = r[2 * j]; chi[j] = r[2 * j + 1];
-            clr[j] = r[ROWG_LO + 2 * j]; cli[j] = r[ROWG_LO + 2 * j + 1];
+            chr[j] = rv[2 * j]; chi[j] = rv[2 * j + 1];
+            clr[j] = rv[ROWG_LO + 2 * j]; cli[j] = rv[ROWG_LO + 2 * j + 1];
         }
-        const T wr = r[ROWG_W], wi = r[ROWG_W + 1];
+        const T wr = rv[ROWG_W], wi = rv[ROWG_W + 1];
         T qr[NG], qi[NG], pr[NG], pi[NG];
 #pragma unroll
         for (int gq = 0; gq < NG; ++gq) {
@@ -383,8 +402,9 @@ __device__ __forceinline__ void eval_points_grp2(unsigned mask, const f32x2 (&y)
     for (int gq = 0; gq < NG; ++gq)
 #pragma unroll
         for (int j = 0; j < MX; ++j) A[gq][j][0] = 0ull;
-    const float *r = tab;
-    for (int p = 0; p < n_real; ++p, r += ROWG) {                    // self-conjugate points
+    for (int p = 0; p < n_real; ++p, tab += ROWG) {                  // self-conjugate points
+        float r[ROWG];
+        load_row(tab, r);
         f32x2 q[NG], pre[NG];
 #pragma unroll
         for (int gq = 0; gq < NG; ++gq) {
@@ -413,7 +433,9 @@ __device__ __forceinline__ void eval_points_grp2(unsigned mask, const f32x2 (&y)
             }
         }
     }
-    for (int p = 0; p < n_cplx; ++p, r += ROWG) {                    // one of each conjugate pair
+    for (int p = 0; p < n_cplx; ++p, tab += ROWG) {                  // one of each conjugate pair
+        float r[ROWG];
+        load_row(tab, r);
         f32x2 qr[NG], qi[NG], nqi[NG], pr[NG], pi[NG];
 #pragma unroll
         for (int gq = 0; gq < NG; ++gq) {
@@ -589,8 +611,8 @@ extern template __global__ void k_eval_split<float, AFSAT_L32_KMIN, AFSAT_MAX_LE
 extern template __global__ void k_eval_split<float, AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, 1, false, AFSAT_L32_THREADS, AFSAT_L32_MINB>(const EvalParams<float>);
 extern template __global__ void k_eval_split<double, AFSAT_L64_KMIN, AFSAT_MAX_LEN, 4, 1, true, AFSAT_L64_THREADS, 1>(const EvalParams<double>);
 extern template __global__ void k_eval_split<double, AFSAT_L64_KMIN, AFSAT_MAX_LEN, 4, 1, false, AFSAT_L64_THREADS, 1>(const EvalParams<double>);
-extern template __global__ void k_eval_split<float, AFSAT_A_KMAX + 1, AFSAT_B_KMAX, 2, 2, true, AFSAT_M32_THREADS, 1>(const EvalParams<float>);
-extern template __global__ void k_eval_split<float, AFSAT_A_KMAX + 1, AFSAT_B_KMAX, 2, 2, false, AFSAT_M32_THREADS, 1>(const EvalParams<float>);
+extern template __global__ void k_eval_split<float, AFSAT_A_KMAX + 1, AFSAT_B_KMAX, 2, 2, true, AFSAT_M32_THREADS, AFSAT_M32_MINB>(const EvalParams<float>);
+extern template __global__ void k_eval_split<float, AFSAT_A_KMAX + 1, AFSAT_B_KMAX, 2, 2, false, AFSAT_M32_THREADS, AFSAT_M32_MINB>(const EvalParams<float>);
 #endif
 
 }  // namespace afsat

@@ -26,7 +26,15 @@ __global__ void __launch_bounds__(CTA_THREADS) k_pack_signs(const T *__restrict_
 // candidates (one 16-byte load / store per array and row), tpr threads span a row of the tile, a CTA pass covers
 // CTA_THREADS / tpr rows and every thread keeps UPD_UNROLL rows in flight.  The sign bits of a 32-candidate word come
 // from the 32 / VW lanes that hold it (one REDUX.OR).
-constexpr int UPD_UNROLL = 4;
+// rows in flight per thread / CTAs per SM of k_update (cfg4, ms of update per step: 4 / 8: 2.52, 8 / 8: 3.10, 8 / 4: 2.92,
+// 1 / 64: 2.47, 2 / 16: 2.28)
+#ifndef AFSAT_UPD_UNROLL
+#define AFSAT_UPD_UNROLL 2
+#endif
+#ifndef AFSAT_UPD_CTAS_PER_SM
+#define AFSAT_UPD_CTAS_PER_SM 16
+#endif
+constexpr int UPD_UNROLL = AFSAT_UPD_UNROLL;
 template <typename T> struct Vec16;
 template <> struct Vec16<float>  { typedef float4 type;  static constexpr int VW = 4; };
 template <> struct Vec16<double> { typedef double2 type; static constexpr int VW = 2; };
