@@ -409,6 +409,27 @@ def measure(cfg, dtype, K, W, *, batch=None, scale=1.0, oracle_seconds=10.0, ran
     return out
 
 
+LTS_BYTES_PER_CLK = 6300.0       # B300_MICROARCH.md "LTS throughput cap ~6300 B/cyc full-chip": the L2's delivery rate
+
+
+def l2_report(inst, ctx, B, kern_ms_per_step, cap):
+    """Second roofline of the evaluation kernels: L2 throughput.  Algorithmic bytes = 4 B gathered + 4 B scatter-added per
+    literal and candidate on the table the kernels run (after substitution).  cfg4 (k = 3..5) is bound
+    here, not by the FP32 pipe: ~23 flop per byte of L2 traffic at k = 4."""
+    from paper_2606_06641_b200 import binding as Bd
+    peaks = load_peaks()
+    alg = 8.0 * ctx.query(Bd.Q_LIVE_NNZ) * B
+    cap_gbs = LTS_BYTES_PER_CLK * peaks["sm_max_mhz"] * 1e6 / 1e9
+    out = {"algorithmic_bytes_per_step": alg, "achieved_gbs": alg / (kern_ms_per_step * 1e-3) / 1e9 if kern_ms_per_step > 0 else 0.0,
+           "peak_gbs": cap_gbs, "peak_source": "guide: ~6300 B/clk full-chip LTS cap (B300_MICROARCH.md) x sm_max_mhz; not measured here",
+           "lts_bytes_per_step_measured": cap.get("lts_bytes_per_step_eval_kernels")}
+    out["frac"] = out["achieved_gbs"] / cap_gbs
+    if cap.get("lts_bytes_per_step_eval_kernels") and kern_ms_per_step > 0:
+        out["measured_traffic_gbs"] = cap["lts_bytes_per_step_eval_kernels"] / (kern_ms_per_step * 1e-3) / 1e9
+        out["measured_traffic_frac_of_peak"] = out["measured_traffic_gbs"] / cap_gbs
+    return out
+
+
 def report(r, world, local, oracle_seconds, rank0_oracle=True):
     """The JSON-able report of one measurement (rank 0)."""
     import torch
@@ -439,8 +460,9 @@ def report(r, world, local, oracle_seconds, rank0_oracle=True):
                               "how": "afsat_probe_peak: 8 independent FMA chains per thread, CUDA events, best of 5"},
             "model_instr_over_issue_peak": (instr_c * B / (kern_ms * 1e-3 / K)) / (sm * FP32_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6)
             if kern_ms > 0 else 0.0,
-            "measured_pipe_utilisation": {k_: cap.get(k_) for k_ in ("sm__pipe_fma_cycles_active_pct", "smsp__issue_active_pct",
-                                                                      "sm__inst_executed_pipe_fma_per_eval", "capture")} if cap else None,
+            "measured_pipe_utilisation": {k_: cap.get(k_) for k_ in ("kernel", "sm__pipe_fma_cycles_active_pct",
+                                                                      "sm__pipe_fp64_cycles_active_pct", "smsp__issue_active_pct",
+                                                                      "executed_warp_instructions_per_launch", "capture")} if cap else None,
             "kernel_ms_per_step": kern_ms / K, "kernel_launches_per_step": max(1, r["kern_launches"] // K) if r["kern_launches"] else 0,
             "kernel_share_of_step": (kern_ms / K) / (1e3 * r["t_total"] / K),
             "update_ms_per_step": r["upd_ms"] / K, "count_ms_per_step": r["chk_ms"] / K,
@@ -449,6 +471,8 @@ def report(r, world, local, oracle_seconds, rank0_oracle=True):
             "frac_after_substitution": (flop_sub * B / (kern_ms * 1e-3 / K) / 1e12) / peak_tf if kern_ms > 0 else 0.0,
             "traffic": cap.get("dram_bytes_per_step_eval_kernels"),
             "traffic_whole_step": cap.get("dram_bytes_per_step"),
+            "traffic_source": cap.get("traffic_capture"),
+            "l2": l2_report(inst, ctx, B, kern_ms / K, cap),
             "hbm_floor_bytes_per_step": 2 * n * B * esz, "hbm_peak_gbs": peaks["hbm_gbs"],
             "note": "achieved = ALGORITHMIC flop of the instance as given (SURVEY.md App. D: 12 / 4 FP32 instructions per literal at a "
                     "complex / real DFT point, every retained point) / measured kernel time.  The kernels execute fewer instructions: "
@@ -578,7 +602,7 @@ def run_ours(args):
                                                                       "frac_of_fp64_peak", "model_instr_over_issue_peak",
                                                                       "kernel_ms_per_step", "kernel_share_of_step",
                                                                       "update_ms_per_step", "count_ms_per_step",
-                                                                      "measured_pipe_utilisation", "traffic", "note_small")}
+                                                                      "measured_pipe_utilisation", "traffic", "l2", "note_small")}
             if c == 3 and dt == 32:
                 # BASELINE.json configs[3]: "run in both fp32 and fp64 and report deviation vs oracle" -- also for the paper's
                 # own product form in fp32 (AFSAT_FLAG_PAPER), which the default context replaces beyond k = 20

@@ -132,16 +132,78 @@ constexpr int CHK_MLP = 8;
 enum { CHK_GENERAL = 0, CHK_OR = 1 /* tau >= 1 */, CHK_NONE = 2 /* tau == 0 */, CHK_ALL = 3 /* tau == k */,
        CHK_NAND = 4 /* tau < k */, CHK_NAE = 5 /* 0 < tau < k */, CHK_EQ = 6 /* tau in {0, k} */, CHK_ODD = 7, CHK_EVEN = 8 };
 
+// satisfied-mask of ONE constraint for the 32 candidates of a word.  bw: the word's column of the sign-bit array; the bit
+// rows of up to MLP literals are requested before any is consumed.
+template <int MLP>
+__device__ __forceinline__ uint32_t chk_constraint(const int32_t *__restrict__ L, int k, const uint32_t *__restrict__ bw, uint32_t ldw,
+                                                   int kind, int nb, uint64_t scan_lo, uint64_t scan_hi, int scan_is_sat)
+{
+    if (kind != CHK_GENERAL) {
+        // predicates that are a function of (any literal true, all literals true, parity): no counting at all
+        uint32_t any = 0u, all = 0xffffffffu, par = 0u;
+        for (int i0 = 0; i0 < k; i0 += MLP) {
+            uint32_t mm[MLP];
+#pragma unroll
+            for (int u = 0; u < MLP; ++u)
+                if (i0 + u < k) {
+                    const int32_t lit = L[i0 + u];
+                    const uint32_t w = __ldg(bw + (size_t)(uint32_t)(lit & LIT_VAR) * ldw);
+                    mm[u] = lit < 0 ? ~w : w;                         // literal true = variable true XOR negated
+                }
+#pragma unroll
+            for (int u = 0; u < MLP; ++u)
+                if (i0 + u < k) { any |= mm[u]; all &= mm[u]; par ^= mm[u]; }
+        }
+        return kind == CHK_OR ? any : kind == CHK_NONE ? ~any : kind == CHK_ALL ? all : kind == CHK_NAND ? ~all
+             : kind == CHK_NAE ? (any & ~all) : kind == CHK_EQ ? (all | ~any) : kind == CHK_ODD ? par : ~par;
+    }
+    uint32_t t[7] = {0u, 0u, 0u, 0u, 0u, 0u, 0u};                     // tau, bit-sliced
+    for (int i0 = 0; i0 < k; i0 += MLP) {
+        uint32_t mm[MLP];
+#pragma unroll
+        for (int u = 0; u < MLP; ++u)
+            if (i0 + u < k) {
+                const int32_t lit = L[i0 + u];
+                const uint32_t w = __ldg(bw + (size_t)(uint32_t)(lit & LIT_VAR) * ldw);
+                mm[u] = lit < 0 ? ~w : w;
+            }
+#pragma unroll
+        for (int u = 0; u < MLP; ++u)
+            if (i0 + u < k) {
+                uint32_t m = mm[u];
+#pragma unroll
+                for (int j = 0; j < 7; ++j)
+                    if (j < nb) { const uint32_t sv = t[j] ^ m; m &= t[j]; t[j] = sv; }
+            }
+    }
+    uint32_t acc = 0u;
+    for (int tau = 0; tau <= k; ++tau) {
+        const uint64_t bit = tau < 64 ? (scan_lo >> tau) : (scan_hi >> (tau - 64));
+        if (!(bit & 1ull)) continue;
+        uint32_t eq = 0xffffffffu;
+#pragma unroll
+        for (int j = 0; j < 7; ++j)
+            if (j < nb) eq &= ((tau >> j) & 1) ? t[j] : ~t[j];
+        acc |= eq;
+    }
+    return scan_is_sat ? acc : ~acc;                                  // 1 = constraint satisfied
+}
+
 __global__ void __launch_bounds__(CTA_THREADS) k_check_bits(const CheckParams p)
 {
     __shared__ int32_t s_lits[LIT_CHUNK];
     __shared__ int32_t s_cnt[32 * 32];
     if (p.step_ctr && blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) ++p.step_ctr[0];
-    for (int i = threadIdx.x; i < p.wpb * 32; i += blockDim.x) s_cnt[i] = 0;
-    const int wi = threadIdx.x % p.wpb, grp = threadIdx.x / p.wpb, ngrp = blockDim.x / p.wpb;
-    const int word = p.w_begin + blockIdx.y * p.wpb + wi;
+    const int wpb = p.wpb, n_items = p.n_items;
+    const uint32_t ldw = (uint32_t)p.ldw;
+    for (int i = threadIdx.x; i < wpb * 32; i += blockDim.x) s_cnt[i] = 0;
+    const int wi = threadIdx.x % wpb, grp = threadIdx.x / wpb, ngrp = blockDim.x / wpb;
+    const int word = p.w_begin + blockIdx.y * wpb + wi;
     const bool valid = word < p.w_end;
     const uint32_t *bw = p.bits + (valid ? word : p.w_begin);
+    const Item *items = p.items;
+    const SigDev *sigs = p.sigs;
+    const int32_t *lits = p.lits;
     // satisfied constraints per candidate, bit-sliced, in two levels: a 3-plane counter takes 7 constraints, then it is
     // added into the 13-plane counter (a full 13-plane ripple per constraint was a third of this kernel's instructions)
     uint32_t cnt[13], lo[3] = {0u, 0u, 0u};
@@ -173,12 +235,13 @@ __global__ void __launch_bounds__(CTA_THREADS) k_check_bits(const CheckParams p)
         for (int j = 0; j < 13; ++j) cnt[j] = 0u;
         nacc = 0;
     };
-    for (int item = blockIdx.x; item < p.n_items; item += gridDim.x) {   // persistent over work items
-        const Item it = p.items[item];
-        const SigDev sg = p.sigs[it.sig];
-        const int k = it.k, nc = it.c_end - it.c_begin, kind = sg.chk_kind;
+    for (int item = blockIdx.x; item < n_items; item += gridDim.x) {  // persistent over work items
+        const Item it = items[item];
+        const SigDev sg = sigs[it.sig];
+        const int k = it.k, nc = it.c_end - it.c_begin, kind = sg.chk_kind, sis = sg.scan_is_sat;
+        const uint64_t slo = sg.scan_lo, shi = sg.scan_hi;
         __syncthreads();                                              // previous item's literals are consumed
-        for (int i = threadIdx.x; i < nc * k; i += blockDim.x) s_lits[i] = __ldg(p.lits + it.lit_base + i);
+        for (int i = threadIdx.x; i < nc * k; i += blockDim.x) s_lits[i] = __ldg(lits + it.lit_base + i);
         __syncthreads();
         if (!valid) continue;
         int nb = 1;
@@ -188,58 +251,8 @@ __global__ void __launch_bounds__(CTA_THREADS) k_check_bits(const CheckParams p)
         nacc += mine > 0 ? mine : 0;
         for (int c = grp; c < nc; c += ngrp) {
             const int32_t *L = s_lits + c * k;
-            uint32_t sat;
-            if (kind != CHK_GENERAL) {
-                // predicates that are a function of (any literal true, all literals true, parity): no counting at all
-                uint32_t any = 0u, all = 0xffffffffu, par = 0u;
-                for (int i0 = 0; i0 < k; i0 += CHK_MLP) {
-                    uint32_t mm[CHK_MLP];
-#pragma unroll
-                    for (int u = 0; u < CHK_MLP; ++u)
-                        if (i0 + u < k) {
-                            const int32_t lit = L[i0 + u];
-                            const uint32_t w = __ldg(bw + (int64_t)(lit & LIT_VAR) * p.ldw);
-                            mm[u] = lit < 0 ? ~w : w;                 // literal true = variable true XOR negated
-                        }
-#pragma unroll
-                    for (int u = 0; u < CHK_MLP; ++u)
-                        if (i0 + u < k) { any |= mm[u]; all &= mm[u]; par ^= mm[u]; }
-                }
-                sat = kind == CHK_OR ? any : kind == CHK_NONE ? ~any : kind == CHK_ALL ? all : kind == CHK_NAND ? ~all
-                    : kind == CHK_NAE ? (any & ~all) : kind == CHK_EQ ? (all | ~any) : kind == CHK_ODD ? par : ~par;
-            } else {
-                uint32_t t[7] = {0u, 0u, 0u, 0u, 0u, 0u, 0u};
-                for (int i0 = 0; i0 < k; i0 += CHK_MLP) {
-                    uint32_t mm[CHK_MLP];
-#pragma unroll
-                    for (int u = 0; u < CHK_MLP; ++u)
-                        if (i0 + u < k) {
-                            const int32_t lit = L[i0 + u];
-                            const uint32_t w = __ldg(bw + (int64_t)(lit & LIT_VAR) * p.ldw);
-                            mm[u] = lit < 0 ? ~w : w;
-                        }
-#pragma unroll
-                    for (int u = 0; u < CHK_MLP; ++u)
-                        if (i0 + u < k) {
-                            uint32_t m = mm[u];
-#pragma unroll
-                            for (int j = 0; j < 7; ++j)
-                                if (j < nb) { const uint32_t sv = t[j] ^ m; m &= t[j]; t[j] = sv; }
-                        }
-                }
-                uint32_t acc = 0u;
-                for (int tau = 0; tau <= k; ++tau) {
-                    const uint64_t bit = tau < 64 ? (sg.scan_lo >> tau) : (sg.scan_hi >> (tau - 64));
-                    if (!(bit & 1ull)) continue;
-                    uint32_t eq = 0xffffffffu;
-#pragma unroll
-                    for (int j = 0; j < 7; ++j)
-                        if (j < nb) eq &= ((tau >> j) & 1) ? t[j] : ~t[j];
-                    acc |= eq;
-                }
-                sat = sg.scan_is_sat ? acc : ~acc;                    // 1 = constraint satisfied
-            }
-            uint32_t carry = sat;
+            uint32_t carry = k <= 4 ? chk_constraint<4>(L, k, bw, ldw, kind, nb, slo, shi, sis)
+                                    : chk_constraint<8>(L, k, bw, ldw, kind, nb, slo, shi, sis);
 #pragma unroll
             for (int j = 0; j < 3; ++j) { const uint32_t sv = lo[j] ^ carry; carry &= lo[j]; lo[j] = sv; }
             if (++nlo == 7) fold();
@@ -247,8 +260,8 @@ __global__ void __launch_bounds__(CTA_THREADS) k_check_bits(const CheckParams p)
     }
     if (valid && nacc) flush();
     __syncthreads();
-    const int64_t b0 = ((int64_t)p.w_begin + (int64_t)blockIdx.y * p.wpb) * 32;
-    for (int i = threadIdx.x; i < p.wpb * 32; i += blockDim.x) {
+    const int64_t b0 = ((int64_t)p.w_begin + (int64_t)blockIdx.y * wpb) * 32;
+    for (int i = threadIdx.x; i < wpb * 32; i += blockDim.x) {
         const int64_t b = b0 + i;
         if (b < p.B && b < (int64_t)p.w_end * 32 && s_cnt[i]) atomicAdd(p.satacc + b, s_cnt[i]);
     }
