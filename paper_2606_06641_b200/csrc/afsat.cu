@@ -92,7 +92,7 @@ struct afsat_ctx {
     uint32_t *d_bits = nullptr;                    // sign bits [n][ldb/32]
     int32_t *d_satacc = nullptr, *d_any = nullptr; // d_any: {flag, first step, finished CTAs, step counter}
     // buffers of afsat_step_host (lazy)
-    void *dh_x = nullptr, *dh_F = nullptr, *dh_Fpre = nullptr;
+    void *dh_x = nullptr, *dh_F = nullptr, *dh_Fpre = nullptr, *dh_G = nullptr;   // dh_G: full-width gradient of the pipelined un-tiled step
     int32_t *dh_sat = nullptr, *dh_first = nullptr;
     uint8_t *dh_sol = nullptr;
     cudaStream_t in_stream = nullptr, out_stream = nullptr;
@@ -623,7 +623,7 @@ int step_host_pipelined(afsat_ctx *ctx, T *h_x, double eta, T *h_F_pre)
     }
     k_reset_state<<<gb, tb, 0, st>>>(B, 1, ctx->dh_sol, ctx->dh_first, ctx->d_any, nullptr, 0);
     ++ctx->launches;
-    T *G = tiled ? (T *)ctx->d_G : (T *)ctx->ls_G;                     // un-tiled: a full-width gradient (the line-search buffer)
+    T *G = tiled ? (T *)ctx->d_G : (T *)ctx->dh_G;                     // un-tiled: a full-width gradient
     if (!tiled) CU(cudaMemsetAsync(G, 0, (size_t)ctx->n * ldb * sizeof(T), st));
     CU(cudaEventRecord(ctx->ev_fork, st));
     CU(cudaStreamWaitEvent(ctx->in_stream, ctx->ev_fork, 0));          // uploads start after earlier work on the buffers
@@ -1131,7 +1131,7 @@ void afsat_destroy(afsat_ctx *ctx)
     cudaFree(ctx->d_satacc); cudaFree(ctx->d_any);
     cudaFree(ctx->ls_G); cudaFree(ctx->ls_xt); cudaFree(ctx->ls_F0); cudaFree(ctx->ls_F1); cudaFree(ctx->ls_Dpart);
     cudaFree(ctx->ls_eta); cudaFree(ctx->ls_state);
-    cudaFree(ctx->dh_x); cudaFree(ctx->dh_F); cudaFree(ctx->dh_Fpre); cudaFree(ctx->dh_sat); cudaFree(ctx->dh_first); cudaFree(ctx->dh_sol);
+    cudaFree(ctx->dh_x); cudaFree(ctx->dh_F); cudaFree(ctx->dh_Fpre); cudaFree(ctx->dh_G); cudaFree(ctx->dh_sat); cudaFree(ctx->dh_first); cudaFree(ctx->dh_sol);
     for (cudaEvent_t e : ctx->chunk_in) cudaEventDestroy(e);
     for (cudaEvent_t e : ctx->chunk_done) cudaEventDestroy(e);
     if (ctx->in_stream) cudaStreamDestroy(ctx->in_stream);
@@ -1290,10 +1290,10 @@ int afsat_step_host(afsat_ctx *ctx, void *h_x, double eta, int32_t n_steps, void
     // one iteration, a batch wide enough to cut: copies pipelined behind the evaluation, chunk by chunk
     const bool pipelined = n_steps == 1 && !h_F && !ctx->profiling && ctx->step_path != AFSAT_STEP_PERSISTENT &&
                            (tiled || ctx->B >= 512);
-    if (pipelined && !tiled && !ctx->ls_G) {                          // un-tiled: a full-width gradient buffer
+    if (pipelined && !tiled && !ctx->dh_G) {                          // un-tiled: a full-width gradient buffer
         char *pg = nullptr;
         if ((rc = dev_alloc(ctx, &pg, xb))) return rc;
-        ctx->ls_G = pg;
+        ctx->dh_G = pg;
     }
     if (pipelined) {
         rc = ctx->dtype == 32 ? step_host_pipelined<float>(ctx, (float *)h_x, eta, (float *)h_F_pre)
