@@ -479,6 +479,10 @@ def report(r, world, local, oracle_seconds, rank0_oracle=True):
                     "trivial twiddles at the points 1, -1, i and the eighth roots (k <= 8; cfg1's k = 7 has only such points), literal "
                     "groups (k >= 21), and a partial assignment is substituted before anything is evaluated (frac_after_substitution "
                     "counts the model on the substituted table); measured_pipe_utilisation is what ncu saw executed"}
+    l2 = roof["l2"]
+    roof["limited_by"] = ("l2 throughput: the measured L2 traffic of the evaluation kernels runs at %.0f %% of the L2's delivery rate "
+                          "(roofline.l2, DESIGN.md 6.7)" % (100 * l2["measured_traffic_frac_of_peak"])
+                          if l2.get("measured_traffic_frac_of_peak", 0) >= 0.75 else "fp pipe / issue (roofline.measured_pipe_utilisation)")
     if dtype == 64:
         roof["fp64_peak"] = probed_peak(2, local)
         roof["frac_of_fp64_peak"] = ach_tf / max(probed_peak(2, local), 1e-9)

@@ -251,6 +251,20 @@ int afsat_step_host(afsat_ctx *ctx, void *h_x, double eta, int32_t n_steps, void
 int afsat_host_tables(int32_t type, int32_t k, int32_t param, uint32_t flags, double *table,
                       int32_t *n_real);
 
+/*
+ * afsat_host_restrict -- HOST ONLY: what a constraint becomes under a partial assignment (the
+ * substitution afsat_create applies).  A constraint (type, k, param) with f_true of its literals fixed true and
+ * f_false fixed false keeps k_free = k - f_true - f_false literals and, on them, the symmetric constraint whose
+ * satisfying counts are  { tau' : tau' + f_true satisfies the original }.  mask[0] / mask[1] receive that set as
+ * bits 0..63 / 64..127.  Returns 0 if the restricted constraint still depends on its free literals, 1 if the
+ * assignment already satisfies it, 2 if it already violates it, or a negative error.
+ * afsat_host_tables_mask -- afsat_host_tables for such a (k_free, mask) signature (flags: 0 = paper tables,
+ * AFSAT_FLAG_ROBUST = robust tables).
+ */
+int afsat_host_restrict(int32_t type, int32_t k, int32_t param, int32_t f_true, int32_t f_false, int32_t *k_free,
+                        uint64_t *mask);
+int afsat_host_tables_mask(int32_t k, uint64_t mask_lo, uint64_t mask_hi, uint32_t flags, double *table, int32_t *n_real);
+
 /* afsat_query -- counters and facts about a context. */
 enum afsat_query_key {
     AFSAT_Q_KERNEL_LAUNCHES = 0,  /* kernels launched by this context so far                     */

@@ -30,7 +30,7 @@ ERROR_NAMES = {0: "AFSAT_OK", -1: "AFSAT_E_INVALID", -2: "AFSAT_E_LENGTH", -3: "
                -4: "AFSAT_E_SIGN", -5: "AFSAT_E_DUPLICATE", -6: "AFSAT_E_PARAM",
                -7: "AFSAT_E_NOMEM", -8: "AFSAT_E_CUDA", -9: "AFSAT_E_UNSAT"}
 
-EXPORTS = ["afsat_create", "afsat_create_ex", "afsat_probe_peak", "afsat_destroy", "afsat_last_error", "afsat_eval_grad", "afsat_check",
+EXPORTS = ["afsat_create", "afsat_create_ex", "afsat_probe_peak", "afsat_host_restrict", "afsat_host_tables_mask", "afsat_destroy", "afsat_last_error", "afsat_eval_grad", "afsat_check",
            "afsat_step", "afsat_step_host", "afsat_host_tables", "afsat_query", "afsat_version",
            "afsat_set_profiling", "afsat_step_ls", "afsat_parse", "afsat_parse_file", "afsat_parse_error",
            "afsat_problem_sizes", "afsat_problem_fill", "afsat_problem_free", "afsat_restart", "afsat_solve"]
@@ -84,6 +84,10 @@ def load_library():
     L.afsat_step_host.argtypes = [vp, vp, dbl, i32, vp, vp, vp, vp, vp]
     L.afsat_host_tables.restype = C.c_int
     L.afsat_host_tables.argtypes = [i32, i32, i32, u32, vp, vp]
+    L.afsat_host_restrict.restype = C.c_int
+    L.afsat_host_restrict.argtypes = [i32, i32, i32, i32, i32, vp, vp]
+    L.afsat_host_tables_mask.restype = C.c_int
+    L.afsat_host_tables_mask.argtypes = [i32, C.c_uint64, C.c_uint64, u32, vp, vp]
     L.afsat_query.restype = i64
     L.afsat_query.argtypes = [vp, i32]
     L.afsat_set_profiling.restype = C.c_int
@@ -128,6 +132,29 @@ def host_tables(ctype: int, k: int, param: int, flags: int = 0):
     rc = L.afsat_host_tables(ctype, k, param, flags, tab.ctypes.data, C.addressof(n_real))
     if rc < 0:
         raise AfsatError(rc, "afsat_host_tables")
+    return tab[:rc].copy(), int(n_real.value)
+
+
+def host_restrict(ctype: int, k: int, param: int, f_true: int, f_false: int):
+    """afsat_host_restrict: (status, k_free, mask) of a constraint under a partial assignment; status 0 = still depends on
+    its free literals, 1 = satisfied, 2 = violated; mask = Python int with bit tau' set iff tau' free true literals satisfy."""
+    L = load_library()
+    kf = C.c_int32(0)
+    mk = (C.c_uint64 * 2)(0, 0)
+    rc = L.afsat_host_restrict(ctype, k, param, f_true, f_false, C.addressof(kf), C.addressof(mk))
+    if rc < 0:
+        raise AfsatError(rc, "afsat_host_restrict")
+    return rc, int(kf.value), int(mk[0]) | (int(mk[1]) << 64)
+
+
+def host_tables_mask(k: int, mask: int, flags: int = 0):
+    """(rows [P,8] float64, n_real) of the signature (k literals, satisfying counts = bits of mask).  Host only."""
+    L = load_library()
+    tab = np.zeros((MAX_LEN // 2 + 1, 8), dtype=np.float64)
+    n_real = C.c_int32(0)
+    rc = L.afsat_host_tables_mask(k, mask & 0xFFFFFFFFFFFFFFFF, mask >> 64, flags, tab.ctypes.data, C.addressof(n_real))
+    if rc < 0:
+        raise AfsatError(rc, "afsat_host_tables_mask")
     return tab[:rc].copy(), int(n_real.value)
 
 

@@ -687,6 +687,38 @@ int afsat_host_tables(int32_t type, int32_t k, int32_t param, uint32_t flags, do
     return rows;
 }
 
+int afsat_host_restrict(int32_t type, int32_t k, int32_t param, int32_t f_true, int32_t f_false, int32_t *k_free, uint64_t *mask)
+{
+    if (!k_free || !mask) return AFSAT_E_INVALID;
+    if (type < AFSAT_OR || type > AFSAT_NAE) return AFSAT_E_INVALID;
+    if (k < 1 || k > AFSAT_MAX_LEN) return AFSAT_E_LENGTH;
+    if (f_true < 0 || f_false < 0 || f_true + f_false > k) return AFSAT_E_INVALID;
+    if (type == AFSAT_XOR && param != 0 && param != 1) return AFSAT_E_PARAM;
+    if ((type == AFSAT_ATLEAST || type == AFSAT_ATMOST || type == AFSAT_EXACTLY) && (param < 0 || param > k)) return AFSAT_E_PARAM;
+    const int kf = k - f_true - f_false;
+    int nsat = 0;
+    mask[0] = mask[1] = 0;
+    for (int tau = 0; tau <= kf; ++tau)
+        if (afsat_sig_satisfied(type, k, param, tau + f_true)) {
+            ++nsat;
+            mask[tau >> 6] |= 1ull << (tau & 63);
+        }
+    *k_free = kf;
+    return nsat == kf + 1 ? 1 : nsat == 0 ? 2 : 0;
+}
+
+int afsat_host_tables_mask(int32_t k, uint64_t mask_lo, uint64_t mask_hi, uint32_t flags, double *table, int32_t *n_real)
+{
+    if (!table) return AFSAT_E_INVALID;
+    AfsatSigHost s;
+    int rc = afsat_sig_build_mask(k, mask_lo, mask_hi, flags & AFSAT_FLAG_ROBUST, &s);
+    if (rc) return rc;
+    const int rows = s.n_real + s.n_cplx;
+    memcpy(table, s.rows, sizeof(double) * 8 * rows);
+    if (n_real) *n_real = s.n_real;
+    return rows;
+}
+
 int afsat_create(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64_t *row_ptr, const int32_t *lit_var,
                  const int8_t *lit_sign, const uint8_t *type, const int32_t *param, const int8_t *fixed,
                  int32_t batch, int64_t ldb, int32_t dtype, int32_t device, uint32_t flags)
@@ -801,18 +833,15 @@ int afsat_create_ex(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64
                 if (!f) ++kf;
                 else if ((f < 0) == (lit_sign[q] > 0)) ++fT;          // variable True and literal positive, or False and negated
             }
-            SigKey key{kf, 0, 0};
-            int nsat = 0;
-            for (int tau = 0; tau <= kf; ++tau)
-                if (afsat_sig_satisfied(type[c], k, cprm[c], tau + fT)) {
-                    ++nsat;
-                    if (tau < 64) key.lo |= 1ull << tau; else key.hi |= 1ull << (tau - 64);
-                }
+            uint64_t mk[2];
+            int kf2 = 0;
+            const int decided = afsat_host_restrict(type[c], k, cprm[c], fT, k - kf - fT, &kf2, mk);
+            SigKey key{kf, mk[0], mk[1]};
             Sub &s = subs[g][c];
             s.key = key;
-            s.live = nsat != 0 && nsat != kf + 1;
+            s.live = decided == 0;
             if (!s.live) {                                             // decided by the partial assignment (or trivial): FE = -1 / +1
-                if (nsat) { ++gp.sat_const; gp.F_const -= 1.0; } else gp.F_const += 1.0;
+                if (decided == 1) { ++gp.sat_const; gp.F_const -= 1.0; } else gp.F_const += 1.0;
             } else {
                 sig_id.emplace(key, 0);
                 ++gp.m_live; gp.nnz += kf; gp.kmax = std::max(gp.kmax, kf);

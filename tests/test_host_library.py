@@ -126,6 +126,43 @@ def test_host_tables_rejects():
     assert L.afsat_host_tables(0, 3, 0, 0, None, None) == -1
 
 
+def test_restriction_under_a_partial_assignment():
+    """afsat_host_restrict (the substitution afsat_create applies) against the test's own predicate: for every
+    type, length <= 9, parameter and split of the fixed literals into true / false, the restricted truth table is the
+    original one shifted by the fixed-true count, and "decided" means constant."""
+    for t, k, p in _cases(9):
+        for f_true in range(k + 1):
+            for f_false in range(k + 1 - f_true):
+                status, kf, mask = Bd.host_restrict(t, k, p, f_true, f_false)
+                assert kf == k - f_true - f_false
+                want = [R.is_sat(t, k, p, tau + f_true) for tau in range(kf + 1)]
+                assert [bool(mask >> tau & 1) for tau in range(kf + 1)] == want and mask >> (kf + 1) == 0
+                assert status == (1 if all(want) else 2 if not any(want) else 0)
+    with pytest.raises(Bd.AfsatError):
+        Bd.host_restrict(R.OR, 3, 0, 2, 2)
+
+
+@pytest.mark.parametrize("flags", [Bd.FLAG_DEFAULT, Bd.FLAG_ROBUST])
+def test_tables_of_restricted_signatures_reproduce_their_truth_table(flags):
+    """P10 for the signatures substitution creates (arbitrary symmetric truth tables, e.g. "2 <= tau <= 4 of 6" from an
+    EXACTLY / ATLEAST mix): sum_p Re(w_p prod_i (a_p + b_p y_i)) = -1 / +1 at the corner with tau true literals."""
+    rng = np.random.default_rng(77)
+    for k in (1, 2, 3, 5, 8, 12, 17):
+        for _ in range(6):
+            mask = int(rng.integers(1, (1 << (k + 1)) - 1))            # non-constant truth table
+            rows, n_real = Bd.host_tables_mask(k, mask, flags)
+            for tau in range(k + 1):
+                y = np.array([-1.0] * tau + [1.0] * (k - tau))
+                fe, _ = _eval_tables(rows, y)
+                assert abs(float(fe) - (-1.0 if mask >> tau & 1 else 1.0)) < 1e-9, (k, mask, tau, float(fe))
+    # the restriction of a Table 1 constraint gets the SAME table as the native constraint with that truth table
+    status, kf, mask = Bd.host_restrict(R.OR, 8, 0, 0, 2)
+    assert status == 0 and kf == 6
+    assert np.array_equal(Bd.host_tables_mask(kf, mask)[0], Bd.host_tables(R.OR, 6, 0)[0])
+    status, kf, mask = Bd.host_restrict(R.ATLEAST, 12, 6, 2, 1)        # "at least 6 of 12" -> "at least 4 of 9"
+    assert np.array_equal(Bd.host_tables_mask(kf, mask)[0], Bd.host_tables(R.ATLEAST, 9, 4)[0])
+
+
 def _has_gpu():
     import torch
     return torch.cuda.is_available()
