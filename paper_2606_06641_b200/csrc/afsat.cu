@@ -194,13 +194,17 @@ void prof_drain(afsat_ctx *c, bool keep)
 
 // ---- kernel selection per length class ------------------------------------------------------------------------------
 template <typename T>
-void (*pick_kernel(int cls, bool grad))(EvalParams<T>)
+void (*pick_kernel(int cls, bool grad, bool csplit))(EvalParams<T>)
 {
     using Fn = void (*)(EvalParams<T>);
     if constexpr (sizeof(T) == 4) {
         switch (cls) {
-        case CLS_S: return grad ? (Fn)k_eval_f2m<1, AFSAT_S_KMAX, 2, true, 2> : (Fn)k_eval_f2m<1, AFSAT_S_KMAX, 2, false, 2>;
-        case CLS_A: return grad ? (Fn)k_eval_f2m<AFSAT_S_KMAX + 1, AFSAT_A_KMAX, 1, true, 2> : (Fn)k_eval_f2m<AFSAT_S_KMAX + 1, AFSAT_A_KMAX, 1, false, 2>;
+        case CLS_S:
+            if (csplit) return grad ? (Fn)k_eval_f2m<1, AFSAT_S_KMAX, 2, true, 2, true> : (Fn)k_eval_f2m<1, AFSAT_S_KMAX, 2, false, 2, true>;
+            return grad ? (Fn)k_eval_f2m<1, AFSAT_S_KMAX, 2, true, 2, false> : (Fn)k_eval_f2m<1, AFSAT_S_KMAX, 2, false, 2, false>;
+        case CLS_A:
+            if (csplit) return grad ? (Fn)k_eval_f2m<AFSAT_S_KMAX + 1, AFSAT_A_KMAX, 1, true, 2, true> : (Fn)k_eval_f2m<AFSAT_S_KMAX + 1, AFSAT_A_KMAX, 1, false, 2, true>;
+            return grad ? (Fn)k_eval_f2m<AFSAT_S_KMAX + 1, AFSAT_A_KMAX, 1, true, 2, false> : (Fn)k_eval_f2m<AFSAT_S_KMAX + 1, AFSAT_A_KMAX, 1, false, 2, false>;
         case CLS_B: return grad ? (Fn)k_eval_split<float, AFSAT_A_KMAX + 1, AFSAT_B_KMAX, 2, 2, true, AFSAT_M32_THREADS, AFSAT_M32_MINB>
                                 : (Fn)k_eval_split<float, AFSAT_A_KMAX + 1, AFSAT_B_KMAX, 2, 2, false, AFSAT_M32_THREADS, AFSAT_M32_MINB>;
         default:    return grad ? (Fn)k_eval_split<float, AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, 1, true, AFSAT_L32_THREADS, AFSAT_L32_MINB>
@@ -256,7 +260,7 @@ int launch_eval(afsat_ctx *ctx, const GroupPlan &gp, const T *x, T *G, int64_t g
         p.Wc = g.Wc; p.Wk = g.Wk; p.cs = g.cs;
         const int64_t per_cta = (int64_t)g.cw * g.Wc;
         dim3 block(32 * g.warps), grid(nit, (unsigned)((width + per_cta - 1) / per_cta));
-        pick_kernel<T>(cls, grad)<<<grid, block, 0, st>>>(p);
+        pick_kernel<T>(cls, grad, g.cs > 1)<<<grid, block, 0, st>>>(p);
         ++ctx->launches;
         CU(cudaPeekAtLastError());
         if (my_side >= 0) {

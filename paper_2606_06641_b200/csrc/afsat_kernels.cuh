@@ -845,7 +845,7 @@ __device__ __forceinline__ void run_item_f2(const EvalParams<float> &p, const in
 // ---- one launch for a RANGE of lengths [KLO, KHI]: the CTA's item picks its length-K body, which is a
 // separately compiled (noinline) function so that every length keeps its own schedule and register
 // allocation while all lengths share one grid (no per-length launch tails) ---------------------------
-template <int K, int NP, bool GRAD>
+template <int K, int NP, bool GRAD, bool CSPLIT>
 __device__ __noinline__ void item_body_f2(const EvalParams<float> &p, const int32_t *s_lits, const f32x2 *s_tab2,
                                           const float *s_tabg, float (*s_F)[64 * NP], int n_real, int n_cplx, int nc, int uv)
 {
@@ -854,7 +854,8 @@ __device__ __noinline__ void item_body_f2(const EvalParams<float> &p, const int3
     const int wc = warp % p.Wc, wk = warp / p.Wc;
     // the warp's lanes take cs constraints at once (a narrow candidate tile still fills the warp: cfg4's tile of 64
     // candidates is 16 lanes x 4 candidates; the per-constraint instructions are issued once for both constraints)
-    const int lpc = 32 / p.cs, sub = lane / lpc, ll = lane % lpc;
+    const int pcs = CSPLIT ? p.cs : 1;                                // (a compile-time 1 saves the registers of the general case)
+    const int lpc = 32 / pcs, sub = lane / lpc, ll = lane % lpc;
     const int64_t b = p.b_begin + ((int64_t)blockIdx.y * p.Wc + wc) * (lpc * V) + ll * V;
     const bool active = b < p.b_end && b < p.B && !lane_skipped(p, b, V);   // this launch owns [b_begin, b_end)
     f32x2 fe2[NP];
@@ -862,7 +863,7 @@ __device__ __noinline__ void item_body_f2(const EvalParams<float> &p, const int3
     for (int q = 0; q < NP; ++q) fe2[q] = 0ull;
     if (active) {
         constexpr bool PF = K <= 5;
-        const int c0 = wk * p.cs + sub, cstep = p.Wk * p.cs;
+        const int c0 = wk * pcs + sub, cstep = p.Wk * pcs;
         if (uv == 1) run_item_f2<K, NP, GRAD, PF, 1>(p, s_lits, s_tab2, s_tabg, n_real, n_cplx, nc, c0, cstep, b, fe2);
         else if (uv == 2) run_item_f2<K, NP, GRAD, PF, 2>(p, s_lits, s_tab2, s_tabg, n_real, n_cplx, nc, c0, cstep, b, fe2);
         else run_item_f2<K, NP, GRAD, PF, 0>(p, s_lits, s_tab2, s_tabg, n_real, n_cplx, nc, c0, cstep, b, fe2);
@@ -880,23 +881,23 @@ __device__ __noinline__ void item_body_f2(const EvalParams<float> &p, const int3
         for (int v = 0; v < V; ++v) {
             float sacc = 0.f;
             for (int g = 0; g < p.Wk; ++g)
-                for (int u = 0; u < p.cs; ++u) sacc += s_F[warp + g * p.Wc][(u * lpc + ll) * V + v];
+                for (int u = 0; u < pcs; ++u) sacc += s_F[warp + g * p.Wc][(u * lpc + ll) * V + v];
             if (b + v < p.B) p.Fpart[(int64_t)(p.frow_base + blockIdx.x) * p.ldb + b + v] = sacc;
         }
     }
 }
 
-template <int K, int KHI, int NP, bool GRAD>
+template <int K, int KHI, int NP, bool GRAD, bool CSPLIT>
 struct SwitchF2 {
     static __device__ __forceinline__ void go(int k, const EvalParams<float> &p, const int32_t *s_lits, const f32x2 *s_tab2,
                                               const float *s_tabg, float (*s_F)[64 * NP], int n_real, int n_cplx, int nc, int uv)
     {
-        if (k == K) item_body_f2<K, NP, GRAD>(p, s_lits, s_tab2, s_tabg, s_F, n_real, n_cplx, nc, uv);
-        else if (K < KHI) SwitchF2<(K < KHI ? K + 1 : K), KHI, NP, GRAD>::go(k, p, s_lits, s_tab2, s_tabg, s_F, n_real, n_cplx, nc, uv);
+        if (k == K) item_body_f2<K, NP, GRAD, CSPLIT>(p, s_lits, s_tab2, s_tabg, s_F, n_real, n_cplx, nc, uv);
+        else if (K < KHI) SwitchF2<(K < KHI ? K + 1 : K), KHI, NP, GRAD, CSPLIT>::go(k, p, s_lits, s_tab2, s_tabg, s_F, n_real, n_cplx, nc, uv);
     }
 };
 
-template <int KLO, int KHI, int NP, bool GRAD, int MINB>
+template <int KLO, int KHI, int NP, bool GRAD, int MINB, bool CSPLIT>
 __global__ void __launch_bounds__(CTA_THREADS, MINB) k_eval_f2m(const EvalParams<float> p)
 {
     constexpr int H = (KHI + 1) / 2 + 1;
@@ -916,7 +917,7 @@ __global__ void __launch_bounds__(CTA_THREADS, MINB) k_eval_f2m(const EvalParams
     const int nl = (it.c_end - it.c_begin) * it.k;
     for (int i = threadIdx.x; i < nl; i += blockDim.x) s_lits[i] = __ldg(p.lits + it.lit_base + i);
     __syncthreads();
-    SwitchF2<KLO, KHI, NP, GRAD>::go(it.k, p, s_lits, s_tab2, s_tabg, s_F, n_unit, n_gen, it.c_end - it.c_begin, uv);
+    SwitchF2<KLO, KHI, NP, GRAD, CSPLIT>::go(it.k, p, s_lits, s_tab2, s_tabg, s_F, n_unit, n_gen, it.c_end - it.c_begin, uv);
 }
 
 // one body per length: KHI <= 20 for both instantiations (fp32 beyond k = 8 runs the lane-split kernels of afsat_split.cuh)
