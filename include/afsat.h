@@ -69,8 +69,9 @@ enum afsat_error {
  *                  gradients beyond k ~ 20 (the floating-point ceiling of PAPER.md:135-139).
  *   robust tables: prod_i ((1 + w^l)/2 + y_i (1 - w^l)/2) contracted with the DFT of the truth table itself
  *                  (reading B4): every factor has modulus <= 1, same FE, holds 1e-4 in fp32 up to k = 64.
- * AFSAT_FLAG_DEFAULT (automatic, SURVEY.md §8(f) NEXT #3 "per-bucket choice"): fp32 contexts use the paper tables
- * for lengths k <= 20 and the robust tables for k > 20; fp64 contexts use the paper tables at every length.
+ * AFSAT_FLAG_DEFAULT (automatic, SURVEY.md §8(f) NEXT #3 "per-bucket choice"): the paper tables for lengths k <= 20 and
+ * the robust tables for k > 20, in both precisions -- at corner points (where projected gradient descent parks variables)
+ * the paper's product form loses 1e-4 in fp32 and 1e-10 in fp64 beyond k ~ 20-25.
  * AFSAT_FLAG_ROBUST: robust tables for every signature.  AFSAT_FLAG_PAPER: paper tables for every signature
  * (the comparison mode BASELINE.json configs[3] "report deviation" asks for).  Lengths are those AFTER the
  * partial assignment has been substituted (see afsat_create).                                                  */

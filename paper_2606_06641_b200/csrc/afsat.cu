@@ -38,7 +38,7 @@ inline int class_of(int k, int dtype)
 {
     return (dtype == 32 && k <= AFSAT_S_KMAX) ? CLS_S : k <= AFSAT_A_KMAX ? CLS_A : k <= AFSAT_B_KMAX ? CLS_B : CLS_LONG;
 }
-constexpr int ROBUST_FROM_K32 = 21;     // AFSAT_FLAG_DEFAULT, fp32: robust tables from this length on (include/afsat.h)
+constexpr int ROBUST_FROM_K = 21;       // AFSAT_FLAG_DEFAULT: robust tables from this length on (include/afsat.h)
 
 struct ClassGeom {              // how one length class maps candidates onto a CTA
     int V = 1;                  // candidates per lane
@@ -868,7 +868,7 @@ int afsat_create_ex(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64
     for (auto &kv : sig_id) {
         AfsatSigHost hs;
         const int kk = kv.first.k;
-        const bool robust = (flags & AFSAT_FLAG_ROBUST) || (!(flags & AFSAT_FLAG_PAPER) && dtype == 32 && kk >= ROBUST_FROM_K32);
+        const bool robust = (flags & AFSAT_FLAG_ROBUST) || (!(flags & AFSAT_FLAG_PAPER) && kk >= ROBUST_FROM_K);
         int rc = afsat_sig_build_mask(kk, kv.first.lo, kv.first.hi, robust ? AFSAT_FLAG_ROBUST : 0u, &hs);
         if (rc) return fail(ctx, rc, "signature table construction failed");
         SigDev &d = sigs[kv.second];

@@ -3,7 +3,7 @@ the long-double CPU oracle on the same seeded inputs.
 
 Tolerances (BASELINE.json north_star, restated in DESIGN.md "Tolerances"):
   fp32: |F - F*| <= 1e-4 * m + 1e-5 * |F*| ; |G - G*| <= 1e-4 per component, at EVERY length (the default context
-        takes the paper's tables for k <= 20 and the robust tables beyond, include/afsat.h)
+        takes the paper's tables for k <= 20 and the robust tables beyond, in both precisions, include/afsat.h)
   fp32 with the paper's tables forced (AFSAT_FLAG_PAPER) at k > 20: the forward-error bound of the product form,
         computed here from the inputs and the host tables (product_form_bound), constant C_BOUND fixed once
   fp64: 1e-10 on F (abs, times max(1, m/1000) for the summation) and on G
@@ -996,3 +996,24 @@ def test_probe_peaks_are_plausible():
     f, f2, d = Bd.probe_peak(0), Bd.probe_peak(1), Bd.probe_peak(2)
     print("probe peaks TFLOP/s: FFMA", f, "FFMA2", f2, "DFMA", d)
     assert 40.0 < f < 90.0 and 40.0 < f2 < 90.0 and 10.0 < d < 50.0
+
+
+@pytest.mark.parametrize("dtype", [32, 64])
+def test_long_constraints_at_corners_default_tables(dtype):
+    """PGD parks variables at exactly +-1, where the paper's product form loses fp32 (and, a little later, fp64)
+    beyond k ~ 20 (its terms reach 2^k / N there).  The DEFAULT context (robust tables beyond k = 20) must hold the
+    north_star's bounds at corner points for k = 21..50 in both precisions: half of the candidates are pure corners, the others have a third of their coordinates
+    interior; FE is exactly -1 / +1 per constraint at pure corners."""
+    inst = I.make_mixed(n=90, m=160, kmin=21, kmax=50, seed=2150, batch=64,
+                        types=[I.ATLEAST, I.ATMOST, I.EXACTLY, I.OR, I.NAE, I.XOR])
+    rng = np.random.default_rng(2151)
+    x = I.corner_x(inst, rng.integers(0, 2, size=(inst.n_vars, 64)).astype(bool))
+    interior = rng.random((inst.n_vars, 32)) < 1.0 / 3.0
+    x[:, 32:64] = np.where(interior, (2.0 * rng.random((inst.n_vars, 32)) - 1.0).astype(np.float32), x[:, 32:64])
+    F, G = assert_eval_parity(inst, x, 64, dtype)                     # fp32: 1e-4 m + 1e-5 |F*|, 1e-4; fp64: 1e-10
+    sat, _ = O.check(inst, x.astype(np.float64), 64)
+    assert np.abs(F[:32] - (inst.n_cons - 2.0 * sat[:32])).max() <= (1e-3 if dtype == 32 else 1e-9)
+    # the paper's tables at the same points, for the record (not gated: this is the ceiling of PAPER.md:135-139)
+    Fp, Gp = run_eval(inst, x, 64, dtype, flags=Bd.FLAG_PAPER)
+    Fo, Go = O.eval_grad(inst, x.astype(np.float64), 64)
+    print(f"corners, k = 21..50, fp{dtype}: default tables max|dG|", np.abs(G - Go).max(), "; paper tables max|dG|", np.abs(Gp - Go).max())
