@@ -32,7 +32,7 @@ thread_local std::string g_create_error;
 //         A  6..8     k_eval_f2m, two candidates per lane
 //         B  9..20    packed lane-split kernel (two lanes x two candidates)
 //         L  21..64   scalar lane-split kernel (two lanes per candidate)
-//   fp64: A  k <= 8 and B 9..20  k_eval_km (one candidate per lane);  L  21..64  lane-split kernel, four lanes per candidate
+//   fp64: A  k <= 8  k_eval_km (one candidate per lane);  B  9..20 / L  21..64  lane-split kernel, two / four lanes per candidate
 enum { CLS_S = 0, CLS_A = 1, CLS_B = 2, CLS_LONG = 3, N_CLS = 4 };
 inline int class_of(int k, int dtype)
 {
@@ -214,7 +214,8 @@ void (*pick_kernel(int cls, bool grad, bool csplit))(EvalParams<T>)
         switch (cls) {
         case CLS_S: return nullptr;                                    // empty for fp64
         case CLS_A: return grad ? (Fn)k_eval_km<T, 1, AFSAT_A_KMAX, 1, true, 1> : (Fn)k_eval_km<T, 1, AFSAT_A_KMAX, 1, false, 1>;
-        case CLS_B: return grad ? (Fn)k_eval_km<T, AFSAT_A_KMAX + 1, AFSAT_B_KMAX, 1, true, 1> : (Fn)k_eval_km<T, AFSAT_A_KMAX + 1, AFSAT_B_KMAX, 1, false, 1>;
+        case CLS_B: return grad ? (Fn)k_eval_split<double, AFSAT_A_KMAX + 1, AFSAT_B_KMAX, 2, 1, true, AFSAT_L64_THREADS, 1>
+                                : (Fn)k_eval_split<double, AFSAT_A_KMAX + 1, AFSAT_B_KMAX, 2, 1, false, AFSAT_L64_THREADS, 1>;
         default:    return grad ? (Fn)k_eval_split<double, AFSAT_L64_KMIN, AFSAT_MAX_LEN, 4, 1, true, AFSAT_L64_THREADS, 1>
                                 : (Fn)k_eval_split<double, AFSAT_L64_KMIN, AFSAT_MAX_LEN, 4, 1, false, AFSAT_L64_THREADS, 1>;
         }
@@ -913,9 +914,9 @@ int afsat_create_ex(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64
             rows2.insert(rows2.end(), packed, packed + (size_t)nrows2 * ROW2);
             rows2g.insert(rows2g.end(), packedg, packedg + (size_t)ng * ROW2G);
         }
-        if (class_of(kk, dtype) == CLS_LONG || (dtype == 32 && class_of(kk, dtype) == CLS_B)) {   // grouped lane-split kernels
+        if (class_of(kk, dtype) == CLS_LONG || class_of(kk, dtype) == CLS_B) {   // grouped lane-split kernels
             double packed[AFSAT_MAX_POINTS * ROWG];
-            const int ns = dtype == 64 ? 4 : 2;                        // lanes per candidate (pair) of the kernel that runs kk
+            const int ns = (dtype == 64 && class_of(kk, dtype) == CLS_LONG) ? 4 : 2;   // lanes per candidate (pair) of the kernel that runs kk
             d.pad = (int8_t)pack_rows_grp(hs.rows, hs.n_real + hs.n_cplx, kk, ns, packed);
             d.row2_off = (int32_t)(rowsg.size() / ROWG);
             rowsg.insert(rowsg.end(), packed, packed + (size_t)(hs.n_real + hs.n_cplx) * ROWG);
@@ -964,6 +965,7 @@ int afsat_create_ex(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64
         if (cls == CLS_B && dtype == 32) { g.warps = AFSAT_M32_THREADS / 32; g.cw = 32; }                 // 2 lanes x 2 candidates
         else if (cls == CLS_LONG && dtype == 32) { g.warps = AFSAT_L32_THREADS / 32; g.cw = 32 / AFSAT_L32_NS; }
         else if (cls == CLS_LONG) { g.warps = AFSAT_L64_THREADS / 32; g.cw = 8; }                         // fp64: four lanes per candidate
+        else if (cls == CLS_B) { g.warps = AFSAT_L64_THREADS / 32; g.cw = 16; }                           // fp64, 9..20: two lanes per candidate
         const int64_t cw = g.cw;
         g.Wc = std::min(g.warps, pow2_floor(std::max<int64_t>(1, (tile_w + cw - 1) / cw)));
         if ((int64_t)g.Wc * cw < tile_w && g.Wc < g.warps && (int64_t)g.Wc * cw * 2 <= tile_w + cw - 1) g.Wc *= 2;

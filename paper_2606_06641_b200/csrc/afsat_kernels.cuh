@@ -920,7 +920,7 @@ __global__ void __launch_bounds__(CTA_THREADS, MINB) k_eval_f2m(const EvalParams
     SwitchF2<KLO, KHI, NP, GRAD, CSPLIT>::go(it.k, p, s_lits, s_tab2, s_tabg, s_F, n_unit, n_gen, it.c_end - it.c_begin, uv);
 }
 
-// one body per length: KHI <= 20 for both instantiations (fp32 beyond k = 8 runs the lane-split kernels of afsat_split.cuh)
+// one body per length, fp64 k <= 8 (everything longer, and fp32 beyond k = 8, runs the lane-split kernels of afsat_split.cuh)
 template <typename T, int K, int V, bool GRAD>
 __device__ __noinline__ void item_body_k(const EvalParams<T> &p, const int32_t *s_lits, const T *s_tab, T (*s_F)[32 * V],
                                          int n_real, int n_cplx, int nc)
@@ -963,7 +963,7 @@ __global__ void __launch_bounds__(CTA_THREADS, MINB) k_eval_km(const EvalParams<
 }
 
 // length classes (afsat.cu class_of): fp32  k <= 5: k_eval_f2m, four candidates per lane | 6..8: k_eval_f2m, two per lane |
-// 9..20: packed lane-split kernel | 21..64: scalar lane-split kernel;  fp64  k <= 8, 9..20: k_eval_km | 21..64: lane-split
+// 9..20: packed lane-split kernel | 21..64: scalar lane-split kernel;  fp64  k <= 8: k_eval_km | 9..20, 21..64: lane-split
 #define AFSAT_S_KMAX 5
 #define AFSAT_A_KMAX 8
 #define AFSAT_B_KMAX 20

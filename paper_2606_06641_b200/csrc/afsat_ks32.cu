@@ -9,6 +9,8 @@ template __global__ void k_eval_split<float, AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSA
 template __global__ void k_eval_split<float, AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, 1, false, AFSAT_L32_THREADS, AFSAT_L32_MINB>(const EvalParams<float>);
 template __global__ void k_eval_split<double, AFSAT_L64_KMIN, AFSAT_MAX_LEN, 4, 1, true, AFSAT_L64_THREADS, 1>(const EvalParams<double>);
 template __global__ void k_eval_split<double, AFSAT_L64_KMIN, AFSAT_MAX_LEN, 4, 1, false, AFSAT_L64_THREADS, 1>(const EvalParams<double>);
+template __global__ void k_eval_split<double, AFSAT_A_KMAX + 1, AFSAT_B_KMAX, 2, 1, true, AFSAT_L64_THREADS, 1>(const EvalParams<double>);
+template __global__ void k_eval_split<double, AFSAT_A_KMAX + 1, AFSAT_B_KMAX, 2, 1, false, AFSAT_L64_THREADS, 1>(const EvalParams<double>);
 template __global__ void k_eval_split<float, AFSAT_A_KMAX + 1, AFSAT_B_KMAX, 2, 2, true, AFSAT_M32_THREADS, AFSAT_M32_MINB>(const EvalParams<float>);
 template __global__ void k_eval_split<float, AFSAT_A_KMAX + 1, AFSAT_B_KMAX, 2, 2, false, AFSAT_M32_THREADS, AFSAT_M32_MINB>(const EvalParams<float>);
 }  // namespace afsat
