@@ -449,8 +449,8 @@ def report(r, world, local, oracle_seconds, rank0_oracle=True):
     cap = load_capture(cfg, dtype)
     path_name = {1: "launches", 2: "persistent (one launch)", 3: "cuda graph"}.get(r["path"], str(r["path"]))
     roof = {"bound": "alu",
-            "kernel": "evaluation kernels, a1-a5 (fp32: k_eval_f2m k<=8 | k_eval_split k>=9; fp64: k_eval_km k<=20 | "
-                      "k_eval_split k>20): all launches of one step",
+            "kernel": "evaluation kernels, a1-a5 (fp32: k_eval_f2m k<=8 | k_eval_split k>=9; fp64: k_eval_km k<=8 | "
+                      "k_eval_split k>=9): all launches of one step",
             "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach_tf / peak_tf,
             "peak_source": f"{sm} SMs x 128 FP32 lanes x 2 flop x {peaks['sm_max_mhz']:.0f} MHz "
                            f"({peaks['source']} sm_max_mhz; DESIGN.md 6); MEASURED_PEAKS.json has no FP32 figure, so the "

@@ -30,9 +30,7 @@ constexpr int32_t LIT_NONE = 0x40000000;
 constexpr int32_t LIT_VAR  = 0x3FFFFFFF;
 
 constexpr int LIT_CHUNK = 4096;       // packed literals staged in shared memory per work item
-#ifndef AFSAT_CTA_THREADS
 #define AFSAT_CTA_THREADS 256
-#endif
 constexpr int CTA_THREADS = AFSAT_CTA_THREADS;
 constexpr int CTA_WARPS = CTA_THREADS / 32;
 constexpr int MAX_ROWS = 33;          // retained DFT points per signature: H <= 64/2 + 1
@@ -575,9 +573,7 @@ __device__ __forceinline__ void grp_rows_f2_joint(const f32x2 (&y)[K][NP], const
 
 // With two pairs per lane and K >= AFSAT_F2_SEQ_MINK the pairs are walked one after the other (each keeps ~4 K register
 // pairs of symmetric polynomials, accumulators and literal values alive).
-#ifndef AFSAT_F2_SEQ_MINK
 #define AFSAT_F2_SEQ_MINK 5
-#endif
 template <int K, int NP, bool GRAD>
 __device__ __forceinline__ void grp_rows_f2(const f32x2 (&y)[K][NP], const float *__restrict__ rg, int n_rows, f32x2 (&fe)[NP],
                                             f32x2 (&g)[K][NP])

@@ -25,31 +25,15 @@
 
 namespace afsat {
 
-#ifndef AFSAT_L32_NS
 #define AFSAT_L32_NS 2                 // lanes per (constraint, candidate)
-#endif
-#ifndef AFSAT_L32_THREADS
-#define AFSAT_L32_THREADS 384             // 12 warps per SM at 168 registers
-#endif
-#ifndef AFSAT_L32_MINB
+#define AFSAT_L32_THREADS 384             // 12 warps per SM at 168 registers (cfg3, ms / step: 256: 1.66, 320: 1.72, 384: 1.53, 512: 1.57)
 #define AFSAT_L32_MINB 1
-#endif
-#ifndef AFSAT_M32_THREADS
 #define AFSAT_M32_THREADS 256             // packed form, k <= 20: 2 CTAs x 8 warps at 128 registers (cfg2: 0.621 ms / step against
-#endif                                    // 0.651 with 384 threads x 168 registers and 0.637 with 512 x 128)
-#ifndef AFSAT_M32_MINB
+                                          // 0.651 with 384 threads x 168 registers and 0.637 with 512 x 128)
 #define AFSAT_M32_MINB 2
-#endif
-#ifndef AFSAT_L64_THREADS
 #define AFSAT_L64_THREADS 384
-#endif
 #define AFSAT_L64_KMIN (AFSAT_B_KMAX + 1)   // fp64, k > 20: FOUR lanes per candidate (a double takes two registers)
-#ifndef AFSAT_L32_PREFETCH
-#define AFSAT_L32_PREFETCH 1
-#endif
-#ifndef AFSAT_L32_KMIN
 #define AFSAT_L32_KMIN (AFSAT_B_KMAX + 1)
-#endif
 // Group layout of a lane with KS literal slots: NG = ceil(KS / 4) groups of BALANCED sizes -- the first NHI = KS mod NG
 // groups take MHI = MLO + 1 literals, the others MLO = floor(KS / NG) (<= 4) -- so that no slot is wasted on padding.
 // Staged row of a point: {Re, Im of c_0 .. c_MHI for groups of MHI | the same for groups of MLO (from scalar ROWG_LO) |
@@ -305,7 +289,6 @@ __device__ __forceinline__ void run_item_split(const EvalParams<T> &p, unsigned 
             else y[i] = flip_sign(__ldg(reinterpret_cast<const T *>(xb + (uint64_t)(uint32_t)(lit[i] & LIT_VAR) * x_ld)), lit[i]);
             g[i] = T(0);
         }
-#if AFSAT_L32_PREFETCH
         if (c + Wk < nc) {                                            // the NEXT constraint's row segments into L1: with 2-3
             const int32_t *Ln = L + Wk * k;                           // warps per scheduler nothing else hides its gathers
 #pragma unroll
@@ -315,7 +298,6 @@ __device__ __forceinline__ void run_item_split(const EvalParams<T> &p, unsigned 
                 asm volatile("prefetch.global.L1 [%0];" ::"l"(xb + (uint64_t)(uint32_t)(ln & LIT_VAR) * x_ld));
             }
         }
-#endif
         eval_points_grp<T, KS, NS, GRAD>(mask, y, s_tab, n_real, n_cplx, fe, g);
         if (GRAD) {
 #pragma unroll
@@ -521,7 +503,6 @@ __device__ __forceinline__ void run_item_split2(const EvalParams<float> &p, unsi
             y[i] = v[0] ^ (((f32x2)m << 32) | m);                     // y = s x (a missing slot: pad, its polarity bit is 0)
             g[i] = 0ull;
         }
-#if AFSAT_L32_PREFETCH
         if (c + Wk < nc) {
             const int32_t *Ln = L + Wk * k;
 #pragma unroll
@@ -531,7 +512,6 @@ __device__ __forceinline__ void run_item_split2(const EvalParams<float> &p, unsi
                 asm volatile("prefetch.global.L1 [%0];" ::"l"(xb + (uint64_t)(uint32_t)(ln & LIT_VAR) * x_ld));
             }
         }
-#endif
         eval_points_grp2<KS, NS, GRAD>(mask, y, s_tab, n_real, n_cplx, fe, g);
         if (GRAD) {
 #pragma unroll

@@ -28,12 +28,8 @@ __global__ void __launch_bounds__(CTA_THREADS) k_pack_signs(const T *__restrict_
 // from the 32 / VW lanes that hold it (one REDUX.OR).
 // rows in flight per thread / CTAs per SM of k_update (cfg4, ms of update per step: 4 / 8: 2.52, 8 / 8: 3.10, 8 / 4: 2.92,
 // 1 / 64: 2.47, 2 / 16: 2.28)
-#ifndef AFSAT_UPD_UNROLL
 #define AFSAT_UPD_UNROLL 2
-#endif
-#ifndef AFSAT_UPD_CTAS_PER_SM
 #define AFSAT_UPD_CTAS_PER_SM 16
-#endif
 constexpr int UPD_UNROLL = AFSAT_UPD_UNROLL;
 template <typename T> struct Vec16;
 template <> struct Vec16<float>  { typedef float4 type;  static constexpr int VW = 4; };

@@ -378,11 +378,12 @@ def test_cfg0_free_running_solve_rate(seed, path):
 
 
 def test_step_multi_equals_repeated_single_and_freeze():
-    """n_steps in one call == the same number of single-step calls with resume (bit for bit), and
-    a solved candidate stays frozen."""
+    """n_steps in one call == the same number of single-step calls with resume, and a solved candidate stays frozen.
+    The property is control flow (step counting, resume, freezing), so it runs in fp64, where the run-to-run order of
+    the partial gradients (1e-16) cannot be amplified into a different discrete outcome within 60 steps."""
     inst = I.make_config(0, instance_seed=6641007)
-    x0 = I.make_x0(inst)
-    ctx = Bd.Context.from_instance(inst)
+    x0 = I.make_x0(inst).astype(np.float64)
+    ctx = Bd.Context.from_instance(inst, dtype=64)
     xa, xb = dev(x0), dev(x0)
     Fa, sata, sola, firsta = ctx.step(xa, 0.1, 60)
     state = None
@@ -390,8 +391,7 @@ def test_step_multi_equals_repeated_single_and_freeze():
         Fb, satb, solb, firstb = ctx.step(xb, 0.1, 1, step_base=t, state=state)
         state = (solb, firstb)
     assert torch.equal(sola, solb) and torch.equal(firsta, firstb) and torch.equal(sata, satb)
-    dab = (xa - xb).abs().flatten()                   # the order of the partial gradients differs run to run; a trajectory
-    assert torch.quantile(dab, 0.99).item() <= 1e-5 and dab.max().item() <= 5e-2   # may amplify that on a coordinate
+    assert (xa - xb).abs().max().item() <= 1e-9
     # frozen: continue 20 steps, solved columns must not move
     solved = sola.cpu().numpy().astype(bool)
     before = xa.clone()
@@ -912,9 +912,19 @@ def test_step_paths_agree(dtype):
     Xo, _, sato, solo, firsto = O.step(inst, x0.astype(np.float64), 0.1, 40, 80, want_F=False)
     assert solo[3] == 1 and firsto[3] == 1                             # the planted candidate: solved by the first step
     for path, o in outs.items():
-        assert np.array_equal(o[1], ref[1]) and np.array_equal(o[2], ref[2]) and np.array_equal(o[3], ref[3]), path
-        assert np.abs(o[0] - ref[0]).max() <= (1e-4 if dtype == 32 else 1e-11), path
-        assert np.array_equal(o[0][:, 80:], x0[:, 80:].astype(np.float64))               # padding untouched
+        # every path: counts bit-exact on ITS OWN final X, solved flags consistent with them, padding untouched
+        s_own, _ = O.check(inst, o[0], 80)
+        assert np.array_equal(o[1], s_own), path
+        assert np.all(o[2][s_own == inst.n_cons] == 1) and np.all((o[3] >= 0) == (o[2] != 0)), path
+        assert o[2][3] == 1 and o[3][3] == 1, path                                       # the planted candidate
+        assert np.array_equal(o[0][:, 80:], x0[:, 80:].astype(np.float64))
+        if dtype == 64:                                                                  # across paths: identical outcome
+            assert np.array_equal(o[1], ref[1]) and np.array_equal(o[2], ref[2]) and np.array_equal(o[3], ref[3]), path
+            assert np.abs(o[0] - ref[0]).max() <= 1e-11, path
+        else:
+            # fp32: the paths sum partial gradients in different orders and a trajectory can amplify that (see
+            # test_cfg0_free_running_solve_rate), so across paths: the same outcome on (nearly) every candidate
+            assert (o[2] == ref[2]).mean() >= 0.95 and np.quantile(np.abs(o[0] - ref[0]), 0.95) <= 1e-4, path
     if dtype == 64:
         assert np.array_equal(ref[2], solo) and np.array_equal(ref[3], firsto) and np.array_equal(ref[1], sato)
 
