@@ -154,6 +154,28 @@ int afsat_check(afsat_ctx *ctx, const void *d_x, int32_t *d_sat_count, uint8_t *
                 void *stream);
 
 /*
+ * afsat_check_static -- afsat_check for callers that cannot allocate at call time (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid cudaMalloc).  Same inputs, same outputs, bit for bit; the difference is
+ * where the scratch of the check lives: the sign bits [n][ldb/32] of a7 and the per-candidate accumulator [ldb] of a8
+ * are placed in ONE file-scope device array of AFSAT_STATIC_SCRATCH_BYTES that the library carries (every GPU that
+ * loads the library holds those bytes until the process exits), not in the context's workspace.  The call makes no
+ * cudaMalloc / cudaFree and calls no allocating routine: one cudaMemsetAsync and the three kernels of the check on
+ * `stream`, nothing else.
+ *   Needs  ldb * 4 (rounded up to 256) + n_vars * (ldb / 32) * 4  bytes; a context that needs more is refused with
+ *   AFSAT_E_NOMEM and a message that names both numbers (cfg2 of BASELINE.json, n = 5000, B = 4096, needs 2.6 MB).
+ *   afsat_static_setup(device) resolves the array's device address (cudaGetSymbolAddress) once per device; call it
+ *   at set-up -- in particular BEFORE starting a graph capture.  afsat_check_static calls it itself if that has
+ *   not happened yet for the context's device.
+ *   EVERY call on a device shares the one array, whatever the context: the array keeps the last call's contents (the
+ *   entry point clears what has to start at zero), and two calls that overlap on the GPU -- different streams, or
+ *   different contexts on different host threads without ordering between them -- RACE on it.  Order them on one
+ *   stream or with events.  The ordinary afsat_check has no such restriction.
+ */
+#define AFSAT_STATIC_SCRATCH_BYTES (8u << 20)
+int afsat_static_setup(int32_t device);
+int afsat_check_static(afsat_ctx *ctx, const void *d_x, int32_t *d_sat_count, uint8_t *d_is_solution, void *stream);
+
+/*
  * afsat_step -- n_steps iterations of Alg. 1 with a fixed step eta, steps
  * a1-a9 fused, no host round trip between iterations:
  *     G = grad F(X(t-1));  X(t) = clamp(X(t-1) - eta G, -1, +1) on free variables of unsolved

@@ -30,7 +30,9 @@ ERROR_NAMES = {0: "AFSAT_OK", -1: "AFSAT_E_INVALID", -2: "AFSAT_E_LENGTH", -3: "
                -4: "AFSAT_E_SIGN", -5: "AFSAT_E_DUPLICATE", -6: "AFSAT_E_PARAM",
                -7: "AFSAT_E_NOMEM", -8: "AFSAT_E_CUDA", -9: "AFSAT_E_UNSAT"}
 
-EXPORTS = ["afsat_create", "afsat_create_ex", "afsat_probe_peak", "afsat_host_restrict", "afsat_host_tables_mask", "afsat_destroy", "afsat_last_error", "afsat_eval_grad", "afsat_check",
+STATIC_SCRATCH_BYTES = 8 << 20      # AFSAT_STATIC_SCRATCH_BYTES of include/afsat.h
+
+EXPORTS = ["afsat_static_setup", "afsat_check_static", "afsat_create", "afsat_create_ex", "afsat_probe_peak", "afsat_host_restrict", "afsat_host_tables_mask", "afsat_destroy", "afsat_last_error", "afsat_eval_grad", "afsat_check",
            "afsat_step", "afsat_step_host", "afsat_host_tables", "afsat_query", "afsat_version",
            "afsat_set_profiling", "afsat_step_ls", "afsat_parse", "afsat_parse_file", "afsat_parse_error",
            "afsat_problem_sizes", "afsat_problem_fill", "afsat_problem_free", "afsat_restart", "afsat_solve"]
@@ -72,6 +74,10 @@ def load_library():
     L.afsat_eval_grad.argtypes = [vp, vp, vp, vp, vp]
     L.afsat_check.restype = C.c_int
     L.afsat_check.argtypes = [vp, vp, vp, vp, vp]
+    L.afsat_static_setup.restype = C.c_int
+    L.afsat_static_setup.argtypes = [i32]
+    L.afsat_check_static.restype = C.c_int
+    L.afsat_check_static.argtypes = [vp, vp, vp, vp, vp]
     L.afsat_step.restype = C.c_int
     L.afsat_step.argtypes = [vp, vp, dbl, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp]
     L.afsat_step_ls.restype = C.c_int
@@ -122,6 +128,15 @@ def probe_peak(kind: int, device: int = 0) -> float:
     if rc != 0:
         raise AfsatError(rc, L.afsat_last_error(None).decode())
     return float(out.value)
+
+
+def static_setup(device: int = 0) -> None:
+    """afsat_static_setup: resolve the device address of the library's static scratch array on `device` (once per
+    device, at set-up; before any graph capture)."""
+    L = load_library()
+    rc = L.afsat_static_setup(int(device))
+    if rc != 0:
+        raise AfsatError(rc, L.afsat_last_error(None).decode())
 
 
 def host_tables(ctype: int, k: int, param: int, flags: int = 0):
@@ -312,6 +327,16 @@ class Context:
             is_solution = torch.empty(self.B, dtype=torch.uint8, device=x.device)
         rc = self._L.afsat_check(self._h, x.data_ptr(), sat_count.data_ptr(), is_solution.data_ptr(),
                                  _stream_ptr(stream))
+        self._raise(rc)
+        return sat_count, is_solution
+
+    def check_static(self, x, sat_count, is_solution, *, stream=None):
+        """afsat_check_static: the check with its scratch in the library's static device array -- the call allocates
+        nothing, so the caller passes the outputs too ([B] int32, [B] uint8 CUDA tensors).  All calls on a device share
+        the array: order them on the GPU."""
+        self._check_x(x)
+        rc = self._L.afsat_check_static(self._h, x.data_ptr(), sat_count.data_ptr(), is_solution.data_ptr(),
+                                        _stream_ptr(stream))
         self._raise(rc)
         return sat_count, is_solution
 

@@ -6,6 +6,7 @@
 #include <cuda_runtime.h>
 #include <algorithm>
 #include <map>
+#include <mutex>
 #include <new>
 #include <string>
 #include <tuple>
@@ -21,7 +22,16 @@
 
 using namespace afsat;
 
+// ---- scratch of afsat_check_static (include/afsat.h): ONE file-scope device array per GPU that loads the library.
+// In HOST code the name g_static_scratch is a host-side stand-in, not a device address: never hand it to a kernel.
+// afsat_static_setup resolves the device address with cudaGetSymbolAddress, once per device, and the launches get THAT.
+static __device__ __align__(256) unsigned char g_static_scratch[AFSAT_STATIC_SCRATCH_BYTES];
+
 namespace {
+
+constexpr int STATIC_MAX_DEVICES = 64;
+void *g_static_ptr[STATIC_MAX_DEVICES] = {};       // device address of g_static_scratch on device i, or null
+std::mutex g_static_mutex;
 
 thread_local std::string g_create_error;
 
@@ -1204,6 +1214,90 @@ int afsat_check(afsat_ctx *ctx, const void *d_x, int32_t *d_sat_count, uint8_t *
     if (!rc) rc = check_all(ctx, false, st);
     if (rc) return rc;
     k_check_finish<<<(ctx->B + 127) / 128, 128, 0, st>>>(ctx->d_satacc, ctx->B, ctx->m, ctx->d_sat_const, ctx->group_w,
+                                                         (int)ctx->groups.size(), d_sat_count, d_is_solution);
+    ++ctx->launches;
+    CU(cudaPeekAtLastError());
+    return AFSAT_OK;
+}
+
+int afsat_static_setup(int32_t device)
+{
+    afsat_ctx *ctx = nullptr;                                         // errors go to the thread-local message
+    if (device < 0 || device >= STATIC_MAX_DEVICES) return fail(ctx, AFSAT_E_INVALID, "afsat_static_setup: device ordinal out of range");
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (g_static_ptr[device]) return AFSAT_OK;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device >= ndev)
+        return fail(ctx, AFSAT_E_CUDA, "afsat_static_setup: no usable CUDA device (no CPU fallback)");
+    int prev = -1;
+    CU(cudaGetDevice(&prev));
+    CU(cudaSetDevice(device));                                        // the symbol resolves on the CURRENT device
+    void *ptr = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&ptr, g_static_scratch);
+    if (prev >= 0 && prev != device) cudaSetDevice(prev);
+    if (e != cudaSuccess || !ptr)
+        return fail(ctx, AFSAT_E_CUDA, std::string("afsat_static_setup: cudaGetSymbolAddress: ") + cudaGetErrorString(e));
+    g_static_ptr[device] = ptr;
+    return AFSAT_OK;
+}
+
+int afsat_check_static(afsat_ctx *ctx, const void *d_x, int32_t *d_sat_count, uint8_t *d_is_solution, void *stream)
+{
+    if (!ctx) return AFSAT_E_INVALID;
+    if (!d_x || !d_sat_count || !d_is_solution) return fail(ctx, AFSAT_E_INVALID, "afsat_check_static: NULL pointer");
+    if (misaligned(d_x)) return fail(ctx, AFSAT_E_INVALID, "afsat_check_static: d_x must be 16-byte aligned");
+    // layout in the array: satacc [ldb] int32, then (256-byte aligned) the sign bits [n][ldb / 32] uint32
+    const size_t ldw = (size_t)(ctx->ldb / 32);
+    const size_t off_bits = ((size_t)ctx->ldb * sizeof(int32_t) + 255) / 256 * 256;
+    const size_t need = off_bits + (size_t)ctx->n * ldw * sizeof(uint32_t);
+    if (need > (size_t)AFSAT_STATIC_SCRATCH_BYTES) {
+        char buf[200];
+        snprintf(buf, sizeof buf, "afsat_check_static: this context needs %zu bytes of scratch, the static array holds %u "
+                                  "(AFSAT_STATIC_SCRATCH_BYTES); use afsat_check", need, (unsigned)AFSAT_STATIC_SCRATCH_BYTES);
+        return fail(ctx, AFSAT_E_NOMEM, buf);
+    }
+    if (ctx->device < 0 || ctx->device >= STATIC_MAX_DEVICES) return fail(ctx, AFSAT_E_INVALID, "afsat_check_static: device ordinal out of range");
+    if (!g_static_ptr[ctx->device]) {                                 // not set up yet (do it BEFORE a graph capture: header)
+        const int rs = afsat_static_setup(ctx->device);
+        if (rs) return fail(ctx, rs, "afsat_check_static: " + g_create_error);
+    }
+    int rc = set_device(ctx);
+    if (rc) return rc;
+    unsigned char *base = (unsigned char *)g_static_ptr[ctx->device]; // the DEVICE address, never the symbol's host stand-in
+    int32_t *satacc = (int32_t *)base;
+    uint32_t *bits = (uint32_t *)(base + off_bits);
+    cudaStream_t st = (cudaStream_t)stream;
+    // the array keeps whatever the last call (of any context) left: the accumulator has to start at zero; the sign bits are
+    // overwritten in full (every word of every row, padding columns as 0) before they are read
+    CU(cudaMemsetAsync(satacc, 0, (size_t)ctx->ldb * sizeof(int32_t), st));
+    {
+        const unsigned gx = (unsigned)((ctx->ldb + CTA_THREADS - 1) / CTA_THREADS);
+        const unsigned gy = (unsigned)std::min<int64_t>(ctx->n, std::max<int64_t>(1, (int64_t)ctx->sm_count * 8 / gx));
+        if (ctx->dtype == 32) k_pack_signs<float><<<dim3(gx, gy), CTA_THREADS, 0, st>>>((const float *)d_x, bits, ctx->n, ctx->B, ctx->ldb);
+        else k_pack_signs<double><<<dim3(gx, gy), CTA_THREADS, 0, st>>>((const double *)d_x, bits, ctx->n, ctx->B, ctx->ldb);
+        ++ctx->launches;
+        CU(cudaPeekAtLastError());
+    }
+    for (size_t g = 0; g < ctx->groups.size(); ++g) {                 // a8: one launch per partial-assignment group
+        const GroupPlan &gp = ctx->groups[g];
+        const int64_t w_begin = gp.b0 / 32, w_end = (g + 1 == ctx->groups.size()) ? ctx->ldb / 32 : gp.b1 / 32;
+        if (w_end <= w_begin) continue;
+        CheckParams p;
+        p.bits = bits; p.ldw = (int64_t)ldw; p.lits = gp.d_lits; p.sigs = ctx->d_sigs; p.items = gp.d_items;
+        p.satacc = satacc; p.B = ctx->B; p.w_begin = (int32_t)w_begin; p.w_end = (int32_t)w_end;
+        p.step_ctr = nullptr;
+        const int64_t nw = w_end - w_begin;
+        p.wpb = std::min(32, pow2_floor(nw));
+        if (p.wpb < nw && p.wpb < 32) p.wpb *= 2;
+        p.wpb = std::min(p.wpb, 32);
+        p.n_items = gp.n_items;
+        const unsigned gy = (unsigned)((nw + p.wpb - 1) / p.wpb);
+        dim3 grid((unsigned)std::max<int64_t>(1, std::min<int64_t>(std::max(1, gp.n_items), (int64_t)ctx->sm_count * 8 / gy)), gy);
+        k_check_bits<<<grid, CTA_THREADS, 0, st>>>(p);
+        ++ctx->launches;
+        CU(cudaPeekAtLastError());
+    }
+    k_check_finish<<<(ctx->B + 127) / 128, 128, 0, st>>>(satacc, ctx->B, ctx->m, ctx->d_sat_const, ctx->group_w,
                                                          (int)ctx->groups.size(), d_sat_count, d_is_solution);
     ++ctx->launches;
     CU(cudaPeekAtLastError());
