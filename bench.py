@@ -412,7 +412,7 @@ def measure(cfg, dtype, K, W, *, batch=None, scale=1.0, oracle_seconds=10.0, ran
 LTS_BYTES_PER_CLK = 6300.0       # B300_MICROARCH.md "LTS throughput cap ~6300 B/cyc full-chip": the L2's delivery rate
 
 
-def l2_report(inst, ctx, B, kern_ms_per_step, cap):
+def l2_report(inst, ctx, B, kern_ms_per_step, cap, local=0):
     """Second roofline of the evaluation kernels: L2 throughput.  Algorithmic bytes = 4 B gathered + 4 B scatter-added per
     literal and candidate on the table the kernels run (after substitution).  cfg4 (k = 3..5) is bound
     here, not by the FP32 pipe: ~23 flop per byte of L2 traffic at k = 4."""
@@ -420,9 +420,16 @@ def l2_report(inst, ctx, B, kern_ms_per_step, cap):
     peaks = load_peaks()
     alg = 8.0 * ctx.query(Bd.Q_LIVE_NNZ) * B
     cap_gbs = LTS_BYTES_PER_CLK * peaks["sm_max_mhz"] * 1e6 / 1e9
+    rd, red, mix = probed_peak(3, local) * 1e3, probed_peak(4, local) * 1e3, probed_peak(5, local) * 1e3
     out = {"algorithmic_bytes_per_step": alg, "achieved_gbs": alg / (kern_ms_per_step * 1e-3) / 1e9 if kern_ms_per_step > 0 else 0.0,
-           "peak_gbs": cap_gbs, "peak_source": "guide: ~6300 B/clk full-chip LTS cap (B300_MICROARCH.md) x sm_max_mhz; not measured here",
+           "peak_gbs": cap_gbs, "peak_source": "guide: ~6300 B/clk full-chip LTS cap (B300_MICROARCH.md) x sm_max_mhz",
+           "peak_measured": {"load_gbs": rd, "red_gbs": red, "half_and_half_gbs": mix,
+                             "how": "afsat_probe_peak kinds 3 / 4 / 5: 16-byte L1-bypassing loads / red.global.add.v4.f32 / both in equal "
+                                    "parts over a 24 MB L2-resident buffer from every SM, CUDA events, best of 3; the evaluation kernels "
+                                    "move half of their algorithmic bytes each way"},
            "lts_bytes_per_step_measured": cap.get("lts_bytes_per_step_eval_kernels")}
+    if out["peak_measured"]["half_and_half_gbs"]:
+        out["frac_of_measured"] = out["achieved_gbs"] / out["peak_measured"]["half_and_half_gbs"]
     out["frac"] = out["achieved_gbs"] / cap_gbs
     if cap.get("lts_bytes_per_step_eval_kernels") and kern_ms_per_step > 0:
         out["measured_traffic_gbs"] = cap["lts_bytes_per_step_eval_kernels"] / (kern_ms_per_step * 1e-3) / 1e9
@@ -472,7 +479,7 @@ def report(r, world, local, oracle_seconds, rank0_oracle=True):
             "traffic": cap.get("dram_bytes_per_step_eval_kernels"),
             "traffic_whole_step": cap.get("dram_bytes_per_step"),
             "traffic_source": cap.get("traffic_capture"),
-            "l2": l2_report(inst, ctx, B, kern_ms / K, cap),
+            "l2": l2_report(inst, ctx, B, kern_ms / K, cap, local),
             "hbm_floor_bytes_per_step": 2 * n * B * esz, "hbm_peak_gbs": peaks["hbm_gbs"],
             "note": "achieved = ALGORITHMIC flop of the instance as given (SURVEY.md App. D: 12 / 4 FP32 instructions per literal at a "
                     "complex / real DFT point, every retained point) / measured kernel time.  The kernels execute fewer instructions: "
@@ -653,7 +660,8 @@ def main():
     if args.probe_peaks:
         from paper_2606_06641_b200 import build as Build
         Build.build()
-        print(json.dumps({"ffma_tflops": probed_peak(0, 0), "ffma2_tflops": probed_peak(1, 0), "dfma_tflops": probed_peak(2, 0)}))
+        print(json.dumps({"ffma_tflops": probed_peak(0, 0), "ffma2_tflops": probed_peak(1, 0), "dfma_tflops": probed_peak(2, 0),
+                          "l2_load_tbs": probed_peak(3, 0), "l2_red_tbs": probed_peak(4, 0), "l2_half_and_half_tbs": probed_peak(5, 0)}))
         return 0
     if args.impl == "reference":
         return run_reference(args)

@@ -359,9 +359,12 @@ int afsat_problem_fill(const afsat_problem *p, int64_t *row_ptr, int32_t *lit_va
 void afsat_problem_free(afsat_problem *p);
 
 /*
- * afsat_probe_peak -- measured issue rate of the FP pipes the path is bound by (the `alu` roofline denominator of
- * bench.py): kind 0 = scalar FFMA, 1 = packed FFMA2 (fma.rn.f32x2), 2 = DFMA; independent chains, nothing else,
- * timed with CUDA events on `device`.  *tflops receives the best of 5 runs (FMA = 2 flop).  SYNCHRONISES.
+ * afsat_probe_peak -- measured rates of what the path is bound by (the roofline denominators of bench.py), timed with
+ * CUDA events on `device`; SYNCHRONISES.  kind 0 = scalar FFMA, 1 = packed FFMA2 (fma.rn.f32x2), 2 = DFMA: independent
+ * chains, nothing else; *tflops receives the best of 5 runs in TFLOP/s (FMA = 2 flop).  kind 3 = L2 loads (16-byte,
+ * bypassing L1), 4 = L2 vector REDs (red.global.add.v4.f32), 5 = both in equal parts, over a 24 MB L2-resident buffer
+ * from every SM -- the access kinds of the evaluation kernels; *tflops then receives TB/s of payload (best of 3).
+ * The probe allocates its own scratch.
  */
 int afsat_probe_peak(int32_t device, int32_t kind, double *tflops);
 

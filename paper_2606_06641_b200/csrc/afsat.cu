@@ -1478,7 +1478,7 @@ int64_t afsat_query(const afsat_ctx *ctx, int32_t key)
 int afsat_probe_peak(int32_t device, int32_t kind, double *tflops)
 {
     afsat_ctx *ctx = nullptr;
-    if (!tflops || kind < 0 || kind > 2) return fail(ctx, AFSAT_E_INVALID, "afsat_probe_peak: bad arguments");
+    if (!tflops || kind < 0 || kind > 5) return fail(ctx, AFSAT_E_INVALID, "afsat_probe_peak: bad arguments");
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev)
         return fail(ctx, AFSAT_E_CUDA, "afsat_probe_peak: no usable CUDA device (no CPU fallback)");
@@ -1489,6 +1489,28 @@ int afsat_probe_peak(int32_t device, int32_t kind, double *tflops)
     CU(cudaMalloc((void **)&d_out, 64));
     cudaEvent_t e0, e1;
     CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1));
+    if (kind >= 3) {                                                  // L2 delivery rate: a 24 MB buffer, resident in either half of the L2
+        const size_t bytes = (size_t)24 << 20, n_vec = bytes / sizeof(float4);
+        float4 *buf = nullptr;
+        CU(cudaMalloc((void **)&buf, bytes));
+        CU(cudaMemset(buf, 0, bytes));
+        const int iters = 400, blocks = prop.multiProcessorCount * 8;
+        double best = 0.0;
+        for (int rep = 0; rep < 4; ++rep) {
+            CU(cudaEventRecord(e0, 0));
+            if (kind == 3) k_probe_l2<0><<<blocks, 256>>>(buf, n_vec, iters, d_out);
+            else if (kind == 4) k_probe_l2<1><<<blocks, 256>>>(buf, n_vec, iters, d_out);
+            else k_probe_l2<2><<<blocks, 256>>>(buf, n_vec, iters, d_out);
+            CU(cudaEventRecord(e1, 0));
+            CU(cudaEventSynchronize(e1));
+            float ms = 0.f;
+            CU(cudaEventElapsedTime(&ms, e0, e1));
+            if (rep > 0 && ms > 0.f) best = std::max(best, (double)bytes * iters / (ms * 1e-3) / 1e12);
+        }
+        cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d_out); cudaFree(buf);
+        *tflops = best;                                               // TB/s
+        return AFSAT_OK;
+    }
     const int iters = 1 << 14, blocks = prop.multiProcessorCount * 8, threads = 256;
     double best = 0.0;
     for (int rep = 0; rep < 6; ++rep) {

@@ -635,4 +635,27 @@ __global__ void __launch_bounds__(256) k_probe(float *out, int iters, float seed
     }
 }
 
+// kinds 3 / 4 / 5: L2 delivery rate -- every thread walks an L2-resident buffer with 16-byte loads that bypass L1
+// (ld.global.cg), 16-byte vector REDs (red.global.add.v4.f32), or both in turn on two halves of the buffer: the access
+// kinds of the evaluation kernels (a1 gathers, a5 scatter-adds; they move the same number of bytes each way)
+template <int MODE>
+__global__ void __launch_bounds__(256) k_probe_l2(float4 *buf, size_t n_vec, int iters, float *out)
+{
+    const size_t stride = (size_t)gridDim.x * blockDim.x, i0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const size_t half = n_vec / 2;
+    float acc = 0.f;
+    for (int it = 0; it < iters; ++it)
+        for (size_t i = i0; i < (MODE == 2 ? half : n_vec); i += stride) {
+            if (MODE == 1 || MODE == 2)
+                asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(buf + i), "f"(1.0f), "f"(0.5f), "f"(0.25f), "f"(2.0f) : "memory");
+            if (MODE == 0 || MODE == 2) {
+                float4 v;
+                asm volatile("ld.global.cg.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
+                             : "l"(buf + (MODE == 2 ? half : 0) + i) : "memory");
+                acc += v.x + v.y + v.z + v.w;
+            }
+        }
+    if (acc == 12345.678f) out[0] = acc;
+}
+
 }  // namespace afsat
