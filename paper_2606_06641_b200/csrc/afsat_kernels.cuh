@@ -536,7 +536,7 @@ __device__ __forceinline__ void grp_rows_f2_joint(const f32x2 (&y)[K][NP], const
     }
     for (int p = 0; p < n_rows; ++p, rg += ROW2G) {
         const float wr = rg[ROW2G_W], wi = rg[ROW2G_W + 1];
-        const f32x2 bwr = bcf(wr), bwi = bcf(wi), bnwi = bcf(-wi);
+        const f32x2 bwr = bcf(wr), bnwr = bcf(-wr), bnwi = bcf(-wi);
 #pragma unroll
         for (int q = 0; q < NP; ++q) {
             f32x2 q0r = bcf(rg[0]), q0i = bcf(rg[1]), q1r = bcf(rg[ROW2G_G1]), q1i = bcf(rg[ROW2G_G1 + 1]);
@@ -551,8 +551,9 @@ __device__ __forceinline__ void grp_rows_f2_joint(const f32x2 (&y)[K][NP], const
             fe[q] = fma2(bnwi, Pi, fe[q]);                            // Re(w P)
             if (GRAD) {
                 // T0 = w q1 (everything but group 0), T1 = w q0;  A_j += Re(c_j T) = Re c_j Re T - Im c_j Im T
-                const f32x2 t0r = fma2(bwr, q1r, mul2(bnwi, q1i)), nt0i = fma2(bwr, q1i, mul2(bwi, q1r)) ^ SGNP;
-                const f32x2 t1r = fma2(bwr, q0r, mul2(bnwi, q0i)), nt1i = fma2(bwr, q0i, mul2(bwi, q0r)) ^ SGNP;
+                // (-Im T from the negated weight: a broadcast operand, so the negation costs nothing)
+                const f32x2 t0r = fma2(bwr, q1r, mul2(bnwi, q1i)), nt0i = fma2(bnwr, q1i, mul2(bnwi, q1r));
+                const f32x2 t1r = fma2(bwr, q0r, mul2(bnwi, q0i)), nt1i = fma2(bnwr, q0i, mul2(bnwi, q0r));
 #pragma unroll
                 for (int j = 0; j < M0; ++j) {
                     A0[j][q] = fma2(bcf(rg[2 + 2 * j]), t0r, A0[j][q]); A0[j][q] = fma2(bcf(rg[3 + 2 * j]), nt0i, A0[j][q]);
@@ -842,7 +843,7 @@ __device__ __forceinline__ void run_item_f2(const EvalParams<float> &p, const in
 // separately compiled (noinline) function so that every length keeps its own schedule and register
 // allocation while all lengths share one grid (no per-length launch tails) ---------------------------
 template <int K, int NP, bool GRAD, bool CSPLIT>
-__device__ __noinline__ void item_body_f2(const EvalParams<float> &p, const int32_t *s_lits, const f32x2 *s_tab2,
+__device__ __forceinline__ void item_body_f2(const EvalParams<float> &p, const int32_t *s_lits, const f32x2 *s_tab2,
                                           const float *s_tabg, float (*s_F)[64 * NP], int n_real, int n_cplx, int nc, int uv)
 {
     constexpr int V = 2 * NP;
