@@ -919,7 +919,7 @@ __global__ void __launch_bounds__(CTA_THREADS, MINB) k_eval_f2m(const EvalParams
 
 // one body per length, fp64 k <= 8 (everything longer, and fp32 beyond k = 8, runs the lane-split kernels of afsat_split.cuh)
 template <typename T, int K, int V, bool GRAD>
-__device__ __noinline__ void item_body_k(const EvalParams<T> &p, const int32_t *s_lits, const T *s_tab, T (*s_F)[32 * V],
+__device__ __forceinline__ void item_body_k(const EvalParams<T> &p, const int32_t *s_lits, const T *s_tab, T (*s_F)[32 * V],
                                          int n_real, int n_cplx, int nc)
 {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;

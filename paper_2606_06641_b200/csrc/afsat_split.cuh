@@ -311,7 +311,7 @@ __device__ __forceinline__ void run_item_split(const EvalParams<T> &p, unsigned 
 }
 
 template <typename T, int KS, int NS, bool GRAD>
-__device__ __noinline__ void item_body_split(const EvalParams<T> &p, const int32_t *s_lits, const T *s_tab,
+__device__ __forceinline__ void item_body_split(const EvalParams<T> &p, const int32_t *s_lits, const T *s_tab,
                                              T (*s_F)[32], int n_real, int n_cplx, int nc, int k, T pad)
 {
     constexpr int CW = 32 / NS;
@@ -526,7 +526,7 @@ __device__ __forceinline__ void run_item_split2(const EvalParams<float> &p, unsi
 }
 
 template <int KS, int NS, bool GRAD>
-__device__ __noinline__ void item_body_split2(const EvalParams<float> &p, const int32_t *s_lits, const float *s_tab,
+__device__ __forceinline__ void item_body_split2(const EvalParams<float> &p, const int32_t *s_lits, const float *s_tab,
                                               float (*s_F)[64], int n_real, int n_cplx, int nc, int k, float pad)
 {
     constexpr int CW = 32 / NS;
