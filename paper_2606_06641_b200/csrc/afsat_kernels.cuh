@@ -794,7 +794,11 @@ template <> struct PairIO<2> {
     }
 };
 
-template <int K, int NP, bool GRAD, bool PF, int UV>
+// PFD = how many constraints AHEAD of the one being evaluated the gathers are requested (register staging): 0 for the long
+// bodies (k > 5: arithmetic hides the gathers), 1 for k = 4, 5, 2 for k <= 3 -- a k = 3 constraint is ~120 instructions per
+// warp, too little to cover a loaded L2 round trip with one constraint in flight (ncu: the wait for the gathers was the
+// top stall of cfg4's kernel, nearly all of it in the k = 3 body).
+template <int K, int NP, bool GRAD, int PFD, int UV>
 __device__ __forceinline__ void run_item_f2(const EvalParams<float> &p, const int32_t *__restrict__ s_lits,
                                             const f32x2 *__restrict__ s_tab2, const float *__restrict__ s_tabg, int n_real,
                                             int n_cplx, int nc, int wk, int Wk, int64_t b, f32x2 (&fe)[NP])
@@ -803,28 +807,29 @@ __device__ __forceinline__ void run_item_f2(const EvalParams<float> &p, const in
     const char *xb = reinterpret_cast<const char *>(p.x + b);
     char *gb = reinterpret_cast<char *>(p.G + (b - p.g_b0));
     const uint32_t x_ld = (uint32_t)(p.ldb * 4), g_ld = (uint32_t)(p.g_ld * 4);
-    int32_t lit_n[K];
-    f32x2 y_n[K][NP];
-    auto fetch = [&](int c) {
+    constexpr int NB = PFD > 1 ? PFD : 1;                             // staging buffers, used in turn
+    int32_t lit_n[NB][K];
+    f32x2 y_n[NB][K][NP];
+    auto fetch = [&](int c, int32_t (&ln)[K], f32x2 (&yn)[K][NP]) {
         const int32_t *L = s_lits + c * K;
 #pragma unroll
-        for (int i = 0; i < K; ++i) lit_n[i] = L[i];
+        for (int i = 0; i < K; ++i) ln[i] = L[i];
 #pragma unroll
-        for (int i = 0; i < K; ++i) PairIO<NP>::load(xb + (uint64_t)(uint32_t)(lit_n[i] & LIT_VAR) * x_ld, y_n[i]);
+        for (int i = 0; i < K; ++i) PairIO<NP>::load(xb + (uint64_t)(uint32_t)(ln[i] & LIT_VAR) * x_ld, yn[i]);
     };
-    if (PF && wk < nc) fetch(wk);
-    for (int c = wk; c < nc; c += Wk) {
-        if (!PF) fetch(c);
+    // constraint c from its staging buffer; the buffer is then free for constraint c + PFD Wk
+    auto one = [&](int c, int32_t (&ln)[K], f32x2 (&yn)[K][NP]) {
+        if (PFD == 0) fetch(c, ln, yn);
         int32_t lit[K];
         f32x2 y[K][NP], g[K][NP];
 #pragma unroll
         for (int i = 0; i < K; ++i) {
-            lit[i] = lit_n[i];
+            lit[i] = ln[i];
             const uint32_t m = (uint32_t)(lit[i] & LIT_NEG);
 #pragma unroll
-            for (int q = 0; q < NP; ++q) { y[i][q] = y_n[i][q] ^ (((f32x2)m << 32) | m); g[i][q] = 0ull; }   // y = s x
+            for (int q = 0; q < NP; ++q) { y[i][q] = yn[i][q] ^ (((f32x2)m << 32) | m); g[i][q] = 0ull; }   // y = s x
         }
-        if (PF && c + Wk < nc) fetch(c + Wk);
+        if (PFD > 0 && c + PFD * Wk < nc) fetch(c + PFD * Wk, ln, yn);
         eval_points_f2<K, NP, GRAD, UV>(y, s_tab2, s_tabg, n_real, n_cplx, fe, g);
         if (GRAD) {
 #pragma unroll
@@ -836,6 +841,14 @@ __device__ __forceinline__ void run_item_f2(const EvalParams<float> &p, const in
                 PairIO<NP>::red(gb + (uint64_t)(uint32_t)(lit[i] & LIT_VAR) * g_ld, gi);
             }
         }
+    };
+#pragma unroll
+    for (int u = 0; u < PFD; ++u)
+        if (wk + u * Wk < nc) fetch(wk + u * Wk, lit_n[u], y_n[u]);
+    for (int c = wk; c < nc; c += NB * Wk) {
+#pragma unroll
+        for (int u = 0; u < NB; ++u)
+            if (u == 0 || c + u * Wk < nc) one(c + u * Wk, lit_n[u], y_n[u]);
     }
 }
 
@@ -859,7 +872,7 @@ __device__ __forceinline__ void item_body_f2(const EvalParams<float> &p, const i
 #pragma unroll
     for (int q = 0; q < NP; ++q) fe2[q] = 0ull;
     if (active) {
-        constexpr bool PF = K <= 5;
+        constexpr int PF = K <= 3 ? 2 : K <= 5 ? 1 : 0;
         const int c0 = wk * pcs + sub, cstep = p.Wk * pcs;
         if (uv == 1) run_item_f2<K, NP, GRAD, PF, 1>(p, s_lits, s_tab2, s_tabg, n_real, n_cplx, nc, c0, cstep, b, fe2);
         else if (uv == 2) run_item_f2<K, NP, GRAD, PF, 2>(p, s_lits, s_tab2, s_tabg, n_real, n_cplx, nc, c0, cstep, b, fe2);
