@@ -352,6 +352,25 @@ def measure(cfg, dtype, K, W, *, batch=None, scale=1.0, oracle_seconds=10.0, ran
     barrier()
     t_warm = e0.elapsed_time(e1) * 1e-3 * K / K_warm
     launches_warm_call = ctx.query(Bd.Q_KERNEL_LAUNCHES) - l1
+    # ---- afsat_eval_grad alone (a1-a5 into a caller-owned full-width G, F reduced) --------
+    t_eg = None
+    if full or n * ldb * (4 if dtype == 32 else 8) <= (2 << 30):
+        Gfull = torch.empty_like(x)
+        Ffull = torch.empty(B, dtype=x.dtype, device=x.device)
+        K_eg = min(K, 5)
+        ctx.eval_grad(x, Ffull, Gfull)
+        barrier()
+        t_eg = 0.0
+        for t in range(K_eg):
+            flush.fill_(t & 0xFF)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            ctx.eval_grad(x, Ffull, Gfull)
+            e1.record(stream)
+            barrier()
+            t_eg += e0.elapsed_time(e1) * 1e-3
+        t_eg = t_eg * K / K_eg
+        del Gfull, Ffull
     # ---- kernels of a step, timed with events inside the library (a second pass of K flushed steps) ----
     path = ctx.query(Bd.Q_STEP_PATH)
     kern_ms = upd_ms = chk_ms = 0.0
@@ -399,11 +418,13 @@ def measure(cfg, dtype, K, W, *, batch=None, scale=1.0, oracle_seconds=10.0, ran
         t_ls = e0.elapsed_time(e1) * 1e-3
         del xl
     esz = 4 if dtype == 32 else 8
-    t_total, t_warm, t_e2e, kern_ms, upd_ms, chk_ms = reduce_max([t_total, t_warm, t_e2e, kern_ms, upd_ms, chk_ms], device="cuda")
+    t_total, t_warm, t_e2e, kern_ms, upd_ms, chk_ms, t_eg_r = reduce_max([t_total, t_warm, t_e2e, kern_ms, upd_ms, chk_ms,
+                                                                          t_eg if t_eg is not None else 0.0], device="cuda")
+    t_eg = t_eg_r if t_eg is not None else None
     out = {"inst": inst, "x0": x0, "ctx": ctx, "K": K, "W": W, "dtype": dtype, "cfg": cfg, "t_total": t_total, "t_warm": t_warm,
            "t_e2e": t_e2e, "kern_ms": kern_ms, "upd_ms": upd_ms, "chk_ms": chk_ms, "kern_launches": kern_launches,
            "launches": launches, "launches_warm_call": launches_warm_call, "K_warm": K_warm, "clocks": clocks, "wall": wall,
-           "h2d": n * ldb * esz, "d2h": n * ldb * esz + B * (esz + 4 + 1 + 4), "t_ls": t_ls, "path": path,
+           "h2d": n * ldb * esz, "d2h": n * ldb * esz + B * (esz + 4 + 1 + 4), "t_ls": t_ls, "t_eg": t_eg, "path": path,
            "solved": int(sol.sum().item()), "scale": scale}
     del x, flush
     return out
@@ -414,8 +435,9 @@ LTS_BYTES_PER_CLK = 6300.0       # B300_MICROARCH.md "LTS throughput cap ~6300 B
 
 def l2_report(inst, ctx, B, kern_ms_per_step, cap, local=0):
     """Second roofline of the evaluation kernels: L2 throughput.  Algorithmic bytes = 4 B gathered + 4 B scatter-added per
-    literal and candidate on the table the kernels run (after substitution).  cfg4 (k = 3..5) is bound
-    here, not by the FP32 pipe: ~23 flop per byte of L2 traffic at k = 4."""
+    literal and candidate on the table the kernels run (after substitution).  Reported beside the ALU
+    roofline because cfg4 (k = 3..5, ~7 flop per byte of L2 traffic) sits close to both; which of them binds is settled by
+    experiment in DESIGN.md 6.7, not by this ratio."""
     from paper_2606_06641_b200 import binding as Bd
     peaks = load_peaks()
     alg = 8.0 * ctx.query(Bd.Q_LIVE_NNZ) * B
@@ -487,9 +509,11 @@ def report(r, world, local, oracle_seconds, rank0_oracle=True):
                     "groups (k >= 21), and a partial assignment is substituted before anything is evaluated (frac_after_substitution "
                     "counts the model on the substituted table); measured_pipe_utilisation is what ncu saw executed"}
     l2 = roof["l2"]
-    roof["limited_by"] = ("l2 throughput: the measured L2 traffic of the evaluation kernels runs at %.0f %% of the L2's delivery rate "
-                          "(roofline.l2, DESIGN.md 6.7)" % (100 * l2["measured_traffic_frac_of_peak"])
-                          if l2.get("measured_traffic_frac_of_peak", 0) >= 0.75 else "fp pipe / issue (roofline.measured_pipe_utilisation)")
+    roof["limited_by"] = ("instruction issue at the occupancy the register file allows (roofline.measured_pipe_utilisation; DESIGN.md 6.7: "
+                          "in three A/B experiments the kernel time followed the executed-instruction count, not the L2 traffic)")
+    if l2.get("measured_traffic_frac_of_peak"):
+        roof["limited_by"] += "; measured L2 traffic of the evaluation kernels at %.0f %% of the guide's L2 cap" % (
+            100 * l2["measured_traffic_frac_of_peak"])
     if dtype == 64:
         roof["fp64_peak"] = probed_peak(2, local)
         roof["frac_of_fp64_peak"] = ach_tf / max(probed_peak(2, local), 1e-9)
@@ -524,6 +548,10 @@ def report(r, world, local, oracle_seconds, rank0_oracle=True):
            "value_l2_warm": world * m * B * K / r["t_warm"], "ms_per_step_l2_warm": 1e3 * r["t_warm"] / K,
            "l2_warm_call": {"n_steps": r["K_warm"], "launches": int(r["launches_warm_call"])},
            "solved_candidates": r["solved"], "wall_s_timed_region": r["wall"]}
+    if r.get("t_eg"):
+        out["eval_grad_alone"] = {"ms_per_call": 1e3 * r["t_eg"] / K, "value": world * m * B * K / r["t_eg"], "unit": UNIT,
+                                  "note": "afsat_eval_grad on its own: F and a caller-owned full-width G (memset + a1-a5 + the "
+                                          "fixed-order reduction of F), L2 flushed between calls; the fused step adds a6-a9"}
     if r["t_ls"] is not None:
         out["line_search"] = {"ms_per_step": 1e3 * r["t_ls"] / K,
                               "note": "afsat_step_ls: 1 FE+grad evaluation + max_trials objective-only "
@@ -606,6 +634,8 @@ def run_ours(args):
             rp = report(rc, 1, local, args.per_config_oracle_seconds)
             keep = {k_: rp[k_] for k_ in ("ms_per_step", "value", "ms_per_step_l2_warm", "value_l2_warm", "l2_warm_call", "step_path",
                                           "gpu_launches", "deviation_vs_oracle", "clocks", "solved_candidates")}
+            if "eval_grad_alone" in rp:
+                keep["eval_grad_alone"] = {k_: rp["eval_grad_alone"][k_] for k_ in ("ms_per_call", "value")}
             keep["steps"] = Kc
             keep["e2e"] = {k_: rp["e2e"][k_] for k_ in ("value", "ms_per_step")}
             keep["cpu_baseline"] = {k_: rp["cpu_baseline"][k_] for k_ in ("value", "cores", "sample")}
