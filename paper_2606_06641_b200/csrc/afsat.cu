@@ -943,12 +943,12 @@ int afsat_create_ex(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64
     const int64_t span = G > 1 ? group_w : ldb;                        // columns a tile sequence has to cover
     int64_t tile_w = span;
     {
-        // X and G tiles: 13/16 of L2 (cfg4: 128 candidates, 102 MB).  Measured with ncu (profiles/r2_traffic_cfg4.md): at that
-        // width the tiles do NOT stay resident -- 44 GB of DRAM traffic per step where X once is 6.6 GB (the L2 is two halves,
-        // one per die, and lines touched from both dies occupy both) -- while tiles of 64 candidates do (12 GB); yet 128 is
-        // the faster width, 20.3 against 21.9 ms per step: the evaluation of such short constraints is bound by L2
-        // THROUGHPUT (2.8 GB of gathers, REDs and inter-die traffic per tile, 10.7 of the ~12.4 TB/s the L2 delivers), the
-        // DRAM traffic hides under it, and the wider tile halves the per-CTA staging of the literal lists.
+        // X and G tiles: 13/16 of L2 (cfg4: 128 candidates, 102 MB).  Measured with ncu (profiles/r2_launches_cfg4.md): at that
+        // width the tiles do NOT stay resident -- 26 GB of DRAM traffic per step where X once is 6.6 GB (the L2 is two halves,
+        // one per die, and lines touched from both dies occupy both) -- while tiles of 64 candidates do; yet 128 is the
+        // faster width, 17.4 against 21.4 ms per step: the evaluation of such short constraints is bound by instruction
+        // issue, the DRAM traffic hides under it, and the wider tile halves the per-CTA staging of the
+        // literal lists.
         const int64_t budget = opt.l2_budget_bytes > 0 ? opt.l2_budget_bytes : l2_bytes / 16 * 13;
         const int64_t per_col = (int64_t)2 * n_vars * (int64_t)esz;
         // a working set within a few budgets is better left whole: the L2 misses hide behind the arithmetic, the small
