@@ -946,7 +946,7 @@ int afsat_create_ex(afsat_ctx **out, int32_t n_vars, int32_t n_cons, const int64
         // X and G tiles: 13/16 of L2 (cfg4: 128 candidates, 102 MB).  Measured with ncu (profiles/r2_launches_cfg4.md): at that
         // width the tiles do NOT stay resident -- 26 GB of DRAM traffic per step where X once is 6.6 GB (the L2 is two halves,
         // one per die, and lines touched from both dies occupy both) -- while tiles of 64 candidates do; yet 128 is the
-        // faster width, 17.4 against 21.4 ms per step: the evaluation of such short constraints is bound by instruction
+        // faster width, 17.4 against 18.0 ms per step (256: 20.0): the evaluation of such short constraints is bound by instruction
         // issue, the DRAM traffic hides under it, and the wider tile halves the per-CTA staging of the
         // literal lists.
         const int64_t budget = opt.l2_budget_bytes > 0 ? opt.l2_budget_bytes : l2_bytes / 16 * 13;
