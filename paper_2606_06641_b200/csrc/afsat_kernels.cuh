@@ -519,7 +519,10 @@ __device__ __forceinline__ void loo_f2(const f32x2 (*y)[NP], const f32x2 (&A)[M]
 constexpr int ROW2G_G1 = ROW2G_G1_H, ROW2G_W = ROW2G_W_H, ROW2G = ROW2G_H;
 
 // all generic complex rows of a signature for the K literals of a lane (K >= 2), two groups
-template <int K, int NP, bool GRAD>
+// ROLLED: the loop over the DFT points is kept as it is written (the compiler's two-fold unrolling pays for itself with a
+// dozen register-renaming moves per constraint: with four candidates per lane cfg4 17.38 -> 17.2 ms per step; with two
+// candidates per lane the unrolled form is the faster one, cfg1)
+template <int K, int NP, bool GRAD, bool ROLLED>
 __device__ __forceinline__ void grp_rows_f2_joint(const f32x2 (&y)[K][NP], const float *__restrict__ rg, int n_rows, f32x2 (&fe)[NP],
                                             f32x2 (&g)[K][NP])
 {
@@ -534,7 +537,7 @@ __device__ __forceinline__ void grp_rows_f2_joint(const f32x2 (&y)[K][NP], const
 #pragma unroll
         for (int j = 0; j < M1; ++j) A1[j][q] = 0ull;
     }
-    for (int p = 0; p < n_rows; ++p, rg += ROW2G) {
+    auto row = [&](const float *__restrict__ rg) {
         const float wr = rg[ROW2G_W], wi = rg[ROW2G_W + 1];
         const f32x2 bwr = bcf(wr), bnwr = bcf(-wr), bnwi = bcf(-wi);
 #pragma unroll
@@ -565,6 +568,12 @@ __device__ __forceinline__ void grp_rows_f2_joint(const f32x2 (&y)[K][NP], const
                 }
             }
         }
+    };
+    if constexpr (ROLLED) {
+#pragma unroll 1
+        for (int p = 0; p < n_rows; ++p, rg += ROW2G) row(rg);
+    } else {
+        for (int p = 0; p < n_rows; ++p, rg += ROW2G) row(rg);
     }
     if (GRAD) {
         loo_f2<M0, NP>(&y[0], A0, &g[0]);
@@ -580,7 +589,7 @@ __device__ __forceinline__ void grp_rows_f2(const f32x2 (&y)[K][NP], const float
                                             f32x2 (&g)[K][NP])
 {
     if constexpr (NP == 1 || K < AFSAT_F2_SEQ_MINK) {
-        grp_rows_f2_joint<K, NP, GRAD>(y, rg, n_rows, fe, g);
+        grp_rows_f2_joint<K, NP, GRAD, NP == 2>(y, rg, n_rows, fe, g);
     } else {
 #pragma unroll
         for (int q = 0; q < NP; ++q) {
@@ -588,7 +597,7 @@ __device__ __forceinline__ void grp_rows_f2(const f32x2 (&y)[K][NP], const float
 #pragma unroll
             for (int i = 0; i < K; ++i) { y1[i][0] = y[i][q]; g1[i][0] = g[i][q]; }
             fe1[0] = fe[q];
-            grp_rows_f2_joint<K, 1, GRAD>(y1, rg, n_rows, fe1, g1);
+            grp_rows_f2_joint<K, 1, GRAD, true>(y1, rg, n_rows, fe1, g1);
 #pragma unroll
             for (int i = 0; i < K; ++i) g[i][q] = g1[i][0];
             fe[q] = fe1[0];
