@@ -71,7 +71,9 @@ __global__ void __launch_bounds__(CTA_THREADS) k_update(T *__restrict__ x, T *__
             const int v = v0 + u * stride;
             if (v < n) {
                 g[u] = *reinterpret_cast<const VT *>(G + (int64_t)v * g_ld + (b - g_b0));
-                xv[u] = *reinterpret_cast<const VT *>(x + (int64_t)v * ldb + b);
+                xv[u] = __ldcs(reinterpret_cast<const VT *>(x + (int64_t)v * ldb + b));   // X streams through (evict-first): it is not
+                                                                                          // needed again before the next step, and the
+                                                                                          // gradient scratch stays in the L2 instead
                 fx[u] = fixed[v];
             }
         }
@@ -97,7 +99,7 @@ __global__ void __launch_bounds__(CTA_THREADS) k_update(T *__restrict__ x, T *__
                     xs[j] = nx;
                     nib |= (uint32_t)(live[j] && (nx < T(0))) << j;
                 }
-                if (any_upd && !fx[u]) *reinterpret_cast<VT *>(x + (int64_t)v * ldb + b) = vec_make(xs);
+                if (any_upd && !fx[u]) __stcs(reinterpret_cast<VT *>(x + (int64_t)v * ldb + b), vec_make(xs));
                 const uint32_t w = __reduce_or_sync(wmask, nib << sh);
                 if (lane % LPW == 0) bits[(int64_t)v * ldw + (b >> 5)] = w;
             }
