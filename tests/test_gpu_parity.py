@@ -296,6 +296,32 @@ def test_check_bit_exact(dtype):
     assert np.array_equal(so, R.recount(inst, x, 200))
 
 
+@pytest.mark.parametrize("B", [100, 1024])
+def test_check_every_countless_predicate_and_length(B):
+    """k_check_bits runs items whose predicate needs no count (any / none / all / not all / not-all-equal / parity) and whose
+    length is <= 8 through loops specialised on length and combination: every such (predicate, k) pair, plus the same
+    predicates beyond k = 8 (general routine), against the oracle's count and the independent recount -- also on the
+    words of candidates where every variable is True, every variable is False, and at the ties x = 0 / -0.0."""
+    rng = np.random.default_rng(97)
+    groups = []
+    for k in list(range(1, 9)) + [9, 13]:
+        rep = np.full(12, k)
+        groups += [(I.OR, rep, np.zeros(12)), (I.ATLEAST, rep, np.full(12, k)), (I.ATMOST, rep, np.zeros(12)),
+                   (I.ATMOST, rep, np.full(12, k - 1)), (I.XOR, rep, np.zeros(12)), (I.XOR, rep, np.ones(12)),
+                   (I.EXACTLY, rep, np.full(12, k)), (I.EXACTLY, rep, np.zeros(12)), (I.ATLEAST, rep, np.ones(12))]
+        if k >= 2:
+            groups.append((I.NAE, rep, np.zeros(12)))
+    inst = I._assemble("countless", 40, groups, rng, batch=B, eta=0.1, steps=1)
+    x = I.make_x0(inst, seed=5, batch=B)
+    x[:, 0] = -1.0; x[:, 1] = 1.0; x[:, 2] = 0.0; x[:, 3] = -0.0
+    x[::2, 4] = -1.0; x[1::2, 4] = 1.0
+    ctx = Bd.Context.from_instance(inst, batch=B, ldb=x.shape[1])
+    sat, sol = ctx.check(dev(x))
+    so, lo = O.check(inst, x.astype(np.float64), B)
+    assert np.array_equal(sat.cpu().numpy(), so) and np.array_equal(sol.cpu().numpy(), lo)
+    assert np.array_equal(so, R.recount(inst, x, B))
+
+
 def test_check_planted_solution():
     base = I.make_mixed(n=64, m=300, kmin=2, kmax=16, seed=29, batch=64, with_fixed=True)
     base.meta["admissible"] = [R.admissible_taus(int(t), int(k), int(p)) or [0]
