@@ -314,10 +314,17 @@ def measure(cfg, dtype, K, W, *, batch=None, scale=1.0, oracle_seconds=10.0, ran
 
     state = None
     sol = None
+    # The timed step delivers the objective too: F_pre = F(X(t-1)), the contraction a3 of the very products the gradient is
+    # made of (one "eval" of the metric = the value AND all k partials of a constraint).  Without it afsat_step runs the
+    # gradient-only form of the packed kernels; that is measured beside it (step_without_objective).  The one-launch loop of
+    # small instances (cfg0) never evaluates the objective, so there the request would only switch the path.
+    persistent = ctx.query(Bd.Q_STEP_PATH) == Bd.STEP_PERSISTENT
+    F_pre_dev = None if persistent else torch.empty(B, dtype=x.dtype, device=x.device)
 
-    def one_step(t):
+    def one_step(t, with_objective=True):
         nonlocal state, sol
-        _, _, sol, first = ctx.step(x, inst.eta, 1, step_base=t, state=state, want_F=False)
+        _, _, sol, first = ctx.step(x, inst.eta, 1, step_base=t, state=state, want_F=False,
+                                    F_pre=F_pre_dev if with_objective else None)
         state = (sol, first)
 
     for t in range(W):
@@ -340,6 +347,20 @@ def measure(cfg, dtype, K, W, *, batch=None, scale=1.0, oracle_seconds=10.0, ran
     launches = ctx.query(Bd.Q_KERNEL_LAUNCHES) - l0
     clocks = sampler.stop()
     t_total = sum(a.elapsed_time(b) for a, b in ev) * 1e-3
+    # ---- the same K flushed steps with no objective requested (gradient-only kernels) ----------------------
+    t_nof = None
+    if F_pre_dev is not None:
+        ev2 = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+        one_step(W + K, with_objective=False)
+        flush.fill_(1)
+        barrier()
+        for t in range(K):
+            ev2[t][0].record(stream)
+            one_step(W + K + 1 + t, with_objective=False)
+            ev2[t][1].record(stream)
+            flush.fill_(t & 0xFF)
+        barrier()
+        t_nof = sum(a.elapsed_time(b) for a, b in ev2) * 1e-3
     # ---- back-to-back (L2-warm) variant: what a solver run sees (ONE call; cfg0: its own 200 steps) -------
     K_warm = max(K, inst.steps) if cfg == 0 else K
     ctx.step(x, inst.eta, min(K_warm, 3), step_base=W + K, state=state, want_F=False)
@@ -418,13 +439,15 @@ def measure(cfg, dtype, K, W, *, batch=None, scale=1.0, oracle_seconds=10.0, ran
         t_ls = e0.elapsed_time(e1) * 1e-3
         del xl
     esz = 4 if dtype == 32 else 8
-    t_total, t_warm, t_e2e, kern_ms, upd_ms, chk_ms, t_eg_r = reduce_max([t_total, t_warm, t_e2e, kern_ms, upd_ms, chk_ms,
-                                                                          t_eg if t_eg is not None else 0.0], device="cuda")
+    t_total, t_warm, t_e2e, kern_ms, upd_ms, chk_ms, t_eg_r, t_nof_r = reduce_max(
+        [t_total, t_warm, t_e2e, kern_ms, upd_ms, chk_ms, t_eg if t_eg is not None else 0.0, t_nof if t_nof is not None else 0.0],
+        device="cuda")
     t_eg = t_eg_r if t_eg is not None else None
+    t_nof = t_nof_r if t_nof is not None else None
     out = {"inst": inst, "x0": x0, "ctx": ctx, "K": K, "W": W, "dtype": dtype, "cfg": cfg, "t_total": t_total, "t_warm": t_warm,
            "t_e2e": t_e2e, "kern_ms": kern_ms, "upd_ms": upd_ms, "chk_ms": chk_ms, "kern_launches": kern_launches,
            "launches": launches, "launches_warm_call": launches_warm_call, "K_warm": K_warm, "clocks": clocks, "wall": wall,
-           "h2d": n * ldb * esz, "d2h": n * ldb * esz + B * (esz + 4 + 1 + 4), "t_ls": t_ls, "t_eg": t_eg, "path": path,
+           "h2d": n * ldb * esz, "d2h": n * ldb * esz + B * (esz + 4 + 1 + 4), "t_ls": t_ls, "t_eg": t_eg, "t_nof": t_nof, "path": path,
            "solved": int(sol.sum().item()), "scale": scale}
     del x, flush
     return out
@@ -548,6 +571,13 @@ def report(r, world, local, oracle_seconds, rank0_oracle=True):
            "value_l2_warm": world * m * B * K / r["t_warm"], "ms_per_step_l2_warm": 1e3 * r["t_warm"] / K,
            "l2_warm_call": {"n_steps": r["K_warm"], "launches": int(r["launches_warm_call"])},
            "solved_candidates": r["solved"], "wall_s_timed_region": r["wall"]}
+    out["objective_in_timed_step"] = ("F(X(t-1)) delivered by every timed step (F_pre: a3 of the same products as the gradient)"
+                                      if r.get("t_nof") else "not evaluated: the one-launch loop of small instances computes gradients only")
+    if r.get("t_nof"):
+        out["step_without_objective"] = {"ms_per_step": 1e3 * r["t_nof"] / K, "value": world * m * B * K / r["t_nof"], "unit": UNIT,
+                                         "note": "afsat_step with no objective requested (what the fixed-step search of Alg. 1 needs: "
+                                                 "X(t), counts, flags): the packed kernels run their gradient-only form, which drops "
+                                                 "the contraction a3; value_l2_warm (K steps in ONE call) is measured this way too"}
     if r.get("t_eg"):
         out["eval_grad_alone"] = {"ms_per_call": 1e3 * r["t_eg"] / K, "value": world * m * B * K / r["t_eg"], "unit": UNIT,
                                   "note": "afsat_eval_grad on its own: F and a caller-owned full-width G (memset + a1-a5 + the "
@@ -636,6 +666,9 @@ def run_ours(args):
                                           "gpu_launches", "deviation_vs_oracle", "clocks", "solved_candidates")}
             if "eval_grad_alone" in rp:
                 keep["eval_grad_alone"] = {k_: rp["eval_grad_alone"][k_] for k_ in ("ms_per_call", "value")}
+            keep["objective_in_timed_step"] = rp["objective_in_timed_step"]
+            if "step_without_objective" in rp:
+                keep["step_without_objective"] = {k_: rp["step_without_objective"][k_] for k_ in ("ms_per_step", "value")}
             keep["steps"] = Kc
             keep["e2e"] = {k_: rp["e2e"][k_] for k_ in ("value", "ms_per_step")}
             keep["cpu_baseline"] = {k_: rp["cpu_baseline"][k_] for k_ in ("value", "cores", "sample")}

@@ -203,18 +203,26 @@ void prof_drain(afsat_ctx *c, bool keep)
 }
 
 // ---- kernel selection per length class ------------------------------------------------------------------------------
+// grad: 0 = objective only, 1 = objective + gradient, 2 = gradient only (the packed fp32 kernel drops the contraction a3 when
+// no partial objective is asked for, which is every afsat_step without F_pre; the other kernels take 2 as 1)
 template <typename T>
-void (*pick_kernel(int cls, bool grad, bool csplit))(EvalParams<T>)
+void (*pick_kernel(int cls, int grad, bool csplit))(EvalParams<T>)
 {
     using Fn = void (*)(EvalParams<T>);
     if constexpr (sizeof(T) == 4) {
         switch (cls) {
         case CLS_S:
-            if (csplit) return grad ? (Fn)k_eval_f2m<1, AFSAT_S_KMAX, 2, true, 2, true> : (Fn)k_eval_f2m<1, AFSAT_S_KMAX, 2, false, 2, true>;
-            return grad ? (Fn)k_eval_f2m<1, AFSAT_S_KMAX, 2, true, 2, false> : (Fn)k_eval_f2m<1, AFSAT_S_KMAX, 2, false, 2, false>;
+            if (csplit) return grad == 2 ? (Fn)k_eval_f2m<1, AFSAT_S_KMAX, 2, 2, 2, true> : grad ? (Fn)k_eval_f2m<1, AFSAT_S_KMAX, 2, 1, 2, true>
+                                                                                                 : (Fn)k_eval_f2m<1, AFSAT_S_KMAX, 2, 0, 2, true>;
+            return grad == 2 ? (Fn)k_eval_f2m<1, AFSAT_S_KMAX, 2, 2, 2, false> : grad ? (Fn)k_eval_f2m<1, AFSAT_S_KMAX, 2, 1, 2, false>
+                                                                                      : (Fn)k_eval_f2m<1, AFSAT_S_KMAX, 2, 0, 2, false>;
         case CLS_A:
-            if (csplit) return grad ? (Fn)k_eval_f2m<AFSAT_S_KMAX + 1, AFSAT_A_KMAX, 1, true, 2, true> : (Fn)k_eval_f2m<AFSAT_S_KMAX + 1, AFSAT_A_KMAX, 1, false, 2, true>;
-            return grad ? (Fn)k_eval_f2m<AFSAT_S_KMAX + 1, AFSAT_A_KMAX, 1, true, 2, false> : (Fn)k_eval_f2m<AFSAT_S_KMAX + 1, AFSAT_A_KMAX, 1, false, 2, false>;
+            if (csplit) return grad == 2 ? (Fn)k_eval_f2m<AFSAT_S_KMAX + 1, AFSAT_A_KMAX, 1, 2, 2, true>
+                                 : grad ? (Fn)k_eval_f2m<AFSAT_S_KMAX + 1, AFSAT_A_KMAX, 1, 1, 2, true>
+                                        : (Fn)k_eval_f2m<AFSAT_S_KMAX + 1, AFSAT_A_KMAX, 1, 0, 2, true>;
+            return grad == 2 ? (Fn)k_eval_f2m<AFSAT_S_KMAX + 1, AFSAT_A_KMAX, 1, 2, 2, false>
+                      : grad ? (Fn)k_eval_f2m<AFSAT_S_KMAX + 1, AFSAT_A_KMAX, 1, 1, 2, false>
+                             : (Fn)k_eval_f2m<AFSAT_S_KMAX + 1, AFSAT_A_KMAX, 1, 0, 2, false>;
         case CLS_B: return grad ? (Fn)k_eval_split<float, AFSAT_A_KMAX + 1, AFSAT_B_KMAX, 2, 2, true, AFSAT_M32_THREADS, AFSAT_M32_MINB>
                                 : (Fn)k_eval_split<float, AFSAT_A_KMAX + 1, AFSAT_B_KMAX, 2, 2, false, AFSAT_M32_THREADS, AFSAT_M32_MINB>;
         default:    return grad ? (Fn)k_eval_split<float, AFSAT_L32_KMIN, AFSAT_MAX_LEN, AFSAT_L32_NS, 1, true, AFSAT_L32_THREADS, AFSAT_L32_MINB>
@@ -243,7 +251,7 @@ int launch_eval(afsat_ctx *ctx, const GroupPlan &gp, const T *x, T *G, int64_t g
     p.rowsg = (const T *)ctx->d_rowsg; p.rows2g = ctx->d_rows2g;
     p.skip = ctx->cur_skip;
     p.B = ctx->B; p.ldb = ctx->ldb; p.b_begin = b_begin; p.b_end = std::min<int64_t>(b_begin + width, ctx->ldb);
-    const bool grad = G != nullptr;
+    const int grad = G == nullptr ? 0 : Fpart == nullptr ? 2 : 1;
     // The length classes are independent (they only share the RED target), so their launches run
     // CONCURRENTLY: the first active class on the caller's stream, the others on forked side streams that join back.
     int n_active = 0;
@@ -333,8 +341,8 @@ int reduce_F(afsat_ctx *ctx, T *F, cudaStream_t st)
     for (const GroupPlan &gp : ctx->groups) {
         const int64_t b1 = std::min<int64_t>(gp.b1, ctx->B);
         if (b1 <= gp.b0) continue;
-        k_reduce_F<T><<<(unsigned)((b1 - gp.b0 + 127) / 128), 128, 0, st>>>((const T *)ctx->d_Fpart, gp.n_items, ctx->ldb, gp.b0, b1,
-                                                                           gp.F_const, F, ctx->cur_skip);
+        k_reduce_F<T><<<(unsigned)((b1 - gp.b0 + 31) / 32), 32 * RED_F_SLICES, 0, st>>>((const T *)ctx->d_Fpart, gp.n_items, ctx->ldb, gp.b0,
+                                                                                      b1, gp.F_const, F, ctx->cur_skip);
         ++ctx->launches;
         CU(cudaPeekAtLastError());
     }

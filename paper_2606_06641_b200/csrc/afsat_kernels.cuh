@@ -337,7 +337,7 @@ constexpr f32x2 NEGP = 0x8000000080000000ull;
 
 // The unit rows of a signature are walked TOGETHER (HP: w = 1, HM: w = -1, HI: w = i): each is a serial
 // chain of dependent FFMA2s, so interleaving them is what keeps the FMA pipe fed at 4 warps per scheduler.
-template <int K, int NP, bool HP, bool HM, bool HI, bool GRAD>
+template <int K, int NP, bool HP, bool HM, bool HI, int GRAD>
 __device__ __forceinline__ void unit_rows_f2(const f32x2 (&y)[K][NP], const f32x2 *__restrict__ rP, const f32x2 *__restrict__ rM,
                                              const f32x2 *__restrict__ rI, f32x2 (&fe)[NP], f32x2 (&g)[K][NP])
 {
@@ -369,6 +369,7 @@ __device__ __forceinline__ void unit_rows_f2(const f32x2 (&y)[K][NP], const f32x
         }
 #pragma unroll
     for (int q = 0; q < NP; ++q) {
+        if (GRAD == 2) break;                                                        // gradient only
         if (HP) fe[q] = fma2(bc(rP, 2), runP[q], fe[q]);
         if (HM) fe[q] = fma2(bc(rM, 2), runM[q], fe[q]);
         if (HI) { fe[q] = fma2(bc(rI, 6), rr[q], fe[q]); fe[q] = fma2(bc(rI, 7), ri[q], fe[q]); }   // + wr Re P - wi Im P
@@ -411,7 +412,7 @@ __device__ __forceinline__ void unit_rows_f2(const f32x2 (&y)[K][NP], const f32x
 //   T <- (Re T + z (Re T + Im T)) + i (Im T + z (Im T - Re T)),      g_i += Re P_i Re T_i + Im P_i Im T_i
 // Its partner w' = (-1 + i)/sqrt 2 = -conj(w) is the same walk at -y with conjugated weights (the row is staged
 // that way): prod (1 + w' y_j) = conj( prod (1 + w (-y_j)) ).  cz = +-1/sqrt 2 selects the row.
-template <int K, int NP, bool GRAD>
+template <int K, int NP, int GRAD>
 __device__ __forceinline__ void oct_row_f2(const f32x2 (&y)[K][NP], const f32x2 *__restrict__ r, float cz, f32x2 (&fe)[NP],
                                            f32x2 (&g)[K][NP])
 {
@@ -432,7 +433,7 @@ __device__ __forceinline__ void oct_row_f2(const f32x2 (&y)[K][NP], const f32x2 
             rr[q] = fma2(z[i][q], d, rr[q]); ri[q] = fma2(z[i][q], s, ri[q]);
         }
 #pragma unroll
-    for (int q = 0; q < NP; ++q) { fe[q] = fma2(bc(r, 6), rr[q], fe[q]); fe[q] = fma2(bc(r, 7), ri[q], fe[q]); }
+    for (int q = 0; q < NP; ++q) if (GRAD != 2) { fe[q] = fma2(bc(r, 6), rr[q], fe[q]); fe[q] = fma2(bc(r, 7), ri[q], fe[q]); }
     if (GRAD) {
         f32x2 tr[NP], ti[NP];                                                         // conjugated suffix, seeded from the row
 #pragma unroll
@@ -522,7 +523,7 @@ constexpr int ROW2G_G1 = ROW2G_G1_H, ROW2G_W = ROW2G_W_H, ROW2G = ROW2G_H;
 // ROLLED: the loop over the DFT points is kept as it is written (the compiler's two-fold unrolling pays for itself with a
 // dozen register-renaming moves per constraint: with four candidates per lane cfg4 17.38 -> 17.2 ms per step; with two
 // candidates per lane the unrolled form is the faster one, cfg1)
-template <int K, int NP, bool GRAD, bool ROLLED>
+template <int K, int NP, int GRAD, bool ROLLED>
 __device__ __forceinline__ void grp_rows_f2_joint(const f32x2 (&y)[K][NP], const float *__restrict__ rg, int n_rows, f32x2 (&fe)[NP],
                                             f32x2 (&g)[K][NP])
 {
@@ -549,9 +550,11 @@ __device__ __forceinline__ void grp_rows_f2_joint(const f32x2 (&y)[K][NP], const
             for (int j = 0; j < M1; ++j) {
                 q1r = fma2(bcf(rg[ROW2G_G1 + 2 + 2 * j]), e1[j][q], q1r); q1i = fma2(bcf(rg[ROW2G_G1 + 3 + 2 * j]), e1[j][q], q1i);
             }
-            const f32x2 Pr = fma2(q0r, q1r, mul2(q0i, q1i ^ SGNP)), Pi = fma2(q0r, q1i, mul2(q0i, q1r));   // P = q0 q1
-            fe[q] = fma2(bwr, Pr, fe[q]);
-            fe[q] = fma2(bnwi, Pi, fe[q]);                            // Re(w P)
+            if (GRAD != 2) {
+                const f32x2 Pr = fma2(q0r, q1r, mul2(q0i, q1i ^ SGNP)), Pi = fma2(q0r, q1i, mul2(q0i, q1r));   // P = q0 q1
+                fe[q] = fma2(bwr, Pr, fe[q]);
+                fe[q] = fma2(bnwi, Pi, fe[q]);                        // Re(w P)
+            }
             if (GRAD) {
                 // T0 = w q1 (everything but group 0), T1 = w q0;  A_j += Re(c_j T) = Re c_j Re T - Im c_j Im T
                 // (-Im T from the negated weight: a broadcast operand, so the negation costs nothing)
@@ -584,7 +587,7 @@ __device__ __forceinline__ void grp_rows_f2_joint(const f32x2 (&y)[K][NP], const
 // With two pairs per lane and K >= AFSAT_F2_SEQ_MINK the pairs are walked one after the other (each keeps ~4 K register
 // pairs of symmetric polynomials, accumulators and literal values alive).
 #define AFSAT_F2_SEQ_MINK 5
-template <int K, int NP, bool GRAD>
+template <int K, int NP, int GRAD>
 __device__ __forceinline__ void grp_rows_f2(const f32x2 (&y)[K][NP], const float *__restrict__ rg, int n_rows, f32x2 (&fe)[NP],
                                             f32x2 (&g)[K][NP])
 {
@@ -608,7 +611,7 @@ __device__ __forceinline__ void grp_rows_f2(const f32x2 (&y)[K][NP], const float
 // UV (unit variant, chosen once per work item when its table is staged): 0 = generic coefficients in
 // every row; 1 / 2 = standard table whose first rows are the trivial twiddles [w = 1 (UV 1 only)]
 // [w = -1 iff K odd] [w = i iff K = 3 mod 4] (n_real = their number), followed by n_cplx generic complex rows.
-template <int K, int NP, bool GRAD, int UV>
+template <int K, int NP, int GRAD, int UV>
 __device__ __forceinline__ void eval_points_f2(const f32x2 (&y)[K][NP], const f32x2 *__restrict__ tab, const float *__restrict__ tabg,
                                                int n_real, int n_cplx, f32x2 (&fe)[NP], f32x2 (&g)[K][NP])
 {
@@ -641,7 +644,7 @@ __device__ __forceinline__ void eval_points_f2(const f32x2 (&y)[K][NP], const f3
 #pragma unroll
             for (int q = 0; q < NP; ++q) { pre[i][q] = run[q]; run[q] = mul2(run[q], f[i][q]); }
 #pragma unroll
-        for (int q = 0; q < NP; ++q) fe[q] = fma2(w, run[q], fe[q]);
+        for (int q = 0; q < NP; ++q) if (GRAD != 2) fe[q] = fma2(w, run[q], fe[q]);
         if (GRAD) {
 #pragma unroll
             for (int q = 0; q < NP; ++q) suf[q] = wb;
@@ -807,7 +810,7 @@ template <> struct PairIO<2> {
 // bodies (k > 5: arithmetic hides the gathers), 1 for k = 4, 5, 2 for k <= 3 -- a k = 3 constraint is ~120 instructions per
 // warp, too little to cover a loaded L2 round trip with one constraint in flight (ncu: the wait for the gathers was the
 // top stall of cfg4's kernel, nearly all of it in the k = 3 body).
-template <int K, int NP, bool GRAD, int PFD, int UV>
+template <int K, int NP, int GRAD, int PFD, int UV>
 __device__ __forceinline__ void run_item_f2(const EvalParams<float> &p, const int32_t *__restrict__ s_lits,
                                             const f32x2 *__restrict__ s_tab2, const float *__restrict__ s_tabg, int n_real,
                                             int n_cplx, int nc, int wk, int Wk, int64_t b, f32x2 (&fe)[NP])
@@ -864,7 +867,7 @@ __device__ __forceinline__ void run_item_f2(const EvalParams<float> &p, const in
 // ---- one launch for a RANGE of lengths [KLO, KHI]: the CTA's item picks its length-K body, which is a
 // separately compiled (noinline) function so that every length keeps its own schedule and register
 // allocation while all lengths share one grid (no per-length launch tails) ---------------------------
-template <int K, int NP, bool GRAD, bool CSPLIT>
+template <int K, int NP, int GRAD, bool CSPLIT>
 __device__ __forceinline__ void item_body_f2(const EvalParams<float> &p, const int32_t *s_lits, const f32x2 *s_tab2,
                                           const float *s_tabg, float (*s_F)[64 * NP], int n_real, int n_cplx, int nc, int uv)
 {
@@ -906,7 +909,7 @@ __device__ __forceinline__ void item_body_f2(const EvalParams<float> &p, const i
     }
 }
 
-template <int K, int KHI, int NP, bool GRAD, bool CSPLIT>
+template <int K, int KHI, int NP, int GRAD, bool CSPLIT>
 struct SwitchF2 {
     static __device__ __forceinline__ void go(int k, const EvalParams<float> &p, const int32_t *s_lits, const f32x2 *s_tab2,
                                               const float *s_tabg, float (*s_F)[64 * NP], int n_real, int n_cplx, int nc, int uv)
@@ -916,7 +919,7 @@ struct SwitchF2 {
     }
 };
 
-template <int KLO, int KHI, int NP, bool GRAD, int MINB, bool CSPLIT>
+template <int KLO, int KHI, int NP, int GRAD, int MINB, bool CSPLIT>
 __global__ void __launch_bounds__(CTA_THREADS, MINB) k_eval_f2m(const EvalParams<float> p)
 {
     constexpr int H = (KHI + 1) / 2 + 1;

@@ -458,17 +458,33 @@ __global__ void k_zero_pad(T *__restrict__ G, int n, int B, int64_t ldb)
         G[(i / np) * ldb + B + (i % np)] = T(0);
 }
 
-// ---- F[b] = F_const + sum over items of Fpart[item][b], fixed order, accumulated in double, for the candidates
-// [b0, b1) of one partial-assignment group (F_const: the constraints the partial assignment already decides) ----
+// ---- F[b] = F_const + sum over items of Fpart[item][b], in a FIXED order, accumulated in double, for the candidates
+// [b0, b1) of one partial-assignment group (F_const: the constraints the partial assignment already decides).
+// A CTA takes 32 candidates; its RED_F_SLICES warps sum the rows i = slice, slice + RED_F_SLICES, ... (a thread per
+// candidate walking all rows alone was latency-bound: 65 us on cfg3), then slice 0 adds the slices' sums in slice order.
+constexpr int RED_F_SLICES = 16;
 template <typename T>
-__global__ void k_reduce_F(const T *__restrict__ Fpart, int n_rows, int64_t ldb, int64_t b0, int64_t b1, double F_const,
-                           T *__restrict__ F, const uint8_t *__restrict__ skip)
+__global__ void __launch_bounds__(32 * RED_F_SLICES) k_reduce_F(const T *__restrict__ Fpart, int n_rows, int64_t ldb, int64_t b0, int64_t b1,
+                                                                double F_const, T *__restrict__ F, const uint8_t *__restrict__ skip)
 {
-    const int64_t b = b0 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= b1 || (skip && skip[b])) return;                          // skipped candidates keep their F
-    double s = F_const;
-    for (int i = 0; i < n_rows; ++i) s += (double)Fpart[(int64_t)i * ldb + b];
-    F[b] = (T)s;
+    __shared__ double s_part[RED_F_SLICES][32];
+    const int lane = threadIdx.x & 31, slice = threadIdx.x >> 5;
+    const int64_t b = b0 + (int64_t)blockIdx.x * 32 + lane;
+    const bool live = b < b1 && !(skip && skip[b]);                    // skipped candidates keep their F
+    double s = 0.0;
+    if (live) {
+        const T *col = Fpart + b;
+#pragma unroll 4
+        for (int i = slice; i < n_rows; i += RED_F_SLICES) s += (double)col[(int64_t)i * ldb];
+    }
+    s_part[slice][lane] = s;
+    __syncthreads();
+    if (slice == 0 && live) {
+        double t = F_const;
+#pragma unroll
+        for (int j = 0; j < RED_F_SLICES; ++j) t += s_part[j][lane];
+        F[b] = (T)t;
+    }
 }
 
 // ---- per-candidate state machine of Alg. 1 (a8, a9): satacc holds the count on the current X over the constraints
