@@ -35,7 +35,7 @@ std::mutex g_static_mutex;
 
 thread_local std::string g_create_error;
 
-// Length classes (one launch each per candidate tile, concurrent; one separately compiled body per length):
+// Length classes (one launch each per candidate tile, concurrent; one body per length, inlined into the class's kernel):
 //   fp32: S  k <= 5   k_eval_f2m, FOUR candidates per lane (two packed pairs) -- the shortest constraints are issue-bound
 //                     on per-constraint overhead (literal and table loads, addresses, sign masks), which a lane then
 //                     pays once per four candidates
