@@ -961,6 +961,31 @@ def test_persistent_path_refused_when_it_does_not_fit():
         Bd.Context.from_instance(inst, step_path=Bd.STEP_PERSISTENT)
 
 
+@pytest.mark.parametrize("B", [96, 200])
+def test_step_with_and_without_objective_agree(B):
+    """afsat_step without F_pre runs the gradient-only form of the packed fp32 kernels (no contraction a3), with F_pre the
+    full form: the same X(t) (to the rounding of the REDs' summation order), identical discrete outputs, and both against
+    the oracle's step.  Every length 1..8 of both packed classes, every type, fixed variables, a ragged batch."""
+    inst = I.make_mixed(n=48, m=600, kmin=1, kmax=8, seed=271, batch=B, with_fixed=True)
+    x0 = I.make_x0(inst, seed=272, batch=B)
+    outs = []
+    for with_obj in (False, True):
+        ctx = Bd.Context.from_instance(inst, batch=B, ldb=x0.shape[1], step_path=Bd.STEP_LAUNCHES)
+        x = dev(x0)
+        F_pre = torch.empty(B, dtype=torch.float32, device="cuda") if with_obj else None
+        _, sat, sol, first = ctx.step(x, 0.1, 1, want_F=False, F_pre=F_pre)
+        torch.cuda.synchronize()
+        outs.append((x.cpu().numpy(), sat.cpu().numpy(), sol.cpu().numpy(), first.cpu().numpy(),
+                     F_pre.cpu().numpy() if with_obj else None))
+    Xo, _, sato, solo, firsto = O.step(inst, x0.astype(np.float64), 0.1, 1, B, want_F=False)
+    for X, sat, sol, first, _ in outs:
+        assert np.abs(X[:, :B] - Xo[:, :B]).max() <= 0.1 * 1e-4
+        assert np.array_equal(sat, sato) and np.array_equal(sol, solo) and np.array_equal(first, firsto)
+    assert np.abs(outs[0][0] - outs[1][0]).max() <= 2e-6
+    Fo = O.eval_grad(inst, x0.astype(np.float64), B, grad=False)
+    assert np.all(np.abs(outs[1][4] - Fo) <= tol_F(inst.n_cons, Fo, 32))
+
+
 def test_F_pre_is_the_objective_of_the_last_gradient_point():
     inst = I.make_mixed(n=60, m=300, kmin=1, kmax=14, seed=181, batch=96, with_fixed=True)
     x0 = I.make_x0(inst, seed=182, batch=96)
