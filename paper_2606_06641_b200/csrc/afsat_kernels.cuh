@@ -837,19 +837,21 @@ __device__ __forceinline__ void run_item_f2(const EvalParams<float> &p, const in
 #pragma unroll
         for (int i = 0; i < K; ++i) {
             lit[i] = ln[i];
-            const uint32_t m = (uint32_t)(lit[i] & LIT_NEG);
+            // y = s x as ONE packed multiply by (s, s), s = +-1 (exact: the same bits as flipping the two sign bits with two
+            // LOP3s, -0.0 included, in half the issue slots)
+            const f32x2 sf = bcf(__int_as_float(0x3f800000 | (lit[i] & LIT_NEG)));
 #pragma unroll
-            for (int q = 0; q < NP; ++q) { y[i][q] = yn[i][q] ^ (((f32x2)m << 32) | m); g[i][q] = 0ull; }   // y = s x
+            for (int q = 0; q < NP; ++q) { y[i][q] = mul2(yn[i][q], sf); g[i][q] = 0ull; }
         }
         if (PFD > 0 && c + PFD * Wk < nc) fetch(c + PFD * Wk, ln, yn);
         eval_points_f2<K, NP, GRAD, UV>(y, s_tab2, s_tabg, n_real, n_cplx, fe, g);
         if (GRAD) {
 #pragma unroll
             for (int i = 0; i < K; ++i) {
-                const uint32_t m = (uint32_t)(lit[i] & LIT_NEG);
+                const f32x2 sf = bcf(__int_as_float(0x3f800000 | (lit[i] & LIT_NEG)));       // d/dx = s d/dy
                 f32x2 gi[NP];
 #pragma unroll
-                for (int q = 0; q < NP; ++q) gi[q] = g[i][q] ^ (((f32x2)m << 32) | m);
+                for (int q = 0; q < NP; ++q) gi[q] = mul2(g[i][q], sf);
                 PairIO<NP>::red(gb + (uint64_t)(uint32_t)(lit[i] & LIT_VAR) * g_ld, gi);
             }
         }
