@@ -550,7 +550,7 @@ __device__ __forceinline__ void grp_rows_f2_joint(const f32x2 (&y)[K][NP], const
             for (int j = 0; j < M1; ++j) {
                 q1r = fma2(bcf(rg[ROW2G_G1 + 2 + 2 * j]), e1[j][q], q1r); q1i = fma2(bcf(rg[ROW2G_G1 + 3 + 2 * j]), e1[j][q], q1i);
             }
-            if (GRAD != 2) {
+            if (GRAD == 0) {
                 const f32x2 Pr = fma2(q0r, q1r, mul2(q0i, q1i ^ SGNP)), Pi = fma2(q0r, q1i, mul2(q0i, q1r));   // P = q0 q1
                 fe[q] = fma2(bwr, Pr, fe[q]);
                 fe[q] = fma2(bnwi, Pi, fe[q]);                        // Re(w P)
@@ -560,6 +560,10 @@ __device__ __forceinline__ void grp_rows_f2_joint(const f32x2 (&y)[K][NP], const
                 // (-Im T from the negated weight: a broadcast operand, so the negation costs nothing)
                 const f32x2 t0r = fma2(bwr, q1r, mul2(bnwi, q1i)), nt0i = fma2(bnwr, q1i, mul2(bnwi, q1r));
                 const f32x2 t1r = fma2(bwr, q0r, mul2(bnwi, q0i)), nt1i = fma2(bnwr, q0i, mul2(bnwi, q0r));
+                if (GRAD == 1) {                                      // the contraction rides on the gradient's T0: Re(w P) = Re(T0 q0),
+                    fe[q] = fma2(t0r, q0r, fe[q]);                    // two packed operations where forming P first takes six
+                    fe[q] = fma2(nt0i, q0i, fe[q]);
+                }
 #pragma unroll
                 for (int j = 0; j < M0; ++j) {
                     A0[j][q] = fma2(bcf(rg[2 + 2 * j]), t0r, A0[j][q]); A0[j][q] = fma2(bcf(rg[3 + 2 * j]), nt0i, A0[j][q]);
