@@ -251,10 +251,10 @@ constexpr int ROW2 = 12;
 // (its weight was exactly zero) staged with weight 0, the halvings folded into their weights (2^-k, 2^-(k-1):
 // exact rescales); then the generic complex rows.  Other tables: rows as they are, uv = 0.
 // The generic complex rows are ALSO staged for literal groups (grp_rows_f2; outg gets ROW2G scalars per generic row, rd are
-// the same rows in double): c_j = a^(M-j) b^j for the two group sizes; for the standard tables un-halved (a = 1, b = w^l,
-// the 2^-k folded into the weight: exact rescales).
+// the same rows in double): c_j = a^(M-j) b^j for the two group sizes, and w c_j (as Re, -Im) beside them; for the standard
+// tables un-halved (a = 1, b = w^l, the 2^-k folded into the weight: exact rescales).
 // Returns the number of staged rows; out gets ROW2 scalars per row.
-constexpr int ROW2G_G1_H = 10, ROW2G_W_H = 20, ROW2G_H = 22;    // = ROW2G_G1, ROW2G_W, ROW2G below
+constexpr int ROW2G_G1_H = 10, ROW2G_D0_H = 20, ROW2G_D1_H = 30, ROW2G_H = 40;    // = ROW2G_G1, ROW2G_D0, ROW2G_D1, ROW2G below
 inline int pack_rows_f2(const float *r0, const double *rd, int n_real, int n_cplx, int k, float *out, float *outg, int *uv_out,
                         int *n_unit_out, int *n_gen_out)
 {
@@ -300,7 +300,7 @@ inline int pack_rows_f2(const float *r0, const double *rd, int n_real, int n_cpl
         }
     }
     {
-        const int M[2] = {(k + 1) / 2, k / 2}, off[2] = {0, ROW2G_G1_H};
+        const int M[2] = {(k + 1) / 2, k / 2}, off[2] = {0, ROW2G_G1_H}, offd[2] = {ROW2G_D0_H, ROW2G_D1_H};
         double scw = 1.0;
         if (std_tab) for (int i = 0; i < k; ++i) scw *= 0.5;
         const double sc = std_tab ? 2.0 : 1.0;
@@ -318,8 +318,10 @@ inline int pack_rows_f2(const float *r0, const double *rd, int n_real, int n_cpl
                         cr = nr2; ci = ni2;
                     }
                     o[off[gq] + 2 * j] = (float)cr; o[off[gq] + 2 * j + 1] = (float)ci;
+                    // the same coefficient times the point's weight, as (Re, -Im): sum_j (w c_j) e_j = w x (the group's factor)
+                    const double wr = r[4] * scw, wi = r[5] * scw;
+                    o[offd[gq] + 2 * j] = (float)(wr * cr - wi * ci); o[offd[gq] + 2 * j + 1] = (float)-(wr * ci + wi * cr);
                 }
-            o[ROW2G_W_H] = (float)(r[4] * scw); o[ROW2G_W_H + 1] = (float)(r[5] * scw);
         }
     }
     *uv_out = uv; *n_unit_out = n_unit; *n_gen_out = n_gen;
@@ -516,8 +518,9 @@ __device__ __forceinline__ void loo_f2(const f32x2 (*y)[NP], const f32x2 (&A)[M]
 }
 
 // Staged row of a generic complex point for TWO groups (sizes M0 = ceil(K/2), M1 = floor(K/2) <= 4): {Re, Im of c0_0 ..
-// c0_M0 | Re, Im of c1_0 .. c1_M1 (from scalar ROW2G_G1) | Re w, Im w (at ROW2G_W)}, c_j = a^(M-j) b^j of the group.
-constexpr int ROW2G_G1 = ROW2G_G1_H, ROW2G_W = ROW2G_W_H, ROW2G = ROW2G_H;
+// c0_M0 | Re, Im of c1_0 .. c1_M1 (from scalar ROW2G_G1) | Re, -Im of w c0_j (ROW2G_D0) | Re, -Im of w c1_j (ROW2G_D1)},
+// c_j = a^(M-j) b^j of the group, w the point's contracted weight.
+constexpr int ROW2G_G1 = ROW2G_G1_H, ROW2G_D0 = ROW2G_D0_H, ROW2G_D1 = ROW2G_D1_H, ROW2G = ROW2G_H;
 
 // all generic complex rows of a signature for the K literals of a lane (K >= 2), two groups
 // ROLLED: the loop over the DFT points is kept as it is written (the compiler's two-fold unrolling pays for itself with a
@@ -538,31 +541,30 @@ __device__ __forceinline__ void grp_rows_f2_joint(const f32x2 (&y)[K][NP], const
 #pragma unroll
         for (int j = 0; j < M1; ++j) A1[j][q] = 0ull;
     }
+    // Per point, with the weight folded into a second set of coefficients on the host: T0 = w q1 = sum_j (w c1_j) e1_j is
+    // everything but group 0, T1 = w q0 everything but group 1 -- each costs what the bare factor costs, and the four
+    // packed multiplications by w of the earlier form are gone.  A_j += Re(c_j T) = Re c_j Re T - Im c_j Im T;
+    // the contraction a3 is Re(w P) = Re(T0 q0) and needs the bare q0 (GRAD != 2 only).
     auto row = [&](const float *__restrict__ rg) {
-        const float wr = rg[ROW2G_W], wi = rg[ROW2G_W + 1];
-        const f32x2 bwr = bcf(wr), bnwr = bcf(-wr), bnwi = bcf(-wi);
 #pragma unroll
         for (int q = 0; q < NP; ++q) {
-            f32x2 q0r = bcf(rg[0]), q0i = bcf(rg[1]), q1r = bcf(rg[ROW2G_G1]), q1i = bcf(rg[ROW2G_G1 + 1]);
-#pragma unroll
-            for (int j = 0; j < M0; ++j) { q0r = fma2(bcf(rg[2 + 2 * j]), e0[j][q], q0r); q0i = fma2(bcf(rg[3 + 2 * j]), e0[j][q], q0i); }
+            f32x2 t0r = bcf(rg[ROW2G_D1]), nt0i = bcf(rg[ROW2G_D1 + 1]);
 #pragma unroll
             for (int j = 0; j < M1; ++j) {
-                q1r = fma2(bcf(rg[ROW2G_G1 + 2 + 2 * j]), e1[j][q], q1r); q1i = fma2(bcf(rg[ROW2G_G1 + 3 + 2 * j]), e1[j][q], q1i);
+                t0r = fma2(bcf(rg[ROW2G_D1 + 2 + 2 * j]), e1[j][q], t0r); nt0i = fma2(bcf(rg[ROW2G_D1 + 3 + 2 * j]), e1[j][q], nt0i);
             }
-            if (GRAD == 0) {
-                const f32x2 Pr = fma2(q0r, q1r, mul2(q0i, q1i ^ SGNP)), Pi = fma2(q0r, q1i, mul2(q0i, q1r));   // P = q0 q1
-                fe[q] = fma2(bwr, Pr, fe[q]);
-                fe[q] = fma2(bnwi, Pi, fe[q]);                        // Re(w P)
+            if (GRAD != 2) {
+                f32x2 q0r = bcf(rg[0]), q0i = bcf(rg[1]);
+#pragma unroll
+                for (int j = 0; j < M0; ++j) { q0r = fma2(bcf(rg[2 + 2 * j]), e0[j][q], q0r); q0i = fma2(bcf(rg[3 + 2 * j]), e0[j][q], q0i); }
+                fe[q] = fma2(t0r, q0r, fe[q]);
+                fe[q] = fma2(nt0i, q0i, fe[q]);                       // Re(T0 q0)
             }
             if (GRAD) {
-                // T0 = w q1 (everything but group 0), T1 = w q0;  A_j += Re(c_j T) = Re c_j Re T - Im c_j Im T
-                // (-Im T from the negated weight: a broadcast operand, so the negation costs nothing)
-                const f32x2 t0r = fma2(bwr, q1r, mul2(bnwi, q1i)), nt0i = fma2(bnwr, q1i, mul2(bnwi, q1r));
-                const f32x2 t1r = fma2(bwr, q0r, mul2(bnwi, q0i)), nt1i = fma2(bnwr, q0i, mul2(bnwi, q0r));
-                if (GRAD == 1) {                                      // the contraction rides on the gradient's T0: Re(w P) = Re(T0 q0),
-                    fe[q] = fma2(t0r, q0r, fe[q]);                    // two packed operations where forming P first takes six
-                    fe[q] = fma2(nt0i, q0i, fe[q]);
+                f32x2 t1r = bcf(rg[ROW2G_D0]), nt1i = bcf(rg[ROW2G_D0 + 1]);
+#pragma unroll
+                for (int j = 0; j < M0; ++j) {
+                    t1r = fma2(bcf(rg[ROW2G_D0 + 2 + 2 * j]), e0[j][q], t1r); nt1i = fma2(bcf(rg[ROW2G_D0 + 3 + 2 * j]), e0[j][q], nt1i);
                 }
 #pragma unroll
                 for (int j = 0; j < M0; ++j) {
