@@ -462,7 +462,6 @@ __device__ __forceinline__ void oct_row_f2(const f32x2 (&y)[K][NP], const f32x2 
 //     A_j += Re( w a^(M-j) b^j x (product of the OTHER groups' factors) ),   dFE/dy_u = sum_j A_j e_{j-1}(group without y_u),
 // expanded once per constraint.  The generating polynomial is still evaluated at every DFT point and contracted with the
 // same weights; the groups only change the order in which its factors are multiplied.
-constexpr f32x2 SGNP = 0x8000000080000000ull;
 __device__ __forceinline__ f32x2 bcf(float c) { return pk(c, c); }
 
 // e[j-1] = e_j(y[0..M)), M <= 4
