@@ -530,7 +530,7 @@ __device__ __forceinline__ void grp_rows_f2_joint(const f32x2 (&y)[K][NP], const
                                             f32x2 (&g)[K][NP])
 {
     constexpr int M0 = (K + 1) / 2, M1 = K / 2;
-    f32x2 e0[M0][NP], e1[M1][NP], A0[M0][NP], A1[M1][NP];
+    f32x2 e0[M0][NP], e1[M1][NP], A0[M0][NP], A1[M1][NP], A00[NP];
     esp_f2<M0, NP>(&y[0], e0);
     esp_f2<M1, NP>(&y[M0], e1);
 #pragma unroll
@@ -539,6 +539,7 @@ __device__ __forceinline__ void grp_rows_f2_joint(const f32x2 (&y)[K][NP], const
         for (int j = 0; j < M0; ++j) A0[j][q] = 0ull;
 #pragma unroll
         for (int j = 0; j < M1; ++j) A1[j][q] = 0ull;
+        A00[q] = 0ull;
     }
     // Per point, with the weight folded into a second set of coefficients on the host: T0 = w q1 = sum_j (w c1_j) e1_j is
     // everything but group 0, T1 = w q0 everything but group 1 -- each costs what the bare factor costs, and the four
@@ -552,12 +553,15 @@ __device__ __forceinline__ void grp_rows_f2_joint(const f32x2 (&y)[K][NP], const
             for (int j = 0; j < M1; ++j) {
                 t0r = fma2(bcf(rg[ROW2G_D1 + 2 + 2 * j]), e1[j][q], t0r); nt0i = fma2(bcf(rg[ROW2G_D1 + 3 + 2 * j]), e1[j][q], nt0i);
             }
-            if (GRAD != 2) {
+            if (GRAD == 0) {
                 f32x2 q0r = bcf(rg[0]), q0i = bcf(rg[1]);
 #pragma unroll
                 for (int j = 0; j < M0; ++j) { q0r = fma2(bcf(rg[2 + 2 * j]), e0[j][q], q0r); q0i = fma2(bcf(rg[3 + 2 * j]), e0[j][q], q0i); }
                 fe[q] = fma2(t0r, q0r, fe[q]);
                 fe[q] = fma2(nt0i, q0i, fe[q]);                       // Re(T0 q0)
+            }
+            if (GRAD == 1) {                                          // the constant term of group 0: see below
+                A00[q] = fma2(bcf(rg[0]), t0r, A00[q]); A00[q] = fma2(bcf(rg[1]), nt0i, A00[q]);
             }
             if (GRAD) {
                 f32x2 t1r = bcf(rg[ROW2G_D0]), nt1i = bcf(rg[ROW2G_D0 + 1]);
@@ -582,6 +586,18 @@ __device__ __forceinline__ void grp_rows_f2_joint(const f32x2 (&y)[K][NP], const
         for (int p = 0; p < n_rows; ++p, rg += ROW2G) row(rg);
     } else {
         for (int p = 0; p < n_rows; ++p, rg += ROW2G) row(rg);
+    }
+    if (GRAD == 1) {
+        // The contraction a3 out of the gradient's accumulators: at every point Re(w P) = Re(T0 q0) is LINEAR in group 0's
+        // symmetric polynomials, q0 = c0_0 + sum_j c0_j e_j, so summed over the points FE = A0_0 + sum_j A0_j e_j with
+        // A0_j = sum_points Re(c0_j T0) -- the accumulators of the gradient plus one for the constant term.
+#pragma unroll
+        for (int q = 0; q < NP; ++q) {
+            f32x2 f = A00[q];
+#pragma unroll
+            for (int j = 0; j < M0; ++j) f = fma2(A0[j][q], e0[j][q], f);
+            fe[q] = add2(fe[q], f);
+        }
     }
     if (GRAD) {
         loo_f2<M0, NP>(&y[0], A0, &g[0]);
