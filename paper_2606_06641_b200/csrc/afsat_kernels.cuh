@@ -246,10 +246,12 @@ constexpr int ROW2 = 12;
 
 // HOST: the staged table of one signature for the packed kernel, from its fp32 rows {Re a, Im a, Re b, Im b,
 // Re w, Im w, Re(wb), Im(wb)} (real rows first).  Standard tables (a = 1/2 exactly in every row): the
-// trivial twiddles first, at fixed positions -- [w = 1 (absent: uv = 2)] [w = -1 iff k odd] [w = i iff k = 3 mod 4]
-// [w = (1+i)/sqrt 2, then its partner (-1+i)/sqrt 2 with CONJUGATED weights, iff k = 7 mod 8] -- a missing one
-// (its weight was exactly zero) staged with weight 0, the halvings folded into their weights (2^-k, 2^-(k-1):
-// exact rescales); then the generic complex rows.  Other tables: rows as they are, uv = 0.
+// trivial twiddles first, at fixed positions -- [w = 1 (absent: uv = 2)] [w = -1 iff k odd] [w = i iff k = 3] -- a missing
+// one (its weight was exactly zero) staged with weight 0, the halvings folded into their weights (2^-k, 2^-(k-1): exact
+// rescales); then the complex rows, which run the literal groups.  (k = 7 has the points i and the eighth roots, which
+// rounds 1 and 2 walked on their own, two adds and two FMAs per multiplication: with the weight folded into the
+// coefficients and the contraction read off the accumulators the grouped rows are the cheaper form for them too, cfg1
+// 1.79 -> 1.68 ms per step with the objective.)  Other tables: rows as they are, uv = 0.
 // The generic complex rows are ALSO staged for literal groups (grp_rows_f2; outg gets ROW2G scalars per generic row, rd are
 // the same rows in double): c_j = a^(M-j) b^j for the two group sizes, and w c_j (as Re, -Im) beside them; for the standard
 // tables un-halved (a = 1, b = w^l, the 2^-k folded into the weight: exact rescales).
@@ -259,26 +261,22 @@ inline int pack_rows_f2(const float *r0, const double *rd, int n_real, int n_cpl
                         int *n_unit_out, int *n_gen_out)
 {
     const int nr = n_real + n_cplx;
-    int src[AFSAT_PACK_MAX_ROWS], n = 0, uv = 0, n_unit = n_real, n_gen = n_cplx, q_conj = -1;
+    int src[AFSAT_PACK_MAX_ROWS], n = 0, uv = 0, n_unit = n_real, n_gen = n_cplx;
     bool std_tab = true;
     for (int q = 0; q < nr; ++q) std_tab = std_tab && r0[8 * q] == 0.5f && r0[8 * q + 1] == 0.f;
     if (std_tab) {
-        int iP = -1, iM = -1, iI = -1, iA = -1, iB = -1;
-        const bool oct = (k & 7) == 7;
+        int iP = -1, iM = -1, iI = -1;
         for (int q = 0; q < nr; ++q) {
             const float br = r0[8 * q + 2], bi = r0[8 * q + 3];
             if (q < n_real) { if (br == 0.5f) iP = q; else if (br == -0.5f) iM = q; }
-            else if (br == 0.f && bi == 0.5f) iI = q;
-            else if (oct && bi > 0.35f && bi < 0.36f && br == bi) iA = q;        // w = (1 + i)/sqrt 2
-            else if (oct && bi > 0.35f && bi < 0.36f && br == -bi) iB = q;       // w = (-1 + i)/sqrt 2
+            else if (k == 3 && br == 0.f && bi == 0.5f) iI = q;
         }
         uv = iP >= 0 ? 1 : 2;
         if (iP >= 0) src[n++] = iP;
         if (k & 1) src[n++] = iM;
-        if ((k & 3) == 3) src[n++] = iI;
-        if (oct) { src[n++] = iA; q_conj = n; src[n++] = iB; }
+        if (k == 3) src[n++] = iI;
         n_unit = n;
-        for (int q = n_real; q < nr; ++q) if (q != iI && q != iA && q != iB) src[n++] = q;
+        for (int q = n_real; q < nr; ++q) if (q != iI) src[n++] = q;
         n_gen = n - n_unit;
     } else {
         for (int q = 0; q < nr; ++q) src[n++] = q;
@@ -292,11 +290,11 @@ inline int pack_rows_f2(const float *r0, const double *rd, int n_real, int n_cpl
         if (src[q] < 0) continue;
         const float *r = r0 + 8 * src[q];
         const bool unit = uv != 0 && q < n_unit;
-        const float fw = unit ? sc_w : 1.f, fwb = unit ? sc_wb : 1.f, cj = q == q_conj ? -1.f : 1.f;
+        const float fw = unit ? sc_w : 1.f, fwb = unit ? sc_wb : 1.f;
         if (src[q] < n_real) { o[0] = r[0]; o[1] = r[2]; o[2] = r[4] * fw; o[3] = r[6] * fwb; }   // a, b, w, wb
         else {
             o[0] = r[0]; o[1] = r[1]; o[2] = -r[1]; o[3] = r[2]; o[4] = r[3]; o[5] = -r[3];
-            o[6] = r[4] * fw; o[7] = -cj * r[5] * fw; o[8] = r[6] * fwb; o[9] = -cj * r[7] * fwb;
+            o[6] = r[4] * fw; o[7] = -r[5] * fw; o[8] = r[6] * fwb; o[9] = -r[7] * fwb;
         }
     }
     {
@@ -404,53 +402,6 @@ __device__ __forceinline__ void unit_rows_f2(const f32x2 (&y)[K][NP], const f32x
             if (HM) g[0][q] = add2(g[0][q], sufM[q]);
             if (HI) g[0][q] = add2(g[0][q], sr[q]);
         }
-    }
-}
-
-// The eighth roots of unity (k = 7 mod 8): at the DFT point w = (1 + i)/sqrt 2 a factor is (1 + z) + i z with
-// z = y/sqrt 2, and multiplying by it needs two adds and two FMAs instead of four multiplies and two FMAs,
-// no stored factors and no negation at all (the suffix is carried CONJUGATED, T = conj(S), T <- T conj(f)):
-//   P <- (Re P + z (Re P - Im P)) + i (Im P + z (Re P + Im P))
-//   T <- (Re T + z (Re T + Im T)) + i (Im T + z (Im T - Re T)),      g_i += Re P_i Re T_i + Im P_i Im T_i
-// Its partner w' = (-1 + i)/sqrt 2 = -conj(w) is the same walk at -y with conjugated weights (the row is staged
-// that way): prod (1 + w' y_j) = conj( prod (1 + w (-y_j)) ).  cz = +-1/sqrt 2 selects the row.
-template <int K, int NP, int GRAD>
-__device__ __forceinline__ void oct_row_f2(const f32x2 (&y)[K][NP], const f32x2 *__restrict__ r, float cz, f32x2 (&fe)[NP],
-                                           f32x2 (&g)[K][NP])
-{
-    const f32x2 one2 = pk(1.0f, 1.0f), c2 = pk(cz, cz);
-    f32x2 z[K][NP], pr[K][NP], pi[K][NP], rr[NP], ri[NP];
-#pragma unroll
-    for (int i = 0; i < K; ++i)
-#pragma unroll
-        for (int q = 0; q < NP; ++q) z[i][q] = mul2(c2, y[i][q]);
-#pragma unroll
-    for (int q = 0; q < NP; ++q) { rr[q] = add2(z[0][q], one2); ri[q] = z[0][q]; }    // (1 + z_0) + i z_0
-#pragma unroll
-    for (int i = 1; i < K; ++i)
-#pragma unroll
-        for (int q = 0; q < NP; ++q) {
-            pr[i][q] = rr[q]; pi[i][q] = ri[q];
-            const f32x2 d = sub2(rr[q], ri[q]), s = add2(rr[q], ri[q]);
-            rr[q] = fma2(z[i][q], d, rr[q]); ri[q] = fma2(z[i][q], s, ri[q]);
-        }
-#pragma unroll
-    for (int q = 0; q < NP; ++q) if (GRAD != 2) { fe[q] = fma2(bc(r, 6), rr[q], fe[q]); fe[q] = fma2(bc(r, 7), ri[q], fe[q]); }
-    if (GRAD) {
-        f32x2 tr[NP], ti[NP];                                                         // conjugated suffix, seeded from the row
-#pragma unroll
-        for (int q = 0; q < NP; ++q) { tr[q] = r[8]; ti[q] = r[9]; }
-#pragma unroll
-        for (int i = K - 1; i >= 1; --i)
-#pragma unroll
-            for (int q = 0; q < NP; ++q) {
-                g[i][q] = fma2(pr[i][q], tr[q], g[i][q]);
-                g[i][q] = fma2(pi[i][q], ti[q], g[i][q]);
-                const f32x2 u = add2(tr[q], ti[q]), v = sub2(ti[q], tr[q]);
-                tr[q] = fma2(z[i][q], u, tr[q]); ti[q] = fma2(z[i][q], v, ti[q]);
-            }
-#pragma unroll
-        for (int q = 0; q < NP; ++q) g[0][q] = add2(g[0][q], tr[q]);                  // prefix_0 = 1
     }
 }
 
@@ -631,23 +582,17 @@ __device__ __forceinline__ void grp_rows_f2(const f32x2 (&y)[K][NP], const float
 
 // UV (unit variant, chosen once per work item when its table is staged): 0 = generic coefficients in
 // every row; 1 / 2 = standard table whose first rows are the trivial twiddles [w = 1 (UV 1 only)]
-// [w = -1 iff K odd] [w = i iff K = 3 mod 4] (n_real = their number), followed by n_cplx generic complex rows.
+// [w = -1 iff K odd] [w = i iff K = 3] (n_real = their number), followed by n_cplx complex rows for the literal groups.
 template <int K, int NP, int GRAD, int UV>
 __device__ __forceinline__ void eval_points_f2(const f32x2 (&y)[K][NP], const f32x2 *__restrict__ tab, const float *__restrict__ tabg,
                                                int n_real, int n_cplx, f32x2 (&fe)[NP], f32x2 (&g)[K][NP])
 {
     if (UV != 0) {
-        constexpr bool HP = UV == 1, HM = (K & 1) != 0, HI = (K & 3) == 3;
+        constexpr bool HP = UV == 1, HM = (K & 1) != 0, HI = K == 3;
         const f32x2 *rP = tab, *rM = tab + (HP ? ROW2 : 0), *rI = rM + (HM ? ROW2 : 0);
         if (HP || HM || HI) unit_rows_f2<K, NP, HP, HM, HI, GRAD>(y, rP, rM, rI, fe, g);
-        constexpr bool HO = (K & 7) == 7;       // the pair of eighth roots, next in the staged order
-        const f32x2 *rO = rI + (HI ? ROW2 : 0);
-        if (HO) {
-            oct_row_f2<K, NP, GRAD>(y, rO, 0.70710678118654752f, fe, g);             // = 2 Re b of the row, bit for bit
-            oct_row_f2<K, NP, GRAD>(y, rO + ROW2, -0.70710678118654752f, fe, g);
-        }
-        // the generic complex points, grouped (K = 3 and K = 7 have none: all their points are trivial twiddles)
-        if constexpr (K >= 2 && K != 3 && K != 7) { if (n_cplx > 0) grp_rows_f2<K, NP, GRAD>(y, tabg, n_cplx, fe, g); }
+        // the other complex points, grouped (K = 3 has none: its one complex point is w = i)
+        if constexpr (K >= 2 && K != 3) { if (n_cplx > 0) grp_rows_f2<K, NP, GRAD>(y, tabg, n_cplx, fe, g); }
         return;
     }
     const f32x2 *r = tab;
