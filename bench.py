@@ -528,8 +528,8 @@ def report(r, world, local, oracle_seconds, rank0_oracle=True):
             "hbm_floor_bytes_per_step": 2 * n * B * esz, "hbm_peak_gbs": peaks["hbm_gbs"],
             "note": "achieved = ALGORITHMIC flop of the instance as given (SURVEY.md App. D: 12 / 4 FP32 instructions per literal at a "
                     "complex / real DFT point, every retained point) / measured kernel time.  The kernels execute fewer instructions: "
-                    "trivial twiddles at the points 1, -1, i and the eighth roots (k <= 8; cfg1's k = 7 has only such points), literal "
-                    "groups (k >= 21), and a partial assignment is substituted before anything is evaluated (frac_after_substitution "
+                    "trivial twiddles at the points 1 and -1, literal groups with folded weights at the complex points (k <= 8) and literal "
+                    "groups in the lane-split kernels (k >= 9), and a partial assignment is substituted before anything is evaluated (frac_after_substitution "
                     "counts the model on the substituted table); measured_pipe_utilisation is what ncu saw executed"}
     l2 = roof["l2"]
     roof["limited_by"] = ("instruction issue at the occupancy the register file allows (roofline.measured_pipe_utilisation; DESIGN.md 6.7: "
