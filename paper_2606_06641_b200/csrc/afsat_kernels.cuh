@@ -226,10 +226,6 @@ __device__ __forceinline__ f32x2 bc(const f32x2 *tab, int j)
     const float c = reinterpret_cast<const float *>(tab)[2 * j];
     return pk(c, c);
 }
-__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b)
-{
-    f32x2 d; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d;   // FADD2 with a negated operand
-}
 __device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b)
 {
     f32x2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d;
